@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the hot path (BASELINE.json: "energy+gradient evals/sec and ligands
+docked/hour (1xB200) vs roofline").
+
+One STEP = one pass of the whole hot path over one batch of synthetic
+input: Lamarckian-GA docking of `--ligands` drug-like ligands (BASELINE.json configs[1]: 40 atoms, 8
+rotatable bonds, 7 atom types, 9 fp32 maps of 64^3 at 0.375 A, 20 runs x population 150 x 2.5M evals per
+run, ADADELTA on 6% of the individuals per generation) docked concurrently against one resident grid set
+(row a7).  value = evaluations performed by all ranks / time.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--ligands L] [--impl reference]
+
+Under torchrun every rank docks its own L ligands (the path shards by ligand with no exchange step:
+"scaling": "weak"); time is the max over ranks.  `--impl reference` times the CPU oracle (test
+infrastructure, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2007_03678_b200 import workloads as W  # noqa: E402
+
+NRUN, POP, MAX_EVALS = 20, 150, 2_500_000
+WORKLOAD = ("drug-like docking: 40-atom ligand, 8 torsions, 7 types, 9 fp32 maps 64^3 @0.375A, "
+            "20 LGA runs x pop 150 x 2.5M evals/run, ADADELTA 300 it on 6%/generation")
+SM_COUNT, FP32_LANES, SM_MAX_MHZ = 148, 128, 1965.0        # B200_PROFILING.md unit counts and clocks
+
+
+def flops_per_eval(N, R, npairs, nmoved):
+    """SURVEY.md section 8(d) op census (FMA = 2 FLOP): pose N*(30*dbar+30), grid N*150, pairs Np*100,
+    back-prop N*20 + R*20; dbar = mean number of torsions acting on an atom."""
+    dbar = nmoved / max(N, 1)
+    return N * (30.0 * dbar + 30.0) + N * 150.0 + npairs * 100.0 + N * 20.0 + R * 20.0
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    return json.load(open(p)) if os.path.exists(p) else {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows, self.proc, self.idx = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.idx)], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        sm = [float(r[1]) for r in self.rows if len(r) >= 8 and r[1].replace(".", "").isdigit()]
+        mx = [float(r[2]) for r in self.rows if len(r) >= 8 and r[2].replace(".", "").isdigit()]
+        reasons = set()
+        for r in self.rows:
+            if len(r) >= 8:
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[4:8]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+def make_batch(L, rank):
+    """grid set of configs[1] + L drug-like ligands (same shape, distinct seeds) for this rank"""
+    grids, lig0 = W.make_config("drug")
+    centre = 0.5 * (grids.box_lo + grids.box_hi)
+    c = W.CONFIGS["drug"]
+    ligs = [lig0 if (rank == 0 and i == 0) else W.make_ligand(c["N"], c["R"], c["T"], 1000 * rank + 100 + i, centre)
+            for i in range(L)]
+    return grids, ligs
+
+
+# ------------------------------------------------------------------------------------------ reference arm (CPU oracle)
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    grids, ligs = make_batch(1, 0)
+    og, ol = oracle.Grids.from_workload(grids), oracle.Ligand.from_workload(ligs[0])
+    par = oracle.params(W.DEFAULT_PARAMS)
+    cores = oracle.num_threads()
+    sample_evals = 40_000                                  # per run; POP + k generations of (POP-1 + 9*300)
+    sample = f"1 ligand x {NRUN} runs x {sample_evals} evals/run of the same workload (full budget {MAX_EVALS})"
+    times, evals = [], 0
+    for s in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        r = oracle.dock(og, ol, par, NRUN, POP, sample_evals, seed=s)
+        dt = time.perf_counter() - t0
+        if s >= args.warmup:
+            times.append(dt)
+            evals += int(r["evals"].sum())
+    total = sum(times)
+    v = evals / total
+    print(json.dumps({
+        "impl": "reference", "metric": "energy+gradient evals/sec", "value": v, "unit": "evals/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / max(1, args.steps), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "sample": sample},
+        "cpu_baseline": {"value": v, "unit": "evals/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "evals/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+# ------------------------------------------------------------------------------------------ CUDA arm
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--ligands", type=int, default=8, help="ligands docked concurrently per step and per GPU")
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="also time adock_score_batch on the sweep config")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2007_03678_b200 import binding as B
+
+    rank, world, local = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    L = args.ligands
+    grids, ligs = make_batch(L, rank)
+    gp = B.make_params(W.DEFAULT_PARAMS)
+    gg = B.Grids.from_workload(grids)
+    gl = [B.Ligand.from_workload(gg, l, gp) for l in ligs]
+    seeds = [10_000 * rank + i for i in range(L)]
+    flop_eval = []
+    for l, h in zip(ligs, gl):
+        flop_eval.append(flops_per_eval(l.N, l.R, len(h.pairs()), int(h.tree()["moved"].sum())))
+    l2_flush = torch.empty(160 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)     # > 126 MB L2
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def step(s):
+        return B.adock_dock_many(gg, gl, gp, NRUN, POP, MAX_EVALS, [sd + 1000 * s for sd in seeds])
+
+    for s in range(args.warmup):
+        l2_flush.zero_()
+        step(s)
+    # ---- device-resident timing: K steps, L2 flushed (outside the events) before each
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    B.adock_launch_count(reset=True)
+    B.adock_profile(True)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    evals = 0
+    for s in range(args.steps):
+        l2_flush.zero_()
+        ev[s][0].record()
+        r = step(args.warmup + s)
+        ev[s][1].record()
+        evals += int(r["evals"].sum())
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    launches = B.adock_launch_count()
+    prof = B.adock_profile_read()
+    B.adock_profile(False)
+    t_ms = sum(a.elapsed_time(b) for a, b in ev)
+
+    # ---- end to end through the C ABI with host buffers: ligand upload (H2D) + docking + results (D2H) per step
+    barrier()
+    t0 = time.perf_counter()
+    e2e_evals, h2d, d2h = 0, 0, 0
+    for s in range(args.steps):
+        hl = [B.Ligand.from_workload(gg, l, gp) for l in ligs]                  # host preprocessing + H2D of the images
+        r = B.adock_dock_many(gg, hl, gp, NRUN, POP, MAX_EVALS, [sd + 77 * (s + 1) for sd in seeds], want_coords=True)
+        e2e_evals += int(r["evals"].sum())
+        h2d = sum(len(h.image()[0]) + 4 * h.N for h in hl) + 128 * L
+        d2h = r["genotypes"].nbytes + r["energies"].nbytes + r["coords"].nbytes + r["evals"].nbytes
+        for h in hl:
+            h.close()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+
+    if world > 1:
+        t = torch.tensor([t_ms, e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        c = torch.tensor([evals, e2e_evals, launches], dtype=torch.float64, device=dev)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+        t_ms, e2e_s = t.tolist()
+        evals, e2e_evals, launches = (int(x) for x in c.tolist())
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    value = evals / (t_ms * 1e-3)
+    peaks = measured_peaks()
+    # roofline of the dominant kernel (dock_ls_kernel: ADADELTA chains, ~95% of all evaluations)
+    ls_ms, ls_n, ls_evals = prof["ls_ms"], prof["ls_launches"], prof["ls_evals"]
+    mean_flop = float(np.mean(flop_eval))
+    peak_tf = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12
+    ach_tf = (ls_evals * mean_flop / (ls_ms * 1e-3) / 1e12) if ls_ms > 0 else None
+    roofline = {"bound": "alu", "kernel": "dock_ls_kernel", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": (ach_tf / peak_tf) if ach_tf else None, "traffic": None,
+                "peak_source": f"derived: {SM_COUNT} SMs x {FP32_LANES} FP32 lanes x 2 x {SM_MAX_MHZ:.0f} MHz (B200_PROFILING.md); "
+                               f"HBM peak {peaks.get('hbm_gbs')} GB/s of measured is not the bound (~120 B/eval)",
+                "flop_per_eval": mean_flop, "avg_launch_ms": (ls_ms / ls_n) if ls_n else None, "launches_timed": ls_n,
+                "evals_per_launch": (ls_evals / ls_n) if ls_n else None}
+    out = {
+        "metric": "energy+gradient evals/sec", "value": value, "unit": "evals/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": t_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "ligands_per_step_per_gpu": L, "nrun": NRUN, "pop_size": POP, "max_evals": MAX_EVALS,
+                   "l2": "160 MB buffer written before every timed step (flush); maps 58.7 MB resident"},
+        "ligands_per_hour": 3600.0 * L * world * args.steps / (t_ms * 1e-3),
+        "e2e": {"value": e2e_evals / e2e_s, "unit": "evals/s", "h2d_bytes_per_step": int(h2d) * world, "d2h_bytes_per_step": int(d2h) * world,
+                "ligands_per_hour": 3600.0 * L * world * args.steps / e2e_s},
+        "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
+    }
+
+    if args.sweep:
+        out["score_batch"] = sweep(B, torch, dev)
+    if world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline()
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def sweep(B, torch, dev):
+    """adock_score_batch on BASELINE.json's sweep sizes for the 40-atom ligand (energy + gradient)."""
+    grids, lig = W.make_config("sweep40")
+    gp = B.make_params(W.DEFAULT_PARAMS)
+    gg = B.Grids.from_workload(grids)
+    gl = B.Ligand.from_workload(gg, lig, gp)
+    fl = flops_per_eval(lig.N, lig.R, len(gl.pairs()), int(gl.tree()["moved"].sum()))
+    res = {}
+    for n in (1024, 16384, 262144, 1048576):
+        G = torch.from_numpy(W.make_genotypes(n, lig.R, grids, seed=4)).to(dev)
+        E = torch.zeros(n, device=dev)
+        gr = torch.zeros((n, 6 + lig.R), device=dev)
+        for _ in range(3):
+            B.adock_score_batch(gg, gl, gp, G, E, None, gr)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(10):
+            B.adock_score_batch(gg, gl, gp, G, E, None, gr)
+        b.record()
+        torch.cuda.synchronize()
+        ms = a.elapsed_time(b) / 10
+        res[str(n)] = {"ms": ms, "evals_per_s": n / (ms * 1e-3), "tflops": n * fl / (ms * 1e-3) / 1e12}
+    return res
+
+
+def cpu_baseline():
+    """The oracle as it stands, timed on this box's host cores on a bounded sample of the same workload."""
+    import oracle
+    grids, ligs = make_batch(1, 0)
+    og, ol = oracle.Grids.from_workload(grids), oracle.Ligand.from_workload(ligs[0])
+    par = oracle.params(W.DEFAULT_PARAMS)
+    sample_evals = 40_000
+    t0 = time.perf_counter()
+    r = oracle.dock(og, ol, par, NRUN, POP, sample_evals, seed=0)
+    dt = time.perf_counter() - t0
+    return {"value": float(r["evals"].sum()) / dt, "unit": "evals/s", "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"1 ligand x {NRUN} runs x {sample_evals} evals/run of the same workload, {dt:.1f} s"}
+
+
+if __name__ == "__main__":
+    main()

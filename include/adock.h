@@ -1,0 +1,162 @@
+/* adock.h -- C ABI of the B200-native (sm_100a) hot path of AutoDock-GPU-style LGA docking.
+ *
+ * Method: arxiv 2007.03678.  The paper names the computation -- AutoDock4 energy function
+ * (line 58), precomputed affinity / electrostatic / desolvation grid maps (line 116), Lamarckian GA with
+ * ADADELTA local search and `nrun` independent runs (lines 58, 64), maps loaded once and reused across
+ * ligands (lines 100-106) -- but prints no formulas; the exact arithmetic is fixed by the readings
+ * R1..R10 in DESIGN.md, which this header cites.
+ *
+ * Conventions
+ *   - Every function returns ADOCK_OK (0) or a negative error code; adock_last_error() returns a
+ *     thread-local description of the last failure on the calling thread.
+ *   - "host" / "device" on each pointer says where the memory must live.  The caller owns every buffer
+ *     it passes; the library owns handles until the matching adock_free_*.
+ *   - cuda_stream arguments are a cudaStream_t passed as void* (NULL = default stream).
+ *   - All work runs in this library's CUDA kernels.  There is no CPU fallback and no other backend:
+ *     without a CUDA device every compute entry point fails with ADOCK_ECUDA.
+ *
+ * Genotype (R1): float[7+R] = t_x,t_y,t_z (Angstrom, grid frame), q_w,q_x,q_y,q_z (any non-zero
+ *   quaternion, normalised on use), tau_1..tau_R (radians, relative to the input conformation, in the
+ *   order the rotatable bonds were passed to adock_load_ligand).
+ * Gradient (R1,R6): float[6+R] = dE/dt (3, kcal/mol/A), dE/domega (3, kcal/mol/rad; omega = rotation
+ *   vector of a left-multiplied infinitesimal rotation about the pivot, q <- exp(omega/2) (x) q),
+ *   dE/dtau (R, kcal/mol/rad).
+ */
+#ifndef ADOCK_H
+#define ADOCK_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ADOCK_OK 0
+#define ADOCK_EINVAL (-1) /* bad shape / index / NULL / non-finite input / params mismatch */
+#define ADOCK_ENOMEM (-2) /* host or device allocation failed */
+#define ADOCK_ECUDA (-3)  /* CUDA runtime error (text in adock_last_error) or no device */
+#define ADOCK_ELIMIT (-4) /* N > 256, R > 64, M > 16, or the ligand does not fit in shared memory */
+
+#define ADOCK_MAX_ATOMS 256
+#define ADOCK_MAX_TORSIONS 64
+#define ADOCK_MAX_MAPS 16
+
+typedef struct adock_grids adock_grids;   /* opaque, device resident, immutable, shareable across streams/ligands */
+typedef struct adock_ligand adock_ligand; /* opaque, preprocessed topology on host and device, immutable */
+
+/* Every tunable constant of the method (R4,R5,R7,R9).  Force-field fields (first ten) are
+ * baked into a ligand at adock_load_ligand; later calls must pass the same values (else ADOCK_EINVAL). */
+typedef struct adock_params {
+    float elec_scale;  /* W_el * 332.06363 (R5) */
+    float diel_A, diel_B, diel_k, diel_lambda; /* eps(r) = A + B/(1 + k exp(-lambda B r)) (R5) */
+    float w_desolv;    /* W_ds (R5) */
+    float ds_sigma;    /* sigma of the desolvation Gaussian, Angstrom (R5) */
+    float qasp;        /* S_i = solpar[type_i] + qasp*|q_i| (R5) */
+    float r_min;       /* pair distance floor, Angstrom; no force below it (R5) */
+    float k_wall;      /* out-of-box linear wall, kcal/mol/Angstrom (R4) */
+    float ad_rho, ad_eps; /* ADADELTA decay and epsilon (R7) */
+    float lsrat;       /* fraction of the population refined per generation (R9) */
+    float tourn_prob, xover_rate, mut_rate; /* GA probabilities (R9) */
+    float dmov, dang;  /* mutation amplitudes: Angstrom, radians (R9) */
+    int lsit;          /* ADADELTA iterations per local search, 1 eval each (R7) */
+    int max_gens;      /* generation cap (R9) */
+} adock_params;
+
+/* Fills *out with the defaults listed in DESIGN.md. */
+int adock_default_params(adock_params* out);
+
+/* Grid maps (R4).  host_maps: host, [M][nz][ny][nx] float32, M = T+2:
+ * maps 0..T-1 per-atom-type affinity, map T electrostatic potential (multiplied by q_i at lookup), map
+ * T+1 desolvation (multiplied by |q_i|).  spacing > 0 in Angstrom; origin: host, xyz of node (0,0,0).
+ * The maps are copied and re-laid-out on the device (caller keeps host_maps); node values must be finite. */
+int adock_load_grids(const float* host_maps, int M, int nx, int ny, int nz, float spacing, const float origin[3],
+                     adock_grids** out);
+void adock_free_grids(adock_grids* g);
+
+/* Ligand (R2).  All arrays host.  xyz [N][3] input conformation in the grid frame; type [N] in [0,T);
+ * charge [N]; bonds [nbonds][2]; rot_bonds [R][2] (either orientation; a ring bond is ADOCK_EINVAL);
+ * root_atom fixes the root fragment; pair_coeffs [T][T][4] = c12, cA, expA (6 or 10), unused -- already
+ * weighted; solpar [T], vol [T].  T+2 must be <= grids' M.  params NULL = defaults.
+ * grids may be NULL: the handle then carries only the host-side structure (accessors below work, no
+ * device memory is touched, compute entry points reject it with ADOCK_EINVAL). */
+int adock_load_ligand(const adock_grids* grids, const adock_params* params, int N, const float* xyz, const int* type,
+                      const float* charge, int nbonds, const int* bonds, int R, const int* rot_bonds, int root_atom, int T,
+                      const float* pair_coeffs, const float* solpar, const float* vol, adock_ligand** out);
+void adock_free_ligand(adock_ligand* l);
+
+/* Integer structure of a loaded ligand, canonical order (R2), for bit-exact checks.  Returned pointers
+ * are host memory owned by the handle.  pairs [npairs][2] lexicographic (i<j); tor_order [R] deepest first;
+ * moved [R][N] 0/1; rot [R][2] oriented (a_k root side, b_k moves); pivot [3]. */
+int adock_ligand_pairs(const adock_ligand* l, int* npairs, const int** ij);
+int adock_ligand_tree(const adock_ligand* l, const int** tor_order, const unsigned char** moved, const int** rot,
+                      const float** pivot);
+
+/* The ligand image the kernels stage into shared memory (host copy, owned by the handle): header,
+ * atoms renumbered fragment-contiguously, fragment tree, and the pair list packed into warp rounds of 32
+ * slots in which no atom occurs twice as i or twice as j (layout: csrc/topology.hpp).  int_of_ext [N]
+ * maps caller atom index -> internal index. */
+int adock_ligand_image(const adock_ligand* l, int* bytes, const unsigned char** image, const int** int_of_ext);
+
+/* Batched scoring (R3-R6): for each of n genotypes build the pose, interpolate the maps, sum the
+ * intramolecular pair terms and back-propagate.  d_genotypes: device [n][gstride], gstride >= 7+R.
+ * d_energies: device [n].  d_energy_terms: device [n][2] = (intermolecular, intramolecular) or NULL.
+ * d_gradients: device [n][dstride], dstride >= 6+R, or NULL for energy only.  A row with |q| < 1e-12
+ * gets NaN energy and gradient.  Asynchronous on cuda_stream. */
+int adock_score_batch(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
+                      const float* d_genotypes, int n, int gstride, float* d_energies, float* d_energy_terms,
+                      float* d_gradients, int dstride, void* cuda_stream);
+
+/* Same computation with HOST buffers: copies genotypes in, results out (synchronous). */
+int adock_score_batch_host(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
+                           const float* h_genotypes, int n, int gstride, float* h_energies, float* h_energy_terms,
+                           float* h_gradients, int dstride, void* cuda_stream);
+
+/* ADADELTA local search (R7) from each of n starting genotypes: d_genotypes device [n][gstride] in/out
+ * (best genotype seen), d_energies device [n] out (its energy), d_iters device [n] out (evals used) or NULL. */
+int adock_local_search(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
+                       float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, void* cuda_stream);
+
+/* Philox4x32-10 (R8): out[i] = philox(key, ctr[i]); key host uint32[2], d_ctr/d_out device uint32 [n][4]. */
+int adock_philox(const unsigned int key[2], const unsigned int* d_ctr, int n, unsigned int* d_out, void* cuda_stream);
+
+/* One GA generation of `nrun` runs without scoring (R9), for bit-exact decision checks.  d_pop device
+ * [nrun][P][G] (G = 7+R), d_energies device [nrun][P]; writes d_newpop [nrun][P][G] (slot 0 = elite),
+ * d_decisions device int [nrun][P][10] = a1,a2,A,b1,b2,B,do_xover,p1,p2,mutation mask; d_ls_picks device
+ * int [nrun][P] (first n_ls entries valid), *n_ls host.  generation >= 1. gen 0 with d_pop NULL:
+ * writes the initial population into d_newpop. */
+int adock_ga_generation(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params, int nrun, int P,
+                        int generation, unsigned long long seed, const float* d_pop, const float* d_energies,
+                        float* d_newpop, int* d_decisions, int* d_ls_picks, int* n_ls, void* cuda_stream);
+
+/* Full LGA docking (R9): nrun independent runs of population pop_size until each
+ * has used max_evals evaluations (checked per generation) or params->max_gens generations.  Outputs host:
+ * best_genotypes [nrun][7+R], best_energies [nrun], best_coords [nrun][N][3] or NULL, evals_used [nrun]
+ * or NULL, gens_used [nrun] or NULL.  Synchronous. */
+int adock_dock(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params, int nrun, int pop_size,
+               long long max_evals, unsigned long long seed, float* best_genotypes, float* best_energies,
+               float* best_coords, long long* evals_used, int* gens_used, void* cuda_stream);
+
+/* Multi-ligand batch (one resident grid set, many ligands): docks nlig ligands
+ * concurrently, every kernel launch covering all ligands and runs.  seeds host [nlig].  Output arrays host,
+ * ligand-major, with per-ligand genotype stride gstride >= max_l(7+R_l) and coordinate stride
+ * cstride >= max_l(N_l): best_genotypes [nlig][nrun][gstride], best_energies [nlig][nrun], best_coords
+ * [nlig][nrun][cstride][3] or NULL, evals_used [nlig][nrun] or NULL.  Synchronous. */
+int adock_dock_many(const adock_grids* grids, const adock_ligand* const* ligands, int nlig, const adock_params* params,
+                    int nrun, int pop_size, long long max_evals, const unsigned long long* seeds, int gstride,
+                    float* best_genotypes, float* best_energies, int cstride, float* best_coords, long long* evals_used,
+                    void* cuda_stream);
+
+/* Timing of the dominant kernel (the ADADELTA kernel of adock_dock / adock_dock_many) for roofline
+ * accounting: while enabled, every launch of it is bracketed by CUDA events on the launching stream.
+ * adock_profile(1) enables and resets, adock_profile(0) disables.  adock_profile_read returns the summed
+ * duration (ms), the number of launches timed and the evaluations they performed (calling thread). */
+int adock_profile(int enable);
+int adock_profile_read(double* ls_ms, long long* ls_launches, long long* ls_evals);
+
+/* Kernel launches issued by this library on the calling thread since the last reset (bench accounting). */
+long long adock_launch_count(int reset);
+
+const char* adock_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ADOCK_H */

@@ -167,7 +167,7 @@ def pair_energy(par: OPar, c12, cA, expA, qq, dsco, d):
 
 
 def score(grids: Grids, lig: Ligand, par: OPar, genos, want_grad=True, nthreads=0):
-    """float32 genotypes [n, >=7+R] -> dict(E[n], terms[n,2], grad[n,6+R], margins[n,2]) in float64."""
+    """float32 genotypes [n, >=7+R] -> dict(E[n], terms[n,2], grad[n,6+R], margins[n,2], scales[n,3]) in float64."""
     genos = _f32(genos)
     if genos.ndim == 1:
         genos = genos[None]
@@ -176,11 +176,12 @@ def score(grids: Grids, lig: Ligand, par: OPar, genos, want_grad=True, nthreads=
     terms = np.zeros((n, 2), np.float64)
     grad = np.zeros((n, 6 + lig.R), np.float64) if want_grad else None
     margins = np.zeros((n, 2), np.float64)
+    scales = np.zeros((n, 3), np.float64)
     rc = lib().orc_score(grids._h, lig._h, C.byref(par), _p(genos), n, gs, _p(E), _p(terms), _p(grad), _p(margins),
-                         int(nthreads))
+                         _p(scales), int(nthreads))
     if rc != 0:
         raise ValueError("oracle: ligand types exceed grid maps")
-    return dict(E=E, terms=terms, grad=grad, margins=margins)
+    return dict(E=E, terms=terms, grad=grad, margins=margins, scales=scales)
 
 
 def score_f64(grids: Grids, lig: Ligand, par: OPar, geno, want_grad=True):

@@ -299,10 +299,13 @@ double pair_energy(const OPar& P, double c12, double cA, double expA, double qq,
 // ------------------------------------------------------------------ R4-R6: full score of one genotype
 // grad (may be null): [dE/dt (3), dE/domega (3), dE/dtau (R)]; terms: [inter, intra];
 // margins (may be null): [min face distance in grid units, min | |x_i-x_j| - r_min | in Angstrom]
-double score(const OGrid& G, const OLig& L, const OPar& P, const double* g, double* grad, double* terms, double* margins) {
+// scales (may be null): [S_t, S_omega, S_tau] = sums of the MAGNITUDES of the terms that are added up in
+// each gradient block (conditioning of the sums; used only to set test tolerances, R10)
+double score(const OGrid& G, const OLig& L, const OPar& P, const double* g, double* grad, double* terms, double* margins,
+             double* scales = nullptr) {
     const int N = L.N;
     const double nan = std::numeric_limits<double>::quiet_NaN();
-    std::vector<double> x(3 * N), f(3 * N, 0.0);
+    std::vector<double> x(3 * N), f(3 * N, 0.0), fabs_i(N, 0.0);
     if (!pose(L, g, x.data())) {
         if (grad) for (int d = 0; d < 6 + L.R; ++d) grad[d] = nan;
         if (terms) terms[0] = terms[1] = nan;
@@ -310,8 +313,10 @@ double score(const OGrid& G, const OLig& L, const OPar& P, const double* g, doub
     }
     double fm = 1.0, pm = 1e30;
     double e_inter = 0, e_intra = 0;
-    for (int i = 0; i < N; ++i)
+    for (int i = 0; i < N; ++i) {
         e_inter += grid_atom(G, P, L.type[i], L.q[i], L.T, &x[3 * i], &f[3 * i], &fm);
+        fabs_i[i] = std::sqrt(dot(&f[3 * i], &f[3 * i]));
+    }
     const size_t np = L.pairs.size() / 2;
     for (size_t p = 0; p < np; ++p) {
         int i = L.pairs[2 * p], j = L.pairs[2 * p + 1];
@@ -323,11 +328,32 @@ double score(const OGrid& G, const OLig& L, const OPar& P, const double* g, doub
         double d = std::sqrt(dot(dv, dv)), dEdr;
         e_intra += pair_energy(P, co[0], co[1], co[2], L.q[i] * L.q[j], dsco, d, &dEdr);
         pm = std::min(pm, std::fabs(d - P.r_min));
-        if (d >= P.r_min)
+        if (d >= P.r_min) {
             for (int c = 0; c < 3; ++c) {
                 f[3 * i + c] += dEdr * dv[c] / d;
                 f[3 * j + c] -= dEdr * dv[c] / d;
             }
+            fabs_i[i] += std::fabs(dEdr);
+            fabs_i[j] += std::fabs(dEdr);
+        }
+    }
+    if (scales) {
+        scales[0] = scales[1] = scales[2] = 0;
+        for (int i = 0; i < N; ++i) {
+            double rel[3] = {x[3 * i] - g[0], x[3 * i + 1] - g[1], x[3 * i + 2] - g[2]};
+            scales[0] += fabs_i[i];
+            scales[1] += std::sqrt(dot(rel, rel)) * fabs_i[i];
+        }
+        for (int k = 0; k < L.R; ++k) {
+            double sk = 0;
+            for (int i = 0; i < N; ++i) {
+                if (!L.moved[(size_t)k * N + i]) continue;
+                double rel[3] = {x[3 * i] - x[3 * L.ta[k]], x[3 * i + 1] - x[3 * L.ta[k] + 1], x[3 * i + 2] - x[3 * L.ta[k] + 2]};
+                sk += std::sqrt(dot(rel, rel)) * fabs_i[i];
+            }
+            scales[2] += sk * sk;
+        }
+        scales[2] = std::sqrt(scales[2]);
     }
     if (terms) { terms[0] = e_inter; terms[1] = e_intra; }
     if (margins) { margins[0] = fm; margins[1] = pm; }
@@ -641,7 +667,7 @@ int orc_pair_energy(const OPar* P, double c12, double cA, double expA, double qq
 }
 
 int orc_score(void* grid, void* lig, const OPar* P, const float* genos, int n, int gstride, double* E, double* terms,
-              double* grad, double* margins, int nthreads) {
+              double* grad, double* margins, double* scales, int nthreads) {
     OGrid* G = (OGrid*)grid;
     OLig* L = (OLig*)lig;
     if (L->T + 2 > G->M) return -1;
@@ -654,7 +680,7 @@ int orc_score(void* grid, void* lig, const OPar* P, const float* genos, int n, i
         std::vector<double> g(Gn);
         for (int d = 0; d < Gn; ++d) g[d] = genos[(size_t)i * gstride + d];
         E[i] = score(*G, *L, *P, g.data(), grad ? grad + (size_t)i * D : nullptr, terms ? terms + 2 * (size_t)i : nullptr,
-                     margins ? margins + 2 * (size_t)i : nullptr);
+                     margins ? margins + 2 * (size_t)i : nullptr, scales ? scales + 3 * (size_t)i : nullptr);
     }
     return 0;
 }

@@ -1,0 +1,860 @@
+// adock.cu -- C-ABI entry points (include/adock.h) and the CUDA kernels behind them.
+// Every step of the hot path runs in the kernels of this file / device.cuh; the host code only
+// validates arguments, preprocesses the ligand topology once (topology.hpp) and launches.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/adock.h"
+#include "device.cuh"
+
+using namespace adock;
+
+// =================================================================== handles and errors
+struct adock_grids {
+    GridDev dev{};
+    int M = 0;
+    float4* cells = nullptr;
+};
+
+struct adock_ligand {
+    Topology tp;
+    unsigned char* d_blob = nullptr;
+    int* d_ext_of_int = nullptr;
+    int blob_bytes = 0;
+    int scratch_floats = 0;
+    float w_desolv = 0, qasp = 0;
+};
+
+static thread_local std::string g_err;
+static thread_local long long g_launches = 0;
+static thread_local bool g_prof = false;                  // adock_profile: time every dock_ls_kernel launch
+static thread_local double g_ls_ms = 0;
+static thread_local long long g_ls_launches = 0, g_ls_evals = 0;
+
+static int fail(int code, const std::string& msg) {
+    g_err = msg;
+    return code;
+}
+#define CUDA_TRY(expr)                                                                     \
+    do {                                                                                   \
+        cudaError_t e_ = (expr);                                                           \
+        if (e_ != cudaSuccess) return fail(ADOCK_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e_)); \
+    } while (0)
+
+extern "C" const char* adock_last_error(void) { return g_err.c_str(); }
+extern "C" long long adock_launch_count(int reset) {
+    long long v = g_launches;
+    if (reset) g_launches = 0;
+    return v;
+}
+
+extern "C" int adock_profile(int enable) {
+    g_prof = enable != 0;
+    g_ls_ms = 0; g_ls_launches = 0; g_ls_evals = 0;
+    return ADOCK_OK;
+}
+extern "C" int adock_profile_read(double* ls_ms, long long* ls_launches, long long* ls_evals) {
+    if (ls_ms) *ls_ms = g_ls_ms;
+    if (ls_launches) *ls_launches = g_ls_launches;
+    if (ls_evals) *ls_evals = g_ls_evals;
+    return ADOCK_OK;
+}
+
+extern "C" int adock_default_params(adock_params* p) {
+    if (!p) return fail(ADOCK_EINVAL, "params is NULL");
+    p->elec_scale = (float)(0.1406 * 332.06363);
+    p->diel_A = -8.5525f; p->diel_B = 86.9525f; p->diel_k = 7.7839f; p->diel_lambda = 0.003627f;
+    p->w_desolv = 0.1322f; p->ds_sigma = 3.6f; p->qasp = 0.01097f; p->r_min = 0.5f; p->k_wall = 1000.0f;
+    p->ad_rho = 0.8f; p->ad_eps = 1e-2f; p->lsrat = 0.06f;
+    p->tourn_prob = 0.60f; p->xover_rate = 0.80f; p->mut_rate = 0.02f; p->dmov = 2.0f; p->dang = 1.57079632679489662f;
+    p->lsit = 300; p->max_gens = 27000;
+    return ADOCK_OK;
+}
+
+static ParDev make_pardev(const adock_params& p) {
+    const double log2e = 1.4426950408889634;
+    ParDev d;
+    d.elec_scale = p.elec_scale; d.diel_A = p.diel_A; d.diel_B = p.diel_B; d.diel_k = p.diel_k;
+    d.lamB = (float)((double)p.diel_lambda * (double)p.diel_B);
+    d.mlamB_log2e = (float)(-(double)p.diel_lambda * (double)p.diel_B * log2e);
+    d.inv_sig2 = (float)(1.0 / ((double)p.ds_sigma * (double)p.ds_sigma));
+    d.mhalf_inv_sig2_log2e = (float)(-0.5 * log2e / ((double)p.ds_sigma * (double)p.ds_sigma));
+    d.rmin2 = p.r_min * p.r_min; d.k_wall = p.k_wall; d.k_wall_h = 0.f;    // k_wall_h set per grid
+    d.ad_rho = p.ad_rho; d.ad_eps = p.ad_eps;
+    d.tourn_prob = p.tourn_prob; d.xover_rate = p.xover_rate; d.mut_rate = p.mut_rate; d.dmov = p.dmov; d.dang = p.dang;
+    d.lsit = p.lsit;
+    return d;
+}
+
+static int check_params(const adock_params* in, const adock_ligand* l, adock_params& out) {
+    if (in) out = *in; else adock_default_params(&out);
+    const float* f = &out.elec_scale;
+    for (int i = 0; i < 18; ++i)
+        if (!std::isfinite(f[i])) return fail(ADOCK_EINVAL, "non-finite parameter");
+    if (!(out.ds_sigma > 0) || !(out.r_min > 0) || out.lsit < 0 || out.max_gens < 0 || !(out.ad_eps > 0))
+        return fail(ADOCK_EINVAL, "parameter out of range");
+    if (l && !l->d_blob) return fail(ADOCK_EINVAL, "host-only ligand handle (loaded with grids == NULL)");
+    if (l && (out.w_desolv != l->w_desolv || out.qasp != l->qasp))
+        return fail(ADOCK_EINVAL, "w_desolv/qasp differ from the values baked into the ligand at load time");
+    return ADOCK_OK;
+}
+
+// =================================================================== grids
+__global__ void relayout_kernel(const float* __restrict__ maps, float4* __restrict__ cells, int T, int nx, int ny, int nz) {
+    const long long ncell = (long long)T * nz * ny * (nx - 1);
+    const long long plane = (long long)nz * ny * nx;
+    for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x) {
+        const int ix = (int)(c % (nx - 1));
+        const long long row = c / (nx - 1);               // (t*nz + z)*ny + y
+        const long long zy = row % ((long long)nz * ny);
+        const int t = (int)(row / ((long long)nz * ny));
+        const long long p = zy * nx + ix;
+        cells[2 * c] = make_float4(maps[t * plane + p], maps[T * plane + p], maps[(T + 1) * plane + p], 0.f);
+        cells[2 * c + 1] = make_float4(maps[t * plane + p + 1], maps[T * plane + p + 1], maps[(T + 1) * plane + p + 1], 0.f);
+    }
+}
+
+extern "C" int adock_load_grids(const float* host_maps, int M, int nx, int ny, int nz, float spacing, const float origin[3],
+                                adock_grids** out) {
+    if (!host_maps || !origin || !out) return fail(ADOCK_EINVAL, "NULL argument");
+    if (M < 3 || nx < 2 || ny < 2 || nz < 2 || !(spacing > 0) || !std::isfinite(spacing)) return fail(ADOCK_EINVAL, "bad grid shape");
+    if (M > ADOCK_MAX_MAPS) return fail(ADOCK_ELIMIT, "more than ADOCK_MAX_MAPS maps");
+    if (nx > 1024 || ny > 1024 || nz > 1024) return fail(ADOCK_ELIMIT, "grid dimension above 1024");
+    const size_t npts = (size_t)nx * ny * nz;
+    for (size_t i = 0; i < (size_t)M * npts; ++i)
+        if (!std::isfinite(host_maps[i])) return fail(ADOCK_EINVAL, "non-finite map value");
+    const int T = M - 2;
+    float* d_raw = nullptr;
+    float4* cells = nullptr;
+    const size_t ncell = (size_t)T * nz * ny * (nx - 1);
+    cudaError_t e = cudaMalloc(&d_raw, (size_t)M * npts * sizeof(float));
+    if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("cudaMalloc: ") + cudaGetErrorString(e));
+    e = cudaMalloc(&cells, ncell * 2 * sizeof(float4));
+    if (e != cudaSuccess) { cudaFree(d_raw); return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("cudaMalloc: ") + cudaGetErrorString(e)); }
+    e = cudaMemcpy(d_raw, host_maps, (size_t)M * npts * sizeof(float), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        relayout_kernel<<<1184, 256>>>(d_raw, cells, T, nx, ny, nz);
+        ++g_launches;
+        e = cudaDeviceSynchronize();
+    }
+    cudaFree(d_raw);
+    if (e != cudaSuccess) { cudaFree(cells); return fail(ADOCK_ECUDA, std::string("grid upload: ") + cudaGetErrorString(e)); }
+    adock_grids* g = new adock_grids;
+    g->M = M; g->cells = cells;
+    g->dev.cells = cells;
+    g->dev.type_stride = (long long)nz * ny * (nx - 1) * 2;
+    g->dev.nx = nx; g->dev.ny = ny; g->dev.nz = nz; g->dev.T = T;
+    g->dev.h = spacing; g->dev.inv_h = 1.0f / spacing;
+    g->dev.ox = origin[0]; g->dev.oy = origin[1]; g->dev.oz = origin[2];
+    g->dev.bx = spacing * (nx - 1); g->dev.by = spacing * (ny - 1); g->dev.bz = spacing * (nz - 1);
+    *out = g;
+    return ADOCK_OK;
+}
+
+extern "C" void adock_free_grids(adock_grids* g) {
+    if (!g) return;
+    cudaFree(g->cells);
+    delete g;
+}
+
+// =================================================================== ligand
+extern "C" int adock_load_ligand(const adock_grids* grids, const adock_params* params, int N, const float* xyz, const int* type,
+                                 const float* charge, int nbonds, const int* bonds, int R, const int* rot_bonds, int root_atom,
+                                 int T, const float* pair_coeffs, const float* solpar, const float* vol, adock_ligand** out) {
+    if (!xyz || !type || !charge || !pair_coeffs || !solpar || !vol || !out || (nbonds > 0 && !bonds) || (R > 0 && !rot_bonds))
+        return fail(ADOCK_EINVAL, "NULL argument");
+    if (N < 1 || R < 0 || T < 1 || nbonds < 0 || root_atom < 0 || root_atom >= N) return fail(ADOCK_EINVAL, "bad ligand shape");
+    if (N > ADOCK_MAX_ATOMS || R > ADOCK_MAX_TORSIONS) return fail(ADOCK_ELIMIT, "ligand exceeds ADOCK_MAX_ATOMS / ADOCK_MAX_TORSIONS");
+    if (grids && T + 2 > grids->M) return fail(ADOCK_EINVAL, "ligand atom types exceed the loaded maps");
+    adock_params p;
+    int rc = check_params(params, nullptr, p);
+    if (rc) return rc;
+    for (int i = 0; i < N; ++i) {
+        if (type[i] < 0 || type[i] >= T) return fail(ADOCK_EINVAL, "atom type out of range");
+        if (!std::isfinite(charge[i]) || !std::isfinite(xyz[3 * i]) || !std::isfinite(xyz[3 * i + 1]) || !std::isfinite(xyz[3 * i + 2]))
+            return fail(ADOCK_EINVAL, "non-finite ligand input");
+    }
+    for (int i = 0; i < T * T * 4; ++i) if (!std::isfinite(pair_coeffs[i])) return fail(ADOCK_EINVAL, "non-finite pair coefficient");
+    adock_ligand* l = new adock_ligand;
+    if (!build_topology(l->tp, N, xyz, type, charge, nbonds, bonds, R, rot_bonds, root_atom, T, pair_coeffs, solpar, vol, p.w_desolv, p.qasp)) {
+        std::string msg = l->tp.error;
+        delete l;
+        return fail(ADOCK_EINVAL, msg);
+    }
+    l->w_desolv = p.w_desolv; l->qasp = p.qasp;
+    l->blob_bytes = (int)l->tp.blob.size();
+    l->scratch_floats = warp_scratch_floats(N, l->tp.nfrag, R);
+    if (16 + l->blob_bytes + 4 * l->scratch_floats > 227 * 1024) {
+        delete l;
+        return fail(ADOCK_ELIMIT, "ligand image does not fit in shared memory");
+    }
+    if (!grids) {           // host-only handle: integer structure and image for inspection
+        *out = l;
+        return ADOCK_OK;
+    }
+    cudaError_t e = cudaMalloc(&l->d_blob, l->blob_bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&l->d_ext_of_int, N * sizeof(int));
+    if (e == cudaSuccess) e = cudaMemcpy(l->d_blob, l->tp.blob.data(), l->blob_bytes, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(l->d_ext_of_int, l->tp.ext_of_int.data(), N * sizeof(int), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        cudaFree(l->d_blob); cudaFree(l->d_ext_of_int);
+        delete l;
+        return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("ligand upload: ") + cudaGetErrorString(e));
+    }
+    *out = l;
+    return ADOCK_OK;
+}
+
+extern "C" void adock_free_ligand(adock_ligand* l) {
+    if (!l) return;
+    cudaFree(l->d_blob);
+    cudaFree(l->d_ext_of_int);
+    delete l;
+}
+
+extern "C" int adock_ligand_pairs(const adock_ligand* l, int* npairs, const int** ij) {
+    if (!l || !npairs || !ij) return fail(ADOCK_EINVAL, "NULL argument");
+    *npairs = (int)l->tp.pairs.size() / 2;
+    *ij = l->tp.pairs.data();
+    return ADOCK_OK;
+}
+
+extern "C" int adock_ligand_tree(const adock_ligand* l, const int** tor_order, const unsigned char** moved, const int** rot,
+                                 const float** pivot) {
+    if (!l) return fail(ADOCK_EINVAL, "NULL argument");
+    if (tor_order) *tor_order = l->tp.tor_order.data();
+    if (moved) *moved = l->tp.moved.data();
+    if (rot) *rot = l->tp.rot.data();
+    if (pivot) *pivot = l->tp.pivot;
+    return ADOCK_OK;
+}
+
+extern "C" int adock_ligand_image(const adock_ligand* l, int* bytes, const unsigned char** image, const int** int_of_ext) {
+    if (!l || !bytes || !image) return fail(ADOCK_EINVAL, "NULL argument");
+    *bytes = l->blob_bytes;
+    *image = l->tp.blob.data();
+    if (int_of_ext) *int_of_ext = l->tp.int_of_ext.data();
+    return ADOCK_OK;
+}
+
+// =================================================================== launch geometry
+static int g_sm_count = 0, g_smem_optin = 0;
+static int device_props() {
+    if (g_sm_count) return ADOCK_OK;
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&g_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    return ADOCK_OK;
+}
+static size_t cta_smem(int blob_bytes, int scratch_floats, int warps) { return 16 + (size_t)blob_bytes + (size_t)warps * scratch_floats * 4; }
+// largest warp count <= want whose shared memory fits
+static int fit_warps(int blob_bytes, int scratch_floats, int want) {
+    int w = want;
+    while (w > 1 && cta_smem(blob_bytes, scratch_floats, w) > (size_t)g_smem_optin) w >>= 1;
+    return cta_smem(blob_bytes, scratch_floats, w) <= (size_t)g_smem_optin ? w : 0;
+}
+
+// =================================================================== scoring kernel (rows a1-a4)
+struct ScoreArgs {
+    const unsigned char* blob;
+    const float* genos;
+    float* E;
+    float* terms;
+    float* grads;
+    int blob_bytes, n, gstride, dstride;
+};
+
+template <bool GRAD>
+__global__ void __launch_bounds__(256) score_kernel(GridDev G, ParDev P, ScoreArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned char* blob = smem + 16;
+    stage_ligand(blob, a.blob, a.blob_bytes, reinterpret_cast<uint64_t*>(smem), 0);
+    const LigS L = lig_view(blob);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
+    const WarpS S = warp_view(reinterpret_cast<float*>(blob + a.blob_bytes) + (size_t)warp * warp_scratch_floats(L.N, L.nfrag, L.R), L);
+    const int Gn = 7 + L.R, D = 6 + L.R;
+    for (int idx = blockIdx.x * W + warp; idx < a.n; idx += gridDim.x * W) {
+        for (int d = lane; d < Gn; d += 32) S.geno[d] = a.genos[(size_t)idx * a.gstride + d];
+        __syncwarp();
+        float ei, ea;
+        const float e = eval_pose<GRAD>(L, G, P, S, lane, ei, ea);
+        if (lane == 0) {
+            a.E[idx] = e;
+            if (a.terms) { a.terms[2 * (size_t)idx] = ei; a.terms[2 * (size_t)idx + 1] = ea; }
+        }
+        if (GRAD)
+            for (int d = lane; d < D; d += 32) a.grads[(size_t)idx * a.dstride + d] = S.grad[d];
+        __syncwarp();
+    }
+}
+
+static int launch_score(const adock_grids* grids, const adock_ligand* lig, const adock_params& p, const float* d_genos, int n,
+                        int gstride, float* d_E, float* d_terms, float* d_grads, int dstride, cudaStream_t st) {
+    int rc = device_props();
+    if (rc) return rc;
+    const int W = fit_warps(lig->blob_bytes, lig->scratch_floats, 8);
+    if (!W) return fail(ADOCK_ELIMIT, "ligand does not fit in shared memory");
+    const size_t smem = cta_smem(lig->blob_bytes, lig->scratch_floats, W);
+    ParDev P = make_pardev(p);
+    P.k_wall_h = p.k_wall * grids->dev.h;
+    ScoreArgs a{lig->d_blob, d_genos, d_E, d_terms, d_grads, lig->blob_bytes, n, gstride, dstride};
+    int per_sm = 1;
+    if (d_grads) {
+        CUDA_TRY(cudaFuncSetAttribute(score_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, score_kernel<true>, W * 32, smem));
+    } else {
+        CUDA_TRY(cudaFuncSetAttribute(score_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, score_kernel<false>, W * 32, smem));
+    }
+    if (per_sm < 1) per_sm = 1;
+    long long want = ((long long)n + W - 1) / W;
+    int grid = (int)std::min<long long>(want, (long long)g_sm_count * per_sm);       // persistent: a multiple of the SM count
+    if (grid < 1) grid = 1;
+    if (d_grads) score_kernel<true><<<grid, W * 32, smem, st>>>(grids->dev, P, a);
+    else score_kernel<false><<<grid, W * 32, smem, st>>>(grids->dev, P, a);
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    return ADOCK_OK;
+}
+
+extern "C" int adock_score_batch(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
+                                 const float* d_genotypes, int n, int gstride, float* d_energies, float* d_energy_terms,
+                                 float* d_gradients, int dstride, void* cuda_stream) {
+    if (!grids || !ligand) return fail(ADOCK_EINVAL, "NULL handle");
+    if (n < 0) return fail(ADOCK_EINVAL, "n < 0");
+    if (n == 0) return ADOCK_OK;
+    if (!d_genotypes || !d_energies) return fail(ADOCK_EINVAL, "NULL buffer");
+    if (gstride < 7 + ligand->tp.R || (d_gradients && dstride < 6 + ligand->tp.R)) return fail(ADOCK_EINVAL, "stride too small");
+    adock_params p;
+    int rc = check_params(params, ligand, p);
+    if (rc) return rc;
+    return launch_score(grids, ligand, p, d_genotypes, n, gstride, d_energies, d_energy_terms, d_gradients, dstride, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int adock_score_batch_host(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
+                                      const float* h_genotypes, int n, int gstride, float* h_energies, float* h_energy_terms,
+                                      float* h_gradients, int dstride, void* cuda_stream) {
+    if (!grids || !ligand) return fail(ADOCK_EINVAL, "NULL handle");
+    if (n < 0) return fail(ADOCK_EINVAL, "n < 0");
+    if (n == 0) return ADOCK_OK;
+    if (!h_genotypes || !h_energies) return fail(ADOCK_EINVAL, "NULL buffer");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    float *dg = nullptr, *dE = nullptr, *dT = nullptr, *dG = nullptr;
+    const size_t gb = (size_t)n * gstride * 4, db = (size_t)n * dstride * 4;
+    CUDA_TRY(cudaMalloc(&dg, gb));
+    int rc = ADOCK_OK;
+    cudaError_t e = cudaMalloc(&dE, (size_t)n * 4);
+    if (e == cudaSuccess && h_energy_terms) e = cudaMalloc(&dT, (size_t)n * 8);
+    if (e == cudaSuccess && h_gradients) e = cudaMalloc(&dG, db);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dg, h_genotypes, gb, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) rc = adock_score_batch(grids, ligand, params, dg, n, gstride, dE, dT, dG, dstride, st);
+    if (e == cudaSuccess && rc == ADOCK_OK) e = cudaMemcpyAsync(h_energies, dE, (size_t)n * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && rc == ADOCK_OK && dT) e = cudaMemcpyAsync(h_energy_terms, dT, (size_t)n * 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && rc == ADOCK_OK && dG) e = cudaMemcpyAsync(h_gradients, dG, db, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(dg); cudaFree(dE); cudaFree(dT); cudaFree(dG);
+    if (e != cudaSuccess) return fail(ADOCK_ECUDA, std::string("score_batch_host: ") + cudaGetErrorString(e));
+    return rc;
+}
+
+// =================================================================== Philox test hook (R8)
+__global__ void philox_kernel(uint32_t k0, uint32_t k1, const uint4* ctr, int n, uint4* out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = philox4x32_10(k0, k1, ctr[i]);
+}
+extern "C" int adock_philox(const unsigned int key[2], const unsigned int* d_ctr, int n, unsigned int* d_out, void* cuda_stream) {
+    if (!key || (n > 0 && (!d_ctr || !d_out)) || n < 0) return fail(ADOCK_EINVAL, "bad argument");
+    if (n == 0) return ADOCK_OK;
+    philox_kernel<<<(n + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(key[0], key[1], (const uint4*)d_ctr, n, (uint4*)d_out);
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    return ADOCK_OK;
+}
+
+// =================================================================== local search on an array (row a5)
+struct LsArgs {
+    const unsigned char* blob;
+    float* genos;
+    float* E;
+    int* iters;
+    int blob_bytes, n, gstride;
+};
+
+__global__ void __launch_bounds__(128) ls_array_kernel(GridDev G, ParDev P, LsArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned char* blob = smem + 16;
+    stage_ligand(blob, a.blob, a.blob_bytes, reinterpret_cast<uint64_t*>(smem), 0);
+    const LigS L = lig_view(blob);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
+    const WarpS S = warp_view(reinterpret_cast<float*>(blob + a.blob_bytes) + (size_t)warp * warp_scratch_floats(L.N, L.nfrag, L.R), L);
+    const int Gn = 7 + L.R;
+    const int idx = blockIdx.x * W + warp;
+    if (idx >= a.n) return;
+    for (int d = lane; d < Gn; d += 32) S.geno[d] = a.genos[(size_t)idx * a.gstride + d];
+    __syncwarp();
+    int iters = 0;
+    const float e = adadelta_search(L, G, P, S, lane, __int_as_float(0x7fc00000), iters);
+    for (int d = lane; d < Gn; d += 32) a.genos[(size_t)idx * a.gstride + d] = S.best[d];
+    if (lane == 0) {
+        a.E[idx] = e;
+        if (a.iters) a.iters[idx] = iters;
+    }
+}
+
+extern "C" int adock_local_search(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
+                                  float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, void* cuda_stream) {
+    if (!grids || !ligand) return fail(ADOCK_EINVAL, "NULL handle");
+    if (n < 0) return fail(ADOCK_EINVAL, "n < 0");
+    if (n == 0) return ADOCK_OK;
+    if (!d_genotypes || !d_energies || gstride < 7 + ligand->tp.R) return fail(ADOCK_EINVAL, "bad buffer");
+    adock_params p;
+    int rc = check_params(params, ligand, p);
+    if (rc) return rc;
+    rc = device_props();
+    if (rc) return rc;
+    const int W = fit_warps(ligand->blob_bytes, ligand->scratch_floats, 4);
+    if (!W) return fail(ADOCK_ELIMIT, "ligand does not fit in shared memory");
+    const size_t smem = cta_smem(ligand->blob_bytes, ligand->scratch_floats, W);
+    CUDA_TRY(cudaFuncSetAttribute(ls_array_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ParDev P = make_pardev(p);
+    P.k_wall_h = p.k_wall * grids->dev.h;
+    LsArgs a{ligand->d_blob, d_genotypes, d_energies, d_iters, ligand->blob_bytes, n, gstride};
+    ls_array_kernel<<<(n + W - 1) / W, W * 32, smem, (cudaStream_t)cuda_stream>>>(grids->dev, P, a);
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    return ADOCK_OK;
+}
+
+// =================================================================== LGA docking (rows a5-a7)
+struct RunState {           // 32 bytes
+    long long evals;
+    int gen, cur, active, ls_acc;
+    int pad[2];
+};
+struct DockJob {
+    const unsigned char* blob;
+    const int* ext_of_int;
+    float* pop;             // [2][nrun][P][Gn]
+    float* E;               // [2][nrun][P]
+    RunState* st;           // [nrun]
+    int* picks;             // [nrun][P]
+    int* fy;                // [nrun][P] Fisher-Yates scratch
+    float* out_geno;        // [nrun][gstride]
+    float* out_E;           // [nrun]
+    float* out_xyz;         // [nrun][cstride][3] or NULL
+    long long* out_evals;   // [nrun]
+    int* out_gens;          // [nrun]
+    unsigned long long seed;
+    int blob_bytes, Gn, N, R;
+};
+struct DockDims {
+    int nrun, P, n_ls, upj;         // upj = CTAs per job for this launch
+    long long max_evals;
+    int max_gens, gstride, cstride;
+};
+
+#define DOCK_PROLOGUE(WARPS_EXPR)                                                                                         \
+    extern __shared__ __align__(128) unsigned char smem[];                                                               \
+    const DockJob job = jobs[blockIdx.x / dm.upj];                                                                       \
+    unsigned char* blob = smem + 16;                                                                                     \
+    stage_ligand(blob, job.blob, job.blob_bytes, reinterpret_cast<uint64_t*>(smem), 0);                                  \
+    const LigS L = lig_view(blob);                                                                                       \
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;                                     \
+    const WarpS S = warp_view(reinterpret_cast<float*>(blob + job.blob_bytes) + (size_t)warp * warp_scratch_floats(L.N, L.nfrag, L.R), L); \
+    const int ind = (blockIdx.x % dm.upj) * W + warp;                                                                    \
+    const int Gn = job.Gn;                                                                                               \
+    (void)Gn; (void)S; (void)lane;
+
+// generation 0: random population + its energies; run bookkeeping
+__global__ void __launch_bounds__(256) dock_init_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs, DockDims dm) {
+    DOCK_PROLOGUE()
+    if (ind >= dm.nrun * dm.P) return;
+    const int run = ind / dm.P, slot = ind % dm.P;
+    ga_init_individual(G, L.R, job.seed, (uint32_t)ind, S.geno, lane);
+    __syncwarp();
+    float* dst = job.pop + (size_t)ind * Gn;
+    for (int d = lane; d < Gn; d += 32) dst[d] = S.geno[d];
+    float ei, ea;
+    const float e = eval_pose<false>(L, G, P, S, lane, ei, ea);
+    if (lane == 0) {
+        job.E[ind] = e;
+        if (slot == 0) {
+            RunState s;
+            s.evals = dm.P; s.gen = 0; s.cur = 0; s.ls_acc = 0; s.pad[0] = s.pad[1] = 0;
+            s.active = (s.evals < dm.max_evals && dm.max_gens > 0) ? 1 : 0;
+            job.st[run] = s;
+        }
+    }
+}
+
+// one GA generation: elitism, tournament selection, two-point crossover, mutation, scoring of the offspring;
+// the slot-0 warp also draws this generation's local-search subset
+template <bool SCORE>
+__global__ void __launch_bounds__(256) dock_ga_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs, DockDims dm,
+                                                      int* __restrict__ decisions) {
+    DOCK_PROLOGUE()
+    if (ind >= dm.nrun * dm.P) return;
+    const int run = ind / dm.P, slot = ind % dm.P;
+    const RunState st = job.st[run];
+    if (!st.active) return;
+    const size_t popsz = (size_t)dm.nrun * dm.P;
+    const float* spop = job.pop + ((size_t)st.cur * popsz + (size_t)run * dm.P) * Gn;
+    const float* sE = job.E + (size_t)st.cur * popsz + (size_t)run * dm.P;
+    float* dpop = job.pop + ((size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P) * Gn;
+    float* dE = job.E + (size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P;
+    const uint32_t gen = (uint32_t)st.gen + 1u;
+    int* dec = decisions ? decisions + ((size_t)(blockIdx.x / dm.upj) * popsz + ind) * 10 : nullptr;
+    if (slot == 0) {
+        float be = __int_as_float(0x7f800000);
+        int bi = 0x7fffffff;
+        for (int s = lane; s < dm.P; s += 32) {
+            const float e = sE[s];
+            if (e < be) { be = e; bi = s; }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const float oe = __shfl_xor_sync(kFull, be, o);
+            const int oi = __shfl_xor_sync(kFull, bi, o);
+            if (oe < be || (oe == be && oi < bi)) { be = oe; bi = oi; }
+        }
+        if (bi == 0x7fffffff) bi = 0;                    // every energy non-finite: keep slot 0
+        for (int d = lane; d < Gn; d += 32) dpop[d] = spop[(size_t)bi * Gn + d];
+        if (lane == 0) {
+            dE[0] = sE[bi];
+            if (dec) { for (int k = 0; k < 10; ++k) dec[k] = 0; dec[2] = bi; }
+        }
+        // local-search subset: slot 0 + first n_ls-1 entries of a partial Fisher-Yates shuffle of 1..P-1
+        int* picks = job.picks + (size_t)run * dm.P;
+        if (dm.n_ls >= dm.P) {
+            for (int s = lane; s < dm.P; s += 32) picks[s] = s;
+        } else if (dm.n_ls > 0) {
+            int* fy = job.fy + (size_t)run * dm.P;
+            for (int s = lane; s < dm.P - 1; s += 32) fy[s] = s + 1;
+            __syncwarp();
+            if (lane == 0) {
+                picks[0] = 0;
+                uint4 r = make_uint4(0, 0, 0, 0);
+                for (int m = 0; m < dm.n_ls - 1; ++m) {
+                    if ((m & 3) == 0) r = draw4(job.seed, (uint32_t)(m >> 2), kLsPick, (uint32_t)(run * dm.P), gen);
+                    const int j = m + below(pick_word(r, m & 3), dm.P - 1 - m);
+                    const int t = fy[m]; fy[m] = fy[j]; fy[j] = t;
+                    picks[1 + m] = fy[m];
+                }
+            }
+        }
+        return;
+    }
+    ga_make_child(P, dm.P, L.R, job.seed, (uint32_t)ind, gen, spop, sE, S.geno, dec, lane);
+    for (int d = lane; d < Gn; d += 32) dpop[(size_t)slot * Gn + d] = S.geno[d];
+    if (SCORE) {
+        float ei, ea;
+        const float e = eval_pose<false>(L, G, P, S, lane, ei, ea);
+        if (lane == 0) dE[slot] = e;
+    }
+}
+
+// ADADELTA on the selected individuals of the new population (Lamarckian write-back)
+__global__ void __launch_bounds__(128) dock_ls_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs, DockDims dm) {
+    DOCK_PROLOGUE()
+    if (ind >= dm.nrun * dm.n_ls) return;
+    const int run = ind / dm.n_ls, l = ind % dm.n_ls;
+    const RunState st = job.st[run];
+    if (!st.active) return;
+    const size_t popsz = (size_t)dm.nrun * dm.P;
+    const int slot = job.picks[(size_t)run * dm.P + l];
+    float* g = job.pop + ((size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P + slot) * Gn;
+    float* e = job.E + (size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P + slot;
+    for (int d = lane; d < Gn; d += 32) S.geno[d] = g[d];
+    __syncwarp();
+    int iters = 0;
+    const float be = adadelta_search(L, G, P, S, lane, *e, iters);
+    for (int d = lane; d < Gn; d += 32) g[d] = S.best[d];
+    if (lane == 0) {
+        *e = be;
+        atomicAdd(&job.st[run].ls_acc, iters);
+    }
+}
+
+// end of generation: eval accounting, buffer flip, termination test
+__global__ void dock_commit_kernel(const DockJob* __restrict__ jobs, int njobs, DockDims dm, int* __restrict__ any_active) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= njobs * dm.nrun) return;
+    RunState* s = jobs[i / dm.nrun].st + (i % dm.nrun);
+    if (!s->active) return;
+    s->evals += (long long)(dm.P - 1) + s->ls_acc;
+    s->ls_acc = 0;
+    s->gen += 1;
+    s->cur ^= 1;
+    s->active = (s->evals < dm.max_evals && s->gen < dm.max_gens) ? 1 : 0;
+    if (s->active) atomicOr(any_active, 1);
+}
+
+// per run: best individual of the final population, its pose in the caller's atom order
+__global__ void __launch_bounds__(128) dock_final_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs, DockDims dm) {
+    DOCK_PROLOGUE()
+    if (ind >= dm.nrun) return;
+    const int run = ind;
+    const RunState st = job.st[run];
+    const size_t popsz = (size_t)dm.nrun * dm.P;
+    const float* pop = job.pop + ((size_t)st.cur * popsz + (size_t)run * dm.P) * Gn;
+    const float* E = job.E + (size_t)st.cur * popsz + (size_t)run * dm.P;
+    float be = __int_as_float(0x7f800000);
+    int bi = 0x7fffffff;
+    for (int s = lane; s < dm.P; s += 32) {
+        const float e = E[s];
+        if (e < be) { be = e; bi = s; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const float oe = __shfl_xor_sync(kFull, be, o);
+        const int oi = __shfl_xor_sync(kFull, bi, o);
+        if (oe < be || (oe == be && oi < bi)) { be = oe; bi = oi; }
+    }
+    if (bi == 0x7fffffff) bi = 0;
+    for (int d = lane; d < Gn; d += 32) {
+        const float v = pop[(size_t)bi * Gn + d];
+        S.geno[d] = v;
+        job.out_geno[(size_t)run * dm.gstride + d] = v;
+    }
+    __syncwarp();
+    float ei, ea;
+    eval_pose<false>(L, G, P, S, lane, ei, ea);
+    if (job.out_xyz)
+        for (int i = lane; i < L.N; i += 32) {
+            const float4 x = S.X[i];
+            float* o = job.out_xyz + ((size_t)run * dm.cstride + job.ext_of_int[i]) * 3;
+            o[0] = x.x; o[1] = x.y; o[2] = x.z;
+        }
+    if (lane == 0) {
+        job.out_E[run] = E[bi];
+        job.out_evals[run] = st.evals;
+        job.out_gens[run] = st.gen;
+    }
+}
+
+namespace {
+struct DevBuf {             // frees on scope exit
+    std::vector<void*> ptrs;
+    ~DevBuf() { for (void* p : ptrs) cudaFree(p); }
+    template <class T> cudaError_t alloc(T** p, size_t n) {
+        cudaError_t e = cudaMalloc((void**)p, n ? n : 1);
+        if (e == cudaSuccess) ptrs.push_back(*p);
+        return e;
+    }
+};
+int n_ls_of(const adock_params& p, int P) {
+    int n = (int)std::ceil((double)p.lsrat * P - 1e-9);
+    return std::max(0, std::min(P, n));
+}
+}  // namespace
+
+static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, int nlig, const adock_params* params, int nrun,
+                     int Pn, long long max_evals, const unsigned long long* seeds, int gstride, float* best_genotypes,
+                     float* best_energies, int cstride, float* best_coords, long long* evals_used, int* gens_used, cudaStream_t stm) {
+    if (!grids || !ligs || !seeds || !best_genotypes || !best_energies) return fail(ADOCK_EINVAL, "NULL argument");
+    if (nlig < 1 || nrun < 1 || Pn < 2 || max_evals < 0) return fail(ADOCK_EINVAL, "bad docking dimensions");
+    if ((long long)nrun * Pn > (1ll << 30)) return fail(ADOCK_ELIMIT, "nrun*pop_size too large");
+    int rc = device_props();
+    if (rc) return rc;
+    adock_params p;
+    int maxblob = 0, maxscr = 0;
+    for (int l = 0; l < nlig; ++l) {
+        if (!ligs[l]) return fail(ADOCK_EINVAL, "NULL ligand");
+        rc = check_params(params, ligs[l], p);
+        if (rc) return rc;
+        if (gstride < 7 + ligs[l]->tp.R || (best_coords && cstride < ligs[l]->tp.N)) return fail(ADOCK_EINVAL, "output stride too small");
+        maxblob = std::max(maxblob, ligs[l]->blob_bytes);
+        maxscr = std::max(maxscr, ligs[l]->scratch_floats);
+    }
+    const int Wga = fit_warps(maxblob, maxscr, 8), Wls = fit_warps(maxblob, maxscr, 4);
+    if (!Wga || !Wls) return fail(ADOCK_ELIMIT, "ligand does not fit in shared memory");
+    ParDev P = make_pardev(p);
+    P.k_wall_h = p.k_wall * grids->dev.h;
+    DockDims dm{};
+    dm.nrun = nrun; dm.P = Pn; dm.n_ls = n_ls_of(p, Pn); dm.max_evals = max_evals; dm.max_gens = p.max_gens;
+    dm.gstride = gstride; dm.cstride = cstride;
+
+    DevBuf buf;
+    std::vector<DockJob> jobs(nlig);
+    const size_t popsz = (size_t)nrun * Pn;
+    float *d_out_geno = nullptr, *d_out_E = nullptr, *d_out_xyz = nullptr;
+    long long* d_out_evals = nullptr;
+    int *d_out_gens = nullptr, *d_flag = nullptr;
+    DockJob* d_jobs = nullptr;
+    cudaError_t e = buf.alloc(&d_out_geno, (size_t)nlig * nrun * gstride * 4);
+    if (e == cudaSuccess) e = buf.alloc(&d_out_E, (size_t)nlig * nrun * 4);
+    if (e == cudaSuccess && best_coords) e = buf.alloc(&d_out_xyz, (size_t)nlig * nrun * cstride * 12);
+    if (e == cudaSuccess) e = buf.alloc(&d_out_evals, (size_t)nlig * nrun * 8);
+    if (e == cudaSuccess) e = buf.alloc(&d_out_gens, (size_t)nlig * nrun * 4);
+    if (e == cudaSuccess) e = buf.alloc(&d_flag, 4);
+    if (e == cudaSuccess) e = buf.alloc(&d_jobs, (size_t)nlig * sizeof(DockJob));
+    for (int l = 0; l < nlig && e == cudaSuccess; ++l) {
+        DockJob& j = jobs[l];
+        const adock_ligand* lg = ligs[l];
+        j.blob = lg->d_blob; j.ext_of_int = lg->d_ext_of_int; j.blob_bytes = lg->blob_bytes;
+        j.Gn = 7 + lg->tp.R; j.N = lg->tp.N; j.R = lg->tp.R; j.seed = seeds[l];
+        e = buf.alloc(&j.pop, 2 * popsz * j.Gn * 4);
+        if (e == cudaSuccess) e = buf.alloc(&j.E, 2 * popsz * 4);
+        if (e == cudaSuccess) e = buf.alloc(&j.st, (size_t)nrun * sizeof(RunState));
+        if (e == cudaSuccess) e = buf.alloc(&j.picks, popsz * 4);
+        if (e == cudaSuccess) e = buf.alloc(&j.fy, popsz * 4);
+        j.out_geno = d_out_geno + (size_t)l * nrun * gstride;
+        j.out_E = d_out_E + (size_t)l * nrun;
+        j.out_xyz = d_out_xyz ? d_out_xyz + (size_t)l * nrun * cstride * 3 : nullptr;
+        j.out_evals = d_out_evals + (size_t)l * nrun;
+        j.out_gens = d_out_gens + (size_t)l * nrun;
+    }
+    if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("dock alloc: ") + cudaGetErrorString(e));
+    CUDA_TRY(cudaMemcpyAsync(d_jobs, jobs.data(), (size_t)nlig * sizeof(DockJob), cudaMemcpyHostToDevice, stm));
+    if (best_coords) CUDA_TRY(cudaMemsetAsync(d_out_xyz, 0, (size_t)nlig * nrun * cstride * 12, stm));
+    CUDA_TRY(cudaMemsetAsync(d_out_geno, 0, (size_t)nlig * nrun * gstride * 4, stm));
+
+    const size_t smem_ga = cta_smem(maxblob, maxscr, Wga), smem_ls = cta_smem(maxblob, maxscr, Wls);
+    CUDA_TRY(cudaFuncSetAttribute(dock_init_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ga));
+    CUDA_TRY(cudaFuncSetAttribute(dock_ga_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ga));
+    CUDA_TRY(cudaFuncSetAttribute(dock_ls_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ls));
+    CUDA_TRY(cudaFuncSetAttribute(dock_final_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ls));
+
+    DockDims dga = dm, dls = dm, dfin = dm;
+    dga.upj = (int)((popsz + Wga - 1) / Wga);
+    dls.upj = std::max(1, (nrun * dm.n_ls + Wls - 1) / Wls);
+    dfin.upj = (nrun + Wls - 1) / Wls;
+    dock_init_kernel<<<dga.upj * nlig, Wga * 32, smem_ga, stm>>>(grids->dev, P, d_jobs, dga);
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    const bool can_run = (long long)Pn < max_evals && p.max_gens > 0;
+    int h_flag = can_run ? 1 : 0;
+    const int poll = 8;
+    std::vector<cudaEvent_t> prof_ev;
+    for (int g = 0; h_flag && g < p.max_gens; ++g) {
+        dock_ga_kernel<true><<<dga.upj * nlig, Wga * 32, smem_ga, stm>>>(grids->dev, P, d_jobs, dga, nullptr);
+        if (dm.n_ls > 0 && p.lsit > 0) {
+            if (g_prof) {
+                cudaEvent_t a, b;
+                CUDA_TRY(cudaEventCreate(&a)); CUDA_TRY(cudaEventCreate(&b));
+                CUDA_TRY(cudaEventRecord(a, stm));
+                dock_ls_kernel<<<dls.upj * nlig, Wls * 32, smem_ls, stm>>>(grids->dev, P, d_jobs, dls);
+                CUDA_TRY(cudaEventRecord(b, stm));
+                prof_ev.push_back(a); prof_ev.push_back(b);
+            } else {
+                dock_ls_kernel<<<dls.upj * nlig, Wls * 32, smem_ls, stm>>>(grids->dev, P, d_jobs, dls);
+            }
+        }
+        const bool check = ((g + 1) % poll) == 0;
+        if (check) CUDA_TRY(cudaMemsetAsync(d_flag, 0, 4, stm));
+        dock_commit_kernel<<<(nlig * nrun + 127) / 128, 128, 0, stm>>>(d_jobs, nlig, dm, d_flag);
+        g_launches += (dm.n_ls > 0 && p.lsit > 0) ? 3 : 2;
+        if (check) {
+            CUDA_TRY(cudaMemcpyAsync(&h_flag, d_flag, 4, cudaMemcpyDeviceToHost, stm));
+            CUDA_TRY(cudaStreamSynchronize(stm));
+        }
+    }
+    dock_final_kernel<<<dfin.upj * nlig, Wls * 32, smem_ls, stm>>>(grids->dev, P, d_jobs, dfin);
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    std::vector<long long> h_evals((size_t)nlig * nrun);
+    CUDA_TRY(cudaMemcpyAsync(best_genotypes, d_out_geno, (size_t)nlig * nrun * gstride * 4, cudaMemcpyDeviceToHost, stm));
+    CUDA_TRY(cudaMemcpyAsync(best_energies, d_out_E, (size_t)nlig * nrun * 4, cudaMemcpyDeviceToHost, stm));
+    if (best_coords) CUDA_TRY(cudaMemcpyAsync(best_coords, d_out_xyz, (size_t)nlig * nrun * cstride * 12, cudaMemcpyDeviceToHost, stm));
+    if (evals_used) CUDA_TRY(cudaMemcpyAsync(evals_used, d_out_evals, (size_t)nlig * nrun * 8, cudaMemcpyDeviceToHost, stm));
+    if (gens_used) CUDA_TRY(cudaMemcpyAsync(gens_used, d_out_gens, (size_t)nlig * nrun * 4, cudaMemcpyDeviceToHost, stm));
+    std::vector<int> h_gens;
+    if (g_prof) {
+        h_gens.resize((size_t)nlig * nrun);
+        CUDA_TRY(cudaMemcpyAsync(h_evals.data(), d_out_evals, (size_t)nlig * nrun * 8, cudaMemcpyDeviceToHost, stm));
+        CUDA_TRY(cudaMemcpyAsync(h_gens.data(), d_out_gens, (size_t)nlig * nrun * 4, cudaMemcpyDeviceToHost, stm));
+    }
+    CUDA_TRY(cudaStreamSynchronize(stm));
+    if (g_prof) {
+        for (size_t i = 0; i + 1 < prof_ev.size(); i += 2) {
+            float ms = 0;
+            cudaEventElapsedTime(&ms, prof_ev[i], prof_ev[i + 1]);
+            g_ls_ms += ms;
+            ++g_ls_launches;
+        }
+        for (cudaEvent_t e2 : prof_ev) cudaEventDestroy(e2);
+        for (size_t i = 0; i < h_gens.size(); ++i) g_ls_evals += h_evals[i] - Pn - (long long)h_gens[i] * (Pn - 1);
+    }
+    return ADOCK_OK;
+}
+
+extern "C" int adock_dock(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params, int nrun, int pop_size,
+                          long long max_evals, unsigned long long seed, float* best_genotypes, float* best_energies,
+                          float* best_coords, long long* evals_used, int* gens_used, void* cuda_stream) {
+    if (!ligand) return fail(ADOCK_EINVAL, "NULL ligand");
+    const adock_ligand* ligs[1] = {ligand};
+    return dock_impl(grids, ligs, 1, params, nrun, pop_size, max_evals, &seed, 7 + ligand->tp.R, best_genotypes, best_energies,
+                     ligand->tp.N, best_coords, evals_used, gens_used, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int adock_dock_many(const adock_grids* grids, const adock_ligand* const* ligands, int nlig, const adock_params* params,
+                               int nrun, int pop_size, long long max_evals, const unsigned long long* seeds, int gstride,
+                               float* best_genotypes, float* best_energies, int cstride, float* best_coords, long long* evals_used,
+                               void* cuda_stream) {
+    return dock_impl(grids, ligands, nlig, params, nrun, pop_size, max_evals, seeds, gstride, best_genotypes, best_energies, cstride,
+                     best_coords, evals_used, nullptr, (cudaStream_t)cuda_stream);
+}
+
+// =================================================================== GA test hook (R9): one generation, no scoring
+extern "C" int adock_ga_generation(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params, int nrun, int Pn,
+                                   int generation, unsigned long long seed, const float* d_pop, const float* d_energies,
+                                   float* d_newpop, int* d_decisions, int* d_ls_picks, int* n_ls, void* cuda_stream) {
+    if (!grids || !ligand || !d_newpop) return fail(ADOCK_EINVAL, "NULL argument");
+    if (nrun < 1 || Pn < 2 || generation < 0 || (generation > 0 && (!d_pop || !d_energies))) return fail(ADOCK_EINVAL, "bad GA arguments");
+    adock_params p;
+    int rc = check_params(params, ligand, p);
+    if (rc) return rc;
+    rc = device_props();
+    if (rc) return rc;
+    cudaStream_t stm = (cudaStream_t)cuda_stream;
+    const int W = fit_warps(ligand->blob_bytes, ligand->scratch_floats, 8);
+    if (!W) return fail(ADOCK_ELIMIT, "ligand does not fit in shared memory");
+    const size_t smem = cta_smem(ligand->blob_bytes, ligand->scratch_floats, W);
+    ParDev P = make_pardev(p);
+    P.k_wall_h = p.k_wall * grids->dev.h;
+    const size_t popsz = (size_t)nrun * Pn;
+    const int Gn = 7 + ligand->tp.R;
+    DevBuf buf;
+    DockJob j{};
+    j.blob = ligand->d_blob; j.ext_of_int = ligand->d_ext_of_int; j.blob_bytes = ligand->blob_bytes;
+    j.Gn = Gn; j.N = ligand->tp.N; j.R = ligand->tp.R; j.seed = seed;
+    DockJob* d_job = nullptr;
+    cudaError_t e = buf.alloc(&j.pop, 2 * popsz * Gn * 4);
+    if (e == cudaSuccess) e = buf.alloc(&j.E, 2 * popsz * 4);
+    if (e == cudaSuccess) e = buf.alloc(&j.st, (size_t)nrun * sizeof(RunState));
+    if (e == cudaSuccess) e = buf.alloc(&j.picks, popsz * 4);
+    if (e == cudaSuccess) e = buf.alloc(&j.fy, popsz * 4);
+    if (e == cudaSuccess) e = buf.alloc(&d_job, sizeof(DockJob));
+    if (e != cudaSuccess) return fail(ADOCK_ENOMEM, std::string("ga alloc: ") + cudaGetErrorString(e));
+    DockDims dm{};
+    dm.nrun = nrun; dm.P = Pn; dm.n_ls = n_ls_of(p, Pn); dm.max_evals = (1ll << 60); dm.max_gens = 1 << 30;
+    dm.upj = (int)((popsz + W - 1) / W);
+    if (n_ls) *n_ls = dm.n_ls;
+    CUDA_TRY(cudaMemcpyAsync(d_job, &j, sizeof(DockJob), cudaMemcpyHostToDevice, stm));
+    if (generation == 0) {
+        CUDA_TRY(cudaFuncSetAttribute(dock_init_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        dock_init_kernel<<<dm.upj, W * 32, smem, stm>>>(grids->dev, P, d_job, dm);
+        ++g_launches;
+        CUDA_TRY(cudaMemcpyAsync(d_newpop, j.pop, popsz * Gn * 4, cudaMemcpyDeviceToDevice, stm));
+    } else {
+        std::vector<RunState> st(nrun);
+        for (auto& s : st) { s.evals = 0; s.gen = generation - 1; s.cur = 0; s.active = 1; s.ls_acc = 0; s.pad[0] = s.pad[1] = 0; }
+        CUDA_TRY(cudaMemcpyAsync(j.st, st.data(), nrun * sizeof(RunState), cudaMemcpyHostToDevice, stm));
+        CUDA_TRY(cudaMemcpyAsync(j.pop, d_pop, popsz * Gn * 4, cudaMemcpyDeviceToDevice, stm));
+        CUDA_TRY(cudaMemcpyAsync(j.E, d_energies, popsz * 4, cudaMemcpyDeviceToDevice, stm));
+        CUDA_TRY(cudaFuncSetAttribute(dock_ga_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        dock_ga_kernel<false><<<dm.upj, W * 32, smem, stm>>>(grids->dev, P, d_job, dm, d_decisions);
+        ++g_launches;
+        CUDA_TRY(cudaMemcpyAsync(d_newpop, j.pop + popsz * Gn, popsz * Gn * 4, cudaMemcpyDeviceToDevice, stm));
+        if (d_ls_picks) CUDA_TRY(cudaMemcpyAsync(d_ls_picks, j.picks, popsz * 4, cudaMemcpyDeviceToDevice, stm));
+    }
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaStreamSynchronize(stm));
+    return ADOCK_OK;
+}

@@ -1,0 +1,527 @@
+// device.cuh -- sm_100a device code of the hot path: pose builder, grid interpolator, intramolecular
+// pair evaluator, reductions and gradient back-propagation (R3-R6), ADADELTA (R7),
+// Philox4x32-10 (R8) and the GA operators (R9).  One WARP per individual; the ligand image (topology.hpp)
+// is staged once per CTA into shared memory by a bulk async copy (TMA, UBLKCP) and shared by its warps.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "topology.hpp"
+
+namespace adock {
+
+constexpr unsigned kFull = 0xffffffffu;
+constexpr float kPi = 3.14159265358979323846f;
+constexpr float kTwoPi = 6.28318530717958647692f;
+
+struct GridDev {
+    const float4* cells;    // [T][nz][ny][nx-1] x-pair cells of 2 float4: {a_t,elec,desolv,0}(ix), same (ix+1)
+    long long type_stride;  // float4 units between types
+    int nx, ny, nz, T;
+    float inv_h, h;
+    float ox, oy, oz;
+    float bx, by, bz;       // box extents h*(n-1)
+};
+
+struct ParDev {             // adock_params with the per-pair constants folded
+    float elec_scale, diel_A, diel_B, diel_k, lamB, mlamB_log2e;   // lamB = lambda*B
+    float inv_sig2, mhalf_inv_sig2_log2e;
+    float rmin2, k_wall, k_wall_h;
+    float ad_rho, ad_eps;
+    float tourn_prob, xover_rate, mut_rate, dmov, dang;
+    int lsit;
+};
+
+// ---------------------------------------------------------------- shared-memory views
+struct LigS {
+    const float4* atoms;    // (x0 - pivot, q), internal order
+    const uint32_t* meta;   // type | frag<<8
+    const float4* fg;       // FragGeom as 2 float4
+    const int4* fi;         // FragIdx
+    const uint4* pairs;     // PairRec rounds
+    int N, R, nfrag, nrounds;
+};
+
+struct WarpS {
+    float* geno;            // [Gpad]
+    float* grad;            // [Dpad]  (also the ADADELTA step)
+    float* best;            // [Gpad]
+    float2* sc;             // [nfrag] sin,cos of the fragment's torsion
+    float4* fragT;          // [nfrag][3] rows of the 3x4 fragment transform
+    float4* fragAx;         // [nfrag][2] posed axis, posed pivot point - t
+    float4* fragFT;         // [nfrag][2] force, torque about t
+    float4* X;              // [N] posed xyz, q
+    float4* Gr;             // [N] dE/dx
+};
+
+__host__ __device__ inline int pad4(int x) { return (x + 3) & ~3; }
+// floats of per-warp scratch for a ligand with N atoms, nfrag fragments, R torsions
+__host__ __device__ inline int warp_scratch_floats(int N, int nfrag, int R) {
+    return 2 * pad4(7 + R) + pad4(6 + R) + pad4(2 * nfrag) + nfrag * 28 + N * 8;
+}
+
+__device__ inline LigS lig_view(const unsigned char* blob) {
+    const LigHeader* h = reinterpret_cast<const LigHeader*>(blob);
+    LigS L;
+    L.atoms = reinterpret_cast<const float4*>(blob + h->off_atoms);
+    L.meta = reinterpret_cast<const uint32_t*>(blob + h->off_meta);
+    L.fg = reinterpret_cast<const float4*>(blob + h->off_frag);
+    L.fi = reinterpret_cast<const int4*>(blob + h->off_fragidx);
+    L.pairs = reinterpret_cast<const uint4*>(blob + h->off_pairs);
+    L.N = h->N; L.R = h->R; L.nfrag = h->nfrag; L.nrounds = h->nrounds;
+    return L;
+}
+
+__device__ inline WarpS warp_view(float* base, const LigS& L) {
+    WarpS S;
+    int Gp = pad4(7 + L.R), Dp = pad4(6 + L.R);
+    S.geno = base; base += Gp;
+    S.best = base; base += Gp;
+    S.grad = base; base += Dp;
+    S.sc = reinterpret_cast<float2*>(base); base += pad4(2 * L.nfrag);
+    S.fragT = reinterpret_cast<float4*>(base); base += 12 * L.nfrag;
+    S.fragAx = reinterpret_cast<float4*>(base); base += 8 * L.nfrag;
+    S.fragFT = reinterpret_cast<float4*>(base); base += 8 * L.nfrag;
+    S.X = reinterpret_cast<float4*>(base); base += 4 * L.N;
+    S.Gr = reinterpret_cast<float4*>(base);
+    return S;
+}
+
+// ---------------------------------------------------------------- TMA bulk copy of the ligand image
+__device__ inline uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// All threads of the CTA call this; returns after the image is visible in shared memory.
+__device__ inline void stage_ligand(unsigned char* dst, const unsigned char* src, int bytes, uint64_t* bar, uint32_t phase) {
+    if (threadIdx.x == 0) {
+        if (phase == 0) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(bar)));
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                     "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                     : "memory");
+    }
+    __syncthreads();
+    uint32_t done = 0;
+    while (!done) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(phase & 1u)
+            : "memory");
+    }
+}
+
+// ---------------------------------------------------------------- grid term (R4)
+struct F8 { float4 lo, hi; };
+__device__ __forceinline__ F8 ld_cell(const float4* p) {     // one aligned 32-byte sector: LDG.256
+    F8 r;
+    asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+        : "=f"(r.lo.x), "=f"(r.lo.y), "=f"(r.lo.z), "=f"(r.lo.w), "=f"(r.hi.x), "=f"(r.hi.y), "=f"(r.hi.z), "=f"(r.hi.w)
+        : "l"(p));
+    return r;
+}
+
+template <bool GRAD>
+__device__ __forceinline__ float grid_atom(const GridDev& G, const ParDev& P, int type, float q, float x, float y, float z,
+                                           float& gx, float& gy, float& gz) {
+    float ux = (x - G.ox) * G.inv_h, uy = (y - G.oy) * G.inv_h, uz = (z - G.oz) * G.inv_h;
+    float cx = fminf(fmaxf(ux, 0.f), (float)(G.nx - 1)), cy = fminf(fmaxf(uy, 0.f), (float)(G.ny - 1)),
+          cz = fminf(fmaxf(uz, 0.f), (float)(G.nz - 1));
+    int ix = min((int)cx, G.nx - 2), iy = min((int)cy, G.ny - 2), iz = min((int)cz, G.nz - 2);
+    float fx = cx - (float)ix, fy = cy - (float)iy, fz = cz - (float)iz;
+    float ox = ux - cx, oy = uy - cy, oz = uz - cz;
+    const int rowlen = (G.nx - 1) * 2;
+    const float4* base = G.cells + (long long)type * G.type_stride + ((long long)(iz * G.ny + iy) * (G.nx - 1) + ix) * 2;
+    F8 c00 = ld_cell(base), c01 = ld_cell(base + rowlen), c10 = ld_cell(base + (long long)G.ny * rowlen),
+       c11 = ld_cell(base + (long long)G.ny * rowlen + rowlen);
+    float aq = fabsf(q);
+    // per-corner field value: affinity + q*elec + |q|*desolv
+    float a00 = fmaf(aq, c00.lo.z, fmaf(q, c00.lo.y, c00.lo.x)), b00 = fmaf(aq, c00.hi.z, fmaf(q, c00.hi.y, c00.hi.x));
+    float a01 = fmaf(aq, c01.lo.z, fmaf(q, c01.lo.y, c01.lo.x)), b01 = fmaf(aq, c01.hi.z, fmaf(q, c01.hi.y, c01.hi.x));
+    float a10 = fmaf(aq, c10.lo.z, fmaf(q, c10.lo.y, c10.lo.x)), b10 = fmaf(aq, c10.hi.z, fmaf(q, c10.hi.y, c10.hi.x));
+    float a11 = fmaf(aq, c11.lo.z, fmaf(q, c11.lo.y, c11.lo.x)), b11 = fmaf(aq, c11.hi.z, fmaf(q, c11.hi.y, c11.hi.x));
+    float d00 = b00 - a00, d01 = b01 - a01, d10 = b10 - a10, d11 = b11 - a11;       // d/dfx per row
+    float v00 = fmaf(fx, d00, a00), v01 = fmaf(fx, d01, a01), v10 = fmaf(fx, d10, a10), v11 = fmaf(fx, d11, a11);
+    float e0 = v01 - v00, e1 = v11 - v10;                                            // d/dfy per z-plane
+    float w0 = fmaf(fy, e0, v00), w1 = fmaf(fy, e1, v10);
+    float val = fmaf(fz, w1 - w0, w0);
+    float wall = fabsf(ox) + fabsf(oy) + fabsf(oz);
+    val = fmaf(P.k_wall_h, wall, val);
+    if (GRAD) {
+        float dx0 = fmaf(fy, d01 - d00, d00), dx1 = fmaf(fy, d11 - d10, d10);
+        float dfx = fmaf(fz, dx1 - dx0, dx0);
+        float dfy = fmaf(fz, e1 - e0, e0);
+        float dfz = w1 - w0;
+        gx = (ox != 0.f) ? copysignf(P.k_wall, ox) : dfx * G.inv_h;
+        gy = (oy != 0.f) ? copysignf(P.k_wall, oy) : dfy * G.inv_h;
+        gz = (oz != 0.f) ? copysignf(P.k_wall, oz) : dfz * G.inv_h;
+    }
+    return val;
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+    return v;
+}
+
+// ---------------------------------------------------------------- full evaluation of one genotype by one warp
+// Reads S.geno; writes S.grad (GRAD) and S.X; returns the total energy in every lane (NaN for |q|<1e-12).
+template <bool GRAD>
+__device__ __forceinline__ float eval_pose(const LigS& L, const GridDev& G, const ParDev& P, const WarpS& S, int lane,
+                                           float& e_inter, float& e_intra) {
+    const float tx = S.geno[0], ty = S.geno[1], tz = S.geno[2];
+    float qw = S.geno[3], qx = S.geno[4], qy = S.geno[5], qz = S.geno[6];
+    const float qn2 = qw * qw + qx * qx + qy * qy + qz * qz;
+    if (!(qn2 >= 1e-24f)) {
+        if (GRAD) for (int d = lane; d < 6 + L.R; d += 32) S.grad[d] = __int_as_float(0x7fc00000);
+        e_inter = e_intra = __int_as_float(0x7fc00000);
+        __syncwarp();
+        return __int_as_float(0x7fc00000);
+    }
+    const float qi = 1.0f / sqrtf(qn2);
+    qw *= qi; qx *= qi; qy *= qi; qz *= qi;
+    const float r00 = 1.f - 2.f * (qy * qy + qz * qz), r01 = 2.f * (qx * qy - qw * qz), r02 = 2.f * (qx * qz + qw * qy);
+    const float r10 = 2.f * (qx * qy + qw * qz), r11 = 1.f - 2.f * (qx * qx + qz * qz), r12 = 2.f * (qy * qz - qw * qx);
+    const float r20 = 2.f * (qx * qz - qw * qy), r21 = 2.f * (qy * qz + qw * qx), r22 = 1.f - 2.f * (qx * qx + qy * qy);
+
+    // (a1) sin/cos of every torsion, then per-fragment rigid transform T_f = T_root o Rot_k1 o ... o Rot_kd
+    for (int f = lane; f < L.nfrag; f += 32) {
+        float s = 0.f, c = 1.f;
+        if (f > 0) sincosf(S.geno[7 + (L.fi[f].w >> 16)], &s, &c);
+        S.sc[f] = make_float2(s, c);
+    }
+    __syncwarp();
+    for (int f = lane; f < L.nfrag; f += 32) {
+        float m00 = 1, m01 = 0, m02 = 0, m03 = 0, m10 = 0, m11 = 1, m12 = 0, m13 = 0, m20 = 0, m21 = 0, m22 = 1, m23 = 0;
+        for (int cur = f; cur > 0; cur = L.fi[cur].x) {
+            const float4 p0 = L.fg[2 * cur], u = L.fg[2 * cur + 1];
+            const float2 sc = S.sc[cur];
+            const float s = sc.x, c = sc.y, k = 1.f - c;
+            const float a00 = fmaf(k * u.x, u.x, c), a01 = fmaf(k * u.x, u.y, -s * u.z), a02 = fmaf(k * u.x, u.z, s * u.y);
+            const float a10 = fmaf(k * u.x, u.y, s * u.z), a11 = fmaf(k * u.y, u.y, c), a12 = fmaf(k * u.y, u.z, -s * u.x);
+            const float a20 = fmaf(k * u.x, u.z, -s * u.y), a21 = fmaf(k * u.y, u.z, s * u.x), a22 = fmaf(k * u.z, u.z, c);
+            // Rot(x) = A (x - p0) + p0 ; compose Rot o M
+            float n00 = a00 * m00 + a01 * m10 + a02 * m20, n01 = a00 * m01 + a01 * m11 + a02 * m21,
+                  n02 = a00 * m02 + a01 * m12 + a02 * m22;
+            float n10 = a10 * m00 + a11 * m10 + a12 * m20, n11 = a10 * m01 + a11 * m11 + a12 * m21,
+                  n12 = a10 * m02 + a11 * m12 + a12 * m22;
+            float n20 = a20 * m00 + a21 * m10 + a22 * m20, n21 = a20 * m01 + a21 * m11 + a22 * m21,
+                  n22 = a20 * m02 + a21 * m12 + a22 * m22;
+            float dx = m03 - p0.x, dy = m13 - p0.y, dz = m23 - p0.z;
+            float n03 = a00 * dx + a01 * dy + a02 * dz + p0.x, n13 = a10 * dx + a11 * dy + a12 * dz + p0.y,
+                  n23 = a20 * dx + a21 * dy + a22 * dz + p0.z;
+            m00 = n00; m01 = n01; m02 = n02; m03 = n03; m10 = n10; m11 = n11; m12 = n12; m13 = n13;
+            m20 = n20; m21 = n21; m22 = n22; m23 = n23;
+        }
+        // T = Root o M, Root(y) = Rq y + t   (y already relative to the pivot)
+        float t00 = r00 * m00 + r01 * m10 + r02 * m20, t01 = r00 * m01 + r01 * m11 + r02 * m21,
+              t02 = r00 * m02 + r01 * m12 + r02 * m22, t03 = r00 * m03 + r01 * m13 + r02 * m23;
+        float t10 = r10 * m00 + r11 * m10 + r12 * m20, t11 = r10 * m01 + r11 * m11 + r12 * m21,
+              t12 = r10 * m02 + r11 * m12 + r12 * m22, t13 = r10 * m03 + r11 * m13 + r12 * m23;
+        float t20 = r20 * m00 + r21 * m10 + r22 * m20, t21 = r20 * m01 + r21 * m11 + r22 * m21,
+              t22 = r20 * m02 + r21 * m12 + r22 * m22, t23 = r20 * m03 + r21 * m13 + r22 * m23;
+        S.fragT[3 * f] = make_float4(t00, t01, t02, t03 + tx);
+        S.fragT[3 * f + 1] = make_float4(t10, t11, t12, t13 + ty);
+        S.fragT[3 * f + 2] = make_float4(t20, t21, t22, t23 + tz);
+        if (GRAD && f > 0) {
+            const float4 p0 = L.fg[2 * f], u = L.fg[2 * f + 1];
+            S.fragAx[2 * f] = make_float4(t00 * u.x + t01 * u.y + t02 * u.z, t10 * u.x + t11 * u.y + t12 * u.z,
+                                          t20 * u.x + t21 * u.y + t22 * u.z, 0.f);
+            S.fragAx[2 * f + 1] = make_float4(t00 * p0.x + t01 * p0.y + t02 * p0.z + t03, t10 * p0.x + t11 * p0.y + t12 * p0.z + t13,
+                                              t20 * p0.x + t21 * p0.y + t22 * p0.z + t23, 0.f);
+        }
+    }
+    __syncwarp();
+
+    // (a1,a2) atoms: pose, then trilinear lookup of the three maps
+    float eg = 0.f;
+    for (int i = lane; i < L.N; i += 32) {
+        const float4 a = L.atoms[i];
+        const uint32_t m = L.meta[i];
+        const int f = m >> 8;
+        const float4 t0 = S.fragT[3 * f], t1 = S.fragT[3 * f + 1], t2 = S.fragT[3 * f + 2];
+        const float x = fmaf(t0.x, a.x, fmaf(t0.y, a.y, fmaf(t0.z, a.z, t0.w)));
+        const float y = fmaf(t1.x, a.x, fmaf(t1.y, a.y, fmaf(t1.z, a.z, t1.w)));
+        const float z = fmaf(t2.x, a.x, fmaf(t2.y, a.y, fmaf(t2.z, a.z, t2.w)));
+        S.X[i] = make_float4(x, y, z, a.w);
+        float gx, gy, gz;
+        eg += grid_atom<GRAD>(G, P, (int)(m & 0xff), a.w, x, y, z, gx, gy, gz);
+        if (GRAD) S.Gr[i] = make_float4(gx, gy, gz, 0.f);
+    }
+    __syncwarp();
+
+    // (a3) intramolecular pairs: conflict-free warp rounds
+    float ep = 0.f;
+    for (int r = 0; r < L.nrounds; ++r) {
+        const uint4 rec = L.pairs[r * 32 + lane];
+        const bool valid = (rec.x >> 17) & 1u;
+        const int i = rec.x & 0xff, j = (rec.x >> 8) & 0xff;
+        const float4 xi = S.X[i], xj = S.X[j];
+        const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
+        const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+        const float r2c = fmaxf(r2, P.rmin2);
+        const float rinv = rsqrtf(r2c);
+        const float rr = r2c * rinv;
+        const float rinv2 = rinv * rinv;
+        const float r6 = rinv2 * rinv2 * rinv2, r12 = r6 * r6;
+        const bool hb = (rec.x >> 16) & 1u;
+        const float rA = hb ? r12 * r2c : r6;
+        const float c12 = __uint_as_float(rec.y), cA = __uint_as_float(rec.z), ds = __uint_as_float(rec.w);
+        const float ev = fmaf(c12, r12, -cA * rA);
+        const float ex = exp2f(rr * P.mlamB_log2e);
+        const float rden = __fdividef(1.f, fmaf(P.diel_k, ex, 1.f));
+        const float eps = fmaf(P.diel_B, rden, P.diel_A);
+        const float inv_er = __fdividef(rinv, eps);
+        const float eel = P.elec_scale * xi.w * xj.w * inv_er;
+        const float egs = ds * exp2f(r2c * P.mhalf_inv_sig2_log2e);
+        if (valid) ep += ev + eel + egs;
+        if (GRAD) {
+            const float dv = fmaf(hb ? 10.f : 6.f, cA * rA, -12.f * c12 * r12) * rinv;
+            const float deps = P.diel_B * P.lamB * (1.f - rden) * rden;
+            const float del = -eel * fmaf(deps, rr, eps) * inv_er;
+            const float dds = -rr * P.inv_sig2 * egs;
+            const float fs = (r2 >= P.rmin2) ? (dv + del + dds) * rinv : 0.f;
+            const float fx = fs * dx, fy = fs * dy, fz = fs * dz;
+            if (valid) {
+                float4 g = S.Gr[i];
+                g.x += fx; g.y += fy; g.z += fz;
+                S.Gr[i] = g;
+            }
+            __syncwarp();
+            if (valid) {
+                float4 g = S.Gr[j];
+                g.x -= fx; g.y -= fy; g.z -= fz;
+                S.Gr[j] = g;
+            }
+            __syncwarp();
+        }
+    }
+    e_inter = warp_sum(eg);
+    e_intra = warp_sum(ep);
+
+    // (a4) back-propagation: per-fragment force/torque, subtree sums, projection on the posed axes
+    if (GRAD) {
+        for (int f = lane; f < L.nfrag; f += 32) {
+            const int4 ix = L.fi[f];
+            float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
+            for (int i = ix.y; i < ix.z; ++i) {
+                const float4 g = S.Gr[i], x = S.X[i];
+                const float rx = x.x - tx, ry = x.y - ty, rz = x.z - tz;
+                Fx += g.x; Fy += g.y; Fz += g.z;
+                Tx += ry * g.z - rz * g.y; Ty += rz * g.x - rx * g.z; Tz += rx * g.y - ry * g.x;
+            }
+            S.fragFT[2 * f] = make_float4(Fx, Fy, Fz, 0.f);
+            S.fragFT[2 * f + 1] = make_float4(Tx, Ty, Tz, 0.f);
+        }
+        __syncwarp();
+        for (int f = lane; f < L.nfrag; f += 32) {
+            const int w = L.fi[f].w;
+            const int sub_end = w & 0xffff;
+            float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
+            for (int g = f; g < sub_end; ++g) {
+                const float4 F = S.fragFT[2 * g], T = S.fragFT[2 * g + 1];
+                Fx += F.x; Fy += F.y; Fz += F.z; Tx += T.x; Ty += T.y; Tz += T.z;
+            }
+            if (f == 0) {
+                S.grad[0] = Fx; S.grad[1] = Fy; S.grad[2] = Fz;
+                S.grad[3] = Tx; S.grad[4] = Ty; S.grad[5] = Tz;
+            } else {
+                const float4 u = S.fragAx[2 * f], xa = S.fragAx[2 * f + 1];     // xa relative to t
+                const float cx = Tx - (xa.y * Fz - xa.z * Fy), cy = Ty - (xa.z * Fx - xa.x * Fz), cz = Tz - (xa.x * Fy - xa.y * Fx);
+                S.grad[6 + (w >> 16)] = u.x * cx + u.y * cy + u.z * cz;
+            }
+        }
+        __syncwarp();
+    }
+    return e_inter + e_intra;
+}
+
+// ---------------------------------------------------------------- Philox4x32-10 (R8)
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t k0, uint32_t k1, uint4 c) {
+#pragma unroll
+    for (int i = 0; i < 10; ++i) {
+        const uint32_t h0 = __umulhi(0xD2511F53u, c.x), l0 = 0xD2511F53u * c.x;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c.z), l1 = 0xCD9E8D57u * c.z;
+        c = make_uint4(h1 ^ c.y ^ k0, l1, h0 ^ c.w ^ k1, l0);
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return c;
+}
+enum : uint32_t { kInit = 0, kTournA = 1, kTournB = 2, kXover = 3, kMut = 4, kLsPick = 5 };
+__device__ __forceinline__ uint4 draw4(unsigned long long seed, uint32_t draw, uint32_t purpose, uint32_t id, uint32_t gen) {
+    return philox4x32_10((uint32_t)seed, (uint32_t)(seed >> 32), make_uint4(draw, purpose, id, gen));
+}
+__device__ __forceinline__ float u01(uint32_t x) { return (float)(x >> 8) * (1.0f / 16777216.0f); }
+__device__ __forceinline__ int below(uint32_t x, int n) { return (int)(((unsigned long long)(x >> 8) * (unsigned)n) >> 24); }
+__device__ __forceinline__ uint32_t pick_word(uint4 r, int w) { return w == 0 ? r.x : w == 1 ? r.y : w == 2 ? r.z : r.w; }
+
+__device__ __forceinline__ float wrap_pi(float a) { return a - kTwoPi * floorf((a + kPi) * (1.0f / kTwoPi)); }
+
+// q <- normalise((cos(th/2), sin(th/2) axis) (x) q) written to out[0..3]
+__device__ __forceinline__ void rotate_quat(float cw, float ax, float ay, float az, const float* q, float* out) {
+    const float n = 1.0f / sqrtf(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
+    const float w = q[0] * n, x = q[1] * n, y = q[2] * n, z = q[3] * n;
+    float ow = cw * w - ax * x - ay * y - az * z;
+    float oxx = cw * x + ax * w + ay * z - az * y;
+    float oy = cw * y - ax * z + ay * w + az * x;
+    float oz = cw * z + ax * y - ay * x + az * w;
+    const float m = 1.0f / sqrtf(ow * ow + oxx * oxx + oy * oy + oz * oz);
+    out[0] = ow * m; out[1] = oxx * m; out[2] = oy * m; out[3] = oz * m;
+}
+
+// ---------------------------------------------------------------- GA operators (R9), one warp per individual
+__device__ inline void ga_init_individual(const GridDev& G, int R, unsigned long long seed, uint32_t id, float* geno, int lane) {
+    if (lane < 3) {
+        const uint4 r = draw4(seed, 0, kInit, id, 0);
+        const float u = u01(pick_word(r, lane));
+        geno[lane] = lane == 0 ? fmaf(u, G.bx, G.ox) : lane == 1 ? fmaf(u, G.by, G.oy) : fmaf(u, G.bz, G.oz);
+    } else if (lane == 3) {
+        const uint4 r = draw4(seed, 1, kInit, id, 0);
+        const float u1 = u01(r.x), u2 = u01(r.y), u3 = u01(r.z);
+        const float s1 = sqrtf(1.f - u1), s2 = sqrtf(u1);
+        float sa, ca, sb, cb;
+        sincospif(2.f * u2, &sa, &ca);
+        sincospif(2.f * u3, &sb, &cb);
+        geno[3] = s2 * cb; geno[4] = s1 * sa; geno[5] = s1 * ca; geno[6] = s2 * sb;
+    }
+    for (int k = lane; k < R; k += 32) {
+        const uint4 r = draw4(seed, 2 + k / 4, kInit, id, 0);
+        geno[7 + k] = fmaf(u01(pick_word(r, k & 3)), kTwoPi, -kPi);
+    }
+}
+
+__device__ __forceinline__ int tournament(const ParDev& P, int Pn, const float* E, unsigned long long seed, uint32_t purpose,
+                                          uint32_t id, uint32_t gen, int* dec) {
+    const uint4 r = draw4(seed, 0, purpose, id, gen);
+    const int s1 = below(r.x, Pn), s2 = below(r.y, Pn);
+    const bool first = E[s1] <= E[s2];
+    const int lo = first ? s1 : s2, hi = first ? s2 : s1;
+    const int pick = (u01(r.z) < P.tourn_prob) ? lo : hi;
+    if (dec) { dec[0] = s1; dec[1] = s2; dec[2] = pick; }
+    return pick;
+}
+
+// child of slot s>=1 written to geno (shared, [7+R]); all lanes call; dec (global, 10 ints) optional
+__device__ inline void ga_make_child(const ParDev& P, int Pn, int R, unsigned long long seed, uint32_t id, uint32_t gen,
+                                     const float* pop, const float* E, float* geno, int* dec, int lane) {
+    const int Gn = 7 + R, NB = 4 + R;
+    int* d0 = (dec && lane == 0) ? dec : nullptr;
+    const int A = tournament(P, Pn, E, seed, kTournA, id, gen, d0);
+    const int B = tournament(P, Pn, E, seed, kTournB, id, gen, d0 ? d0 + 3 : nullptr);
+    const uint4 rx = draw4(seed, 0, kXover, id, gen);
+    const int c1 = below(rx.y, NB + 1), c2 = below(rx.z, NB + 1);
+    const int p1 = min(c1, c2), p2 = max(c1, c2);
+    const bool xo = u01(rx.x) < P.xover_rate;
+    if (d0) { d0[6] = xo; d0[7] = p1; d0[8] = p2; }
+    const float* gA = pop + (size_t)A * Gn;
+    const float* gB = pop + (size_t)B * Gn;
+    unsigned mutmask = 0;
+    for (int b0 = 0; b0 < NB; b0 += 32) {
+        const int b = b0 + lane;
+        bool mut = false;
+        if (b < NB) {
+            const float* src = (xo && b >= p1 && b < p2) ? gB : gA;
+            const uint4 rm = draw4(seed, (uint32_t)b, kMut, id, gen);
+            mut = u01(rm.x) < P.mut_rate;
+            const float amt = 2.f * u01(rm.y) - 1.f;
+            if (b < 3) {
+                geno[b] = mut ? src[b] + amt * P.dmov : src[b];
+            } else if (b == 3) {
+                if (mut) {
+                    const float ang = amt * P.dang, z = 2.f * u01(rm.z) - 1.f;
+                    const float sxy = sqrtf(fmaxf(0.f, 1.f - z * z));
+                    float sp, cp, sh, ch;
+                    sincospif(2.f * u01(rm.w), &sp, &cp);
+                    sincosf(0.5f * ang, &sh, &ch);
+                    const float q[4] = {src[3], src[4], src[5], src[6]};
+                    float o[4];
+                    rotate_quat(ch, sh * sxy * cp, sh * sxy * sp, sh * z, q, o);
+                    geno[3] = o[0]; geno[4] = o[1]; geno[5] = o[2]; geno[6] = o[3];
+                } else {
+                    geno[3] = src[3]; geno[4] = src[4]; geno[5] = src[5]; geno[6] = src[6];
+                }
+            } else {
+                const int gi = 4 + b - 1;
+                geno[gi] = mut ? wrap_pi(src[gi] + amt * P.dang) : src[gi];
+            }
+        }
+        const unsigned bal = __ballot_sync(kFull, mut);
+        if (b0 == 0) mutmask = bal & 0x7fffffffu;
+    }
+    if (d0) d0[9] = (int)mutmask;
+    __syncwarp();
+}
+
+// ---------------------------------------------------------------- ADADELTA local search (R7), one warp
+// Start genotype in S.geno; on return S.best holds the best genotype seen and the function returns its
+// energy (the carried energy e_start if no finite evaluation happened).  iters = evaluations performed.
+__device__ inline float adadelta_search(const LigS& L, const GridDev& G, const ParDev& P, const WarpS& S, int lane,
+                                        float e_start, int& iters) {
+    const int R = L.R, D = 6 + R, Gn = 7 + R;
+    float Eg2[3] = {0.f, 0.f, 0.f}, Ed2[3] = {0.f, 0.f, 0.f};         // component d = lane + 32*c  (D <= 70)
+    float bestE = __int_as_float(0x7f800000);
+    for (int d = lane; d < Gn; d += 32) S.best[d] = S.geno[d];
+    __syncwarp();
+    int it = 0;
+    while (it < P.lsit) {
+        float ei, ea;
+        const float e = eval_pose<true>(L, G, P, S, lane, ei, ea);
+        ++it;
+        bool ok = isfinite(e);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const int d = lane + 32 * c;
+            if (d < D) ok = ok && isfinite(S.grad[d]);
+        }
+        if (!__all_sync(kFull, ok)) break;
+        if (e < bestE) {
+            bestE = e;
+            for (int d = lane; d < Gn; d += 32) S.best[d] = S.geno[d];
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const int d = lane + 32 * c;
+            if (d < D) {
+                const float g = S.grad[d];
+                Eg2[c] = P.ad_rho * Eg2[c] + (1.f - P.ad_rho) * g * g;
+                const float dl = -(sqrtf(Ed2[c] + P.ad_eps) / sqrtf(Eg2[c] + P.ad_eps)) * g;
+                Ed2[c] = P.ad_rho * Ed2[c] + (1.f - P.ad_rho) * dl * dl;
+                S.grad[d] = dl;
+            }
+        }
+        __syncwarp();
+        // apply the step: t += dt ; q <- normalise(exp(dw/2) (x) q) ; tau <- wrap(tau + dtau)
+        float newv[3];
+        float newq[4];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const int gI = lane + 32 * c;
+            if (gI < 3) newv[c] = S.geno[gI] + S.grad[gI];
+            else if (gI >= 7 && gI < Gn) newv[c] = wrap_pi(S.geno[gI] + S.grad[gI - 1]);
+        }
+        if (lane == 3) {
+            const float wx = S.grad[3], wy = S.grad[4], wz = S.grad[5];
+            const float th = sqrtf(wx * wx + wy * wy + wz * wz);
+            float sh, ch;
+            sincosf(0.5f * th, &sh, &ch);
+            const float k = th > 1e-12f ? sh / th : 0.5f;
+            rotate_quat(ch, k * wx, k * wy, k * wz, S.geno + 3, newq);
+        }
+        __syncwarp();
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const int gI = lane + 32 * c;
+            if (gI < 3 || (gI >= 7 && gI < Gn)) S.geno[gI] = newv[c];
+        }
+        if (lane == 3) { S.geno[3] = newq[0]; S.geno[4] = newq[1]; S.geno[5] = newq[2]; S.geno[6] = newq[3]; }
+        __syncwarp();
+    }
+    iters = it;
+    return isfinite(bestE) ? bestE : e_start;
+}
+
+}  // namespace adock

@@ -1,0 +1,406 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star; R10):
+  energies  |dE| <= max(1e-4*|E_ref|, 1e-3 kcal/mol)
+  gradients per block b in {t, omega, tau}: ||d_b|| <= 1e-3*||g_b|| + 1e-5*S_b + 1e-4, where S_b is the sum of
+      the magnitudes of the per-atom / per-pair terms added up in that block (fp32 cancellation floor: the
+      oracle reports S_b as `scales`)
+  integer data (pair lists, trees, Philox words, GA decisions, LS picks): bit-exact.
+Gradients are compared only for poses the oracle reports as away from the kinks of the energy surface
+(cell faces / box faces / r_min), where fp32 and fp64 may legitimately sit on different sides.
+"""
+import math
+import os
+import subprocess
+
+import numpy as np
+import pytest
+from scipy import stats
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required for -m gpu tests")
+    from paper_2007_03678_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def dev():
+    return torch.device("cuda:0")
+
+
+class Case:
+    def __init__(self, B, orc, W, grids, lig, params=None):
+        self.grids, self.lig = grids, lig
+        self.pd = dict(W.DEFAULT_PARAMS)
+        self.pd.update(params or {})
+        self.gp = B.make_params(self.pd)
+        self.op = orc.params(self.pd)
+        self.gg = B.Grids.from_workload(grids)
+        self.gl = B.Ligand.from_workload(self.gg, lig, self.gp)
+        self.og = orc.Grids.from_workload(grids)
+        self.ol = orc.Ligand.from_workload(lig)
+
+
+@pytest.fixture(scope="module")
+def cases(B, orc, W):
+    cache = {}
+
+    def get(name, **params):
+        key = (name, tuple(sorted(params.items())))
+        if key not in cache:
+            grids, lig = W.make_config(name)
+            cache[key] = Case(B, orc, W, grids, lig, params)
+        return cache[key]
+    return get
+
+
+def gpu_score(B, c, G, dev, grad=True, gstride=None, dstride=None):
+    n = G.shape[0]
+    R = c.lig.R
+    gs = gstride or G.shape[1]
+    buf = torch.full((n, gs), 7.0, dtype=torch.float32, device=dev)
+    buf[:, :G.shape[1]] = torch.from_numpy(G).to(dev)
+    E = torch.full((n,), -1.0, dtype=torch.float32, device=dev)
+    terms = torch.zeros((n, 2), dtype=torch.float32, device=dev)
+    gr = torch.full((n, dstride or 6 + R), 5.0, dtype=torch.float32, device=dev) if grad else None
+    B.adock_score_batch(c.gg, c.gl, c.gp, buf, E, terms, gr)
+    torch.cuda.synchronize()
+    return E.cpu().numpy(), terms.cpu().numpy(), (gr.cpu().numpy() if grad else None)
+
+
+def assert_energy(E, ref, what=""):
+    tol = np.maximum(1e-4 * np.abs(ref), 1e-3)
+    bad = np.flatnonzero(~(np.abs(E.astype(np.float64) - ref) <= tol))
+    assert len(bad) == 0, f"{what}: {len(bad)} energies off, worst {np.abs(E - ref)[bad].max()} at {bad[:5]} ref {ref[bad[:5]]}"
+
+
+def assert_gradient(g, ref, R, ok, what=""):
+    """ref: the oracle's score() dict (grad, scales)"""
+    g = g.astype(np.float64)
+    rg, sc = ref["grad"], ref["scales"]
+    worst = 0.0
+    for b, (lo, hi) in enumerate(((0, 3), (3, 6), (6, 6 + R))):
+        if hi == lo:
+            continue
+        d = np.linalg.norm(g[:, lo:hi] - rg[:, lo:hi], axis=1)
+        tol = 1e-3 * np.linalg.norm(rg[:, lo:hi], axis=1) + 1e-5 * sc[:, b] + 1e-4
+        bad = np.flatnonzero(ok & ~(d <= tol))
+        assert len(bad) == 0, f"{what}: block [{lo},{hi}) off for {len(bad)} poses, e.g. {bad[:5]}: {d[bad[:5]]} > {tol[bad[:5]]}"
+        if ok.any():
+            worst = max(worst, float((d / tol)[ok].max()))
+    return worst
+
+
+# ------------------------------------------------------------------------------- integer structure on the device path
+@pytest.mark.parametrize("name", ["tiny", "drug", "sweep80", "sweep128"])
+def test_integer_structure_bit_exact(B, cases, name):
+    c = cases(name)
+    assert np.array_equal(c.gl.pairs(), c.ol.pairs)
+    t = c.gl.tree()
+    assert np.array_equal(t["tor_order"], c.ol.tor_order) and np.array_equal(t["moved"], c.ol.moved)
+    assert np.array_equal(t["rot"], c.ol.rot)
+
+
+# ------------------------------------------------------------------------------- scoring parity (rows a1-a4)
+@pytest.mark.parametrize("name,n", [("tiny", 1024), ("drug", 2500), ("sweep16", 777), ("sweep80", 1100), ("sweep128", 600)])
+def test_score_parity(B, orc, W, cases, dev, name, n):
+    c = cases(name)
+    G = W.make_genotypes(n, c.lig.R, c.grids, seed=100 + n)
+    ref = orc.score(c.og, c.ol, c.op, G)
+    E, terms, gr = gpu_score(B, c, G, dev)
+    assert_energy(E, ref["E"], name)
+    assert_energy(terms[:, 0], ref["terms"][:, 0], name + " inter")
+    assert_energy(terms[:, 1], ref["terms"][:, 1], name + " intra")
+    ok = (ref["margins"][:, 0] > 1e-3) & (ref["margins"][:, 1] > 1e-3)
+    assert ok.mean() > 0.5
+    w = assert_gradient(gr, ref, c.lig.R, ok, name)
+    print(f"{name}: worst gradient error / tolerance = {w:.3f}")
+    # energy-only launch gives the same energies
+    E2, _, _ = gpu_score(B, c, G, dev, grad=False)
+    assert_energy(E2, ref["E"], name + " energy-only")
+    assert np.allclose(E2, E, rtol=1e-6, atol=1e-6)
+
+
+def test_score_strides_ragged_and_empty(B, orc, W, cases, dev):
+    c = cases("tiny")
+    for n in (1, 7, 33, 255):                           # ragged tails of the warp/CTA tiling
+        G = W.make_genotypes(n, c.lig.R, c.grids, seed=n)
+        ref = orc.score(c.og, c.ol, c.op, G)
+        E, _, gr = gpu_score(B, c, G, dev, gstride=16, dstride=12)
+        assert_energy(E, ref["E"])
+        assert (gr[:, 8:] == 5.0).all()                 # padding columns untouched
+    B.adock_score_batch(c.gg, c.gl, c.gp, torch.zeros((0, 9), device=dev), torch.zeros(0, device=dev), None, None)
+    with pytest.raises(B.AdockError) as e:
+        B.adock_score_batch(c.gg, c.gl, c.gp, torch.zeros((4, 8), device=dev), torch.zeros(4, device=dev), None, None)
+    assert e.value.code == B.ADOCK_EINVAL
+
+
+def test_score_special_poses(B, orc, W, cases, dev):
+    c = cases("tiny")
+    R = c.lig.R
+    ident = c.ol.identity_genotype().astype(np.float32)
+    far = ident.copy(); far[0] = c.grids.box_hi[0] + 12.0           # every atom beyond +x: wall only
+    zero_q = ident.copy(); zero_q[3:7] = 0
+    scaled = ident.copy(); scaled[3:7] = [-3, 0, 0, 0]              # non-unit, negated quaternion
+    G = np.stack([ident, far, zero_q, scaled])
+    ref = orc.score(c.og, c.ol, c.op, G)
+    E, terms, gr = gpu_score(B, c, G, dev)
+    assert np.isnan(E[2]) and np.isnan(gr[2]).all() and np.isnan(ref["E"][2])
+    keep = np.array([0, 1, 3])
+    assert_energy(E[keep], ref["E"][keep])
+    assert math.isclose(gr[1, 0], c.lig.N * c.pd["k_wall"], rel_tol=1e-5)
+    assert_energy(E[3:4], ref["E"][0:1])                             # q and -3q are the same pose
+    assert_gradient(gr[keep], {k: ref[k][keep] for k in ("grad", "scales")}, R, np.array([False, True, False]))
+
+
+def test_score_rigid_ligand_without_torsions(B, orc, W, dev):
+    grids, _ = W.make_config("tiny")
+    lig = W.make_ligand(12, 0, 4, seed=8, centre=0.5 * (grids.box_lo + grids.box_hi))
+    c = Case(B, orc, W, grids, lig)
+    assert c.ol.npairs == 0
+    G = W.make_genotypes(300, 0, grids, seed=9)
+    ref = orc.score(c.og, c.ol, c.op, G)
+    E, terms, gr = gpu_score(B, c, G, dev)
+    assert_energy(E, ref["E"])
+    assert (terms[:, 1] == 0).all()
+    assert_gradient(gr, ref, 0, ref["margins"][:, 0] > 1e-3)
+
+
+def test_score_affine_field_is_exact_property(B, orc, W, dev):
+    """a property that holds at any size: on affine maps with zero charges and no pair terms the
+    translational gradient is sum_i (a,b,c)_{type_i}/h for every pose"""
+    T = 3
+    coef = [[1.5, -2.0, 0.25, 3.0], [0.5, 1.0, -1.0, 0.0], [-4.0, 0.5, 2.0, 1.0], [9, 9, 9, 9], [7, 7, 7, 7]]
+    grids = W.make_affine_grids(64, T, coef)
+    lig = W.make_ligand(20, 4, T, seed=3, centre=0.5 * (grids.box_lo + grids.box_hi))
+    lig.charge[:] = 0; lig.pair_coeffs[:] = 0; lig.solpar[:] = 0
+    c = Case(B, orc, W, grids, lig)
+    G = W.make_genotypes(4096, lig.R, grids, seed=1, wall_tail=0.0)
+    E, _, gr = gpu_score(B, c, G, dev)
+    want = sum(np.array(coef[t][:3]) for t in lig.type) / grids.spacing
+    assert np.allclose(gr[:, :3], want, rtol=2e-4, atol=1e-3)
+
+
+def test_score_full_size_sampled(B, orc, W, cases, dev):
+    """BASELINE.json sweep size (262144 genotypes, 40 atoms, 64^3 maps) in the launch configuration
+    bench.py times; 512 sampled outputs against the oracle."""
+    c = cases("sweep40")
+    n = 262144
+    G = W.make_genotypes(n, c.lig.R, c.grids, seed=4)
+    E, terms, gr = gpu_score(B, c, G, dev)
+    assert np.isfinite(E).all()
+    idx = np.random.default_rng(0).choice(n, 512, replace=False)
+    ref = orc.score(c.og, c.ol, c.op, G[idx])
+    assert_energy(E[idx], ref["E"], "sampled")
+    ok = (ref["margins"][:, 0] > 1e-3) & (ref["margins"][:, 1] > 1e-3)
+    assert_gradient(gr[idx], ref, c.lig.R, ok, "sampled")
+    # launching twice gives bit-identical results (fixed reduction order, no float atomics)
+    E2, _, gr2 = gpu_score(B, c, G, dev)
+    assert np.array_equal(E, E2) and np.array_equal(gr, gr2)
+
+
+# ------------------------------------------------------------------------------- Philox (R8)
+def test_philox_bit_exact_vs_oracle(B, orc, dev):
+    n = 1 << 20
+    rng = np.random.default_rng(5)
+    ctr = rng.integers(0, 2 ** 32, (n, 4), dtype=np.uint64).astype(np.uint32)
+    ctr[:4] = [[0, 0, 0, 0], [0xFFFFFFFF] * 4, [1, 0, 0, 0], [0, 4, 149, 27000]]
+    key = [0xDEADBEEF, 0x12345678]
+    d_ctr = torch.from_numpy(ctr.view(np.int32)).to(dev)
+    d_out = torch.zeros_like(d_ctr)
+    B.adock_philox(key, d_ctr, d_out)
+    torch.cuda.synchronize()
+    got = d_out.cpu().numpy().view(np.uint32)
+    assert np.array_equal(got, orc.philox(key, ctr))
+
+
+def test_philox_vs_curand_library(orc, tmp_path):
+    """Library special case: cuRAND's device Philox4x32-10, curand_init(seed, subsequence, offset) + curand4,
+    whose counter is (offset/4 lo, offset/4 hi, subsequence lo, subsequence hi) and key (seed lo, seed hi)."""
+    nvcc = "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        pytest.skip("nvcc not on the GPU box")
+    src = tmp_path / "cr.cu"
+    src.write_text(r'''
+#include <curand_kernel.h>
+#include <cstdio>
+__global__ void k(unsigned long long seed, unsigned int* out, int n) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    curandStatePhilox4_32_10_t s;
+    unsigned long long subseq = ((unsigned long long)(7u + i) << 32) | (1000u + 3u * i);
+    unsigned long long offset4 = ((unsigned long long)4u << 32) | (unsigned)(i * 5u);
+    curand_init(seed, subseq, 0, &s);
+    skipahead(offset4 * 4ull, &s);
+    uint4 r = curand4(&s);
+    out[4 * i] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
+}
+int main() {
+    const int n = 256;
+    unsigned int* d; cudaMalloc(&d, n * 16);
+    k<<<1, 256>>>(0x1234567887654321ull, d, n);
+    unsigned int h[4 * n]; cudaMemcpy(h, d, n * 16, cudaMemcpyDeviceToHost);
+    for (int i = 0; i < 4 * n; ++i) printf("%u\n", h[i]);
+    return cudaGetLastError() != cudaSuccess;
+}''')
+    exe = tmp_path / "cr"
+    subprocess.check_call([nvcc, "-arch=sm_100a", "-o", str(exe), str(src)])
+    out = subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()
+    want = np.array(out, dtype=np.uint64).astype(np.uint32).reshape(-1, 4)
+    i = np.arange(256, dtype=np.uint64)
+    ctr = np.stack([i * 5, 0 * i + 4, 1000 + 3 * i, 7 + i], 1).astype(np.uint32)
+    assert np.array_equal(orc.philox([0x87654321, 0x12345678], ctr), want)
+
+
+# ------------------------------------------------------------------------------- GA generation (row a6)
+def test_initial_population_matches_oracle(B, orc, cases, dev):
+    c = cases("drug")
+    nrun, P, seed = 3, 150, 12345
+    G = 7 + c.lig.R
+    newpop = torch.zeros((nrun, P, G), dtype=torch.float32, device=dev)
+    B.adock_ga_generation(c.gg, c.gl, c.gp, nrun, P, 0, seed, None, None, newpop)
+    got = newpop.cpu().numpy().astype(np.float64)
+    for run in range(nrun):
+        want = orc.ga_init(c.og, c.lig.R, seed, run, P)
+        assert np.abs(got[run] - want).max() < 4e-6          # exact uniforms; fp32 affine map / trig
+
+
+def test_ga_decisions_bit_exact_and_children_match(B, orc, cases, dev):
+    c = cases("drug")
+    R = c.lig.R
+    nrun, P, seed, G = 4, 150, 777, 7 + c.lig.R
+    rng = np.random.default_rng(1)
+    pop = np.stack([orc.ga_init(c.og, R, 99, run, P) for run in range(nrun)]).astype(np.float32)
+    E = rng.normal(size=(nrun, P)).astype(np.float32)
+    E[0, 10] = E[0, 20] = E[0].min() - 1.0                   # a tie for the elite: lowest slot wins
+    d_pop = torch.from_numpy(pop).to(dev)
+    d_E = torch.from_numpy(E).to(dev)
+    for gen in (1, 2, 57):
+        newpop = torch.zeros_like(d_pop)
+        dec = torch.zeros((nrun, P, 10), dtype=torch.int32, device=dev)
+        picks = torch.full((nrun, P), -1, dtype=torch.int32, device=dev)
+        n_ls = B.adock_ga_generation(c.gg, c.gl, c.gp, nrun, P, gen, seed, d_pop, d_E, newpop, dec, picks)
+        torch.cuda.synchronize()
+        assert n_ls == 9
+        for run in range(nrun):
+            wpop, wE, wdec = orc.ga_offspring(c.op, R, run, gen, seed, pop[run].astype(np.float64), E[run].astype(np.float64))
+            assert np.array_equal(dec[run].cpu().numpy(), wdec)                       # every integer decision
+            assert np.array_equal(picks[run, :n_ls].cpu().numpy(), orc.ls_pick(c.op, P, run, gen, seed))
+            got = newpop[run].cpu().numpy().astype(np.float64)
+            assert np.abs(got - wpop).max() < 2e-6
+            unmut = wdec[:, 9] == 0
+            assert np.array_equal(got[unmut], wpop[unmut])                            # copied genes are bit-identical
+    assert dec[0, 0, 2].item() == 10
+
+
+# ------------------------------------------------------------------------------- ADADELTA (row a5)
+def test_local_search_first_iterations_track_oracle(B, orc, W, cases, dev):
+    c = cases("drug", lsit=4)
+    G = W.make_genotypes(256, c.lig.R, c.grids, seed=21, wall_tail=0.0)
+    d_g = torch.from_numpy(G).to(dev)
+    d_E = torch.zeros(256, device=dev)
+    d_it = torch.zeros(256, dtype=torch.int32, device=dev)
+    B.adock_local_search(c.gg, c.gl, c.gp, d_g, d_E, d_it)
+    torch.cuda.synchronize()
+    assert (d_it.cpu().numpy() == 4).all()
+    gE, gG = d_E.cpu().numpy(), d_g.cpu().numpy()
+    close = 0
+    for i in range(256):
+        og, oE, it = orc.adadelta(c.og, c.ol, c.op, G[i].astype(np.float64))
+        assert it == 4
+        if abs(gE[i] - oE) <= max(1e-4 * abs(oE), 1e-3) and np.abs(gG[i] - og).max() < 1e-3:
+            close += 1
+    assert close >= 250          # a few starts sit on a cell face, where the two precisions take different cells
+
+
+def test_local_search_statistics_match_oracle(B, orc, W, cases, dev):
+    c = cases("drug")
+    n = 384
+    G = W.make_genotypes(n, c.lig.R, c.grids, seed=22, wall_tail=0.0)
+    E0 = orc.score(c.og, c.ol, c.op, G, want_grad=False)["E"]
+    d_g = torch.from_numpy(G).to(dev)
+    d_E = torch.zeros(n, device=dev)
+    d_it = torch.zeros(n, dtype=torch.int32, device=dev)
+    B.adock_local_search(c.gg, c.gl, c.gp, d_g, d_E, d_it)
+    torch.cuda.synchronize()
+    gE = d_E.cpu().numpy().astype(np.float64)
+    assert (d_it.cpu().numpy() == 300).all()
+    assert (gE <= E0 + np.maximum(1e-4 * np.abs(E0), 1e-3)).all()                       # never worse than the start
+    # the returned genotype really has the returned energy
+    chk = orc.score(c.og, c.ol, c.op, d_g.cpu().numpy(), want_grad=False)["E"]
+    assert_energy(gE.astype(np.float32), chk, "LS result")
+    oE = np.array([orc.adadelta(c.og, c.ol, c.op, G[i].astype(np.float64))[1] for i in range(n)])
+    assert stats.ks_2samp(gE, oE).pvalue > 0.01
+    assert stats.mannwhitneyu(gE, oE).pvalue > 0.01
+
+
+# ------------------------------------------------------------------------------- full LGA docking (rows a5-a7)
+def test_dock_tiny_accounting_and_validity(B, orc, cases):
+    c = cases("tiny", lsit=15)
+    P, nrun = 16, 5
+    max_evals = 16 + 20 * (15 + 15)                       # BASELINE.json configs[0]: pop 16, 20 generations
+    r = B.adock_dock(c.gg, c.gl, c.gp, nrun, P, max_evals, seed=0)
+    assert (r["gens"] == 20).all() and (r["evals"] == P + 20 * ((P - 1) + 15)).all()
+    chk = orc.score(c.og, c.ol, c.op, r["genotypes"], want_grad=False)["E"]
+    assert_energy(r["energies"], chk, "dock result energy")
+    for run in range(nrun):
+        x = c.ol.pose(r["genotypes"][run].astype(np.float64))
+        assert np.abs(x - r["coords"][run]).max() < 2e-4
+    assert np.allclose(np.linalg.norm(r["genotypes"][:, 3:7], axis=1), 1.0, atol=1e-5)
+    assert (r["genotypes"][:, 7:] >= -math.pi - 1e-6).all() and (r["genotypes"][:, 7:] <= math.pi + 1e-6).all()
+    r2 = B.adock_dock(c.gg, c.gl, c.gp, nrun, P, max_evals, seed=0)
+    assert np.array_equal(r["energies"], r2["energies"]) and np.array_equal(r["genotypes"], r2["genotypes"])   # deterministic
+    r3 = B.adock_dock(c.gg, c.gl, c.gp, nrun, P, max_evals, seed=1)
+    assert not np.array_equal(r["energies"], r3["energies"])
+    # budget smaller than the initial population: generation 0 only
+    r0 = B.adock_dock(c.gg, c.gl, c.gp, 2, P, 10, seed=0)
+    assert (r0["gens"] == 0).all() and (r0["evals"] == P).all()
+    init = orc.ga_init(c.og, c.lig.R, 0, 0, P)
+    e_init = orc.score(c.og, c.ol, c.op, init.astype(np.float32), want_grad=False)["E"]
+    assert_energy(r0["energies"][:1], np.array([e_init.min()]), "generation-0 best")
+
+
+def test_dock_distribution_matches_oracle(B, orc, cases):
+    """'best-energy distributions over runs statistically indistinguishable' (north_star):
+    5 seeds x 20 runs per side on the tiny config."""
+    c = cases("tiny", lsit=30)
+    P, nrun, max_evals = 16, 20, 16 + 20 * (15 + 30)
+    g, o = [], []
+    for seed in range(5):
+        g.append(B.adock_dock(c.gg, c.gl, c.gp, nrun, P, max_evals, seed=seed)["energies"].astype(np.float64))
+        o.append(orc.dock(c.og, c.ol, c.op, nrun, P, max_evals, seed=seed)["energies"])
+    g, o = np.concatenate(g), np.concatenate(o)
+    assert stats.ks_2samp(g, o).pvalue > 0.01
+    assert stats.mannwhitneyu(g, o).pvalue > 0.01
+    iqr = np.subtract(*np.percentile(o, [75, 25]))
+    assert abs(np.median(g) - np.median(o)) < 0.5 * iqr
+
+
+def test_dock_many_equals_single_docks(B, W, orc, cases):
+    c = cases("drug", lsit=10)
+    ligs = W.make_screen_ligands(3, c.grids)
+    gl = [B.Ligand.from_workload(c.gg, l, c.gp) for l in ligs]
+    seeds = [11, 12, 13]
+    many = B.adock_dock_many(c.gg, gl, c.gp, 4, 30, 2000, seeds, want_coords=True)
+    for k, l in enumerate(gl):
+        one = B.adock_dock(c.gg, l, c.gp, 4, 30, 2000, seeds[k])
+        assert np.array_equal(many["energies"][k], one["energies"])
+        assert np.array_equal(many["genotypes"][k, :, :7 + l.R], one["genotypes"])
+        assert np.array_equal(many["coords"][k, :, :l.N], one["coords"])
+        assert np.array_equal(many["evals"][k], one["evals"])
+
+
+def test_host_only_handle_is_rejected_by_compute_calls(B, cases, dev):
+    c = cases("tiny")
+    hl = B.Ligand.from_workload(None, c.lig)
+    with pytest.raises(B.AdockError) as e:
+        B.adock_score_batch(c.gg, hl, c.gp, torch.zeros((4, 9), device=dev), torch.zeros(4, device=dev), None, None)
+    assert e.value.code == B.ADOCK_EINVAL
