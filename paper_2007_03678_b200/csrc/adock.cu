@@ -79,8 +79,8 @@ extern "C" int adock_default_params(adock_params* p) {
 static ParDev make_pardev(const adock_params& p) {
     const double log2e = 1.4426950408889634;
     ParDev d;
-    d.elec_scale = p.elec_scale; d.diel_A = p.diel_A; d.diel_B = p.diel_B; d.diel_k = p.diel_k;
-    d.lamB = (float)((double)p.diel_lambda * (double)p.diel_B);
+    d.elec_sqrt = (float)std::sqrt((double)p.elec_scale); d.diel_A = p.diel_A; d.diel_B = p.diel_B; d.diel_k = p.diel_k;
+    d.BlamB = (float)((double)p.diel_B * (double)p.diel_lambda * (double)p.diel_B);
     d.mlamB_log2e = (float)(-(double)p.diel_lambda * (double)p.diel_B * log2e);
     d.inv_sig2 = (float)(1.0 / ((double)p.ds_sigma * (double)p.ds_sigma));
     d.mhalf_inv_sig2_log2e = (float)(-0.5 * log2e / ((double)p.ds_sigma * (double)p.ds_sigma));
@@ -96,7 +96,7 @@ static int check_params(const adock_params* in, const adock_ligand* l, adock_par
     const float* f = &out.elec_scale;
     for (int i = 0; i < 18; ++i)
         if (!std::isfinite(f[i])) return fail(ADOCK_EINVAL, "non-finite parameter");
-    if (!(out.ds_sigma > 0) || !(out.r_min > 0) || out.lsit < 0 || out.max_gens < 0 || !(out.ad_eps > 0))
+    if (!(out.ds_sigma > 0) || !(out.r_min > 0) || !(out.elec_scale >= 0) || out.lsit < 0 || out.max_gens < 0 || !(out.ad_eps > 0))
         return fail(ADOCK_EINVAL, "parameter out of range");
     if (l && !l->d_blob) return fail(ADOCK_EINVAL, "host-only ligand handle (loaded with grids == NULL)");
     if (l && (out.w_desolv != l->w_desolv || out.qasp != l->qasp))
@@ -198,9 +198,9 @@ extern "C" int adock_load_ligand(const adock_grids* grids, const adock_params* p
         return ADOCK_OK;
     }
     cudaError_t e = cudaMalloc(&l->d_blob, l->blob_bytes);
-    if (e == cudaSuccess) e = cudaMalloc(&l->d_ext_of_int, N * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&l->d_ext_of_int, l->tp.ext_of_int.size() * sizeof(int));
     if (e == cudaSuccess) e = cudaMemcpy(l->d_blob, l->tp.blob.data(), l->blob_bytes, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy(l->d_ext_of_int, l->tp.ext_of_int.data(), N * sizeof(int), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(l->d_ext_of_int, l->tp.ext_of_int.data(), l->tp.ext_of_int.size() * sizeof(int), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
         cudaFree(l->d_blob); cudaFree(l->d_ext_of_int);
         delete l;
@@ -626,10 +626,12 @@ __global__ void __launch_bounds__(128) dock_final_kernel(GridDev G, ParDev P, co
     float ei, ea;
     eval_pose<false>(L, G, P, S, lane, ei, ea);
     if (job.out_xyz)
-        for (int i = lane; i < L.N; i += 32) {
-            const float4 x = S.X[i];
-            float* o = job.out_xyz + ((size_t)run * dm.cstride + job.ext_of_int[i]) * 3;
-            o[0] = x.x; o[1] = x.y; o[2] = x.z;
+        for (int i = lane; i < L.npos; i += 32) {
+            const int e = job.ext_of_int[i];
+            if (e < 0) continue;
+            const float* b = S.blk + atom_slot_dev(i);
+            float* o = job.out_xyz + ((size_t)run * dm.cstride + e) * 3;
+            o[0] = b[kX]; o[1] = b[kY]; o[2] = b[kZ];
         }
     if (lane == 0) {
         job.out_E[run] = E[bi];

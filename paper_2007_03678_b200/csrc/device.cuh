@@ -24,7 +24,7 @@ struct GridDev {
 };
 
 struct ParDev {             // adock_params with the per-pair constants folded
-    float elec_scale, diel_A, diel_B, diel_k, lamB, mlamB_log2e;   // lamB = lambda*B
+    float elec_sqrt, diel_A, diel_B, diel_k, BlamB, mlamB_log2e;   // elec_sqrt = sqrt(elec_scale); BlamB = B*lambda*B
     float inv_sig2, mhalf_inv_sig2_log2e;
     float rmin2, k_wall, k_wall_h;
     float ad_rho, ad_eps;
@@ -34,12 +34,13 @@ struct ParDev {             // adock_params with the per-pair constants folded
 
 // ---------------------------------------------------------------- shared-memory views
 struct LigS {
-    const float4* atoms;    // (x0 - pivot, q), internal order
-    const uint32_t* meta;   // type | frag<<8
+    const float4* atoms;    // (x0 - pivot, q) by position
+    const uint32_t* meta;   // type | frag<<8 ; 0xffffffff = hole
+    const uint16_t* fragatoms;  // positions grouped by fragment
     const float4* fg;       // FragGeom as 2 float4
     const int4* fi;         // FragIdx
     const uint4* pairs;     // PairRec rounds
-    int N, R, nfrag, nrounds;
+    int N, R, nfrag, nrounds, npos, nfull;
 };
 
 struct WarpS {
@@ -49,15 +50,17 @@ struct WarpS {
     float2* sc;             // [nfrag] sin,cos of the fragment's torsion
     float4* fragT;          // [nfrag][3] rows of the 3x4 fragment transform
     float4* fragAx;         // [nfrag][2] posed axis, posed pivot point - t
-    float4* fragFT;         // [nfrag][2] force, torque about t
-    float4* X;              // [N] posed xyz, q
-    float4* Gr;             // [N] dE/dx
+    float4* fragFT;         // [nfrag][2] force, torque about the fragment's own pivot point
+    float* blk;             // pose block, 256 floats per 32 atoms: x|y|z|q|gx|gy|gz|-  (32 each), so atom a
+                            // lives at slot(a) = (a>>5)*256 + (a&31) and distinct a mod 32 hit distinct banks
 };
+constexpr int kX = 0, kY = 32, kZ = 64, kQ = 96, kGX = 128, kGY = 160, kGZ = 192;
+__host__ __device__ inline int atom_slot_dev(int a) { return (a >> 5) * 256 + (a & 31); }
 
 __host__ __device__ inline int pad4(int x) { return (x + 3) & ~3; }
 // floats of per-warp scratch for a ligand with N atoms, nfrag fragments, R torsions
 __host__ __device__ inline int warp_scratch_floats(int N, int nfrag, int R) {
-    return 2 * pad4(7 + R) + pad4(6 + R) + pad4(2 * nfrag) + nfrag * 28 + N * 8;
+    return 2 * pad4(7 + R) + pad4(6 + R) + pad4(2 * nfrag) + nfrag * 28 + ((N + 31) / 32) * 256;
 }
 
 __device__ inline LigS lig_view(const unsigned char* blob) {
@@ -68,7 +71,8 @@ __device__ inline LigS lig_view(const unsigned char* blob) {
     L.fg = reinterpret_cast<const float4*>(blob + h->off_frag);
     L.fi = reinterpret_cast<const int4*>(blob + h->off_fragidx);
     L.pairs = reinterpret_cast<const uint4*>(blob + h->off_pairs);
-    L.N = h->N; L.R = h->R; L.nfrag = h->nfrag; L.nrounds = h->nrounds;
+    L.fragatoms = reinterpret_cast<const uint16_t*>(blob + h->off_fragatoms);
+    L.N = h->N; L.R = h->R; L.nfrag = h->nfrag; L.nrounds = h->nrounds; L.npos = h->npos; L.nfull = h->nfull;
     return L;
 }
 
@@ -82,8 +86,7 @@ __device__ inline WarpS warp_view(float* base, const LigS& L) {
     S.fragT = reinterpret_cast<float4*>(base); base += 12 * L.nfrag;
     S.fragAx = reinterpret_cast<float4*>(base); base += 8 * L.nfrag;
     S.fragFT = reinterpret_cast<float4*>(base); base += 8 * L.nfrag;
-    S.X = reinterpret_cast<float4*>(base); base += 4 * L.N;
-    S.Gr = reinterpret_cast<float4*>(base);
+    S.blk = base;
     return S;
 }
 
@@ -124,6 +127,24 @@ __device__ __forceinline__ F8 ld_cell(const float4* p) {     // one aligned 32-b
     return r;
 }
 
+// trilinear interpolant of 8 corner values (a = ix, b = ix+1; first index z, second y) at fractions fx,fy,fz:
+// value and derivatives with respect to the fractions
+template <bool GRAD>
+__device__ __forceinline__ void trilinear8(float a00, float b00, float a01, float b01, float a10, float b10, float a11, float b11,
+                                           float fx, float fy, float fz, float& val, float& dfx, float& dfy, float& dfz) {
+    const float d00 = b00 - a00, d01 = b01 - a01, d10 = b10 - a10, d11 = b11 - a11;       // d/dfx per row
+    const float v00 = fmaf(fx, d00, a00), v01 = fmaf(fx, d01, a01), v10 = fmaf(fx, d10, a10), v11 = fmaf(fx, d11, a11);
+    const float e0 = v01 - v00, e1 = v11 - v10;                                            // d/dfy per z-plane
+    const float w0 = fmaf(fy, e0, v00), w1 = fmaf(fy, e1, v10);
+    val = fmaf(fz, w1 - w0, w0);
+    if (GRAD) {
+        const float dx0 = fmaf(fy, d01 - d00, d00), dx1 = fmaf(fy, d11 - d10, d10);
+        dfx = fmaf(fz, dx1 - dx0, dx0);
+        dfy = fmaf(fz, e1 - e0, e0);
+        dfz = w1 - w0;
+    }
+}
+
 template <bool GRAD>
 __device__ __forceinline__ float grid_atom(const GridDev& G, const ParDev& P, int type, float q, float x, float y, float z,
                                            float& gx, float& gy, float& gz) {
@@ -137,35 +158,78 @@ __device__ __forceinline__ float grid_atom(const GridDev& G, const ParDev& P, in
     const float4* base = G.cells + (long long)type * G.type_stride + ((long long)(iz * G.ny + iy) * (G.nx - 1) + ix) * 2;
     F8 c00 = ld_cell(base), c01 = ld_cell(base + rowlen), c10 = ld_cell(base + (long long)G.ny * rowlen),
        c11 = ld_cell(base + (long long)G.ny * rowlen + rowlen);
-    float aq = fabsf(q);
-    // per-corner field value: affinity + q*elec + |q|*desolv
-    float a00 = fmaf(aq, c00.lo.z, fmaf(q, c00.lo.y, c00.lo.x)), b00 = fmaf(aq, c00.hi.z, fmaf(q, c00.hi.y, c00.hi.x));
-    float a01 = fmaf(aq, c01.lo.z, fmaf(q, c01.lo.y, c01.lo.x)), b01 = fmaf(aq, c01.hi.z, fmaf(q, c01.hi.y, c01.hi.x));
-    float a10 = fmaf(aq, c10.lo.z, fmaf(q, c10.lo.y, c10.lo.x)), b10 = fmaf(aq, c10.hi.z, fmaf(q, c10.hi.y, c10.hi.x));
-    float a11 = fmaf(aq, c11.lo.z, fmaf(q, c11.lo.y, c11.lo.x)), b11 = fmaf(aq, c11.hi.z, fmaf(q, c11.hi.y, c11.hi.x));
-    float d00 = b00 - a00, d01 = b01 - a01, d10 = b10 - a10, d11 = b11 - a11;       // d/dfx per row
-    float v00 = fmaf(fx, d00, a00), v01 = fmaf(fx, d01, a01), v10 = fmaf(fx, d10, a10), v11 = fmaf(fx, d11, a11);
-    float e0 = v01 - v00, e1 = v11 - v10;                                            // d/dfy per z-plane
-    float w0 = fmaf(fy, e0, v00), w1 = fmaf(fy, e1, v10);
-    float val = fmaf(fz, w1 - w0, w0);
+    const float aq = fabsf(q);
+    // Two interpolants, combined only at the end: the affinity map (values up to the 1e5 clamp) and
+    // q*elec + |q|*desolv (values O(1)).  Mixing them per corner would round the small field to the ulp of the
+    // large one (0.008 at 1e5) before the corner differences that make the gradient are taken.
+    float val, dfx, dfy, dfz;
+    trilinear8<GRAD>(c00.lo.x, c00.hi.x, c01.lo.x, c01.hi.x, c10.lo.x, c10.hi.x, c11.lo.x, c11.hi.x, fx, fy, fz, val, dfx, dfy, dfz);
+    float vs, sfx, sfy, sfz;
+    trilinear8<GRAD>(fmaf(aq, c00.lo.z, q * c00.lo.y), fmaf(aq, c00.hi.z, q * c00.hi.y), fmaf(aq, c01.lo.z, q * c01.lo.y),
+                     fmaf(aq, c01.hi.z, q * c01.hi.y), fmaf(aq, c10.lo.z, q * c10.lo.y), fmaf(aq, c10.hi.z, q * c10.hi.y),
+                     fmaf(aq, c11.lo.z, q * c11.lo.y), fmaf(aq, c11.hi.z, q * c11.hi.y), fx, fy, fz, vs, sfx, sfy, sfz);
+    val += vs;
     float wall = fabsf(ox) + fabsf(oy) + fabsf(oz);
     val = fmaf(P.k_wall_h, wall, val);
     if (GRAD) {
-        float dx0 = fmaf(fy, d01 - d00, d00), dx1 = fmaf(fy, d11 - d10, d10);
-        float dfx = fmaf(fz, dx1 - dx0, dx0);
-        float dfy = fmaf(fz, e1 - e0, e0);
-        float dfz = w1 - w0;
-        gx = (ox != 0.f) ? copysignf(P.k_wall, ox) : dfx * G.inv_h;
-        gy = (oy != 0.f) ? copysignf(P.k_wall, oy) : dfy * G.inv_h;
-        gz = (oz != 0.f) ? copysignf(P.k_wall, oz) : dfz * G.inv_h;
+        gx = (ox != 0.f) ? copysignf(P.k_wall, ox) : (dfx + sfx) * G.inv_h;
+        gy = (oy != 0.f) ? copysignf(P.k_wall, oy) : (dfy + sfy) * G.inv_h;
+        gz = (oz != 0.f) ? copysignf(P.k_wall, oz) : (dfz + sfz) * G.inv_h;
     }
     return val;
 }
+
+// single-instruction MUFU forms (flush-to-zero): reciprocal, reciprocal square root, 2^x
+__device__ __forceinline__ float frcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float frsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float fex2(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
     return v;
+}
+
+// ---------------------------------------------------------------- intramolecular pair term (R5): one warp round
+// Each lane evaluates one pair (i,j) of the round and adds +f to atom i, then -f to atom j.  Within a round no
+// atom occurs twice on a side (topology.hpp), so the read-modify-writes need no atomics and their order is fixed.
+template <bool GRAD, bool MAYPAD>
+__device__ __forceinline__ float pair_round(const LigS& L, const ParDev& P, const WarpS& S, int r, int lane) {
+    const uint4 rec = L.pairs[r * 32 + lane];
+    const bool valid = !MAYPAD || ((rec.x >> 23) & 1u);
+    float* pi = S.blk + (rec.x & 0x7ffu);
+    float* pj = S.blk + ((rec.x >> 11) & 0x7ffu);
+    const float dx = pi[kX] - pj[kX], dy = pi[kY] - pj[kY], dz = pi[kZ] - pj[kZ];
+    const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+    const float r2c = fmaxf(r2, P.rmin2);
+    const float rinv = frsqrt(r2c);
+    const float rr = r2c * rinv;
+    const float rinv2 = rinv * rinv;
+    const float r6 = rinv2 * rinv2 * rinv2, r12 = r6 * r6;
+    const bool hb = (rec.x >> 22) & 1u;
+    const float rA = hb ? r12 * r2c : r6;
+    const float c12 = __uint_as_float(rec.y), cA = __uint_as_float(rec.z), ds = __uint_as_float(rec.w);
+    const float u12 = c12 * r12, uA = cA * rA;
+    const float ex = fex2(rr * P.mlamB_log2e);
+    const float rden = frcp(fmaf(P.diel_k, ex, 1.f));
+    const float eps = fmaf(P.diel_B, rden, P.diel_A);
+    const float inv_er = rinv * frcp(eps);
+    const float eel = pi[kQ] * pj[kQ] * inv_er;                 // charges are stored pre-scaled by sqrt(elec_scale)
+    const float egs = ds * fex2(r2c * P.mhalf_inv_sig2_log2e);
+    const float e = (u12 - uA) + eel + egs;
+    if (GRAD) {
+        const float dv = fmaf(hb ? 10.f : 6.f, uA, -12.f * u12);            // r * d(vdw)/dr
+        const float deps = P.BlamB * (1.f - rden) * rden;
+        const float del = -eel * fmaf(deps, rr, eps) * inv_er;             // d(elec)/dr
+        const float dds = -rr * P.inv_sig2 * egs;                          // d(desolv)/dr
+        const float fs = (r2 >= P.rmin2) ? fmaf(dv, rinv, del + dds) * rinv : 0.f;
+        const float fx = fs * dx, fy = fs * dy, fz = fs * dz;
+        if (valid) { pi[kGX] += fx; pi[kGY] += fy; pi[kGZ] += fz; }
+        __syncwarp();
+        if (valid) { pj[kGX] -= fx; pj[kGY] -= fy; pj[kGZ] -= fz; }
+        __syncwarp();
+    }
+    return valid ? e : 0.f;
 }
 
 // ---------------------------------------------------------------- full evaluation of one genotype by one warp
@@ -227,6 +291,7 @@ __device__ __forceinline__ float eval_pose(const LigS& L, const GridDev& G, cons
         S.fragT[3 * f] = make_float4(t00, t01, t02, t03 + tx);
         S.fragT[3 * f + 1] = make_float4(t10, t11, t12, t13 + ty);
         S.fragT[3 * f + 2] = make_float4(t20, t21, t22, t23 + tz);
+        if (GRAD && f == 0) S.fragAx[1] = make_float4(0.f, 0.f, 0.f, 0.f);        // root pivot point = t
         if (GRAD && f > 0) {
             const float4 p0 = L.fg[2 * f], u = L.fg[2 * f + 1];
             S.fragAx[2 * f] = make_float4(t00 * u.x + t01 * u.y + t02 * u.z, t10 * u.x + t11 * u.y + t12 * u.z,
@@ -239,67 +304,27 @@ __device__ __forceinline__ float eval_pose(const LigS& L, const GridDev& G, cons
 
     // (a1,a2) atoms: pose, then trilinear lookup of the three maps
     float eg = 0.f;
-    for (int i = lane; i < L.N; i += 32) {
-        const float4 a = L.atoms[i];
+    for (int i = lane; i < L.npos; i += 32) {
         const uint32_t m = L.meta[i];
+        if (m == 0xffffffffu) continue;                  // hole
+        const float4 a = L.atoms[i];
         const int f = m >> 8;
         const float4 t0 = S.fragT[3 * f], t1 = S.fragT[3 * f + 1], t2 = S.fragT[3 * f + 2];
         const float x = fmaf(t0.x, a.x, fmaf(t0.y, a.y, fmaf(t0.z, a.z, t0.w)));
         const float y = fmaf(t1.x, a.x, fmaf(t1.y, a.y, fmaf(t1.z, a.z, t1.w)));
         const float z = fmaf(t2.x, a.x, fmaf(t2.y, a.y, fmaf(t2.z, a.z, t2.w)));
-        S.X[i] = make_float4(x, y, z, a.w);
+        float* b = S.blk + atom_slot_dev(i);
+        b[kX] = x; b[kY] = y; b[kZ] = z; b[kQ] = a.w * P.elec_sqrt;
         float gx, gy, gz;
         eg += grid_atom<GRAD>(G, P, (int)(m & 0xff), a.w, x, y, z, gx, gy, gz);
-        if (GRAD) S.Gr[i] = make_float4(gx, gy, gz, 0.f);
+        if (GRAD) { b[kGX] = gx; b[kGY] = gy; b[kGZ] = gz; }
     }
     __syncwarp();
 
-    // (a3) intramolecular pairs: conflict-free warp rounds
+    // (a3) intramolecular pairs: conflict-free warp rounds; the first nfull rounds have no padding slot
     float ep = 0.f;
-    for (int r = 0; r < L.nrounds; ++r) {
-        const uint4 rec = L.pairs[r * 32 + lane];
-        const bool valid = (rec.x >> 17) & 1u;
-        const int i = rec.x & 0xff, j = (rec.x >> 8) & 0xff;
-        const float4 xi = S.X[i], xj = S.X[j];
-        const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
-        const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-        const float r2c = fmaxf(r2, P.rmin2);
-        const float rinv = rsqrtf(r2c);
-        const float rr = r2c * rinv;
-        const float rinv2 = rinv * rinv;
-        const float r6 = rinv2 * rinv2 * rinv2, r12 = r6 * r6;
-        const bool hb = (rec.x >> 16) & 1u;
-        const float rA = hb ? r12 * r2c : r6;
-        const float c12 = __uint_as_float(rec.y), cA = __uint_as_float(rec.z), ds = __uint_as_float(rec.w);
-        const float ev = fmaf(c12, r12, -cA * rA);
-        const float ex = exp2f(rr * P.mlamB_log2e);
-        const float rden = __fdividef(1.f, fmaf(P.diel_k, ex, 1.f));
-        const float eps = fmaf(P.diel_B, rden, P.diel_A);
-        const float inv_er = __fdividef(rinv, eps);
-        const float eel = P.elec_scale * xi.w * xj.w * inv_er;
-        const float egs = ds * exp2f(r2c * P.mhalf_inv_sig2_log2e);
-        if (valid) ep += ev + eel + egs;
-        if (GRAD) {
-            const float dv = fmaf(hb ? 10.f : 6.f, cA * rA, -12.f * c12 * r12) * rinv;
-            const float deps = P.diel_B * P.lamB * (1.f - rden) * rden;
-            const float del = -eel * fmaf(deps, rr, eps) * inv_er;
-            const float dds = -rr * P.inv_sig2 * egs;
-            const float fs = (r2 >= P.rmin2) ? (dv + del + dds) * rinv : 0.f;
-            const float fx = fs * dx, fy = fs * dy, fz = fs * dz;
-            if (valid) {
-                float4 g = S.Gr[i];
-                g.x += fx; g.y += fy; g.z += fz;
-                S.Gr[i] = g;
-            }
-            __syncwarp();
-            if (valid) {
-                float4 g = S.Gr[j];
-                g.x -= fx; g.y -= fy; g.z -= fz;
-                S.Gr[j] = g;
-            }
-            __syncwarp();
-        }
-    }
+    for (int r = 0; r < L.nfull; ++r) ep += pair_round<GRAD, false>(L, P, S, r, lane);
+    for (int r = L.nfull; r < L.nrounds; ++r) ep += pair_round<GRAD, true>(L, P, S, r, lane);
     e_inter = warp_sum(eg);
     e_intra = warp_sum(ep);
 
@@ -307,12 +332,15 @@ __device__ __forceinline__ float eval_pose(const LigS& L, const GridDev& G, cons
     if (GRAD) {
         for (int f = lane; f < L.nfrag; f += 32) {
             const int4 ix = L.fi[f];
+            const float4 pv = S.fragAx[2 * f + 1];               // this fragment's pivot point, relative to t
+            const float px = tx + pv.x, py = ty + pv.y, pz = tz + pv.z;
             float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
-            for (int i = ix.y; i < ix.z; ++i) {
-                const float4 g = S.Gr[i], x = S.X[i];
-                const float rx = x.x - tx, ry = x.y - ty, rz = x.z - tz;
-                Fx += g.x; Fy += g.y; Fz += g.z;
-                Tx += ry * g.z - rz * g.y; Ty += rz * g.x - rx * g.z; Tz += rx * g.y - ry * g.x;
+            for (int k = ix.y; k < ix.z; ++k) {
+                const float* b = S.blk + atom_slot_dev(L.fragatoms[k]);
+                const float gx = b[kGX], gy = b[kGY], gz = b[kGZ];
+                const float rx = b[kX] - px, ry = b[kY] - py, rz = b[kZ] - pz;
+                Fx += gx; Fy += gy; Fz += gz;
+                Tx += ry * gz - rz * gy; Ty += rz * gx - rx * gz; Tz += rx * gy - ry * gx;
             }
             S.fragFT[2 * f] = make_float4(Fx, Fy, Fz, 0.f);
             S.fragFT[2 * f + 1] = make_float4(Tx, Ty, Tz, 0.f);
@@ -321,18 +349,22 @@ __device__ __forceinline__ float eval_pose(const LigS& L, const GridDev& G, cons
         for (int f = lane; f < L.nfrag; f += 32) {
             const int w = L.fi[f].w;
             const int sub_end = w & 0xffff;
+            const float4 pf = S.fragAx[2 * f + 1];
+            // force and torque ABOUT THIS fragment's pivot point of the whole subtree: each member's torque
+            // (about its own pivot) is shifted by the short lever between the two pivots
             float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
             for (int g = f; g < sub_end; ++g) {
-                const float4 F = S.fragFT[2 * g], T = S.fragFT[2 * g + 1];
-                Fx += F.x; Fy += F.y; Fz += F.z; Tx += T.x; Ty += T.y; Tz += T.z;
+                const float4 F = S.fragFT[2 * g], T = S.fragFT[2 * g + 1], pg = S.fragAx[2 * g + 1];
+                const float lx = pg.x - pf.x, ly = pg.y - pf.y, lz = pg.z - pf.z;
+                Fx += F.x; Fy += F.y; Fz += F.z;
+                Tx += T.x + (ly * F.z - lz * F.y); Ty += T.y + (lz * F.x - lx * F.z); Tz += T.z + (lx * F.y - ly * F.x);
             }
             if (f == 0) {
                 S.grad[0] = Fx; S.grad[1] = Fy; S.grad[2] = Fz;
                 S.grad[3] = Tx; S.grad[4] = Ty; S.grad[5] = Tz;
             } else {
-                const float4 u = S.fragAx[2 * f], xa = S.fragAx[2 * f + 1];     // xa relative to t
-                const float cx = Tx - (xa.y * Fz - xa.z * Fy), cy = Ty - (xa.z * Fx - xa.x * Fz), cz = Tz - (xa.x * Fy - xa.y * Fx);
-                S.grad[6 + (w >> 16)] = u.x * cx + u.y * cy + u.z * cz;
+                const float4 u = S.fragAx[2 * f];
+                S.grad[6 + (w >> 16)] = u.x * Tx + u.y * Ty + u.z * Tz;
             }
         }
         __syncwarp();

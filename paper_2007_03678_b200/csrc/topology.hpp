@@ -21,11 +21,12 @@ constexpr int kMaxTors = 64;
 using AtomSet = std::bitset<kMaxAtoms>;
 
 // ---- device blob layout (all sections 16-byte aligned; staged into shared memory in one bulk copy)
-struct LigHeader {          // 64 bytes
+struct LigHeader {          // 80 bytes
     int N, R, nfrag, npairs;
     int nrounds, T, off_atoms, off_meta;
     int off_frag, off_fragidx, off_pairs, bytes;
-    int max_frag_atoms, max_depth, pad0, pad1;
+    int max_frag_atoms, max_depth, npos, off_fragatoms;   // npos = 32*ceil(N/32) atom positions (some may be holes)
+    int nfull, pad1, pad2, pad3;                          // rounds [0,nfull) have all 32 slots valid
 };
 struct FragGeom {           // 32 bytes: torsion axis of the bond that attaches fragment f to its parent
     float p0[3]; float pad0;   // x0[a_k] - pivot
@@ -33,13 +34,15 @@ struct FragGeom {           // 32 bytes: torsion axis of the bond that attaches 
 };
 struct FragIdx {            // 16 bytes
     int parent;             // parent fragment (internal id); -1 for the root
-    int atom_begin, atom_end;   // internal atom range of this fragment
+    int atom_begin, atom_end;   // this fragment's range in the fragatoms list (uint16 positions)
     int sub_end_tor;        // (subtree end fragment id) | (external torsion index << 16); root: tor = 0xffff
 };
 struct PairRec {            // 16 bytes: one slot of a warp round
-    uint32_t ij;            // i | j<<8 | hbond<<16 | valid<<17   (internal atom ids)
+    uint32_t ij;            // slot(i) | slot(j)<<11 | hbond<<22 | valid<<23, slot(q) = (q>>5)*256 + (q&31):
+                            // word offset of the atom at position q in the per-warp pose block (device.cuh)
     float c12, cA, ds;      // weighted coefficients; ds = w_desolv*(S_i V_j + S_j V_i)
 };
+inline uint32_t atom_slot(int a) { return (uint32_t)((a >> 5) * 256 + (a & 31)); }
 
 struct Topology {
     int N = 0, R = 0, T = 0, nfrag = 0;
@@ -49,7 +52,7 @@ struct Topology {
     std::vector<unsigned char> moved;     // [R][N]
     std::vector<int> depth;
     float pivot[3] = {0, 0, 0};
-    // internal numbering
+    // positions: int_of_ext [N] atom -> position, ext_of_int [npos] position -> atom or -1 (hole)
     std::vector<int> ext_of_int, int_of_ext;
     std::vector<unsigned char> blob;      // device image
     std::string error;
@@ -135,7 +138,7 @@ inline bool build_topology(Topology& tp, int N, const float* xyz, const int* typ
             if (flex) { tp.pairs.push_back(i); tp.pairs.push_back(j); }
         }
 
-    // ---- internal numbering: fragments in DFS preorder (children by torsion index), atoms by fragment
+    // ---- fragments in DFS preorder (children by torsion index): every torsion subtree is a contiguous fragment range
     std::vector<int> frag_of(N, -1);
     struct Frag { int parent, tor; std::vector<int> atoms; int sub_end; };
     std::vector<Frag> frags;
@@ -152,21 +155,44 @@ inline bool build_topology(Topology& tp, int N, const float* xyz, const int* typ
     tp.nfrag = (int)frags.size();
     for (int i = 0; i < N; ++i)
         if (frag_of[i] < 0) { tp.error = "ligand graph is not connected"; return false; }
-    tp.ext_of_int.clear(); tp.int_of_ext.assign(N, -1);
+    // ---- atom positions.  Position q = pass*32 + lane is the atom's slot in every per-warp array, so its
+    // shared-memory bank is q mod 32.  Crowded atoms (many pairs) get a bank of their own; when N > 32 the
+    // atoms with the fewest pairs share banks (longest-processing-time assignment of pair counts to banks).
+    std::vector<int> deg_ext(N, 0);
+    for (size_t p = 0; p < tp.pairs.size(); ++p) ++deg_ext[tp.pairs[p]];
+    const int npass = (N + 31) / 32, npos = npass * 32;
+    std::vector<int> by_deg(N);
+    for (int i = 0; i < N; ++i) by_deg[i] = i;
+    std::stable_sort(by_deg.begin(), by_deg.end(), [&](int x, int y) { return deg_ext[x] > deg_ext[y]; });
+    std::vector<int> bank_load(32, 0), bank_cnt(32, 0);
+    tp.ext_of_int.assign(npos, -1); tp.int_of_ext.assign(N, -1);
+    for (int e : by_deg) {
+        int best = -1;
+        for (int r = 0; r < 32; ++r)
+            if (bank_cnt[r] < npass && (best < 0 || bank_load[r] < bank_load[best])) best = r;
+        const int q = bank_cnt[best] * 32 + best;
+        tp.int_of_ext[e] = q; tp.ext_of_int[q] = e;
+        ++bank_cnt[best]; bank_load[best] += deg_ext[e];
+    }
+    // fragment member lists (positions), fragment by fragment
+    std::vector<uint16_t> fragatoms;
     std::vector<int> fbeg(tp.nfrag), fend(tp.nfrag);
     int max_frag_atoms = 0;
     for (int f = 0; f < tp.nfrag; ++f) {
-        fbeg[f] = (int)tp.ext_of_int.size();
-        for (int e : frags[f].atoms) { tp.int_of_ext[e] = (int)tp.ext_of_int.size(); tp.ext_of_int.push_back(e); }
-        fend[f] = (int)tp.ext_of_int.size();
+        fbeg[f] = (int)fragatoms.size();
+        for (int e : frags[f].atoms) fragatoms.push_back((uint16_t)tp.int_of_ext[e]);
+        fend[f] = (int)fragatoms.size();
         max_frag_atoms = std::max(max_frag_atoms, fend[f] - fbeg[f]);
     }
 
-    // ---- pair schedule: rounds of 32 slots, every atom at most once as i and once as j per round
+    // ---- pair schedule: rounds of 32 slots.  Hard rule (correctness of the atomics-free force scatter): within a
+    // round no atom occurs twice as i or twice as j.  Soft rule (speed): the i positions of a round are distinct
+    // modulo 32, and so are the j positions, so each side touches 32 different banks; a slot that cannot be
+    // filled under the soft rule is filled under the hard rule alone (a 2-way conflict beats an extra round).
     struct P { int a, b; };
     std::vector<P> rem;
     for (size_t p = 0; p < tp.pairs.size(); p += 2) rem.push_back({tp.int_of_ext[tp.pairs[p]], tp.int_of_ext[tp.pairs[p + 1]]});
-    std::vector<int> deg(N, 0);
+    std::vector<int> deg(npos, 0);
     for (auto& p : rem) { ++deg[p.a]; ++deg[p.b]; }
     std::vector<PairRec> recs;
     auto make_rec = [&](int i, int j) {
@@ -176,44 +202,68 @@ inline bool build_topology(Topology& tp, int N, const float* xyz, const int* typ
         double Si = (double)solpar[ti] + (double)qasp * std::fabs((double)charge[ei]);
         double Sj = (double)solpar[tj] + (double)qasp * std::fabs((double)charge[ej]);
         PairRec r;
-        r.ij = (uint32_t)i | ((uint32_t)j << 8) | ((co[2] > 8.0f ? 1u : 0u) << 16) | (1u << 17);
+        r.ij = atom_slot(i) | (atom_slot(j) << 11) | ((co[2] > 8.0f ? 1u : 0u) << 22) | (1u << 23);
         r.c12 = co[0]; r.cA = co[1];
         r.ds = (float)((double)w_desolv * (Si * (double)vol[tj] + Sj * (double)vol[ti]));
         return r;
     };
-    int nrounds = 0;
+    int nrounds = 0, nfull = 0;
     while (!rem.empty()) {
         // highest remaining degree first, so crowded atoms are spread over the rounds
         std::stable_sort(rem.begin(), rem.end(), [&](const P& x, const P& y) {
             return std::max(deg[x.a], deg[x.b]) > std::max(deg[y.a], deg[y.b]);
         });
-        AtomSet usedI, usedJ;
-        std::vector<P> keep;
+        AtomSet atomI, atomJ;
+        std::bitset<32> bankI, bankJ;
+        std::vector<char> taken(rem.size(), 0);
         int filled = 0;
-        for (auto& p : rem) {
-            if (filled < 32 && !usedI.test(p.a) && !usedJ.test(p.b)) {
-                usedI.set(p.a); usedJ.set(p.b); recs.push_back(make_rec(p.a, p.b)); ++filled; --deg[p.a]; --deg[p.b];
-            } else if (filled < 32 && !usedI.test(p.b) && !usedJ.test(p.a)) {
-                usedI.set(p.b); usedJ.set(p.a); recs.push_back(make_rec(p.b, p.a)); ++filled; --deg[p.a]; --deg[p.b];
-            } else {
-                keep.push_back(p);
+        for (int pass = 0; pass < 2 && filled < 32; ++pass)          // pass 0: soft + hard rule, pass 1: hard rule only
+            for (size_t k = 0; k < rem.size() && filled < 32; ++k) {
+                if (taken[k]) continue;
+                const P p = rem[k];
+                auto fits = [&](int i, int j) {
+                    if (atomI.test(i) || atomJ.test(j)) return false;
+                    return pass == 1 || (!bankI.test(i & 31) && !bankJ.test(j & 31));
+                };
+                int i = -1, j = -1;
+                if (fits(p.a, p.b)) { i = p.a; j = p.b; } else if (fits(p.b, p.a)) { i = p.b; j = p.a; }
+                if (i < 0) continue;
+                atomI.set(i); atomJ.set(j); bankI.set(i & 31); bankJ.set(j & 31);
+                recs.push_back(make_rec(i, j));
+                taken[k] = 1; ++filled; --deg[p.a]; --deg[p.b];
             }
-        }
+        if (filled == 32) ++nfull;
         for (; filled < 32; ++filled) recs.push_back(PairRec{0u, 0.f, 0.f, 0.f});
+        std::vector<P> keep;
+        for (size_t k = 0; k < rem.size(); ++k) if (!taken[k]) keep.push_back(rem[k]);
         rem.swap(keep);
         ++nrounds;
+    }
+
+    {   // full rounds first (their kernel loop carries no validity tests), padded rounds after
+        std::vector<PairRec> full, part;
+        for (int r = 0; r < nrounds; ++r) {
+            bool all = true;
+            for (int l = 0; l < 32; ++l) all = all && ((recs[(size_t)r * 32 + l].ij >> 23) & 1u);
+            auto& dst = all ? full : part;
+            dst.insert(dst.end(), recs.begin() + (size_t)r * 32, recs.begin() + (size_t)(r + 1) * 32);
+        }
+        full.insert(full.end(), part.begin(), part.end());
+        recs.swap(full);
     }
 
     // ---- blob
     auto align16 = [](size_t x) { return (x + 15) & ~(size_t)15; };
     LigHeader h{};
     h.N = N; h.R = R; h.nfrag = tp.nfrag; h.npairs = (int)tp.pairs.size() / 2; h.nrounds = nrounds; h.T = T;
+    h.npos = npos; h.nfull = nfull;
     size_t off = sizeof(LigHeader);
-    h.off_atoms = (int)off;   off = align16(off + (size_t)N * 16);
-    h.off_meta = (int)off;    off = align16(off + (size_t)N * 4);
-    h.off_frag = (int)off;    off = align16(off + (size_t)tp.nfrag * sizeof(FragGeom));
-    h.off_fragidx = (int)off; off = align16(off + (size_t)tp.nfrag * sizeof(FragIdx));
-    h.off_pairs = (int)off;   off = align16(off + recs.size() * sizeof(PairRec));
+    h.off_atoms = (int)off;     off = align16(off + (size_t)npos * 16);
+    h.off_meta = (int)off;      off = align16(off + (size_t)npos * 4);
+    h.off_frag = (int)off;      off = align16(off + (size_t)tp.nfrag * sizeof(FragGeom));
+    h.off_fragidx = (int)off;   off = align16(off + (size_t)tp.nfrag * sizeof(FragIdx));
+    h.off_fragatoms = (int)off; off = align16(off + fragatoms.size() * sizeof(uint16_t));
+    h.off_pairs = (int)off;     off = align16(off + recs.size() * sizeof(PairRec));
     h.bytes = (int)off;
     h.max_frag_atoms = max_frag_atoms;
     int maxd = 0;
@@ -223,11 +273,12 @@ inline bool build_topology(Topology& tp, int N, const float* xyz, const int* typ
     std::memcpy(tp.blob.data(), &h, sizeof(h));
     float* atoms = (float*)(tp.blob.data() + h.off_atoms);
     uint32_t* meta = (uint32_t*)(tp.blob.data() + h.off_meta);
-    for (int i = 0; i < N; ++i) {
-        int e = tp.ext_of_int[i];
-        for (int d = 0; d < 3; ++d) atoms[4 * i + d] = (float)((double)xyz[3 * e + d] - (double)tp.pivot[d]);
-        atoms[4 * i + 3] = charge[e];
-        meta[i] = (uint32_t)type[e] | ((uint32_t)frag_of[e] << 8);
+    for (int q = 0; q < npos; ++q) {
+        const int e = tp.ext_of_int[q];
+        if (e < 0) { meta[q] = 0xffffffffu; continue; }          // hole
+        for (int d = 0; d < 3; ++d) atoms[4 * q + d] = (float)((double)xyz[3 * e + d] - (double)tp.pivot[d]);
+        atoms[4 * q + 3] = charge[e];
+        meta[q] = (uint32_t)type[e] | ((uint32_t)frag_of[e] << 8);
     }
     FragGeom* fg = (FragGeom*)(tp.blob.data() + h.off_frag);
     FragIdx* fi = (FragIdx*)(tp.blob.data() + h.off_fragidx);
@@ -248,6 +299,7 @@ inline bool build_topology(Topology& tp, int N, const float* xyz, const int* typ
             }
         }
     }
+    if (!fragatoms.empty()) std::memcpy(tp.blob.data() + h.off_fragatoms, fragatoms.data(), fragatoms.size() * sizeof(uint16_t));
     if (!recs.empty()) std::memcpy(tp.blob.data() + h.off_pairs, recs.data(), recs.size() * sizeof(PairRec));
     return true;
 }

@@ -64,12 +64,13 @@ def test_integer_structure_bit_exact_vs_oracle(B, W, orc, name, request):
 
 
 def _parse_image(blob):
-    h = struct.unpack_from("16i", blob, 0)
+    h = struct.unpack_from("17i", blob, 0)
     keys = ["N", "R", "nfrag", "npairs", "nrounds", "T", "off_atoms", "off_meta", "off_frag", "off_fragidx", "off_pairs",
-            "bytes", "max_frag_atoms", "max_depth"]
+            "bytes", "max_frag_atoms", "max_depth", "npos", "off_fragatoms", "nfull"]
     H = dict(zip(keys, h))
-    atoms = np.frombuffer(blob, np.float32, 4 * H["N"], H["off_atoms"]).reshape(-1, 4)
-    meta = np.frombuffer(blob, np.uint32, H["N"], H["off_meta"])
+    atoms = np.frombuffer(blob, np.float32, 4 * H["npos"], H["off_atoms"]).reshape(-1, 4)
+    meta = np.frombuffer(blob, np.uint32, H["npos"], H["off_meta"])
+    H["fragatoms"] = np.frombuffer(blob, np.uint16, H["N"], H["off_fragatoms"]).astype(int)
     fg = np.frombuffer(blob, np.float32, 8 * H["nfrag"], H["off_frag"]).reshape(-1, 8)
     fi = np.frombuffer(blob, np.int32, 4 * H["nfrag"], H["off_fragidx"]).reshape(-1, 4)
     pr = np.frombuffer(blob, np.uint32, 4 * 32 * H["nrounds"], H["off_pairs"]).reshape(-1, 32, 4)
@@ -84,18 +85,25 @@ def test_image_layout_and_conflict_free_schedule(B, W, orc, name, request):
     blob, int_of_ext = hl.image()
     H, atoms, meta, fg, fi, pr = _parse_image(blob)
     assert (H["N"], H["R"], H["nfrag"], H["npairs"], H["bytes"]) == (lig.N, lig.R, ol.nfrag, ol.npairs, len(blob))
-    assert sorted(int_of_ext.tolist()) == list(range(lig.N))
-    ext_of_int = np.argsort(int_of_ext)
-    # atoms: coordinates relative to the pivot, charge, type, fragment-contiguous numbering
+    npos = H["npos"]
+    assert npos == 32 * ((lig.N + 31) // 32) and len(set(int_of_ext.tolist())) == lig.N and int_of_ext.max() < npos
+    ext_of_int = np.full(npos, -1)
+    ext_of_int[int_of_ext] = np.arange(lig.N)
+    holes = ext_of_int < 0
+    assert (meta[holes] == 0xFFFFFFFF).all() and (meta[~holes] != 0xFFFFFFFF).all()
+    occ = np.flatnonzero(~holes)
+    # atoms by position: coordinates relative to the pivot, charge, type, fragment id
     piv = hl.tree()["pivot"].astype(np.float64)
-    assert np.allclose(atoms[:, :3], lig.xyz[ext_of_int].astype(np.float64) - piv, atol=1e-6)
-    assert np.array_equal(atoms[:, 3], lig.charge[ext_of_int])
-    assert np.array_equal(meta & 0xFF, lig.type[ext_of_int].astype(np.uint32))
-    frag = (meta >> 8).astype(int)
-    assert (np.diff(frag) >= 0).all() and frag[0] == 0
+    assert np.allclose(atoms[occ, :3], lig.xyz[ext_of_int[occ]].astype(np.float64) - piv, atol=1e-6)
+    assert np.array_equal(atoms[occ, 3], lig.charge[ext_of_int[occ]])
+    assert np.array_equal(meta[occ] & 0xFF, lig.type[ext_of_int[occ]].astype(np.uint32))
+    frag = np.full(npos, -1)
+    frag[occ] = (meta[occ] >> 8).astype(int)
+    assert sorted(H["fragatoms"].tolist()) == sorted(occ.tolist())
     for f in range(H["nfrag"]):
         parent, a0, a1, w = fi[f]
-        assert (frag[a0:a1] == f).all() and (a1 - a0) == (frag == f).sum()
+        members = H["fragatoms"][a0:a1]
+        assert (frag[members] == f).all() and (a1 - a0) == (frag == f).sum()
         sub_end, tor = w & 0xFFFF, (w >> 16) & 0xFFFF
         assert f < sub_end <= H["nfrag"]
         if f == 0:
@@ -103,31 +111,37 @@ def test_image_layout_and_conflict_free_schedule(B, W, orc, name, request):
         else:
             assert 0 <= parent < f and tor < lig.R
             # the subtree's atoms are exactly the torsion's moved set (canonical numbering)
-            sub_atoms = ext_of_int[np.isin(frag, range(f, sub_end))]
+            sub_atoms = ext_of_int[np.flatnonzero(np.isin(frag, range(f, sub_end)))]
             assert sorted(sub_atoms.tolist()) == np.flatnonzero(ol.moved[tor]).tolist()
             a, b = ol.rot[tor]
             u = lig.xyz[b].astype(np.float64) - lig.xyz[a].astype(np.float64)
             assert np.allclose(fg[f, 4:7], u / np.linalg.norm(u), atol=1e-6)
             assert np.allclose(fg[f, 0:3], lig.xyz[a].astype(np.float64) - piv, atol=1e-6)
-    # schedule: a permutation of the canonical pair list, at most once per side per round
+    # schedule: a permutation of the canonical pair list, every atom at most once per side per round (hard rule);
+    # positions on one side distinct modulo 32 (soft rule, bank-conflict free) in nearly every round
     seen = []
+    wavefronts = []
     for r in range(H["nrounds"]):
         ij = pr[r, :, 0]
-        valid = ((ij >> 17) & 1).astype(bool)
-        i, j = (ij & 0xFF)[valid].astype(int), ((ij >> 8) & 0xFF)[valid].astype(int)
+        valid = ((ij >> 23) & 1).astype(bool)
+        si, sj = (ij & 0x7FF)[valid].astype(int), ((ij >> 11) & 0x7FF)[valid].astype(int)     # slot = (a>>5)*256 + (a&31)
+        i, j = (si >> 8) * 32 + (si & 31), (sj >> 8) * 32 + (sj & 31)
+        assert ((si & 255) < 32).all() and ((sj & 255) < 32).all() and (ext_of_int[i] >= 0).all() and (ext_of_int[j] >= 0).all()
         assert len(set(i.tolist())) == len(i) and len(set(j.tolist())) == len(j)
-        assert (pr[r, ~valid] == 0).all()
+        wavefronts += [np.bincount(i & 31).max(), np.bincount(j & 31).max()]      # replays of one 4-byte access
+        assert (pr[r, ~valid] == 0).all() and (valid.all() == (r < H["nfull"]))
         for a, b, rec in zip(i, j, pr[r, valid]):
             ea, eb = int(ext_of_int[a]), int(ext_of_int[b])
             seen.append((min(ea, eb), max(ea, eb)))
             c12, cA = np.frombuffer(rec[1:3].tobytes(), np.float32)
             co = lig.pair_coeffs[lig.type[ea], lig.type[eb]]
-            assert (c12, cA) == (co[0], co[1]) and int((rec[0] >> 16) & 1) == int(co[2] > 8)
+            assert (c12, cA) == (co[0], co[1]) and int((rec[0] >> 22) & 1) == int(co[2] > 8)
     assert sorted(seen) == [tuple(p) for p in ol.pairs.tolist()]
     # packing efficiency against the lower bound max(ceil(np/32), ceil(max degree / 2))
     deg = np.bincount(ol.pairs.ravel(), minlength=lig.N).max()
     lower = max(int(np.ceil(ol.npairs / 32)), int(np.ceil(deg / 2)))
     assert H["nrounds"] <= int(np.ceil(1.3 * lower)) + 1, (H["nrounds"], lower)
+    assert np.mean(wavefronts) <= 2.0 and max(wavefronts) <= 3, (np.mean(wavefronts), max(wavefronts))
 
 
 def test_load_ligand_rejects_bad_input(B, W):
