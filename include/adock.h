@@ -110,9 +110,12 @@ int adock_score_batch_host(const adock_grids* grids, const adock_ligand* ligand,
                            float* h_gradients, int dstride, void* cuda_stream);
 
 /* ADADELTA local search (R7) from each of n starting genotypes: d_genotypes device [n][gstride] in/out
- * (best genotype seen), d_energies device [n] out (its energy), d_iters device [n] out (evals used) or NULL. */
+ * (best genotype seen), d_energies device [n] out (its energy), d_iters device [n] out (evals used) or NULL,
+ * d_trace device [n][params->lsit] out or NULL: the energy evaluated at iteration k (x_k before its step;
+ * entries past the iterations performed are left untouched). */
 int adock_local_search(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
-                       float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, void* cuda_stream);
+                       float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, float* d_trace,
+                       void* cuda_stream);
 
 /* Philox4x32-10 (R8): out[i] = philox(key, ctr[i]); key host uint32[2], d_ctr/d_out device uint32 [n][4]. */
 int adock_philox(const unsigned int key[2], const unsigned int* d_ctr, int n, unsigned int* d_out, void* cuda_stream);

@@ -60,7 +60,7 @@ def lib():
         L.adock_ligand_image.argtypes = [vp, C.POINTER(ci), C.POINTER(vp), C.POINTER(vp)]
         L.adock_score_batch.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, ci, vp]
         L.adock_score_batch_host.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, ci, vp]
-        L.adock_local_search.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp]
+        L.adock_local_search.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, vp]
         L.adock_philox.argtypes = [vp, vp, ci, vp, vp]
         L.adock_ga_generation.argtypes = [vp, vp, pp, ci, ci, ci, C.c_ulonglong, vp, vp, vp, vp, vp, C.POINTER(ci), vp]
         L.adock_dock.argtypes = [vp, vp, pp, ci, ci, C.c_longlong, C.c_ulonglong, vp, vp, vp, vp, vp, vp]
@@ -201,10 +201,12 @@ def adock_score_batch_host(grids: Grids, lig: Ligand, params, h_genotypes, want_
     return dict(E=E, terms=terms, grad=grad)
 
 
-def adock_local_search(grids: Grids, lig: Ligand, params, d_genotypes, d_energies, d_iters=None):
+def adock_local_search(grids: Grids, lig: Ligand, params, d_genotypes, d_energies, d_iters=None, d_trace=None):
     n, gs = d_genotypes.shape
+    if d_trace is not None:
+        assert tuple(d_trace.shape) == (n, params.lsit)
     _check(lib().adock_local_search(grids.h, lig.h, C.byref(params) if params is not None else None, _dp(d_genotypes), n, gs,
-                                    _dp(d_energies), _dp(d_iters), _stream()))
+                                    _dp(d_energies), _dp(d_iters), _dp(d_trace), _stream()))
 
 
 def adock_philox(key, d_ctr, d_out):

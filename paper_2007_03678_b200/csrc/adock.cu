@@ -383,6 +383,7 @@ struct LsArgs {
     float* genos;
     float* E;
     int* iters;
+    float* trace;
     int blob_bytes, n, gstride;
 };
 
@@ -399,7 +400,8 @@ __global__ void __launch_bounds__(128) ls_array_kernel(GridDev G, ParDev P, LsAr
     for (int d = lane; d < Gn; d += 32) S.geno[d] = a.genos[(size_t)idx * a.gstride + d];
     __syncwarp();
     int iters = 0;
-    const float e = adadelta_search(L, G, P, S, lane, __int_as_float(0x7fc00000), iters);
+    const float e = adadelta_search(L, G, P, S, lane, __int_as_float(0x7fc00000), iters,
+                                    a.trace ? a.trace + (size_t)idx * P.lsit : nullptr);
     for (int d = lane; d < Gn; d += 32) a.genos[(size_t)idx * a.gstride + d] = S.best[d];
     if (lane == 0) {
         a.E[idx] = e;
@@ -408,7 +410,8 @@ __global__ void __launch_bounds__(128) ls_array_kernel(GridDev G, ParDev P, LsAr
 }
 
 extern "C" int adock_local_search(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
-                                  float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, void* cuda_stream) {
+                                  float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, float* d_trace,
+                                  void* cuda_stream) {
     if (!grids || !ligand) return fail(ADOCK_EINVAL, "NULL handle");
     if (n < 0) return fail(ADOCK_EINVAL, "n < 0");
     if (n == 0) return ADOCK_OK;
@@ -424,7 +427,7 @@ extern "C" int adock_local_search(const adock_grids* grids, const adock_ligand* 
     CUDA_TRY(cudaFuncSetAttribute(ls_array_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ParDev P = make_pardev(p);
     P.k_wall_h = p.k_wall * grids->dev.h;
-    LsArgs a{ligand->d_blob, d_genotypes, d_energies, d_iters, ligand->blob_bytes, n, gstride};
+    LsArgs a{ligand->d_blob, d_genotypes, d_energies, d_iters, d_trace, ligand->blob_bytes, n, gstride};
     ls_array_kernel<<<(n + W - 1) / W, W * 32, smem, (cudaStream_t)cuda_stream>>>(grids->dev, P, a);
     ++g_launches;
     CUDA_TRY(cudaGetLastError());

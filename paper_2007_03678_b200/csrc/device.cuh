@@ -492,7 +492,7 @@ __device__ inline void ga_make_child(const ParDev& P, int Pn, int R, unsigned lo
 // Start genotype in S.geno; on return S.best holds the best genotype seen and the function returns its
 // energy (the carried energy e_start if no finite evaluation happened).  iters = evaluations performed.
 __device__ inline float adadelta_search(const LigS& L, const GridDev& G, const ParDev& P, const WarpS& S, int lane,
-                                        float e_start, int& iters) {
+                                        float e_start, int& iters, float* trace = nullptr) {
     const int R = L.R, D = 6 + R, Gn = 7 + R;
     float Eg2[3] = {0.f, 0.f, 0.f}, Ed2[3] = {0.f, 0.f, 0.f};         // component d = lane + 32*c  (D <= 70)
     float bestE = __int_as_float(0x7f800000);
@@ -502,6 +502,7 @@ __device__ inline float adadelta_search(const LigS& L, const GridDev& G, const P
     while (it < P.lsit) {
         float ei, ea;
         const float e = eval_pose<true>(L, G, P, S, lane, ei, ea);
+        if (trace && lane == 0) trace[it] = e;
         ++it;
         bool ok = isfinite(e);
 #pragma unroll

@@ -120,7 +120,8 @@ def test_score_parity(B, orc, W, cases, dev, name, n):
     assert_energy(terms[:, 0], ref["terms"][:, 0], name + " inter")
     assert_energy(terms[:, 1], ref["terms"][:, 1], name + " intra")
     ok = (ref["margins"][:, 0] > 1e-3) & (ref["margins"][:, 1] > 1e-3)
-    assert ok.mean() > 0.5
+    # an atom lies within 1e-3 of a cell face on some axis with probability ~6e-3: exp(-6e-3 N) of the poses stay
+    assert ok.mean() > 0.6 * math.exp(-6e-3 * c.lig.N)
     w = assert_gradient(gr, ref, c.lig.R, ok, name)
     print(f"{name}: worst gradient error / tolerance = {w:.3f}")
     # energy-only launch gives the same energies
@@ -303,22 +304,55 @@ def test_ga_decisions_bit_exact_and_children_match(B, orc, cases, dev):
 
 # ------------------------------------------------------------------------------- ADADELTA (row a5)
 def test_local_search_first_iterations_track_oracle(B, orc, W, cases, dev):
+    """Per-iteration energies E(x_k) of the ADADELTA chain (d_trace) against the oracle's trace.  Starts are
+    relaxed poses (the oracle's own 300-iteration search from random genotypes, then a small seeded kick):
+    random starts sit in 1e6..1e9 kcal/mol clashes where the fp32 cancellation floor of the gradient
+    (1e-5 * scales) exceeds whole gradient components and the two precisions legitimately part at step 1.
+    The chain amplifies rounding differences ~2x per iteration (measured), so the bar is statistical:
+    a wrong decay, epsilon or update order moves E(x_1) by O(0.1..1) relative (rho 0.9 instead of 0.8: 0.45 median)."""
+    c300 = cases("drug")
     c = cases("drug", lsit=4)
-    G = W.make_genotypes(256, c.lig.R, c.grids, seed=21, wall_tail=0.0)
-    d_g = torch.from_numpy(G).to(dev)
-    d_E = torch.zeros(256, device=dev)
-    d_it = torch.zeros(256, dtype=torch.int32, device=dev)
-    B.adock_local_search(c.gg, c.gl, c.gp, d_g, d_E, d_it)
+    n = 192
+    G0 = W.make_genotypes(n, c.lig.R, c.grids, seed=21, wall_tail=0.0)
+    rng = np.random.default_rng(5)
+    S = np.zeros_like(G0)
+    for i in range(n):
+        g = orc.adadelta(c300.og, c300.ol, c300.op, G0[i].astype(np.float64))[0].copy()
+        g[0:3] += rng.normal(0, 0.05, 3)
+        g[7:] += rng.normal(0, 0.05, c.lig.R)
+        S[i] = g
+    ref = orc.score(c.og, c.ol, c.op, S)
+    sel = np.flatnonzero((ref["scales"].max(1) <= 2e4) & (ref["margins"][:, 0] > 1e-3) & (ref["margins"][:, 1] > 1e-3))
+    assert len(sel) >= 64
+    d_g = torch.from_numpy(S).to(dev)
+    d_E = torch.zeros(n, device=dev)
+    d_it = torch.zeros(n, dtype=torch.int32, device=dev)
+    d_tr = torch.full((n, 4), float("nan"), device=dev)
+    B.adock_local_search(c.gg, c.gl, c.gp, d_g, d_E, d_it, d_tr)
     torch.cuda.synchronize()
     assert (d_it.cpu().numpy() == 4).all()
-    gE, gG = d_E.cpu().numpy(), d_g.cpu().numpy()
-    close = 0
-    for i in range(256):
-        og, oE, it = orc.adadelta(c.og, c.ol, c.op, G[i].astype(np.float64))
+    T = d_tr.cpu().numpy().astype(np.float64)
+    gE, gG = d_E.cpu().numpy().astype(np.float64), d_g.cpu().numpy().astype(np.float64)
+    O, oG, oE = [], [], []
+    for i in range(n):
+        g, e, it, tE, _ = orc.adadelta(c.og, c.ol, c.op, S[i].astype(np.float64), trace=True)
         assert it == 4
-        if abs(gE[i] - oE) <= max(1e-4 * abs(oE), 1e-3) and np.abs(gG[i] - og).max() < 1e-3:
-            close += 1
-    assert close >= 250          # a few starts sit on a cell face, where the two precisions take different cells
+        O.append(tE); oG.append(g); oE.append(e)
+    O, oG, oE = np.array(O), np.array(oG), np.array(oE)
+    assert_energy(T[:, 0].astype(np.float32), O[:, 0], "trace k=0")            # E(x_0): plain scoring parity, every start
+    rel = np.abs(T - O) / np.maximum(np.abs(O), 1.0)
+    for k in (1, 2, 3):
+        r = rel[sel, k]
+        assert np.median(r) < 5e-5 and (r < 1e-3).mean() >= 0.9, (k, np.median(r), (r < 1e-3).mean())
+    # the returned (best genotype, energy) is the arg-min of the trace: identical wherever the traces agree
+    agree = sel[(rel[sel] < 1e-4).all(1)]
+    assert len(agree) >= len(sel) // 2
+    same_k = T[agree].argmin(1) == O[agree].argmin(1)
+    assert same_k.mean() > 0.95
+    a = agree[same_k]
+    assert np.allclose(gE[a], T[a].min(1), rtol=0, atol=0)
+    assert_energy(gE[a].astype(np.float32), oE[a], "LS best energy")
+    assert np.abs(gG[a] - oG[a]).max() < 2e-3
 
 
 def test_local_search_statistics_match_oracle(B, orc, W, cases, dev):
