@@ -18,7 +18,8 @@ _lib = None
 ADOCK_OK, ADOCK_EINVAL, ADOCK_ENOMEM, ADOCK_ECUDA, ADOCK_ELIMIT = 0, -1, -2, -3, -4
 EXPORTS = ["adock_default_params", "adock_load_grids", "adock_free_grids", "adock_load_ligand", "adock_free_ligand",
            "adock_ligand_pairs", "adock_ligand_tree", "adock_ligand_image", "adock_score_batch", "adock_score_batch_host", "adock_local_search",
-           "adock_philox", "adock_ga_generation", "adock_dock", "adock_dock_many", "adock_launch_count", "adock_last_error", "adock_profile", "adock_profile_read"]
+           "adock_philox", "adock_ga_generation", "adock_dock", "adock_dock_many", "adock_launch_count", "adock_last_error", "adock_profile", "adock_profile_read",
+           "adock_ligand_lane_image", "adock_set_path"]
 
 
 class AdockError(RuntimeError):
@@ -58,6 +59,8 @@ def lib():
         L.adock_ligand_pairs.argtypes = [vp, C.POINTER(ci), C.POINTER(vp)]
         L.adock_ligand_tree.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.adock_ligand_image.argtypes = [vp, C.POINTER(ci), C.POINTER(vp), C.POINTER(vp)]
+        L.adock_ligand_lane_image.argtypes = [vp, C.POINTER(ci), C.POINTER(vp), C.POINTER(vp)]
+        L.adock_set_path.argtypes = [ci]
         L.adock_score_batch.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, ci, vp]
         L.adock_score_batch_host.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, ci, vp]
         L.adock_local_search.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, vp]
@@ -175,6 +178,13 @@ class Ligand:
         blob = bytes(np.ctypeslib.as_array(C.cast(p, C.POINTER(C.c_ubyte)), (n.value,)))
         return blob, np.ctypeslib.as_array(C.cast(m, C.POINTER(C.c_int)), (self.N,)).copy()
 
+    def lane_image(self):
+        """(host copy of the lane-per-individual image as bytes, pos_of_ext [N])"""
+        n, p, m = C.c_int(), C.c_void_p(), C.c_void_p()
+        _check(lib().adock_ligand_lane_image(self.h, C.byref(n), C.byref(p), C.byref(m)))
+        blob = bytes(np.ctypeslib.as_array(C.cast(p, C.POINTER(C.c_ubyte)), (n.value,)))
+        return blob, np.ctypeslib.as_array(C.cast(m, C.POINTER(C.c_int)), (self.N,)).copy()
+
     def close(self):
         if getattr(self, "h", None) and _lib is not None:
             _lib.adock_free_ligand(self.h)
@@ -259,6 +269,14 @@ def adock_profile_read() -> dict:
     ms, n, ev = C.c_double(), C.c_longlong(), C.c_longlong()
     _check(lib().adock_profile_read(C.byref(ms), C.byref(n), C.byref(ev)))
     return dict(ls_ms=ms.value, ls_launches=n.value, ls_evals=ev.value)
+
+
+PATHS = {"auto": 0, "warp": 1, "lane": 2}
+
+
+def adock_set_path(path) -> None:
+    """kernel family: 'auto' (by problem size), 'warp' (warp per individual) or 'lane' (thread per individual)"""
+    _check(lib().adock_set_path(PATHS[path] if isinstance(path, str) else int(path)))
 
 
 def adock_launch_count(reset: bool = False) -> int:

@@ -8,7 +8,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libadock.so")
 SOURCES = ["adock.cu"]
-DEPS = ["adock.cu", "device.cuh", "topology.hpp", os.path.join("..", "..", "include", "adock.h")]
+DEPS = ["adock.cu", "device.cuh", "lane.cuh", "lane_image.hpp", "topology.hpp", os.path.join("..", "..", "include", "adock.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-ftz=true",
               "-Xcompiler", "-fPIC", "-shared"]
 

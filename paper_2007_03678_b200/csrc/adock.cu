@@ -11,6 +11,7 @@
 
 #include "../../include/adock.h"
 #include "device.cuh"
+#include "lane.cuh"
 
 using namespace adock;
 
@@ -27,11 +28,15 @@ struct adock_ligand {
     int* d_ext_of_int = nullptr;
     int blob_bytes = 0;
     int scratch_floats = 0;
-    float w_desolv = 0, qasp = 0;
+    float w_desolv = 0, qasp = 0, elec_scale = 0;
+    LaneImage lane;                         // image of the lane-per-individual kernels (lane_image.hpp)
+    unsigned char* d_lane = nullptr;
+    int lane_bytes = 0, lane_warp_floats = 0;
 };
 
 static thread_local std::string g_err;
 static thread_local long long g_launches = 0;
+static int g_path = 0;                                    // adock_set_path: 0 auto, 1 warp-per-individual, 2 lane-per-individual
 static thread_local bool g_prof = false;                  // adock_profile: time every dock_ls_kernel launch
 static thread_local double g_ls_ms = 0;
 static thread_local long long g_ls_launches = 0, g_ls_evals = 0;
@@ -99,8 +104,8 @@ static int check_params(const adock_params* in, const adock_ligand* l, adock_par
     if (!(out.ds_sigma > 0) || !(out.r_min > 0) || !(out.elec_scale >= 0) || out.lsit < 0 || out.max_gens < 0 || !(out.ad_eps > 0))
         return fail(ADOCK_EINVAL, "parameter out of range");
     if (l && !l->d_blob) return fail(ADOCK_EINVAL, "host-only ligand handle (loaded with grids == NULL)");
-    if (l && (out.w_desolv != l->w_desolv || out.qasp != l->qasp))
-        return fail(ADOCK_EINVAL, "w_desolv/qasp differ from the values baked into the ligand at load time");
+    if (l && (out.w_desolv != l->w_desolv || out.qasp != l->qasp || out.elec_scale != l->elec_scale))
+        return fail(ADOCK_EINVAL, "elec_scale/w_desolv/qasp differ from the values baked into the ligand at load time");
     return ADOCK_OK;
 }
 
@@ -186,7 +191,10 @@ extern "C" int adock_load_ligand(const adock_grids* grids, const adock_params* p
         delete l;
         return fail(ADOCK_EINVAL, msg);
     }
-    l->w_desolv = p.w_desolv; l->qasp = p.qasp;
+    l->w_desolv = p.w_desolv; l->qasp = p.qasp; l->elec_scale = p.elec_scale;
+    build_lane_image(l->lane, l->tp, xyz, type, charge, pair_coeffs, solpar, vol, p.w_desolv, p.qasp, p.elec_scale);
+    l->lane_bytes = (int)l->lane.blob.size();
+    l->lane_warp_floats = l->lane.warp_floats;
     l->blob_bytes = (int)l->tp.blob.size();
     l->scratch_floats = warp_scratch_floats(N, l->tp.nfrag, R);
     if (16 + l->blob_bytes + 4 * l->scratch_floats > 227 * 1024) {
@@ -199,10 +207,12 @@ extern "C" int adock_load_ligand(const adock_grids* grids, const adock_params* p
     }
     cudaError_t e = cudaMalloc(&l->d_blob, l->blob_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&l->d_ext_of_int, l->tp.ext_of_int.size() * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&l->d_lane, l->lane_bytes);
+    if (e == cudaSuccess) e = cudaMemcpy(l->d_lane, l->lane.blob.data(), l->lane_bytes, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(l->d_blob, l->tp.blob.data(), l->blob_bytes, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(l->d_ext_of_int, l->tp.ext_of_int.data(), l->tp.ext_of_int.size() * sizeof(int), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
-        cudaFree(l->d_blob); cudaFree(l->d_ext_of_int);
+        cudaFree(l->d_blob); cudaFree(l->d_ext_of_int); cudaFree(l->d_lane);
         delete l;
         return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("ligand upload: ") + cudaGetErrorString(e));
     }
@@ -214,6 +224,7 @@ extern "C" void adock_free_ligand(adock_ligand* l) {
     if (!l) return;
     cudaFree(l->d_blob);
     cudaFree(l->d_ext_of_int);
+    cudaFree(l->d_lane);
     delete l;
 }
 
@@ -239,6 +250,20 @@ extern "C" int adock_ligand_image(const adock_ligand* l, int* bytes, const unsig
     *bytes = l->blob_bytes;
     *image = l->tp.blob.data();
     if (int_of_ext) *int_of_ext = l->tp.int_of_ext.data();
+    return ADOCK_OK;
+}
+
+extern "C" int adock_ligand_lane_image(const adock_ligand* l, int* bytes, const unsigned char** image, const int** pos_of_ext) {
+    if (!l || !bytes || !image) return fail(ADOCK_EINVAL, "NULL argument");
+    *bytes = l->lane_bytes;
+    *image = l->lane.blob.data();
+    if (pos_of_ext) *pos_of_ext = l->lane.pos_of_ext.data();
+    return ADOCK_OK;
+}
+
+extern "C" int adock_set_path(int path) {
+    if (path < 0 || path > 2) return fail(ADOCK_EINVAL, "path must be 0 (auto), 1 (warp per individual) or 2 (lane per individual)");
+    g_path = path;
     return ADOCK_OK;
 }
 
@@ -294,10 +319,75 @@ __global__ void __launch_bounds__(256) score_kernel(GridDev G, ParDev P, ScoreAr
     }
 }
 
+
+// =================================================================== lane-per-individual geometry (lane.cuh)
+constexpr int kLaneMaxWarps = 8;
+static size_t lane_smem(int lane_bytes, int warp_floats, int warps) { return 16 + (size_t)lane_bytes + (size_t)warps * warp_floats * 128; }
+// largest warp count <= kLaneMaxWarps whose shared memory fits (0: not even one)
+static int lane_fit_warps(int lane_bytes, int warp_floats) {
+    int w = kLaneMaxWarps;
+    while (w > 0 && lane_smem(lane_bytes, warp_floats, w) > (size_t)g_smem_optin) --w;
+    return w;
+}
+// the lane kernels want at least one warp per scheduler
+static bool lane_ok(const adock_ligand* l) { return lane_fit_warps(l->lane_bytes, l->lane_warp_floats) >= 4; }
+
+template <bool GRAD>
+__global__ void __launch_bounds__(kLaneMaxWarps * 32, 1) score_lane_kernel(GridDev G, ParDev P, ScoreArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned char* blob = smem + 16;
+    stage_ligand(blob, a.blob, a.blob_bytes, reinterpret_cast<uint64_t*>(smem), 0);
+    const LaneL L = lane_view(blob);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
+    const int wf = reinterpret_cast<const LaneHeader*>(blob)->warp_floats;
+    const LaneS S = lane_scratch(reinterpret_cast<float*>(blob + a.blob_bytes) + (size_t)warp * wf * 32, L, lane);
+    const int Gn = 7 + L.R;
+    const int nchunks = (a.n + 31) >> 5;
+    for (int c = blockIdx.x * W + warp; c < nchunks; c += gridDim.x * W) {
+        const int idx = c * 32 + lane;
+        const bool act = idx < a.n;
+        const int src = act ? idx : a.n - 1;
+        for (int d = 0; d < Gn; ++d) S.geno[d * 32] = a.genos[(size_t)src * a.gstride + d];
+        float ei, ea;
+        bool gf;
+        const float e = lane_eval<GRAD>(L, G, P, S, GRAD ? a.grads + (size_t)src * a.dstride : nullptr, 1, act, ei, ea, gf);
+        if (act) {
+            a.E[idx] = e;
+            if (a.terms) { a.terms[2 * (size_t)idx] = ei; a.terms[2 * (size_t)idx + 1] = ea; }
+        }
+    }
+}
+
+static int launch_score_lane(const adock_grids* grids, const adock_ligand* lig, const adock_params& p, const float* d_genos, int n,
+                             int gstride, float* d_E, float* d_terms, float* d_grads, int dstride, cudaStream_t st) {
+    const int nchunks = (n + 31) / 32;
+    int W = lane_fit_warps(lig->lane_bytes, lig->lane_warp_floats);
+    if (!W) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
+    // few chunks: spread them over the SMs (one warp per scheduler first)
+    while (W > 1 && (long long)g_sm_count * W > (long long)nchunks * 2 && W > 4) W >>= 1;
+    const size_t smem = lane_smem(lig->lane_bytes, lig->lane_warp_floats, W);
+    ParDev P = make_pardev(p);
+    P.k_wall_h = p.k_wall * grids->dev.h;
+    ScoreArgs a{lig->d_lane, d_genos, d_E, d_terms, d_grads, lig->lane_bytes, n, gstride, dstride};
+    const int grid = (int)std::max<long long>(1, std::min<long long>(((long long)nchunks + W - 1) / W, g_sm_count));
+    if (d_grads) {
+        CUDA_TRY(cudaFuncSetAttribute(score_lane_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        score_lane_kernel<true><<<grid, W * 32, smem, st>>>(grids->dev, P, a);
+    } else {
+        CUDA_TRY(cudaFuncSetAttribute(score_lane_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        score_lane_kernel<false><<<grid, W * 32, smem, st>>>(grids->dev, P, a);
+    }
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    return ADOCK_OK;
+}
+
 static int launch_score(const adock_grids* grids, const adock_ligand* lig, const adock_params& p, const float* d_genos, int n,
                         int gstride, float* d_E, float* d_terms, float* d_grads, int dstride, cudaStream_t st) {
     int rc = device_props();
     if (rc) return rc;
+    if (g_path == 2 || (g_path == 0 && n >= 2048 && lane_ok(lig)))
+        return launch_score_lane(grids, lig, p, d_genos, n, gstride, d_E, d_terms, d_grads, dstride, st);
     const int W = fit_warps(lig->blob_bytes, lig->scratch_floats, 8);
     if (!W) return fail(ADOCK_ELIMIT, "ligand does not fit in shared memory");
     const size_t smem = cta_smem(lig->blob_bytes, lig->scratch_floats, W);

@@ -1,0 +1,411 @@
+// lane.cuh -- lane-per-individual device code of the hot path.
+// One THREAD evaluates one genotype: pose (R3), grid term (R4), intramolecular pairs (R5), back-propagation (R6)
+// and the ADADELTA chain (R7).  The 32 lanes of a warp hold 32 individuals of the SAME ligand, so the ligand image
+// (lane_image.hpp) is read from shared memory by broadcast, control flow is warp-uniform, and no shuffle, atomic or
+// cross-lane reduction is needed anywhere.  Per-thread state lives in shared memory as [index][lane] columns
+// (conflict-free): atom positions relative to the translation, and per-fragment (force, torque) accumulators.
+// The pair loop keeps an I-block of 4 atoms in registers and evaluates each active row against an aligned J-pair
+// with packed f32x2 arithmetic (FFMA2/FMUL2/FADD2: two pairs per instruction issue).
+#pragma once
+#include "device.cuh"
+#include "lane_image.hpp"
+
+namespace adock {
+
+// ---------------------------------------------------------------- packed f32x2
+struct f2 { unsigned long long v; };
+__device__ __forceinline__ f2 pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r.v) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ f2 bc(float x) { return pk(x, x); }
+__device__ __forceinline__ void unpk(f2 a, float& lo, float& hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.v)); }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
+__device__ __forceinline__ f2 sub2(f2 a, f2 b) { f2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d.v) : "l"(a.v), "l"(b.v), "l"(c.v)); return d; }
+__device__ __forceinline__ f2 neg2(f2 a) { f2 d; d.v = a.v ^ 0x8000000080000000ull; return d; }
+__device__ __forceinline__ float hsum(f2 a) { float l, h; unpk(a, l, h); return l + h; }
+__device__ __forceinline__ f2 ld2(const float2* p) { const float2 v = *p; return pk(v.x, v.y); }
+
+// ---------------------------------------------------------------- views
+struct LaneL {              // the staged image
+    const float4* atoms;    // [Npad] x0 - pivot, q
+    const int* types;       // [Npad] type, -1 = pad
+    const int4* fragi;      // LaneFrag as 3 x 16 bytes
+    const int4* blocks;
+    const uint2* tiles;
+    const float4* rows;
+    int N, Npad, R, nfrag, nblocks, own_floats;
+};
+__device__ inline LaneL lane_view(const unsigned char* blob) {
+    const LaneHeader* h = reinterpret_cast<const LaneHeader*>(blob);
+    LaneL L;
+    L.atoms = reinterpret_cast<const float4*>(blob + h->off_atoms);
+    L.types = reinterpret_cast<const int*>(blob + h->off_types);
+    L.fragi = reinterpret_cast<const int4*>(blob + h->off_frags);
+    L.blocks = reinterpret_cast<const int4*>(blob + h->off_blocks);
+    L.tiles = reinterpret_cast<const uint2*>(blob + h->off_tiles);
+    L.rows = reinterpret_cast<const float4*>(blob + h->off_rows);
+    L.N = h->N; L.Npad = h->Npad; L.R = h->R; L.nfrag = h->nfrag; L.nblocks = h->nblocks; L.own_floats = h->own_floats;
+    return L;
+}
+struct LaneS {              // this thread's columns of the warp's scratch; element k of an array sits at [k*32]
+    float2* X; float2* Y; float2* Z;    // [Npad/2]: positions RELATIVE TO t of atoms 2m (.x) and 2m+1 (.y)
+    float* own;             // [own_floats]: per fragment F(3), T(3) about t; during the pose: the transform stack
+    float* geno;            // [7+R]
+};
+__device__ inline LaneS lane_scratch(float* warp_base, const LaneL& L, int lane) {
+    LaneS S;
+    const int half = L.Npad / 2;
+    S.X = reinterpret_cast<float2*>(warp_base) + lane;
+    S.Y = S.X + half * 32;
+    S.Z = S.Y + half * 32;
+    S.own = warp_base + 3 * L.Npad * 32 + lane;
+    S.geno = S.own + L.own_floats * 32;
+    return S;
+}
+
+// ---------------------------------------------------------------- one packed row of the pair tile (R5)
+struct PairK {              // packed constants
+    f2 k1, dk, one, A, B, BlamB, k2, six, isig2;
+    float rmin2;
+};
+__device__ __forceinline__ PairK make_pairk(const ParDev& P) {
+    PairK K;
+    K.k1 = bc(P.mlamB_log2e); K.dk = bc(P.diel_k); K.one = bc(1.f); K.A = bc(P.diel_A); K.B = bc(P.diel_B);
+    K.BlamB = bc(P.BlamB); K.k2 = bc(P.mhalf_inv_sig2_log2e); K.six = bc(6.f); K.isig2 = bc(P.inv_sig2);
+    K.rmin2 = P.rmin2;
+    return K;
+}
+
+// Row atom i (broadcast to both halves) against J atoms (j0 | j1).  Accumulates the pair energies into e2, and
+// ns*d into BOTH gi (which therefore holds MINUS the gradient on i) and gj (the gradient on j), ns = -(dE/dr)/r.
+template <bool GRAD>
+__device__ __forceinline__ void pair_row(const PairK& K, f2 xi, f2 yi, f2 zi, f2 xj, f2 yj, f2 zj, float4 ra, float4 rb,
+                                         unsigned hb, f2& e2, f2& gix, f2& giy, f2& giz, f2& gjx, f2& gjy, f2& gjz) {
+    const f2 dx = sub2(xi, xj), dy = sub2(yi, yj), dz = sub2(zi, zj);
+    const f2 r2 = fma2(dx, dx, fma2(dy, dy, mul2(dz, dz)));
+    float r2l, r2h;
+    unpk(r2, r2l, r2h);
+    const float cl = fmaxf(r2l, K.rmin2), ch = fmaxf(r2h, K.rmin2);
+    const f2 r2c = pk(cl, ch);
+    const f2 rinv = pk(frsqrt(cl), frsqrt(ch));
+    const f2 rr = mul2(r2c, rinv);
+    const f2 rinv2 = mul2(rinv, rinv);
+    const f2 rinv4 = mul2(rinv2, rinv2);
+    const f2 r6 = mul2(rinv4, rinv2);
+    const f2 c12 = pk(ra.x, ra.y), ncA = pk(ra.z, ra.w), ds = pk(rb.x, rb.y), qq = pk(rb.z, rb.w);
+    const f2 u12 = mul2(mul2(c12, r6), r6);
+    f2 rA = r6;
+    if (hb) {                                   // 12-10 slot(s): warp-uniform branch, rare
+        float a, b, l, h;
+        unpk(mul2(r6, rinv4), a, b);
+        unpk(r6, l, h);
+        rA = pk((hb & 1u) ? a : l, (hb & 2u) ? b : h);
+    }
+    const f2 nuA = mul2(ncA, rA);               // -cA r^-A
+    const f2 evdw = add2(u12, nuA);
+    // electrostatics with the distance-dependent dielectric: eps = A + B/den, den = 1 + k exp(-lambda B r)
+    float tl, th;
+    unpk(mul2(rr, K.k1), tl, th);
+    const f2 kex = mul2(K.dk, pk(fex2(tl), fex2(th)));
+    const f2 den = add2(kex, K.one);
+    const f2 num = fma2(K.A, den, K.B);          // eps = num/den
+    unpk(mul2(den, num), tl, th);
+    const f2 inv = pk(frcp(tl), frcp(th));       // 1/(den num)
+    const f2 ieps = mul2(mul2(den, den), inv);   // 1/eps
+    const f2 eel = mul2(mul2(qq, rinv), ieps);
+    // desolvation
+    unpk(mul2(r2c, K.k2), tl, th);
+    const f2 egs = mul2(ds, pk(fex2(tl), fex2(th)));
+    e2 = add2(e2, add2(evdw, add2(eel, egs)));
+    if (GRAD) {
+        // -dE/dr = rinv (12 u12 - nA uA + eel) + eel (deps/dr)/eps + (r/sigma^2) egs
+        const f2 s = add2(evdw, u12);
+        f2 A1 = fma2(K.six, s, eel);
+        if (hb) A1 = fma2(pk((hb & 1u) ? 4.f : 0.f, (hb & 2u) ? 4.f : 0.f), nuA, A1);
+        const f2 dee = mul2(mul2(K.BlamB, kex), inv);
+        const f2 A3 = fma2(eel, dee, mul2(A1, rinv));
+        const f2 A4 = fma2(K.isig2, mul2(rr, egs), A3);
+        float nl, nh;
+        unpk(mul2(A4, rinv), nl, nh);
+        const f2 ns = pk(r2l >= K.rmin2 ? nl : 0.f, r2h >= K.rmin2 ? nh : 0.f);
+        gix = fma2(ns, dx, gix); giy = fma2(ns, dy, giy); giz = fma2(ns, dz, giz);
+        gjx = fma2(ns, dx, gjx); gjy = fma2(ns, dy, gjy); gjz = fma2(ns, dz, gjz);
+    }
+}
+
+// own[f] += (F, T)
+__device__ __forceinline__ void own_add(float* own, int f, float Fx, float Fy, float Fz, float Tx, float Ty, float Tz) {
+    float* o = own + f * 6 * 32;
+    o[0] += Fx; o[32] += Fy; o[64] += Fz; o[96] += Tx; o[128] += Ty; o[160] += Tz;
+}
+
+// ---------------------------------------------------------------- full evaluation of this thread's genotype
+// Reads S.geno.  GRAD: writes grad[d*gs] for d < 6+R when `wr`, and clears `gfin` if a component is not finite.
+// Returns the total energy (NaN for |q| < 1e-12, with NaN gradient).  Every lane of the warp must call.
+template <bool GRAD>
+__device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, const ParDev& P, const LaneS& S, float* grad, int gs,
+                                           bool wr, float& e_inter, float& e_intra, bool& gfin) {
+    const float tx = S.geno[0], ty = S.geno[32], tz = S.geno[64];
+    float qw = S.geno[96], qx = S.geno[128], qy = S.geno[160], qz = S.geno[192];
+    const float qn2 = qw * qw + qx * qx + qy * qy + qz * qz;
+    const bool badq = !(qn2 >= 1e-24f);
+    if (badq) { qw = 1.f; qx = qy = qz = 0.f; }
+    const float qi = badq ? 1.f : 1.0f / sqrtf(qn2);
+    qw *= qi; qx *= qi; qy *= qi; qz *= qi;
+    float* Xf = reinterpret_cast<float*>(S.X);
+    float* Yf = reinterpret_cast<float*>(S.Y);
+    float* Zf = reinterpret_cast<float*>(S.Z);
+
+    // (a1) pose: per-fragment transform = parent's o rotation about the reference-frame axis; positions relative to t
+    {
+        float m00 = 1.f - 2.f * (qy * qy + qz * qz), m01 = 2.f * (qx * qy - qw * qz), m02 = 2.f * (qx * qz + qw * qy);
+        float m10 = 2.f * (qx * qy + qw * qz), m11 = 1.f - 2.f * (qx * qx + qz * qz), m12 = 2.f * (qy * qz - qw * qx);
+        float m20 = 2.f * (qx * qz - qw * qy), m21 = 2.f * (qy * qz + qw * qx), m22 = 1.f - 2.f * (qx * qx + qy * qy);
+        float m03 = 0.f, m13 = 0.f, m23 = 0.f;
+        for (int f = 0; f < L.nfrag; ++f) {
+            const int4 fi = L.fragi[3 * f];             // parent, depth|kids<<16, abeg, aend
+            const int depth = fi.y & 0xffff;
+            if (f > 0) {
+                const int4 fa = L.fragi[3 * f + 1], fb = L.fragi[3 * f + 2];
+                const float p0x = __int_as_float(fa.x), p0y = __int_as_float(fa.y), p0z = __int_as_float(fa.z);
+                const float ux = __int_as_float(fb.x), uy = __int_as_float(fb.y), uz = __int_as_float(fb.z);
+                const float* st = S.own + (depth - 1) * 12 * 32;
+                const float b00 = st[0], b01 = st[32], b02 = st[64], b03 = st[96];
+                const float b10 = st[128], b11 = st[160], b12 = st[192], b13 = st[224];
+                const float b20 = st[256], b21 = st[288], b22 = st[320], b23 = st[352];
+                float s, c;
+                sincosf(S.geno[(7 + fa.w) * 32], &s, &c);
+                const float k = 1.f - c;
+                const float a00 = fmaf(k * ux, ux, c), a01 = fmaf(k * ux, uy, -s * uz), a02 = fmaf(k * ux, uz, s * uy);
+                const float a10 = fmaf(k * ux, uy, s * uz), a11 = fmaf(k * uy, uy, c), a12 = fmaf(k * uy, uz, -s * ux);
+                const float a20 = fmaf(k * ux, uz, -s * uy), a21 = fmaf(k * uy, uz, s * ux), a22 = fmaf(k * uz, uz, c);
+                // x = B (A (y - p0) + p0) + b3  =>  M = B A,  m3 = B (p0 - A p0) + b3
+                const float wx = p0x - (a00 * p0x + a01 * p0y + a02 * p0z), wy = p0y - (a10 * p0x + a11 * p0y + a12 * p0z),
+                            wz = p0z - (a20 * p0x + a21 * p0y + a22 * p0z);
+                m00 = b00 * a00 + b01 * a10 + b02 * a20; m01 = b00 * a01 + b01 * a11 + b02 * a21; m02 = b00 * a02 + b01 * a12 + b02 * a22;
+                m10 = b10 * a00 + b11 * a10 + b12 * a20; m11 = b10 * a01 + b11 * a11 + b12 * a21; m12 = b10 * a02 + b11 * a12 + b12 * a22;
+                m20 = b20 * a00 + b21 * a10 + b22 * a20; m21 = b20 * a01 + b21 * a11 + b22 * a21; m22 = b20 * a02 + b21 * a12 + b22 * a22;
+                m03 = b00 * wx + b01 * wy + b02 * wz + b03;
+                m13 = b10 * wx + b11 * wy + b12 * wz + b13;
+                m23 = b20 * wx + b21 * wy + b22 * wz + b23;
+            }
+            if (fi.y >> 16) {                           // has children: push
+                float* st = S.own + depth * 12 * 32;
+                st[0] = m00; st[32] = m01; st[64] = m02; st[96] = m03;
+                st[128] = m10; st[160] = m11; st[192] = m12; st[224] = m13;
+                st[256] = m20; st[288] = m21; st[320] = m22; st[352] = m23;
+            }
+            for (int i = fi.z; i < fi.w; ++i) {
+                const float4 a = L.atoms[i];
+                const int o = (i >> 1) * 64 + (i & 1);
+                Xf[o] = fmaf(m00, a.x, fmaf(m01, a.y, fmaf(m02, a.z, m03)));
+                Yf[o] = fmaf(m10, a.x, fmaf(m11, a.y, fmaf(m12, a.z, m13)));
+                Zf[o] = fmaf(m20, a.x, fmaf(m21, a.y, fmaf(m22, a.z, m23)));
+            }
+        }
+        for (int i = L.N; i < L.Npad; ++i) {            // pad atoms: finite, in no pair
+            const int o = (i >> 1) * 64 + (i & 1);
+            Xf[o] = 0.f; Yf[o] = 0.f; Zf[o] = 0.f;
+        }
+    }
+
+    // (a2) grid term, two atoms per step (eight independent sector loads in flight); the gradient goes straight into
+    // the (force, torque about t) sums of the atom's fragment, which initialises own[]
+    float eg = 0.f;
+    {
+        float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
+        int cur = 0;
+        for (int m = 0; m < L.Npad / 2; ++m) {
+            const int t0 = L.types[2 * m], t1 = L.types[2 * m + 1];       // type | frag << 8 ; -1 = pad
+            if (t0 < 0) break;
+            const float2 xr = S.X[m * 32], yr = S.Y[m * 32], zr = S.Z[m * 32];
+            const float q0 = L.atoms[2 * m].w, q1 = L.atoms[2 * m + 1].w;
+            float g0x = 0, g0y = 0, g0z = 0, g1x = 0, g1y = 0, g1z = 0;
+            eg += grid_atom<GRAD>(G, P, t0 & 0xff, q0, xr.x + tx, yr.x + ty, zr.x + tz, g0x, g0y, g0z);
+            if (t1 >= 0) eg += grid_atom<GRAD>(G, P, t1 & 0xff, q1, xr.y + tx, yr.y + ty, zr.y + tz, g1x, g1y, g1z);
+            if (GRAD) {
+                const int f0 = t0 >> 8, f1 = t1 >= 0 ? t1 >> 8 : f0;
+                if (f0 != cur) {
+                    float* o = S.own + cur * 6 * 32;
+                    o[0] = Fx; o[32] = Fy; o[64] = Fz; o[96] = Tx; o[128] = Ty; o[160] = Tz;
+                    Fx = Fy = Fz = Tx = Ty = Tz = 0.f; cur = f0;
+                }
+                Fx += g0x; Fy += g0y; Fz += g0z;
+                Tx += yr.x * g0z - zr.x * g0y; Ty += zr.x * g0x - xr.x * g0z; Tz += xr.x * g0y - yr.x * g0x;
+                if (f1 != cur) {
+                    float* o = S.own + cur * 6 * 32;
+                    o[0] = Fx; o[32] = Fy; o[64] = Fz; o[96] = Tx; o[128] = Ty; o[160] = Tz;
+                    Fx = Fy = Fz = Tx = Ty = Tz = 0.f; cur = f1;
+                }
+                Fx += g1x; Fy += g1y; Fz += g1z;
+                Tx += yr.y * g1z - zr.y * g1y; Ty += zr.y * g1x - xr.y * g1z; Tz += xr.y * g1y - yr.y * g1x;
+            }
+        }
+        if (GRAD) {
+            float* o = S.own + cur * 6 * 32;
+            o[0] = Fx; o[32] = Fy; o[64] = Fz; o[96] = Tx; o[128] = Ty; o[160] = Tz;
+        }
+    }
+
+    // (a3) intramolecular pairs: register tiles
+    f2 e2 = bc(0.f);
+    {
+        const PairK K = make_pairk(P);
+        const float4* rowp = L.rows;
+        const f2 zero = bc(0.f);
+        for (int kb = 0; kb < L.nblocks; ++kb) {
+            const int4 blk = L.blocks[kb];              // b, tile_begin, tile_end, frags
+            const float2 xa = S.X[(2 * blk.x) * 32], xb = S.X[(2 * blk.x + 1) * 32];
+            const float2 ya = S.Y[(2 * blk.x) * 32], yb = S.Y[(2 * blk.x + 1) * 32];
+            const float2 za = S.Z[(2 * blk.x) * 32], zb = S.Z[(2 * blk.x + 1) * 32];
+            const float xi[4] = {xa.x, xa.y, xb.x, xb.y}, yi[4] = {ya.x, ya.y, yb.x, yb.y}, zi[4] = {za.x, za.y, zb.x, zb.y};
+            f2 gix[4], giy[4], giz[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) gix[r] = giy[r] = giz[r] = zero;
+            for (int t = blk.y; t < blk.z; ++t) {
+                const uint2 tw = L.tiles[t];
+                const int jp = tw.x & 0xff;
+                const f2 xj = ld2(S.X + jp * 32), yj = ld2(S.Y + jp * 32), zj = ld2(S.Z + jp * 32);
+                f2 gjx = zero, gjy = zero, gjz = zero;
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    if (tw.x & (0x100u << r)) {
+                        const float4 ra = rowp[0], rb = rowp[1];
+                        rowp += 2;
+                        pair_row<GRAD>(K, bc(xi[r]), bc(yi[r]), bc(zi[r]), xj, yj, zj, ra, rb, (tw.y >> (2 * r)) & 3u, e2,
+                                       gix[r], giy[r], giz[r], gjx, gjy, gjz);
+                    }
+                }
+                if (GRAD) {                             // J side: gradient gj at rel (xj,yj,zj) -> fragment sums
+                    const f2 tqx = fma2(yj, gjz, neg2(mul2(zj, gjy)));
+                    const f2 tqy = fma2(zj, gjx, neg2(mul2(xj, gjz)));
+                    const f2 tqz = fma2(xj, gjy, neg2(mul2(yj, gjx)));
+                    const int f0 = (tw.y >> 16) & 0xff, f1 = tw.y >> 24;
+                    if (f0 == f1) {
+                        own_add(S.own, f0, hsum(gjx), hsum(gjy), hsum(gjz), hsum(tqx), hsum(tqy), hsum(tqz));
+                    } else {
+                        float ax, bx, ay, by, az, bz, cx, dx, cy, dy, cz, dz;
+                        unpk(gjx, ax, bx); unpk(gjy, ay, by); unpk(gjz, az, bz);
+                        unpk(tqx, cx, dx); unpk(tqy, cy, dy); unpk(tqz, cz, dz);
+                        own_add(S.own, f0, ax, ay, az, cx, cy, cz);
+                        own_add(S.own, f1, bx, by, bz, dx, dy, dz);
+                    }
+                }
+            }
+            if (GRAD) {                                 // I side: gi holds MINUS the gradient
+                float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const float gx = -hsum(gix[r]), gy = -hsum(giy[r]), gz = -hsum(giz[r]);
+                    Fx += gx; Fy += gy; Fz += gz;
+                    Tx += yi[r] * gz - zi[r] * gy; Ty += zi[r] * gx - xi[r] * gz; Tz += xi[r] * gy - yi[r] * gx;
+                    const int fr = (blk.w >> (8 * r)) & 0xff;
+                    if (r == 3 || fr != (int)((blk.w >> (8 * (r + 1))) & 0xff)) {
+                        own_add(S.own, fr, Fx, Fy, Fz, Tx, Ty, Tz);
+                        Fx = Fy = Fz = Tx = Ty = Tz = 0.f;
+                    }
+                }
+            }
+        }
+    }
+    e_inter = eg;
+    e_intra = hsum(e2);
+    float e = eg + e_intra;
+    const float qnan = __int_as_float(0x7fc00000);
+    if (badq) { e = qnan; e_inter = qnan; e_intra = qnan; }
+
+    // (a4) back-propagation: subtree sums in place (children before parents), projection on the posed axes
+    if (GRAD) {
+        bool fin = true;
+        for (int f = L.nfrag - 1; f > 0; --f) {
+            const int4 fi = L.fragi[3 * f];
+            const int tor = L.fragi[3 * f + 1].w, ab = L.fragi[3 * f + 2].w;
+            float* o = S.own + f * 6 * 32;
+            const float Fx = o[0], Fy = o[32], Fz = o[64], Tx = o[96], Ty = o[128], Tz = o[160];
+            const int ia = ab & 0xffff, ib = ab >> 16;
+            const int oa = (ia >> 1) * 64 + (ia & 1), ob = (ib >> 1) * 64 + (ib & 1);
+            const float ax = Xf[oa], ay = Yf[oa], az = Zf[oa];
+            float ux = Xf[ob] - ax, uy = Yf[ob] - ay, uz = Zf[ob] - az;
+            const float un = rsqrtf(ux * ux + uy * uy + uz * uz);
+            ux *= un; uy *= un; uz *= un;
+            // torque about the pivot atom a: T - a x F
+            const float px = Tx - (ay * Fz - az * Fy), py = Ty - (az * Fx - ax * Fz), pz = Tz - (ax * Fy - ay * Fx);
+            float dt = ux * px + uy * py + uz * pz;
+            if (badq) dt = qnan;
+            fin = fin && isfinite(dt);
+            if (wr) grad[(6 + tor) * gs] = dt;
+            own_add(S.own, fi.x, Fx, Fy, Fz, Tx, Ty, Tz);
+        }
+        float g[6] = {S.own[0], S.own[32], S.own[64], S.own[96], S.own[128], S.own[160]};
+#pragma unroll
+        for (int d = 0; d < 6; ++d) {
+            if (badq) g[d] = qnan;
+            fin = fin && isfinite(g[d]);
+            if (wr) grad[d * gs] = g[d];
+        }
+        gfin = fin;
+    }
+    return e;
+}
+
+// ---------------------------------------------------------------- ADADELTA chain of this thread (R7)
+struct LaneLS {             // global scratch columns of this thread: element d at [d*stride]
+    float* best;            // [7+R]
+    float* Eg2;             // [6+R]
+    float* Ed2;             // [6+R]
+    float* grad;            // [6+R]
+    int stride;
+};
+
+// Start genotype in S.geno.  On return ls.best holds the best genotype seen; returns its energy (e_start if no finite
+// evaluation happened).  `active` lanes run the chain; the others only keep the warp's control flow uniform.
+__device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const ParDev& P, const LaneS& S, const LaneLS& ls,
+                                      bool active, float e_start, int& iters, float* trace, int trace_stride) {
+    const int R = L.R, D = 6 + R, Gn = 7 + R;
+    float bestE = __int_as_float(0x7f800000);
+    for (int d = 0; d < Gn; ++d) ls.best[d * ls.stride] = S.geno[d * 32];
+    for (int d = 0; d < D; ++d) { ls.Eg2[d * ls.stride] = 0.f; ls.Ed2[d * ls.stride] = 0.f; }
+    bool live = active;
+    int it = 0;
+    iters = 0;
+    for (; it < P.lsit; ++it) {
+        if (!__any_sync(kFull, live)) break;
+        float ei, ea;
+        bool gfin = true;
+        const float e = lane_eval<true>(L, G, P, S, ls.grad, ls.stride, true, ei, ea, gfin);
+        if (live) {
+            if (trace) trace[it * trace_stride] = e;
+            ++iters;
+            if (!(isfinite(e) && gfin)) live = false;
+        }
+        if (live) {
+            if (e < bestE) {
+                bestE = e;
+                for (int d = 0; d < Gn; ++d) ls.best[d * ls.stride] = S.geno[d * 32];
+            }
+            float w[3] = {0.f, 0.f, 0.f};
+            for (int d = 0; d < D; ++d) {
+                const float g = ls.grad[d * ls.stride];
+                const float eg2 = P.ad_rho * ls.Eg2[d * ls.stride] + (1.f - P.ad_rho) * g * g;
+                const float ed2o = ls.Ed2[d * ls.stride];
+                const float dl = -(sqrtf(ed2o + P.ad_eps) / sqrtf(eg2 + P.ad_eps)) * g;
+                ls.Eg2[d * ls.stride] = eg2;
+                ls.Ed2[d * ls.stride] = P.ad_rho * ed2o + (1.f - P.ad_rho) * dl * dl;
+                if (d < 3) S.geno[d * 32] += dl;
+                else if (d < 6) { if (d == 3) w[0] = dl; else if (d == 4) w[1] = dl; else w[2] = dl; }
+                else S.geno[(d + 1) * 32] = wrap_pi(S.geno[(d + 1) * 32] + dl);
+            }
+            const float th = sqrtf(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
+            float sh, ch;
+            sincosf(0.5f * th, &sh, &ch);
+            const float k = th > 1e-12f ? sh / th : 0.5f;
+            const float q[4] = {S.geno[96], S.geno[128], S.geno[160], S.geno[192]};
+            float nq[4];
+            rotate_quat(ch, k * w[0], k * w[1], k * w[2], q, nq);
+            S.geno[96] = nq[0]; S.geno[128] = nq[1]; S.geno[160] = nq[2]; S.geno[192] = nq[3];
+        }
+    }
+    return isfinite(bestE) ? bestE : e_start;
+}
+
+}  // namespace adock

@@ -55,6 +55,11 @@ struct Topology {
     // positions: int_of_ext [N] atom -> position, ext_of_int [npos] position -> atom or -1 (hole)
     std::vector<int> ext_of_int, int_of_ext;
     std::vector<unsigned char> blob;      // device image
+    // rigid fragments in DFS preorder (parent < child; a torsion's subtree is the range [f, sub_end)); tor = caller's
+    // torsion index of the bond that attaches the fragment to its parent (-1 for the root); atoms in caller order
+    struct FragInfo { int parent, tor, sub_end; std::vector<int> atoms; };
+    std::vector<FragInfo> frag_info;
+    std::vector<int> frag_of_ext;         // [N]
     std::string error;
 };
 
@@ -155,6 +160,9 @@ inline bool build_topology(Topology& tp, int N, const float* xyz, const int* typ
     tp.nfrag = (int)frags.size();
     for (int i = 0; i < N; ++i)
         if (frag_of[i] < 0) { tp.error = "ligand graph is not connected"; return false; }
+    tp.frag_of_ext = frag_of;
+    tp.frag_info.clear();
+    for (const Frag& f : frags) tp.frag_info.push_back({f.parent, f.tor, f.sub_end, f.atoms});
     // ---- atom positions.  Position q = pass*32 + lane is the atom's slot in every per-warp array, so its
     // shared-memory bank is q mod 32.  Crowded atoms (many pairs) get a bank of their own; when N > 32 the
     // atoms with the fewest pairs share banks (longest-processing-time assignment of pair counts to banks).
