@@ -95,6 +95,18 @@ int adock_ligand_tree(const adock_ligand* l, const int** tor_order, const unsign
  * maps caller atom index -> internal index. */
 int adock_ligand_image(const adock_ligand* l, int* bytes, const unsigned char** image, const int** int_of_ext);
 
+/* The ligand image of the lane-per-individual kernels (host copy, owned by the handle): atoms in fragment
+ * DFS preorder, fragment tree, and the pair list cut into 4-row x 2-column register tiles (layout:
+ * csrc/lane_image.hpp).  pos_of_ext [N] maps caller atom index -> position in that order. */
+int adock_ligand_lane_image(const adock_ligand* l, int* bytes, const unsigned char** image, const int** pos_of_ext);
+
+/* Kernel family used by the compute entry points of this process: 0 = chosen by problem
+ * size (default), 1 = one warp per individual, 2 = one thread (lane) per individual.  Both families compute
+ * the same function (R3-R7) and pass the same parity tests; they differ in summation order only. */
+int adock_set_path(int path);
+/* Family (1 or 2) the local search of the last adock_dock / adock_dock_many on this thread ran in; 0 = none yet. */
+int adock_last_dock_path(void);
+
 /* Batched scoring (R3-R6): for each of n genotypes build the pose, interpolate the maps, sum the
  * intramolecular pair terms and back-propagate.  d_genotypes: device [n][gstride], gstride >= 7+R.
  * d_energies: device [n].  d_energy_terms: device [n][2] = (intermolecular, intramolecular) or NULL.

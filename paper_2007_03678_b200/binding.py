@@ -19,7 +19,7 @@ ADOCK_OK, ADOCK_EINVAL, ADOCK_ENOMEM, ADOCK_ECUDA, ADOCK_ELIMIT = 0, -1, -2, -3,
 EXPORTS = ["adock_default_params", "adock_load_grids", "adock_free_grids", "adock_load_ligand", "adock_free_ligand",
            "adock_ligand_pairs", "adock_ligand_tree", "adock_ligand_image", "adock_score_batch", "adock_score_batch_host", "adock_local_search",
            "adock_philox", "adock_ga_generation", "adock_dock", "adock_dock_many", "adock_launch_count", "adock_last_error", "adock_profile", "adock_profile_read",
-           "adock_ligand_lane_image", "adock_set_path"]
+           "adock_ligand_lane_image", "adock_set_path", "adock_last_dock_path"]
 
 
 class AdockError(RuntimeError):
@@ -277,6 +277,10 @@ PATHS = {"auto": 0, "warp": 1, "lane": 2}
 def adock_set_path(path) -> None:
     """kernel family: 'auto' (by problem size), 'warp' (warp per individual) or 'lane' (thread per individual)"""
     _check(lib().adock_set_path(PATHS[path] if isinstance(path, str) else int(path)))
+
+
+def adock_last_dock_path() -> str:
+    return {0: "none", 1: "warp", 2: "lane"}[int(lib().adock_last_dock_path())]
 
 
 def adock_launch_count(reset: bool = False) -> int:

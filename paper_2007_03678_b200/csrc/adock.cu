@@ -40,6 +40,7 @@ static int g_path = 0;                                    // adock_set_path: 0 a
 static thread_local bool g_prof = false;                  // adock_profile: time every dock_ls_kernel launch
 static thread_local double g_ls_ms = 0;
 static thread_local long long g_ls_launches = 0, g_ls_evals = 0;
+static thread_local int g_last_dock_path = 0;             // kernel family of the last docking's local search
 
 static int fail(int code, const std::string& msg) {
     g_err = msg;
@@ -261,6 +262,8 @@ extern "C" int adock_ligand_lane_image(const adock_ligand* l, int* bytes, const 
     return ADOCK_OK;
 }
 
+extern "C" int adock_last_dock_path(void) { return g_last_dock_path; }
+
 extern "C" int adock_set_path(int path) {
     if (path < 0 || path > 2) return fail(ADOCK_EINVAL, "path must be 0 (auto), 1 (warp per individual) or 2 (lane per individual)");
     g_path = path;
@@ -331,6 +334,14 @@ static int lane_fit_warps(int lane_bytes, int warp_floats) {
 }
 // the lane kernels want at least one warp per scheduler
 static bool lane_ok(const adock_ligand* l) { return lane_fit_warps(l->lane_bytes, l->lane_warp_floats) >= 4; }
+// ADADELTA chains (threads) from which the lane-per-individual kernels are preferred over warp-per-individual:
+// one warp per scheduler (measured at 40 atoms: 18k chains is where the lane family overtakes, profiles/)
+constexpr int kLaneMinChains = 148 * 4 * 32;
+// few warps of work: fewer warps per CTA so that they spread over the SMs
+static int lane_spread_warps(int W, int nwarps) {
+    while (W > 1 && (long long)g_sm_count * W > (long long)nwarps) --W;
+    return W;
+}
 
 template <bool GRAD>
 __global__ void __launch_bounds__(kLaneMaxWarps * 32, 1) score_lane_kernel(GridDev G, ParDev P, ScoreArgs a) {
@@ -499,6 +510,33 @@ __global__ void __launch_bounds__(128) ls_array_kernel(GridDev G, ParDev P, LsAr
     }
 }
 
+// lane-per-individual variant: thread c runs chain c; ADADELTA state in global scratch columns [row][nthreads]
+__global__ void __launch_bounds__(kLaneMaxWarps * 32, 1) ls_array_lane_kernel(GridDev G, ParDev P, LsArgs a, float* __restrict__ scratch) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned char* blob = smem + 16;
+    stage_ligand(blob, a.blob, a.blob_bytes, reinterpret_cast<uint64_t*>(smem), 0);
+    const LaneL L = lane_view(blob);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wf = reinterpret_cast<const LaneHeader*>(blob)->warp_floats;
+    const LaneS S = lane_scratch(reinterpret_cast<float*>(blob + a.blob_bytes) + (size_t)warp * wf * 32, L, lane);
+    const int Gn = 7 + L.R, D = 6 + L.R;
+    const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, T = (size_t)gridDim.x * blockDim.x;
+    const bool act = tid < (size_t)a.n;
+    const size_t idx = act ? tid : (size_t)a.n - 1;
+    for (int d = 0; d < Gn; ++d) S.geno[d * 32] = a.genos[idx * a.gstride + d];
+    LaneLS ls;
+    ls.best = scratch + tid; ls.Eg2 = ls.best + (size_t)Gn * T; ls.Ed2 = ls.Eg2 + (size_t)D * T; ls.grad = ls.Ed2 + (size_t)D * T;
+    ls.stride = (int)T;
+    int iters = 0;
+    const float e = lane_adadelta(L, G, P, S, ls, act, __int_as_float(0x7fc00000), iters,
+                                  a.trace ? a.trace + idx * P.lsit : nullptr, 1);
+    if (act) {
+        for (int d = 0; d < Gn; ++d) a.genos[idx * a.gstride + d] = ls.best[(size_t)d * T];
+        a.E[idx] = e;
+        if (a.iters) a.iters[idx] = iters;
+    }
+}
+
 extern "C" int adock_local_search(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
                                   float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, float* d_trace,
                                   void* cuda_stream) {
@@ -511,6 +549,30 @@ extern "C" int adock_local_search(const adock_grids* grids, const adock_ligand* 
     if (rc) return rc;
     rc = device_props();
     if (rc) return rc;
+    if (g_path == 2 || (g_path == 0 && n >= kLaneMinChains && lane_ok(ligand))) {
+        int W = lane_fit_warps(ligand->lane_bytes, ligand->lane_warp_floats);
+        if (!W) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
+        const int nwarps = (n + 31) / 32;
+        W = lane_spread_warps(W, nwarps);
+        const int grid = (nwarps + W - 1) / W;
+        const size_t smem = lane_smem(ligand->lane_bytes, ligand->lane_warp_floats, W);
+        const size_t T = (size_t)grid * W * 32;
+        const int R = ligand->tp.R;
+        float* scratch = nullptr;
+        cudaStream_t stm = (cudaStream_t)cuda_stream;
+        cudaError_t e = cudaMallocAsync(&scratch, T * (size_t)(7 + R + 3 * (6 + R)) * 4, stm);
+        if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("ls scratch: ") + cudaGetErrorString(e));
+        CUDA_TRY(cudaFuncSetAttribute(ls_array_lane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ParDev P = make_pardev(p);
+        P.k_wall_h = p.k_wall * grids->dev.h;
+        LsArgs a{ligand->d_lane, d_genotypes, d_energies, d_iters, d_trace, ligand->lane_bytes, n, gstride};
+        ls_array_lane_kernel<<<grid, W * 32, smem, stm>>>(grids->dev, P, a, scratch);
+        ++g_launches;
+        e = cudaGetLastError();
+        cudaFreeAsync(scratch, stm);
+        if (e != cudaSuccess) return fail(ADOCK_ECUDA, std::string("ls_array_lane_kernel: ") + cudaGetErrorString(e));
+        return ADOCK_OK;
+    }
     const int W = fit_warps(ligand->blob_bytes, ligand->scratch_floats, 4);
     if (!W) return fail(ADOCK_ELIMIT, "ligand does not fit in shared memory");
     const size_t smem = cta_smem(ligand->blob_bytes, ligand->scratch_floats, W);
@@ -545,6 +607,8 @@ struct DockJob {
     int* out_gens;          // [nrun]
     unsigned long long seed;
     int blob_bytes, Gn, N, R;
+    const unsigned char* lane;  // lane-per-individual image (lane_image.hpp)
+    int lane_bytes, pad0;
 };
 struct DockDims {
     int nrun, P, n_ls, upj;         // upj = CTAs per job for this launch
@@ -674,6 +738,45 @@ __global__ void __launch_bounds__(128) dock_ls_kernel(GridDev G, ParDev P, const
     }
 }
 
+// the same step, lane-per-individual: thread c of a job runs chain c = run*n_ls + l; every CTA stages its job's lane
+// image; ADADELTA state in global scratch columns [row][all threads of the launch] (rows: Gmax best, 3 x Dmax)
+__global__ void __launch_bounds__(kLaneMaxWarps * 32, 1) dock_ls_lane_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs,
+                                                                             DockDims dm, float* __restrict__ scratch, int Gmax) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const DockJob job = jobs[blockIdx.x / dm.upj];
+    unsigned char* blob = smem + 16;
+    stage_ligand(blob, job.lane, job.lane_bytes, reinterpret_cast<uint64_t*>(smem), 0);
+    const LaneL L = lane_view(blob);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wf = reinterpret_cast<const LaneHeader*>(blob)->warp_floats;
+    const LaneS S = lane_scratch(reinterpret_cast<float*>(blob + job.lane_bytes) + (size_t)warp * wf * 32, L, lane);
+    const int Gn = job.Gn;
+    const int c = (blockIdx.x % dm.upj) * blockDim.x + threadIdx.x;
+    bool act = c < dm.nrun * dm.n_ls;
+    const int cc = act ? c : 0;
+    const int run = cc / dm.n_ls, l = cc % dm.n_ls;
+    const RunState st = job.st[run];
+    act = act && st.active;
+    if (!__any_sync(kFull, act)) return;
+    const size_t popsz = (size_t)dm.nrun * dm.P;
+    const int slot = job.picks[(size_t)run * dm.P + l];
+    float* g = job.pop + ((size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P + slot) * Gn;
+    float* e = job.E + (size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P + slot;
+    for (int d = 0; d < Gn; ++d) S.geno[d * 32] = g[d];
+    const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, T = (size_t)gridDim.x * blockDim.x;
+    const int Dmax = Gmax - 1;
+    LaneLS ls;
+    ls.best = scratch + tid; ls.Eg2 = ls.best + (size_t)Gmax * T; ls.Ed2 = ls.Eg2 + (size_t)Dmax * T; ls.grad = ls.Ed2 + (size_t)Dmax * T;
+    ls.stride = (int)T;
+    int iters = 0;
+    const float be = lane_adadelta(L, G, P, S, ls, act, act ? *e : 0.f, iters, nullptr, 0);
+    if (act) {
+        for (int d = 0; d < Gn; ++d) g[d] = ls.best[(size_t)d * T];
+        *e = be;
+        atomicAdd(&job.st[run].ls_acc, iters);
+    }
+}
+
 // end of generation: eval accounting, buffer flip, termination test
 __global__ void dock_commit_kernel(const DockJob* __restrict__ jobs, int njobs, DockDims dm, int* __restrict__ any_active) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -769,6 +872,23 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     }
     const int Wga = fit_warps(maxblob, maxscr, 8), Wls = fit_warps(maxblob, maxscr, 4);
     if (!Wga || !Wls) return fail(ADOCK_ELIMIT, "ligand does not fit in shared memory");
+    // local search: lane-per-individual when there are enough chains to fill the SMs with whole warps
+    const int n_ls0 = n_ls_of(p, Pn);
+    const long long chains = (long long)nlig * nrun * n_ls0;
+    int maxlane = 0, maxwf = 0, Gmax = 7;
+    bool lanes_fit = true;
+    for (int l = 0; l < nlig; ++l) {
+        maxlane = std::max(maxlane, ligs[l]->lane_bytes);
+        maxwf = std::max(maxwf, ligs[l]->lane_warp_floats);
+        Gmax = std::max(Gmax, 7 + ligs[l]->tp.R);
+        lanes_fit = lanes_fit && lane_ok(ligs[l]);
+    }
+    int Wlane = 0;
+    for (int w = kLaneMaxWarps; w > 0 && !Wlane; --w)
+        if (lane_smem(maxlane, maxwf, w) <= (size_t)g_smem_optin) Wlane = w;
+    const bool ls_lane = Wlane > 0 && (g_path == 2 || (g_path == 0 && lanes_fit && chains >= kLaneMinChains));
+    if (g_path == 2 && !Wlane) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
+    g_last_dock_path = ls_lane ? 2 : 1;
     ParDev P = make_pardev(p);
     P.k_wall_h = p.k_wall * grids->dev.h;
     DockDims dm{};
@@ -794,6 +914,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         const adock_ligand* lg = ligs[l];
         j.blob = lg->d_blob; j.ext_of_int = lg->d_ext_of_int; j.blob_bytes = lg->blob_bytes;
         j.Gn = 7 + lg->tp.R; j.N = lg->tp.N; j.R = lg->tp.R; j.seed = seeds[l];
+        j.lane = lg->d_lane; j.lane_bytes = lg->lane_bytes; j.pad0 = 0;
         e = buf.alloc(&j.pop, 2 * popsz * j.Gn * 4);
         if (e == cudaSuccess) e = buf.alloc(&j.E, 2 * popsz * 4);
         if (e == cudaSuccess) e = buf.alloc(&j.st, (size_t)nrun * sizeof(RunState));
@@ -820,6 +941,25 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     dga.upj = (int)((popsz + Wga - 1) / Wga);
     dls.upj = std::max(1, (nrun * dm.n_ls + Wls - 1) / Wls);
     dfin.upj = (nrun + Wls - 1) / Wls;
+    // lane family: warps of a job's chains split evenly over the fewest CTAs that fit
+    DockDims dll = dm;
+    int Wl = 1;
+    size_t smem_ll = 0;
+    float* d_lscratch = nullptr;
+    if (ls_lane && dm.n_ls > 0) {
+        const int jw = (nrun * dm.n_ls + 31) / 32;                  // warps per job
+        dll.upj = (jw + Wlane - 1) / Wlane;
+        Wl = (jw + dll.upj - 1) / dll.upj;
+        smem_ll = lane_smem(maxlane, maxwf, Wl);
+        const size_t T = (size_t)nlig * dll.upj * Wl * 32;
+        cudaError_t e2 = buf.alloc(&d_lscratch, T * (size_t)(Gmax + 3 * (Gmax - 1)) * 4);
+        if (e2 != cudaSuccess) return fail(e2 == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("dock alloc: ") + cudaGetErrorString(e2));
+        CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ll));
+    }
+    auto launch_ls = [&]() {
+        if (ls_lane) dock_ls_lane_kernel<<<dll.upj * nlig, Wl * 32, smem_ll, stm>>>(grids->dev, P, d_jobs, dll, d_lscratch, Gmax);
+        else dock_ls_kernel<<<dls.upj * nlig, Wls * 32, smem_ls, stm>>>(grids->dev, P, d_jobs, dls);
+    };
     dock_init_kernel<<<dga.upj * nlig, Wga * 32, smem_ga, stm>>>(grids->dev, P, d_jobs, dga);
     ++g_launches;
     CUDA_TRY(cudaGetLastError());
@@ -834,11 +974,11 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
                 cudaEvent_t a, b;
                 CUDA_TRY(cudaEventCreate(&a)); CUDA_TRY(cudaEventCreate(&b));
                 CUDA_TRY(cudaEventRecord(a, stm));
-                dock_ls_kernel<<<dls.upj * nlig, Wls * 32, smem_ls, stm>>>(grids->dev, P, d_jobs, dls);
+                launch_ls();
                 CUDA_TRY(cudaEventRecord(b, stm));
                 prof_ev.push_back(a); prof_ev.push_back(b);
             } else {
-                dock_ls_kernel<<<dls.upj * nlig, Wls * 32, smem_ls, stm>>>(grids->dev, P, d_jobs, dls);
+                launch_ls();
             }
         }
         const bool check = ((g + 1) % poll) == 0;

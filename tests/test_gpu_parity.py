@@ -36,6 +36,14 @@ def dev():
     return torch.device("cuda:0")
 
 
+@pytest.fixture(params=["warp", "lane"])
+def family(request, B):
+    """run the test once per kernel family (warp per individual / thread per individual); restores 'auto'"""
+    B.adock_set_path(request.param)
+    yield request.param
+    B.adock_set_path("auto")
+
+
 class Case:
     def __init__(self, B, orc, W, grids, lig, params=None):
         self.grids, self.lig = grids, lig
@@ -111,7 +119,7 @@ def test_integer_structure_bit_exact(B, cases, name):
 
 # ------------------------------------------------------------------------------- scoring parity (rows a1-a4)
 @pytest.mark.parametrize("name,n", [("tiny", 1024), ("drug", 2500), ("sweep16", 777), ("sweep80", 1100), ("sweep128", 600)])
-def test_score_parity(B, orc, W, cases, dev, name, n):
+def test_score_parity(B, orc, W, cases, dev, family, name, n):
     c = cases(name)
     G = W.make_genotypes(n, c.lig.R, c.grids, seed=100 + n)
     ref = orc.score(c.og, c.ol, c.op, G)
@@ -130,7 +138,7 @@ def test_score_parity(B, orc, W, cases, dev, name, n):
     assert np.allclose(E2, E, rtol=1e-6, atol=1e-6)
 
 
-def test_score_strides_ragged_and_empty(B, orc, W, cases, dev):
+def test_score_strides_ragged_and_empty(B, orc, W, cases, dev, family):
     c = cases("tiny")
     for n in (1, 7, 33, 255):                           # ragged tails of the warp/CTA tiling
         G = W.make_genotypes(n, c.lig.R, c.grids, seed=n)
@@ -144,7 +152,7 @@ def test_score_strides_ragged_and_empty(B, orc, W, cases, dev):
     assert e.value.code == B.ADOCK_EINVAL
 
 
-def test_score_special_poses(B, orc, W, cases, dev):
+def test_score_special_poses(B, orc, W, cases, dev, family):
     c = cases("tiny")
     R = c.lig.R
     ident = c.ol.identity_genotype().astype(np.float32)
@@ -162,7 +170,7 @@ def test_score_special_poses(B, orc, W, cases, dev):
     assert_gradient(gr[keep], {k: ref[k][keep] for k in ("grad", "scales")}, R, np.array([False, True, False]))
 
 
-def test_score_rigid_ligand_without_torsions(B, orc, W, dev):
+def test_score_rigid_ligand_without_torsions(B, orc, W, dev, family):
     grids, _ = W.make_config("tiny")
     lig = W.make_ligand(12, 0, 4, seed=8, centre=0.5 * (grids.box_lo + grids.box_hi))
     c = Case(B, orc, W, grids, lig)
@@ -303,7 +311,7 @@ def test_ga_decisions_bit_exact_and_children_match(B, orc, cases, dev):
 
 
 # ------------------------------------------------------------------------------- ADADELTA (row a5)
-def test_local_search_first_iterations_track_oracle(B, orc, W, cases, dev):
+def test_local_search_first_iterations_track_oracle(B, orc, W, cases, dev, family):
     """Per-iteration energies E(x_k) of the ADADELTA chain (d_trace) against the oracle's trace.  Starts are
     relaxed poses (the oracle's own 300-iteration search from random genotypes, then a small seeded kick):
     random starts sit in 1e6..1e9 kcal/mol clashes where the fp32 cancellation floor of the gradient
@@ -355,7 +363,7 @@ def test_local_search_first_iterations_track_oracle(B, orc, W, cases, dev):
     assert np.abs(gG[a] - oG[a]).max() < 2e-3
 
 
-def test_local_search_statistics_match_oracle(B, orc, W, cases, dev):
+def test_local_search_statistics_match_oracle(B, orc, W, cases, dev, family):
     c = cases("drug")
     n = 384
     G = W.make_genotypes(n, c.lig.R, c.grids, seed=22, wall_tail=0.0)
@@ -377,7 +385,7 @@ def test_local_search_statistics_match_oracle(B, orc, W, cases, dev):
 
 
 # ------------------------------------------------------------------------------- full LGA docking (rows a5-a7)
-def test_dock_tiny_accounting_and_validity(B, orc, cases):
+def test_dock_tiny_accounting_and_validity(B, orc, cases, family):
     c = cases("tiny", lsit=15)
     P, nrun = 16, 5
     max_evals = 16 + 20 * (15 + 15)                       # BASELINE.json configs[0]: pop 16, 20 generations
@@ -402,7 +410,7 @@ def test_dock_tiny_accounting_and_validity(B, orc, cases):
     assert_energy(r0["energies"][:1], np.array([e_init.min()]), "generation-0 best")
 
 
-def test_dock_distribution_matches_oracle(B, orc, cases):
+def test_dock_distribution_matches_oracle(B, orc, cases, family):
     """'best-energy distributions over runs statistically indistinguishable' (north_star):
     5 seeds x 20 runs per side on the tiny config."""
     c = cases("tiny", lsit=30)
@@ -418,7 +426,9 @@ def test_dock_distribution_matches_oracle(B, orc, cases):
     assert abs(np.median(g) - np.median(o)) < 0.5 * iqr
 
 
-def test_dock_many_equals_single_docks(B, W, orc, cases):
+def test_dock_many_equals_single_docks(B, W, orc, cases, family):
+    """within one kernel family a ligand's docking does not depend on what else is in the batch (the families differ
+    in summation order, so 'auto', which picks by batch size, may not be bit-identical between the two calls)"""
     c = cases("drug", lsit=10)
     ligs = W.make_screen_ligands(3, c.grids)
     gl = [B.Ligand.from_workload(c.gg, l, c.gp) for l in ligs]
@@ -430,6 +440,7 @@ def test_dock_many_equals_single_docks(B, W, orc, cases):
         assert np.array_equal(many["genotypes"][k, :, :7 + l.R], one["genotypes"])
         assert np.array_equal(many["coords"][k, :, :l.N], one["coords"])
         assert np.array_equal(many["evals"][k], one["evals"])
+    assert B.adock_last_dock_path() == family
 
 
 def test_host_only_handle_is_rejected_by_compute_calls(B, cases, dev):
