@@ -119,9 +119,12 @@ __device__ inline void stage_ligand(unsigned char* dst, const unsigned char* src
 
 // ---------------------------------------------------------------- grid term (R4)
 struct F8 { float4 lo, hi; };
-__device__ __forceinline__ F8 ld_cell(const float4* p) {     // one aligned 32-byte sector: LDG.256
+// One aligned 32-byte sector (LDG.256).  The lookups of a warp are scattered over the maps (32 lanes = 32 poses), so a
+// line brought into L1 is not touched again before it is evicted: L1::no_allocate skips the allocation and is +31 %
+// on the lane-per-individual scoring kernel (profiles/r01b_grid_load_variants.md); the maps stay L2 resident.
+__device__ __forceinline__ F8 ld_cell(const float4* p) {
     F8 r;
-    asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+    asm("ld.global.nc.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
         : "=f"(r.lo.x), "=f"(r.lo.y), "=f"(r.lo.z), "=f"(r.lo.w), "=f"(r.hi.x), "=f"(r.hi.y), "=f"(r.hi.z), "=f"(r.hi.w)
         : "l"(p));
     return r;
@@ -175,6 +178,51 @@ __device__ __forceinline__ float grid_atom(const GridDev& G, const ParDev& P, in
         gx = (ox != 0.f) ? copysignf(P.k_wall, ox) : (dfx + sfx) * G.inv_h;
         gy = (oy != 0.f) ? copysignf(P.k_wall, oy) : (dfy + sfy) * G.inv_h;
         gz = (oz != 0.f) ? copysignf(P.k_wall, oz) : (dfz + sfz) * G.inv_h;
+    }
+    return val;
+}
+
+// The same lookup in three stages, so that a caller can issue the sector loads of several atoms before consuming
+// any of them: grid_cell (clamp, cell index, fractions), grid_fetch (4 sector loads), grid_finish (interpolation).
+struct GridCell {
+    const float4* base;     // sector of corner (iz, iy, ix..ix+1) of the atom's type
+    float fx, fy, fz;       // fractions inside the cell
+    float ox, oy, oz;       // signed distance outside the box in grid units (0 inside)
+};
+__device__ __forceinline__ GridCell grid_cell(const GridDev& G, int type, float x, float y, float z) {
+    const float ux = (x - G.ox) * G.inv_h, uy = (y - G.oy) * G.inv_h, uz = (z - G.oz) * G.inv_h;
+    const float cx = fminf(fmaxf(ux, 0.f), (float)(G.nx - 1)), cy = fminf(fmaxf(uy, 0.f), (float)(G.ny - 1)),
+                cz = fminf(fmaxf(uz, 0.f), (float)(G.nz - 1));
+    const int ix = min((int)cx, G.nx - 2), iy = min((int)cy, G.ny - 2), iz = min((int)cz, G.nz - 2);
+    GridCell c;
+    c.fx = cx - (float)ix; c.fy = cy - (float)iy; c.fz = cz - (float)iz;
+    c.ox = ux - cx; c.oy = uy - cy; c.oz = uz - cz;
+    c.base = G.cells + (long long)type * G.type_stride + ((long long)(iz * G.ny + iy) * (G.nx - 1) + ix) * 2;
+    return c;
+}
+__device__ __forceinline__ void grid_fetch(const GridDev& G, const GridCell& c, F8 (&v)[4]) {
+    const int rowlen = (G.nx - 1) * 2;
+    v[0] = ld_cell(c.base);
+    v[1] = ld_cell(c.base + rowlen);
+    v[2] = ld_cell(c.base + (long long)G.ny * rowlen);
+    v[3] = ld_cell(c.base + (long long)G.ny * rowlen + rowlen);
+}
+template <bool GRAD>
+__device__ __forceinline__ float grid_finish(const GridDev& G, const ParDev& P, const GridCell& c, const F8 (&v)[4], float q,
+                                             float& gx, float& gy, float& gz) {
+    const float aq = fabsf(q);
+    float val, dfx, dfy, dfz, vs, sfx, sfy, sfz;
+    trilinear8<GRAD>(v[0].lo.x, v[0].hi.x, v[1].lo.x, v[1].hi.x, v[2].lo.x, v[2].hi.x, v[3].lo.x, v[3].hi.x, c.fx, c.fy, c.fz,
+                     val, dfx, dfy, dfz);
+    trilinear8<GRAD>(fmaf(aq, v[0].lo.z, q * v[0].lo.y), fmaf(aq, v[0].hi.z, q * v[0].hi.y), fmaf(aq, v[1].lo.z, q * v[1].lo.y),
+                     fmaf(aq, v[1].hi.z, q * v[1].hi.y), fmaf(aq, v[2].lo.z, q * v[2].lo.y), fmaf(aq, v[2].hi.z, q * v[2].hi.y),
+                     fmaf(aq, v[3].lo.z, q * v[3].lo.y), fmaf(aq, v[3].hi.z, q * v[3].hi.y), c.fx, c.fy, c.fz, vs, sfx, sfy, sfz);
+    val += vs;
+    val = fmaf(P.k_wall_h, fabsf(c.ox) + fabsf(c.oy) + fabsf(c.oz), val);
+    if (GRAD) {
+        gx = (c.ox != 0.f) ? copysignf(P.k_wall, c.ox) : (dfx + sfx) * G.inv_h;
+        gy = (c.oy != 0.f) ? copysignf(P.k_wall, c.oy) : (dfy + sfy) * G.inv_h;
+        gz = (c.oz != 0.f) ? copysignf(P.k_wall, c.oz) : (dfz + sfz) * G.inv_h;
     }
     return val;
 }

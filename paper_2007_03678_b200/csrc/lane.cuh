@@ -78,7 +78,7 @@ __device__ __forceinline__ PairK make_pairk(const ParDev& P) {
 
 // Row atom i (broadcast to both halves) against J atoms (j0 | j1).  Accumulates the pair energies into e2, and
 // ns*d into BOTH gi (which therefore holds MINUS the gradient on i) and gj (the gradient on j), ns = -(dE/dr)/r.
-template <bool GRAD>
+template <bool GRAD, bool HB>
 __device__ __forceinline__ void pair_row(const PairK& K, f2 xi, f2 yi, f2 zi, f2 xj, f2 yj, f2 zj, float4 ra, float4 rb,
                                          unsigned hb, f2& e2, f2& gix, f2& giy, f2& giz, f2& gjx, f2& gjy, f2& gjz) {
     const f2 dx = sub2(xi, xj), dy = sub2(yi, yj), dz = sub2(zi, zj);
@@ -95,7 +95,7 @@ __device__ __forceinline__ void pair_row(const PairK& K, f2 xi, f2 yi, f2 zi, f2
     const f2 c12 = pk(ra.x, ra.y), ncA = pk(ra.z, ra.w), ds = pk(rb.x, rb.y), qq = pk(rb.z, rb.w);
     const f2 u12 = mul2(mul2(c12, r6), r6);
     f2 rA = r6;
-    if (hb) {                                   // 12-10 slot(s): warp-uniform branch, rare
+    if (HB) {                                   // 12-10 slot(s) in this half: rare
         float a, b, l, h;
         unpk(mul2(r6, rinv4), a, b);
         unpk(r6, l, h);
@@ -121,7 +121,7 @@ __device__ __forceinline__ void pair_row(const PairK& K, f2 xi, f2 yi, f2 zi, f2
         // -dE/dr = rinv (12 u12 - nA uA + eel) + eel (deps/dr)/eps + (r/sigma^2) egs
         const f2 s = add2(evdw, u12);
         f2 A1 = fma2(K.six, s, eel);
-        if (hb) A1 = fma2(pk((hb & 1u) ? 4.f : 0.f, (hb & 2u) ? 4.f : 0.f), nuA, A1);
+        if (HB) A1 = fma2(pk((hb & 1u) ? 4.f : 0.f, (hb & 2u) ? 4.f : 0.f), nuA, A1);
         const f2 dee = mul2(mul2(K.BlamB, kex), inv);
         const f2 A3 = fma2(eel, dee, mul2(A1, rinv));
         const f2 A4 = fma2(K.isig2, mul2(rr, egs), A3);
@@ -209,36 +209,50 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
         }
     }
 
-    // (a2) grid term, two atoms per step (eight independent sector loads in flight); the gradient goes straight into
-    // the (force, torque about t) sums of the atom's fragment, which initialises own[]
+    // (a2) grid term, kLaneBI = 4 atoms per step: the 16 sector loads of a step are issued back to back before the first
+    // is consumed (the lookups are pure L2 latency: one dependent round per step instead of one per atom); the
+    // gradient goes straight into the (force, torque about t) sums of the atom's fragment, which initialises own[]
     float eg = 0.f;
     {
         float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
         int cur = 0;
-        for (int m = 0; m < L.Npad / 2; ++m) {
-            const int t0 = L.types[2 * m], t1 = L.types[2 * m + 1];       // type | frag << 8 ; -1 = pad
-            if (t0 < 0) break;
-            const float2 xr = S.X[m * 32], yr = S.Y[m * 32], zr = S.Z[m * 32];
-            const float q0 = L.atoms[2 * m].w, q1 = L.atoms[2 * m + 1].w;
-            float g0x = 0, g0y = 0, g0z = 0, g1x = 0, g1y = 0, g1z = 0;
-            eg += grid_atom<GRAD>(G, P, t0 & 0xff, q0, xr.x + tx, yr.x + ty, zr.x + tz, g0x, g0y, g0z);
-            if (t1 >= 0) eg += grid_atom<GRAD>(G, P, t1 & 0xff, q1, xr.y + tx, yr.y + ty, zr.y + tz, g1x, g1y, g1z);
-            if (GRAD) {
-                const int f0 = t0 >> 8, f1 = t1 >= 0 ? t1 >> 8 : f0;
-                if (f0 != cur) {
-                    float* o = S.own + cur * 6 * 32;
-                    o[0] = Fx; o[32] = Fy; o[64] = Fz; o[96] = Tx; o[128] = Ty; o[160] = Tz;
-                    Fx = Fy = Fz = Tx = Ty = Tz = 0.f; cur = f0;
+        for (int m = 0; m < L.Npad / 2; m += 2) {
+            int tt[4];
+            float q[4], rx[4], ry[4], rz[4];
+            GridCell gc[4];
+            F8 c[4][4];
+            {
+                const int4 t4 = *reinterpret_cast<const int4*>(L.types + 2 * m);      // type | frag << 8 ; -1 = pad
+                tt[0] = t4.x; tt[1] = t4.y; tt[2] = t4.z; tt[3] = t4.w;
+                const float2 xa = S.X[m * 32], ya = S.Y[m * 32], za = S.Z[m * 32];
+                const float2 xb = S.X[(m + 1) * 32], yb = S.Y[(m + 1) * 32], zb = S.Z[(m + 1) * 32];
+                rx[0] = xa.x; rx[1] = xa.y; rx[2] = xb.x; rx[3] = xb.y;
+                ry[0] = ya.x; ry[1] = ya.y; ry[2] = yb.x; ry[3] = yb.y;
+                rz[0] = za.x; rz[1] = za.y; rz[2] = zb.x; rz[3] = zb.y;
+            }
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                q[a] = L.atoms[2 * m + a].w;
+                gc[a] = grid_cell(G, tt[a] < 0 ? 0 : (tt[a] & 0xff), rx[a] + tx, ry[a] + ty, rz[a] + tz);
+            }
+#pragma unroll
+            for (int a = 0; a < 4; ++a) grid_fetch(G, gc[a], c[a]);
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                float gx, gy, gz;
+                const float e = grid_finish<GRAD>(G, P, gc[a], c[a], q[a], gx, gy, gz);
+                if (tt[a] < 0) continue;                    // pad atom (warp-uniform): looked up, not counted
+                eg += e;
+                if (GRAD) {
+                    const int f = tt[a] >> 8;
+                    if (f != cur) {
+                        float* o = S.own + cur * 6 * 32;
+                        o[0] = Fx; o[32] = Fy; o[64] = Fz; o[96] = Tx; o[128] = Ty; o[160] = Tz;
+                        Fx = Fy = Fz = Tx = Ty = Tz = 0.f; cur = f;
+                    }
+                    Fx += gx; Fy += gy; Fz += gz;
+                    Tx += ry[a] * gz - rz[a] * gy; Ty += rz[a] * gx - rx[a] * gz; Tz += rx[a] * gy - ry[a] * gx;
                 }
-                Fx += g0x; Fy += g0y; Fz += g0z;
-                Tx += yr.x * g0z - zr.x * g0y; Ty += zr.x * g0x - xr.x * g0z; Tz += xr.x * g0y - yr.x * g0x;
-                if (f1 != cur) {
-                    float* o = S.own + cur * 6 * 32;
-                    o[0] = Fx; o[32] = Fy; o[64] = Fz; o[96] = Tx; o[128] = Ty; o[160] = Tz;
-                    Fx = Fy = Fz = Tx = Ty = Tz = 0.f; cur = f1;
-                }
-                Fx += g1x; Fy += g1y; Fz += g1z;
-                Tx += yr.y * g1z - zr.y * g1y; Ty += zr.y * g1x - xr.y * g1z; Tz += xr.y * g1y - yr.y * g1x;
             }
         }
         if (GRAD) {
@@ -268,12 +282,22 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                 const f2 xj = ld2(S.X + jp * 32), yj = ld2(S.Y + jp * 32), zj = ld2(S.Z + jp * 32);
                 f2 gjx = zero, gjy = zero, gjz = zero;
 #pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    if (tw.x & (0x100u << r)) {
-                        const float4 ra = rowp[0], rb = rowp[1];
-                        rowp += 2;
-                        pair_row<GRAD>(K, bc(xi[r]), bc(yi[r]), bc(zi[r]), xj, yj, zj, ra, rb, (tw.y >> (2 * r)) & 3u, e2,
-                                       gix[r], giy[r], giz[r], gjx, gjy, gjz);
+                for (int hf = 0; hf < 2; ++hf) {        // a half = two rows = two independent chains in one basic block
+                    if (tw.x & (0x100u << hf)) {
+                        const float4 ra0 = rowp[0], rb0 = rowp[1], ra1 = rowp[2], rb1 = rowp[3];
+                        rowp += 4;
+                        const int r0 = 2 * hf, r1 = 2 * hf + 1;
+                        if (!(tw.x & (0x400u << hf))) {
+                            pair_row<GRAD, false>(K, bc(xi[r0]), bc(yi[r0]), bc(zi[r0]), xj, yj, zj, ra0, rb0, 0u, e2,
+                                                  gix[r0], giy[r0], giz[r0], gjx, gjy, gjz);
+                            pair_row<GRAD, false>(K, bc(xi[r1]), bc(yi[r1]), bc(zi[r1]), xj, yj, zj, ra1, rb1, 0u, e2,
+                                                  gix[r1], giy[r1], giz[r1], gjx, gjy, gjz);
+                        } else {
+                            pair_row<GRAD, true>(K, bc(xi[r0]), bc(yi[r0]), bc(zi[r0]), xj, yj, zj, ra0, rb0, (tw.y >> (2 * r0)) & 3u,
+                                                 e2, gix[r0], giy[r0], giz[r0], gjx, gjy, gjz);
+                            pair_row<GRAD, true>(K, bc(xi[r1]), bc(yi[r1]), bc(zi[r1]), xj, yj, zj, ra1, rb1, (tw.y >> (2 * r1)) & 3u,
+                                                 e2, gix[r1], giy[r1], giz[r1], gjx, gjy, gjz);
+                        }
                     }
                 }
                 if (GRAD) {                             // J side: gradient gj at rel (xj,yj,zj) -> fragment sums

@@ -4,8 +4,10 @@
 // DFS preorder ("lane order"): every rigid fragment is a contiguous range and parents precede children.
 // The non-excluded pair list (R2) is cut into register tiles: an I-block of kLaneBI consecutive atoms
 // (kept in registers with their force accumulators) against one aligned J-pair (atoms 2m, 2m+1: the two halves
-// of a packed f32x2 operand).  A tile lists only its active rows; a slot of an active row whose pair is
-// excluded carries zero coefficients and contributes exactly zero.
+// of a packed f32x2 operand).  A tile is evaluated as two HALVES of two rows (rows 0-1, rows 2-3): the two rows of a
+// half are independent dependency chains issued in one basic block.  A tile lists only its active halves; a slot
+// whose pair is excluded (including a whole row of an active half) carries zero coefficients and contributes
+// exactly zero.
 #pragma once
 #include <algorithm>
 #include <cmath>
@@ -40,7 +42,8 @@ struct LaneBlock {              // 16 bytes: I atoms 4b .. 4b+3 of an active blo
     uint32_t frags;             // fragment id of row r in byte r
 };
 struct LaneTile {               // 8 bytes
-    uint32_t w0;                // jp | rowmask << 8 ; the row records of all tiles are consumed in sequence
+    uint32_t w0;                // jp | halfmask << 8 (bit 0: rows 0-1, bit 1: rows 2-3) | half-has-12-10-slot << 10 ;
+                                // each active half owns two consecutive row records, consumed in sequence
     uint32_t w1;                // hbmask (bit 2r+h) | frag(j0) << 16 | frag(j1) << 24
 };
 struct LaneRow {                // 32 bytes: one active row against the two J atoms (h = 0, 1)
@@ -83,12 +86,14 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
     std::vector<LaneBlock> blocks;
     std::vector<LaneTile> tiles;
     std::vector<LaneRow> rows;
-    int nslots = 0;
+    int npair_slots = 0;
     for (int b = 0; b < nblk_all; ++b) {
         LaneBlock blk{b, (int)tiles.size(), 0, 0};
         for (int r = 0; r < kLaneBI; ++r) blk.frags |= (uint32_t)frag_of_pos[b * kLaneBI + r] << (8 * r);
         for (int jp = 0; jp < njp; ++jp) {
-            uint32_t rowmask = 0, hbmask = 0;
+            uint32_t halfmask = 0, hbmask = 0, hbhalf = 0;
+            LaneRow trow[kLaneBI];
+            bool ron[kLaneBI];
             for (int r = 0; r < kLaneBI; ++r) {
                 const int I = b * kLaneBI + r;
                 LaneRow row{};
@@ -105,14 +110,18 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
                     row.ncA[h] = -co[1];
                     row.ds[h] = (float)((double)w_desolv * (Si * (double)vol[tj] + Sj * (double)vol[ti]));
                     row.qq[h] = (float)((double)elec_scale * (double)charge[s.ei] * (double)charge[s.ej]);
-                    if (co[2] > 8.0f) hbmask |= 1u << (2 * r + h);
-                    ++nslots;
+                    if (co[2] > 8.0f) { hbmask |= 1u << (2 * r + h); hbhalf |= 1u << (r / 2); }
+                    ++npair_slots;
                 }
-                if (any) { rowmask |= 1u << r; rows.push_back(row); }
+                trow[r] = row; ron[r] = any;
+                if (any) halfmask |= 1u << (r / 2);
             }
-            if (!rowmask) continue;
+            if (!halfmask) continue;
+            for (int hf = 0; hf < 2; ++hf)
+                if (halfmask & (1u << hf)) { rows.push_back(trow[2 * hf]); rows.push_back(trow[2 * hf + 1]); }
+            (void)ron;
             LaneTile t;
-            t.w0 = (uint32_t)jp | (rowmask << 8);
+            t.w0 = (uint32_t)jp | (halfmask << 8) | (hbhalf << 10);
             t.w1 = hbmask | ((uint32_t)frag_of_pos[2 * jp] << 16) | ((uint32_t)frag_of_pos[2 * jp + 1] << 24);
             tiles.push_back(t);
         }
@@ -135,7 +144,8 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
     h.off_tiles = (int)off;  off = align16(off + tiles.size() * sizeof(LaneTile));
     h.off_rows = (int)off;   off = align16(off + rows.size() * sizeof(LaneRow));
     h.bytes = (int)off;
-    h.nslots = nslots;                  // pair slots evaluated = 2 nrows; npairs of them carry a pair
+    h.nslots = 2 * (int)rows.size();    // pair slots evaluated; npairs of them carry a pair
+    (void)npair_slots;
     im.warp_floats = h.warp_floats;
     im.blob.assign(off, 0);
     std::memcpy(im.blob.data(), &h, sizeof(h));
