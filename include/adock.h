@@ -101,7 +101,8 @@ int adock_ligand_image(const adock_ligand* l, int* bytes, const unsigned char** 
 int adock_ligand_lane_image(const adock_ligand* l, int* bytes, const unsigned char** image, const int** pos_of_ext);
 
 /* Kernel family used by the compute entry points of this process: 0 = chosen by problem
- * size (default), 1 = one warp per individual, 2 = one thread (lane) per individual.  Both families compute
+ * size (default), 1 = one warp per individual, 2 = one lane per individual with K = 1, 2 or 4 warps sharing the
+ * work of each group of 32 individuals (K chosen by size; 21, 22, 24 force K = 1, 2, 4).  All of them compute
  * the same function (R3-R7) and pass the same parity tests; they differ in summation order only. */
 int adock_set_path(int path);
 /* Family (1 or 2) the local search of the last adock_dock / adock_dock_many on this thread ran in; 0 = none yet. */

@@ -271,11 +271,12 @@ def adock_profile_read() -> dict:
     return dict(ls_ms=ms.value, ls_launches=n.value, ls_evals=ev.value)
 
 
-PATHS = {"auto": 0, "warp": 1, "lane": 2}
+PATHS = {"auto": 0, "warp": 1, "lane": 2, "lane1": 21, "lane2": 22, "lane4": 24}
 
 
 def adock_set_path(path) -> None:
-    """kernel family: 'auto' (by problem size), 'warp' (warp per individual) or 'lane' (thread per individual)"""
+    """kernel family: 'auto' (by problem size), 'warp' (warp per individual), 'lane' (lane per individual, warps per
+    group of 32 individuals chosen by size) or 'lane1' / 'lane2' / 'lane4' (that number of warps per group)"""
     _check(lib().adock_set_path(PATHS[path] if isinstance(path, str) else int(path)))
 
 

@@ -31,12 +31,13 @@ struct adock_ligand {
     float w_desolv = 0, qasp = 0, elec_scale = 0;
     LaneImage lane;                         // image of the lane-per-individual kernels (lane_image.hpp)
     unsigned char* d_lane = nullptr;
-    int lane_bytes = 0, lane_warp_floats = 0;
+    int lane_bytes = 0, lane_npad = 0, lane_own = 0;      // group scratch = lane_group_floats(npad, own, R, K) per lane
 };
 
 static thread_local std::string g_err;
 static thread_local long long g_launches = 0;
-static int g_path = 0;                                    // adock_set_path: 0 auto, 1 warp-per-individual, 2 lane-per-individual
+static int g_path = 0;                                    // adock_set_path: 0 auto, 1 warp per individual, 2 lane per individual
+static int g_lane_k = 0;                                  // warps per lane group forced by adock_set_path(21|22|24); 0 = by size
 static thread_local bool g_prof = false;                  // adock_profile: time every dock_ls_kernel launch
 static thread_local double g_ls_ms = 0;
 static thread_local long long g_ls_launches = 0, g_ls_evals = 0;
@@ -195,7 +196,7 @@ extern "C" int adock_load_ligand(const adock_grids* grids, const adock_params* p
     l->w_desolv = p.w_desolv; l->qasp = p.qasp; l->elec_scale = p.elec_scale;
     build_lane_image(l->lane, l->tp, xyz, type, charge, pair_coeffs, solpar, vol, p.w_desolv, p.qasp, p.elec_scale);
     l->lane_bytes = (int)l->lane.blob.size();
-    l->lane_warp_floats = l->lane.warp_floats;
+    l->lane_npad = l->lane.npad; l->lane_own = l->lane.own_floats;
     l->blob_bytes = (int)l->tp.blob.size();
     l->scratch_floats = warp_scratch_floats(N, l->tp.nfrag, R);
     if (16 + l->blob_bytes + 4 * l->scratch_floats > 227 * 1024) {
@@ -265,8 +266,9 @@ extern "C" int adock_ligand_lane_image(const adock_ligand* l, int* bytes, const 
 extern "C" int adock_last_dock_path(void) { return g_last_dock_path; }
 
 extern "C" int adock_set_path(int path) {
-    if (path < 0 || path > 2) return fail(ADOCK_EINVAL, "path must be 0 (auto), 1 (warp per individual) or 2 (lane per individual)");
-    g_path = path;
+    if (path == 21 || path == 22 || path == 24) { g_path = 2; g_lane_k = path - 20; return ADOCK_OK; }
+    if (path < 0 || path > 2) return fail(ADOCK_EINVAL, "path must be 0 (auto), 1 (warp per individual), 2 (lane per individual) or 21/22/24");
+    g_path = path; g_lane_k = 0;
     return ADOCK_OK;
 }
 
@@ -324,73 +326,112 @@ __global__ void __launch_bounds__(256) score_kernel(GridDev G, ParDev P, ScoreAr
 
 
 // =================================================================== lane-per-individual geometry (lane.cuh)
-constexpr int kLaneMaxWarps = 8;
-static size_t lane_smem(int lane_bytes, int warp_floats, int warps) { return 16 + (size_t)lane_bytes + (size_t)warps * warp_floats * 128; }
-// largest warp count <= kLaneMaxWarps whose shared memory fits (0: not even one)
-static int lane_fit_warps(int lane_bytes, int warp_floats) {
-    int w = kLaneMaxWarps;
-    while (w > 0 && lane_smem(lane_bytes, warp_floats, w) > (size_t)g_smem_optin) --w;
-    return w;
+// A group of K warps shares 32 individuals.  Warps per CTA are bounded by the register file: 8 (K=1, 255 registers per
+// thread), 12 (K=2, 170), 16 (K=4, 128), and by the shared memory of the groups.
+template <int K> struct LaneCfg { static constexpr int kMaxWarps = K == 1 ? 8 : K == 2 ? 12 : 16; };
+static int lane_max_warps(int K) { return K == 1 ? 8 : K == 2 ? 12 : 16; }
+struct LaneGeom { int bytes, npad, own, R; };            // of the largest ligand of a launch
+static LaneGeom lane_geom(const adock_ligand* l) { return LaneGeom{l->lane_bytes, l->lane_npad, l->lane_own, l->tp.R}; }
+static LaneGeom lane_geom_max(LaneGeom a, LaneGeom b) {
+    return LaneGeom{std::max(a.bytes, b.bytes), std::max(a.npad, b.npad), std::max(a.own, b.own), std::max(a.R, b.R)};
+}
+static size_t lane_smem(const LaneGeom& g, int K, int groups) {
+    return 16 + (size_t)g.bytes + (size_t)groups * lane_group_floats(g.npad, g.own, g.R, K) * 128;
+}
+// most groups per CTA that fit (0: not even one)
+static int lane_fit_groups(const LaneGeom& g, int K) {
+    int n = lane_max_warps(K) / K;
+    while (n > 0 && lane_smem(g, K, n) > (size_t)g_smem_optin) --n;
+    return n;
 }
 // the lane kernels want at least one warp per scheduler
-static bool lane_ok(const adock_ligand* l) { return lane_fit_warps(l->lane_bytes, l->lane_warp_floats) >= 4; }
-// ADADELTA chains (threads) from which the lane-per-individual kernels are preferred over warp-per-individual:
-// one warp per scheduler (measured at 40 atoms: 18k chains is where the lane family overtakes, profiles/)
+static bool lane_ok(const adock_ligand* l) {
+    const LaneGeom g = lane_geom(l);
+    return lane_fit_groups(g, 1) >= 4 || lane_fit_groups(g, 2) >= 2 || lane_fit_groups(g, 4) >= 1;
+}
+// ADADELTA chains (threads) from which the lane-per-individual kernels are preferred over warp-per-individual
 constexpr int kLaneMinChains = 148 * 4 * 32;
-// few warps of work: fewer warps per CTA so that they spread over the SMs
-static int lane_spread_warps(int W, int nwarps) {
-    while (W > 1 && (long long)g_sm_count * W > (long long)nwarps) --W;
-    return W;
+// warps per group for `ngroups` groups of 32 individuals: the K that puts the most warps on the SMs; a forced K
+// (adock_set_path 21/22/24) wins if it fits
+static int lane_pick_k(const LaneGeom& g, long long ngroups) {
+    if (g_lane_k && lane_fit_groups(g, g_lane_k) > 0) return g_lane_k;
+    int best = 0;
+    double best_score = -1;
+    for (int K = 1; K <= 4; K *= 2) {
+        const int fit = lane_fit_groups(g, K);
+        if (!fit) continue;
+        // resident warps per SM when the groups are spread over the SMs, capped by what fits
+        const double per_sm = std::min<double>((double)fit, std::max(1.0, (double)ngroups / g_sm_count)) * K;
+        const double score = per_sm * (K == 1 ? 1.0 : K == 2 ? 0.97 : 0.93);     // redundant pose work of the extra parts
+        if (score > best_score) { best_score = score; best = K; }
+    }
+    return best;
+}
+// groups per CTA: as many as fit, fewer when that would leave SMs idle
+static int lane_spread_groups(int fit, long long ngroups) {
+    int n = fit;
+    while (n > 1 && (long long)g_sm_count * n > ngroups) --n;
+    return n;
 }
 
-template <bool GRAD>
-__global__ void __launch_bounds__(kLaneMaxWarps * 32, 1) score_lane_kernel(GridDev G, ParDev P, ScoreArgs a) {
+template <bool GRAD, int K>
+__global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) score_lane_kernel(GridDev G, ParDev P, ScoreArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char* blob = smem + 16;
     stage_ligand(blob, a.blob, a.blob_bytes, reinterpret_cast<uint64_t*>(smem), 0);
     const LaneL L = lane_view(blob);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
-    const int wf = reinterpret_cast<const LaneHeader*>(blob)->warp_floats;
-    const LaneS S = lane_scratch(reinterpret_cast<float*>(blob + a.blob_bytes) + (size_t)warp * wf * 32, L, lane);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, NG = (blockDim.x >> 5) / K;
+    const LaneS S = lane_scratch<K>(reinterpret_cast<float*>(blob + a.blob_bytes), L, warp, lane);
     const int Gn = 7 + L.R;
     const int nchunks = (a.n + 31) >> 5;
-    for (int c = blockIdx.x * W + warp; c < nchunks; c += gridDim.x * W) {
+    for (int c = blockIdx.x * NG + S.gid; c < nchunks; c += gridDim.x * NG) {
         const int idx = c * 32 + lane;
         const bool act = idx < a.n;
         const int src = act ? idx : a.n - 1;
-        for (int d = 0; d < Gn; ++d) S.geno[d * 32] = a.genos[(size_t)src * a.gstride + d];
+        if (S.part == 0)
+            for (int d = 0; d < Gn; ++d) S.geno[d * 32] = a.genos[(size_t)src * a.gstride + d];
+        group_sync<K>(S);
         float ei, ea;
         bool gf;
-        const float e = lane_eval<GRAD>(L, G, P, S, GRAD ? a.grads + (size_t)src * a.dstride : nullptr, 1, act, ei, ea, gf);
-        if (act) {
+        const float e = lane_eval<GRAD, K>(L, G, P, S, GRAD ? a.grads + (size_t)src * a.dstride : nullptr, 1, act, ei, ea, gf);
+        if (act && S.part == 0) {
             a.E[idx] = e;
             if (a.terms) { a.terms[2 * (size_t)idx] = ei; a.terms[2 * (size_t)idx + 1] = ea; }
         }
+        group_sync<K>(S);                               // part 0 is done with the positions and own[]
     }
+}
+
+template <bool GRAD, int K>
+static int launch_score_lane_k(const adock_grids* grids, const adock_ligand* lig, const ParDev& P, const ScoreArgs& a, int ngroups,
+                               cudaStream_t st) {
+    const LaneGeom g = lane_geom(lig);
+    const int NG = lane_spread_groups(lane_fit_groups(g, K), ngroups);
+    const size_t smem = lane_smem(g, K, NG);
+    const int grid = (int)std::max<long long>(1, std::min<long long>(((long long)ngroups + NG - 1) / NG, g_sm_count));
+    CUDA_TRY(cudaFuncSetAttribute(score_lane_kernel<GRAD, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    score_lane_kernel<GRAD, K><<<grid, NG * K * 32, smem, st>>>(grids->dev, P, a);
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    return ADOCK_OK;
 }
 
 static int launch_score_lane(const adock_grids* grids, const adock_ligand* lig, const adock_params& p, const float* d_genos, int n,
                              int gstride, float* d_E, float* d_terms, float* d_grads, int dstride, cudaStream_t st) {
-    const int nchunks = (n + 31) / 32;
-    int W = lane_fit_warps(lig->lane_bytes, lig->lane_warp_floats);
-    if (!W) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
-    // few chunks: spread them over the SMs (one warp per scheduler first)
-    while (W > 1 && (long long)g_sm_count * W > (long long)nchunks * 2 && W > 4) W >>= 1;
-    const size_t smem = lane_smem(lig->lane_bytes, lig->lane_warp_floats, W);
+    const int ngroups = (n + 31) / 32;
+    const int K = lane_pick_k(lane_geom(lig), ngroups);
+    if (!K) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
     ParDev P = make_pardev(p);
     P.k_wall_h = p.k_wall * grids->dev.h;
     ScoreArgs a{lig->d_lane, d_genos, d_E, d_terms, d_grads, lig->lane_bytes, n, gstride, dstride};
-    const int grid = (int)std::max<long long>(1, std::min<long long>(((long long)nchunks + W - 1) / W, g_sm_count));
     if (d_grads) {
-        CUDA_TRY(cudaFuncSetAttribute(score_lane_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        score_lane_kernel<true><<<grid, W * 32, smem, st>>>(grids->dev, P, a);
-    } else {
-        CUDA_TRY(cudaFuncSetAttribute(score_lane_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        score_lane_kernel<false><<<grid, W * 32, smem, st>>>(grids->dev, P, a);
+        if (K == 1) return launch_score_lane_k<true, 1>(grids, lig, P, a, ngroups, st);
+        if (K == 2) return launch_score_lane_k<true, 2>(grids, lig, P, a, ngroups, st);
+        return launch_score_lane_k<true, 4>(grids, lig, P, a, ngroups, st);
     }
-    ++g_launches;
-    CUDA_TRY(cudaGetLastError());
-    return ADOCK_OK;
+    if (K == 1) return launch_score_lane_k<false, 1>(grids, lig, P, a, ngroups, st);
+    if (K == 2) return launch_score_lane_k<false, 2>(grids, lig, P, a, ngroups, st);
+    return launch_score_lane_k<false, 4>(grids, lig, P, a, ngroups, st);
 }
 
 static int launch_score(const adock_grids* grids, const adock_ligand* lig, const adock_params& p, const float* d_genos, int n,
@@ -510,31 +551,57 @@ __global__ void __launch_bounds__(128) ls_array_kernel(GridDev G, ParDev P, LsAr
     }
 }
 
-// lane-per-individual variant: thread c runs chain c; ADADELTA state in global scratch columns [row][nthreads]
-__global__ void __launch_bounds__(kLaneMaxWarps * 32, 1) ls_array_lane_kernel(GridDev G, ParDev P, LsArgs a, float* __restrict__ scratch) {
+// lane-per-individual variant: lane c of the launch's groups runs chain c; ADADELTA state in global scratch columns
+// [row][all group lanes of the launch]
+template <int K>
+__global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) ls_array_lane_kernel(GridDev G, ParDev P, LsArgs a, float* __restrict__ scratch) {
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char* blob = smem + 16;
     stage_ligand(blob, a.blob, a.blob_bytes, reinterpret_cast<uint64_t*>(smem), 0);
     const LaneL L = lane_view(blob);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int wf = reinterpret_cast<const LaneHeader*>(blob)->warp_floats;
-    const LaneS S = lane_scratch(reinterpret_cast<float*>(blob + a.blob_bytes) + (size_t)warp * wf * 32, L, lane);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, NG = (blockDim.x >> 5) / K;
+    const LaneS S = lane_scratch<K>(reinterpret_cast<float*>(blob + a.blob_bytes), L, warp, lane);
     const int Gn = 7 + L.R, D = 6 + L.R;
-    const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, T = (size_t)gridDim.x * blockDim.x;
+    const size_t tid = ((size_t)blockIdx.x * NG + S.gid) * 32 + lane, T = (size_t)gridDim.x * NG * 32;
     const bool act = tid < (size_t)a.n;
     const size_t idx = act ? tid : (size_t)a.n - 1;
-    for (int d = 0; d < Gn; ++d) S.geno[d * 32] = a.genos[idx * a.gstride + d];
+    if (S.part == 0)
+        for (int d = 0; d < Gn; ++d) S.geno[d * 32] = a.genos[idx * a.gstride + d];
+    group_sync<K>(S);
     LaneLS ls;
     ls.best = scratch + tid; ls.Eg2 = ls.best + (size_t)Gn * T; ls.Ed2 = ls.Eg2 + (size_t)D * T; ls.grad = ls.Ed2 + (size_t)D * T;
     ls.stride = (int)T;
     int iters = 0;
-    const float e = lane_adadelta(L, G, P, S, ls, act, __int_as_float(0x7fc00000), iters,
-                                  a.trace ? a.trace + idx * P.lsit : nullptr, 1);
-    if (act) {
+    const float e = lane_adadelta<K>(L, G, P, S, ls, act, __int_as_float(0x7fc00000), iters,
+                                     a.trace ? a.trace + idx * P.lsit : nullptr, 1);
+    if (act && S.part == 0) {
         for (int d = 0; d < Gn; ++d) a.genos[idx * a.gstride + d] = ls.best[(size_t)d * T];
         a.E[idx] = e;
         if (a.iters) a.iters[idx] = iters;
     }
+}
+
+template <int K>
+static int launch_ls_array_lane(const adock_grids* grids, const adock_ligand* ligand, const ParDev& P, LsArgs a, int n, cudaStream_t stm) {
+    const LaneGeom g = lane_geom(ligand);
+    const int ngroups = (n + 31) / 32;
+    const int NG = lane_spread_groups(lane_fit_groups(g, K), ngroups);
+    const int grid = (ngroups + NG - 1) / NG;
+    const size_t smem = lane_smem(g, K, NG);
+    const size_t T = (size_t)grid * NG * 32;
+    const int R = ligand->tp.R;
+    float* scratch = nullptr;
+    cudaError_t e = cudaMallocAsync(&scratch, T * (size_t)(7 + R + 3 * (6 + R)) * 4, stm);
+    if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("ls scratch: ") + cudaGetErrorString(e));
+    e = cudaFuncSetAttribute(ls_array_lane_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) {
+        ls_array_lane_kernel<K><<<grid, NG * K * 32, smem, stm>>>(grids->dev, P, a, scratch);
+        ++g_launches;
+        e = cudaGetLastError();
+    }
+    cudaFreeAsync(scratch, stm);
+    if (e != cudaSuccess) return fail(ADOCK_ECUDA, std::string("ls_array_lane_kernel: ") + cudaGetErrorString(e));
+    return ADOCK_OK;
 }
 
 extern "C" int adock_local_search(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
@@ -550,28 +617,15 @@ extern "C" int adock_local_search(const adock_grids* grids, const adock_ligand* 
     rc = device_props();
     if (rc) return rc;
     if (g_path == 2 || (g_path == 0 && n >= kLaneMinChains && lane_ok(ligand))) {
-        int W = lane_fit_warps(ligand->lane_bytes, ligand->lane_warp_floats);
-        if (!W) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
-        const int nwarps = (n + 31) / 32;
-        W = lane_spread_warps(W, nwarps);
-        const int grid = (nwarps + W - 1) / W;
-        const size_t smem = lane_smem(ligand->lane_bytes, ligand->lane_warp_floats, W);
-        const size_t T = (size_t)grid * W * 32;
-        const int R = ligand->tp.R;
-        float* scratch = nullptr;
-        cudaStream_t stm = (cudaStream_t)cuda_stream;
-        cudaError_t e = cudaMallocAsync(&scratch, T * (size_t)(7 + R + 3 * (6 + R)) * 4, stm);
-        if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("ls scratch: ") + cudaGetErrorString(e));
-        CUDA_TRY(cudaFuncSetAttribute(ls_array_lane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        const int K = lane_pick_k(lane_geom(ligand), (n + 31) / 32);
+        if (!K) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
         ParDev P = make_pardev(p);
         P.k_wall_h = p.k_wall * grids->dev.h;
         LsArgs a{ligand->d_lane, d_genotypes, d_energies, d_iters, d_trace, ligand->lane_bytes, n, gstride};
-        ls_array_lane_kernel<<<grid, W * 32, smem, stm>>>(grids->dev, P, a, scratch);
-        ++g_launches;
-        e = cudaGetLastError();
-        cudaFreeAsync(scratch, stm);
-        if (e != cudaSuccess) return fail(ADOCK_ECUDA, std::string("ls_array_lane_kernel: ") + cudaGetErrorString(e));
-        return ADOCK_OK;
+        cudaStream_t stm = (cudaStream_t)cuda_stream;
+        if (K == 1) return launch_ls_array_lane<1>(grids, ligand, P, a, n, stm);
+        if (K == 2) return launch_ls_array_lane<2>(grids, ligand, P, a, n, stm);
+        return launch_ls_array_lane<4>(grids, ligand, P, a, n, stm);
     }
     const int W = fit_warps(ligand->blob_bytes, ligand->scratch_floats, 4);
     if (!W) return fail(ADOCK_ELIMIT, "ligand does not fit in shared memory");
@@ -738,39 +792,41 @@ __global__ void __launch_bounds__(128) dock_ls_kernel(GridDev G, ParDev P, const
     }
 }
 
-// the same step, lane-per-individual: thread c of a job runs chain c = run*n_ls + l; every CTA stages its job's lane
-// image; ADADELTA state in global scratch columns [row][all threads of the launch] (rows: Gmax best, 3 x Dmax)
-__global__ void __launch_bounds__(kLaneMaxWarps * 32, 1) dock_ls_lane_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs,
-                                                                             DockDims dm, float* __restrict__ scratch, int Gmax) {
+// the same step, lane-per-individual: lane c of a job's groups runs chain c = run*n_ls + l; every CTA stages its job's
+// lane image; ADADELTA state in global scratch columns [row][all group lanes of the launch] (rows: Gmax best, 3 x Dmax)
+template <int K>
+__global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_ls_lane_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs,
+                                                                                     DockDims dm, float* __restrict__ scratch, int Gmax) {
     extern __shared__ __align__(128) unsigned char smem[];
     const DockJob job = jobs[blockIdx.x / dm.upj];
     unsigned char* blob = smem + 16;
     stage_ligand(blob, job.lane, job.lane_bytes, reinterpret_cast<uint64_t*>(smem), 0);
     const LaneL L = lane_view(blob);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int wf = reinterpret_cast<const LaneHeader*>(blob)->warp_floats;
-    const LaneS S = lane_scratch(reinterpret_cast<float*>(blob + job.lane_bytes) + (size_t)warp * wf * 32, L, lane);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, NG = (blockDim.x >> 5) / K;
+    const LaneS S = lane_scratch<K>(reinterpret_cast<float*>(blob + job.lane_bytes), L, warp, lane);
     const int Gn = job.Gn;
-    const int c = (blockIdx.x % dm.upj) * blockDim.x + threadIdx.x;
+    const int c = ((blockIdx.x % dm.upj) * NG + S.gid) * 32 + lane;
     bool act = c < dm.nrun * dm.n_ls;
     const int cc = act ? c : 0;
     const int run = cc / dm.n_ls, l = cc % dm.n_ls;
     const RunState st = job.st[run];
     act = act && st.active;
-    if (!__any_sync(kFull, act)) return;
+    if (!__any_sync(kFull, act)) return;                // the same for every warp of the group
     const size_t popsz = (size_t)dm.nrun * dm.P;
     const int slot = job.picks[(size_t)run * dm.P + l];
     float* g = job.pop + ((size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P + slot) * Gn;
     float* e = job.E + (size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P + slot;
-    for (int d = 0; d < Gn; ++d) S.geno[d * 32] = g[d];
-    const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, T = (size_t)gridDim.x * blockDim.x;
+    if (S.part == 0)
+        for (int d = 0; d < Gn; ++d) S.geno[d * 32] = g[d];
+    group_sync<K>(S);
+    const size_t tid = ((size_t)blockIdx.x * NG + S.gid) * 32 + lane, T = (size_t)gridDim.x * NG * 32;
     const int Dmax = Gmax - 1;
     LaneLS ls;
     ls.best = scratch + tid; ls.Eg2 = ls.best + (size_t)Gmax * T; ls.Ed2 = ls.Eg2 + (size_t)Dmax * T; ls.grad = ls.Ed2 + (size_t)Dmax * T;
     ls.stride = (int)T;
     int iters = 0;
-    const float be = lane_adadelta(L, G, P, S, ls, act, act ? *e : 0.f, iters, nullptr, 0);
-    if (act) {
+    const float be = lane_adadelta<K>(L, G, P, S, ls, act, (act && S.part == 0) ? *e : 0.f, iters, nullptr, 0);
+    if (act && S.part == 0) {
         for (int d = 0; d < Gn; ++d) g[d] = ls.best[(size_t)d * T];
         *e = be;
         atomicAdd(&job.st[run].ls_acc, iters);
@@ -875,19 +931,18 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     // local search: lane-per-individual when there are enough chains to fill the SMs with whole warps
     const int n_ls0 = n_ls_of(p, Pn);
     const long long chains = (long long)nlig * nrun * n_ls0;
-    int maxlane = 0, maxwf = 0, Gmax = 7;
+    LaneGeom lg{0, 0, 0, 0};
+    int Gmax = 7;
     bool lanes_fit = true;
     for (int l = 0; l < nlig; ++l) {
-        maxlane = std::max(maxlane, ligs[l]->lane_bytes);
-        maxwf = std::max(maxwf, ligs[l]->lane_warp_floats);
+        lg = lane_geom_max(lg, lane_geom(ligs[l]));
         Gmax = std::max(Gmax, 7 + ligs[l]->tp.R);
         lanes_fit = lanes_fit && lane_ok(ligs[l]);
     }
-    int Wlane = 0;
-    for (int w = kLaneMaxWarps; w > 0 && !Wlane; --w)
-        if (lane_smem(maxlane, maxwf, w) <= (size_t)g_smem_optin) Wlane = w;
-    const bool ls_lane = Wlane > 0 && (g_path == 2 || (g_path == 0 && lanes_fit && chains >= kLaneMinChains));
-    if (g_path == 2 && !Wlane) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
+    const int jg = (nrun * n_ls0 + 31) / 32;                        // groups of 32 chains per job
+    const int Klane = lane_pick_k(lg, (long long)nlig * jg);
+    const bool ls_lane = Klane > 0 && (g_path == 2 || (g_path == 0 && lanes_fit && chains >= kLaneMinChains));
+    if (g_path == 2 && !Klane) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
     g_last_dock_path = ls_lane ? 2 : 1;
     ParDev P = make_pardev(p);
     P.k_wall_h = p.k_wall * grids->dev.h;
@@ -941,23 +996,28 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     dga.upj = (int)((popsz + Wga - 1) / Wga);
     dls.upj = std::max(1, (nrun * dm.n_ls + Wls - 1) / Wls);
     dfin.upj = (nrun + Wls - 1) / Wls;
-    // lane family: warps of a job's chains split evenly over the fewest CTAs that fit
+    // lane family: the groups of a job's chains split evenly over the fewest CTAs that fit
     DockDims dll = dm;
-    int Wl = 1;
+    int NGl = 1;
     size_t smem_ll = 0;
     float* d_lscratch = nullptr;
     if (ls_lane && dm.n_ls > 0) {
-        const int jw = (nrun * dm.n_ls + 31) / 32;                  // warps per job
-        dll.upj = (jw + Wlane - 1) / Wlane;
-        Wl = (jw + dll.upj - 1) / dll.upj;
-        smem_ll = lane_smem(maxlane, maxwf, Wl);
-        const size_t T = (size_t)nlig * dll.upj * Wl * 32;
+        const int fit = lane_fit_groups(lg, Klane);
+        dll.upj = (jg + fit - 1) / fit;
+        NGl = (jg + dll.upj - 1) / dll.upj;
+        smem_ll = lane_smem(lg, Klane, NGl);
+        const size_t T = (size_t)nlig * dll.upj * NGl * 32;
         cudaError_t e2 = buf.alloc(&d_lscratch, T * (size_t)(Gmax + 3 * (Gmax - 1)) * 4);
         if (e2 != cudaSuccess) return fail(e2 == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("dock alloc: ") + cudaGetErrorString(e2));
-        CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ll));
+        if (Klane == 1) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ll));
+        if (Klane == 2) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ll));
+        if (Klane == 4) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ll));
     }
     auto launch_ls = [&]() {
-        if (ls_lane) dock_ls_lane_kernel<<<dll.upj * nlig, Wl * 32, smem_ll, stm>>>(grids->dev, P, d_jobs, dll, d_lscratch, Gmax);
+        const int thr = NGl * Klane * 32;
+        if (ls_lane && Klane == 1) dock_ls_lane_kernel<1><<<dll.upj * nlig, thr, smem_ll, stm>>>(grids->dev, P, d_jobs, dll, d_lscratch, Gmax);
+        else if (ls_lane && Klane == 2) dock_ls_lane_kernel<2><<<dll.upj * nlig, thr, smem_ll, stm>>>(grids->dev, P, d_jobs, dll, d_lscratch, Gmax);
+        else if (ls_lane) dock_ls_lane_kernel<4><<<dll.upj * nlig, thr, smem_ll, stm>>>(grids->dev, P, d_jobs, dll, d_lscratch, Gmax);
         else dock_ls_kernel<<<dls.upj * nlig, Wls * 32, smem_ls, stm>>>(grids->dev, P, d_jobs, dls);
     };
     dock_init_kernel<<<dga.upj * nlig, Wga * 32, smem_ga, stm>>>(grids->dev, P, d_jobs, dga);

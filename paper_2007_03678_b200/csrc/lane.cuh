@@ -1,11 +1,14 @@
 // lane.cuh -- lane-per-individual device code of the hot path.
-// One THREAD evaluates one genotype: pose (R3), grid term (R4), intramolecular pairs (R5), back-propagation (R6)
-// and the ADADELTA chain (R7).  The 32 lanes of a warp hold 32 individuals of the SAME ligand, so the ligand image
+// One LANE holds one genotype: pose (R3), grid term (R4), intramolecular pairs (R5), back-propagation (R6) and the
+// ADADELTA chain (R7).  The 32 lanes of a warp hold 32 individuals of the SAME ligand, so the ligand image
 // (lane_image.hpp) is read from shared memory by broadcast, control flow is warp-uniform, and no shuffle, atomic or
-// cross-lane reduction is needed anywhere.  Per-thread state lives in shared memory as [index][lane] columns
+// cross-lane reduction is needed anywhere.  Per-lane state lives in shared memory as [index][lane] columns
 // (conflict-free): atom positions relative to the translation, and per-fragment (force, torque) accumulators.
-// The pair loop keeps an I-block of 4 atoms in registers and evaluates each active row against an aligned J-pair
-// with packed f32x2 arithmetic (FFMA2/FMUL2/FADD2: two pairs per instruction issue).
+// A GROUP of K warps (K = 1, 2, 4) works on the same 32 individuals: the atoms of the grid phase and the parts of the
+// pair-tile sequence are dealt out to the K warps, each accumulating into its own (force, torque) columns; part 0 adds
+// them up and runs the serial tail.  More warps per individual = more warps per SM for the same shared memory (the
+// positions are shared) and shorter chains.  The pair loop keeps an I-block of 4 atoms in registers and evaluates
+// two rows at a time against an aligned J-pair with packed f32x2 arithmetic (FFMA2/FMUL2/FADD2).
 #pragma once
 #include "device.cuh"
 #include "lane_image.hpp"
@@ -34,6 +37,8 @@ struct LaneL {              // the staged image
     const uint2* tiles;
     const float4* rows;
     int N, Npad, R, nfrag, nblocks, own_floats;
+    const int* part_blk;    // [kLaneParts+1]
+    const int* part_row;    // [kLaneParts+1]
 };
 __device__ inline LaneL lane_view(const unsigned char* blob) {
     const LaneHeader* h = reinterpret_cast<const LaneHeader*>(blob);
@@ -45,22 +50,40 @@ __device__ inline LaneL lane_view(const unsigned char* blob) {
     L.tiles = reinterpret_cast<const uint2*>(blob + h->off_tiles);
     L.rows = reinterpret_cast<const float4*>(blob + h->off_rows);
     L.N = h->N; L.Npad = h->Npad; L.R = h->R; L.nfrag = h->nfrag; L.nblocks = h->nblocks; L.own_floats = h->own_floats;
+    L.part_blk = h->part_blk; L.part_row = h->part_row;
     return L;
 }
-struct LaneS {              // this thread's columns of the warp's scratch; element k of an array sits at [k*32]
+struct LaneS {              // this lane's columns of the group's scratch; element k of an array sits at [k*32]
     float2* X; float2* Y; float2* Z;    // [Npad/2]: positions RELATIVE TO t of atoms 2m (.x) and 2m+1 (.y)
-    float* own;             // [own_floats]: per fragment F(3), T(3) about t; during the pose: the transform stack
+    float* own;             // [own_floats] of THIS part: per fragment F(3), T(3) about t; during the pose: the transform stack
+    float* own0;            // part 0's (the K parts' arrays are consecutive, own_floats*32 apart)
     float* geno;            // [7+R]
+    float* ex;              // [2K+1]: (e_grid, e_pairs) of each part, then the chain's live flag
+    int part, gid;          // this warp's part in the group; group index in the CTA (named barrier gid+1)
 };
-__device__ inline LaneS lane_scratch(float* warp_base, const LaneL& L, int lane) {
+// floats per lane of one group's scratch
+__host__ __device__ inline int lane_group_floats(int Npad, int own_floats, int R, int K) {
+    return 3 * Npad + K * own_floats + (7 + R) + 2 * K + 1;
+}
+template <int K>
+__device__ inline LaneS lane_scratch(float* cta_base, const LaneL& L, int warp, int lane) {
     LaneS S;
+    S.gid = warp / K; S.part = warp % K;
+    float* base = cta_base + (size_t)S.gid * lane_group_floats(L.Npad, L.own_floats, L.R, K) * 32;
     const int half = L.Npad / 2;
-    S.X = reinterpret_cast<float2*>(warp_base) + lane;
+    S.X = reinterpret_cast<float2*>(base) + lane;
     S.Y = S.X + half * 32;
     S.Z = S.Y + half * 32;
-    S.own = warp_base + 3 * L.Npad * 32 + lane;
-    S.geno = S.own + L.own_floats * 32;
+    S.own0 = base + 3 * L.Npad * 32 + lane;
+    S.own = S.own0 + S.part * L.own_floats * 32;
+    S.geno = S.own0 + K * L.own_floats * 32;
+    S.ex = S.geno + (7 + L.R) * 32;
     return S;
+}
+// barrier of the K warps of a group
+template <int K>
+__device__ __forceinline__ void group_sync(const LaneS& S) {
+    if (K > 1) asm volatile("bar.sync %0, %1;" ::"r"(S.gid + 1), "r"(K * 32) : "memory");
 }
 
 // ---------------------------------------------------------------- one packed row of the pair tile (R5)
@@ -139,10 +162,21 @@ __device__ __forceinline__ void own_add(float* own, int f, float Fx, float Fy, f
     o[0] += Fx; o[32] += Fy; o[64] += Fz; o[96] += Tx; o[128] += Ty; o[160] += Tz;
 }
 
-// ---------------------------------------------------------------- full evaluation of this thread's genotype
-// Reads S.geno.  GRAD: writes grad[d*gs] for d < 6+R when `wr`, and clears `gfin` if a component is not finite.
-// Returns the total energy (NaN for |q| < 1e-12, with NaN gradient).  Every lane of the warp must call.
-template <bool GRAD>
+// flush a fragment's (force, torque) sums: one warp per group visits every fragment exactly once (store); with K > 1 a
+// part may skip fragments, so own[] is zeroed first and the sums are added
+template <int K>
+__device__ __forceinline__ void own_flush(float* own, int f, float Fx, float Fy, float Fz, float Tx, float Ty, float Tz) {
+    float* o = own + f * 6 * 32;
+    if (K == 1) { o[0] = Fx; o[32] = Fy; o[64] = Fz; o[96] = Tx; o[128] = Ty; o[160] = Tz; }
+    else { o[0] += Fx; o[32] += Fy; o[64] += Fz; o[96] += Tx; o[128] += Ty; o[160] += Tz; }
+}
+
+// ---------------------------------------------------------------- full evaluation of this lane's genotype
+// Called by all K warps of the group with S.geno ready (and visible to all of them).  Part 0 returns the total energy
+// (NaN for |q| < 1e-12, with NaN gradient) and, with GRAD, writes grad[d*gs] for d < 6+R when `wr` and clears `gfin`
+// if a component is not finite; the other parts return 0.  The caller must group_sync before S.geno, the positions
+// or own[] are touched again (part 0 still reads them in its tail).
+template <bool GRAD, int K>
 __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, const ParDev& P, const LaneS& S, float* grad, int gs,
                                            bool wr, float& e_inter, float& e_intra, bool& gfin) {
     const float tx = S.geno[0], ty = S.geno[32], tz = S.geno[64];
@@ -196,6 +230,7 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                 st[256] = m20; st[288] = m21; st[320] = m22; st[352] = m23;
             }
             for (int i = fi.z; i < fi.w; ++i) {
+                if (K > 1 && ((i >> 2) % K) != S.part) continue;   // atoms are dealt out by grid step (4 atoms)
                 const float4 a = L.atoms[i];
                 const int o = (i >> 1) * 64 + (i & 1);
                 Xf[o] = fmaf(m00, a.x, fmaf(m01, a.y, fmaf(m02, a.z, m03)));
@@ -204,6 +239,7 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
             }
         }
         for (int i = L.N; i < L.Npad; ++i) {            // pad atoms: finite, in no pair
+            if (K > 1 && ((i >> 2) % K) != S.part) continue;
             const int o = (i >> 1) * 64 + (i & 1);
             Xf[o] = 0.f; Yf[o] = 0.f; Zf[o] = 0.f;
         }
@@ -214,9 +250,11 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
     // gradient goes straight into the (force, torque about t) sums of the atom's fragment, which initialises own[]
     float eg = 0.f;
     {
+        if (GRAD && K > 1)
+            for (int d = 0; d < 6 * L.nfrag; ++d) S.own[d * 32] = 0.f;
         float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
         int cur = 0;
-        for (int m = 0; m < L.Npad / 2; m += 2) {
+        for (int m = 2 * S.part; m < L.Npad / 2; m += 2 * K) {
             int tt[4];
             float q[4], rx[4], ry[4], rz[4];
             GridCell gc[4];
@@ -246,8 +284,7 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                 if (GRAD) {
                     const int f = tt[a] >> 8;
                     if (f != cur) {
-                        float* o = S.own + cur * 6 * 32;
-                        o[0] = Fx; o[32] = Fy; o[64] = Fz; o[96] = Tx; o[128] = Ty; o[160] = Tz;
+                        own_flush<K>(S.own, cur, Fx, Fy, Fz, Tx, Ty, Tz);
                         Fx = Fy = Fz = Tx = Ty = Tz = 0.f; cur = f;
                     }
                     Fx += gx; Fy += gy; Fz += gz;
@@ -255,19 +292,17 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                 }
             }
         }
-        if (GRAD) {
-            float* o = S.own + cur * 6 * 32;
-            o[0] = Fx; o[32] = Fy; o[64] = Fz; o[96] = Tx; o[128] = Ty; o[160] = Tz;
-        }
+        if (GRAD) own_flush<K>(S.own, cur, Fx, Fy, Fz, Tx, Ty, Tz);
     }
+    group_sync<K>(S);                                   // every part's positions are in place
 
-    // (a3) intramolecular pairs: register tiles
+    // (a3) intramolecular pairs: register tiles; this warp's parts of the tile sequence
     f2 e2 = bc(0.f);
-    {
-        const PairK K = make_pairk(P);
-        const float4* rowp = L.rows;
+    for (int part = S.part; part < kLaneParts; part += K) {
+        const PairK PK = make_pairk(P);
+        const float4* rowp = L.rows + 2 * L.part_row[part];
         const f2 zero = bc(0.f);
-        for (int kb = 0; kb < L.nblocks; ++kb) {
+        for (int kb = L.part_blk[part]; kb < L.part_blk[part + 1]; ++kb) {
             const int4 blk = L.blocks[kb];              // b, tile_begin, tile_end, frags
             const float2 xa = S.X[(2 * blk.x) * 32], xb = S.X[(2 * blk.x + 1) * 32];
             const float2 ya = S.Y[(2 * blk.x) * 32], yb = S.Y[(2 * blk.x + 1) * 32];
@@ -288,14 +323,14 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                         rowp += 4;
                         const int r0 = 2 * hf, r1 = 2 * hf + 1;
                         if (!(tw.x & (0x400u << hf))) {
-                            pair_row<GRAD, false>(K, bc(xi[r0]), bc(yi[r0]), bc(zi[r0]), xj, yj, zj, ra0, rb0, 0u, e2,
+                            pair_row<GRAD, false>(PK, bc(xi[r0]), bc(yi[r0]), bc(zi[r0]), xj, yj, zj, ra0, rb0, 0u, e2,
                                                   gix[r0], giy[r0], giz[r0], gjx, gjy, gjz);
-                            pair_row<GRAD, false>(K, bc(xi[r1]), bc(yi[r1]), bc(zi[r1]), xj, yj, zj, ra1, rb1, 0u, e2,
+                            pair_row<GRAD, false>(PK, bc(xi[r1]), bc(yi[r1]), bc(zi[r1]), xj, yj, zj, ra1, rb1, 0u, e2,
                                                   gix[r1], giy[r1], giz[r1], gjx, gjy, gjz);
                         } else {
-                            pair_row<GRAD, true>(K, bc(xi[r0]), bc(yi[r0]), bc(zi[r0]), xj, yj, zj, ra0, rb0, (tw.y >> (2 * r0)) & 3u,
+                            pair_row<GRAD, true>(PK, bc(xi[r0]), bc(yi[r0]), bc(zi[r0]), xj, yj, zj, ra0, rb0, (tw.y >> (2 * r0)) & 3u,
                                                  e2, gix[r0], giy[r0], giz[r0], gjx, gjy, gjz);
-                            pair_row<GRAD, true>(K, bc(xi[r1]), bc(yi[r1]), bc(zi[r1]), xj, yj, zj, ra1, rb1, (tw.y >> (2 * r1)) & 3u,
+                            pair_row<GRAD, true>(PK, bc(xi[r1]), bc(yi[r1]), bc(zi[r1]), xj, yj, zj, ra1, rb1, (tw.y >> (2 * r1)) & 3u,
                                                  e2, gix[r1], giy[r1], giz[r1], gjx, gjy, gjz);
                         }
                     }
@@ -334,7 +369,20 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
     }
     e_inter = eg;
     e_intra = hsum(e2);
-    float e = eg + e_intra;
+    if (K > 1) {                                        // hand the partial sums to part 0
+        S.ex[(2 * S.part) * 32] = e_inter; S.ex[(2 * S.part + 1) * 32] = e_intra;
+        group_sync<K>(S);
+        if (S.part != 0) { gfin = true; return 0.f; }
+        e_inter = 0.f; e_intra = 0.f;
+        for (int k = 0; k < K; ++k) { e_inter += S.ex[(2 * k) * 32]; e_intra += S.ex[(2 * k + 1) * 32]; }
+        if (GRAD)
+            for (int d = 0; d < 6 * L.nfrag; ++d) {
+                float v = S.own0[d * 32];
+                for (int k = 1; k < K; ++k) v += S.own0[(k * L.own_floats + d) * 32];
+                S.own0[d * 32] = v;
+            }
+    }
+    float e = e_inter + e_intra;
     const float qnan = __int_as_float(0x7fc00000);
     if (badq) { e = qnan; e_inter = qnan; e_intra = qnan; }
 
@@ -381,53 +429,64 @@ struct LaneLS {             // global scratch columns of this thread: element d 
     int stride;
 };
 
-// Start genotype in S.geno.  On return ls.best holds the best genotype seen; returns its energy (e_start if no finite
-// evaluation happened).  `active` lanes run the chain; the others only keep the warp's control flow uniform.
+// Start genotype in S.geno (visible to the whole group).  Called by all K warps of the group; part 0 owns the chain's
+// state (ls, in global scratch columns) and on return ls.best holds the best genotype seen; part 0 returns its energy
+// (e_start if no finite evaluation happened) and the evaluations done.  `active` lanes run the chain; the others only
+// keep the warp's control flow uniform.
+template <int K>
 __device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const ParDev& P, const LaneS& S, const LaneLS& ls,
                                       bool active, float e_start, int& iters, float* trace, int trace_stride) {
     const int R = L.R, D = 6 + R, Gn = 7 + R;
+    const bool lead = S.part == 0;
     float bestE = __int_as_float(0x7f800000);
-    for (int d = 0; d < Gn; ++d) ls.best[d * ls.stride] = S.geno[d * 32];
-    for (int d = 0; d < D; ++d) { ls.Eg2[d * ls.stride] = 0.f; ls.Ed2[d * ls.stride] = 0.f; }
+    if (lead) {
+        for (int d = 0; d < Gn; ++d) ls.best[d * ls.stride] = S.geno[d * 32];
+        for (int d = 0; d < D; ++d) { ls.Eg2[d * ls.stride] = 0.f; ls.Ed2[d * ls.stride] = 0.f; }
+    }
     bool live = active;
     int it = 0;
     iters = 0;
     for (; it < P.lsit; ++it) {
-        if (!__any_sync(kFull, live)) break;
+        if (!__any_sync(kFull, live)) break;            // same decision in every warp of the group
         float ei, ea;
         bool gfin = true;
-        const float e = lane_eval<true>(L, G, P, S, ls.grad, ls.stride, true, ei, ea, gfin);
-        if (live) {
-            if (trace) trace[it * trace_stride] = e;
-            ++iters;
-            if (!(isfinite(e) && gfin)) live = false;
-        }
-        if (live) {
-            if (e < bestE) {
-                bestE = e;
-                for (int d = 0; d < Gn; ++d) ls.best[d * ls.stride] = S.geno[d * 32];
+        const float e = lane_eval<true, K>(L, G, P, S, ls.grad, ls.stride, true, ei, ea, gfin);
+        if (lead) {
+            if (live) {
+                if (trace) trace[it * trace_stride] = e;
+                ++iters;
+                if (!(isfinite(e) && gfin)) live = false;
             }
-            float w[3] = {0.f, 0.f, 0.f};
-            for (int d = 0; d < D; ++d) {
-                const float g = ls.grad[d * ls.stride];
-                const float eg2 = P.ad_rho * ls.Eg2[d * ls.stride] + (1.f - P.ad_rho) * g * g;
-                const float ed2o = ls.Ed2[d * ls.stride];
-                const float dl = -(sqrtf(ed2o + P.ad_eps) / sqrtf(eg2 + P.ad_eps)) * g;
-                ls.Eg2[d * ls.stride] = eg2;
-                ls.Ed2[d * ls.stride] = P.ad_rho * ed2o + (1.f - P.ad_rho) * dl * dl;
-                if (d < 3) S.geno[d * 32] += dl;
-                else if (d < 6) { if (d == 3) w[0] = dl; else if (d == 4) w[1] = dl; else w[2] = dl; }
-                else S.geno[(d + 1) * 32] = wrap_pi(S.geno[(d + 1) * 32] + dl);
+            if (live) {
+                if (e < bestE) {
+                    bestE = e;
+                    for (int d = 0; d < Gn; ++d) ls.best[d * ls.stride] = S.geno[d * 32];
+                }
+                float w[3] = {0.f, 0.f, 0.f};
+                for (int d = 0; d < D; ++d) {
+                    const float g = ls.grad[d * ls.stride];
+                    const float eg2 = P.ad_rho * ls.Eg2[d * ls.stride] + (1.f - P.ad_rho) * g * g;
+                    const float ed2o = ls.Ed2[d * ls.stride];
+                    const float dl = -(sqrtf(ed2o + P.ad_eps) / sqrtf(eg2 + P.ad_eps)) * g;
+                    ls.Eg2[d * ls.stride] = eg2;
+                    ls.Ed2[d * ls.stride] = P.ad_rho * ed2o + (1.f - P.ad_rho) * dl * dl;
+                    if (d < 3) S.geno[d * 32] += dl;
+                    else if (d < 6) { if (d == 3) w[0] = dl; else if (d == 4) w[1] = dl; else w[2] = dl; }
+                    else S.geno[(d + 1) * 32] = wrap_pi(S.geno[(d + 1) * 32] + dl);
+                }
+                const float th = sqrtf(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
+                float sh, ch;
+                sincosf(0.5f * th, &sh, &ch);
+                const float k = th > 1e-12f ? sh / th : 0.5f;
+                const float q[4] = {S.geno[96], S.geno[128], S.geno[160], S.geno[192]};
+                float nq[4];
+                rotate_quat(ch, k * w[0], k * w[1], k * w[2], q, nq);
+                S.geno[96] = nq[0]; S.geno[128] = nq[1]; S.geno[160] = nq[2]; S.geno[192] = nq[3];
             }
-            const float th = sqrtf(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
-            float sh, ch;
-            sincosf(0.5f * th, &sh, &ch);
-            const float k = th > 1e-12f ? sh / th : 0.5f;
-            const float q[4] = {S.geno[96], S.geno[128], S.geno[160], S.geno[192]};
-            float nq[4];
-            rotate_quat(ch, k * w[0], k * w[1], k * w[2], q, nq);
-            S.geno[96] = nq[0]; S.geno[128] = nq[1]; S.geno[160] = nq[2]; S.geno[192] = nq[3];
+            if (K > 1) S.ex[(2 * K) * 32] = live ? 1.f : 0.f;
         }
+        group_sync<K>(S);                               // new genotype and live flag visible; part 0 is done with own[]
+        if (K > 1) live = S.ex[(2 * K) * 32] != 0.f;
     }
     return isfinite(bestE) ? bestE : e_start;
 }

@@ -20,15 +20,21 @@
 namespace adock {
 
 constexpr int kLaneBI = 4;      // rows (I atoms) per register block
+constexpr int kLaneParts = 4;   // the tile sequence is cut into this many runs of (nearly) equal row count, so that
+                                // K = 1, 2 or 4 warps can share the pair work of the same 32 individuals (lane.cuh)
 
-struct LaneHeader {             // 80 bytes
+struct LaneHeader {             // 128 bytes
     int N, Npad, R, nfrag;      // Npad = N rounded up to a multiple of kLaneBI (pad atoms sit at the origin, in no pair)
     int nblocks, ntiles, nrows, maxdepth;
     int off_atoms, off_types, off_frags, off_blocks;    // types: type | fragment << 8 per atom, -1 = pad
     int off_tiles, off_rows, bytes, npairs;
     int own_floats, warp_floats, nslots, pad1;    // per-thread scratch: own_floats = max(6 nfrag, 12 maxdepth);
-                                                // warp_floats = 3 Npad + own_floats + (7+R)
+                                                // warp_floats = 3 Npad + own_floats + (7+R)  (one warp per group)
+    int part_blk[kLaneParts + 1];               // part p owns blocks [part_blk[p], part_blk[p+1])
+    int part_row[kLaneParts + 1];               // and row records from part_row[p] on (a block may be cut between parts)
+    int pad2[2];
 };
+static_assert(sizeof(LaneHeader) == 128, "LaneHeader layout");
 struct LaneFrag {               // 48 bytes; fragments in DFS preorder
     int parent;                 // -1 for the root
     int depth_kids;             // depth (root 0) | has_children << 16
@@ -54,7 +60,7 @@ struct LaneRow {                // 32 bytes: one active row against the two J at
 struct LaneImage {
     std::vector<unsigned char> blob;
     std::vector<int> pos_of_ext, ext_of_pos;    // [N], [Npad] (-1 = pad)
-    int warp_floats = 0;
+    int warp_floats = 0, npad = 0, own_floats = 0;
 };
 
 inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz, const int* type, const float* charge,
@@ -93,7 +99,6 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
         for (int jp = 0; jp < njp; ++jp) {
             uint32_t halfmask = 0, hbmask = 0, hbhalf = 0;
             LaneRow trow[kLaneBI];
-            bool ron[kLaneBI];
             for (int r = 0; r < kLaneBI; ++r) {
                 const int I = b * kLaneBI + r;
                 LaneRow row{};
@@ -113,13 +118,12 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
                     if (co[2] > 8.0f) { hbmask |= 1u << (2 * r + h); hbhalf |= 1u << (r / 2); }
                     ++npair_slots;
                 }
-                trow[r] = row; ron[r] = any;
+                trow[r] = row;
                 if (any) halfmask |= 1u << (r / 2);
             }
             if (!halfmask) continue;
             for (int hf = 0; hf < 2; ++hf)
                 if (halfmask & (1u << hf)) { rows.push_back(trow[2 * hf]); rows.push_back(trow[2 * hf + 1]); }
-            (void)ron;
             LaneTile t;
             t.w0 = (uint32_t)jp | (halfmask << 8) | (hbhalf << 10);
             t.w1 = hbmask | ((uint32_t)frag_of_pos[2 * jp] << 16) | ((uint32_t)frag_of_pos[2 * jp + 1] << 24);
@@ -127,6 +131,30 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
         }
         blk.tile_end = (int)tiles.size();
         if (blk.tile_end > blk.tile_begin) blocks.push_back(blk);
+    }
+    // ---- parts: cut the tile sequence where the running row count crosses p/kLaneParts of the total
+    int part_blk[kLaneParts + 1], part_row[kLaneParts + 1];
+    {
+        auto tile_rows = [&](int t) { const uint32_t hm = (tiles[t].w0 >> 8) & 3u; return 2 * (int)((hm & 1u) + (hm >> 1)); };
+        const int total = (int)rows.size();
+        std::vector<LaneBlock> cut;
+        int p = 0, acc = 0;
+        part_blk[0] = 0; part_row[0] = 0;
+        for (const LaneBlock& b : blocks) {
+            LaneBlock cur = b;
+            for (int t = b.tile_begin; t < b.tile_end; ++t) {
+                // a tile starts the next part when the rows before it reach the part's share
+                while (p + 1 < kLaneParts && acc >= (long long)total * (p + 1) / kLaneParts && acc > part_row[p]) {
+                    if (t > cur.tile_begin) { LaneBlock head = cur; head.tile_end = t; cut.push_back(head); cur.tile_begin = t; }
+                    ++p;
+                    part_blk[p] = (int)cut.size(); part_row[p] = acc;
+                }
+                acc += tile_rows(t);
+            }
+            cut.push_back(cur);
+        }
+        while (p < kLaneParts) { ++p; part_blk[p] = (int)cut.size(); part_row[p] = acc; }
+        blocks.swap(cut);
     }
     // ---- blob
     auto align16 = [](size_t x) { return (x + 15) & ~(size_t)15; };
@@ -136,6 +164,7 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
     h.npairs = (int)tp.pairs.size() / 2;
     h.own_floats = std::max(6 * nfrag, 12 * maxdepth);
     h.warp_floats = 3 * Npad + h.own_floats + 7 + R;
+    for (int q = 0; q <= kLaneParts; ++q) { h.part_blk[q] = part_blk[q]; h.part_row[q] = part_row[q]; }
     size_t off = sizeof(LaneHeader);
     h.off_atoms = (int)off;  off = align16(off + (size_t)Npad * 16);
     h.off_types = (int)off;  off = align16(off + (size_t)Npad * 4);
@@ -146,7 +175,7 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
     h.bytes = (int)off;
     h.nslots = 2 * (int)rows.size();    // pair slots evaluated; npairs of them carry a pair
     (void)npair_slots;
-    im.warp_floats = h.warp_floats;
+    im.warp_floats = h.warp_floats; im.npad = Npad; im.own_floats = h.own_floats;
     im.blob.assign(off, 0);
     std::memcpy(im.blob.data(), &h, sizeof(h));
     float* atoms = (float*)(im.blob.data() + h.off_atoms);
