@@ -350,23 +350,65 @@ static bool lane_ok(const adock_ligand* l) {
     return lane_fit_groups(g, 1) >= 4 || lane_fit_groups(g, 2) >= 2 || lane_fit_groups(g, 4) >= 1;
 }
 // ADADELTA chains (threads) from which the lane-per-individual kernels are preferred over warp-per-individual
-constexpr int kLaneMinChains = 148 * 4 * 32;
-// warps per group for `ngroups` groups of 32 individuals: the K that puts the most warps on the SMs; a forced K
-// (adock_set_path 21/22/24) wins if it fits
-static int lane_pick_k(const LaneGeom& g, long long ngroups) {
-    if (g_lane_k && lane_fit_groups(g, g_lane_k) > 0) return g_lane_k;
-    int best = 0;
-    double best_score = -1;
-    for (int K = 1; K <= 4; K *= 2) {
-        const int fit = lane_fit_groups(g, K);
-        if (!fit) continue;
-        // resident warps per SM when the groups are spread over the SMs, capped by what fits
-        const double per_sm = std::min<double>((double)fit, std::max(1.0, (double)ngroups / g_sm_count)) * K;
-        const double score = per_sm * (K == 1 ? 1.0 : K == 2 ? 0.97 : 0.93);     // redundant pose work of the extra parts
-        if (score > best_score) { best_score = score; best = K; }
+constexpr int kLaneMinChains = 148 * 64;     // measured cross-over on the drug config: between 32 and 64 ligands x 180 chains
+// ---- launch plan of a lane-per-individual kernel over `total` groups of 32 individuals, `jg` consecutive groups per
+// ligand image (jg >= total: one image).  CTA b takes groups [b*ng, (b+1)*ng) and stages every image they touch.
+struct LanePlan {
+    int K = 0;              // warps per group (0: nothing fits)
+    int ng = 0;             // groups per CTA
+    int nctas = 0;
+    int nimg = 1;           // image slots per CTA
+    int slot = 0;           // bytes per image slot (multiple of 128)
+    int gfloats = 0;        // floats per lane between groups
+    size_t smem = 0;
+};
+static int lane_plan_images(long long total, int jg, int ng) {        // most images any CTA of the partition touches
+    if (jg >= total) return 1;
+    int worst = 1;
+    for (long long first = 0; first < total; first += ng) {
+        const long long last = std::min<long long>(first + ng, total) - 1;
+        worst = std::max(worst, (int)(last / jg - first / jg) + 1);
+        if (worst >= (ng - 1) / jg + 2) break;                          // the bound is reached
     }
+    return worst;
+}
+static size_t lane_plan_smem(const LaneGeom& g, int K, int ng, int nimg) {
+    const size_t slot = ((size_t)g.bytes + 127) & ~(size_t)127;
+    return 16 + (size_t)nimg * slot + (size_t)ng * lane_group_floats(g.npad, g.own, g.R, K) * 128;
+}
+// Measured on sweep40 / drug (profiles/r01c_lane_plan.md): with enough groups K = 1 at 8 warps per SM is the fastest
+// (5.0e8 evals/s), K = 2 at 12 warps 0.95x, K = 4 at 16 warps 0.85x; K = 2 at 8 warps only 0.7x; with few groups per SM
+// the extra warps of K = 2, 4 win.  Model: an SM with w resident warps works at min(w, cap_K)/cap_K of its rate
+// (cap = the most warps of that K: 8, 12, 16), times the efficiency of K; waves of CTAs run one after another.
+static LanePlan lane_plan(const LaneGeom& g, long long total, int jg) {
+    LanePlan best;
+    double best_t = 1e300;
+    if (total < 1) total = 1;
+    if (jg < 1) jg = 1;
+    for (int pass = 0; pass < 2 && !best.K; ++pass)             // pass 0 honours a forced K; pass 1: any K that fits
+    for (int K = 1; K <= 4; K *= 2) {
+        if (pass == 0 && g_lane_k && K != g_lane_k) continue;
+        const double eff = K == 1 ? 1.0 : K == 2 ? 0.95 : 0.85;
+        for (int ng = lane_max_warps(K) / K; ng >= 1; --ng) {
+            if (lane_plan_smem(g, K, ng, lane_plan_images(total, jg, ng)) > (size_t)g_smem_optin) continue;
+            const long long nctas = (total + ng - 1) / ng, waves = (nctas + g_sm_count - 1) / g_sm_count;
+            const double t = (double)waves * ng / (eff * (double)(ng * K) / lane_max_warps(K));
+            if (t < best_t * 0.999) {
+                best_t = t;
+                best.K = K; best.ng = ng;
+            }
+        }
+    }
+    if (!best.K) return best;
+    best.nctas = (int)((total + best.ng - 1) / best.ng);
+    best.nimg = lane_plan_images(total, jg, best.ng);
+    best.slot = (g.bytes + 127) & ~127;
+    best.gfloats = lane_group_floats(g.npad, g.own, g.R, best.K);
+    best.smem = lane_plan_smem(g, best.K, best.ng, best.nimg);
     return best;
 }
+// warps per group for `ngroups` groups of 32 individuals of one ligand
+static int lane_pick_k(const LaneGeom& g, long long ngroups) { return lane_plan(g, ngroups, (int)std::min<long long>(ngroups, 1 << 30)).K; }
 // groups per CTA: as many as fit, fewer when that would leave SMs idle
 static int lane_spread_groups(int fit, long long ngroups) {
     int n = fit;
@@ -792,20 +834,48 @@ __global__ void __launch_bounds__(128) dock_ls_kernel(GridDev G, ParDev P, const
     }
 }
 
-// the same step, lane-per-individual: lane c of a job's groups runs chain c = run*n_ls + l; every CTA stages its job's
-// lane image; ADADELTA state in global scratch columns [row][all group lanes of the launch] (rows: Gmax best, 3 x Dmax)
+// ---- lane-per-individual kernels of the docking loop.  The groups (32 chains / individuals each) of all jobs of a
+// launch form one flat sequence, jg groups per job; CTA b takes groups [b*ng, (b+1)*ng), which may belong to several
+// consecutive jobs: it stages the lane image of each of them (slot s = job j0+s) in one bulk-copy transaction.
+struct LaneDockArgs {
+    float* scratch;         // ADADELTA state columns (LS kernel)
+    int Gmax;               // largest 7+R of the launch
+    int ng, total_groups, jg;
+    int slot_bytes, nimg;   // image slots per CTA (the most any CTA needs), slot size (multiple of 128)
+    int group_floats;       // floats per lane between groups (largest ligand)
+};
+struct LaneCtaGroup { int jidx, gi; const unsigned char* blob; float* scratch; bool valid; };
+template <int K>
+__device__ __forceinline__ LaneCtaGroup lane_cta_group(unsigned char* smem, const DockJob* __restrict__ jobs, const LaneDockArgs& a) {
+    const int first = blockIdx.x * a.ng, last = min(first + a.ng, a.total_groups) - 1;
+    const int j0 = first / a.jg, nimg = last / a.jg - j0 + 1;
+    stage_images(smem + 16, a.slot_bytes, nimg,
+                 [&](int s, const unsigned char*& p, int& b) { p = jobs[j0 + s].lane; b = jobs[j0 + s].lane_bytes; },
+                 reinterpret_cast<uint64_t*>(smem));
+    LaneCtaGroup c;
+    const int g = first + (int)(threadIdx.x >> 5) / K;
+    c.valid = g <= last;
+    c.jidx = c.valid ? g / a.jg : j0;
+    c.gi = c.valid ? g % a.jg : 0;
+    c.blob = smem + 16 + (size_t)(c.jidx - j0) * a.slot_bytes;
+    c.scratch = reinterpret_cast<float*>(smem + 16 + (size_t)a.nimg * a.slot_bytes);
+    return c;
+}
+
+// ADADELTA on the selected individuals (Lamarckian write-back): lane c of a job's groups runs chain c = run*n_ls + l;
+// ADADELTA state in global scratch columns [row][all group lanes of the launch] (rows: Gmax best, 3 x Dmax)
 template <int K>
 __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_ls_lane_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs,
-                                                                                     DockDims dm, float* __restrict__ scratch, int Gmax) {
+                                                                                     DockDims dm, LaneDockArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
-    const DockJob job = jobs[blockIdx.x / dm.upj];
-    unsigned char* blob = smem + 16;
-    stage_ligand(blob, job.lane, job.lane_bytes, reinterpret_cast<uint64_t*>(smem), 0);
-    const LaneL L = lane_view(blob);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, NG = (blockDim.x >> 5) / K;
-    const LaneS S = lane_scratch<K>(reinterpret_cast<float*>(blob + job.lane_bytes), L, warp, lane);
+    const LaneCtaGroup cg = lane_cta_group<K>(smem, jobs, a);
+    if (!cg.valid) return;                              // whole groups leave: the named barriers are per group
+    const DockJob job = jobs[cg.jidx];
+    const LaneL L = lane_view(cg.blob);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const LaneS S = lane_scratch<K>(cg.scratch, L, warp, lane, a.group_floats);
     const int Gn = job.Gn;
-    const int c = ((blockIdx.x % dm.upj) * NG + S.gid) * 32 + lane;
+    const int c = cg.gi * 32 + lane;
     bool act = c < dm.nrun * dm.n_ls;
     const int cc = act ? c : 0;
     const int run = cc / dm.n_ls, l = cc % dm.n_ls;
@@ -819,10 +889,10 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_ls_lane_ke
     if (S.part == 0)
         for (int d = 0; d < Gn; ++d) S.geno[d * 32] = g[d];
     group_sync<K>(S);
-    const size_t tid = ((size_t)blockIdx.x * NG + S.gid) * 32 + lane, T = (size_t)gridDim.x * NG * 32;
-    const int Dmax = Gmax - 1;
+    const size_t tid = ((size_t)blockIdx.x * a.ng + S.gid) * 32 + lane, T = (size_t)gridDim.x * a.ng * 32;
+    const int Dmax = a.Gmax - 1;
     LaneLS ls;
-    ls.best = scratch + tid; ls.Eg2 = ls.best + (size_t)Gmax * T; ls.Ed2 = ls.Eg2 + (size_t)Dmax * T; ls.grad = ls.Ed2 + (size_t)Dmax * T;
+    ls.best = a.scratch + tid; ls.Eg2 = ls.best + (size_t)a.Gmax * T; ls.Ed2 = ls.Eg2 + (size_t)Dmax * T; ls.grad = ls.Ed2 + (size_t)Dmax * T;
     ls.stride = (int)T;
     int iters = 0;
     const float be = lane_adadelta<K>(L, G, P, S, ls, act, (act && S.part == 0) ? *e : 0.f, iters, nullptr, 0);
@@ -831,6 +901,37 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_ls_lane_ke
         *e = be;
         atomicAdd(&job.st[run].ls_acc, iters);
     }
+}
+
+// energies of the offspring written by dock_ga_kernel<false> (slot 0, the elite, carries its energy): lane c of a
+// job's groups scores individual c = run*P + slot of the new population
+template <int K>
+__global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_score_lane_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs,
+                                                                                        DockDims dm, LaneDockArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const LaneCtaGroup cg = lane_cta_group<K>(smem, jobs, a);
+    if (!cg.valid) return;
+    const DockJob job = jobs[cg.jidx];
+    const LaneL L = lane_view(cg.blob);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const LaneS S = lane_scratch<K>(cg.scratch, L, warp, lane, a.group_floats);
+    const int Gn = job.Gn;
+    const int c = cg.gi * 32 + lane, n = dm.nrun * dm.P;
+    bool act = c < n;
+    const int cc = act ? c : n - 1;
+    const int run = cc / dm.P, slot = cc % dm.P;
+    const RunState st = job.st[run];
+    act = act && st.active && slot != 0;
+    if (!__any_sync(kFull, act)) return;
+    const size_t popsz = (size_t)dm.nrun * dm.P;
+    const float* g = job.pop + ((size_t)(st.cur ^ 1) * popsz + cc) * Gn;
+    if (S.part == 0)
+        for (int d = 0; d < Gn; ++d) S.geno[d * 32] = g[d];
+    group_sync<K>(S);
+    float ei, ea;
+    bool gf;
+    const float e = lane_eval<false, K>(L, G, P, S, nullptr, 1, false, ei, ea, gf);
+    if (act && S.part == 0) job.E[(size_t)(st.cur ^ 1) * popsz + cc] = e;
 }
 
 // end of generation: eval accounting, buffer flip, termination test
@@ -940,10 +1041,14 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         lanes_fit = lanes_fit && lane_ok(ligs[l]);
     }
     const int jg = (nrun * n_ls0 + 31) / 32;                        // groups of 32 chains per job
-    const int Klane = lane_pick_k(lg, (long long)nlig * jg);
-    const bool ls_lane = Klane > 0 && (g_path == 2 || (g_path == 0 && lanes_fit && chains >= kLaneMinChains));
-    if (g_path == 2 && !Klane) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
+    const LanePlan pl = lane_plan(lg, (long long)nlig * jg, jg);
+    const bool ls_lane = pl.K > 0 && (g_path == 2 || (g_path == 0 && lanes_fit && chains >= kLaneMinChains));
+    if (g_path == 2 && !pl.K) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
     g_last_dock_path = ls_lane ? 2 : 1;
+    // offspring scoring: lane-per-individual under the same condition (populations are 1/lsrat times larger)
+    const int jgs = (int)(((long long)nrun * Pn + 31) / 32);
+    const LanePlan ps = lane_plan(lg, (long long)nlig * jgs, jgs);
+    const bool ga_lane = ls_lane && ps.K > 0;
     ParDev P = make_pardev(p);
     P.k_wall_h = p.k_wall * grids->dev.h;
     DockDims dm{};
@@ -996,29 +1101,44 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     dga.upj = (int)((popsz + Wga - 1) / Wga);
     dls.upj = std::max(1, (nrun * dm.n_ls + Wls - 1) / Wls);
     dfin.upj = (nrun + Wls - 1) / Wls;
-    // lane family: the groups of a job's chains split evenly over the fewest CTAs that fit
-    DockDims dll = dm;
-    int NGl = 1;
-    size_t smem_ll = 0;
+    // lane family: flat group sequence over all jobs (lane_plan)
+    LaneDockArgs al{}, as{};
     float* d_lscratch = nullptr;
     if (ls_lane && dm.n_ls > 0) {
-        const int fit = lane_fit_groups(lg, Klane);
-        dll.upj = (jg + fit - 1) / fit;
-        NGl = (jg + dll.upj - 1) / dll.upj;
-        smem_ll = lane_smem(lg, Klane, NGl);
-        const size_t T = (size_t)nlig * dll.upj * NGl * 32;
+        const size_t T = (size_t)pl.nctas * pl.ng * 32;
         cudaError_t e2 = buf.alloc(&d_lscratch, T * (size_t)(Gmax + 3 * (Gmax - 1)) * 4);
         if (e2 != cudaSuccess) return fail(e2 == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("dock alloc: ") + cudaGetErrorString(e2));
-        if (Klane == 1) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ll));
-        if (Klane == 2) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ll));
-        if (Klane == 4) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ll));
+        al = LaneDockArgs{d_lscratch, Gmax, pl.ng, nlig * jg, jg, pl.slot, pl.nimg, pl.gfloats};
+        if (pl.K == 1) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        if (pl.K == 2) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        if (pl.K == 4) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+    }
+    if (ga_lane) {
+        as = LaneDockArgs{nullptr, Gmax, ps.ng, nlig * jgs, jgs, ps.slot, ps.nimg, ps.gfloats};
+        if (ps.K == 1) CUDA_TRY(cudaFuncSetAttribute(dock_score_lane_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps.smem));
+        if (ps.K == 2) CUDA_TRY(cudaFuncSetAttribute(dock_score_lane_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps.smem));
+        if (ps.K == 4) CUDA_TRY(cudaFuncSetAttribute(dock_score_lane_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps.smem));
+        CUDA_TRY(cudaFuncSetAttribute(dock_ga_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ga));
     }
     auto launch_ls = [&]() {
-        const int thr = NGl * Klane * 32;
-        if (ls_lane && Klane == 1) dock_ls_lane_kernel<1><<<dll.upj * nlig, thr, smem_ll, stm>>>(grids->dev, P, d_jobs, dll, d_lscratch, Gmax);
-        else if (ls_lane && Klane == 2) dock_ls_lane_kernel<2><<<dll.upj * nlig, thr, smem_ll, stm>>>(grids->dev, P, d_jobs, dll, d_lscratch, Gmax);
-        else if (ls_lane) dock_ls_lane_kernel<4><<<dll.upj * nlig, thr, smem_ll, stm>>>(grids->dev, P, d_jobs, dll, d_lscratch, Gmax);
+        const int thr = pl.ng * pl.K * 32;
+        if (ls_lane && pl.K == 1) dock_ls_lane_kernel<1><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
+        else if (ls_lane && pl.K == 2) dock_ls_lane_kernel<2><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
+        else if (ls_lane) dock_ls_lane_kernel<4><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
         else dock_ls_kernel<<<dls.upj * nlig, Wls * 32, smem_ls, stm>>>(grids->dev, P, d_jobs, dls);
+    };
+    // one GA generation: offspring + their energies (one launch, or two when the scoring runs lane-per-individual)
+    auto launch_ga = [&]() {
+        if (!ga_lane) {
+            dock_ga_kernel<true><<<dga.upj * nlig, Wga * 32, smem_ga, stm>>>(grids->dev, P, d_jobs, dga, nullptr);
+            return 1;
+        }
+        dock_ga_kernel<false><<<dga.upj * nlig, Wga * 32, smem_ga, stm>>>(grids->dev, P, d_jobs, dga, nullptr);
+        const int thr = ps.ng * ps.K * 32;
+        if (ps.K == 1) dock_score_lane_kernel<1><<<ps.nctas, thr, ps.smem, stm>>>(grids->dev, P, d_jobs, dm, as);
+        else if (ps.K == 2) dock_score_lane_kernel<2><<<ps.nctas, thr, ps.smem, stm>>>(grids->dev, P, d_jobs, dm, as);
+        else dock_score_lane_kernel<4><<<ps.nctas, thr, ps.smem, stm>>>(grids->dev, P, d_jobs, dm, as);
+        return 2;
     };
     dock_init_kernel<<<dga.upj * nlig, Wga * 32, smem_ga, stm>>>(grids->dev, P, d_jobs, dga);
     ++g_launches;
@@ -1028,7 +1148,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     const int poll = 8;
     std::vector<cudaEvent_t> prof_ev;
     for (int g = 0; h_flag && g < p.max_gens; ++g) {
-        dock_ga_kernel<true><<<dga.upj * nlig, Wga * 32, smem_ga, stm>>>(grids->dev, P, d_jobs, dga, nullptr);
+        g_launches += launch_ga() - 1;
         if (dm.n_ls > 0 && p.lsit > 0) {
             if (g_prof) {
                 cudaEvent_t a, b;

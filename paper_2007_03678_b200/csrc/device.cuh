@@ -117,6 +117,37 @@ __device__ inline void stage_ligand(unsigned char* dst, const unsigned char* src
     }
 }
 
+// Several images in one transaction: image s (src(s), bytes(s), both multiples of 16) lands at dst + s*slot_bytes.
+// All threads of the CTA call this once (phase 0); returns after every image is visible in shared memory.
+template <class SrcFn>
+__device__ inline void stage_images(unsigned char* dst, int slot_bytes, int nimg, SrcFn src, uint64_t* bar) {
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(bar)));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        uint32_t total = 0;
+        for (int s = 0; s < nimg; ++s) { const unsigned char* p; int b; src(s, p, b); total += (uint32_t)b; }
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(total) : "memory");
+        for (int s = 0; s < nimg; ++s) {
+            const unsigned char* p; int b;
+            src(s, p, b);
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                             smem_u32(dst + (size_t)s * slot_bytes)),
+                         "l"(p), "r"(b), "r"(smem_u32(bar))
+                         : "memory");
+        }
+    }
+    __syncthreads();
+    uint32_t done = 0;
+    while (!done) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(0u)
+            : "memory");
+    }
+}
+
 // ---------------------------------------------------------------- grid term (R4)
 struct F8 { float4 lo, hi; };
 // One aligned 32-byte sector (LDG.256).  The lookups of a warp are scattered over the maps (32 lanes = 32 poses), so a

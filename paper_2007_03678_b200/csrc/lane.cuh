@@ -65,11 +65,14 @@ struct LaneS {              // this lane's columns of the group's scratch; eleme
 __host__ __device__ inline int lane_group_floats(int Npad, int own_floats, int R, int K) {
     return 3 * Npad + K * own_floats + (7 + R) + 2 * K + 1;
 }
+// group_floats = floats per lane between consecutive groups of the CTA: lane_group_floats of the ligand, or of the
+// largest ligand of the launch when the groups of a CTA belong to different ligands (0 = this ligand's)
 template <int K>
-__device__ inline LaneS lane_scratch(float* cta_base, const LaneL& L, int warp, int lane) {
+__device__ inline LaneS lane_scratch(float* cta_base, const LaneL& L, int warp, int lane, int group_floats = 0) {
     LaneS S;
     S.gid = warp / K; S.part = warp % K;
-    float* base = cta_base + (size_t)S.gid * lane_group_floats(L.Npad, L.own_floats, L.R, K) * 32;
+    if (group_floats == 0) group_floats = lane_group_floats(L.Npad, L.own_floats, L.R, K);
+    float* base = cta_base + (size_t)S.gid * group_floats * 32;
     const int half = L.Npad / 2;
     S.X = reinterpret_cast<float2*>(base) + lane;
     S.Y = S.X + half * 32;
