@@ -36,6 +36,11 @@ NRUN, POP, MAX_EVALS = 20, 150, 2_500_000
 WORKLOAD = ("drug-like docking: 40-atom ligand, 8 torsions, 7 types, 9 fp32 maps 64^3 @0.375A, "
             "20 LGA runs x pop 150 x 2.5M evals/run, ADADELTA 300 it on 6%/generation")
 SM_COUNT, FP32_LANES, SM_MAX_MHZ = 148, 128, 1965.0        # B200_PROFILING.md unit counts and clocks
+# 197 ligands x 20 runs x 9 ADADELTA chains = 35460 chains = 1182 groups of 32 lanes: 8 resident warps on each of the 148 SMs
+DEFAULT_LIGANDS = 197
+# dram__bytes_read.sum + dram__bytes_write.sum of one dock_ls_lane_kernel launch at the default batch
+# (profiles/r01c_dock_ls_lane_ncu.md); other batch sizes report null
+LS_TRAFFIC_BYTES = {197: 163.08e6 + 28.31e6}
 
 
 def flops_per_eval(N, R, npairs, nmoved):
@@ -134,10 +139,12 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--ligands", type=int, default=8, help="ligands docked concurrently per step and per GPU")
+    ap.add_argument("--ligands", type=int, default=DEFAULT_LIGANDS, help="ligands docked concurrently per step and per GPU")
+    ap.add_argument("--e2e-steps", type=int, default=2, help="steps of the host-buffer (end-to-end) leg, at most --steps")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--sweep", action="store_true", help="also time adock_score_batch on the sweep config")
+    ap.add_argument("--sweep", action="store_true", help="time adock_score_batch on all four sweep ligands (default: the 40-atom one)")
+    ap.add_argument("--no-sweep", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -196,6 +203,7 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     launches = B.adock_launch_count()
     prof = B.adock_profile_read()
+    dock_path = B.lib().adock_last_dock_path()
     B.adock_profile(False)
     t_ms = sum(a.elapsed_time(b) for a, b in ev)
 
@@ -203,7 +211,8 @@ def main():
     barrier()
     t0 = time.perf_counter()
     e2e_evals, h2d, d2h = 0, 0, 0
-    for s in range(args.steps):
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    for s in range(e2e_steps):
         hl = [B.Ligand.from_workload(gg, l, gp) for l in ligs]                  # host preprocessing + H2D of the images
         r = B.adock_dock_many(gg, hl, gp, NRUN, POP, MAX_EVALS, [sd + 77 * (s + 1) for sd in seeds], want_coords=True)
         e2e_evals += int(r["evals"].sum())
@@ -233,8 +242,9 @@ def main():
     mean_flop = float(np.mean(flop_eval))
     peak_tf = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12
     ach_tf = (ls_evals * mean_flop / (ls_ms * 1e-3) / 1e12) if ls_ms > 0 else None
-    roofline = {"bound": "alu", "kernel": "dock_ls_kernel", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": (ach_tf / peak_tf) if ach_tf else None, "traffic": None,
+    kernel = "dock_ls_lane_kernel" if dock_path == 2 else "dock_ls_kernel"
+    roofline = {"bound": "alu", "kernel": kernel, "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": (ach_tf / peak_tf) if ach_tf else None, "traffic": LS_TRAFFIC_BYTES.get(L) if dock_path == 2 else None,
                 "peak_source": f"derived: {SM_COUNT} SMs x {FP32_LANES} FP32 lanes x 2 x {SM_MAX_MHZ:.0f} MHz (B200_PROFILING.md); "
                                f"HBM peak {peaks.get('hbm_gbs')} GB/s of measured is not the bound (~120 B/eval)",
                 "flop_per_eval": mean_flop, "avg_launch_ms": (ls_ms / ls_n) if ls_n else None, "launches_timed": ls_n,
@@ -244,15 +254,16 @@ def main():
         "warmup": args.warmup, "ms_per_step": t_ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": WORKLOAD, "ligands_per_step_per_gpu": L, "nrun": NRUN, "pop_size": POP, "max_evals": MAX_EVALS,
-                   "l2": "160 MB buffer written before every timed step (flush); maps 58.7 MB resident"},
+                   "l2": "160 MB buffer written before every timed step (flush); maps 58.7 MB resident",
+                   "kernel_family": "lane-per-individual" if dock_path == 2 else "warp-per-individual"},
         "ligands_per_hour": 3600.0 * L * world * args.steps / (t_ms * 1e-3),
         "e2e": {"value": e2e_evals / e2e_s, "unit": "evals/s", "h2d_bytes_per_step": int(h2d) * world, "d2h_bytes_per_step": int(d2h) * world,
-                "ligands_per_hour": 3600.0 * L * world * args.steps / e2e_s},
+                "ligands_per_hour": 3600.0 * L * world * e2e_steps / e2e_s, "steps": e2e_steps},
         "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
     }
 
-    if args.sweep:
-        out["score_batch"] = sweep(B, torch, dev)
+    if not args.no_sweep:
+        out["score_batch"] = sweep(B, torch, dev, ("sweep16", "sweep40", "sweep80", "sweep128") if args.sweep else ("sweep40",))
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline()
     print(json.dumps(out))
@@ -260,29 +271,38 @@ def main():
         dist.destroy_process_group()
 
 
-def sweep(B, torch, dev):
-    """adock_score_batch on BASELINE.json's sweep sizes for the 40-atom ligand (energy + gradient)."""
-    grids, lig = W.make_config("sweep40")
+def sweep(B, torch, dev, configs=("sweep40",)):
+    """adock_score_batch (energy + gradient) on BASELINE.json's scoring-kernel sweep: 1k..1M random genotypes for the
+    16/40/80/128-atom ligands on a 64^3 grid set; evals/s and the ALU-roofline fraction of each point."""
+    peak_tf = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ * 1e6 / 1e12
     gp = B.make_params(W.DEFAULT_PARAMS)
-    gg = B.Grids.from_workload(grids)
-    gl = B.Ligand.from_workload(gg, lig, gp)
-    fl = flops_per_eval(lig.N, lig.R, len(gl.pairs()), int(gl.tree()["moved"].sum()))
-    res = {}
-    for n in (1024, 16384, 262144, 1048576):
-        G = torch.from_numpy(W.make_genotypes(n, lig.R, grids, seed=4)).to(dev)
-        E = torch.zeros(n, device=dev)
-        gr = torch.zeros((n, 6 + lig.R), device=dev)
-        for _ in range(3):
-            B.adock_score_batch(gg, gl, gp, G, E, None, gr)
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        for _ in range(10):
-            B.adock_score_batch(gg, gl, gp, G, E, None, gr)
-        b.record()
-        torch.cuda.synchronize()
-        ms = a.elapsed_time(b) / 10
-        res[str(n)] = {"ms": ms, "evals_per_s": n / (ms * 1e-3), "tflops": n * fl / (ms * 1e-3) / 1e12}
-    return res
+    out = {}
+    for cfg in configs:
+        grids, lig = W.make_config(cfg)
+        gg = B.Grids.from_workload(grids)
+        gl = B.Ligand.from_workload(gg, lig, gp)
+        fl = flops_per_eval(lig.N, lig.R, len(gl.pairs()), int(gl.tree()["moved"].sum()))
+        res = {"atoms": lig.N, "torsions": lig.R, "pairs": len(gl.pairs()), "flop_per_eval": fl}
+        for n in (1024, 16384, 262144, 1048576):
+            G = torch.from_numpy(W.make_genotypes(n, lig.R, grids, seed=4)).to(dev)
+            E = torch.zeros(n, device=dev)
+            gr = torch.zeros((n, 6 + lig.R), device=dev)
+            for _ in range(3):
+                B.adock_score_batch(gg, gl, gp, G, E, None, gr)
+            reps = 10 if n * lig.N <= 1048576 * 40 else 3
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(reps):
+                B.adock_score_batch(gg, gl, gp, G, E, None, gr)
+            b.record()
+            torch.cuda.synchronize()
+            ms = a.elapsed_time(b) / reps
+            tf = n * fl / (ms * 1e-3) / 1e12
+            res[str(n)] = {"ms": ms, "evals_per_s": n / (ms * 1e-3), "tflops": tf, "alu_frac": tf / peak_tf}
+        out[cfg] = res
+        gl.close()
+        gg.close()
+    return out
 
 
 def cpu_baseline():
