@@ -133,6 +133,17 @@ def run_reference(args):
     }))
 
 
+def reduce_over_ranks(dist, dev, times, counts):
+    """Whole-job numbers from per-rank ones: times -> MAX over ranks, counts -> SUM over ranks (the path has no other
+    collective: ranks dock disjoint ligand shards)."""
+    import torch
+    t = torch.tensor(list(times), dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor(list(counts), dtype=torch.float64, device=dev)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return t.tolist(), [int(x) for x in c.tolist()]
+
+
 # ------------------------------------------------------------------------------------------ CUDA arm
 def main():
     ap = argparse.ArgumentParser()
@@ -224,12 +235,7 @@ def main():
     e2e_s = time.perf_counter() - t0
 
     if world > 1:
-        t = torch.tensor([t_ms, e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        c = torch.tensor([evals, e2e_evals, launches], dtype=torch.float64, device=dev)
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        t_ms, e2e_s = t.tolist()
-        evals, e2e_evals, launches = (int(x) for x in c.tolist())
+        (t_ms, e2e_s), (evals, e2e_evals, launches) = reduce_over_ranks(dist, dev, [t_ms, e2e_s], [evals, e2e_evals, launches])
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
