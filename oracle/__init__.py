@@ -27,13 +27,15 @@ def build(force: bool = False) -> str:
 class OPar(C.Structure):
     _fields_ = [(k, C.c_double) for k in (
         "elec_scale", "diel_A", "diel_B", "diel_k", "diel_lambda", "w_desolv", "ds_sigma", "qasp", "r_min", "k_wall",
-        "ad_rho", "ad_eps", "lsrat", "tourn_prob", "xover_rate", "mut_rate", "dmov", "dang")] + [
-        ("lsit", C.c_int), ("max_gens", C.c_int)]
+        "ad_rho", "ad_eps", "lsrat", "tourn_prob", "xover_rate", "mut_rate", "dmov", "dang",
+        "sw_rho0", "sw_rho_lb", "sw_expand", "sw_contract", "sw_bias_keep", "sw_bias_gain", "sw_bias_decay", "as_tol")] + [
+        (k, C.c_int) for k in ("lsit", "max_gens", "ls_method", "sw_max_succ", "sw_max_fail", "autostop", "as_window")]
 
 
 # GA probabilities and step sizes are float32 parameters of the method: both sides see the same
 # float32 value (decisions u < p are then identical), so round them once here.
-_F32_FIELDS = ("lsrat", "tourn_prob", "xover_rate", "mut_rate", "dmov", "dang")
+_F32_FIELDS = ("lsrat", "tourn_prob", "xover_rate", "mut_rate", "dmov", "dang",
+               "sw_rho0", "sw_rho_lb", "sw_expand", "sw_contract", "sw_bias_keep", "sw_bias_gain", "sw_bias_decay", "as_tol")
 
 
 def params(d: dict) -> OPar:
@@ -227,6 +229,37 @@ def adadelta(grids: Grids, lig: Ligand, par: OPar, geno, trace=False):
     tX = np.full((par.lsit, 7 + lig.R), np.nan) if trace else None
     lib().orc_adadelta(grids._h, lig._h, C.byref(par), _p(g), C.byref(E), C.byref(it), _p(tE), _p(tX))
     return (g, E.value, it.value, tE, tX) if trace else (g, E.value, it.value)
+
+
+def solis_wets_rn(x0, E0, fn, amp, par: OPar, seed, id, gen):
+    """generic R^n Solis-Wets (R11); fn(x)->f. Returns (x, E, evals, iterations, final rho, trace of E after each iteration)."""
+    x = _f64(x0).copy()
+    n = x.shape[0]
+
+    def cb(n_, xp, _gp, _user):
+        return float(fn(np.ctypeslib.as_array(xp, (n_,)).copy()))
+
+    E = C.c_double(float(E0)); it = C.c_int(); rho = C.c_double()
+    tE = np.full(par.lsit, np.nan)
+    L = lib()
+    L.orc_solis_wets_rn.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_ulonglong, C.c_uint, C.c_uint,
+                                    _FN, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    ev = L.orc_solis_wets_rn(n, _p(x), C.addressof(E), _p(_f64(amp)), C.addressof(par), int(seed), int(id), int(gen), _FN(cb), None,
+                             C.addressof(it), C.addressof(rho), _p(tE))
+    return x, E.value, ev, it.value, rho.value, tE
+
+
+def solis_wets(grids: Grids, lig: Ligand, par: OPar, geno, E0, seed, id, gen):
+    """docking Solis-Wets from one genotype with carried energy E0: (genotype, E, evals, iterations, rho, traceE)."""
+    g = _f64(geno).copy()
+    E = C.c_double(float(E0)); it = C.c_int(); rho = C.c_double()
+    tE = np.full(par.lsit, np.nan)
+    L = lib()
+    L.orc_solis_wets.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_ulonglong, C.c_uint, C.c_uint, C.c_void_p, C.c_void_p,
+                                 C.c_void_p, C.c_void_p, C.c_void_p]
+    ev = L.orc_solis_wets(grids._h, lig._h, C.addressof(par), int(seed), int(id), int(gen), _p(g), C.addressof(E),
+                          C.addressof(it), C.addressof(rho), _p(tE))
+    return g, E.value, ev, it.value, rho.value, tE
 
 
 def philox(key, ctr):

@@ -37,7 +37,13 @@ struct OPar {               // mirrors workloads.DEFAULT_PARAMS by name (own lay
     double w_desolv, ds_sigma, qasp, r_min, k_wall;
     double ad_rho, ad_eps;
     double lsrat, tourn_prob, xover_rate, mut_rate, dmov, dang;
+    // R11 Solis-Wets: initial / smallest step scale, expansion / contraction factors, bias update coefficients
+    double sw_rho0, sw_rho_lb, sw_expand, sw_contract, sw_bias_keep, sw_bias_gain, sw_bias_decay;
+    double as_tol;          // R12 autostop: threshold on the std-dev of a run's best energy over as_window generations
     int lsit, max_gens;
+    int ls_method;          // 0 = ADADELTA (R7), 1 = Solis-Wets (R11)
+    int sw_max_succ, sw_max_fail;
+    int autostop, as_window;
 };
 
 struct OLig {
@@ -454,6 +460,63 @@ inline void draw4(uint64_t seed, uint32_t draw, uint32_t purpose, uint32_t id, u
 inline double u01(uint32_t x) { return (double)(x >> 8) * (1.0 / 16777216.0); }          // exact, in [0,1)
 inline int below(uint32_t x, int n) { return (int)std::floor(u01(x) * n); }               // floor(u*n), exact in fp64
 
+// ------------------------------------------------------------------ R11: Solis-Wets local search
+// PAPER.md lines 58, 64, 136 name the method and cite Solis & Wets 1981 [27] ("Minimization by random search
+// techniques", the variant with an adaptive step scale and a bias vector); constants [LIT] -> params.  One iteration:
+//   delta_d = rho * amp_d * (2 u_d - 1) + b_d        u_d: Philox word d&3 of draw (it*ceil(D/4) + d/4, P_SW, id, gen)
+//   E(x (+) delta) < E : accept, b <- keep b + gain delta, success
+//   else E(x (-) delta) < E : accept, b <- keep b - gain delta, success          (second evaluation only in this branch)
+//   else b <- decay b, failure
+//   sw_max_succ successes in a row: rho *= expand ; sw_max_fail failures in a row: rho *= contract
+// until it == lsit or rho < rho_lb.  (+) is the step application of R7 (translation, left rotation by the rotation
+// vector, wrapped torsions); amp = dmov for the translation, dang for the rotation vector and the torsions.
+// E(x) is the carried energy (no evaluation).  A non-finite trial energy is a failure (comparison false).
+struct SwFn { virtual double operator()(const double* x) = 0; virtual void step(double* x, const double* delta, double sign) = 0; virtual ~SwFn() {} };
+enum { P_SW = 6 };
+// returns evaluations used; x, E updated in place; iters = iterations done; rho_out = final step scale
+int solis_wets(SwFn& f, int n, int D, const double* amp, const OPar& P, uint64_t seed, uint32_t id, uint32_t gen, double* x, double* E,
+               int* iters, double* rho_out, double* traceE) {
+    std::vector<double> b(D, 0.0), delta(D), cand(n);
+    double rho = P.sw_rho0;
+    int ns = 0, nf = 0, it = 0, evals = 0;
+    const int nq = (D + 3) / 4;
+    while (it < P.lsit && !(rho < P.sw_rho_lb)) {
+        for (int q = 0; q < nq; ++q) {
+            uint32_t r[4];
+            draw4(seed, (uint32_t)(it * nq + q), P_SW, id, gen, r);
+            for (int w = 0; w < 4 && 4 * q + w < D; ++w) delta[4 * q + w] = rho * amp[4 * q + w] * (2.0 * u01(r[w]) - 1.0) + b[4 * q + w];
+        }
+        std::copy(x, x + n, cand.begin());
+        f.step(cand.data(), delta.data(), +1.0);
+        double e = f(cand.data());
+        ++evals;
+        bool ok = false;
+        if (e < *E) {
+            for (int d = 0; d < D; ++d) b[d] = P.sw_bias_keep * b[d] + P.sw_bias_gain * delta[d];
+            ok = true;
+        } else {
+            std::copy(x, x + n, cand.begin());
+            f.step(cand.data(), delta.data(), -1.0);
+            e = f(cand.data());
+            ++evals;
+            if (e < *E) {
+                for (int d = 0; d < D; ++d) b[d] = P.sw_bias_keep * b[d] - P.sw_bias_gain * delta[d];
+                ok = true;
+            } else {
+                for (int d = 0; d < D; ++d) b[d] = P.sw_bias_decay * b[d];
+            }
+        }
+        if (ok) { std::copy(cand.begin(), cand.end(), x); *E = e; ++ns; nf = 0; } else { ++nf; ns = 0; }
+        if (ns >= P.sw_max_succ) { rho *= P.sw_expand; ns = 0; }
+        else if (nf >= P.sw_max_fail) { rho *= P.sw_contract; nf = 0; }
+        if (traceE) traceE[it] = *E;
+        ++it;
+    }
+    if (iters) *iters = it;
+    if (rho_out) *rho_out = rho;
+    return evals;
+}
+
 // ------------------------------------------------------------------ R9: GA
 void ga_init_one(const OGrid& G, int R, uint64_t seed, uint32_t id, double* g) {
     uint32_t r[4];
@@ -557,6 +620,38 @@ int ls_pick(const OPar& P, int Pn, int run, int gen, uint64_t seed, int* picks) 
     return n_ls;
 }
 
+struct SwDock : SwFn {
+    const OGrid& G; const OLig& L; const OPar& P;
+    SwDock(const OGrid& g, const OLig& l, const OPar& p) : G(g), L(l), P(p) {}
+    double operator()(const double* x) override { return score(G, L, P, x, nullptr, nullptr, nullptr); }
+    void step(double* x, const double* delta, double sign) override {
+        std::vector<double> d(delta, delta + 6 + L.R);
+        for (auto& v : d) v *= sign;
+        apply_step(L.R, x, d.data());
+    }
+};
+int solis_wets_dock(const OGrid& G, const OLig& L, const OPar& P, uint64_t seed, uint32_t id, uint32_t gen, double* x, double* E,
+                    int* iters, double* rho_out, double* traceE) {
+    const int D = 6 + L.R;
+    std::vector<double> amp(D, P.dang);
+    amp[0] = amp[1] = amp[2] = P.dmov;
+    SwDock f(G, L, P);
+    return solis_wets(f, 7 + L.R, D, amp.data(), P, seed, id, gen, x, E, iters, rho_out, traceE);
+}
+
+// R12 autostop ("stop ... if no progress is being made"; criterion [CHOICE] -> params): a run ends
+// after generation g >= as_window when the population std-dev of its best energy over the last as_window generations
+// is < as_tol.
+bool autostop_hit(const OPar& P, const std::vector<double>& best_hist) {
+    const int W = P.as_window;
+    if (!P.autostop || W < 1 || (int)best_hist.size() < W) return false;
+    double m = 0, v = 0;
+    for (int i = 0; i < W; ++i) m += best_hist[best_hist.size() - W + i];
+    m /= W;
+    for (int i = 0; i < W; ++i) { const double d = best_hist[best_hist.size() - W + i] - m; v += d * d; }
+    return std::sqrt(v / W) < P.as_tol;
+}
+
 struct RunResult { std::vector<double> best; double bestE; long long evals; int gens; };
 
 RunResult dock_run(const OGrid& G, const OLig& L, const OPar& P, int run, int Pn, long long max_evals, uint64_t seed,
@@ -570,6 +665,7 @@ RunResult dock_run(const OGrid& G, const OLig& L, const OPar& P, int run, int Pn
     }
     long long evals = Pn;
     int gen = 0;
+    std::vector<double> best_hist;                          // per generation >= 1 (R12)
     if (history) history->push_back(*std::min_element(E.begin(), E.end()));
     while (evals < max_evals && gen < P.max_gens) {
         ++gen;
@@ -577,11 +673,18 @@ RunResult dock_run(const OGrid& G, const OLig& L, const OPar& P, int run, int Pn
         for (int s = 1; s < Pn; ++s) nE[s] = score(G, L, P, &npop[(size_t)s * Gn], nullptr, nullptr, nullptr);
         evals += Pn - 1;
         int n_ls = ls_pick(P, Pn, run, gen, seed, picks.data());
-        for (int l = 0; l < n_ls; ++l)                      // Lamarckian write-back
-            evals += adadelta_dock(G, L, P, &npop[(size_t)picks[l] * Gn], &nE[picks[l]], nullptr, nullptr);
+        for (int l = 0; l < n_ls; ++l) {                    // Lamarckian write-back
+            double* xl = &npop[(size_t)picks[l] * Gn];
+            if (P.ls_method == 1)
+                evals += solis_wets_dock(G, L, P, seed, (uint32_t)(run * Pn + picks[l]), (uint32_t)gen, xl, &nE[picks[l]], nullptr, nullptr, nullptr);
+            else
+                evals += adadelta_dock(G, L, P, xl, &nE[picks[l]], nullptr, nullptr);
+        }
         pop.swap(npop);
         E.swap(nE);
-        if (history) history->push_back(*std::min_element(E.begin(), E.end()));
+        best_hist.push_back(*std::min_element(E.begin(), E.end()));
+        if (history) history->push_back(best_hist.back());
+        if (autostop_hit(P, best_hist)) break;
     }
     int b = 0;
     for (int s = 1; s < Pn; ++s) if (E[s] < E[b]) b = s;
@@ -701,6 +804,22 @@ int orc_adadelta_rn(int n, double* x, double rho, double eps, int iters, orc_fn 
         for (int d = 0; d < n; ++d) x[d] += delta[d];
     }
     return 0;
+}
+
+// generic R^n Solis-Wets (R11) on a callback; step = x + sign*delta; x0's value E0 is passed in (carried energy)
+struct SwRn : SwFn {
+    int n; orc_fn fn; void* user;
+    double operator()(const double* x) override { return fn(n, x, nullptr, user); }
+    void step(double* x, const double* delta, double sign) override { for (int d = 0; d < n; ++d) x[d] += sign * delta[d]; }
+};
+int orc_solis_wets_rn(int n, double* x, double* E, const double* amp, const OPar* P, unsigned long long seed, unsigned id, unsigned gen,
+                      orc_fn fn, void* user, int* iters, double* rho_out, double* traceE) {
+    SwRn f; f.n = n; f.fn = fn; f.user = user;
+    return solis_wets(f, n, n, amp, *P, seed, id, gen, x, E, iters, rho_out, traceE);
+}
+int orc_solis_wets(void* grid, void* lig, const OPar* P, unsigned long long seed, unsigned id, unsigned gen, double* geno, double* E,
+                   int* iters, double* rho_out, double* traceE) {
+    return solis_wets_dock(*(OGrid*)grid, *(OLig*)lig, *P, seed, id, gen, geno, E, iters, rho_out, traceE);
 }
 
 int orc_apply_step(int R, double* x, const double* delta) { apply_step(R, x, delta); return 0; }

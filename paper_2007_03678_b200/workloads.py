@@ -28,6 +28,9 @@ DEFAULT_PARAMS = dict(
     w_desolv=W_DS, ds_sigma=DS_SIGMA, qasp=0.01097, r_min=0.5, k_wall=1000.0,
     ad_rho=0.8, ad_eps=1e-2, lsit=300, lsrat=0.06,
     tourn_prob=0.60, xover_rate=0.80, mut_rate=0.02, dmov=2.0, dang=math.pi / 2, max_gens=27000,
+    # R11 Solis-Wets [LIT] and R12 autostop [CHOICE]; ls_method 0 = ADADELTA, 1 = Solis-Wets
+    ls_method=0, sw_rho0=1.0, sw_rho_lb=0.01, sw_expand=2.0, sw_contract=0.5, sw_bias_keep=0.6, sw_bias_gain=0.4,
+    sw_bias_decay=0.5, sw_max_succ=4, sw_max_fail=4, autostop=0, as_window=10, as_tol=0.15,
 )
 
 
