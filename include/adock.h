@@ -56,8 +56,19 @@ typedef struct adock_params {
     float lsrat;       /* fraction of the population refined per generation (R9) */
     float tourn_prob, xover_rate, mut_rate; /* GA probabilities (R9) */
     float dmov, dang;  /* mutation amplitudes: Angstrom, radians (R9) */
-    int lsit;          /* ADADELTA iterations per local search, 1 eval each (R7) */
+    int lsit;          /* local-search iterations: ADADELTA 1 eval each (R7); Solis-Wets 1 or 2 evals each (R11) */
     int max_gens;      /* generation cap (R9) */
+    /* Local-search method ("Solis-Wets" or "ADADELTA"): 0 = ADADELTA (R7),
+     * 1 = Solis-Wets (R11; Solis & Wets 1981 rule, gradient-free). */
+    int ls_method;
+    int sw_max_succ, sw_max_fail; /* R11: consecutive successes / failures that expand / contract the step scale */
+    /* Autostop (R12): when non-zero a run ends after generation g >= as_window once the
+     * std-dev of its best energy over the last as_window (1..64) generations is < as_tol (kcal/mol). */
+    int autostop, as_window;
+    float sw_rho0, sw_rho_lb;       /* R11: initial step scale; the search ends when the scale falls below sw_rho_lb */
+    float sw_expand, sw_contract;   /* R11: scale factors (2, 0.5) */
+    float sw_bias_keep, sw_bias_gain, sw_bias_decay; /* R11: b <- keep b +- gain delta on success, decay b on failure */
+    float as_tol;
 } adock_params;
 
 /* Fills *out with the defaults listed in DESIGN.md. */
@@ -129,6 +140,16 @@ int adock_score_batch_host(const adock_grids* grids, const adock_ligand* ligand,
 int adock_local_search(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
                        float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, float* d_trace,
                        void* cuda_stream);
+
+/* Solis-Wets local search (R11; Solis & Wets 1981) from each of n genotypes:
+ * d_genotypes device [n][gstride] in/out (the accepted genotype), d_energies device [n] IN/OUT: on entry the energy
+ * of each starting genotype (carried, not re-evaluated), on return the accepted energy; d_evals device [n] out
+ * (evaluations used: 1 or 2 per iteration) or NULL; d_trace device [n][params->lsit] out or NULL: the accepted
+ * energy after iteration k.  Chain i draws its steps from Philox (R8) with counter (it*ceil(D/4)+d/4, 6, i,
+ * generation) and key seed.  Runs params->lsit iterations at most, whatever params->ls_method says. */
+int adock_solis_wets(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
+                     float* d_genotypes, int n, int gstride, float* d_energies, int* d_evals, float* d_trace,
+                     unsigned long long seed, unsigned int generation, void* cuda_stream);
 
 /* Philox4x32-10 (R8): out[i] = philox(key, ctr[i]); key host uint32[2], d_ctr/d_out device uint32 [n][4]. */
 int adock_philox(const unsigned int key[2], const unsigned int* d_ctr, int n, unsigned int* d_out, void* cuda_stream);

@@ -19,7 +19,7 @@ ADOCK_OK, ADOCK_EINVAL, ADOCK_ENOMEM, ADOCK_ECUDA, ADOCK_ELIMIT = 0, -1, -2, -3,
 EXPORTS = ["adock_default_params", "adock_load_grids", "adock_free_grids", "adock_load_ligand", "adock_free_ligand",
            "adock_ligand_pairs", "adock_ligand_tree", "adock_ligand_image", "adock_score_batch", "adock_score_batch_host", "adock_local_search",
            "adock_philox", "adock_ga_generation", "adock_dock", "adock_dock_many", "adock_launch_count", "adock_last_error", "adock_profile", "adock_profile_read",
-           "adock_ligand_lane_image", "adock_set_path", "adock_last_dock_path"]
+           "adock_ligand_lane_image", "adock_set_path", "adock_last_dock_path", "adock_solis_wets"]
 
 
 class AdockError(RuntimeError):
@@ -32,7 +32,9 @@ class adock_params(C.Structure):
     _fields_ = [(k, C.c_float) for k in (
         "elec_scale", "diel_A", "diel_B", "diel_k", "diel_lambda", "w_desolv", "ds_sigma", "qasp", "r_min", "k_wall",
         "ad_rho", "ad_eps", "lsrat", "tourn_prob", "xover_rate", "mut_rate", "dmov", "dang")] + [
-        ("lsit", C.c_int), ("max_gens", C.c_int)]
+        (k, C.c_int) for k in ("lsit", "max_gens", "ls_method", "sw_max_succ", "sw_max_fail", "autostop", "as_window")] + [
+        (k, C.c_float) for k in ("sw_rho0", "sw_rho_lb", "sw_expand", "sw_contract", "sw_bias_keep", "sw_bias_gain",
+                                 "sw_bias_decay", "as_tol")]
 
 
 def lib():
@@ -64,6 +66,7 @@ def lib():
         L.adock_score_batch.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, ci, vp]
         L.adock_score_batch_host.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, ci, vp]
         L.adock_local_search.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, vp]
+        L.adock_solis_wets.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, C.c_ulonglong, C.c_uint, vp]
         L.adock_philox.argtypes = [vp, vp, ci, vp, vp]
         L.adock_ga_generation.argtypes = [vp, vp, pp, ci, ci, ci, C.c_ulonglong, vp, vp, vp, vp, vp, C.POINTER(ci), vp]
         L.adock_dock.argtypes = [vp, vp, pp, ci, ci, C.c_longlong, C.c_ulonglong, vp, vp, vp, vp, vp, vp]
@@ -217,6 +220,15 @@ def adock_local_search(grids: Grids, lig: Ligand, params, d_genotypes, d_energie
         assert tuple(d_trace.shape) == (n, params.lsit)
     _check(lib().adock_local_search(grids.h, lig.h, C.byref(params) if params is not None else None, _dp(d_genotypes), n, gs,
                                     _dp(d_energies), _dp(d_iters), _dp(d_trace), _stream()))
+
+
+def adock_solis_wets(grids: Grids, lig: Ligand, params, d_genotypes, d_energies, seed, generation, d_evals=None, d_trace=None):
+    """d_energies: in (energies of the starting genotypes) / out (accepted energies)"""
+    n, gs = d_genotypes.shape
+    if d_trace is not None:
+        assert tuple(d_trace.shape) == (n, params.lsit)
+    _check(lib().adock_solis_wets(grids.h, lig.h, C.byref(params) if params is not None else None, _dp(d_genotypes), n, gs,
+                                  _dp(d_energies), _dp(d_evals), _dp(d_trace), int(seed), int(generation), _stream()))
 
 
 def adock_philox(key, d_ctr, d_out):

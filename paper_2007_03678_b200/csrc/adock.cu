@@ -80,6 +80,9 @@ extern "C" int adock_default_params(adock_params* p) {
     p->ad_rho = 0.8f; p->ad_eps = 1e-2f; p->lsrat = 0.06f;
     p->tourn_prob = 0.60f; p->xover_rate = 0.80f; p->mut_rate = 0.02f; p->dmov = 2.0f; p->dang = 1.57079632679489662f;
     p->lsit = 300; p->max_gens = 27000;
+    p->ls_method = 0; p->sw_max_succ = 4; p->sw_max_fail = 4; p->autostop = 0; p->as_window = 10;
+    p->sw_rho0 = 1.0f; p->sw_rho_lb = 0.01f; p->sw_expand = 2.0f; p->sw_contract = 0.5f;
+    p->sw_bias_keep = 0.6f; p->sw_bias_gain = 0.4f; p->sw_bias_decay = 0.5f; p->as_tol = 0.15f;
     return ADOCK_OK;
 }
 
@@ -95,6 +98,10 @@ static ParDev make_pardev(const adock_params& p) {
     d.ad_rho = p.ad_rho; d.ad_eps = p.ad_eps;
     d.tourn_prob = p.tourn_prob; d.xover_rate = p.xover_rate; d.mut_rate = p.mut_rate; d.dmov = p.dmov; d.dang = p.dang;
     d.lsit = p.lsit;
+    d.ls_method = p.ls_method; d.sw_max_succ = p.sw_max_succ; d.sw_max_fail = p.sw_max_fail;
+    d.autostop = p.autostop; d.as_window = p.as_window;
+    d.sw_rho0 = p.sw_rho0; d.sw_rho_lb = p.sw_rho_lb; d.sw_expand = p.sw_expand; d.sw_contract = p.sw_contract;
+    d.sw_bias_keep = p.sw_bias_keep; d.sw_bias_gain = p.sw_bias_gain; d.sw_bias_decay = p.sw_bias_decay; d.as_tol = p.as_tol;
     return d;
 }
 
@@ -104,6 +111,12 @@ static int check_params(const adock_params* in, const adock_ligand* l, adock_par
     for (int i = 0; i < 18; ++i)
         if (!std::isfinite(f[i])) return fail(ADOCK_EINVAL, "non-finite parameter");
     if (!(out.ds_sigma > 0) || !(out.r_min > 0) || !(out.elec_scale >= 0) || out.lsit < 0 || out.max_gens < 0 || !(out.ad_eps > 0))
+        return fail(ADOCK_EINVAL, "parameter out of range");
+    const float* f2 = &out.sw_rho0;
+    for (int i = 0; i < 7; ++i)
+        if (!std::isfinite(f2[i])) return fail(ADOCK_EINVAL, "non-finite parameter");
+    if (out.ls_method < 0 || out.ls_method > 1 || out.sw_max_succ < 1 || out.sw_max_fail < 1 || !(out.sw_rho0 > 0) ||
+        !(out.sw_expand > 0) || !(out.sw_contract > 0) || std::isnan(out.as_tol) || (out.autostop && (out.as_window < 1 || out.as_window > kAsMaxWindow)))
         return fail(ADOCK_EINVAL, "parameter out of range");
     if (l && !l->d_blob) return fail(ADOCK_EINVAL, "host-only ligand handle (loaded with grids == NULL)");
     if (l && (out.w_desolv != l->w_desolv || out.qasp != l->qasp || out.elec_scale != l->elec_scale))
@@ -569,6 +582,8 @@ struct LsArgs {
     int* iters;
     float* trace;
     int blob_bytes, n, gstride;
+    unsigned long long seed;    // Solis-Wets (R11): Philox key; chain i draws with id = i, generation = gen
+    unsigned int gen;
 };
 
 __global__ void __launch_bounds__(128) ls_array_kernel(GridDev G, ParDev P, LsArgs a) {
@@ -584,8 +599,9 @@ __global__ void __launch_bounds__(128) ls_array_kernel(GridDev G, ParDev P, LsAr
     for (int d = lane; d < Gn; d += 32) S.geno[d] = a.genos[(size_t)idx * a.gstride + d];
     __syncwarp();
     int iters = 0;
-    const float e = adadelta_search(L, G, P, S, lane, __int_as_float(0x7fc00000), iters,
-                                    a.trace ? a.trace + (size_t)idx * P.lsit : nullptr);
+    float* tr = a.trace ? a.trace + (size_t)idx * P.lsit : nullptr;
+    const float e = P.ls_method == 1 ? solis_wets_search(L, G, P, S, lane, a.E[idx], a.seed, (uint32_t)idx, a.gen, iters, tr)
+                                     : adadelta_search(L, G, P, S, lane, __int_as_float(0x7fc00000), iters, tr);
     for (int d = lane; d < Gn; d += 32) a.genos[(size_t)idx * a.gstride + d] = S.best[d];
     if (lane == 0) {
         a.E[idx] = e;
@@ -595,7 +611,7 @@ __global__ void __launch_bounds__(128) ls_array_kernel(GridDev G, ParDev P, LsAr
 
 // lane-per-individual variant: lane c of the launch's groups runs chain c; ADADELTA state in global scratch columns
 // [row][all group lanes of the launch]
-template <int K>
+template <int K, bool SW>
 __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) ls_array_lane_kernel(GridDev G, ParDev P, LsArgs a, float* __restrict__ scratch) {
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char* blob = smem + 16;
@@ -614,8 +630,9 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) ls_array_lane_k
     ls.best = scratch + tid; ls.Eg2 = ls.best + (size_t)Gn * T; ls.Ed2 = ls.Eg2 + (size_t)D * T; ls.grad = ls.Ed2 + (size_t)D * T;
     ls.stride = (int)T;
     int iters = 0;
-    const float e = lane_adadelta<K>(L, G, P, S, ls, act, __int_as_float(0x7fc00000), iters,
-                                     a.trace ? a.trace + idx * P.lsit : nullptr, 1);
+    float* tr = a.trace ? a.trace + idx * P.lsit : nullptr;
+    const float e = SW ? lane_solis_wets<K>(L, G, P, S, ls, act, (act && S.part == 0) ? a.E[idx] : 0.f, a.seed, (uint32_t)idx, a.gen, iters, tr, 1)
+                       : lane_adadelta<K>(L, G, P, S, ls, act, __int_as_float(0x7fc00000), iters, tr, 1);
     if (act && S.part == 0) {
         for (int d = 0; d < Gn; ++d) a.genos[idx * a.gstride + d] = ls.best[(size_t)d * T];
         a.E[idx] = e;
@@ -623,7 +640,7 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) ls_array_lane_k
     }
 }
 
-template <int K>
+template <int K, bool SW>
 static int launch_ls_array_lane(const adock_grids* grids, const adock_ligand* ligand, const ParDev& P, LsArgs a, int n, cudaStream_t stm) {
     const LaneGeom g = lane_geom(ligand);
     const int ngroups = (n + 31) / 32;
@@ -635,9 +652,9 @@ static int launch_ls_array_lane(const adock_grids* grids, const adock_ligand* li
     float* scratch = nullptr;
     cudaError_t e = cudaMallocAsync(&scratch, T * (size_t)(7 + R + 3 * (6 + R)) * 4, stm);
     if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("ls scratch: ") + cudaGetErrorString(e));
-    e = cudaFuncSetAttribute(ls_array_lane_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    e = cudaFuncSetAttribute(ls_array_lane_kernel<K, SW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) {
-        ls_array_lane_kernel<K><<<grid, NG * K * 32, smem, stm>>>(grids->dev, P, a, scratch);
+        ls_array_lane_kernel<K, SW><<<grid, NG * K * 32, smem, stm>>>(grids->dev, P, a, scratch);
         ++g_launches;
         e = cudaGetLastError();
     }
@@ -646,9 +663,10 @@ static int launch_ls_array_lane(const adock_grids* grids, const adock_ligand* li
     return ADOCK_OK;
 }
 
-extern "C" int adock_local_search(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
-                                  float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, float* d_trace,
-                                  void* cuda_stream) {
+// method: 0 = ADADELTA, 1 = Solis-Wets (d_energies then carries the starting energies in)
+static int local_search_impl(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params, int method,
+                             float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, float* d_trace,
+                             unsigned long long seed, unsigned int gen, void* cuda_stream) {
     if (!grids || !ligand) return fail(ADOCK_EINVAL, "NULL handle");
     if (n < 0) return fail(ADOCK_EINVAL, "n < 0");
     if (n == 0) return ADOCK_OK;
@@ -656,6 +674,7 @@ extern "C" int adock_local_search(const adock_grids* grids, const adock_ligand* 
     adock_params p;
     int rc = check_params(params, ligand, p);
     if (rc) return rc;
+    p.ls_method = method;
     rc = device_props();
     if (rc) return rc;
     if (g_path == 2 || (g_path == 0 && n >= kLaneMinChains && lane_ok(ligand))) {
@@ -663,11 +682,16 @@ extern "C" int adock_local_search(const adock_grids* grids, const adock_ligand* 
         if (!K) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
         ParDev P = make_pardev(p);
         P.k_wall_h = p.k_wall * grids->dev.h;
-        LsArgs a{ligand->d_lane, d_genotypes, d_energies, d_iters, d_trace, ligand->lane_bytes, n, gstride};
+        LsArgs a{ligand->d_lane, d_genotypes, d_energies, d_iters, d_trace, ligand->lane_bytes, n, gstride, seed, gen};
         cudaStream_t stm = (cudaStream_t)cuda_stream;
-        if (K == 1) return launch_ls_array_lane<1>(grids, ligand, P, a, n, stm);
-        if (K == 2) return launch_ls_array_lane<2>(grids, ligand, P, a, n, stm);
-        return launch_ls_array_lane<4>(grids, ligand, P, a, n, stm);
+        if (method == 1) {
+            if (K == 1) return launch_ls_array_lane<1, true>(grids, ligand, P, a, n, stm);
+            if (K == 2) return launch_ls_array_lane<2, true>(grids, ligand, P, a, n, stm);
+            return launch_ls_array_lane<4, true>(grids, ligand, P, a, n, stm);
+        }
+        if (K == 1) return launch_ls_array_lane<1, false>(grids, ligand, P, a, n, stm);
+        if (K == 2) return launch_ls_array_lane<2, false>(grids, ligand, P, a, n, stm);
+        return launch_ls_array_lane<4, false>(grids, ligand, P, a, n, stm);
     }
     const int W = fit_warps(ligand->blob_bytes, ligand->scratch_floats, 4);
     if (!W) return fail(ADOCK_ELIMIT, "ligand does not fit in shared memory");
@@ -675,11 +699,23 @@ extern "C" int adock_local_search(const adock_grids* grids, const adock_ligand* 
     CUDA_TRY(cudaFuncSetAttribute(ls_array_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ParDev P = make_pardev(p);
     P.k_wall_h = p.k_wall * grids->dev.h;
-    LsArgs a{ligand->d_blob, d_genotypes, d_energies, d_iters, d_trace, ligand->blob_bytes, n, gstride};
+    LsArgs a{ligand->d_blob, d_genotypes, d_energies, d_iters, d_trace, ligand->blob_bytes, n, gstride, seed, gen};
     ls_array_kernel<<<(n + W - 1) / W, W * 32, smem, (cudaStream_t)cuda_stream>>>(grids->dev, P, a);
     ++g_launches;
     CUDA_TRY(cudaGetLastError());
     return ADOCK_OK;
+}
+
+extern "C" int adock_local_search(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
+                                  float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, float* d_trace,
+                                  void* cuda_stream) {
+    return local_search_impl(grids, ligand, params, 0, d_genotypes, n, gstride, d_energies, d_iters, d_trace, 0ull, 0u, cuda_stream);
+}
+
+extern "C" int adock_solis_wets(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
+                                float* d_genotypes, int n, int gstride, float* d_energies, int* d_evals, float* d_trace,
+                                unsigned long long seed, unsigned int generation, void* cuda_stream) {
+    return local_search_impl(grids, ligand, params, 1, d_genotypes, n, gstride, d_energies, d_evals, d_trace, seed, generation, cuda_stream);
 }
 
 // =================================================================== LGA docking (rows a5-a7)
@@ -705,11 +741,14 @@ struct DockJob {
     int blob_bytes, Gn, N, R;
     const unsigned char* lane;  // lane-per-individual image (lane_image.hpp)
     int lane_bytes, pad0;
+    float* hist;            // [nrun][as_window] ring of each run's best energy per generation (R12 autostop) or NULL
 };
 struct DockDims {
     int nrun, P, n_ls, upj;         // upj = CTAs per job for this launch
     long long max_evals;
     int max_gens, gstride, cstride;
+    int autostop, as_window;        // R12
+    float as_tol;
 };
 
 #define DOCK_PROLOGUE(WARPS_EXPR)                                                                                         \
@@ -826,7 +865,9 @@ __global__ void __launch_bounds__(128) dock_ls_kernel(GridDev G, ParDev P, const
     for (int d = lane; d < Gn; d += 32) S.geno[d] = g[d];
     __syncwarp();
     int iters = 0;
-    const float be = adadelta_search(L, G, P, S, lane, *e, iters);
+    const float be = P.ls_method == 1
+                         ? solis_wets_search(L, G, P, S, lane, *e, job.seed, (uint32_t)(run * dm.P + slot), (uint32_t)st.gen + 1u, iters)
+                         : adadelta_search(L, G, P, S, lane, *e, iters);
     for (int d = lane; d < Gn; d += 32) g[d] = S.best[d];
     if (lane == 0) {
         *e = be;
@@ -864,7 +905,7 @@ __device__ __forceinline__ LaneCtaGroup lane_cta_group(unsigned char* smem, cons
 
 // ADADELTA on the selected individuals (Lamarckian write-back): lane c of a job's groups runs chain c = run*n_ls + l;
 // ADADELTA state in global scratch columns [row][all group lanes of the launch] (rows: Gmax best, 3 x Dmax)
-template <int K>
+template <int K, bool SW>
 __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_ls_lane_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs,
                                                                                      DockDims dm, LaneDockArgs a) {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -895,7 +936,9 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_ls_lane_ke
     ls.best = a.scratch + tid; ls.Eg2 = ls.best + (size_t)a.Gmax * T; ls.Ed2 = ls.Eg2 + (size_t)Dmax * T; ls.grad = ls.Ed2 + (size_t)Dmax * T;
     ls.stride = (int)T;
     int iters = 0;
-    const float be = lane_adadelta<K>(L, G, P, S, ls, act, (act && S.part == 0) ? *e : 0.f, iters, nullptr, 0);
+    const float e0 = (act && S.part == 0) ? *e : 0.f;
+    const float be = SW ? lane_solis_wets<K>(L, G, P, S, ls, act, e0, job.seed, (uint32_t)(run * dm.P + slot), (uint32_t)st.gen + 1u, iters, nullptr, 0)
+                        : lane_adadelta<K>(L, G, P, S, ls, act, e0, iters, nullptr, 0);
     if (act && S.part == 0) {
         for (int d = 0; d < Gn; ++d) g[d] = ls.best[(size_t)d * T];
         *e = be;
@@ -944,7 +987,24 @@ __global__ void dock_commit_kernel(const DockJob* __restrict__ jobs, int njobs, 
     s->ls_acc = 0;
     s->gen += 1;
     s->cur ^= 1;
-    s->active = (s->evals < dm.max_evals && s->gen < dm.max_gens) ? 1 : 0;
+    bool stop = false;
+    if (dm.autostop) {              // R12: std-dev of the run's best energy over the last as_window generations < as_tol
+        const DockJob& job = jobs[i / dm.nrun];
+        const int run = i % dm.nrun, W = dm.as_window;
+        const float* E = job.E + ((size_t)s->cur * dm.nrun + run) * dm.P;
+        float best = E[0];
+        for (int k = 1; k < dm.P; ++k) best = fminf(best, E[k]);
+        float* h = job.hist + (size_t)run * W;
+        h[(s->gen - 1) % W] = best;
+        if (s->gen >= W) {
+            float m = 0.f, v = 0.f;
+            for (int k = 0; k < W; ++k) m += h[k];
+            m /= (float)W;
+            for (int k = 0; k < W; ++k) { const float d = h[k] - m; v += d * d; }
+            stop = sqrtf(v / (float)W) < dm.as_tol;
+        }
+    }
+    s->active = (!stop && s->evals < dm.max_evals && s->gen < dm.max_gens) ? 1 : 0;
     if (s->active) atomicOr(any_active, 1);
 }
 
@@ -1054,6 +1114,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     DockDims dm{};
     dm.nrun = nrun; dm.P = Pn; dm.n_ls = n_ls_of(p, Pn); dm.max_evals = max_evals; dm.max_gens = p.max_gens;
     dm.gstride = gstride; dm.cstride = cstride;
+    dm.autostop = p.autostop; dm.as_window = p.as_window; dm.as_tol = p.as_tol;
 
     DevBuf buf;
     std::vector<DockJob> jobs(nlig);
@@ -1080,6 +1141,8 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         if (e == cudaSuccess) e = buf.alloc(&j.st, (size_t)nrun * sizeof(RunState));
         if (e == cudaSuccess) e = buf.alloc(&j.picks, popsz * 4);
         if (e == cudaSuccess) e = buf.alloc(&j.fy, popsz * 4);
+        j.hist = nullptr;
+        if (e == cudaSuccess && p.autostop) e = buf.alloc(&j.hist, (size_t)nrun * p.as_window * 4);
         j.out_geno = d_out_geno + (size_t)l * nrun * gstride;
         j.out_E = d_out_E + (size_t)l * nrun;
         j.out_xyz = d_out_xyz ? d_out_xyz + (size_t)l * nrun * cstride * 3 : nullptr;
@@ -1109,9 +1172,12 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         cudaError_t e2 = buf.alloc(&d_lscratch, T * (size_t)(Gmax + 3 * (Gmax - 1)) * 4);
         if (e2 != cudaSuccess) return fail(e2 == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("dock alloc: ") + cudaGetErrorString(e2));
         al = LaneDockArgs{d_lscratch, Gmax, pl.ng, nlig * jg, jg, pl.slot, pl.nimg, pl.gfloats};
-        if (pl.K == 1) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-        if (pl.K == 2) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-        if (pl.K == 4) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        if (pl.K == 1) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        if (pl.K == 2) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        if (pl.K == 4) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        if (pl.K == 1) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        if (pl.K == 2) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        if (pl.K == 4) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
     }
     if (ga_lane) {
         as = LaneDockArgs{nullptr, Gmax, ps.ng, nlig * jgs, jgs, ps.slot, ps.nimg, ps.gfloats};
@@ -1122,9 +1188,13 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     }
     auto launch_ls = [&]() {
         const int thr = pl.ng * pl.K * 32;
-        if (ls_lane && pl.K == 1) dock_ls_lane_kernel<1><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
-        else if (ls_lane && pl.K == 2) dock_ls_lane_kernel<2><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
-        else if (ls_lane) dock_ls_lane_kernel<4><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
+        const bool sw = p.ls_method == 1;
+        if (ls_lane && pl.K == 1 && !sw) dock_ls_lane_kernel<1, false><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
+        else if (ls_lane && pl.K == 2 && !sw) dock_ls_lane_kernel<2, false><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
+        else if (ls_lane && !sw) dock_ls_lane_kernel<4, false><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
+        else if (ls_lane && pl.K == 1) dock_ls_lane_kernel<1, true><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
+        else if (ls_lane && pl.K == 2) dock_ls_lane_kernel<2, true><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
+        else if (ls_lane) dock_ls_lane_kernel<4, true><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
         else dock_ls_kernel<<<dls.upj * nlig, Wls * 32, smem_ls, stm>>>(grids->dev, P, d_jobs, dls);
     };
     // one GA generation: offspring + their energies (one launch, or two when the scoring runs lane-per-individual)

@@ -30,7 +30,11 @@ struct ParDev {             // adock_params with the per-pair constants folded
     float ad_rho, ad_eps;
     float tourn_prob, xover_rate, mut_rate, dmov, dang;
     int lsit;
+    // R11 Solis-Wets, R12 autostop
+    int ls_method, sw_max_succ, sw_max_fail, autostop, as_window;
+    float sw_rho0, sw_rho_lb, sw_expand, sw_contract, sw_bias_keep, sw_bias_gain, sw_bias_decay, as_tol;
 };
+constexpr int kAsMaxWindow = 64;
 
 // ---------------------------------------------------------------- shared-memory views
 struct LigS {
@@ -462,7 +466,7 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t k0, uint32_t k1, uint4 c
     }
     return c;
 }
-enum : uint32_t { kInit = 0, kTournA = 1, kTournB = 2, kXover = 3, kMut = 4, kLsPick = 5 };
+enum : uint32_t { kInit = 0, kTournA = 1, kTournB = 2, kXover = 3, kMut = 4, kLsPick = 5, kSolisWets = 6 };
 __device__ __forceinline__ uint4 draw4(unsigned long long seed, uint32_t draw, uint32_t purpose, uint32_t id, uint32_t gen) {
     return philox4x32_10((uint32_t)seed, (uint32_t)(seed >> 32), make_uint4(draw, purpose, id, gen));
 }
@@ -634,6 +638,81 @@ __device__ inline float adadelta_search(const LigS& L, const GridDev& G, const P
     }
     iters = it;
     return isfinite(bestE) ? bestE : e_start;
+}
+
+// ---------------------------------------------------------------- Solis-Wets local search (R11), one warp
+// Start genotype in S.geno with carried energy e_start (not re-evaluated).  Per iteration: delta = rho*amp*(2u-1) + bias
+// (u: Philox word d&3 of draw (it*ceil(D/4) + d/4, kSolisWets, id, gen)); x (+) delta is tried, then x (-) delta; a
+// strictly better trial is accepted and pulls the bias its way, a double failure halves the bias; sw_max_succ
+// successes in a row expand rho, sw_max_fail failures contract it; ends at lsit iterations or rho < sw_rho_lb.
+// On return S.best holds the accepted genotype; returns its energy; evals = evaluations performed.
+__device__ inline float solis_wets_search(const LigS& L, const GridDev& G, const ParDev& P, const WarpS& S, int lane, float e_start,
+                                          unsigned long long seed, uint32_t id, uint32_t gen, int& evals, float* trace = nullptr) {
+    const int R = L.R, D = 6 + R, Gn = 7 + R, nq = (D + 3) / 4;
+    float bias[3] = {0.f, 0.f, 0.f}, delta[3] = {0.f, 0.f, 0.f};      // component d = lane + 32*c  (D <= 70)
+    for (int d = lane; d < Gn; d += 32) S.best[d] = S.geno[d];
+    __syncwarp();
+    float E = e_start, rho = P.sw_rho0;
+    int ns = 0, nf = 0, it = 0;
+    evals = 0;
+    while (it < P.lsit && !(rho < P.sw_rho_lb)) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const int d = lane + 32 * c;
+            if (d < D) {
+                const uint4 r = draw4(seed, (uint32_t)(it * nq + (d >> 2)), kSolisWets, id, gen);
+                const float xi = 2.f * u01(pick_word(r, d & 3)) - 1.f;
+                delta[c] = rho * (d < 3 ? P.dmov : P.dang) * xi + bias[c];
+            }
+        }
+        bool ok = false;
+        float e = E;
+        for (int trial = 0; trial < 2 && !ok; ++trial) {
+            const float sg = trial ? -1.f : 1.f;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const int d = lane + 32 * c;
+                if (d < D) S.grad[d] = sg * delta[c];
+            }
+            __syncwarp();
+            for (int gI = lane; gI < Gn; gI += 32) {
+                if (gI < 3) S.geno[gI] = S.best[gI] + S.grad[gI];
+                else if (gI >= 7) S.geno[gI] = wrap_pi(S.best[gI] + S.grad[gI - 1]);
+            }
+            if (lane == 3) {
+                const float wx = S.grad[3], wy = S.grad[4], wz = S.grad[5];
+                const float th = sqrtf(wx * wx + wy * wy + wz * wz);
+                float sh, ch, nq4[4];
+                sincosf(0.5f * th, &sh, &ch);
+                const float k = th > 1e-12f ? sh / th : 0.5f;
+                rotate_quat(ch, k * wx, k * wy, k * wz, S.best + 3, nq4);
+                S.geno[3] = nq4[0]; S.geno[4] = nq4[1]; S.geno[5] = nq4[2]; S.geno[6] = nq4[3];
+            }
+            __syncwarp();
+            float ei, ea;
+            e = __shfl_sync(kFull, eval_pose<false>(L, G, P, S, lane, ei, ea), 0);
+            ++evals;
+            ok = e < E;
+            if (ok) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) bias[c] = P.sw_bias_keep * bias[c] + P.sw_bias_gain * (sg * delta[c]);
+            }
+        }
+        if (ok) {
+            for (int d = lane; d < Gn; d += 32) S.best[d] = S.geno[d];
+            E = e; ++ns; nf = 0;
+        } else {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) bias[c] *= P.sw_bias_decay;
+            ++nf; ns = 0;
+        }
+        __syncwarp();
+        if (ns >= P.sw_max_succ) { rho *= P.sw_expand; ns = 0; }
+        else if (nf >= P.sw_max_fail) { rho *= P.sw_contract; nf = 0; }
+        if (trace && lane == 0) trace[it] = E;
+        ++it;
+    }
+    return E;
 }
 
 }  // namespace adock

@@ -494,4 +494,87 @@ __device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const Pa
     return isfinite(bestE) ? bestE : e_start;
 }
 
+// ---------------------------------------------------------------- Solis-Wets chain of this thread (R11)
+// Start genotype in S.geno (visible to the whole group) with carried energy e_start.  Every pass of the loop is ONE
+// evaluation of the whole warp; each lane runs its own state machine (phase 0: try x (+) delta, phase 1: try x (-) delta),
+// so a lane whose first trial succeeded draws its next step at once instead of idling through the other lanes'
+// second trial.  Part 0 owns the state: x in ls.best, bias in ls.Eg2, delta in ls.Ed2 (global scratch columns).
+// On return ls.best holds the accepted genotype; part 0 returns its energy and the evaluations done.
+template <int K>
+__device__ inline float lane_solis_wets(const LaneL& L, const GridDev& G, const ParDev& P, const LaneS& S, const LaneLS& ls,
+                                        bool active, float e_start, unsigned long long seed, uint32_t id, uint32_t gen, int& evals,
+                                        float* trace, int trace_stride) {
+    const int R = L.R, D = 6 + R, Gn = 7 + R, nq = (D + 3) / 4;
+    const bool lead = S.part == 0;
+    float E = e_start, rho = P.sw_rho0;
+    int ns = 0, nf = 0, it = 0, phase = 0;
+    evals = 0;
+    if (lead) {
+        for (int d = 0; d < Gn; ++d) ls.best[d * ls.stride] = S.geno[d * 32];
+        for (int d = 0; d < D; ++d) ls.Eg2[d * ls.stride] = 0.f;
+    }
+    bool live = active && P.lsit > 0 && !(rho < P.sw_rho_lb);
+    for (;;) {
+        float sg = 1.f;
+        if (lead && live) {                             // candidate = x (+) sg*delta into S.geno
+            if (phase == 0) {
+                for (int q = 0; q < nq; ++q) {
+                    const uint4 r = draw4(seed, (uint32_t)(it * nq + q), kSolisWets, id, gen);
+                    for (int w = 0; w < 4 && 4 * q + w < D; ++w) {
+                        const int d = 4 * q + w;
+                        const float xi = 2.f * u01(pick_word(r, w)) - 1.f;
+                        ls.Ed2[d * ls.stride] = rho * (d < 3 ? P.dmov : P.dang) * xi + ls.Eg2[d * ls.stride];
+                    }
+                }
+            } else {
+                sg = -1.f;
+            }
+            for (int d = 0; d < 3; ++d) S.geno[d * 32] = ls.best[d * ls.stride] + sg * ls.Ed2[d * ls.stride];
+            const float wx = sg * ls.Ed2[3 * ls.stride], wy = sg * ls.Ed2[4 * ls.stride], wz = sg * ls.Ed2[5 * ls.stride];
+            const float th = sqrtf(wx * wx + wy * wy + wz * wz);
+            float sh, ch;
+            sincosf(0.5f * th, &sh, &ch);
+            const float k = th > 1e-12f ? sh / th : 0.5f;
+            const float q0[4] = {ls.best[3 * ls.stride], ls.best[4 * ls.stride], ls.best[5 * ls.stride], ls.best[6 * ls.stride]};
+            float nq4[4];
+            rotate_quat(ch, k * wx, k * wy, k * wz, q0, nq4);
+            S.geno[96] = nq4[0]; S.geno[128] = nq4[1]; S.geno[160] = nq4[2]; S.geno[192] = nq4[3];
+            for (int d = 6; d < D; ++d) S.geno[(d + 1) * 32] = wrap_pi(ls.best[(d + 1) * ls.stride] + sg * ls.Ed2[d * ls.stride]);
+        }
+        if (K > 1 && lead) S.ex[(2 * K) * 32] = live ? 1.f : 0.f;
+        group_sync<K>(S);                               // candidate and live flag visible; part 0 is done with the last pass
+        if (K > 1) live = S.ex[(2 * K) * 32] != 0.f;
+        if (!__any_sync(kFull, live)) break;            // same decision in every warp of the group
+        float ei, ea;
+        bool gfin = true;
+        const float e = lane_eval<false, K>(L, G, P, S, nullptr, 1, false, ei, ea, gfin);
+        if (lead && live) {
+            ++evals;
+            const bool ok = e < E;
+            bool done = true;
+            if (ok) {
+                E = e;
+                for (int d = 0; d < Gn; ++d) ls.best[d * ls.stride] = S.geno[d * 32];
+                for (int d = 0; d < D; ++d)
+                    ls.Eg2[d * ls.stride] = P.sw_bias_keep * ls.Eg2[d * ls.stride] + P.sw_bias_gain * (sg * ls.Ed2[d * ls.stride]);
+                ++ns; nf = 0;
+            } else if (phase == 0) {
+                phase = 1; done = false;
+            } else {
+                for (int d = 0; d < D; ++d) ls.Eg2[d * ls.stride] *= P.sw_bias_decay;
+                ++nf; ns = 0;
+            }
+            if (done) {
+                phase = 0;
+                if (ns >= P.sw_max_succ) { rho *= P.sw_expand; ns = 0; }
+                else if (nf >= P.sw_max_fail) { rho *= P.sw_contract; nf = 0; }
+                if (trace) trace[it * trace_stride] = E;
+                ++it;
+                live = it < P.lsit && !(rho < P.sw_rho_lb);
+            }
+        }
+    }
+    return E;
+}
+
 }  // namespace adock

@@ -449,3 +449,106 @@ def test_host_only_handle_is_rejected_by_compute_calls(B, cases, dev):
     with pytest.raises(B.AdockError) as e:
         B.adock_score_batch(c.gg, hl, c.gp, torch.zeros((4, 9), device=dev), torch.zeros(4, device=dev), None, None)
     assert e.value.code == B.ADOCK_EINVAL
+
+
+# ------------------------------------------------------------------------------- Solis-Wets local search (R11)
+def _sw_run(B, c, dev, G, E0, seed, gen, trace=True):
+    n = G.shape[0]
+    d_g = torch.from_numpy(G).to(dev)
+    d_E = torch.from_numpy(E0.astype(np.float32)).to(dev)
+    d_ev = torch.zeros(n, dtype=torch.int32, device=dev)
+    d_tr = torch.full((n, c.gp.lsit), float("nan"), device=dev) if trace else None
+    B.adock_solis_wets(c.gg, c.gl, c.gp, d_g, d_E, seed, gen, d_ev, d_tr)
+    torch.cuda.synchronize()
+    return d_g.cpu().numpy(), d_E.cpu().numpy().astype(np.float64), d_ev.cpu().numpy(), (d_tr.cpu().numpy() if trace else None)
+
+
+def test_solis_wets_first_iterations_track_oracle(B, orc, W, cases, dev, family):
+    """same Philox words -> same proposals; the accepted-energy trace and the evaluation count agree with the oracle
+    until an `e < E` decision falls inside the fp32 noise (rare in 10 iterations)."""
+    c = cases("tiny", lsit=10, ls_method=1)
+    n = 96
+    G = W.make_genotypes(n, c.lig.R, c.grids, seed=31, wall_tail=0.0)
+    E0 = orc.score(c.og, c.ol, c.op, G, want_grad=False)["E"]
+    g, E, ev, tr = _sw_run(B, c, dev, G, E0, seed=77, gen=3)
+    same = 0
+    for i in range(n):
+        og_, oE, oev, oit, orho, otr = orc.solis_wets(c.og, c.ol, c.op, G[i].astype(np.float64), float(np.float32(E0[i])), 77, i, 3)
+        k = oit
+        ok = ev[i] == oev and np.all(np.abs(tr[i, :k] - otr[:k]) <= np.maximum(1e-4 * np.abs(otr[:k]), 1e-3)) and np.isnan(tr[i, k:]).all()
+        same += bool(ok)
+    assert same >= 0.9 * n, f"only {same}/{n} chains follow the oracle's trace"
+
+
+def test_solis_wets_statistics_match_oracle(B, orc, W, cases, dev, family):
+    c = cases("drug", lsit=60, ls_method=1)
+    n = 256
+    G = W.make_genotypes(n, c.lig.R, c.grids, seed=23, wall_tail=0.0)
+    E0 = orc.score(c.og, c.ol, c.op, G, want_grad=False)["E"]
+    g, gE, ev, _ = _sw_run(B, c, dev, G, E0, seed=5, gen=1, trace=False)
+    assert (gE <= E0 + np.maximum(1e-4 * np.abs(E0), 1e-3)).all()                       # never worse than the start
+    assert ((ev >= 1) & (ev <= 120)).all()
+    chk = orc.score(c.og, c.ol, c.op, g, want_grad=False)["E"]
+    assert_energy(gE.astype(np.float32), chk, "Solis-Wets result")
+    assert np.allclose(np.linalg.norm(g[:, 3:7], axis=1), 1.0, atol=1e-5)
+    o = [orc.solis_wets(c.og, c.ol, c.op, G[i].astype(np.float64), float(np.float32(E0[i])), 5, i, 1) for i in range(n)]
+    oE, oev = np.array([x[1] for x in o]), np.array([x[2] for x in o])
+    assert stats.ks_2samp(gE, oE).pvalue > 0.01
+    assert stats.ks_2samp(ev, oev).pvalue > 0.01
+
+
+def test_dock_solis_wets_distribution_matches_oracle(B, orc, cases, family):
+    c = cases("tiny", lsit=30, ls_method=1)
+    P, nrun, max_evals = 16, 20, 16 + 20 * (15 + 45)
+    g, o, ge, oe = [], [], [], []
+    for seed in range(5):
+        rg = B.adock_dock(c.gg, c.gl, c.gp, nrun, P, max_evals, seed=seed)
+        ro = orc.dock(c.og, c.ol, c.op, nrun, P, max_evals, seed=seed)
+        g.append(rg["energies"].astype(np.float64)); o.append(ro["energies"])
+        ge.append(rg["evals"] / np.maximum(rg["gens"], 1)); oe.append(ro["evals"] / np.maximum(ro["gens"], 1))
+        chk = orc.score(c.og, c.ol, c.op, rg["genotypes"], want_grad=False)["E"]
+        assert_energy(rg["energies"], chk, "dock result energy")
+        # accounting: P + gens (P-1) <= evals <= P + gens (P-1 + n_ls 2 lsit), n_ls = ceil(0.06*16) = 1
+        assert ((rg["evals"] >= P + rg["gens"] * (P - 1)) & (rg["evals"] <= P + rg["gens"] * (P - 1 + 2 * 30))).all()
+    g, o = np.concatenate(g), np.concatenate(o)
+    assert stats.ks_2samp(g, o).pvalue > 0.01
+    assert stats.mannwhitneyu(g, o).pvalue > 0.01
+    assert stats.ks_2samp(np.concatenate(ge), np.concatenate(oe)).pvalue > 0.01        # evals per generation
+
+
+# ------------------------------------------------------------------------------- autostop (R12)
+def test_autostop_limits(B, orc, cases, family):
+    """as_tol huge: every run ends at generation as_window exactly (as in the oracle); as_tol = 0: never fires, the
+    docking is bit-identical to the one without autostop."""
+    P, nrun = 16, 6
+    c_inf = cases("tiny", lsit=10, autostop=1, as_window=5, as_tol=1e30)
+    r = B.adock_dock(c_inf.gg, c_inf.gl, c_inf.gp, nrun, P, 10 ** 6, seed=3)
+    ro = orc.dock(c_inf.og, c_inf.ol, c_inf.op, nrun, P, 10 ** 6, seed=3)
+    assert (r["gens"] == 5).all() and (ro["gens"] == 5).all()
+    assert (r["evals"] == P + 5 * (P - 1 + 10)).all() and np.array_equal(r["evals"], ro["evals"])
+    c_off = cases("tiny", lsit=10, max_gens=12)
+    c_zero = cases("tiny", lsit=10, max_gens=12, autostop=1, as_window=5, as_tol=0.0)
+    a = B.adock_dock(c_off.gg, c_off.gl, c_off.gp, nrun, P, 10 ** 6, seed=3)
+    b = B.adock_dock(c_zero.gg, c_zero.gl, c_zero.gp, nrun, P, 10 ** 6, seed=3)
+    assert (a["gens"] == 12).all() and np.array_equal(a["gens"], b["gens"])
+    assert np.array_equal(a["energies"], b["energies"]) and np.array_equal(a["genotypes"], b["genotypes"])
+
+
+def test_autostop_ends_converged_runs_like_the_oracle(B, orc, W, family):
+    """bowl maps + rigid ligand: every run converges in a few generations and autostop ends it long before the budget,
+    at the known minimiser; the generation counts are distributed as the oracle's."""
+    n, T, h = 40, 2, 0.375
+    centre = 0.5 * (n - 1) * h
+    ax = np.arange(n) * h - centre
+    bowl = 0.05 * (ax[:, None, None] ** 2 + ax[None, :, None] ** 2 + ax[None, None, :] ** 2)
+    maps = np.zeros((T + 2, n, n, n), np.float32); maps[:T] = bowl
+    lig = W.make_ligand(10, 0, T, seed=5, centre=(centre,) * 3)
+    d = dict(W.DEFAULT_PARAMS, lsit=60, autostop=1, as_window=6, as_tol=0.01)
+    gp, op = B.make_params(d), orc.params(d)
+    gg = B.Grids(maps, h, np.zeros(3, np.float32)); gl = B.Ligand.from_workload(gg, lig, gp)
+    og = orc.Grids(maps, h, np.zeros(3, np.float32)); ol = orc.Ligand.from_workload(lig)
+    r = B.adock_dock(gg, gl, gp, 24, 30, 200000, seed=2)
+    ro = orc.dock(og, ol, op, 24, 30, 200000, seed=2)
+    assert (r["evals"] < 200000).all() and (r["gens"] >= 6).all()
+    assert np.abs(r["genotypes"][:, :3] - centre).max() < 0.1
+    assert stats.ks_2samp(r["gens"], ro["gens"]).pvalue > 0.01
