@@ -742,6 +742,8 @@ struct DockJob {
     const unsigned char* lane;  // lane-per-individual image (lane_image.hpp)
     int lane_bytes, pad0;
     float* hist;            // [nrun][as_window] ring of each run's best energy per generation (R12 autostop) or NULL
+    int* act;               // act[0] = number of active runs, act[1 + k] = k-th active run (ascending): the lane kernels
+                            // deal their lanes out over the active runs only (runs end at different generations)
 };
 struct DockDims {
     int nrun, P, n_ls, upj;         // upj = CTAs per job for this launch
@@ -917,9 +919,9 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_ls_lane_ke
     const LaneS S = lane_scratch<K>(cg.scratch, L, warp, lane, a.group_floats);
     const int Gn = job.Gn;
     const int c = cg.gi * 32 + lane;
-    bool act = c < dm.nrun * dm.n_ls;
+    bool act = c < job.act[0] * dm.n_ls;
     const int cc = act ? c : 0;
-    const int run = cc / dm.n_ls, l = cc % dm.n_ls;
+    const int run = job.act[1 + cc / dm.n_ls], l = cc % dm.n_ls;
     const RunState st = job.st[run];
     act = act && st.active;
     if (!__any_sync(kFull, act)) return;                // the same for every warp of the group
@@ -959,10 +961,11 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_score_lane
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const LaneS S = lane_scratch<K>(cg.scratch, L, warp, lane, a.group_floats);
     const int Gn = job.Gn;
-    const int c = cg.gi * 32 + lane, n = dm.nrun * dm.P;
+    const int c = cg.gi * 32 + lane, n = job.act[0] * dm.P;
     bool act = c < n;
-    const int cc = act ? c : n - 1;
-    const int run = cc / dm.P, slot = cc % dm.P;
+    const int ca = act ? c : 0;
+    const int run = job.act[1 + ca / dm.P], slot = ca % dm.P;
+    const int cc = run * dm.P + slot;
     const RunState st = job.st[run];
     act = act && st.active && slot != 0;
     if (!__any_sync(kFull, act)) return;
@@ -978,10 +981,21 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_score_lane
 }
 
 // end of generation: eval accounting, buffer flip, termination test
-__global__ void dock_commit_kernel(const DockJob* __restrict__ jobs, int njobs, DockDims dm, int* __restrict__ any_active) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= njobs * dm.nrun) return;
-    RunState* s = jobs[i / dm.nrun].st + (i % dm.nrun);
+// one CTA per job, threads over its runs; thread 0 then rebuilds the job's list of active runs
+__device__ __forceinline__ void dock_commit_run(const DockJob& job, int run, const DockDims& dm, int* __restrict__ any_active);
+__global__ void __launch_bounds__(128) dock_commit_kernel(const DockJob* __restrict__ jobs, int njobs, DockDims dm, int* __restrict__ any_active) {
+    const DockJob& job = jobs[blockIdx.x];
+    for (int run = threadIdx.x; run < dm.nrun; run += blockDim.x) dock_commit_run(job, run, dm, any_active);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int n = 0;
+        for (int run = 0; run < dm.nrun; ++run)
+            if (job.st[run].active) job.act[1 + n++] = run;
+        job.act[0] = n;
+    }
+}
+__device__ __forceinline__ void dock_commit_run(const DockJob& job, int run, const DockDims& dm, int* __restrict__ any_active) {
+    RunState* s = job.st + run;
     if (!s->active) return;
     s->evals += (long long)(dm.P - 1) + s->ls_acc;
     s->ls_acc = 0;
@@ -989,8 +1003,7 @@ __global__ void dock_commit_kernel(const DockJob* __restrict__ jobs, int njobs, 
     s->cur ^= 1;
     bool stop = false;
     if (dm.autostop) {              // R12: std-dev of the run's best energy over the last as_window generations < as_tol
-        const DockJob& job = jobs[i / dm.nrun];
-        const int run = i % dm.nrun, W = dm.as_window;
+        const int W = dm.as_window;
         const float* E = job.E + ((size_t)s->cur * dm.nrun + run) * dm.P;
         float best = E[0];
         for (int k = 1; k < dm.P; ++k) best = fminf(best, E[k]);
@@ -1102,13 +1115,16 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     }
     const int jg = (nrun * n_ls0 + 31) / 32;                        // groups of 32 chains per job
     const LanePlan pl = lane_plan(lg, (long long)nlig * jg, jg);
-    const bool ls_lane = pl.K > 0 && (g_path == 2 || (g_path == 0 && lanes_fit && chains >= kLaneMinChains));
+    // Solis-Wets chains end after very different numbers of evaluations (28 to lsit iterations), which leaves most lanes
+    // of a lane-per-chain warp idle; one warp per chain is 2x faster there (profiles/r01d_next_rows.md)
+    const bool many = g_path == 0 && lanes_fit && chains >= kLaneMinChains;
+    const bool ls_lane = pl.K > 0 && (g_path == 2 || (many && p.ls_method == 0));
     if (g_path == 2 && !pl.K) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
     g_last_dock_path = ls_lane ? 2 : 1;
     // offspring scoring: lane-per-individual under the same condition (populations are 1/lsrat times larger)
     const int jgs = (int)(((long long)nrun * Pn + 31) / 32);
     const LanePlan ps = lane_plan(lg, (long long)nlig * jgs, jgs);
-    const bool ga_lane = ls_lane && ps.K > 0;
+    const bool ga_lane = ps.K > 0 && (g_path == 2 || many);
     ParDev P = make_pardev(p);
     P.k_wall_h = p.k_wall * grids->dev.h;
     DockDims dm{};
@@ -1130,6 +1146,9 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     if (e == cudaSuccess) e = buf.alloc(&d_out_gens, (size_t)nlig * nrun * 4);
     if (e == cudaSuccess) e = buf.alloc(&d_flag, 4);
     if (e == cudaSuccess) e = buf.alloc(&d_jobs, (size_t)nlig * sizeof(DockJob));
+    std::vector<int> act0(nrun + 1);                    // every run starts active
+    act0[0] = nrun;
+    for (int r = 0; r < nrun; ++r) act0[1 + r] = r;
     for (int l = 0; l < nlig && e == cudaSuccess; ++l) {
         DockJob& j = jobs[l];
         const adock_ligand* lg = ligs[l];
@@ -1142,6 +1161,8 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         if (e == cudaSuccess) e = buf.alloc(&j.picks, popsz * 4);
         if (e == cudaSuccess) e = buf.alloc(&j.fy, popsz * 4);
         j.hist = nullptr;
+        if (e == cudaSuccess) e = buf.alloc(&j.act, (size_t)(nrun + 1) * 4);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(j.act, act0.data(), (size_t)(nrun + 1) * 4, cudaMemcpyHostToDevice, stm);
         if (e == cudaSuccess && p.autostop) e = buf.alloc(&j.hist, (size_t)nrun * p.as_window * 4);
         j.out_geno = d_out_geno + (size_t)l * nrun * gstride;
         j.out_E = d_out_E + (size_t)l * nrun;
@@ -1233,7 +1254,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         }
         const bool check = ((g + 1) % poll) == 0;
         if (check) CUDA_TRY(cudaMemsetAsync(d_flag, 0, 4, stm));
-        dock_commit_kernel<<<(nlig * nrun + 127) / 128, 128, 0, stm>>>(d_jobs, nlig, dm, d_flag);
+        dock_commit_kernel<<<nlig, 128, 0, stm>>>(d_jobs, nlig, dm, d_flag);
         g_launches += (dm.n_ls > 0 && p.lsit > 0) ? 3 : 2;
         if (check) {
             CUDA_TRY(cudaMemcpyAsync(&h_flag, d_flag, 4, cudaMemcpyDeviceToHost, stm));

@@ -1,7 +1,7 @@
 """Timing probe for one kernel family (used for the ncu captures under profiles/).
 
     python -m paper_2007_03678_b200.probe score <config> <n> <path> [reps]     # adock_score_batch, energy + gradient
-    python -m paper_2007_03678_b200.probe dock <ligands> <path> [max_evals]    # adock_dock_many, drug-like config
+    python -m paper_2007_03678_b200.probe dock <ligands> <path> [max_evals] [ls_method] [autostop]   # adock_dock_many, drug-like config
 
 <path> is the argument of adock_set_path: 0 auto, 1 warp per individual, 2 / 21 / 22 / 24 lane per individual
 (K chosen / 1 / 2 / 4 warps per group).  Needs a CUDA device."""
@@ -39,7 +39,9 @@ def main():
         grids, lig0 = W.make_config("drug")
         centre = 0.5 * (grids.box_lo + grids.box_hi); c = W.CONFIGS["drug"]
         ligs = [W.make_ligand(c["N"], c["R"], c["T"], 100 + i, centre) for i in range(L)]
-        gp = B.make_params(W.DEFAULT_PARAMS)
+        lsm = int(sys.argv[5]) if len(sys.argv) > 5 else 0
+        ast = int(sys.argv[6]) if len(sys.argv) > 6 else 0
+        gp = B.make_params(dict(W.DEFAULT_PARAMS, ls_method=lsm, autostop=ast))
         gg = B.Grids.from_workload(grids); gl = [B.Ligand.from_workload(gg, l, gp) for l in ligs]
         B.lib().adock_set_path(path)
         B.adock_dock_many(gg, gl, gp, 20, 150, min(me, 100000), list(range(L)))
@@ -49,7 +51,7 @@ def main():
         torch.cuda.synchronize(); dt = time.perf_counter() - t0
         p = B.adock_profile_read()
         ev = int(r["evals"].sum())
-        print(f"dock L={L} path={path}: {dt:.3f} s {ev/dt:.4g} evals/s; ls kernel {p['ls_ms']:.1f} ms {p['ls_launches']} launches "
+        print(f"dock L={L} path={path} ls_method={lsm} autostop={ast} evals per run median {np.median(r['evals']):.0f}: {dt:.3f} s {ev/dt:.4g} evals/s; ls kernel {p['ls_ms']:.1f} ms {p['ls_launches']} launches "
               f"{p['ls_evals']/p['ls_ms']*1e3:.4g} evals/s in-kernel; best E median {np.median(r['energies']):.3f}", flush=True)
 
 
