@@ -4,7 +4,8 @@
 // (arxiv 2007.03678; AutoDock4 energy function + Lamarckian GA; line 64: ADADELTA
 // local search, nrun independent runs; line 116: affinity / electrostatic / desolvation grid maps).
 // The paper gives no formulas; every formula below follows the reading fixed in DESIGN.md
-// ("Readings", R1..R10, taken from SURVEY.md section 8(c) C1..C10).  Written in the order and
+// ("Readings", R1..R10, taken from SURVEY.md section 8(c) C1..C10; R11 Solis-Wets local search, lines
+// 58/64/136 + Solis & Wets 1981; R12 autostop, line 197).  Written in the order and
 // notation of those readings, no blocking, no fusion, no reordering.
 //
 // Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may use
@@ -15,7 +16,8 @@
 // trilinear node/affine exactness + scipy map_coordinates, two-atom closed forms, brute-force pair
 // enumeration, Newton's third law, central finite differences, ADADELTA first-step closed form and
 // convergence on quadratics, Philox statistical/bijectivity checks (+ cuRAND on the GPU box),
-// GA invariants and eval accounting.  Parity unpinned: per-run LGA trajectories beyond the first
+// GA invariants and eval accounting, Solis-Wets contraction/expansion schedules and first two steps in
+// closed form, autostop limits (tests/test_oracle_solis_wets.py).  Parity unpinned: per-run LGA trajectories beyond the first
 // generations (chaotic; compared in distribution only).
 #include <algorithm>
 #include <cmath>
