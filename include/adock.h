@@ -181,6 +181,34 @@ int adock_dock_many(const adock_grids* grids, const adock_ligand* const* ligands
                     float* best_genotypes, float* best_energies, int cstride, float* best_coords, long long* evals_used,
                     void* cuda_stream);
 
+/* Screening pipeline (Fig. 1: host-side ligand setup overlapped with the docking of
+ * the previous ligand; lines 100-106: one resident grid set for all ligands).  Docks nlig ligands against one grid
+ * set in batches of `batch` ligands (one adock_dock_many-style launch sequence per batch on cuda_stream).  While
+ * batch b is docked, host_threads worker threads run the ligand preprocessing (R2) of batch b+1 and its images are
+ * uploaded from pinned memory on an internal copy stream, so the device never waits for the host except before the
+ * first batch.  Ligands are dealt into batches by atom count (similar sizes share a launch); outputs keep the
+ * caller's order.  ligs: host array of descriptors whose arrays are host and laid out as for adock_load_ligand;
+ * force-field tables (T, pair_coeffs, solpar, vol) are shared by all ligands.  seeds host [nlig].  Outputs host:
+ * best_genotypes [nlig][nrun][gstride] (gstride >= max(7+R)), best_energies [nlig][nrun], evals_used [nlig][nrun] or
+ * NULL.  stats may be NULL.  A ligand the library rejects fails the whole call with that error (its index is in
+ * adock_last_error).  Synchronous. */
+typedef struct adock_ligand_desc {
+    int N; const float* xyz; const int* type; const float* charge;
+    int nbonds; const int* bonds; int R; const int* rot_bonds; int root_atom;
+} adock_ligand_desc;
+typedef struct adock_screen_stats {
+    double wall_s;        /* whole call */
+    double dock_s;        /* sum over batches of the time inside the docking call of that batch */
+    double prep_s;        /* sum over batches of the host preprocessing + upload time (worker wall clock) */
+    double exposed_s;     /* time the docking loop waited for a batch that was not ready (first batch included) */
+    int batches;
+    int host_threads;
+} adock_screen_stats;
+int adock_screen(const adock_grids* grids, const adock_params* params, int T, const float* pair_coeffs, const float* solpar,
+                 const float* vol, int nlig, const adock_ligand_desc* ligs, int nrun, int pop_size, long long max_evals,
+                 const unsigned long long* seeds, int batch, int host_threads, int gstride, float* best_genotypes,
+                 float* best_energies, long long* evals_used, adock_screen_stats* stats, void* cuda_stream);
+
 /* Timing of the dominant kernel (the ADADELTA kernel of adock_dock / adock_dock_many) for roofline
  * accounting: while enabled, every launch of it is bracketed by CUDA events on the launching stream.
  * adock_profile(1) enables and resets, adock_profile(0) disables.  adock_profile_read returns the summed

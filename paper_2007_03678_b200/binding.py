@@ -19,7 +19,17 @@ ADOCK_OK, ADOCK_EINVAL, ADOCK_ENOMEM, ADOCK_ECUDA, ADOCK_ELIMIT = 0, -1, -2, -3,
 EXPORTS = ["adock_default_params", "adock_load_grids", "adock_free_grids", "adock_load_ligand", "adock_free_ligand",
            "adock_ligand_pairs", "adock_ligand_tree", "adock_ligand_image", "adock_score_batch", "adock_score_batch_host", "adock_local_search",
            "adock_philox", "adock_ga_generation", "adock_dock", "adock_dock_many", "adock_launch_count", "adock_last_error", "adock_profile", "adock_profile_read",
-           "adock_ligand_lane_image", "adock_set_path", "adock_last_dock_path", "adock_solis_wets"]
+           "adock_ligand_lane_image", "adock_set_path", "adock_last_dock_path", "adock_solis_wets", "adock_screen"]
+
+
+class adock_ligand_desc(C.Structure):
+    _fields_ = [("N", C.c_int), ("xyz", C.c_void_p), ("type", C.c_void_p), ("charge", C.c_void_p), ("nbonds", C.c_int),
+                ("bonds", C.c_void_p), ("R", C.c_int), ("rot_bonds", C.c_void_p), ("root_atom", C.c_int)]
+
+
+class adock_screen_stats(C.Structure):
+    _fields_ = [("wall_s", C.c_double), ("dock_s", C.c_double), ("prep_s", C.c_double), ("exposed_s", C.c_double),
+                ("batches", C.c_int), ("host_threads", C.c_int)]
 
 
 class AdockError(RuntimeError):
@@ -271,6 +281,36 @@ def adock_dock_many(grids: Grids, ligs, params, nrun, pop_size, max_evals, seeds
                                  int(nrun), int(pop_size), int(max_evals), _hp(sd), gs, _hp(bg), _hp(bE), cs, _hp(bx), _hp(ev),
                                  _stream()))
     return dict(genotypes=bg, energies=bE, coords=bx, evals=ev)
+
+
+def adock_screen(grids: Grids, ligs, params, nrun, pop_size, max_evals, seeds, batch, host_threads=4):
+    """ligs: workloads.Ligand objects sharing one force-field table (T, pair_coeffs, solpar, vol).  Host buffers in,
+    host results out; returns dict(genotypes [nlig][nrun][G], energies, evals, stats)."""
+    nlig = len(ligs)
+    keep = []                                   # the arrays the descriptors point into
+    desc = (adock_ligand_desc * max(nlig, 1))()
+    for i, l in enumerate(ligs):
+        a = [_np(l.xyz, np.float32), _np(l.type, np.int32), _np(l.charge, np.float32), _np(l.bonds, np.int32).reshape(-1, 2),
+             _np(l.rot_bonds, np.int32).reshape(-1, 2)]
+        keep.append(a)
+        desc[i] = adock_ligand_desc(a[0].shape[0], _hp(a[0]), _hp(a[1]), _hp(a[2]), a[3].shape[0], _hp(a[3]), a[4].shape[0], _hp(a[4]),
+                                    int(l.root_atom))
+    l0 = ligs[0]
+    co, sp, vo = _np(l0.pair_coeffs, np.float32), _np(l0.solpar, np.float32), _np(l0.vol, np.float32)
+    gs = max(7 + a[4].shape[0] for a in keep)
+    sd = _np(seeds, np.uint64)
+    bg = np.zeros((nlig, nrun, gs), np.float32)
+    bE = np.zeros((nlig, nrun), np.float32)
+    ev = np.zeros((nlig, nrun), np.int64)
+    st = adock_screen_stats()
+    L = lib()
+    L.adock_screen.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int,
+                               C.c_longlong, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    _check(L.adock_screen(grids.h, C.addressof(params) if params is not None else None, int(l0.T), _hp(co), _hp(sp), _hp(vo), nlig,
+                          C.addressof(desc), int(nrun), int(pop_size), int(max_evals), _hp(sd), int(batch), int(host_threads), gs,
+                          _hp(bg), _hp(bE), _hp(ev), C.addressof(st), _stream()))
+    return dict(genotypes=bg, energies=bE, evals=ev,
+                stats={k: getattr(st, k) for k, _ in adock_screen_stats._fields_})
 
 
 def adock_profile(enable: bool) -> None:

@@ -6,7 +6,12 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <algorithm>
+#include <atomic>
+#include <chrono>
+#include <numeric>
 #include <string>
+#include <thread>
 #include <vector>
 
 #include "../../include/adock.h"
@@ -32,6 +37,7 @@ struct adock_ligand {
     LaneImage lane;                         // image of the lane-per-individual kernels (lane_image.hpp)
     unsigned char* d_lane = nullptr;
     int lane_bytes = 0, lane_npad = 0, lane_own = 0;      // group scratch = lane_group_floats(npad, own, R, K) per lane
+    bool owns_dev = true;                   // false: the device images live in a batch slab of adock_screen
 };
 
 static thread_local std::string g_err;
@@ -237,9 +243,11 @@ extern "C" int adock_load_ligand(const adock_grids* grids, const adock_params* p
 
 extern "C" void adock_free_ligand(adock_ligand* l) {
     if (!l) return;
-    cudaFree(l->d_blob);
-    cudaFree(l->d_ext_of_int);
-    cudaFree(l->d_lane);
+    if (l->owns_dev) {
+        cudaFree(l->d_blob);
+        cudaFree(l->d_ext_of_int);
+        cudaFree(l->d_lane);
+    }
     delete l;
 }
 
@@ -1305,6 +1313,176 @@ extern "C" int adock_dock_many(const adock_grids* grids, const adock_ligand* con
                                void* cuda_stream) {
     return dock_impl(grids, ligands, nlig, params, nrun, pop_size, max_evals, seeds, gstride, best_genotypes, best_energies, cstride,
                      best_coords, evals_used, nullptr, (cudaStream_t)cuda_stream);
+}
+
+// =================================================================== screening pipeline (row a7; S8(f) NEXT-3)
+// PAPER.md lines 102, 124, 180 and Fig. 1 hide the host-side setup of ligand i+1 behind the docking of ligand i with
+// OpenMP threads.  Here the unit is a BATCH of ligands (one launch sequence docks all of them): a prepared batch owns
+// its host-only ligand handles, one pinned staging buffer and one device slab holding every image of the batch.
+namespace {
+struct ScreenBatch {
+    std::vector<adock_ligand*> ligs;        // host-only handles, device pointers patched into the slab
+    std::vector<int> index;                 // caller's ligand index of each
+    unsigned char* pinned = nullptr;
+    unsigned char* slab = nullptr;
+    size_t bytes = 0;
+    cudaEvent_t ready = nullptr;
+    int rc = ADOCK_OK;
+    std::string err;
+    double prep_s = 0;
+    void release() {
+        for (adock_ligand* l : ligs) adock_free_ligand(l);
+        ligs.clear();
+        if (pinned) cudaFreeHost(pinned);
+        if (slab) cudaFree(slab);
+        if (ready) cudaEventDestroy(ready);
+        pinned = slab = nullptr; ready = nullptr;
+    }
+};
+inline size_t up128(size_t x) { return (x + 127) & ~(size_t)127; }
+
+// host preprocessing of the batch on `nthr` threads, then one pinned -> device copy of all images on `copy`
+void screen_prepare(ScreenBatch& b, int dev, const adock_params* params, int T, const float* coeffs, const float* solpar,
+                    const float* vol, const adock_ligand_desc* ligs, int nthr, cudaStream_t copy) {
+    const auto t0 = std::chrono::steady_clock::now();
+    const int n = (int)b.index.size();
+    b.ligs.assign(n, nullptr);
+    std::atomic<int> next{0}, bad{-1};
+    std::vector<std::string> errs(n);
+    std::vector<int> rcs(n, ADOCK_OK);
+    auto work = [&]() {
+        for (int k = next.fetch_add(1); k < n; k = next.fetch_add(1)) {
+            const adock_ligand_desc& d = ligs[b.index[k]];
+            rcs[k] = adock_load_ligand(nullptr, params, d.N, d.xyz, d.type, d.charge, d.nbonds, d.bonds, d.R, d.rot_bonds, d.root_atom,
+                                       T, coeffs, solpar, vol, &b.ligs[k]);
+            if (rcs[k] != ADOCK_OK) { errs[k] = g_err; int exp = -1; bad.compare_exchange_strong(exp, k); }
+        }
+    };
+    std::vector<std::thread> pool;
+    for (int t = 1; t < nthr; ++t) pool.emplace_back(work);
+    work();
+    for (auto& th : pool) th.join();
+    if (bad.load() >= 0) {
+        const int k = bad.load();
+        b.rc = rcs[k]; b.err = "ligand " + std::to_string(b.index[k]) + ": " + errs[k];
+        return;
+    }
+    size_t off = 0;
+    std::vector<size_t> o_blob(n), o_ext(n), o_lane(n);
+    for (int k = 0; k < n; ++k) {
+        const adock_ligand* l = b.ligs[k];
+        o_blob[k] = off; off += up128((size_t)l->blob_bytes);
+        o_ext[k] = off; off += up128(l->tp.ext_of_int.size() * sizeof(int));
+        o_lane[k] = off; off += up128((size_t)l->lane_bytes);
+    }
+    b.bytes = off;
+    cudaError_t e = cudaSetDevice(dev);
+    if (e == cudaSuccess) e = cudaMallocHost(&b.pinned, off);
+    if (e == cudaSuccess) e = cudaMalloc(&b.slab, off);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&b.ready, cudaEventDisableTiming);
+    if (e == cudaSuccess) {
+        for (int k = 0; k < n; ++k) {
+            adock_ligand* l = b.ligs[k];
+            std::memcpy(b.pinned + o_blob[k], l->tp.blob.data(), (size_t)l->blob_bytes);
+            std::memcpy(b.pinned + o_ext[k], l->tp.ext_of_int.data(), l->tp.ext_of_int.size() * sizeof(int));
+            std::memcpy(b.pinned + o_lane[k], l->lane.blob.data(), (size_t)l->lane_bytes);
+            l->d_blob = b.slab + o_blob[k];
+            l->d_ext_of_int = reinterpret_cast<int*>(b.slab + o_ext[k]);
+            l->d_lane = b.slab + o_lane[k];
+            l->owns_dev = false;
+        }
+        e = cudaMemcpyAsync(b.slab, b.pinned, off, cudaMemcpyHostToDevice, copy);
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(b.ready, copy);
+    if (e != cudaSuccess) { b.rc = e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA; b.err = std::string("screen upload: ") + cudaGetErrorString(e); }
+    b.prep_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+}
+}  // namespace
+
+extern "C" int adock_screen(const adock_grids* grids, const adock_params* params, int T, const float* pair_coeffs, const float* solpar,
+                            const float* vol, int nlig, const adock_ligand_desc* ligs, int nrun, int pop_size, long long max_evals,
+                            const unsigned long long* seeds, int batch, int host_threads, int gstride, float* best_genotypes,
+                            float* best_energies, long long* evals_used, adock_screen_stats* stats, void* cuda_stream) {
+    if (stats) *stats = adock_screen_stats{};
+    if (!grids || !pair_coeffs || !solpar || !vol || !best_genotypes || !best_energies) return fail(ADOCK_EINVAL, "NULL argument");
+    if (nlig < 0 || batch < 1 || host_threads < 1 || nrun < 1 || pop_size < 2) return fail(ADOCK_EINVAL, "bad screening dimensions");
+    if (nlig == 0) return ADOCK_OK;
+    if (!ligs || !seeds) return fail(ADOCK_EINVAL, "NULL argument");
+    int maxG = 7;
+    for (int i = 0; i < nlig; ++i) {
+        if (ligs[i].N < 1 || ligs[i].R < 0) return fail(ADOCK_EINVAL, "ligand " + std::to_string(i) + ": bad shape");
+        maxG = std::max(maxG, 7 + ligs[i].R);
+    }
+    if (gstride < maxG) return fail(ADOCK_EINVAL, "output stride too small");
+    int rc = device_props();
+    if (rc) return rc;
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    const auto t_start = std::chrono::steady_clock::now();
+    // batches of similar size: stable sort by atom count (largest first)
+    std::vector<int> order(nlig);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return ligs[a].N > ligs[b].N; });
+    const int nb = (nlig + batch - 1) / batch;
+    cudaStream_t stm = (cudaStream_t)cuda_stream, copy = nullptr;
+    CUDA_TRY(cudaStreamCreateWithFlags(&copy, cudaStreamNonBlocking));
+    ScreenBatch slot[2];
+    auto fill = [&](ScreenBatch& b, int bi) {
+        b.index.assign(order.begin() + (size_t)bi * batch, order.begin() + std::min<size_t>((size_t)(bi + 1) * batch, (size_t)nlig));
+        screen_prepare(b, dev, params, T, pair_coeffs, solpar, vol, ligs, host_threads, copy);
+    };
+    double dock_s = 0, prep_s = 0, exposed_s = 0;
+    std::string err;
+    std::thread producer;
+    {
+        const auto t0 = std::chrono::steady_clock::now();
+        fill(slot[0], 0);
+        exposed_s += std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    }
+    std::vector<float> bg, bE;
+    std::vector<long long> bev;
+    std::vector<unsigned long long> bseed;
+    for (int bi = 0; bi < nb && rc == ADOCK_OK; ++bi) {
+        ScreenBatch& cur = slot[bi & 1];
+        if (bi + 1 < nb) producer = std::thread(fill, std::ref(slot[(bi + 1) & 1]), bi + 1);     // overlaps the docking below
+        if (cur.rc != ADOCK_OK) { rc = cur.rc; err = cur.err; }
+        if (rc == ADOCK_OK) {
+            const int n = (int)cur.index.size();
+            prep_s += cur.prep_s;
+            cudaError_t e = cudaStreamWaitEvent(stm, cur.ready, 0);
+            if (e != cudaSuccess) { rc = ADOCK_ECUDA; err = std::string("screen: ") + cudaGetErrorString(e); }
+            if (rc == ADOCK_OK) {
+                bg.assign((size_t)n * nrun * gstride, 0.f); bE.assign((size_t)n * nrun, 0.f); bev.assign((size_t)n * nrun, 0); bseed.resize(n);
+                for (int k = 0; k < n; ++k) bseed[k] = seeds[cur.index[k]];
+                const auto t0 = std::chrono::steady_clock::now();
+                rc = dock_impl(grids, cur.ligs.data(), n, params, nrun, pop_size, max_evals, bseed.data(), gstride, bg.data(), bE.data(), 0,
+                               nullptr, bev.data(), nullptr, stm);
+                dock_s += std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+                if (rc != ADOCK_OK) err = g_err;
+                for (int k = 0; k < n && rc == ADOCK_OK; ++k) {
+                    const size_t dst = (size_t)cur.index[k];
+                    std::memcpy(best_genotypes + dst * nrun * gstride, bg.data() + (size_t)k * nrun * gstride, (size_t)nrun * gstride * 4);
+                    std::memcpy(best_energies + dst * nrun, bE.data() + (size_t)k * nrun, (size_t)nrun * 4);
+                    if (evals_used) std::memcpy(evals_used + dst * nrun, bev.data() + (size_t)k * nrun, (size_t)nrun * 8);
+                }
+            }
+        }
+        if (producer.joinable()) {
+            const auto t0 = std::chrono::steady_clock::now();
+            producer.join();
+            exposed_s += std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+        }
+        cur.release();
+    }
+    if (producer.joinable()) producer.join();
+    slot[0].release(); slot[1].release();
+    cudaStreamDestroy(copy);
+    if (stats) {
+        stats->wall_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+        stats->dock_s = dock_s; stats->prep_s = prep_s; stats->exposed_s = exposed_s; stats->batches = nb; stats->host_threads = host_threads;
+    }
+    if (rc != ADOCK_OK) return fail(rc, err);
+    return ADOCK_OK;
 }
 
 // =================================================================== GA test hook (R9): one generation, no scoring

@@ -269,6 +269,13 @@ def make_screen_ligands(count: int, grids: GridSet, T: int = 7, seed: int = 2):
     return out
 
 
+def share_type_table(ligs):
+    """the same ligands with ONE force-field table (that of the first): a screen uses one atom-type table"""
+    import dataclasses
+    l0 = ligs[0]
+    return [dataclasses.replace(l, pair_coeffs=l0.pair_coeffs, solpar=l0.solpar, vol=l0.vol) for l in ligs]
+
+
 def shard(n_items: int, rank: int, world: int):
     """Ligand indices owned by `rank` (round-robin; the path shards with no exchange step)."""
     return list(range(rank, n_items, world))

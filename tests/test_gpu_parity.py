@@ -552,3 +552,36 @@ def test_autostop_ends_converged_runs_like_the_oracle(B, orc, W, family):
     assert (r["evals"] < 200000).all() and (r["gens"] >= 6).all()
     assert np.abs(r["genotypes"][:, :3] - centre).max() < 0.1
     assert stats.ks_2samp(r["gens"], ro["gens"]).pvalue > 0.01
+
+
+# ------------------------------------------------------------------------------- screening pipeline (row a7, NEXT-3)
+def test_screen_equals_single_docks_and_reports_overlap(B, W, orc, family):
+    """adock_screen (batches by size, preprocessing of batch b+1 overlapped with the docking of batch b, images in one
+    slab per batch) returns, ligand by ligand in the caller's order, exactly what adock_dock returns for that ligand
+    and seed in the same kernel family; its energies are the oracle's energies of its genotypes."""
+    grids, _ = W.make_config("drug", grid_n=32)
+    ligs = W.share_type_table(W.make_screen_ligands(11, grids, T=7, seed=50))
+    pd = dict(W.DEFAULT_PARAMS, lsit=12)
+    gp, op = B.make_params(pd), orc.params(pd)
+    gg = B.Grids.from_workload(grids); og = orc.Grids.from_workload(grids)
+    nrun, P, max_evals = 3, 20, 20 + 6 * (19 + 2 * 12)
+    seeds = [100 + i for i in range(len(ligs))]
+    r = B.adock_screen(gg, ligs, gp, nrun, P, max_evals, seeds, batch=4, host_threads=3)
+    assert r["stats"]["batches"] == 3 and r["stats"]["wall_s"] > 0 and r["stats"]["dock_s"] > 0
+    for i, l in enumerate(ligs):
+        gl = B.Ligand.from_workload(gg, l, gp)
+        s = B.adock_dock(gg, gl, gp, nrun, P, max_evals, seed=seeds[i], want_coords=False)
+        G = 7 + l.R
+        assert np.array_equal(r["energies"][i], s["energies"]), i
+        assert np.array_equal(r["genotypes"][i][:, :G], s["genotypes"][:, :G]), i
+        assert np.array_equal(r["evals"][i], s["evals"]), i
+        chk = orc.score(og, orc.Ligand.from_workload(l), op, s["genotypes"][:, :G], want_grad=False)["E"]
+        assert_energy(r["energies"][i], chk, f"screen ligand {i}")
+    # a bad ligand fails the call and names its index
+    bad = list(ligs)
+    import dataclasses
+    bad[5] = dataclasses.replace(bad[5], type=np.full_like(bad[5].type, 99))
+    with pytest.raises(B.AdockError, match="ligand 5"):
+        B.adock_screen(gg, bad, gp, nrun, P, max_evals, seeds, batch=4, host_threads=2)
+    # empty screen
+    assert B.adock_screen(gg, ligs[:1], gp, 1, 4, 4, [0], batch=1, host_threads=1)["energies"].shape == (1, 1)
