@@ -310,3 +310,31 @@ def dock(grids: Grids, lig: Ligand, par: OPar, nrun, pop_size, max_evals, seed, 
 
 def num_threads() -> int:
     return int(lib().orc_num_threads())
+
+
+# ------------------------------------------------------------------ R13 pose post-processing (RMSD)
+def pose_rmsd(a, b):
+    """sqrt(mean_i |a_i - b_i|^2): same atom order, no superposition, no symmetry correction.  a [..., N, 3], b [N, 3]"""
+    a = np.asarray(a, np.float64); b = np.asarray(b, np.float64)
+    return np.sqrt(((a - b) ** 2).sum(-1).mean(-1))
+
+
+def pose_rmsd_pairs(x):
+    x = np.asarray(x, np.float64)
+    return np.array([[pose_rmsd(x[i], x[j]) for j in range(x.shape[0])] for i in range(x.shape[0])])
+
+
+def cluster_poses(energies, pair, tol):
+    """poses in order of increasing energy (ties: lower index); a pose joins the first cluster (creation order) whose seed
+    is within tol, else it seeds a new one [LIT: AutoDock's RMSD-tolerance clustering].  Returns (cluster id per pose, n)."""
+    order = sorted(range(len(energies)), key=lambda k: (energies[k], k))
+    seeds, out = [], [0] * len(energies)
+    for k in order:
+        for c, s in enumerate(seeds):
+            if pair[k][s] <= tol:
+                out[k] = c
+                break
+        else:
+            out[k] = len(seeds)
+            seeds.append(k)
+    return np.array(out, np.int32), len(seeds)
