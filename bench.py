@@ -39,8 +39,8 @@ SM_COUNT, FP32_LANES, SM_MAX_MHZ = 148, 128, 1965.0        # B200_PROFILING.md u
 # 197 ligands x 20 runs x 9 ADADELTA chains = 35460 chains = 1182 groups of 32 lanes: 8 resident warps on each of the 148 SMs
 DEFAULT_LIGANDS = 197
 # dram__bytes_read.sum + dram__bytes_write.sum of one dock_ls_lane_kernel launch at the default batch
-# (profiles/r01c_dock_ls_lane_ncu.md); other batch sizes report null
-LS_TRAFFIC_BYTES = {197: 163.08e6 + 28.31e6}
+# (profiles/r01d_launches.md); other batch sizes report null
+LS_TRAFFIC_BYTES = {197: 344.74e6 + 145.57e6}
 
 
 def flops_per_eval(N, R, npairs, nmoved):
@@ -156,6 +156,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="time adock_score_batch on all four sweep ligands (default: the 40-atom one)")
     ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-screen", action="store_true", help="skip the virtual-screen sample (BASELINE.json configs[2]) through adock_screen")
+    ap.add_argument("--screen-ligands", type=int, default=592)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -272,6 +274,8 @@ def main():
         "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
     }
 
+    if not args.no_screen:
+        out["virtual_screen"] = screen_sample(B, torch, args.screen_ligands)
     if not args.no_sweep:
         out["score_batch"] = sweep(B, torch, dev, ("sweep16", "sweep40", "sweep80", "sweep128") if args.sweep else ("sweep40",))
     if world == 1 and not args.no_cpu_baseline:
@@ -279,6 +283,31 @@ def main():
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+def screen_sample(B, torch, nlig):
+    """BASELINE.json configs[2] (virtual-screen batch) on a bounded sample: `nlig` synthetic ligands (15-60 atoms, 0-15
+    torsions) against one shared 80^3 grid set, 10 runs x pop 150 x 250 k evals each, host buffers in and out through
+    adock_screen (two batches: the second batch's preprocessing overlaps the first batch's docking)."""
+    grids, _ = W.make_config("screen")
+    ligs = W.share_type_table(W.make_screen_ligands(nlig, grids, T=7, seed=2))
+    gp = B.make_params(W.DEFAULT_PARAMS)
+    gg = B.Grids.from_workload(grids)
+    nrun, max_evals, batch = 10, 250_000, (nlig + 1) // 2
+    threads = max(1, min(8, (os.cpu_count() or 2) - 1))
+    B.adock_screen(gg, ligs[:batch], gp, nrun, POP, 20_000, list(range(batch)), batch=batch, host_threads=threads)     # warm-up
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    r = B.adock_screen(gg, ligs, gp, nrun, POP, max_evals, [7000 + i for i in range(nlig)], batch=batch, host_threads=threads)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    st = r["stats"]
+    return {"workload": f"{nlig} of the 10,000 synthetic ligands (atoms 15-60, torsions 0-15), 9 maps 80^3 @0.375A, {nrun} runs x pop {POP} x "
+                        f"{max_evals} evals, ADADELTA; adock_screen, batch {batch}, {threads} host threads",
+            "ligands_per_hour": 3600.0 * nlig / dt, "evals_per_s": float(r["evals"].sum()) / dt, "seconds": dt,
+            "extrapolated_10000_ligands_s": dt * 10000.0 / nlig,
+            "host_prep_s": st["prep_s"], "host_exposed_s": st["exposed_s"], "gpu_idle_frac": max(0.0, 1.0 - st["dock_s"] / st["wall_s"]),
+            "best_energy_median": float(np.median(r["energies"].min(axis=1)))}
 
 
 def sweep(B, torch, dev, configs=("sweep40",)):

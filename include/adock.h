@@ -209,6 +209,18 @@ int adock_screen(const adock_grids* grids, const adock_params* params, int T, co
                  const unsigned long long* seeds, int batch, int host_threads, int gstride, float* best_genotypes,
                  float* best_energies, long long* evals_used, adock_screen_stats* stats, void* cuda_stream);
 
+/* Pose post-processing (S8(f) NEXT-4; "root mean squared (Euclidean) distance (RMSD) ... between
+ * the final best pose from docking and the crystallographic pose"; R13).  coords: host [n][N][3] (e.g. best_coords of
+ * adock_dock), same atom order everywhere, no superposition, no symmetry correction.
+ *   rmsd_ref  host [n] out or NULL: RMSD of pose k against ref (host [N][3]; required if rmsd_ref != NULL)
+ *   rmsd_pair host [n][n] out or NULL: RMSD between poses a and b (symmetric, zero diagonal)
+ *   cluster   host [n] out or NULL (needs energies host [n] and tol > 0): poses visited in order of increasing
+ *             energy (ties: lower index); a pose joins the first cluster, in creation order, whose seed (its
+ *             lowest-energy member) is within tol Angstrom RMSD, else it seeds cluster number *nclusters++ [LIT].
+ * The distances are computed on the device (one warp per pose pair), the clustering on the host from them. */
+int adock_pose_rmsd(int n, int N, const float* coords, const float* ref, float* rmsd_ref, float* rmsd_pair,
+                    const float* energies, float tol, int* cluster, int* nclusters, void* cuda_stream);
+
 /* Timing of the dominant kernel (the ADADELTA kernel of adock_dock / adock_dock_many) for roofline
  * accounting: while enabled, every launch of it is bracketed by CUDA events on the launching stream.
  * adock_profile(1) enables and resets, adock_profile(0) disables.  adock_profile_read returns the summed

@@ -1485,6 +1485,72 @@ extern "C" int adock_screen(const adock_grids* grids, const adock_params* params
     return ADOCK_OK;
 }
 
+// =================================================================== pose post-processing (R13)
+// one warp per ordered pair (a, b), b in [0, n]: b == n is the reference pose
+__global__ void __launch_bounds__(256) pose_rmsd_kernel(const float* __restrict__ x, const float* __restrict__ ref, int n, int N,
+                                                        float* __restrict__ out_ref, float* __restrict__ out_pair) {
+    const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (w >= n * (n + 1)) return;
+    const int a = w / (n + 1), b = w % (n + 1);
+    if (b == n ? !out_ref : (!out_pair || b < a)) return;
+    const float* pa = x + (size_t)a * N * 3;
+    const float* pb = b == n ? ref : x + (size_t)b * N * 3;
+    float s = 0.f;
+    for (int i = lane; i < 3 * N; i += 32) { const float d = pa[i] - pb[i]; s = fmaf(d, d, s); }
+    s = warp_sum(s);
+    if (lane == 0) {
+        const float r = sqrtf(s / (float)N);
+        if (b == n) out_ref[a] = r;
+        else { out_pair[(size_t)a * n + b] = r; out_pair[(size_t)b * n + a] = r; }
+    }
+}
+
+extern "C" int adock_pose_rmsd(int n, int N, const float* coords, const float* ref, float* rmsd_ref, float* rmsd_pair,
+                               const float* energies, float tol, int* cluster, int* nclusters, void* cuda_stream) {
+    if (n < 0 || N < 1) return fail(ADOCK_EINVAL, "bad pose dimensions");
+    if (nclusters) *nclusters = 0;
+    if (n == 0) return ADOCK_OK;
+    if (!coords || (rmsd_ref && !ref) || (cluster && (!energies || !(tol > 0) || !nclusters))) return fail(ADOCK_EINVAL, "NULL argument");
+    for (size_t i = 0; i < (size_t)n * N * 3; ++i) if (!std::isfinite(coords[i])) return fail(ADOCK_EINVAL, "non-finite coordinate");
+    cudaStream_t stm = (cudaStream_t)cuda_stream;
+    const bool want_pair = rmsd_pair || cluster;
+    DevBuf buf;
+    float *d_x = nullptr, *d_ref = nullptr, *d_or = nullptr, *d_op = nullptr;
+    cudaError_t e = buf.alloc(&d_x, (size_t)n * N * 12);
+    if (e == cudaSuccess && rmsd_ref) e = buf.alloc(&d_ref, (size_t)N * 12);
+    if (e == cudaSuccess && rmsd_ref) e = buf.alloc(&d_or, (size_t)n * 4);
+    if (e == cudaSuccess && want_pair) e = buf.alloc(&d_op, (size_t)n * n * 4);
+    if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("rmsd alloc: ") + cudaGetErrorString(e));
+    CUDA_TRY(cudaMemcpyAsync(d_x, coords, (size_t)n * N * 12, cudaMemcpyHostToDevice, stm));
+    if (rmsd_ref) CUDA_TRY(cudaMemcpyAsync(d_ref, ref, (size_t)N * 12, cudaMemcpyHostToDevice, stm));
+    const long long warps = (long long)n * (n + 1);
+    pose_rmsd_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, stm>>>(d_x, d_ref, n, N, d_or, d_op);
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    std::vector<float> pair;
+    if (rmsd_ref) CUDA_TRY(cudaMemcpyAsync(rmsd_ref, d_or, (size_t)n * 4, cudaMemcpyDeviceToHost, stm));
+    if (want_pair) {
+        pair.resize((size_t)n * n);
+        CUDA_TRY(cudaMemcpyAsync(pair.data(), d_op, (size_t)n * n * 4, cudaMemcpyDeviceToHost, stm));
+    }
+    CUDA_TRY(cudaStreamSynchronize(stm));
+    if (rmsd_pair) std::memcpy(rmsd_pair, pair.data(), (size_t)n * n * 4);
+    if (cluster) {
+        std::vector<int> order(n), seeds;
+        std::iota(order.begin(), order.end(), 0);
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return energies[a] < energies[b]; });
+        for (int k : order) {
+            int c = -1;
+            for (size_t s = 0; s < seeds.size() && c < 0; ++s)
+                if (pair[(size_t)k * n + seeds[s]] <= tol) c = (int)s;
+            if (c < 0) { c = (int)seeds.size(); seeds.push_back(k); }
+            cluster[k] = c;
+        }
+        *nclusters = (int)seeds.size();
+    }
+    return ADOCK_OK;
+}
+
 // =================================================================== GA test hook (R9): one generation, no scoring
 extern "C" int adock_ga_generation(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params, int nrun, int Pn,
                                    int generation, unsigned long long seed, const float* d_pop, const float* d_energies,

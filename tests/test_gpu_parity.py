@@ -585,3 +585,19 @@ def test_screen_equals_single_docks_and_reports_overlap(B, W, orc, family):
         B.adock_screen(gg, bad, gp, nrun, P, max_evals, seeds, batch=4, host_threads=2)
     # empty screen
     assert B.adock_screen(gg, ligs[:1], gp, 1, 4, 4, [0], batch=1, host_threads=1)["energies"].shape == (1, 1)
+
+
+def test_screen_config_full_grid_mixed_sizes(B, W, orc):
+    """BASELINE.json configs[2] at its own grid size (80^3, 9 maps) and launch path (auto family, 10 runs x pop 150):
+    a mixed-size sample through adock_screen; every reported energy is the oracle's energy of the reported genotype."""
+    grids, _ = W.make_config("screen")
+    ligs = W.share_type_table(W.make_screen_ligands(40, grids, T=7, seed=2))
+    gp, op = B.make_params(W.DEFAULT_PARAMS), orc.params(W.DEFAULT_PARAMS)
+    gg = B.Grids.from_workload(grids); og = orc.Grids.from_workload(grids)
+    r = B.adock_screen(gg, ligs, gp, 10, 150, 12_000, [900 + i for i in range(40)], batch=20, host_threads=4)
+    assert r["stats"]["batches"] == 2
+    for i in (0, 7, 19, 20, 33, 39):
+        l = ligs[i]
+        chk = orc.score(og, orc.Ligand.from_workload(l), op, r["genotypes"][i][:, :7 + l.R], want_grad=False)["E"]
+        assert_energy(r["energies"][i], chk, f"screen ligand {i} (N={l.N}, R={l.R})")
+        assert (r["evals"][i] >= 12_000).all() and (r["evals"][i] < 12_000 + 149 + 9 * 300).all()
