@@ -19,7 +19,7 @@ ADOCK_OK, ADOCK_EINVAL, ADOCK_ENOMEM, ADOCK_ECUDA, ADOCK_ELIMIT = 0, -1, -2, -3,
 EXPORTS = ["adock_default_params", "adock_load_grids", "adock_free_grids", "adock_load_ligand", "adock_free_ligand",
            "adock_ligand_pairs", "adock_ligand_tree", "adock_ligand_image", "adock_score_batch", "adock_score_batch_host", "adock_local_search",
            "adock_philox", "adock_ga_generation", "adock_dock", "adock_dock_many", "adock_launch_count", "adock_last_error", "adock_profile", "adock_profile_read",
-           "adock_ligand_lane_image", "adock_set_path", "adock_last_dock_path", "adock_solis_wets", "adock_screen"]
+           "adock_ligand_lane_image", "adock_set_path", "adock_last_dock_path", "adock_solis_wets", "adock_screen", "adock_pose_rmsd"]
 
 
 class adock_ligand_desc(C.Structure):
@@ -311,6 +311,23 @@ def adock_screen(grids: Grids, ligs, params, nrun, pop_size, max_evals, seeds, b
                           _hp(bg), _hp(bE), _hp(ev), C.addressof(st), _stream()))
     return dict(genotypes=bg, energies=bE, evals=ev,
                 stats={k: getattr(st, k) for k, _ in adock_screen_stats._fields_})
+
+
+def adock_pose_rmsd(coords, ref=None, energies=None, tol=2.0, want_pairs=True):
+    """coords host [n][N][3]; returns dict(rmsd_ref [n] or None, rmsd_pair [n][n] or None, cluster [n] or None, nclusters)"""
+    x = _np(coords, np.float32)
+    n, N = x.shape[0], x.shape[1]
+    r = _np(ref, np.float32) if ref is not None else None
+    E = _np(energies, np.float32) if energies is not None else None
+    rr = np.zeros(n, np.float32) if r is not None else None
+    rp = np.zeros((n, n), np.float32) if want_pairs else None
+    cl = np.zeros(n, np.int32) if E is not None else None
+    nc = C.c_int()
+    L = lib()
+    L.adock_pose_rmsd.argtypes = [C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p,
+                                  C.c_void_p, C.c_void_p]
+    _check(L.adock_pose_rmsd(n, N, _hp(x), _hp(r), _hp(rr), _hp(rp), _hp(E), float(tol), _hp(cl), C.addressof(nc), _stream()))
+    return dict(rmsd_ref=rr, rmsd_pair=rp, cluster=cl, nclusters=nc.value)
 
 
 def adock_profile(enable: bool) -> None:

@@ -601,3 +601,28 @@ def test_screen_config_full_grid_mixed_sizes(B, W, orc):
         chk = orc.score(og, orc.Ligand.from_workload(l), op, r["genotypes"][i][:, :7 + l.R], want_grad=False)["E"]
         assert_energy(r["energies"][i], chk, f"screen ligand {i} (N={l.N}, R={l.R})")
         assert (r["evals"][i] >= 12_000).all() and (r["evals"][i] < 12_000 + 149 + 9 * 300).all()
+
+
+# ------------------------------------------------------------------------------- pose post-processing (R13, NEXT-4)
+def test_pose_rmsd_and_clustering_match_oracle(B, orc, cases):
+    c = cases("drug", lsit=30)
+    r = B.adock_dock(c.gg, c.gl, c.gp, 24, 50, 20_000, seed=11)
+    x = r["coords"]
+    ref = c.lig.xyz
+    out = B.adock_pose_rmsd(x, ref, r["energies"], tol=4.0)
+    o_ref = orc.pose_rmsd(x, ref)
+    o_pair = orc.pose_rmsd_pairs(x)
+    assert np.allclose(out["rmsd_ref"], o_ref, rtol=1e-5, atol=1e-5)
+    assert np.allclose(out["rmsd_pair"], o_pair, rtol=1e-5, atol=1e-5)
+    assert np.array_equal(out["rmsd_pair"], out["rmsd_pair"].T) and (np.diag(out["rmsd_pair"]) == 0).all()
+    # the integer decisions are taken on the same float32 distances on both sides
+    oc, on = orc.cluster_poses(r["energies"], out["rmsd_pair"], 4.0)
+    assert np.array_equal(out["cluster"], oc) and out["nclusters"] == on
+    # edge cases: a single pose, no reference; tol so large that everything is one cluster
+    one = B.adock_pose_rmsd(x[:1], None, r["energies"][:1], tol=1.0)
+    assert one["nclusters"] == 1 and one["rmsd_pair"].shape == (1, 1) and one["rmsd_pair"][0, 0] == 0
+    assert B.adock_pose_rmsd(x, None, r["energies"], tol=1e9)["nclusters"] == 1
+    # rigid shift: |t|
+    t = np.array([1.0, -2.0, 2.0], np.float32)
+    assert np.allclose(B.adock_pose_rmsd(x + t, None, None, want_pairs=False)["nclusters"], 0)
+    assert np.allclose(B.adock_pose_rmsd((ref + t)[None], ref, None, want_pairs=False)["rmsd_ref"], 3.0, rtol=1e-6)
