@@ -193,8 +193,10 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
     float* Yf = reinterpret_cast<float*>(S.Y);
     float* Zf = reinterpret_cast<float*>(S.Z);
 
-    // (a1) pose: per-fragment transform = parent's o rotation about the reference-frame axis; positions relative to t
-    {
+    // (a1) pose: per-fragment transform = parent's o rotation about the reference-frame axis; positions relative to t.
+    // With K > 1 part 0 builds the whole pose and the others wait: the chain of fragment transforms is serial, and
+    // repeating it in every part costs issue slots (the scarce resource), an idle warp costs none.
+    if (K == 1 || S.part == 0) {
         float m00 = 1.f - 2.f * (qy * qy + qz * qz), m01 = 2.f * (qx * qy - qw * qz), m02 = 2.f * (qx * qz + qw * qy);
         float m10 = 2.f * (qx * qy + qw * qz), m11 = 1.f - 2.f * (qx * qx + qz * qz), m12 = 2.f * (qy * qz - qw * qx);
         float m20 = 2.f * (qx * qz - qw * qy), m21 = 2.f * (qy * qz + qw * qx), m22 = 1.f - 2.f * (qx * qx + qy * qy);
@@ -233,7 +235,6 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                 st[256] = m20; st[288] = m21; st[320] = m22; st[352] = m23;
             }
             for (int i = fi.z; i < fi.w; ++i) {
-                if (K > 1 && ((i >> 2) % K) != S.part) continue;   // atoms are dealt out by grid step (4 atoms)
                 const float4 a = L.atoms[i];
                 const int o = (i >> 1) * 64 + (i & 1);
                 Xf[o] = fmaf(m00, a.x, fmaf(m01, a.y, fmaf(m02, a.z, m03)));
@@ -242,12 +243,12 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
             }
         }
         for (int i = L.N; i < L.Npad; ++i) {            // pad atoms: finite, in no pair
-            if (K > 1 && ((i >> 2) % K) != S.part) continue;
             const int o = (i >> 1) * 64 + (i & 1);
             Xf[o] = 0.f; Yf[o] = 0.f; Zf[o] = 0.f;
         }
     }
 
+    group_sync<K>(S);                                   // the positions are in place
     // (a2) grid term, kLaneBI = 4 atoms per step: the 16 sector loads of a step are issued back to back before the first
     // is consumed (the lookups are pure L2 latency: one dependent round per step instead of one per atom); the
     // gradient goes straight into the (force, torque about t) sums of the atom's fragment, which initialises own[]
@@ -297,7 +298,6 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
         }
         if (GRAD) own_flush<K>(S.own, cur, Fx, Fy, Fz, Tx, Ty, Tz);
     }
-    group_sync<K>(S);                                   // every part's positions are in place
 
     // (a3) intramolecular pairs: register tiles; this warp's parts of the tile sequence
     f2 e2 = bc(0.f);
