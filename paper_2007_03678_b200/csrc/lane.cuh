@@ -306,26 +306,29 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
         const float4* rowp = L.rows + 2 * L.part_row[part];
         const f2 zero = bc(0.f);
         for (int kb = L.part_blk[part]; kb < L.part_blk[part + 1]; ++kb) {
-            const int4 blk = L.blocks[kb];              // b, tile_begin, tile_end, frags
-            const float2 xa = S.X[(2 * blk.x) * 32], xb = S.X[(2 * blk.x + 1) * 32];
-            const float2 ya = S.Y[(2 * blk.x) * 32], yb = S.Y[(2 * blk.x + 1) * 32];
-            const float2 za = S.Z[(2 * blk.x) * 32], zb = S.Z[(2 * blk.x + 1) * 32];
-            const float xi[4] = {xa.x, xa.y, xb.x, xb.y}, yi[4] = {ya.x, ya.y, yb.x, yb.y}, zi[4] = {za.x, za.y, zb.x, zb.y};
-            f2 gix[4], giy[4], giz[4];
+            const int4 blk = L.blocks[2 * kb], bf = L.blocks[2 * kb + 1];   // b, tile_begin, tile_end, - ; frags of rows 0-3, 4-7
+            float xi[kLaneBI], yi[kLaneBI], zi[kLaneBI];
 #pragma unroll
-            for (int r = 0; r < 4; ++r) gix[r] = giy[r] = giz[r] = zero;
+            for (int h2 = 0; h2 < kLaneBI / 2; ++h2) {
+                const int o = ((kLaneBI / 2) * blk.x + h2) * 32;
+                const float2 xa = S.X[o], ya = S.Y[o], za = S.Z[o];
+                xi[2 * h2] = xa.x; xi[2 * h2 + 1] = xa.y; yi[2 * h2] = ya.x; yi[2 * h2 + 1] = ya.y; zi[2 * h2] = za.x; zi[2 * h2 + 1] = za.y;
+            }
+            f2 gix[kLaneBI], giy[kLaneBI], giz[kLaneBI];
+#pragma unroll
+            for (int r = 0; r < kLaneBI; ++r) gix[r] = giy[r] = giz[r] = zero;
             for (int t = blk.y; t < blk.z; ++t) {
                 const uint2 tw = L.tiles[t];
                 const int jp = tw.x & 0xff;
                 const f2 xj = ld2(S.X + jp * 32), yj = ld2(S.Y + jp * 32), zj = ld2(S.Z + jp * 32);
                 f2 gjx = zero, gjy = zero, gjz = zero;
 #pragma unroll
-                for (int hf = 0; hf < 2; ++hf) {        // a half = two rows = two independent chains in one basic block
+                for (int hf = 0; hf < kLaneBI / 2; ++hf) {   // a half = two rows = two independent chains in one basic block
                     if (tw.x & (0x100u << hf)) {
                         const float4 ra0 = rowp[0], rb0 = rowp[1], ra1 = rowp[2], rb1 = rowp[3];
                         rowp += 4;
                         const int r0 = 2 * hf, r1 = 2 * hf + 1;
-                        if (!(tw.x & (0x400u << hf))) {
+                        if (!(tw.x & (0x1000u << hf))) {
                             pair_row<GRAD, false>(PK, bc(xi[r0]), bc(yi[r0]), bc(zi[r0]), xj, yj, zj, ra0, rb0, 0u, e2,
                                                   gix[r0], giy[r0], giz[r0], gjx, gjy, gjz);
                             pair_row<GRAD, false>(PK, bc(xi[r1]), bc(yi[r1]), bc(zi[r1]), xj, yj, zj, ra1, rb1, 0u, e2,
@@ -356,13 +359,14 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
             }
             if (GRAD) {                                 // I side: gi holds MINUS the gradient
                 float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
+                auto frag_of_row = [&](int r) { return (int)(((r < 4 ? bf.x : bf.y) >> (8 * (r & 3))) & 0xff); };
 #pragma unroll
-                for (int r = 0; r < 4; ++r) {
+                for (int r = 0; r < kLaneBI; ++r) {
                     const float gx = -hsum(gix[r]), gy = -hsum(giy[r]), gz = -hsum(giz[r]);
                     Fx += gx; Fy += gy; Fz += gz;
                     Tx += yi[r] * gz - zi[r] * gy; Ty += zi[r] * gx - xi[r] * gz; Tz += xi[r] * gy - yi[r] * gx;
-                    const int fr = (blk.w >> (8 * r)) & 0xff;
-                    if (r == 3 || fr != (int)((blk.w >> (8 * (r + 1))) & 0xff)) {
+                    const int fr = frag_of_row(r);
+                    if (r == kLaneBI - 1 || fr != frag_of_row(r + 1)) {
                         own_add(S.own, fr, Fx, Fy, Fz, Tx, Ty, Tz);
                         Fx = Fy = Fz = Tx = Ty = Tz = 0.f;
                     }

@@ -19,7 +19,10 @@
 
 namespace adock {
 
-constexpr int kLaneBI = 4;      // rows (I atoms) per register block
+#ifndef ADOCK_LANE_BI
+#define ADOCK_LANE_BI 4
+#endif
+constexpr int kLaneBI = ADOCK_LANE_BI;      // rows (I atoms) per register block: 4 or 8
 constexpr int kLaneParts = 4;   // the tile sequence is cut into this many runs of (nearly) equal row count, so that
                                 // K = 1, 2 or 4 warps can share the pair work of the same 32 individuals (lane.cuh)
 
@@ -34,6 +37,7 @@ struct LaneHeader {             // 128 bytes
     int part_row[kLaneParts + 1];               // and row records from part_row[p] on (a block may be cut between parts)
     int pad2[2];
 };
+static_assert(kLaneBI == 4 || kLaneBI == 8, "kLaneBI");
 static_assert(sizeof(LaneHeader) == 128, "LaneHeader layout");
 struct LaneFrag {               // 48 bytes; fragments in DFS preorder
     int parent;                 // -1 for the root
@@ -42,13 +46,16 @@ struct LaneFrag {               // 48 bytes; fragments in DFS preorder
     float p0[3]; int tor;       // x0[a_k] - pivot ; caller's torsion index (-1 for the root)
     float u[3];  int ab;        // unit(x0[b_k] - x0[a_k]) ; lane position of a_k | lane position of b_k << 16
 };
-struct LaneBlock {              // 16 bytes: I atoms 4b .. 4b+3 of an active block
-    int b;                      // block index: atoms kLaneBI*b ...
+struct LaneBlock {              // 32 bytes: I atoms kLaneBI*b .. kLaneBI*b + kLaneBI-1 of an active block
+    int b;                      // block index
     int tile_begin, tile_end;
-    uint32_t frags;             // fragment id of row r in byte r
+    int pad0;
+    uint32_t frags[2];          // fragment id of row r in byte r&3 of frags[r>>2]
+    int pad1[2];
 };
+static_assert(sizeof(LaneBlock) == 32, "LaneBlock layout");
 struct LaneTile {               // 8 bytes
-    uint32_t w0;                // jp | halfmask << 8 (bit 0: rows 0-1, bit 1: rows 2-3) | half-has-12-10-slot << 10 ;
+    uint32_t w0;                // jp | halfmask << 8 (bit h: rows 2h, 2h+1) | half-has-12-10-slot << 12 ;
                                 // each active half owns two consecutive row records, consumed in sequence
     uint32_t w1;                // hbmask (bit 2r+h) | frag(j0) << 16 | frag(j1) << 24
 };
@@ -94,8 +101,9 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
     std::vector<LaneRow> rows;
     int npair_slots = 0;
     for (int b = 0; b < nblk_all; ++b) {
-        LaneBlock blk{b, (int)tiles.size(), 0, 0};
-        for (int r = 0; r < kLaneBI; ++r) blk.frags |= (uint32_t)frag_of_pos[b * kLaneBI + r] << (8 * r);
+        LaneBlock blk{};
+        blk.b = b; blk.tile_begin = (int)tiles.size();
+        for (int r = 0; r < kLaneBI; ++r) blk.frags[r >> 2] |= (uint32_t)frag_of_pos[b * kLaneBI + r] << (8 * (r & 3));
         for (int jp = 0; jp < njp; ++jp) {
             uint32_t halfmask = 0, hbmask = 0, hbhalf = 0;
             LaneRow trow[kLaneBI];
@@ -122,10 +130,10 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
                 if (any) halfmask |= 1u << (r / 2);
             }
             if (!halfmask) continue;
-            for (int hf = 0; hf < 2; ++hf)
+            for (int hf = 0; hf < kLaneBI / 2; ++hf)
                 if (halfmask & (1u << hf)) { rows.push_back(trow[2 * hf]); rows.push_back(trow[2 * hf + 1]); }
             LaneTile t;
-            t.w0 = (uint32_t)jp | (halfmask << 8) | (hbhalf << 10);
+            t.w0 = (uint32_t)jp | (halfmask << 8) | (hbhalf << 12);
             t.w1 = hbmask | ((uint32_t)frag_of_pos[2 * jp] << 16) | ((uint32_t)frag_of_pos[2 * jp + 1] << 24);
             tiles.push_back(t);
         }
@@ -135,7 +143,7 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
     // ---- parts: cut the tile sequence where the running row count crosses p/kLaneParts of the total
     int part_blk[kLaneParts + 1], part_row[kLaneParts + 1];
     {
-        auto tile_rows = [&](int t) { const uint32_t hm = (tiles[t].w0 >> 8) & 3u; return 2 * (int)((hm & 1u) + (hm >> 1)); };
+        auto tile_rows = [&](int t) { const uint32_t hm = (tiles[t].w0 >> 8) & 15u; return 2 * (int)((hm & 1u) + ((hm >> 1) & 1u) + ((hm >> 2) & 1u) + (hm >> 3)); };
         const int total = (int)rows.size();
         std::vector<LaneBlock> cut;
         int p = 0, acc = 0;
