@@ -288,14 +288,14 @@ def main():
 def screen_sample(B, torch, nlig):
     """BASELINE.json configs[2] (virtual-screen batch) on a bounded sample: `nlig` synthetic ligands (15-60 atoms, 0-15
     torsions) against one shared 80^3 grid set, 10 runs x pop 150 x 250 k evals each, host buffers in and out through
-    adock_screen (two batches: the second batch's preprocessing overlaps the first batch's docking)."""
+    adock_screen (batches sized by the library; the next batch's preprocessing overlaps the current batch's docking)."""
     grids, _ = W.make_config("screen")
     ligs = W.share_type_table(W.make_screen_ligands(nlig, grids, T=7, seed=2))
     gp = B.make_params(W.DEFAULT_PARAMS)
     gg = B.Grids.from_workload(grids)
-    nrun, max_evals, batch = 10, 250_000, (nlig + 1) // 2
+    nrun, max_evals, batch = 10, 250_000, 0                 # batch 0: sized by the library to one wave per launch
     threads = max(1, min(8, (os.cpu_count() or 2) - 1))
-    B.adock_screen(gg, ligs[:batch], gp, nrun, POP, 20_000, list(range(batch)), batch=batch, host_threads=threads)     # warm-up
+    B.adock_screen(gg, ligs[:200], gp, nrun, POP, 20_000, list(range(len(ligs[:200]))), batch=0, host_threads=threads)     # warm-up
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     r = B.adock_screen(gg, ligs, gp, nrun, POP, max_evals, [7000 + i for i in range(nlig)], batch=batch, host_threads=threads)
@@ -303,7 +303,7 @@ def screen_sample(B, torch, nlig):
     dt = time.perf_counter() - t0
     st = r["stats"]
     return {"workload": f"{nlig} of the 10,000 synthetic ligands (atoms 15-60, torsions 0-15), 9 maps 80^3 @0.375A, {nrun} runs x pop {POP} x "
-                        f"{max_evals} evals, ADADELTA; adock_screen, batch {batch}, {threads} host threads",
+                        f"{max_evals} evals, ADADELTA; adock_screen, {st['batches']} batches sized by the library, {threads} host threads",
             "ligands_per_hour": 3600.0 * nlig / dt, "evals_per_s": float(r["evals"].sum()) / dt, "seconds": dt,
             "extrapolated_10000_ligands_s": dt * 10000.0 / nlig,
             "host_prep_s": st["prep_s"], "host_exposed_s": st["exposed_s"], "gpu_idle_frac": max(0.0, 1.0 - st["dock_s"] / st["wall_s"]),

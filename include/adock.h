@@ -175,15 +175,17 @@ int adock_dock(const adock_grids* grids, const adock_ligand* ligand, const adock
  * concurrently, every kernel launch covering all ligands and runs.  seeds host [nlig].  Output arrays host,
  * ligand-major, with per-ligand genotype stride gstride >= max_l(7+R_l) and coordinate stride
  * cstride >= max_l(N_l): best_genotypes [nlig][nrun][gstride], best_energies [nlig][nrun], best_coords
- * [nlig][nrun][cstride][3] or NULL, evals_used [nlig][nrun] or NULL.  Synchronous. */
+ * [nlig][nrun][cstride][3] or NULL, evals_used [nlig][nrun] or NULL, gens_used [nlig][nrun] or NULL (generations each
+ * run lasted: below max_gens when the eval budget or autostop ended it).  Synchronous. */
 int adock_dock_many(const adock_grids* grids, const adock_ligand* const* ligands, int nlig, const adock_params* params,
                     int nrun, int pop_size, long long max_evals, const unsigned long long* seeds, int gstride,
                     float* best_genotypes, float* best_energies, int cstride, float* best_coords, long long* evals_used,
-                    void* cuda_stream);
+                    int* gens_used, void* cuda_stream);
 
 /* Screening pipeline (Fig. 1: host-side ligand setup overlapped with the docking of
  * the previous ligand; lines 100-106: one resident grid set for all ligands).  Docks nlig ligands against one grid
- * set in batches of `batch` ligands (one adock_dock_many-style launch sequence per batch on cuda_stream).  While
+ * set in batches of `batch` ligands (one adock_dock_many-style launch sequence per batch on cuda_stream; batch = 0:
+ * the library sizes each batch to fill one wave of its local-search kernel on this device).  While
  * batch b is docked, host_threads worker threads run the ligand preprocessing (R2) of batch b+1 and its images are
  * uploaded from pinned memory on an internal copy stream, so the device never waits for the host except before the
  * first batch.  Ligands are dealt into batches by atom count (similar sizes share a launch); outputs keep the

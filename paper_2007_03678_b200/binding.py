@@ -80,7 +80,7 @@ def lib():
         L.adock_philox.argtypes = [vp, vp, ci, vp, vp]
         L.adock_ga_generation.argtypes = [vp, vp, pp, ci, ci, ci, C.c_ulonglong, vp, vp, vp, vp, vp, C.POINTER(ci), vp]
         L.adock_dock.argtypes = [vp, vp, pp, ci, ci, C.c_longlong, C.c_ulonglong, vp, vp, vp, vp, vp, vp]
-        L.adock_dock_many.argtypes = [vp, vp, ci, pp, ci, ci, C.c_longlong, vp, ci, vp, vp, ci, vp, vp, vp]
+        L.adock_dock_many.argtypes = [vp, vp, ci, pp, ci, ci, C.c_longlong, vp, ci, vp, vp, ci, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -277,10 +277,11 @@ def adock_dock_many(grids: Grids, ligs, params, nrun, pop_size, max_evals, seeds
     bE = np.zeros((nlig, nrun), np.float32)
     bx = np.zeros((nlig, nrun, cs, 3), np.float32) if want_coords else None
     ev = np.zeros((nlig, nrun), np.int64)
+    gens = np.zeros((nlig, nrun), np.int32)
     _check(lib().adock_dock_many(grids.h, C.cast(handles, C.c_void_p), nlig, C.byref(params) if params is not None else None,
                                  int(nrun), int(pop_size), int(max_evals), _hp(sd), gs, _hp(bg), _hp(bE), cs, _hp(bx), _hp(ev),
-                                 _stream()))
-    return dict(genotypes=bg, energies=bE, coords=bx, evals=ev)
+                                 _hp(gens), _stream()))
+    return dict(genotypes=bg, energies=bE, coords=bx, evals=ev, gens=gens)
 
 
 def adock_screen(grids: Grids, ligs, params, nrun, pop_size, max_evals, seeds, batch, host_threads=4):

@@ -1310,9 +1310,9 @@ extern "C" int adock_dock(const adock_grids* grids, const adock_ligand* ligand, 
 extern "C" int adock_dock_many(const adock_grids* grids, const adock_ligand* const* ligands, int nlig, const adock_params* params,
                                int nrun, int pop_size, long long max_evals, const unsigned long long* seeds, int gstride,
                                float* best_genotypes, float* best_energies, int cstride, float* best_coords, long long* evals_used,
-                               void* cuda_stream) {
+                               int* gens_used, void* cuda_stream) {
     return dock_impl(grids, ligands, nlig, params, nrun, pop_size, max_evals, seeds, gstride, best_genotypes, best_energies, cstride,
-                     best_coords, evals_used, nullptr, (cudaStream_t)cuda_stream);
+                     best_coords, evals_used, gens_used, (cudaStream_t)cuda_stream);
 }
 
 // =================================================================== screening pipeline (row a7; S8(f) NEXT-3)
@@ -1405,7 +1405,7 @@ extern "C" int adock_screen(const adock_grids* grids, const adock_params* params
                             float* best_energies, long long* evals_used, adock_screen_stats* stats, void* cuda_stream) {
     if (stats) *stats = adock_screen_stats{};
     if (!grids || !pair_coeffs || !solpar || !vol || !best_genotypes || !best_energies) return fail(ADOCK_EINVAL, "NULL argument");
-    if (nlig < 0 || batch < 1 || host_threads < 1 || nrun < 1 || pop_size < 2) return fail(ADOCK_EINVAL, "bad screening dimensions");
+    if (nlig < 0 || batch < 0 || host_threads < 1 || nrun < 1 || pop_size < 2) return fail(ADOCK_EINVAL, "bad screening dimensions");
     if (nlig == 0) return ADOCK_OK;
     if (!ligs || !seeds) return fail(ADOCK_EINVAL, "NULL argument");
     int maxG = 7;
@@ -1423,12 +1423,33 @@ extern "C" int adock_screen(const adock_grids* grids, const adock_params* params
     std::vector<int> order(nlig);
     std::iota(order.begin(), order.end(), 0);
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return ligs[a].N > ligs[b].N; });
-    const int nb = (nlig + batch - 1) / batch;
+    // batch boundaries: fixed length, or (batch == 0) as many ligands as fill ONE wave of the lane-per-individual local-search
+    // kernel at the estimated geometry of the batch's largest ligand (first of the batch): 148 SMs x groups per CTA
+    std::vector<int> bstart{0};
+    if (batch > 0) {
+        for (int i = batch; i < nlig; i += batch) bstart.push_back(i);
+    } else {
+        adock_params pp;
+        rc = check_params(params, nullptr, pp);
+        if (rc) return rc;
+        const int jg = std::max(1, (nrun * n_ls_of(pp, pop_size) + 31) / 32);
+        for (int i = 0; i < nlig;) {
+            const adock_ligand_desc& d = ligs[order[i]];
+            const int npad = (d.N + kLaneBI - 1) / kLaneBI * kLaneBI;
+            LaneGeom g{2 * (8 * d.N * d.N + 1024), npad, std::max(6 * (d.R + 1), 12 * d.R), d.R};   // two image slots, upper bounds
+            const int ng = std::max(1, lane_fit_groups(g, 1));
+            const int len = std::max(1, g_sm_count * ng / jg);
+            i += len;
+            if (i < nlig) bstart.push_back(i);
+        }
+    }
+    bstart.push_back(nlig);
+    const int nb = (int)bstart.size() - 1;
     cudaStream_t stm = (cudaStream_t)cuda_stream, copy = nullptr;
     CUDA_TRY(cudaStreamCreateWithFlags(&copy, cudaStreamNonBlocking));
     ScreenBatch slot[2];
     auto fill = [&](ScreenBatch& b, int bi) {
-        b.index.assign(order.begin() + (size_t)bi * batch, order.begin() + std::min<size_t>((size_t)(bi + 1) * batch, (size_t)nlig));
+        b.index.assign(order.begin() + bstart[bi], order.begin() + bstart[bi + 1]);
         screen_prepare(b, dev, params, T, pair_coeffs, solpar, vol, ligs, host_threads, copy);
     };
     double dock_s = 0, prep_s = 0, exposed_s = 0;

@@ -51,7 +51,7 @@ def main():
         torch.cuda.synchronize(); dt = time.perf_counter() - t0
         p = B.adock_profile_read()
         ev = int(r["evals"].sum())
-        print(f"dock L={L} path={path} ls_method={lsm} autostop={ast} evals per run median {np.median(r['evals']):.0f}: {dt:.3f} s {ev/dt:.4g} evals/s; ls kernel {p['ls_ms']:.1f} ms {p['ls_launches']} launches "
+        print(f"dock L={L} path={path} ls_method={lsm} autostop={ast} evals per run median {np.median(r['evals']):.0f} gens median {np.median(r['gens']):.0f}: {dt:.3f} s {ev/dt:.4g} evals/s; ls kernel {p['ls_ms']:.1f} ms {p['ls_launches']} launches "
               f"{p['ls_evals']/p['ls_ms']*1e3:.4g} evals/s in-kernel; best E median {np.median(r['energies']):.3f}", flush=True)
 
 

@@ -601,6 +601,13 @@ def test_screen_config_full_grid_mixed_sizes(B, W, orc):
         chk = orc.score(og, orc.Ligand.from_workload(l), op, r["genotypes"][i][:, :7 + l.R], want_grad=False)["E"]
         assert_energy(r["energies"][i], chk, f"screen ligand {i} (N={l.N}, R={l.R})")
         assert (r["evals"][i] >= 12_000).all() and (r["evals"][i] < 12_000 + 149 + 9 * 300).all()
+    # batch = 0: the library sizes the batches itself; same contract
+    r0 = B.adock_screen(gg, ligs, gp, 10, 150, 12_000, [900 + i for i in range(40)], batch=0, host_threads=4)
+    assert r0["stats"]["batches"] >= 1
+    for i in (3, 21, 38):
+        l = ligs[i]
+        chk = orc.score(og, orc.Ligand.from_workload(l), op, r0["genotypes"][i][:, :7 + l.R], want_grad=False)["E"]
+        assert_energy(r0["energies"][i], chk, f"screen (auto batch) ligand {i}")
 
 
 # ------------------------------------------------------------------------------- pose post-processing (R13, NEXT-4)
