@@ -276,6 +276,14 @@ def main():
 
     if not args.no_screen:
         out["virtual_screen"] = screen_sample(B, torch, args.screen_ligands)
+        # BASELINE.json configs[1] taken literally: ONE ligand per call (180 ADADELTA chains: latency-bound, warp per chain)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        r1 = B.adock_dock(gg, gl[0], gp, NRUN, POP, MAX_EVALS, seed=4242, want_coords=True)
+        dt1 = time.perf_counter() - t0
+        out["single_ligand"] = {"workload": "configs[1] as one adock_dock call (1 ligand x 20 runs x 2.5M evals, host results)",
+                                "seconds_per_ligand": dt1, "evals_per_s": float(r1["evals"].sum()) / dt1,
+                                "ligands_per_hour": 3600.0 / dt1, "best_energy": float(r1["energies"].min())}
     if not args.no_sweep:
         out["score_batch"] = sweep(B, torch, dev, ("sweep16", "sweep40", "sweep80", "sweep128") if args.sweep else ("sweep40",))
     if world == 1 and not args.no_cpu_baseline:
