@@ -633,3 +633,33 @@ def test_pose_rmsd_and_clustering_match_oracle(B, orc, cases):
     t = np.array([1.0, -2.0, 2.0], np.float32)
     assert np.allclose(B.adock_pose_rmsd(x + t, None, None, want_pairs=False)["nclusters"], 0)
     assert np.allclose(B.adock_pose_rmsd((ref + t)[None], ref, None, want_pairs=False)["rmsd_ref"], 3.0, rtol=1e-6)
+
+
+def test_dock_bench_launch_configuration_sampled(B, W, orc):
+    """the launch configuration bench.py times (197 drug-like ligands x 20 runs x pop 150 in one adock_dock_many call:
+    lane-per-individual local search and offspring scoring, several ligand images per CTA), for three generations;
+    sampled ligands: reported energy = oracle energy of the reported genotype, eval accounting, and the same ligand
+    docked alone in the same kernel family gives the same result."""
+    grids, lig0 = W.make_config("drug")
+    centre = 0.5 * (grids.box_lo + grids.box_hi); c = W.CONFIGS["drug"]
+    ligs = W.share_type_table([W.make_ligand(c["N"], c["R"], c["T"], 100 + i, centre) for i in range(197)])
+    gp, op = B.make_params(W.DEFAULT_PARAMS), orc.params(W.DEFAULT_PARAMS)
+    gg = B.Grids.from_workload(grids); og = orc.Grids.from_workload(grids)
+    gl = [B.Ligand.from_workload(gg, l, gp) for l in ligs]
+    P, nrun = 150, 20
+    max_evals = P + 2 * (P - 1 + 9 * 300) + 1                                  # ends after generation 3
+    seeds = [5000 + i for i in range(197)]
+    B.adock_set_path("auto")
+    r = B.adock_dock_many(gg, gl, gp, nrun, P, max_evals, seeds)
+    assert B.lib().adock_last_dock_path() == 2
+    assert (r["gens"] == 3).all() and (r["evals"] == P + 3 * (P - 1 + 9 * 300)).all()
+    for i in (0, 57, 131, 196):
+        l = ligs[i]
+        chk = orc.score(og, orc.Ligand.from_workload(l), op, r["genotypes"][i][:, :7 + l.R], want_grad=False)["E"]
+        assert_energy(r["energies"][i], chk, f"bench-configuration ligand {i}")
+    B.adock_set_path("lane1")
+    try:
+        s = B.adock_dock(gg, gl[57], gp, nrun, P, max_evals, seed=seeds[57], want_coords=False)
+    finally:
+        B.adock_set_path("auto")
+    assert np.array_equal(s["energies"], r["energies"][57]) and np.array_equal(s["genotypes"], r["genotypes"][57][:, :7 + ligs[57].R])
