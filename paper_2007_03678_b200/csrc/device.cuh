@@ -276,8 +276,11 @@ __device__ __forceinline__ float warp_sum(float v) {
 // ---------------------------------------------------------------- intramolecular pair term (R5): one warp round
 // Each lane evaluates one pair (i,j) of the round and adds +f to atom i, then -f to atom j.  Within a round no
 // atom occurs twice on a side (topology.hpp), so the read-modify-writes need no atomics and their order is fixed.
+// The arithmetic of a round (pair_compute) touches only positions and charges, so several rounds can be in flight at
+// once; the force updates (pair_apply) then run round by round in the fixed order.
+struct PairOut { float* pi; float* pj; float fx, fy, fz, e; bool valid; };
 template <bool GRAD, bool MAYPAD>
-__device__ __forceinline__ float pair_round(const LigS& L, const ParDev& P, const WarpS& S, int r, int lane) {
+__device__ __forceinline__ PairOut pair_compute(const LigS& L, const ParDev& P, const WarpS& S, int r, int lane) {
     const uint4 rec = L.pairs[r * 32 + lane];
     const bool valid = !MAYPAD || ((rec.x >> 23) & 1u);
     float* pi = S.blk + (rec.x & 0x7ffu);
@@ -300,19 +303,33 @@ __device__ __forceinline__ float pair_round(const LigS& L, const ParDev& P, cons
     const float eel = pi[kQ] * pj[kQ] * inv_er;                 // charges are stored pre-scaled by sqrt(elec_scale)
     const float egs = ds * fex2(r2c * P.mhalf_inv_sig2_log2e);
     const float e = (u12 - uA) + eel + egs;
+    PairOut o;
+    o.fx = o.fy = o.fz = 0.f;
     if (GRAD) {
         const float dv = fmaf(hb ? 10.f : 6.f, uA, -12.f * u12);            // r * d(vdw)/dr
         const float deps = P.BlamB * (1.f - rden) * rden;
         const float del = -eel * fmaf(deps, rr, eps) * inv_er;             // d(elec)/dr
         const float dds = -rr * P.inv_sig2 * egs;                          // d(desolv)/dr
         const float fs = (r2 >= P.rmin2) ? fmaf(dv, rinv, del + dds) * rinv : 0.f;
-        const float fx = fs * dx, fy = fs * dy, fz = fs * dz;
-        if (valid) { pi[kGX] += fx; pi[kGY] += fy; pi[kGZ] += fz; }
+        o.fx = fs * dx; o.fy = fs * dy; o.fz = fs * dz;
+    }
+    o.pi = pi; o.pj = pj; o.valid = valid;
+    o.e = valid ? e : 0.f;
+    return o;
+}
+template <bool GRAD>
+__device__ __forceinline__ float pair_apply(const PairOut& o) {
+    if (GRAD) {
+        if (o.valid) { o.pi[kGX] += o.fx; o.pi[kGY] += o.fy; o.pi[kGZ] += o.fz; }
         __syncwarp();
-        if (valid) { pj[kGX] -= fx; pj[kGY] -= fy; pj[kGZ] -= fz; }
+        if (o.valid) { o.pj[kGX] -= o.fx; o.pj[kGY] -= o.fy; o.pj[kGZ] -= o.fz; }
         __syncwarp();
     }
-    return valid ? e : 0.f;
+    return o.e;
+}
+template <bool GRAD, bool MAYPAD>
+__device__ __forceinline__ float pair_round(const LigS& L, const ParDev& P, const WarpS& S, int r, int lane) {
+    return pair_apply<GRAD>(pair_compute<GRAD, MAYPAD>(L, P, S, r, lane));
 }
 
 // ---------------------------------------------------------------- full evaluation of one genotype by one warp
@@ -406,7 +423,13 @@ __device__ __forceinline__ float eval_pose(const LigS& L, const GridDev& G, cons
 
     // (a3) intramolecular pairs: conflict-free warp rounds; the first nfull rounds have no padding slot
     float ep = 0.f;
-    for (int r = 0; r < L.nfull; ++r) ep += pair_round<GRAD, false>(L, P, S, r, lane);
+    int r4 = 0;
+    for (; r4 + 4 <= L.nfull; r4 += 4) {                // four rounds of arithmetic in flight, updates in round order
+        const PairOut o0 = pair_compute<GRAD, false>(L, P, S, r4, lane), o1 = pair_compute<GRAD, false>(L, P, S, r4 + 1, lane),
+                      o2 = pair_compute<GRAD, false>(L, P, S, r4 + 2, lane), o3 = pair_compute<GRAD, false>(L, P, S, r4 + 3, lane);
+        ep += pair_apply<GRAD>(o0); ep += pair_apply<GRAD>(o1); ep += pair_apply<GRAD>(o2); ep += pair_apply<GRAD>(o3);
+    }
+    for (int r = r4; r < L.nfull; ++r) ep += pair_round<GRAD, false>(L, P, S, r, lane);
     for (int r = L.nfull; r < L.nrounds; ++r) ep += pair_round<GRAD, true>(L, P, S, r, lane);
     e_inter = warp_sum(eg);
     e_intra = warp_sum(ep);
