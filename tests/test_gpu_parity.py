@@ -663,3 +663,16 @@ def test_dock_bench_launch_configuration_sampled(B, W, orc):
     finally:
         B.adock_set_path("auto")
     assert np.array_equal(s["energies"], r["energies"][57]) and np.array_equal(s["genotypes"], r["genotypes"][57][:, :7 + ligs[57].R])
+
+
+def test_score_matches_golden_fixture(B, cases, dev, family):
+    """the CUDA path against tests/golden/tiny_score.json (written by the oracle alone, tests/golden/make_golden.py)"""
+    import json, os
+    with open(os.path.join(os.path.dirname(__file__), "golden", "tiny_score.json")) as f:
+        g = json.load(f)
+    G = np.stack([np.frombuffer(bytes.fromhex(h), np.float32) for h in g["genotypes_f32_hex"]])
+    E_ref = np.array([float.fromhex(v) for v in g["E"]])
+    c = cases("tiny")
+    E, _, _ = gpu_score(B, c, G, dev)
+    assert_energy(E, E_ref, "golden fixture")
+    assert c.gl.pairs()[:8].tolist() == g["pairs_head"] and len(c.gl.pairs()) == g["npairs"]
