@@ -470,16 +470,30 @@ __device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const Pa
                     for (int d = 0; d < Gn; ++d) ls.best[d * ls.stride] = S.geno[d * 32];
                 }
                 float w[3] = {0.f, 0.f, 0.f};
-                for (int d = 0; d < D; ++d) {
-                    const float g = ls.grad[d * ls.stride];
-                    const float eg2 = P.ad_rho * ls.Eg2[d * ls.stride] + (1.f - P.ad_rho) * g * g;
-                    const float ed2o = ls.Ed2[d * ls.stride];
-                    const float dl = -(sqrtf(ed2o + P.ad_eps) / sqrtf(eg2 + P.ad_eps)) * g;
-                    ls.Eg2[d * ls.stride] = eg2;
-                    ls.Ed2[d * ls.stride] = P.ad_rho * ed2o + (1.f - P.ad_rho) * dl * dl;
-                    if (d < 3) S.geno[d * 32] += dl;
-                    else if (d < 6) { if (d == 3) w[0] = dl; else if (d == 4) w[1] = dl; else w[2] = dl; }
-                    else S.geno[(d + 1) * 32] = wrap_pi(S.geno[(d + 1) * 32] + dl);
+                // the state columns live in global memory (L2): load a chunk of 8 components before the first store, so
+                // the chunk costs one round trip instead of one per component (a store may alias the next load)
+                for (int d0 = 0; d0 < D; d0 += 8) {
+                    float gv[8], av[8], bv[8];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) {
+                        const int d = min(d0 + k, D - 1);
+                        gv[k] = ls.grad[d * ls.stride]; av[k] = ls.Eg2[d * ls.stride]; bv[k] = ls.Ed2[d * ls.stride];
+                    }
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) {
+                        const int d = d0 + k;
+                        if (d < D) {
+                            const float g = gv[k];
+                            const float eg2 = P.ad_rho * av[k] + (1.f - P.ad_rho) * g * g;
+                            const float ed2o = bv[k];
+                            const float dl = -(sqrtf(ed2o + P.ad_eps) / sqrtf(eg2 + P.ad_eps)) * g;
+                            ls.Eg2[d * ls.stride] = eg2;
+                            ls.Ed2[d * ls.stride] = P.ad_rho * ed2o + (1.f - P.ad_rho) * dl * dl;
+                            if (d < 3) S.geno[d * 32] += dl;
+                            else if (d < 6) { if (d == 3) w[0] = dl; else if (d == 4) w[1] = dl; else w[2] = dl; }
+                            else S.geno[(d + 1) * 32] = wrap_pi(S.geno[(d + 1) * 32] + dl);
+                        }
+                    }
                 }
                 const float th = sqrtf(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
                 float sh, ch;
