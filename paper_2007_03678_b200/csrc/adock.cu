@@ -1451,15 +1451,17 @@ extern "C" int adock_screen(const adock_grids* grids, const adock_params* params
         rc = check_params(params, nullptr, pp);
         if (rc) return rc;
         const int jg = std::max(1, (nrun * n_ls_of(pp, pop_size) + 31) / 32);
-        for (int i = 0; i < nlig;) {
-            const adock_ligand_desc& d = ligs[order[i]];
-            const int npad = (d.N + kLaneBI - 1) / kLaneBI * kLaneBI;
-            LaneGeom g{2 * (8 * d.N * d.N + 1024), npad, std::max(6 * (d.R + 1), 12 * d.R), d.R};   // two image slots, upper bounds
-            const int ng = std::max(1, lane_fit_groups(g, 1));
-            const int len = std::max(1, g_sm_count * ng / jg);
-            i += len;
-            if (i < nlig) bstart.push_back(i);
-        }
+        // geometry of the largest ligand (first in the order), estimated from its descriptor: image ~ 7.6 N^2 bytes (two
+        // slots), 6 accumulator floats per fragment.  Batch length = 1.5 waves of groups at that geometry (the ligands
+        // further down the order are smaller; measured on configs[2]: profiles/r01d_next_rows.md), equalised over the
+        // batches so that no small tail batch falls back to the warp-per-individual kernels.
+        const adock_ligand_desc& d = ligs[order[0]];
+        const int npad = (d.N + kLaneBI - 1) / kLaneBI * kLaneBI;
+        LaneGeom g{2 * (8 * d.N * d.N + 512), npad, 6 * (d.R + 1), d.R};
+        const int ng = std::max(1, lane_fit_groups(g, 1));
+        const int target = std::max(1, 3 * g_sm_count * ng / (2 * jg));
+        const int nbat = (nlig + target - 1) / target;
+        for (int b = 1; b < nbat; ++b) bstart.push_back((int)((long long)nlig * b / nbat));
     }
     bstart.push_back(nlig);
     const int nb = (int)bstart.size() - 1;
