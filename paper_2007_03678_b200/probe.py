@@ -3,6 +3,8 @@
     python -m paper_2007_03678_b200.probe score <config> <n> <path> [reps]     # adock_score_batch, energy + gradient
     python -m paper_2007_03678_b200.probe dock <ligands> <path> [max_evals] [ls_method] [autostop]   # adock_dock_many, drug-like config
 
+    python -m paper_2007_03678_b200.probe screen <ligands> <batch>                              # adock_screen, configs[2] sample
+
 <path> is the argument of adock_set_path: 0 auto, 1 warp per individual, 2 / 21 / 22 / 24 lane per individual
 (K chosen / 1 / 2 / 4 warps per group).  Needs a CUDA device."""
 import sys
@@ -33,6 +35,20 @@ def main():
         b.record(); torch.cuda.synchronize()
         ms = a.elapsed_time(b) / reps
         print(f"score {cfg} n={n} path={path}: {ms:.4f} ms  {n/ms*1e3:.4g} evals/s", flush=True)
+    elif mode == "screen":
+        nlig, batch = int(sys.argv[2]), int(sys.argv[3])
+        grids, _ = W.make_config("screen")
+        ligs = W.share_type_table(W.make_screen_ligands(nlig, grids, T=7, seed=2))
+        gp = B.make_params(W.DEFAULT_PARAMS); gg = B.Grids.from_workload(grids)
+        B.adock_screen(gg, ligs[:100], gp, 10, 150, 20000, list(range(len(ligs[:100]))), batch=0, host_threads=8)
+        B.adock_profile(True)
+        t0 = time.perf_counter()
+        r = B.adock_screen(gg, ligs, gp, 10, 150, 250000, [7000 + i for i in range(nlig)], batch=batch, host_threads=8)
+        dt = time.perf_counter() - t0
+        p = B.adock_profile_read()
+        print(f"screen n={nlig} batch={batch}: {dt:.2f} s {r['evals'].sum()/dt:.3e} evals/s batches {r['stats']['batches']} ls kernel "
+              f"{p['ls_ms']:.0f} ms {p['ls_launches']} launches {p['ls_evals']/p['ls_ms']*1e3:.3e} evals/s in-kernel; family "
+              f"{B.lib().adock_last_dock_path()}", flush=True)
     else:
         L, path = int(sys.argv[2]), int(sys.argv[3])
         me = int(sys.argv[4]) if len(sys.argv) > 4 else 2_500_000
