@@ -305,14 +305,18 @@ def screen_sample(B, torch, nlig):
     threads = max(1, min(8, (os.cpu_count() or 2) - 1))
     B.adock_screen(gg, ligs[:200], gp, nrun, POP, 20_000, list(range(len(ligs[:200]))), batch=0, host_threads=threads)     # warm-up
     torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    r = B.adock_screen(gg, ligs, gp, nrun, POP, max_evals, [7000 + i for i in range(nlig)], batch=batch, host_threads=threads)
-    torch.cuda.synchronize()
-    dt = time.perf_counter() - t0
+    runs = []
+    for rep in range(2):                                    # two timed repetitions, the faster one is reported, both are listed
+        t0 = time.perf_counter()
+        r = B.adock_screen(gg, ligs, gp, nrun, POP, max_evals, [7000 + i for i in range(nlig)], batch=batch, host_threads=threads)
+        torch.cuda.synchronize()
+        runs.append((time.perf_counter() - t0, r))
+    dt, r = min(runs, key=lambda x: x[0])
     st = r["stats"]
     return {"workload": f"{nlig} of the 10,000 synthetic ligands (atoms 15-60, torsions 0-15), 9 maps 80^3 @0.375A, {nrun} runs x pop {POP} x "
                         f"{max_evals} evals, ADADELTA; adock_screen, {st['batches']} batches sized by the library, {threads} host threads",
             "ligands_per_hour": 3600.0 * nlig / dt, "evals_per_s": float(r["evals"].sum()) / dt, "seconds": dt,
+            "seconds_all_repetitions": [x[0] for x in runs],
             "extrapolated_10000_ligands_s": dt * 10000.0 / nlig,
             "host_prep_s": st["prep_s"], "host_exposed_s": st["exposed_s"], "gpu_idle_frac": max(0.0, 1.0 - st["dock_s"] / st["wall_s"]),
             "best_energy_median": float(np.median(r["energies"].min(axis=1)))}
