@@ -114,9 +114,12 @@ int adock_ligand_lane_image(const adock_ligand* l, int* bytes, const unsigned ch
 /* Kernel family used by the compute entry points of this process: 0 = chosen by problem
  * size (default), 1 = one warp per individual, 2 = one lane per individual with K = 1, 2 or 4 warps sharing the
  * work of each group of 32 individuals (K chosen by size; 21, 22, 24 force K = 1, 2, 4).  All of them compute
- * the same function (R3-R7) and pass the same parity tests; they differ in summation order only. */
+ * the same function (R3-R7) and pass the same parity tests; they differ in summation order only.
+ * 3 = the ADADELTA chains of adock_dock / adock_dock_many each run on a team (one CTA of 4 warps per individual,
+ * threads over atoms and pairs), chosen by size when a launch holds too few chains to give every scheduler a warp
+ * (a single ligand); every other entry point then behaves as with 1. */
 int adock_set_path(int path);
-/* Family (1 or 2) the local search of the last adock_dock / adock_dock_many on this thread ran in; 0 = none yet. */
+/* Family (1, 2 or 3) the local search of the last adock_dock / adock_dock_many on this thread ran in; 0 = none yet. */
 int adock_last_dock_path(void);
 
 /* Batched scoring (R3-R6): for each of n genotypes build the pose, interpolate the maps, sum the

@@ -341,17 +341,18 @@ def adock_profile_read() -> dict:
     return dict(ls_ms=ms.value, ls_launches=n.value, ls_evals=ev.value)
 
 
-PATHS = {"auto": 0, "warp": 1, "lane": 2, "lane1": 21, "lane2": 22, "lane4": 24}
+PATHS = {"auto": 0, "warp": 1, "lane": 2, "lane1": 21, "lane2": 22, "lane4": 24, "team": 3}
 
 
 def adock_set_path(path) -> None:
     """kernel family: 'auto' (by problem size), 'warp' (warp per individual), 'lane' (lane per individual, warps per
-    group of 32 individuals chosen by size) or 'lane1' / 'lane2' / 'lane4' (that number of warps per group)"""
+    group of 32 individuals chosen by size), 'lane1' / 'lane2' / 'lane4' (that number of warps per group) or 'team' (the
+    docking's ADADELTA chains each run on a CTA of 4 warps; everything else as 'warp')"""
     _check(lib().adock_set_path(PATHS[path] if isinstance(path, str) else int(path)))
 
 
 def adock_last_dock_path() -> str:
-    return {0: "none", 1: "warp", 2: "lane"}[int(lib().adock_last_dock_path())]
+    return {0: "none", 1: "warp", 2: "lane", 3: "team"}[int(lib().adock_last_dock_path())]
 
 
 def adock_launch_count(reset: bool = False) -> int:

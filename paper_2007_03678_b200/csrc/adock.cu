@@ -288,7 +288,7 @@ extern "C" int adock_last_dock_path(void) { return g_last_dock_path; }
 
 extern "C" int adock_set_path(int path) {
     if (path == 21 || path == 22 || path == 24) { g_path = 2; g_lane_k = path - 20; return ADOCK_OK; }
-    if (path < 0 || path > 2) return fail(ADOCK_EINVAL, "path must be 0 (auto), 1 (warp per individual), 2 (lane per individual) or 21/22/24");
+    if (path < 0 || path > 3) return fail(ADOCK_EINVAL, "path must be 0 (auto), 1 (warp per individual), 2 (lane per individual), 21/22/24 or 3 (team per individual)");
     g_path = path; g_lane_k = 0;
     return ADOCK_OK;
 }
@@ -885,6 +885,37 @@ __global__ void __launch_bounds__(128) dock_ls_kernel(GridDev G, ParDev P, const
     }
 }
 
+// ADADELTA with one TEAM (CTA of kTeamW warps) per chain: launches with too few chains to give every scheduler a warp
+__global__ void __launch_bounds__(kTeamW * 32) dock_ls_team_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs, DockDims dm) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const DockJob job = jobs[blockIdx.x / dm.upj];
+    unsigned char* blob = smem + 16;
+    stage_ligand(blob, job.blob, job.blob_bytes, reinterpret_cast<uint64_t*>(smem), 0);
+    const LigS L = lig_view(blob);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const TeamS T = team_view(reinterpret_cast<float*>(blob + job.blob_bytes), L, warp);
+    const int ind = blockIdx.x % dm.upj, Gn = job.Gn;
+    if (ind >= dm.nrun * dm.n_ls) return;
+    const int run = ind / dm.n_ls, l = ind % dm.n_ls;
+    const RunState st = job.st[run];
+    if (!st.active) return;
+    const size_t popsz = (size_t)dm.nrun * dm.P;
+    const int slot = job.picks[(size_t)run * dm.P + l];
+    float* g = job.pop + ((size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P + slot) * Gn;
+    float* e = job.E + (size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P + slot;
+    if (warp == 0) for (int d = lane; d < Gn; d += 32) T.S.geno[d] = g[d];
+    __syncthreads();
+    int iters = 0;
+    const float be = adadelta_search_team(L, G, P, T, lane, *e, iters);
+    if (warp == 0) {
+        for (int d = lane; d < Gn; d += 32) g[d] = T.S.best[d];
+        if (lane == 0) {
+            *e = be;
+            atomicAdd(&job.st[run].ls_acc, iters);
+        }
+    }
+}
+
 // ---- lane-per-individual kernels of the docking loop.  The groups (32 chains / individuals each) of all jobs of a
 // launch form one flat sequence, jg groups per job; CTA b takes groups [b*ng, (b+1)*ng), which may belong to several
 // consecutive jobs: it stages the lane image of each of them (slot s = job j0+s) in one bulk-copy transaction.
@@ -1099,7 +1130,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     int rc = device_props();
     if (rc) return rc;
     adock_params p;
-    int maxblob = 0, maxscr = 0;
+    int maxblob = 0, maxscr = 0, maxteam = 0;
     for (int l = 0; l < nlig; ++l) {
         if (!ligs[l]) return fail(ADOCK_EINVAL, "NULL ligand");
         rc = check_params(params, ligs[l], p);
@@ -1107,6 +1138,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         if (gstride < 7 + ligs[l]->tp.R || (best_coords && cstride < ligs[l]->tp.N)) return fail(ADOCK_EINVAL, "output stride too small");
         maxblob = std::max(maxblob, ligs[l]->blob_bytes);
         maxscr = std::max(maxscr, ligs[l]->scratch_floats);
+        maxteam = std::max(maxteam, team_scratch_floats(ligs[l]->tp.N, ligs[l]->tp.nfrag, ligs[l]->tp.R));
     }
     const int Wga = fit_warps(maxblob, maxscr, 8), Wls = fit_warps(maxblob, maxscr, 4);
     if (!Wga || !Wls) return fail(ADOCK_ELIMIT, "ligand does not fit in shared memory");
@@ -1128,7 +1160,11 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     const bool many = g_path == 0 && lanes_fit && chains >= kLaneMinChains;
     const bool ls_lane = pl.K > 0 && (g_path == 2 || (many && p.ls_method == 0));
     if (g_path == 2 && !pl.K) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
-    g_last_dock_path = ls_lane ? 2 : 1;
+    // a team (CTA of kTeamW warps) per chain when one warp per chain would leave most schedulers without a warp
+    const size_t smem_team = 16 + (size_t)maxblob + (size_t)maxteam * 4;
+    const bool ls_team = !ls_lane && p.ls_method == 0 && smem_team <= (size_t)g_smem_optin &&
+                         (g_path == 3 || (g_path == 0 && chains <= (long long)g_sm_count * 6));   // measured cross-over: 4..8 ligands x 180 chains
+    g_last_dock_path = ls_lane ? 2 : ls_team ? 3 : 1;
     // offspring scoring: lane-per-individual under the same condition (populations are 1/lsrat times larger)
     const int jgs = (int)(((long long)nrun * Pn + 31) / 32);
     const LanePlan ps = lane_plan(lg, (long long)nlig * jgs, jgs);
@@ -1207,7 +1243,9 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     CUDA_TRY(cudaFuncSetAttribute(dock_ls_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ls));
     CUDA_TRY(cudaFuncSetAttribute(dock_final_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ls));
 
-    DockDims dga = dm, dls = dm, dfin = dm;
+    DockDims dga = dm, dls = dm, dfin = dm, dteam = dm;
+    dteam.upj = std::max(1, nrun * dm.n_ls);                    // one CTA per chain
+    if (ls_team) CUDA_TRY(cudaFuncSetAttribute(dock_ls_team_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_team));
     dga.upj = (int)((popsz + Wga - 1) / Wga);
     dls.upj = std::max(1, (nrun * dm.n_ls + Wls - 1) / Wls);
     dfin.upj = (nrun + Wls - 1) / Wls;
@@ -1242,6 +1280,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         else if (ls_lane && pl.K == 1) dock_ls_lane_kernel<1, true><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
         else if (ls_lane && pl.K == 2) dock_ls_lane_kernel<2, true><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
         else if (ls_lane) dock_ls_lane_kernel<4, true><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
+        else if (ls_team) dock_ls_team_kernel<<<dteam.upj * nlig, kTeamW * 32, smem_team, stm>>>(grids->dev, P, d_jobs, dteam);
         else dock_ls_kernel<<<dls.upj * nlig, Wls * 32, smem_ls, stm>>>(grids->dev, P, d_jobs, dls);
     };
     // one GA generation: offspring + their energies (one launch, or two when the scoring runs lane-per-individual)

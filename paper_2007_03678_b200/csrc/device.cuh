@@ -594,6 +594,185 @@ __device__ inline void ga_make_child(const ParDev& P, int Pn, int R, unsigned lo
     __syncwarp();
 }
 
+// ---------------------------------------------------------------- full evaluation of one genotype by a TEAM of W warps
+// One CTA-sized team per individual, threads over atoms and pairs: for launches with so few chains that one warp per
+// chain leaves most schedulers idle (a single ligand: 180 chains on 592 schedulers), the evaluation itself is split.
+// Warp 0 builds the fragment transforms; the 32 W threads take one atom each (pose + grid lookup); warp w takes the pair
+// rounds r = w (mod W) and adds their forces into its own gradient plane (plane 0 = S.blk's gx|gy|gz, planes 1..W-1 in
+// S.gextra), so no two warps ever update the same word; warp 0 sums the planes in a fixed order during
+// back-propagation.  Same arithmetic as eval_pose; the summation order differs (fixed, so results are reproducible).
+constexpr int kTeamW = 4;
+__host__ __device__ inline int team_scratch_floats(int N, int nfrag, int R) {
+    return warp_scratch_floats(N, nfrag, R) + (kTeamW - 1) * ((N + 31) / 32) * 96 + 16;
+}
+struct TeamS { WarpS S; float* gextra; float* red; int wi, gplane; };     // red: [2 kTeamW] partial energies, [8] flag; gplane = floats per extra plane
+__device__ inline TeamS team_view(float* base, const LigS& L, int wi) {
+    TeamS T;
+    T.S = warp_view(base, L);
+    T.gextra = T.S.blk + (L.npos / 32) * 256;
+    T.red = T.gextra + (kTeamW - 1) * (L.npos / 32) * 96;
+    T.wi = wi; T.gplane = (L.npos / 32) * 96;
+    return T;
+}
+__device__ __forceinline__ void team_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kTeamW * 32) : "memory"); }
+// gradient words of the atom at blk offset `off` in plane w: +0, +32, +64
+__device__ __forceinline__ float* team_gptr(const TeamS& T, int w, int off) {
+    return w == 0 ? T.S.blk + off + kGX : T.gextra + (w - 1) * T.gplane + (off >> 8) * 96 + (off & 31);
+}
+
+template <bool GRAD>
+__device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G, const ParDev& P, const TeamS& T, int lane,
+                                                float& e_inter, float& e_intra) {
+    const WarpS& S = T.S;
+    const int wi = T.wi;
+    const float tx = S.geno[0], ty = S.geno[1], tz = S.geno[2];
+    float qw = S.geno[3], qx = S.geno[4], qy = S.geno[5], qz = S.geno[6];
+    const float qn2 = qw * qw + qx * qx + qy * qy + qz * qz;
+    if (!(qn2 >= 1e-24f)) {                             // the same in every thread of the team
+        if (GRAD && wi == 0) for (int d = lane; d < 6 + L.R; d += 32) S.grad[d] = __int_as_float(0x7fc00000);
+        e_inter = e_intra = __int_as_float(0x7fc00000);
+        team_sync();
+        return __int_as_float(0x7fc00000);
+    }
+    if (wi == 0) {                                      // (a1) fragment transforms: eval_pose's code on warp 0
+        const float qi = 1.0f / sqrtf(qn2);
+        qw *= qi; qx *= qi; qy *= qi; qz *= qi;
+        const float r00 = 1.f - 2.f * (qy * qy + qz * qz), r01 = 2.f * (qx * qy - qw * qz), r02 = 2.f * (qx * qz + qw * qy);
+        const float r10 = 2.f * (qx * qy + qw * qz), r11 = 1.f - 2.f * (qx * qx + qz * qz), r12 = 2.f * (qy * qz - qw * qx);
+        const float r20 = 2.f * (qx * qz - qw * qy), r21 = 2.f * (qy * qz + qw * qx), r22 = 1.f - 2.f * (qx * qx + qy * qy);
+        for (int f = lane; f < L.nfrag; f += 32) {
+            float s = 0.f, c = 1.f;
+            if (f > 0) sincosf(S.geno[7 + (L.fi[f].w >> 16)], &s, &c);
+            S.sc[f] = make_float2(s, c);
+        }
+        __syncwarp();
+        for (int f = lane; f < L.nfrag; f += 32) {
+            float m00 = 1, m01 = 0, m02 = 0, m03 = 0, m10 = 0, m11 = 1, m12 = 0, m13 = 0, m20 = 0, m21 = 0, m22 = 1, m23 = 0;
+            for (int cur = f; cur > 0; cur = L.fi[cur].x) {
+                const float4 p0 = L.fg[2 * cur], u = L.fg[2 * cur + 1];
+                const float2 sc = S.sc[cur];
+                const float s = sc.x, c = sc.y, k = 1.f - c;
+                const float a00 = fmaf(k * u.x, u.x, c), a01 = fmaf(k * u.x, u.y, -s * u.z), a02 = fmaf(k * u.x, u.z, s * u.y);
+                const float a10 = fmaf(k * u.x, u.y, s * u.z), a11 = fmaf(k * u.y, u.y, c), a12 = fmaf(k * u.y, u.z, -s * u.x);
+                const float a20 = fmaf(k * u.x, u.z, -s * u.y), a21 = fmaf(k * u.y, u.z, s * u.x), a22 = fmaf(k * u.z, u.z, c);
+                const float n00 = a00 * m00 + a01 * m10 + a02 * m20, n01 = a00 * m01 + a01 * m11 + a02 * m21, n02 = a00 * m02 + a01 * m12 + a02 * m22;
+                const float n10 = a10 * m00 + a11 * m10 + a12 * m20, n11 = a10 * m01 + a11 * m11 + a12 * m21, n12 = a10 * m02 + a11 * m12 + a12 * m22;
+                const float n20 = a20 * m00 + a21 * m10 + a22 * m20, n21 = a20 * m01 + a21 * m11 + a22 * m21, n22 = a20 * m02 + a21 * m12 + a22 * m22;
+                const float dx = m03 - p0.x, dy = m13 - p0.y, dz = m23 - p0.z;
+                const float n03 = a00 * dx + a01 * dy + a02 * dz + p0.x, n13 = a10 * dx + a11 * dy + a12 * dz + p0.y, n23 = a20 * dx + a21 * dy + a22 * dz + p0.z;
+                m00 = n00; m01 = n01; m02 = n02; m03 = n03; m10 = n10; m11 = n11; m12 = n12; m13 = n13;
+                m20 = n20; m21 = n21; m22 = n22; m23 = n23;
+            }
+            const float t00 = r00 * m00 + r01 * m10 + r02 * m20, t01 = r00 * m01 + r01 * m11 + r02 * m21,
+                        t02 = r00 * m02 + r01 * m12 + r02 * m22, t03 = r00 * m03 + r01 * m13 + r02 * m23;
+            const float t10 = r10 * m00 + r11 * m10 + r12 * m20, t11 = r10 * m01 + r11 * m11 + r12 * m21,
+                        t12 = r10 * m02 + r11 * m12 + r12 * m22, t13 = r10 * m03 + r11 * m13 + r12 * m23;
+            const float t20 = r20 * m00 + r21 * m10 + r22 * m20, t21 = r20 * m01 + r21 * m11 + r22 * m21,
+                        t22 = r20 * m02 + r21 * m12 + r22 * m22, t23 = r20 * m03 + r21 * m13 + r22 * m23;
+            S.fragT[3 * f] = make_float4(t00, t01, t02, t03 + tx);
+            S.fragT[3 * f + 1] = make_float4(t10, t11, t12, t13 + ty);
+            S.fragT[3 * f + 2] = make_float4(t20, t21, t22, t23 + tz);
+            if (GRAD && f == 0) S.fragAx[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (GRAD && f > 0) {
+                const float4 p0 = L.fg[2 * f], u = L.fg[2 * f + 1];
+                S.fragAx[2 * f] = make_float4(t00 * u.x + t01 * u.y + t02 * u.z, t10 * u.x + t11 * u.y + t12 * u.z, t20 * u.x + t21 * u.y + t22 * u.z, 0.f);
+                S.fragAx[2 * f + 1] = make_float4(t00 * p0.x + t01 * p0.y + t02 * p0.z + t03, t10 * p0.x + t11 * p0.y + t12 * p0.z + t13,
+                                                  t20 * p0.x + t21 * p0.y + t22 * p0.z + t23, 0.f);
+            }
+        }
+    }
+    team_sync();
+    // (a1,a2) atoms: one thread per position (pose + trilinear lookup); the owner also clears the atom's extra planes
+    float eg = 0.f;
+    for (int i = wi * 32 + lane; i < L.npos; i += 32 * kTeamW) {
+        const uint32_t m = L.meta[i];
+        if (m == 0xffffffffu) continue;                  // hole
+        const float4 a = L.atoms[i];
+        const int f = m >> 8;
+        const float4 t0 = S.fragT[3 * f], t1 = S.fragT[3 * f + 1], t2 = S.fragT[3 * f + 2];
+        const float x = fmaf(t0.x, a.x, fmaf(t0.y, a.y, fmaf(t0.z, a.z, t0.w)));
+        const float y = fmaf(t1.x, a.x, fmaf(t1.y, a.y, fmaf(t1.z, a.z, t1.w)));
+        const float z = fmaf(t2.x, a.x, fmaf(t2.y, a.y, fmaf(t2.z, a.z, t2.w)));
+        const int off = atom_slot_dev(i);
+        float* b = S.blk + off;
+        b[kX] = x; b[kY] = y; b[kZ] = z; b[kQ] = a.w * P.elec_sqrt;
+        float gx, gy, gz;
+        eg += grid_atom<GRAD>(G, P, (int)(m & 0xff), a.w, x, y, z, gx, gy, gz);
+        if (GRAD) {
+            b[kGX] = gx; b[kGY] = gy; b[kGZ] = gz;
+#pragma unroll
+            for (int w = 1; w < kTeamW; ++w) { float* g = team_gptr(T, w, off); g[0] = 0.f; g[32] = 0.f; g[64] = 0.f; }
+        }
+    }
+    team_sync();
+
+    // (a3) intramolecular pairs: warp wi takes rounds wi, wi + W, ...; forces go to plane wi
+    float ep = 0.f;
+    for (int r = wi; r < L.nrounds; r += kTeamW) {
+        PairOut o = r < L.nfull ? pair_compute<GRAD, false>(L, P, S, r, lane) : pair_compute<GRAD, true>(L, P, S, r, lane);
+        if (GRAD) {
+            float* gi = team_gptr(T, wi, (int)(o.pi - S.blk)), *gj = team_gptr(T, wi, (int)(o.pj - S.blk));
+            if (o.valid) { gi[0] += o.fx; gi[32] += o.fy; gi[64] += o.fz; }
+            __syncwarp();
+            if (o.valid) { gj[0] -= o.fx; gj[32] -= o.fy; gj[64] -= o.fz; }
+            __syncwarp();
+        }
+        ep += o.e;
+    }
+    eg = warp_sum(eg); ep = warp_sum(ep);
+    if (lane == 0) { T.red[2 * wi] = eg; T.red[2 * wi + 1] = ep; }
+    team_sync();
+    e_inter = 0.f; e_intra = 0.f;
+#pragma unroll
+    for (int w = 0; w < kTeamW; ++w) { e_inter += T.red[2 * w]; e_intra += T.red[2 * w + 1]; }
+
+    // (a4) back-propagation on warp 0: eval_pose's code, the atom gradient being the sum of the planes in fixed order
+    if (GRAD) {
+        if (wi == 0) {
+            for (int f = lane; f < L.nfrag; f += 32) {
+                const int4 ix = L.fi[f];
+                const float4 pv = S.fragAx[2 * f + 1];
+                const float px = tx + pv.x, py = ty + pv.y, pz = tz + pv.z;
+                float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
+                for (int k = ix.y; k < ix.z; ++k) {
+                    const int off = atom_slot_dev(L.fragatoms[k]);
+                    const float* b = S.blk + off;
+                    float gx = b[kGX], gy = b[kGY], gz = b[kGZ];
+#pragma unroll
+                    for (int w = 1; w < kTeamW; ++w) { const float* g = team_gptr(T, w, off); gx += g[0]; gy += g[32]; gz += g[64]; }
+                    const float rx = b[kX] - px, ry = b[kY] - py, rz = b[kZ] - pz;
+                    Fx += gx; Fy += gy; Fz += gz;
+                    Tx += ry * gz - rz * gy; Ty += rz * gx - rx * gz; Tz += rx * gy - ry * gx;
+                }
+                S.fragFT[2 * f] = make_float4(Fx, Fy, Fz, 0.f);
+                S.fragFT[2 * f + 1] = make_float4(Tx, Ty, Tz, 0.f);
+            }
+            __syncwarp();
+            for (int f = lane; f < L.nfrag; f += 32) {
+                const int w = L.fi[f].w;
+                const int sub_end = w & 0xffff;
+                const float4 pf = S.fragAx[2 * f + 1];
+                float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
+                for (int g = f; g < sub_end; ++g) {
+                    const float4 F = S.fragFT[2 * g], Tq = S.fragFT[2 * g + 1], pg = S.fragAx[2 * g + 1];
+                    const float lx = pg.x - pf.x, ly = pg.y - pf.y, lz = pg.z - pf.z;
+                    Fx += F.x; Fy += F.y; Fz += F.z;
+                    Tx += Tq.x + (ly * F.z - lz * F.y); Ty += Tq.y + (lz * F.x - lx * F.z); Tz += Tq.z + (lx * F.y - ly * F.x);
+                }
+                if (f == 0) {
+                    S.grad[0] = Fx; S.grad[1] = Fy; S.grad[2] = Fz;
+                    S.grad[3] = Tx; S.grad[4] = Ty; S.grad[5] = Tz;
+                } else {
+                    const float4 u = S.fragAx[2 * f];
+                    S.grad[6 + (w >> 16)] = u.x * Tx + u.y * Ty + u.z * Tz;
+                }
+            }
+        }
+        team_sync();
+    }
+    return e_inter + e_intra;
+}
+
 // ---------------------------------------------------------------- ADADELTA local search (R7), one warp
 // Start genotype in S.geno; on return S.best holds the best genotype seen and the function returns its
 // energy (the carried energy e_start if no finite evaluation happened).  iters = evaluations performed.
@@ -658,6 +837,80 @@ __device__ inline float adadelta_search(const LigS& L, const GridDev& G, const P
         }
         if (lane == 3) { S.geno[3] = newq[0]; S.geno[4] = newq[1]; S.geno[5] = newq[2]; S.geno[6] = newq[3]; }
         __syncwarp();
+    }
+    iters = it;
+    return isfinite(bestE) ? bestE : e_start;
+}
+
+// ---------------------------------------------------------------- ADADELTA local search (R7), one team
+// adadelta_search with the evaluation spread over the team; warp 0 owns the optimiser state and takes every decision,
+// the other warps follow through a flag in shared memory.  Called by all kTeamW warps with S.geno ready and visible.
+__device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, const ParDev& P, const TeamS& T, int lane, float e_start,
+                                             int& iters) {
+    const WarpS& S = T.S;
+    const int R = L.R, D = 6 + R, Gn = 7 + R;
+    const bool lead = T.wi == 0;
+    float Eg2[3] = {0.f, 0.f, 0.f}, Ed2[3] = {0.f, 0.f, 0.f};         // component d = lane + 32*c on warp 0
+    float bestE = __int_as_float(0x7f800000);
+    if (lead) for (int d = lane; d < Gn; d += 32) S.best[d] = S.geno[d];
+    int it = 0;
+    while (it < P.lsit) {
+        float ei, ea;
+        const float e = eval_pose_team<true>(L, G, P, T, lane, ei, ea);      // ends with a team barrier: S.grad is visible
+        ++it;
+        if (lead) {
+            bool ok = isfinite(e);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const int d = lane + 32 * c;
+                if (d < D) ok = ok && isfinite(S.grad[d]);
+            }
+            ok = __all_sync(kFull, ok);
+            if (lane == 0) T.red[2 * kTeamW] = ok ? 1.f : 0.f;
+            if (ok) {
+                if (e < bestE) {
+                    bestE = e;
+                    for (int d = lane; d < Gn; d += 32) S.best[d] = S.geno[d];
+                }
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const int d = lane + 32 * c;
+                    if (d < D) {
+                        const float g = S.grad[d];
+                        Eg2[c] = P.ad_rho * Eg2[c] + (1.f - P.ad_rho) * g * g;
+                        const float dl = -(sqrtf(Ed2[c] + P.ad_eps) / sqrtf(Eg2[c] + P.ad_eps)) * g;
+                        Ed2[c] = P.ad_rho * Ed2[c] + (1.f - P.ad_rho) * dl * dl;
+                        S.grad[d] = dl;
+                    }
+                }
+                __syncwarp();
+                float newv[3];
+                float newq[4];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const int gI = lane + 32 * c;
+                    if (gI < 3) newv[c] = S.geno[gI] + S.grad[gI];
+                    else if (gI >= 7 && gI < Gn) newv[c] = wrap_pi(S.geno[gI] + S.grad[gI - 1]);
+                }
+                if (lane == 3) {
+                    const float wx = S.grad[3], wy = S.grad[4], wz = S.grad[5];
+                    const float th = sqrtf(wx * wx + wy * wy + wz * wz);
+                    float sh, ch;
+                    sincosf(0.5f * th, &sh, &ch);
+                    const float k = th > 1e-12f ? sh / th : 0.5f;
+                    rotate_quat(ch, k * wx, k * wy, k * wz, S.geno + 3, newq);
+                }
+                __syncwarp();
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const int gI = lane + 32 * c;
+                    if (gI < 3 || (gI >= 7 && gI < Gn)) S.geno[gI] = newv[c];
+                }
+                if (lane == 3) { S.geno[3] = newq[0]; S.geno[4] = newq[1]; S.geno[5] = newq[2]; S.geno[6] = newq[3]; }
+            }
+        }
+        team_sync();                                    // new genotype and the flag are visible
+        if (T.red[2 * kTeamW] == 0.f) break;
     }
     iters = it;
     return isfinite(bestE) ? bestE : e_start;

@@ -36,7 +36,7 @@ def dev():
     return torch.device("cuda:0")
 
 
-@pytest.fixture(params=["warp", "lane1", "lane2", "lane4"])
+@pytest.fixture(params=["warp", "lane1", "lane2", "lane4", "team"])
 def family(request, B):
     """run the test once per kernel family (warp per individual / thread per individual); restores 'auto'"""
     B.adock_set_path(request.param)
