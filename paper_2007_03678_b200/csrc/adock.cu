@@ -885,8 +885,9 @@ __global__ void __launch_bounds__(128) dock_ls_kernel(GridDev G, ParDev P, const
     }
 }
 
-// ADADELTA with one TEAM (CTA of kTeamW warps) per chain: launches with too few chains to give every scheduler a warp
-__global__ void __launch_bounds__(kTeamW * 32) dock_ls_team_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs, DockDims dm) {
+// ADADELTA with one TEAM (CTA of kTeamW warps) per chain: launches with too few chains to give every scheduler a warp.
+// 5 CTAs per SM (<= 102 registers): 4 ligands x 180 chains are one wave; at 4 CTAs per SM they were two (1.85 s -> 3.08 s).
+__global__ void __launch_bounds__(kTeamW * 32, 5) dock_ls_team_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs, DockDims dm) {
     extern __shared__ __align__(128) unsigned char smem[];
     const DockJob job = jobs[blockIdx.x / dm.upj];
     unsigned char* blob = smem + 16;
