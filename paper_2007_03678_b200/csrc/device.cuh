@@ -726,8 +726,19 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
 #pragma unroll
     for (int w = 0; w < kTeamW; ++w) { e_inter += T.red[2 * w]; e_intra += T.red[2 * w + 1]; }
 
-    // (a4) back-propagation on warp 0: eval_pose's code, the atom gradient being the sum of the planes in fixed order
+    // (a4) the planes are summed per atom (one thread each, fixed order 0+1+2+3), then back-propagation on warp 0:
+    // eval_pose's code
     if (GRAD) {
+        for (int i = wi * 32 + lane; i < L.npos; i += 32 * kTeamW) {
+            if (L.meta[i] == 0xffffffffu) continue;
+            const int off = atom_slot_dev(i);
+            float* b = S.blk + off;
+            float gx = b[kGX], gy = b[kGY], gz = b[kGZ];
+#pragma unroll
+            for (int w = 1; w < kTeamW; ++w) { const float* g = team_gptr(T, w, off); gx += g[0]; gy += g[32]; gz += g[64]; }
+            b[kGX] = gx; b[kGY] = gy; b[kGZ] = gz;
+        }
+        team_sync();
         if (wi == 0) {
             for (int f = lane; f < L.nfrag; f += 32) {
                 const int4 ix = L.fi[f];
@@ -737,9 +748,7 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
                 for (int k = ix.y; k < ix.z; ++k) {
                     const int off = atom_slot_dev(L.fragatoms[k]);
                     const float* b = S.blk + off;
-                    float gx = b[kGX], gy = b[kGY], gz = b[kGZ];
-#pragma unroll
-                    for (int w = 1; w < kTeamW; ++w) { const float* g = team_gptr(T, w, off); gx += g[0]; gy += g[32]; gz += g[64]; }
+                    const float gx = b[kGX], gy = b[kGY], gz = b[kGZ];
                     const float rx = b[kX] - px, ry = b[kY] - py, rz = b[kZ] - pz;
                     Fx += gx; Fy += gy; Fz += gz;
                     Tx += ry * gz - rz * gy; Ty += rz * gx - rx * gz; Tz += rx * gy - ry * gx;
