@@ -40,7 +40,7 @@ SM_COUNT, FP32_LANES, SM_MAX_MHZ = 148, 128, 1965.0        # B200_PROFILING.md u
 DEFAULT_LIGANDS = 197
 # dram__bytes_read.sum + dram__bytes_write.sum of one dock_ls_lane_kernel launch at the default batch
 # (profiles/r01d_launches.md); other batch sizes report null
-LS_TRAFFIC_BYTES = {197: 344.74e6 + 145.57e6}
+LS_TRAFFIC_BYTES = {197: 343.06e6 + 143.18e6}
 
 
 def flops_per_eval(N, R, npairs, nmoved):
