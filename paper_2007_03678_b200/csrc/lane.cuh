@@ -176,15 +176,15 @@ __device__ __forceinline__ void pair_row(const PairK& K, f2 xi, f2 yi, f2 zi, f2
     const f2 egs = mul2(ds, pk(fex2(tl), fex2(th)));
     e2 = add2(e2, add2(evdw, add2(eel, egs)));
     if (GRAD) {
-        // -dE/dr = rinv (12 u12 - nA uA + eel) + eel (deps/dr)/eps + (r/sigma^2) egs
+        // -dE/dr = rinv (12 u12 - nA uA + eel) + eel (deps/dr)/eps + (r/sigma^2) egs ;  ns = -(dE/dr)/r
         const f2 s = add2(evdw, u12);
         f2 A1 = fma2(K.six, s, eel);
         if (HB) A1 = fma2(pk((hb & 1u) ? 4.f : 0.f, (hb & 2u) ? 4.f : 0.f), nuA, A1);
         const f2 dee = mul2(mul2(K.BlamB, kex), inv);
         const f2 A3 = fma2(eel, dee, mul2(A1, rinv));
-        const f2 A4 = fma2(K.isig2, mul2(rr, egs), A3);
+        // desolvation: (r/sigma^2) egs / r = egs/sigma^2 (the clamped case is zeroed below)
         float nl, nh;
-        unpk(mul2(A4, rinv), nl, nh);
+        unpk(fma2(A3, rinv, mul2(K.isig2, egs)), nl, nh);
         const f2 ns = pk(r2l >= K.rmin2 ? nl : 0.f, r2h >= K.rmin2 ? nh : 0.f);
         gix = fma2(ns, dx, gix); giy = fma2(ns, dy, giy); giz = fma2(ns, dz, giz);
         gjx = fma2(ns, dx, gjx); gjy = fma2(ns, dy, gjy); gjz = fma2(ns, dz, gjz);
