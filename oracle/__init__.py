@@ -14,13 +14,18 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "adock_oracle.cpp")
 _LIB = os.path.join(_HERE, "liboracle.so")
+_LIB32 = os.path.join(_HERE, "liboracle_f32.so")
 _lib = None
+_lib32 = None
 
 
 def build(force: bool = False) -> str:
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off",
-                               "-o", _LIB, _SRC])
+    """liboracle.so = the oracle (fp64).  liboracle_f32.so = the same source with the score path (R3-R6) in honest
+    fp32 (-DORC_REAL=float): a measuring stick for tolerances, never a parity reference."""
+    for out, extra in ((_LIB, []), (_LIB32, ["-DORC_REAL=float"])):
+        if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(_SRC):
+            subprocess.check_call(["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off",
+                                   *extra, "-o", out, _SRC])
     return _LIB
 
 
@@ -56,6 +61,16 @@ def lib():
         _lib.orc_dock.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(OPar), C.c_int, C.c_int, C.c_longlong, C.c_ulonglong,
                                   C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int]
     return _lib
+
+
+def lib_f32():
+    """the fp32 build of the score path; handles (Ligand, Grids) of the fp64 library are valid in it (same structs)"""
+    global _lib32
+    if _lib32 is None:
+        build()
+        _lib32 = C.CDLL(_LIB32)
+        assert _lib32.orc_real_bytes() == 4 and lib().orc_real_bytes() == 8
+    return _lib32
 
 
 def _p(a):
@@ -168,8 +183,9 @@ def pair_energy(par: OPar, c12, cA, expA, qq, dsco, d):
     return E.value, dE.value
 
 
-def score(grids: Grids, lig: Ligand, par: OPar, genos, want_grad=True, nthreads=0):
-    """float32 genotypes [n, >=7+R] -> dict(E[n], terms[n,2], grad[n,6+R], margins[n,2], scales[n,3]) in float64."""
+def score(grids: Grids, lig: Ligand, par: OPar, genos, want_grad=True, nthreads=0, fp32=False):
+    """float32 genotypes [n, >=7+R] -> dict(E[n], terms[n,2], grad[n,6+R], margins[n,2], scales[n,3]) in float64.
+    fp32=True runs the same statements in float (liboracle_f32.so): how far honest fp32 lands from the oracle."""
     genos = _f32(genos)
     if genos.ndim == 1:
         genos = genos[None]
@@ -179,8 +195,8 @@ def score(grids: Grids, lig: Ligand, par: OPar, genos, want_grad=True, nthreads=
     grad = np.zeros((n, 6 + lig.R), np.float64) if want_grad else None
     margins = np.zeros((n, 2), np.float64)
     scales = np.zeros((n, 3), np.float64)
-    rc = lib().orc_score(grids._h, lig._h, C.byref(par), _p(genos), n, gs, _p(E), _p(terms), _p(grad), _p(margins),
-                         _p(scales), int(nthreads))
+    rc = (lib_f32() if fp32 else lib()).orc_score(grids._h, lig._h, C.byref(par), _p(genos), n, gs, _p(E), _p(terms), _p(grad),
+                                                  _p(margins), _p(scales), int(nthreads))
     if rc != 0:
         raise ValueError("oracle: ligand types exceed grid maps")
     return dict(E=E, terms=terms, grad=grad, margins=margins, scales=scales)

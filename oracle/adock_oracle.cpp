@@ -30,6 +30,16 @@
 #include <omp.h>
 #endif
 
+// Precision of the SCORE path (R3-R6: pose, trilinear, grid_atom, pair_energy, score).  fp64 is the oracle.  Compiled a
+// second time with -DORC_REAL=float (oracle/liboracle_f32.so) the very same statements run in honest fp32 (SURVEY.md
+// section 8(c): "also a compile-time fp32 mode to measure how far honest fp32 lands from fp64 -- sets expectations
+// for the GPU tolerance").  That build is a measuring stick for tolerances only; it is never the reference of a parity
+// test.  Interfaces stay double in both builds; search (R7-R12) always runs in fp64 around the score.
+#ifndef ORC_REAL
+#define ORC_REAL double
+#endif
+typedef ORC_REAL real;
+
 namespace {
 
 const double PI = 3.14159265358979323846;
@@ -184,12 +194,12 @@ int prep(OLig& L, const int* rot) {
 }
 
 // ------------------------------------------------------------------ small vector helpers
-inline void cross(const double* a, const double* b, double* o) {
+template <class F> inline void cross(const F* a, const F* b, F* o) {
     o[0] = a[1] * b[2] - a[2] * b[1];
     o[1] = a[2] * b[0] - a[0] * b[2];
     o[2] = a[0] * b[1] - a[1] * b[0];
 }
-inline double dot(const double* a, const double* b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
+template <class F> inline F dot(const F* a, const F* b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
 
 // Hamilton product p (x) q, components (w,x,y,z)
 inline void qmul(const double* p, const double* q, double* o) {
@@ -203,36 +213,37 @@ inline double wrap_pi(double a) { return a - 2 * PI * std::floor((a + PI) / (2 *
 
 // ------------------------------------------------------------------ R3: pose builder
 // g = (t[3], q[4] = w,x,y,z, tau[R]).  Returns false for |q| < 1e-12.
-bool pose(const OLig& L, const double* g, double* x) {
+bool pose(const OLig& L, const double* g, real* x) {
     const int N = L.N;
-    std::vector<double> y(L.x0);
+    std::vector<real> y(L.x0.begin(), L.x0.end());
     for (int o = 0; o < L.R; ++o) {                       // deepest first: reference-frame axes valid
         int k = L.tor_order[o];
-        const double* xa = &L.x0[3 * L.ta[k]];
-        const double* xb = &L.x0[3 * L.tb[k]];
-        double u[3] = {xb[0] - xa[0], xb[1] - xa[1], xb[2] - xa[2]};
-        double n = std::sqrt(dot(u, u));
-        for (double& c : u) c /= n;
-        double ct = std::cos(g[7 + k]), st = std::sin(g[7 + k]);
+        const real xa[3] = {(real)L.x0[3 * L.ta[k]], (real)L.x0[3 * L.ta[k] + 1], (real)L.x0[3 * L.ta[k] + 2]};
+        const real xb[3] = {(real)L.x0[3 * L.tb[k]], (real)L.x0[3 * L.tb[k] + 1], (real)L.x0[3 * L.tb[k] + 2]};
+        real u[3] = {xb[0] - xa[0], xb[1] - xa[1], xb[2] - xa[2]};
+        real n = std::sqrt(dot(u, u));
+        for (real& c : u) c /= n;
+        real ct = std::cos((real)g[7 + k]), st = std::sin((real)g[7 + k]);
         for (int i = 0; i < N; ++i) {
             if (!L.moved[(size_t)k * N + i]) continue;
-            double v[3] = {y[3 * i] - xa[0], y[3 * i + 1] - xa[1], y[3 * i + 2] - xa[2]};
-            double uxv[3];
+            real v[3] = {y[3 * i] - xa[0], y[3 * i + 1] - xa[1], y[3 * i + 2] - xa[2]};
+            real uxv[3];
             cross(u, v, uxv);
-            double ud = dot(u, v);
+            real ud = dot(u, v);
             for (int d = 0; d < 3; ++d)                   // Rodrigues, right-hand about a->b
                 y[3 * i + d] = xa[d] + v[d] * ct + uxv[d] * st + u[d] * ud * (1 - ct);
         }
     }
-    double qn = std::sqrt(g[3] * g[3] + g[4] * g[4] + g[5] * g[5] + g[6] * g[6]);
-    if (!(qn >= 1e-12)) return false;
-    double w = g[3] / qn, a = g[4] / qn, b = g[5] / qn, c = g[6] / qn;
-    double Rm[9] = {1 - 2 * (b * b + c * c), 2 * (a * b - w * c),     2 * (a * c + w * b),
-                    2 * (a * b + w * c),     1 - 2 * (a * a + c * c), 2 * (b * c - w * a),
-                    2 * (a * c - w * b),     2 * (b * c + w * a),     1 - 2 * (a * a + b * b)};
+    const real q0 = (real)g[3], q1 = (real)g[4], q2 = (real)g[5], q3 = (real)g[6];
+    real qn = std::sqrt(q0 * q0 + q1 * q1 + q2 * q2 + q3 * q3);
+    if (!(qn >= (real)1e-12)) return false;
+    real w = q0 / qn, a = q1 / qn, b = q2 / qn, c = q3 / qn;
+    real Rm[9] = {1 - 2 * (b * b + c * c), 2 * (a * b - w * c),     2 * (a * c + w * b),
+                  2 * (a * b + w * c),     1 - 2 * (a * a + c * c), 2 * (b * c - w * a),
+                  2 * (a * c - w * b),     2 * (b * c + w * a),     1 - 2 * (a * a + b * b)};
     for (int i = 0; i < N; ++i) {
-        double v[3] = {y[3 * i] - L.c[0], y[3 * i + 1] - L.c[1], y[3 * i + 2] - L.c[2]};
-        for (int d = 0; d < 3; ++d) x[3 * i + d] = g[d] + Rm[3 * d] * v[0] + Rm[3 * d + 1] * v[1] + Rm[3 * d + 2] * v[2];
+        real v[3] = {y[3 * i] - (real)L.c[0], y[3 * i + 1] - (real)L.c[1], y[3 * i + 2] - (real)L.c[2]};
+        for (int d = 0; d < 3; ++d) x[3 * i + d] = (real)g[d] + Rm[3 * d] * v[0] + Rm[3 * d + 1] * v[1] + Rm[3 * d + 2] * v[2];
     }
     return true;
 }
@@ -240,46 +251,46 @@ bool pose(const OLig& L, const double* g, double* x) {
 // ------------------------------------------------------------------ R4: grid term
 // trilinear value and gradient (per Angstrom) of map m at point p, clamp + floor rule.
 // margin (optional) = min over in-box axes of the distance (grid units) to the nearest cell face.
-double trilinear(const OGrid& G, int m, const double* p, double* grad, double* outside /*[3] u-uc*/, double* margin) {
+real trilinear(const OGrid& G, int m, const real* p, real* grad, real* outside /*[3] u-uc*/, double* margin) {
     const int n[3] = {G.nx, G.ny, G.nz};
     int i0[3];
-    double f[3];
+    real f[3];
     for (int d = 0; d < 3; ++d) {
-        double u = (p[d] - G.org[d]) / G.h;
-        double uc = std::min(std::max(u, 0.0), (double)(n[d] - 1));
+        real u = (p[d] - (real)G.org[d]) / (real)G.h;
+        real uc = std::min(std::max(u, (real)0.0), (real)(n[d] - 1));
         i0[d] = std::min((int)std::floor(uc), n[d] - 2);
         f[d] = uc - i0[d];
         if (outside) outside[d] = u - uc;
         if (margin)      // gradient kinks sit at integer u (cell faces, box faces)
-            *margin = std::min(*margin, (u != uc) ? std::fabs(u - uc) : std::fabs(u - std::round(u)));
+            *margin = std::min(*margin, (double)((u != uc) ? std::fabs(u - uc) : std::fabs(u - std::round(u))));
     }
     const float* map = &G.maps[(size_t)m * G.nz * G.ny * G.nx];
-    double val = 0, gx = 0, gy = 0, gz = 0;
+    real val = 0, gx = 0, gy = 0, gz = 0;
     for (int cz = 0; cz < 2; ++cz)
         for (int cy = 0; cy < 2; ++cy)
             for (int cx = 0; cx < 2; ++cx) {
-                double v = map[((size_t)(i0[2] + cz) * G.ny + (i0[1] + cy)) * G.nx + (i0[0] + cx)];
-                double wx = cx ? f[0] : 1 - f[0], wy = cy ? f[1] : 1 - f[1], wz = cz ? f[2] : 1 - f[2];
+                real v = map[((size_t)(i0[2] + cz) * G.ny + (i0[1] + cy)) * G.nx + (i0[0] + cx)];
+                real wx = cx ? f[0] : 1 - f[0], wy = cy ? f[1] : 1 - f[1], wz = cz ? f[2] : 1 - f[2];
                 val += wz * wy * wx * v;
-                gx += wz * wy * (cx ? 1.0 : -1.0) * v;
-                gy += wz * (cy ? 1.0 : -1.0) * wx * v;
-                gz += (cz ? 1.0 : -1.0) * wy * wx * v;
+                gx += wz * wy * (cx ? (real)1.0 : (real)-1.0) * v;
+                gy += wz * (cy ? (real)1.0 : (real)-1.0) * wx * v;
+                gz += (cz ? (real)1.0 : (real)-1.0) * wy * wx * v;
             }
-    if (grad) { grad[0] = gx / G.h; grad[1] = gy / G.h; grad[2] = gz / G.h; }
+    if (grad) { grad[0] = gx / (real)G.h; grad[1] = gy / (real)G.h; grad[2] = gz / (real)G.h; }
     return val;
 }
 
 // E_i and g_i of atom i at x (R4): type map + q*elec + |q|*desolv + linear wall outside the box
-double grid_atom(const OGrid& G, const OPar& P, int type, double q, int T, const double* x, double* g, double* margin) {
-    double gt[3], ge[3], gd[3], out[3];
-    double vt = trilinear(G, type, x, gt, out, margin);
-    double ve = trilinear(G, T, x, ge, nullptr, nullptr);
-    double vd = trilinear(G, T + 1, x, gd, nullptr, nullptr);
-    double E = vt + q * ve + std::fabs(q) * vd;
+real grid_atom(const OGrid& G, const OPar& P, int type, real q, int T, const real* x, real* g, double* margin) {
+    real gt[3], ge[3], gd[3], out[3];
+    real vt = trilinear(G, type, x, gt, out, margin);
+    real ve = trilinear(G, T, x, ge, nullptr, nullptr);
+    real vd = trilinear(G, T + 1, x, gd, nullptr, nullptr);
+    real E = vt + q * ve + std::fabs(q) * vd;
     for (int d = 0; d < 3; ++d) {
         if (out[d] != 0.0) {                    // violated axis: interpolant constant along it
-            E += P.k_wall * G.h * std::fabs(out[d]);
-            g[d] = P.k_wall * (out[d] > 0 ? 1.0 : -1.0);
+            E += (real)P.k_wall * (real)G.h * std::fabs(out[d]);
+            g[d] = (real)P.k_wall * (out[d] > 0 ? (real)1.0 : (real)-1.0);
         } else {
             g[d] = gt[d] + q * ge[d] + std::fabs(q) * gd[d];
         }
@@ -289,18 +300,20 @@ double grid_atom(const OGrid& G, const OPar& P, int type, double q, int T, const
 
 // ------------------------------------------------------------------ R5: intramolecular pair term
 // energy and dE/dr of one pair at separation d (before the r_min floor); dsco = S_i V_j + S_j V_i
-double pair_energy(const OPar& P, double c12, double cA, double expA, double qq, double dsco, double d, double* dEdr) {
-    double r = std::max(d, P.r_min);
-    double e_vdw = c12 / std::pow(r, 12) - cA / std::pow(r, expA);
-    double d_vdw = -12 * c12 / std::pow(r, 13) + expA * cA / std::pow(r, expA + 1);
-    double ex = std::exp(-P.diel_lambda * P.diel_B * r);
-    double eps = P.diel_A + P.diel_B / (1 + P.diel_k * ex);
-    double deps = P.diel_B * P.diel_k * P.diel_lambda * P.diel_B * ex / ((1 + P.diel_k * ex) * (1 + P.diel_k * ex));
-    double e_el = P.elec_scale * qq / (eps * r);
-    double d_el = -P.elec_scale * qq * (deps * r + eps) / ((eps * r) * (eps * r));
-    double e_ds = P.w_desolv * dsco * std::exp(-r * r / (2 * P.ds_sigma * P.ds_sigma));
-    double d_ds = -(r / (P.ds_sigma * P.ds_sigma)) * e_ds;
-    if (dEdr) *dEdr = (d < P.r_min) ? 0.0 : d_vdw + d_el + d_ds;
+real pair_energy(const OPar& P, real c12, real cA, real expA, real qq, real dsco, real d, real* dEdr) {
+    const real r_min = (real)P.r_min, A = (real)P.diel_A, B = (real)P.diel_B, k = (real)P.diel_k, lam = (real)P.diel_lambda;
+    const real sig = (real)P.ds_sigma;
+    real r = std::max(d, r_min);
+    real e_vdw = c12 / std::pow(r, (real)12) - cA / std::pow(r, expA);
+    real d_vdw = -12 * c12 / std::pow(r, (real)13) + expA * cA / std::pow(r, expA + 1);
+    real ex = std::exp(-lam * B * r);
+    real eps = A + B / (1 + k * ex);
+    real deps = B * k * lam * B * ex / ((1 + k * ex) * (1 + k * ex));
+    real e_el = (real)P.elec_scale * qq / (eps * r);
+    real d_el = -(real)P.elec_scale * qq * (deps * r + eps) / ((eps * r) * (eps * r));
+    real e_ds = (real)P.w_desolv * dsco * std::exp(-r * r / (2 * sig * sig));
+    real d_ds = -(r / (sig * sig)) * e_ds;
+    if (dEdr) *dEdr = (d < r_min) ? (real)0.0 : d_vdw + d_el + d_ds;
     return e_vdw + e_el + e_ds;
 }
 
@@ -313,16 +326,17 @@ double score(const OGrid& G, const OLig& L, const OPar& P, const double* g, doub
              double* scales = nullptr) {
     const int N = L.N;
     const double nan = std::numeric_limits<double>::quiet_NaN();
-    std::vector<double> x(3 * N), f(3 * N, 0.0), fabs_i(N, 0.0);
+    std::vector<real> x(3 * N), f(3 * N, (real)0.0), fabs_i(N, (real)0.0);
     if (!pose(L, g, x.data())) {
         if (grad) for (int d = 0; d < 6 + L.R; ++d) grad[d] = nan;
         if (terms) terms[0] = terms[1] = nan;
         return nan;
     }
+    const real gt[3] = {(real)g[0], (real)g[1], (real)g[2]};
     double fm = 1.0, pm = 1e30;
-    double e_inter = 0, e_intra = 0;
+    real e_inter = 0, e_intra = 0;
     for (int i = 0; i < N; ++i) {
-        e_inter += grid_atom(G, P, L.type[i], L.q[i], L.T, &x[3 * i], &f[3 * i], &fm);
+        e_inter += grid_atom(G, P, L.type[i], (real)L.q[i], L.T, &x[3 * i], &f[3 * i], &fm);
         fabs_i[i] = std::sqrt(dot(&f[3 * i], &f[3 * i]));
     }
     const size_t np = L.pairs.size() / 2;
@@ -330,13 +344,13 @@ double score(const OGrid& G, const OLig& L, const OPar& P, const double* g, doub
         int i = L.pairs[2 * p], j = L.pairs[2 * p + 1];
         int ti = L.type[i], tj = L.type[j];
         const double* co = &L.coef[((size_t)ti * L.T + tj) * 4];
-        double Si = L.solpar[ti] + P.qasp * std::fabs(L.q[i]), Sj = L.solpar[tj] + P.qasp * std::fabs(L.q[j]);
-        double dsco = Si * L.vol[tj] + Sj * L.vol[ti];
-        double dv[3] = {x[3 * i] - x[3 * j], x[3 * i + 1] - x[3 * j + 1], x[3 * i + 2] - x[3 * j + 2]};
-        double d = std::sqrt(dot(dv, dv)), dEdr;
-        e_intra += pair_energy(P, co[0], co[1], co[2], L.q[i] * L.q[j], dsco, d, &dEdr);
-        pm = std::min(pm, std::fabs(d - P.r_min));
-        if (d >= P.r_min) {
+        real Si = (real)L.solpar[ti] + (real)P.qasp * std::fabs((real)L.q[i]), Sj = (real)L.solpar[tj] + (real)P.qasp * std::fabs((real)L.q[j]);
+        real dsco = Si * (real)L.vol[tj] + Sj * (real)L.vol[ti];
+        real dv[3] = {x[3 * i] - x[3 * j], x[3 * i + 1] - x[3 * j + 1], x[3 * i + 2] - x[3 * j + 2]};
+        real d = std::sqrt(dot(dv, dv)), dEdr;
+        e_intra += pair_energy(P, (real)co[0], (real)co[1], (real)co[2], (real)L.q[i] * (real)L.q[j], dsco, d, &dEdr);
+        pm = std::min(pm, (double)std::fabs(d - (real)P.r_min));
+        if (d >= (real)P.r_min) {
             for (int c = 0; c < 3; ++c) {
                 f[3 * i + c] += dEdr * dv[c] / d;
                 f[3 * j + c] -= dEdr * dv[c] / d;
@@ -348,7 +362,7 @@ double score(const OGrid& G, const OLig& L, const OPar& P, const double* g, doub
     if (scales) {
         scales[0] = scales[1] = scales[2] = 0;
         for (int i = 0; i < N; ++i) {
-            double rel[3] = {x[3 * i] - g[0], x[3 * i + 1] - g[1], x[3 * i + 2] - g[2]};
+            real rel[3] = {x[3 * i] - gt[0], x[3 * i + 1] - gt[1], x[3 * i + 2] - gt[2]};
             scales[0] += fabs_i[i];
             scales[1] += std::sqrt(dot(rel, rel)) * fabs_i[i];
         }
@@ -356,7 +370,7 @@ double score(const OGrid& G, const OLig& L, const OPar& P, const double* g, doub
             double sk = 0;
             for (int i = 0; i < N; ++i) {
                 if (!L.moved[(size_t)k * N + i]) continue;
-                double rel[3] = {x[3 * i] - x[3 * L.ta[k]], x[3 * i + 1] - x[3 * L.ta[k] + 1], x[3 * i + 2] - x[3 * L.ta[k] + 2]};
+                real rel[3] = {x[3 * i] - x[3 * L.ta[k]], x[3 * i + 1] - x[3 * L.ta[k] + 1], x[3 * i + 2] - x[3 * L.ta[k] + 2]};
                 sk += std::sqrt(dot(rel, rel)) * fabs_i[i];
             }
             scales[2] += sk * sk;
@@ -366,27 +380,28 @@ double score(const OGrid& G, const OLig& L, const OPar& P, const double* g, doub
     if (terms) { terms[0] = e_inter; terms[1] = e_intra; }
     if (margins) { margins[0] = fm; margins[1] = pm; }
     if (grad) {                                            // R6: back-propagation
-        for (int d = 0; d < 6 + L.R; ++d) grad[d] = 0;
+        std::vector<real> gr(6 + L.R, (real)0.0);
         for (int i = 0; i < N; ++i) {
-            double rel[3] = {x[3 * i] - g[0], x[3 * i + 1] - g[1], x[3 * i + 2] - g[2]}, t[3];
+            real rel[3] = {x[3 * i] - gt[0], x[3 * i + 1] - gt[1], x[3 * i + 2] - gt[2]}, t[3];
             cross(rel, &f[3 * i], t);
-            for (int d = 0; d < 3; ++d) { grad[d] += f[3 * i + d]; grad[3 + d] += t[d]; }
+            for (int d = 0; d < 3; ++d) { gr[d] += f[3 * i + d]; gr[3 + d] += t[d]; }
         }
         for (int k = 0; k < L.R; ++k) {
-            const double* xa = &x[3 * L.ta[k]];
-            const double* xb = &x[3 * L.tb[k]];
-            double u[3] = {xb[0] - xa[0], xb[1] - xa[1], xb[2] - xa[2]};
-            double n = std::sqrt(dot(u, u));
-            for (double& c : u) c /= n;
-            double tq[3] = {0, 0, 0};
+            const real* xa = &x[3 * L.ta[k]];
+            const real* xb = &x[3 * L.tb[k]];
+            real u[3] = {xb[0] - xa[0], xb[1] - xa[1], xb[2] - xa[2]};
+            real n = std::sqrt(dot(u, u));
+            for (real& c : u) c /= n;
+            real tq[3] = {0, 0, 0};
             for (int i = 0; i < N; ++i) {
                 if (!L.moved[(size_t)k * N + i]) continue;
-                double rel[3] = {x[3 * i] - xa[0], x[3 * i + 1] - xa[1], x[3 * i + 2] - xa[2]}, t[3];
+                real rel[3] = {x[3 * i] - xa[0], x[3 * i + 1] - xa[1], x[3 * i + 2] - xa[2]}, t[3];
                 cross(rel, &f[3 * i], t);
                 for (int d = 0; d < 3; ++d) tq[d] += t[d];
             }
-            grad[6 + k] = dot(u, tq);
+            gr[6 + k] = dot(u, tq);
         }
+        for (int d = 0; d < 6 + L.R; ++d) grad[d] = gr[d];
     }
     return e_inter + e_intra;
 }
@@ -751,23 +766,39 @@ int orc_grid_create(const float* maps, int M, int nx, int ny, int nz, double spa
 }
 void orc_grid_free(void* p) { delete (OGrid*)p; }
 
-int orc_pose(void* lig, const double* geno, double* xyz) { return pose(*(OLig*)lig, geno, xyz) ? 0 : -1; }
+int orc_pose(void* lig, const double* geno, double* xyz) {
+    OLig* L = (OLig*)lig;
+    std::vector<real> x(3 * L->N);
+    if (!pose(*L, geno, x.data())) return -1;
+    std::copy(x.begin(), x.end(), xyz);
+    return 0;
+}
 
 int orc_trilinear(void* grid, int m, const double* xyz, int n, double* val, double* grad) {
     OGrid* G = (OGrid*)grid;
     if (m < 0 || m >= G->M) return -1;
-    for (int i = 0; i < n; ++i) val[i] = trilinear(*G, m, xyz + 3 * i, grad ? grad + 3 * i : nullptr, nullptr, nullptr);
+    for (int i = 0; i < n; ++i) {
+        const real p[3] = {(real)xyz[3 * i], (real)xyz[3 * i + 1], (real)xyz[3 * i + 2]};
+        real g[3];
+        val[i] = trilinear(*G, m, p, grad ? g : nullptr, nullptr, nullptr);
+        if (grad) for (int d = 0; d < 3; ++d) grad[3 * i + d] = g[d];
+    }
     return 0;
 }
 
 int orc_grid_atom(void* grid, const OPar* P, int type, double q, int T, const double* x, double* E, double* g) {
     double fm = 1.0;
-    *E = grid_atom(*(OGrid*)grid, *P, type, q, T, x, g, &fm);
+    const real p[3] = {(real)x[0], (real)x[1], (real)x[2]};
+    real gg[3];
+    *E = grid_atom(*(OGrid*)grid, *P, type, (real)q, T, p, gg, &fm);
+    for (int d = 0; d < 3; ++d) g[d] = gg[d];
     return 0;
 }
 
 int orc_pair_energy(const OPar* P, double c12, double cA, double expA, double qq, double dsco, double d, double* E, double* dEdr) {
-    *E = pair_energy(*P, c12, cA, expA, qq, dsco, d, dEdr);
+    real de;
+    *E = pair_energy(*P, (real)c12, (real)cA, (real)expA, (real)qq, (real)dsco, (real)d, &de);
+    if (dEdr) *dEdr = de;
     return 0;
 }
 
@@ -868,7 +899,11 @@ int orc_dock(void* grid, void* lig, const OPar* P, int nrun, int Pn, long long m
         RunResult r = dock_run(*G, *L, *P, run, Pn, max_evals, seed, hist ? &h : nullptr);
         std::copy(r.best.begin(), r.best.end(), best_geno + (size_t)run * Gn);
         best_E[run] = r.bestE;
-        if (best_xyz) pose(*L, r.best.data(), best_xyz + (size_t)run * 3 * L->N);
+        if (best_xyz) {
+            std::vector<real> x(3 * L->N);
+            pose(*L, r.best.data(), x.data());
+            std::copy(x.begin(), x.end(), best_xyz + (size_t)run * 3 * L->N);
+        }
         if (evals) evals[run] = r.evals;
         if (gens) gens[run] = r.gens;
         if (hist)
@@ -877,6 +912,8 @@ int orc_dock(void* grid, void* lig, const OPar* P, int nrun, int Pn, long long m
     }
     return 0;
 }
+
+int orc_real_bytes(void) { return (int)sizeof(real); }
 
 int orc_num_threads(void) {
 #ifdef _OPENMP

@@ -106,25 +106,42 @@ def make_type_params(T: int, seed: int):
     return Rii, eii, coeffs.astype(np.float32), solpar.astype(np.float32), vol.astype(np.float32)
 
 
-def make_ligand(N: int, R: int, T: int, seed: int, centre=(0.0, 0.0, 0.0)) -> Ligand:
-    """Random bonded tree, 1.5 A bonds, degree <= 4, atoms >= 1.3 A apart; R rotatable bonds drawn
-    from bonds whose two ends both have degree >= 2 (all of them if fewer than R exist)."""
+def make_ligand(N: int, R: int, T: int, seed: int, centre=(0.0, 0.0, 0.0), far_sep: float | None = None,
+                max_deg: int = 4) -> Ligand:
+    """Random bonded tree, 1.5 A bonds, degree <= max_deg, atoms >= 1.3 A apart; R rotatable bonds drawn
+    from bonds whose two ends both have degree >= 2 (all of them if fewer than R exist).
+    far_sep (the non-clashing variant): atoms four or more bonds apart are also kept at least
+    far_sep Angstrom apart in the input conformation, so that no non-excluded pair starts inside its repulsive wall."""
     g = _rng(seed)
     xyz = np.zeros((N, 3), np.float64)
     deg = np.zeros(N, np.int64)
+    topo = np.zeros((N, N), np.int64)                   # bond-count distance in the tree built so far
     bonds = []
     for k in range(1, N):
-        for _ in range(200):
-            cand = np.flatnonzero(deg[:k] < 4)
+        best, best_pos, best_p = -np.inf, None, None
+        for _ in range(200 if far_sep is None else 2000):
+            cand = np.flatnonzero(deg[:k] < max_deg)
             p = int(cand[g.integers(len(cand))])
             d = g.normal(size=3)
             d /= np.linalg.norm(d)
             pos = xyz[p] + 1.5 * d
             dist = np.linalg.norm(xyz[:k] - pos, axis=1)
             dist[p] = np.inf
-            if dist.min() >= 1.3:
+            if far_sep is None:
+                if dist.min() >= 1.3:
+                    break
+                continue
+            far = topo[p, :k] + 1 >= 4
+            slack = min(dist.min() - 1.3, (dist[far].min() - far_sep) if far.any() else np.inf)
+            if slack > best:
+                best, best_pos, best_p = slack, pos, p
+            if slack >= 0:
                 break
+        if far_sep is not None:
+            pos, p = best_pos, best_p
         xyz[k] = pos
+        topo[k, :k] = topo[p, :k] + 1
+        topo[:k, k] = topo[k, :k]
         deg[p] += 1
         deg[k] += 1
         bonds.append((p, k))
@@ -231,6 +248,20 @@ def make_genotypes(n: int, R: int, grids: GridSet, seed: int, wall_tail: float =
         side = g.integers(0, 2, ntail)
         off = g.uniform(-1.5, 1.5, ntail)
         G[rows, axis] = np.where(side == 0, lo[axis] + off, hi[axis] + off)
+    return G.astype(np.float32)
+
+
+def make_pocket_genotypes(n: int, R: int, grids: GridSet, seed: int, sigma_t: float = 1.0, sigma_tau: float = 0.25) -> np.ndarray:
+    """[n, 7+R] float32 poses NEAR the input conformation inside the carved pocket: t = box centre + N(0, sigma_t) A,
+    q uniform (normalised N(0,1)^4), tau ~ N(0, sigma_tau) rad.  With a far_sep ligand these are the non-clashing
+    poses (energies O(1..100) kcal/mol, like a real complex) of DESIGN.md section 4."""
+    g = _rng(271828 * seed + 11)
+    c = 0.5 * (grids.box_lo + grids.box_hi)
+    G = np.empty((n, 7 + R), np.float64)
+    G[:, 0:3] = c + g.normal(0.0, sigma_t, (n, 3))
+    q = g.normal(size=(n, 4))
+    G[:, 3:7] = q / np.linalg.norm(q, axis=1, keepdims=True)
+    G[:, 7:] = g.normal(0.0, sigma_tau, (n, R))
     return G.astype(np.float32)
 
 

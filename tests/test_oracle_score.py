@@ -129,6 +129,26 @@ def test_two_atom_closed_forms(orc, W, par):
     assert math.isclose(E1, p0.w_desolv * 2.5 * math.exp(-0.5), rel_tol=1e-12)
 
 
+def test_dielectric_rate_mid_range_closed_forms(orc, W):
+    """eps(r) = A + B/(1 + k exp(-lambda*B*r)) (R5): the limits r -> 0 and r -> inf above do not see the RATE
+    lambda*B of the sigmoid (lambda*r instead would pass them).  Two hand-worked mid-range points do:
+    r = 1/(lambda*B): exp(-1), eps = A + B/(1 + k/e);  r = ln(k)/(lambda*B): k exp(.) = 1, eps = A + B/2."""
+    p0 = _par_with(orc, W, r_min=1e-12)
+    A, B, k, lam = p0.diel_A, p0.diel_B, p0.diel_k, p0.diel_lambda
+    r1 = 1.0 / (lam * B)
+    E, _ = orc.pair_energy(p0, 0, 0, 6.0, -0.25, 0.0, r1)
+    assert math.isclose(E, p0.elec_scale * -0.25 / ((A + B / (1.0 + k / math.e)) * r1), rel_tol=1e-12)
+    r2 = math.log(k) / (lam * B)
+    E, _ = orc.pair_energy(p0, 0, 0, 6.0, 0.4, 0.0, r2)
+    assert math.isclose(E, p0.elec_scale * 0.4 / ((A + 0.5 * B) * r2), rel_tol=1e-12)
+    # the rate is lambda*B = 0.3154 per Angstrom with the literature constants: both points are a few Angstrom out
+    assert 3.0 < r1 < 3.3 and 6.0 < r2 < 7.0
+    # a wrong rate (lambda alone in the exponent) gives eps(r1) = 1.45 instead of 13.95: the pin is sharp
+    E1, _ = orc.pair_energy(p0, 0, 0, 6.0, -0.25, 0.0, r1)
+    wrong = p0.elec_scale * -0.25 / ((A + B / (1.0 + k * math.exp(-lam * r1))) * r1)
+    assert abs(wrong / E1) > 9.0
+
+
 def test_pair_derivative_vs_central_difference_and_rmin(orc, par):
     for expA, cA in ((6.0, 800.0), (10.0, 9000.0)):
         for r in (0.9, 1.7, 3.3, 6.0, 11.0):
