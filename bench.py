@@ -146,6 +146,8 @@ def reduce_over_ranks(dist, dev, times, counts):
 
 # ------------------------------------------------------------------------------------------ CUDA arm
 def main():
+    if "--probe" in sys.argv:
+        return probe(sys.argv[sys.argv.index("--probe") + 1:])
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
@@ -354,6 +356,89 @@ def sweep(B, torch, dev, configs=("sweep40",)):
         gl.close()
         gg.close()
     return out
+
+
+def probe(argv):
+    """Single-kernel-family timing runs (the commands the ncu captures under profiles/ are taken from):
+
+        python bench.py --probe score <config> <n> <path> [reps]                       # adock_score_batch, energy + gradient
+        python bench.py --probe dock <ligands> <path> [max_evals] [ls_method] [autostop]   # adock_dock_many, drug-like config
+        python bench.py --probe large <path> [max_evals]                               # adock_dock, configs[3]
+        python bench.py --probe screen <ligands> <batch>                               # adock_screen, configs[2] sample
+        python bench.py --probe alu                                                    # adock_alu_peak
+
+    <path> is the argument of adock_set_path: 0 auto, 1 warp per individual, 2 / 21 / 22 / 24 lane per individual
+    (K chosen / 1 / 2 / 4 warps per group), 3 team per individual.  Prints one line; not the bench contract."""
+    import torch
+    from paper_2007_03678_b200 import binding as B
+    mode = argv[0]
+    dev = torch.device("cuda:0")
+    if mode == "alu":
+        print(B.adock_alu_peak(), flush=True)
+    elif mode == "score":
+        cfg, n, path = argv[1], int(argv[2]), int(argv[3])
+        reps = int(argv[4]) if len(argv) > 4 else 10
+        grids, lig = W.make_config(cfg)
+        gp = B.make_params(W.DEFAULT_PARAMS)
+        gg = B.Grids.from_workload(grids); gl = B.Ligand.from_workload(gg, lig, gp)
+        B.lib().adock_set_path(path)
+        G = torch.from_numpy(W.make_genotypes(n, lig.R, grids, seed=4)).to(dev)
+        E = torch.zeros(n, device=dev); gr = torch.zeros((n, 6 + lig.R), device=dev)
+        for _ in range(3):
+            B.adock_score_batch(gg, gl, gp, G, E, None, gr)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            B.adock_score_batch(gg, gl, gp, G, E, None, gr)
+        b.record(); torch.cuda.synchronize()
+        ms = a.elapsed_time(b) / reps
+        print(f"score {cfg} n={n} path={path}: {ms:.4f} ms  {n/ms*1e3:.4g} evals/s", flush=True)
+    elif mode == "screen":
+        nlig, batch = int(argv[1]), int(argv[2])
+        grids, _ = W.make_config("screen")
+        ligs = W.share_type_table(W.make_screen_ligands(nlig, grids, T=7, seed=2))
+        gp = B.make_params(W.DEFAULT_PARAMS); gg = B.Grids.from_workload(grids)
+        B.adock_screen(gg, ligs[:100], gp, 10, 150, 20000, list(range(len(ligs[:100]))), batch=0, host_threads=8)
+        B.adock_profile(True)
+        t0 = time.perf_counter()
+        r = B.adock_screen(gg, ligs, gp, 10, 150, 250000, [7000 + i for i in range(nlig)], batch=batch, host_threads=8)
+        dt = time.perf_counter() - t0
+        p = B.adock_profile_read()
+        print(f"screen n={nlig} batch={batch}: {dt:.2f} s {r['evals'].sum()/dt:.3e} evals/s batches {r['stats']['batches']} ls kernel "
+              f"{p['ls_ms']:.0f} ms {p['ls_launches']} launches {p['ls_evals']/max(p['ls_ms'], 1e-9)*1e3:.3e} evals/s in-kernel; family "
+              f"{B.lib().adock_last_dock_path()}", flush=True)
+    elif mode in ("dock", "large"):
+        if mode == "dock":
+            L, path = int(argv[1]), int(argv[2])
+            me = int(argv[3]) if len(argv) > 3 else MAX_EVALS
+            lsm = int(argv[4]) if len(argv) > 4 else 0
+            ast = int(argv[5]) if len(argv) > 5 else 0
+            grids, lig0 = W.make_config("drug")
+            centre = 0.5 * (grids.box_lo + grids.box_hi); c = W.CONFIGS["drug"]
+            ligs = [W.make_ligand(c["N"], c["R"], c["T"], 100 + i, centre) for i in range(L)]
+            nrun = NRUN
+        else:
+            L, path = 1, int(argv[1])
+            me = int(argv[2]) if len(argv) > 2 else MAX_EVALS
+            lsm = ast = 0
+            grids, lig0 = W.make_config("large")
+            ligs, nrun = [lig0], 50
+        gp = B.make_params(dict(W.DEFAULT_PARAMS, ls_method=lsm, autostop=ast))
+        gg = B.Grids.from_workload(grids); gl = [B.Ligand.from_workload(gg, l, gp) for l in ligs]
+        B.lib().adock_set_path(path)
+        B.adock_dock_many(gg, gl, gp, nrun, POP, min(me, 100000), list(range(L)))
+        B.adock_profile(True)
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        r = B.adock_dock_many(gg, gl, gp, nrun, POP, me, [7 + i for i in range(L)])
+        torch.cuda.synchronize(); dt = time.perf_counter() - t0
+        p = B.adock_profile_read()
+        ev = int(r["evals"].sum())
+        print(f"{mode} L={L} path={path} ls_method={lsm} autostop={ast} evals per run median {np.median(r['evals']):.0f} gens median "
+              f"{np.median(r['gens']):.0f}: {dt:.3f} s {ev/dt:.4g} evals/s; ls kernel {p['ls_ms']:.1f} ms {p['ls_launches']} launches "
+              f"{p['ls_evals']/max(p['ls_ms'], 1e-9)*1e3:.4g} evals/s in-kernel; family {B.adock_last_dock_path()}; "
+              f"best E median {np.median(r['energies']):.3f}", flush=True)
+    else:
+        raise SystemExit(f"unknown probe mode {mode!r}")
 
 
 def cpu_baseline():

@@ -113,7 +113,8 @@ int adock_ligand_lane_image(const adock_ligand* l, int* bytes, const unsigned ch
 
 /* Kernel family used by the compute entry points of this process: 0 = chosen by problem
  * size (default), 1 = one warp per individual, 2 = one lane per individual with K = 1, 2 or 4 warps sharing the
- * work of each group of 32 individuals (K chosen by size; 21, 22, 24 force K = 1, 2, 4).  All of them compute
+ * work of each group of 32 individuals (K chosen by size; 21, 22, 24 force K = 1, 2, 4; a forced K whose per-lane state
+ * does not fit in shared memory for a ligand makes the compute calls return ADOCK_ELIMIT).  All of them compute
  * the same function (R3-R7) and pass the same parity tests; they differ in summation order only.
  * 3 = the ADADELTA chains of adock_dock / adock_dock_many each run on a team (one CTA of 4 warps per individual,
  * threads over atoms and pairs), chosen by size when a launch holds too few chains to give every scheduler a warp
@@ -232,6 +233,12 @@ int adock_pose_rmsd(int n, int N, const float* coords, const float* ref, float* 
  * duration (ms), the number of launches timed and the evaluations they performed (calling thread). */
 int adock_profile(int enable);
 int adock_profile_read(double* ls_ms, long long* ls_launches, long long* ls_evals);
+
+/* Measured peak of the roofline that bounds the path (plain FP32 arithmetic, "bound": "alu"):
+ * times a kernel of independent fma.rn.f32x2 chains (16 warps on every SM) on cuda_stream and returns the achieved
+ * TFLOP/s (FMA = 2 FLOP) and FMA lanes per clock and SM at the device's nominal maximum clock (128 = one FP32 FMA per
+ * lane and clock).  Synchronous.  MEASURED_PEAKS.json carries HBM and tensor figures only; bench.py reports this one. */
+int adock_alu_peak(double* tflops, double* fma_lanes_per_clk_sm, void* cuda_stream);
 
 /* Kernel launches issued by this library on the calling thread since the last reset (bench accounting). */
 long long adock_launch_count(int reset);

@@ -23,7 +23,7 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB,
+        cmd = [nvcc, *NVCC_FLAGS, *os.environ.get("ADOCK_NVCC_EXTRA", "").split(), *(["-Xptxas", "-v"] if verbose else []), "-o", LIB,
                *[os.path.join(CSRC, s) for s in SOURCES]]
         subprocess.check_call(cmd)
     return LIB

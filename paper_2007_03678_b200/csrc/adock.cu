@@ -131,17 +131,26 @@ static int check_params(const adock_params* in, const adock_ligand* l, adock_par
 }
 
 // =================================================================== grids
+// caller's [M][nz][ny][nx] maps -> xy-patch cells per (type, charge sign): cells[2t + s][z][y][x] (y < ny-1, x < nx-1)
+// = one 32-byte sector {a_t, pm}(x,y) {a_t, pm}(x+1,y) | {a_t, pm}(x,y+1) {a_t, pm}(x+1,y+1) of plane z, with
+// pm = elec + desolv (s = 0) or elec - desolv (s = 1)   (device.cuh, grid term)
 __global__ void relayout_kernel(const float* __restrict__ maps, float4* __restrict__ cells, int T, int nx, int ny, int nz) {
-    const long long ncell = (long long)T * nz * ny * (nx - 1);
+    const long long per_set = (long long)nz * (ny - 1) * (nx - 1);
+    const long long ncell = 2ll * T * per_set;
     const long long plane = (long long)nz * ny * nx;
+    const float* el = maps + T * plane;
+    const float* ds = maps + (T + 1) * plane;
     for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x) {
         const int ix = (int)(c % (nx - 1));
-        const long long row = c / (nx - 1);               // (t*nz + z)*ny + y
-        const long long zy = row % ((long long)nz * ny);
-        const int t = (int)(row / ((long long)nz * ny));
-        const long long p = zy * nx + ix;
-        cells[2 * c] = make_float4(maps[t * plane + p], maps[T * plane + p], maps[(T + 1) * plane + p], 0.f);
-        cells[2 * c + 1] = make_float4(maps[t * plane + p + 1], maps[T * plane + p + 1], maps[(T + 1) * plane + p + 1], 0.f);
+        const long long row = c / (nx - 1);               // (set*nz + z)*(ny-1) + y
+        const int iy = (int)(row % (ny - 1));
+        const long long sz = row / (ny - 1);               // set*nz + z
+        const int iz = (int)(sz % nz), set = (int)(sz / nz);
+        const float* at = maps + (set >> 1) * plane;
+        const float sg = (set & 1) ? -1.f : 1.f;
+        const long long p = ((long long)iz * ny + iy) * nx + ix, p1 = p + nx;
+        cells[2 * c] = make_float4(at[p], el[p] + sg * ds[p], at[p + 1], el[p + 1] + sg * ds[p + 1]);
+        cells[2 * c + 1] = make_float4(at[p1], el[p1] + sg * ds[p1], at[p1 + 1], el[p1 + 1] + sg * ds[p1 + 1]);
     }
 }
 
@@ -157,7 +166,7 @@ extern "C" int adock_load_grids(const float* host_maps, int M, int nx, int ny, i
     const int T = M - 2;
     float* d_raw = nullptr;
     float4* cells = nullptr;
-    const size_t ncell = (size_t)T * nz * ny * (nx - 1);
+    const size_t ncell = (size_t)2 * T * nz * (ny - 1) * (nx - 1);
     cudaError_t e = cudaMalloc(&d_raw, (size_t)M * npts * sizeof(float));
     if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("cudaMalloc: ") + cudaGetErrorString(e));
     e = cudaMalloc(&cells, ncell * 2 * sizeof(float4));
@@ -173,7 +182,7 @@ extern "C" int adock_load_grids(const float* host_maps, int M, int nx, int ny, i
     adock_grids* g = new adock_grids;
     g->M = M; g->cells = cells;
     g->dev.cells = cells;
-    g->dev.type_stride = (long long)nz * ny * (nx - 1) * 2;
+    g->dev.set_stride = (long long)nz * (ny - 1) * (nx - 1) * 2;
     g->dev.nx = nx; g->dev.ny = ny; g->dev.nz = nz; g->dev.T = T;
     g->dev.h = spacing; g->dev.inv_h = 1.0f / spacing;
     g->dev.ox = origin[0]; g->dev.oy = origin[1]; g->dev.oz = origin[2];
@@ -206,6 +215,9 @@ extern "C" int adock_load_ligand(const adock_grids* grids, const adock_params* p
             return fail(ADOCK_EINVAL, "non-finite ligand input");
     }
     for (int i = 0; i < T * T * 4; ++i) if (!std::isfinite(pair_coeffs[i])) return fail(ADOCK_EINVAL, "non-finite pair coefficient");
+    for (int i = 0; i < T * T; ++i)         // the kernels evaluate r^-6 and r^-10 only (R5)
+        if (pair_coeffs[4 * i + 2] != 6.0f && pair_coeffs[4 * i + 2] != 10.0f) return fail(ADOCK_EINVAL, "pair exponent expA must be 6 or 10");
+    for (int i = 0; i < T; ++i) if (!std::isfinite(solpar[i]) || !std::isfinite(vol[i])) return fail(ADOCK_EINVAL, "non-finite solpar / vol");
     adock_ligand* l = new adock_ligand;
     if (!build_topology(l->tp, N, xyz, type, charge, nbonds, bonds, R, rot_bonds, root_atom, T, pair_coeffs, solpar, vol, p.w_desolv, p.qasp)) {
         std::string msg = l->tp.error;
@@ -406,9 +418,8 @@ static LanePlan lane_plan(const LaneGeom& g, long long total, int jg) {
     double best_t = 1e300;
     if (total < 1) total = 1;
     if (jg < 1) jg = 1;
-    for (int pass = 0; pass < 2 && !best.K; ++pass)             // pass 0 honours a forced K; pass 1: any K that fits
     for (int K = 1; K <= 4; K *= 2) {
-        if (pass == 0 && g_lane_k && K != g_lane_k) continue;
+        if (g_lane_k && K != g_lane_k) continue;                // a forced K that does not fit is an error (ADOCK_ELIMIT), never a silent substitute
         const double eff = K == 1 ? 1.0 : K == 2 ? 0.95 : 0.85;
         for (int ng = lane_max_warps(K) / K; ng >= 1; --ng) {
             if (lane_plan_smem(g, K, ng, lane_plan_images(total, jg, ng)) > (size_t)g_smem_optin) continue;
@@ -635,7 +646,7 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) ls_array_lane_k
         for (int d = 0; d < Gn; ++d) S.geno[d * 32] = a.genos[idx * a.gstride + d];
     group_sync<K>(S);
     LaneLS ls;
-    ls.best = scratch + tid; ls.Eg2 = ls.best + (size_t)Gn * T; ls.Ed2 = ls.Eg2 + (size_t)D * T; ls.grad = ls.Ed2 + (size_t)D * T;
+    ls.best = scratch + tid; ls.Eg2 = ls.best + (size_t)Gn * T; ls.Ed2 = ls.Eg2 + (size_t)D * T;
     ls.stride = (int)T;
     int iters = 0;
     float* tr = a.trace ? a.trace + idx * P.lsit : nullptr;
@@ -658,7 +669,7 @@ static int launch_ls_array_lane(const adock_grids* grids, const adock_ligand* li
     const size_t T = (size_t)grid * NG * 32;
     const int R = ligand->tp.R;
     float* scratch = nullptr;
-    cudaError_t e = cudaMallocAsync(&scratch, T * (size_t)(7 + R + 3 * (6 + R)) * 4, stm);
+    cudaError_t e = cudaMallocAsync(&scratch, T * (size_t)(7 + R + 2 * (6 + R)) * 4, stm);
     if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("ls scratch: ") + cudaGetErrorString(e));
     e = cudaFuncSetAttribute(ls_array_lane_kernel<K, SW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) {
@@ -946,7 +957,7 @@ __device__ __forceinline__ LaneCtaGroup lane_cta_group(unsigned char* smem, cons
 }
 
 // ADADELTA on the selected individuals (Lamarckian write-back): lane c of a job's groups runs chain c = run*n_ls + l;
-// ADADELTA state in global scratch columns [row][all group lanes of the launch] (rows: Gmax best, 3 x Dmax)
+// ADADELTA state in global scratch columns [row][all group lanes of the launch] (rows: Gmax best, 2 x Dmax)
 template <int K, bool SW>
 __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_ls_lane_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs,
                                                                                      DockDims dm, LaneDockArgs a) {
@@ -975,7 +986,7 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_ls_lane_ke
     const size_t tid = ((size_t)blockIdx.x * a.ng + S.gid) * 32 + lane, T = (size_t)gridDim.x * a.ng * 32;
     const int Dmax = a.Gmax - 1;
     LaneLS ls;
-    ls.best = a.scratch + tid; ls.Eg2 = ls.best + (size_t)a.Gmax * T; ls.Ed2 = ls.Eg2 + (size_t)Dmax * T; ls.grad = ls.Ed2 + (size_t)Dmax * T;
+    ls.best = a.scratch + tid; ls.Eg2 = ls.best + (size_t)a.Gmax * T; ls.Ed2 = ls.Eg2 + (size_t)Dmax * T;
     ls.stride = (int)T;
     int iters = 0;
     const float e0 = (act && S.part == 0) ? *e : 0.f;
@@ -1255,7 +1266,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     float* d_lscratch = nullptr;
     if (ls_lane && dm.n_ls > 0) {
         const size_t T = (size_t)pl.nctas * pl.ng * 32;
-        cudaError_t e2 = buf.alloc(&d_lscratch, T * (size_t)(Gmax + 3 * (Gmax - 1)) * 4);
+        cudaError_t e2 = buf.alloc(&d_lscratch, T * (size_t)(Gmax + 2 * (Gmax - 1)) * 4);
         if (e2 != cudaSuccess) return fail(e2 == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("dock alloc: ") + cudaGetErrorString(e2));
         al = LaneDockArgs{d_lscratch, Gmax, pl.ng, nlig * jg, jg, pl.slot, pl.nimg, pl.gfloats};
         if (pl.K == 1) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
@@ -1570,9 +1581,10 @@ extern "C" int adock_screen(const adock_grids* grids, const adock_params* params
 // one warp per ordered pair (a, b), b in [0, n]: b == n is the reference pose
 __global__ void __launch_bounds__(256) pose_rmsd_kernel(const float* __restrict__ x, const float* __restrict__ ref, int n, int N,
                                                         float* __restrict__ out_ref, float* __restrict__ out_pair) {
-    const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (w >= n * (n + 1)) return;
-    const int a = w / (n + 1), b = w % (n + 1);
+    const long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (w >= (long long)n * (n + 1)) return;
+    const int a = (int)(w / (n + 1)), b = (int)(w % (n + 1));
     if (b == n ? !out_ref : (!out_pair || b < a)) return;
     const float* pa = x + (size_t)a * N * 3;
     const float* pb = b == n ? ref : x + (size_t)b * N * 3;
@@ -1589,6 +1601,7 @@ __global__ void __launch_bounds__(256) pose_rmsd_kernel(const float* __restrict_
 extern "C" int adock_pose_rmsd(int n, int N, const float* coords, const float* ref, float* rmsd_ref, float* rmsd_pair,
                                const float* energies, float tol, int* cluster, int* nclusters, void* cuda_stream) {
     if (n < 0 || N < 1) return fail(ADOCK_EINVAL, "bad pose dimensions");
+    if (n > 32768) return fail(ADOCK_ELIMIT, "more than 32768 poses");
     if (nclusters) *nclusters = 0;
     if (n == 0) return ADOCK_OK;
     if (!coords || (rmsd_ref && !ref) || (cluster && (!energies || !(tol > 0) || !nclusters))) return fail(ADOCK_EINVAL, "NULL argument");
@@ -1687,5 +1700,61 @@ extern "C" int adock_ga_generation(const adock_grids* grids, const adock_ligand*
     }
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaStreamSynchronize(stm));
+    return ADOCK_OK;
+}
+
+// =================================================================== measurement utility: the ALU roofline's peak
+// The hot path is bound by plain FP32 arithmetic, for which MEASURED_PEAKS.json has no figure.
+// This kernel measures it where the benchmark runs: 8 independent chains of fma.rn.f32x2 per thread, 16 warps per SM,
+// one CTA per SM; FLOP = 2 (FMA) x 2 (lanes of the packed operand) per instruction and thread.
+__global__ void __launch_bounds__(512) alu_peak_kernel(float* out, int iters, float seed) {
+    f2 p[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) p[i] = pk(seed + i, seed - i);
+    const f2 a = pk(0.999f, 1.001f), b = pk(1e-3f, -1e-3f);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(p[i].v) : "l"(p[i].v), "l"(a.v), "l"(b.v));
+        }
+    }
+    float acc = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc += hsum(p[i]);
+    if (acc == 12345.678f) out[0] = acc;
+}
+
+extern "C" int adock_alu_peak(double* tflops, double* fma_lanes_per_clk_sm, void* cuda_stream) {
+    int rc = device_props();
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, khz = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev));
+    float* d = nullptr;
+    CUDA_TRY(cudaMalloc(&d, 4));
+    const int iters = 20000, warps = 16;
+    cudaEvent_t a = nullptr, b = nullptr;
+    cudaError_t e = cudaEventCreate(&a);
+    if (e == cudaSuccess) e = cudaEventCreate(&b);
+    float best = 1e30f;
+    for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {         // first launch = warm-up; best of the other three
+        e = cudaEventRecord(a, st);
+        alu_peak_kernel<<<g_sm_count, warps * 32, 0, st>>>(d, iters, 1.0f);
+        ++g_launches;
+        if (e == cudaSuccess) e = cudaEventRecord(b, st);
+        if (e == cudaSuccess) e = cudaEventSynchronize(b);
+        float ms = 0;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    if (a) cudaEventDestroy(a);
+    if (b) cudaEventDestroy(b);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(ADOCK_ECUDA, std::string("alu_peak: ") + cudaGetErrorString(e));
+    const double lanes = (double)g_sm_count * warps * 32 * iters * 4 * 8 * 2.0;       // FMA lanes executed
+    if (tflops) *tflops = 2.0 * lanes / (best * 1e-3) / 1e12;
+    if (fma_lanes_per_clk_sm) *fma_lanes_per_clk_sm = lanes / (best * 1e-3 * khz * 1e3) / g_sm_count;
     return ADOCK_OK;
 }

@@ -15,8 +15,10 @@ constexpr float kPi = 3.14159265358979323846f;
 constexpr float kTwoPi = 6.28318530717958647692f;
 
 struct GridDev {
-    const float4* cells;    // [T][nz][ny][nx-1] x-pair cells of 2 float4: {a_t,elec,desolv,0}(ix), same (ix+1)
-    long long type_stride;  // float4 units between types
+    const float4* cells;    // [2T][nz][ny-1][nx-1] xy-patch cells of one 32-byte sector (2 float4): the pair (a_t, pm) at the
+                            // nodes (ix,iy), (ix+1,iy), (ix,iy+1), (ix+1,iy+1) of plane iz, for cell set 2t + s;
+                            // pm = elec + desolv (s = 0: atoms with q >= 0) or elec - desolv (s = 1: q < 0)
+    long long set_stride;   // float4 units between cell sets
     int nx, ny, nz, T;
     float inv_h, h;
     float ox, oy, oz;
@@ -152,11 +154,36 @@ __device__ inline void stage_images(unsigned char* dst, int slot_bytes, int nimg
     }
 }
 
+// ---------------------------------------------------------------- packed f32x2 (FFMA2 / FMUL2 / FADD2)
+struct f2 { unsigned long long v; };
+__device__ __forceinline__ f2 pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r.v) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ f2 bc(float x) { return pk(x, x); }
+__device__ __forceinline__ void unpk(f2 a, float& lo, float& hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.v)); }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
+__device__ __forceinline__ f2 sub2(f2 a, f2 b) { f2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d.v) : "l"(a.v), "l"(b.v), "l"(c.v)); return d; }
+__device__ __forceinline__ f2 neg2(f2 a) { f2 d; d.v = a.v ^ 0x8000000080000000ull; return d; }
+__device__ __forceinline__ float hsum(f2 a) { float l, h; unpk(a, l, h); return l + h; }
+__device__ __forceinline__ f2 ld2(const float2* p) { const float2 v = *p; return pk(v.x, v.y); }
+
 // ---------------------------------------------------------------- grid term (R4)
+// One routine for every kernel family, in three stages so that a caller can issue the loads of several atoms before
+// consuming any of them: grid_cell (clamp, cell index, fractions), grid_fetch (2 sector loads), grid_finish
+// (trilinear value and gradient).
+// The atom's energy is a_t + q*elec + |q|*desolv = a_t + q*(elec + sign(q)*desolv): the maps are re-laid-out once
+// (relayout_kernel) into cell sets indexed by (type, sign of the charge) holding the pair (a_t, pm = elec +- desolv) per
+// node, so the two fields an atom interpolates arrive as the two halves of packed f32x2 operands, register-aligned
+// straight from the load: no per-corner mixing and no packing moves.  The small field pm (O(1..10)) and the affinity
+// field (up to the 1e5 clamp) stay in separate halves until the very end, so the small one is never rounded to the
+// ulp of the large one before the corner differences that make the gradient are taken.
+// A cell is the 2x2 (x, y) patch of one z-plane = one aligned 32-byte sector, fetched whole by one LDG.256: a lookup is
+// two sector loads (planes iz, iz+1), all 64 bytes used.  Measured (profiles/r02_grid_layout.md): the cost of the grid
+// phase is per load request and lane (L1 miss handling), not per byte -- a 256-bit sector load is faster than a 128-bit
+// load of half of it -- so the layout minimises requests; the price is every node stored four times per set.
+// The lookups of a warp are scattered over the maps (32 lanes = 32 poses), so a line brought into L1 is not touched
+// again before it is evicted: L1::no_allocate skips the allocation (profiles/r01b_grid_load_variants.md).
 struct F8 { float4 lo, hi; };
-// One aligned 32-byte sector (LDG.256).  The lookups of a warp are scattered over the maps (32 lanes = 32 poses), so a
-// line brought into L1 is not touched again before it is evicted: L1::no_allocate skips the allocation and is +31 %
-// on the lane-per-individual scoring kernel (profiles/r01b_grid_load_variants.md); the maps stay L2 resident.
 __device__ __forceinline__ F8 ld_cell(const float4* p) {
     F8 r;
     asm("ld.global.nc.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
@@ -164,67 +191,13 @@ __device__ __forceinline__ F8 ld_cell(const float4* p) {
         : "l"(p));
     return r;
 }
-
-// trilinear interpolant of 8 corner values (a = ix, b = ix+1; first index z, second y) at fractions fx,fy,fz:
-// value and derivatives with respect to the fractions
-template <bool GRAD>
-__device__ __forceinline__ void trilinear8(float a00, float b00, float a01, float b01, float a10, float b10, float a11, float b11,
-                                           float fx, float fy, float fz, float& val, float& dfx, float& dfy, float& dfz) {
-    const float d00 = b00 - a00, d01 = b01 - a01, d10 = b10 - a10, d11 = b11 - a11;       // d/dfx per row
-    const float v00 = fmaf(fx, d00, a00), v01 = fmaf(fx, d01, a01), v10 = fmaf(fx, d10, a10), v11 = fmaf(fx, d11, a11);
-    const float e0 = v01 - v00, e1 = v11 - v10;                                            // d/dfy per z-plane
-    const float w0 = fmaf(fy, e0, v00), w1 = fmaf(fy, e1, v10);
-    val = fmaf(fz, w1 - w0, w0);
-    if (GRAD) {
-        const float dx0 = fmaf(fy, d01 - d00, d00), dx1 = fmaf(fy, d11 - d10, d10);
-        dfx = fmaf(fz, dx1 - dx0, dx0);
-        dfy = fmaf(fz, e1 - e0, e0);
-        dfz = w1 - w0;
-    }
-}
-
-template <bool GRAD>
-__device__ __forceinline__ float grid_atom(const GridDev& G, const ParDev& P, int type, float q, float x, float y, float z,
-                                           float& gx, float& gy, float& gz) {
-    float ux = (x - G.ox) * G.inv_h, uy = (y - G.oy) * G.inv_h, uz = (z - G.oz) * G.inv_h;
-    float cx = fminf(fmaxf(ux, 0.f), (float)(G.nx - 1)), cy = fminf(fmaxf(uy, 0.f), (float)(G.ny - 1)),
-          cz = fminf(fmaxf(uz, 0.f), (float)(G.nz - 1));
-    int ix = min((int)cx, G.nx - 2), iy = min((int)cy, G.ny - 2), iz = min((int)cz, G.nz - 2);
-    float fx = cx - (float)ix, fy = cy - (float)iy, fz = cz - (float)iz;
-    float ox = ux - cx, oy = uy - cy, oz = uz - cz;
-    const int rowlen = (G.nx - 1) * 2;
-    const float4* base = G.cells + (long long)type * G.type_stride + ((long long)(iz * G.ny + iy) * (G.nx - 1) + ix) * 2;
-    F8 c00 = ld_cell(base), c01 = ld_cell(base + rowlen), c10 = ld_cell(base + (long long)G.ny * rowlen),
-       c11 = ld_cell(base + (long long)G.ny * rowlen + rowlen);
-    const float aq = fabsf(q);
-    // Two interpolants, combined only at the end: the affinity map (values up to the 1e5 clamp) and
-    // q*elec + |q|*desolv (values O(1)).  Mixing them per corner would round the small field to the ulp of the
-    // large one (0.008 at 1e5) before the corner differences that make the gradient are taken.
-    float val, dfx, dfy, dfz;
-    trilinear8<GRAD>(c00.lo.x, c00.hi.x, c01.lo.x, c01.hi.x, c10.lo.x, c10.hi.x, c11.lo.x, c11.hi.x, fx, fy, fz, val, dfx, dfy, dfz);
-    float vs, sfx, sfy, sfz;
-    trilinear8<GRAD>(fmaf(aq, c00.lo.z, q * c00.lo.y), fmaf(aq, c00.hi.z, q * c00.hi.y), fmaf(aq, c01.lo.z, q * c01.lo.y),
-                     fmaf(aq, c01.hi.z, q * c01.hi.y), fmaf(aq, c10.lo.z, q * c10.lo.y), fmaf(aq, c10.hi.z, q * c10.hi.y),
-                     fmaf(aq, c11.lo.z, q * c11.lo.y), fmaf(aq, c11.hi.z, q * c11.hi.y), fx, fy, fz, vs, sfx, sfy, sfz);
-    val += vs;
-    float wall = fabsf(ox) + fabsf(oy) + fabsf(oz);
-    val = fmaf(P.k_wall_h, wall, val);
-    if (GRAD) {
-        gx = (ox != 0.f) ? copysignf(P.k_wall, ox) : (dfx + sfx) * G.inv_h;
-        gy = (oy != 0.f) ? copysignf(P.k_wall, oy) : (dfy + sfy) * G.inv_h;
-        gz = (oz != 0.f) ? copysignf(P.k_wall, oz) : (dfz + sfz) * G.inv_h;
-    }
-    return val;
-}
-
-// The same lookup in three stages, so that a caller can issue the sector loads of several atoms before consuming
-// any of them: grid_cell (clamp, cell index, fractions), grid_fetch (4 sector loads), grid_finish (interpolation).
 struct GridCell {
-    const float4* base;     // sector of corner (iz, iy, ix..ix+1) of the atom's type
+    const float4* base;     // cell (iz, iy, ix) of the atom's cell set
     float fx, fy, fz;       // fractions inside the cell
     float ox, oy, oz;       // signed distance outside the box in grid units (0 inside)
 };
-__device__ __forceinline__ GridCell grid_cell(const GridDev& G, int type, float x, float y, float z) {
+// `set` = 2*type + (q < 0)
+__device__ __forceinline__ GridCell grid_cell(const GridDev& G, int set, float x, float y, float z) {
     const float ux = (x - G.ox) * G.inv_h, uy = (y - G.oy) * G.inv_h, uz = (z - G.oz) * G.inv_h;
     const float cx = fminf(fmaxf(ux, 0.f), (float)(G.nx - 1)), cy = fminf(fmaxf(uy, 0.f), (float)(G.ny - 1)),
                 cz = fminf(fmaxf(uz, 0.f), (float)(G.nz - 1));
@@ -232,34 +205,53 @@ __device__ __forceinline__ GridCell grid_cell(const GridDev& G, int type, float 
     GridCell c;
     c.fx = cx - (float)ix; c.fy = cy - (float)iy; c.fz = cz - (float)iz;
     c.ox = ux - cx; c.oy = uy - cy; c.oz = uz - cz;
-    c.base = G.cells + (long long)type * G.type_stride + ((long long)(iz * G.ny + iy) * (G.nx - 1) + ix) * 2;
+    c.base = G.cells + (long long)set * G.set_stride + ((long long)(iz * (G.ny - 1) + iy) * (G.nx - 1) + ix) * 2;
     return c;
 }
-__device__ __forceinline__ void grid_fetch(const GridDev& G, const GridCell& c, F8 (&v)[4]) {
-    const int rowlen = (G.nx - 1) * 2;
+// v[0] = plane iz, v[1] = plane iz+1; each {a,pm}(ix,iy) {a,pm}(ix+1,iy) | {a,pm}(ix,iy+1) {a,pm}(ix+1,iy+1)
+__device__ __forceinline__ void grid_fetch(const GridDev& G, const GridCell& c, F8 (&v)[2]) {
     v[0] = ld_cell(c.base);
-    v[1] = ld_cell(c.base + rowlen);
-    v[2] = ld_cell(c.base + (long long)G.ny * rowlen);
-    v[3] = ld_cell(c.base + (long long)G.ny * rowlen + rowlen);
+    v[1] = ld_cell(c.base + (long long)(G.ny - 1) * (G.nx - 1) * 2);
 }
+// value and (GRAD) gradient in kcal/mol/A of the atom's grid energy; packed halves (affinity | pm), joined as
+// lo + q*hi at the very end
 template <bool GRAD>
-__device__ __forceinline__ float grid_finish(const GridDev& G, const ParDev& P, const GridCell& c, const F8 (&v)[4], float q,
+__device__ __forceinline__ float grid_finish(const GridDev& G, const ParDev& P, const GridCell& c, const F8 (&v)[2], float q,
                                              float& gx, float& gy, float& gz) {
-    const float aq = fabsf(q);
-    float val, dfx, dfy, dfz, vs, sfx, sfy, sfz;
-    trilinear8<GRAD>(v[0].lo.x, v[0].hi.x, v[1].lo.x, v[1].hi.x, v[2].lo.x, v[2].hi.x, v[3].lo.x, v[3].hi.x, c.fx, c.fy, c.fz,
-                     val, dfx, dfy, dfz);
-    trilinear8<GRAD>(fmaf(aq, v[0].lo.z, q * v[0].lo.y), fmaf(aq, v[0].hi.z, q * v[0].hi.y), fmaf(aq, v[1].lo.z, q * v[1].lo.y),
-                     fmaf(aq, v[1].hi.z, q * v[1].hi.y), fmaf(aq, v[2].lo.z, q * v[2].lo.y), fmaf(aq, v[2].hi.z, q * v[2].hi.y),
-                     fmaf(aq, v[3].lo.z, q * v[3].lo.y), fmaf(aq, v[3].hi.z, q * v[3].hi.y), c.fx, c.fy, c.fz, vs, sfx, sfy, sfz);
-    val += vs;
+    const f2 a00 = pk(v[0].lo.x, v[0].lo.y), b00 = pk(v[0].lo.z, v[0].lo.w), a01 = pk(v[0].hi.x, v[0].hi.y), b01 = pk(v[0].hi.z, v[0].hi.w);
+    const f2 a10 = pk(v[1].lo.x, v[1].lo.y), b10 = pk(v[1].lo.z, v[1].lo.w), a11 = pk(v[1].hi.x, v[1].hi.y), b11 = pk(v[1].hi.z, v[1].hi.w);
+    const f2 fx = bc(c.fx), fy = bc(c.fy), fz = bc(c.fz);
+    const f2 d00 = sub2(b00, a00), d01 = sub2(b01, a01), d10 = sub2(b10, a10), d11 = sub2(b11, a11);       // d/dfx per row
+    const f2 v00 = fma2(fx, d00, a00), v01 = fma2(fx, d01, a01), v10 = fma2(fx, d10, a10), v11 = fma2(fx, d11, a11);
+    const f2 e0 = sub2(v01, v00), e1 = sub2(v11, v10);                                                    // d/dfy per z-plane
+    const f2 w0 = fma2(fy, e0, v00), w1 = fma2(fy, e1, v10);
+    const f2 dz = sub2(w1, w0);
+    float lo, hi;
+    unpk(fma2(fz, dz, w0), lo, hi);
+    float val = fmaf(q, hi, lo);
     val = fmaf(P.k_wall_h, fabsf(c.ox) + fabsf(c.oy) + fabsf(c.oz), val);
     if (GRAD) {
-        gx = (c.ox != 0.f) ? copysignf(P.k_wall, c.ox) : (dfx + sfx) * G.inv_h;
-        gy = (c.oy != 0.f) ? copysignf(P.k_wall, c.oy) : (dfy + sfy) * G.inv_h;
-        gz = (c.oz != 0.f) ? copysignf(P.k_wall, c.oz) : (dfz + sfz) * G.inv_h;
+        const f2 dx0 = fma2(fy, sub2(d01, d00), d00), dx1 = fma2(fy, sub2(d11, d10), d10);
+        unpk(fma2(fz, sub2(dx1, dx0), dx0), lo, hi);
+        const float dfx = fmaf(q, hi, lo);
+        unpk(fma2(fz, sub2(e1, e0), e0), lo, hi);
+        const float dfy = fmaf(q, hi, lo);
+        unpk(dz, lo, hi);
+        const float dfz = fmaf(q, hi, lo);
+        gx = (c.ox != 0.f) ? copysignf(P.k_wall, c.ox) : dfx * G.inv_h;
+        gy = (c.oy != 0.f) ? copysignf(P.k_wall, c.oy) : dfy * G.inv_h;
+        gz = (c.oz != 0.f) ? copysignf(P.k_wall, c.oz) : dfz * G.inv_h;
     }
     return val;
+}
+// the three stages for one atom
+template <bool GRAD>
+__device__ __forceinline__ float grid_atom(const GridDev& G, const ParDev& P, int set, float q, float x, float y, float z,
+                                           float& gx, float& gy, float& gz) {
+    const GridCell c = grid_cell(G, set, x, y, z);
+    F8 v[2];
+    grid_fetch(G, c, v);
+    return grid_finish<GRAD>(G, P, c, v, q, gx, gy, gz);
 }
 
 // single-instruction MUFU forms (flush-to-zero): reciprocal, reciprocal square root, 2^x
@@ -403,7 +395,10 @@ __device__ __forceinline__ float eval_pose(const LigS& L, const GridDev& G, cons
     __syncwarp();
 
     // (a1,a2) atoms: pose, then trilinear lookup of the three maps
-    float eg = 0.f;
+    // The rigid-body gradient (dE/dt, dE/domega) is summed from the GRID forces alone: intramolecular pair forces
+    // cancel exactly in both (Newton's third law), so adding them would only put their rounding (r^-13 clash terms)
+    // into two blocks they contribute nothing to.
+    float eg = 0.f, rFx = 0.f, rFy = 0.f, rFz = 0.f, rTx = 0.f, rTy = 0.f, rTz = 0.f;
     for (int i = lane; i < L.npos; i += 32) {
         const uint32_t m = L.meta[i];
         if (m == 0xffffffffu) continue;                  // hole
@@ -417,7 +412,16 @@ __device__ __forceinline__ float eval_pose(const LigS& L, const GridDev& G, cons
         b[kX] = x; b[kY] = y; b[kZ] = z; b[kQ] = a.w * P.elec_sqrt;
         float gx, gy, gz;
         eg += grid_atom<GRAD>(G, P, (int)(m & 0xff), a.w, x, y, z, gx, gy, gz);
-        if (GRAD) { b[kGX] = gx; b[kGY] = gy; b[kGZ] = gz; }
+        if (GRAD) {
+            b[kGX] = gx; b[kGY] = gy; b[kGZ] = gz;
+            const float rx = x - tx, ry = y - ty, rz = z - tz;
+            rFx += gx; rFy += gy; rFz += gz;
+            rTx += ry * gz - rz * gy; rTy += rz * gx - rx * gz; rTz += rx * gy - ry * gx;
+        }
+    }
+    if (GRAD) {
+        rFx = warp_sum(rFx); rFy = warp_sum(rFy); rFz = warp_sum(rFz);
+        rTx = warp_sum(rTx); rTy = warp_sum(rTy); rTz = warp_sum(rTz);
     }
     __syncwarp();
 
@@ -465,9 +469,9 @@ __device__ __forceinline__ float eval_pose(const LigS& L, const GridDev& G, cons
                 Fx += F.x; Fy += F.y; Fz += F.z;
                 Tx += T.x + (ly * F.z - lz * F.y); Ty += T.y + (lz * F.x - lx * F.z); Tz += T.z + (lx * F.y - ly * F.x);
             }
-            if (f == 0) {
-                S.grad[0] = Fx; S.grad[1] = Fy; S.grad[2] = Fz;
-                S.grad[3] = Tx; S.grad[4] = Ty; S.grad[5] = Tz;
+            if (f == 0) {                               // rigid-body blocks: grid forces only (see the atom loop)
+                S.grad[0] = rFx; S.grad[1] = rFy; S.grad[2] = rFz;
+                S.grad[3] = rTx; S.grad[4] = rTy; S.grad[5] = rTz;
             } else {
                 const float4 u = S.fragAx[2 * f];
                 S.grad[6 + (w >> 16)] = u.x * Tx + u.y * Ty + u.z * Tz;
@@ -603,9 +607,10 @@ __device__ inline void ga_make_child(const ParDev& P, int Pn, int R, unsigned lo
 // back-propagation.  Same arithmetic as eval_pose; the summation order differs (fixed, so results are reproducible).
 constexpr int kTeamW = 4;
 __host__ __device__ inline int team_scratch_floats(int N, int nfrag, int R) {
-    return warp_scratch_floats(N, nfrag, R) + (kTeamW - 1) * ((N + 31) / 32) * 96 + 16;
+    return warp_scratch_floats(N, nfrag, R) + (kTeamW - 1) * ((N + 31) / 32) * 96 + 8 * kTeamW + 8;
 }
-struct TeamS { WarpS S; float* gextra; float* red; int wi, gplane; };     // red: [2 kTeamW] partial energies, [8] flag; gplane = floats per extra plane
+// red: per warp w [8w .. 8w+8) = partial (e_grid, e_pairs, grid force F(3), grid torque about t T(3)); [8 kTeamW] = flag
+struct TeamS { WarpS S; float* gextra; float* red; int wi, gplane; };     // gplane = floats per extra plane
 __device__ inline TeamS team_view(float* base, const LigS& L, int wi) {
     TeamS T;
     T.S = warp_view(base, L);
@@ -683,7 +688,7 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
     }
     team_sync();
     // (a1,a2) atoms: one thread per position (pose + trilinear lookup); the owner also clears the atom's extra planes
-    float eg = 0.f;
+    float eg = 0.f, rFx = 0.f, rFy = 0.f, rFz = 0.f, rTx = 0.f, rTy = 0.f, rTz = 0.f;     // rigid-body sums: grid forces only (eval_pose)
     for (int i = wi * 32 + lane; i < L.npos; i += 32 * kTeamW) {
         const uint32_t m = L.meta[i];
         if (m == 0xffffffffu) continue;                  // hole
@@ -700,8 +705,19 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
         eg += grid_atom<GRAD>(G, P, (int)(m & 0xff), a.w, x, y, z, gx, gy, gz);
         if (GRAD) {
             b[kGX] = gx; b[kGY] = gy; b[kGZ] = gz;
+            const float rx = x - tx, ry = y - ty, rz = z - tz;
+            rFx += gx; rFy += gy; rFz += gz;
+            rTx += ry * gz - rz * gy; rTy += rz * gx - rx * gz; rTz += rx * gy - ry * gx;
 #pragma unroll
             for (int w = 1; w < kTeamW; ++w) { float* g = team_gptr(T, w, off); g[0] = 0.f; g[32] = 0.f; g[64] = 0.f; }
+        }
+    }
+    if (GRAD) {
+        rFx = warp_sum(rFx); rFy = warp_sum(rFy); rFz = warp_sum(rFz);
+        rTx = warp_sum(rTx); rTy = warp_sum(rTy); rTz = warp_sum(rTz);
+        if (lane == 0) {
+            float* r = T.red + 8 * wi + 2;
+            r[0] = rFx; r[1] = rFy; r[2] = rFz; r[3] = rTx; r[4] = rTy; r[5] = rTz;
         }
     }
     team_sync();
@@ -720,11 +736,11 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
         ep += o.e;
     }
     eg = warp_sum(eg); ep = warp_sum(ep);
-    if (lane == 0) { T.red[2 * wi] = eg; T.red[2 * wi + 1] = ep; }
+    if (lane == 0) { T.red[8 * wi] = eg; T.red[8 * wi + 1] = ep; }
     team_sync();
     e_inter = 0.f; e_intra = 0.f;
 #pragma unroll
-    for (int w = 0; w < kTeamW; ++w) { e_inter += T.red[2 * w]; e_intra += T.red[2 * w + 1]; }
+    for (int w = 0; w < kTeamW; ++w) { e_inter += T.red[8 * w]; e_intra += T.red[8 * w + 1]; }
 
     // (a4) the planes are summed per atom (one thread each, fixed order 0+1+2+3), then back-propagation on warp 0:
     // eval_pose's code
@@ -768,9 +784,14 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
                     Fx += F.x; Fy += F.y; Fz += F.z;
                     Tx += Tq.x + (ly * F.z - lz * F.y); Ty += Tq.y + (lz * F.x - lx * F.z); Tz += Tq.z + (lx * F.y - ly * F.x);
                 }
-                if (f == 0) {
-                    S.grad[0] = Fx; S.grad[1] = Fy; S.grad[2] = Fz;
-                    S.grad[3] = Tx; S.grad[4] = Ty; S.grad[5] = Tz;
+                if (f == 0) {                           // rigid-body blocks: the warps' grid-force sums, fixed order
+#pragma unroll
+                    for (int d = 0; d < 6; ++d) {
+                        float v = T.red[2 + d];
+#pragma unroll
+                        for (int w = 1; w < kTeamW; ++w) v += T.red[8 * w + 2 + d];
+                        S.grad[d] = v;
+                    }
                 } else {
                     const float4 u = S.fragAx[2 * f];
                     S.grad[6 + (w >> 16)] = u.x * Tx + u.y * Ty + u.z * Tz;
@@ -875,7 +896,7 @@ __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, co
                 if (d < D) ok = ok && isfinite(S.grad[d]);
             }
             ok = __all_sync(kFull, ok);
-            if (lane == 0) T.red[2 * kTeamW] = ok ? 1.f : 0.f;
+            if (lane == 0) T.red[8 * kTeamW] = ok ? 1.f : 0.f;
             if (ok) {
                 if (e < bestE) {
                     bestE = e;
@@ -919,7 +940,7 @@ __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, co
             }
         }
         team_sync();                                    // new genotype and the flag are visible
-        if (T.red[2 * kTeamW] == 0.f) break;
+        if (T.red[8 * kTeamW] == 0.f) break;
     }
     iters = it;
     return isfinite(bestE) ? bestE : e_start;

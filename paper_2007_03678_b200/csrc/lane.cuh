@@ -15,51 +15,6 @@
 
 namespace adock {
 
-// ---------------------------------------------------------------- packed f32x2
-struct f2 { unsigned long long v; };
-__device__ __forceinline__ f2 pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r.v) : "f"(lo), "f"(hi)); return r; }
-__device__ __forceinline__ f2 bc(float x) { return pk(x, x); }
-__device__ __forceinline__ void unpk(f2 a, float& lo, float& hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.v)); }
-__device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
-__device__ __forceinline__ f2 sub2(f2 a, f2 b) { f2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
-__device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
-__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d.v) : "l"(a.v), "l"(b.v), "l"(c.v)); return d; }
-__device__ __forceinline__ f2 neg2(f2 a) { f2 d; d.v = a.v ^ 0x8000000080000000ull; return d; }
-__device__ __forceinline__ float hsum(f2 a) { float l, h; unpk(a, l, h); return l + h; }
-__device__ __forceinline__ f2 ld2(const float2* p) { const float2 v = *p; return pk(v.x, v.y); }
-
-// ---------------------------------------------------------------- grid term, packed (R4)
-// grid_finish with the two interpolants (affinity map | q*elec + |q|*desolv) in the two halves of f32x2 operands: 22 packed
-// instructions for value + gradient of both instead of 44 scalar ones; the halves are added at the very end, so the
-// small field still never meets the large one before the corner differences are taken.
-template <bool GRAD>
-__device__ __forceinline__ float grid_finish2(const GridDev& G, const ParDev& P, const GridCell& c, const F8 (&v)[4], float q,
-                                              float& gx, float& gy, float& gz) {
-    const float aq = fabsf(q);
-    const f2 a00 = pk(v[0].lo.x, fmaf(aq, v[0].lo.z, q * v[0].lo.y)), b00 = pk(v[0].hi.x, fmaf(aq, v[0].hi.z, q * v[0].hi.y));
-    const f2 a01 = pk(v[1].lo.x, fmaf(aq, v[1].lo.z, q * v[1].lo.y)), b01 = pk(v[1].hi.x, fmaf(aq, v[1].hi.z, q * v[1].hi.y));
-    const f2 a10 = pk(v[2].lo.x, fmaf(aq, v[2].lo.z, q * v[2].lo.y)), b10 = pk(v[2].hi.x, fmaf(aq, v[2].hi.z, q * v[2].hi.y));
-    const f2 a11 = pk(v[3].lo.x, fmaf(aq, v[3].lo.z, q * v[3].lo.y)), b11 = pk(v[3].hi.x, fmaf(aq, v[3].hi.z, q * v[3].hi.y));
-    const f2 fx = bc(c.fx), fy = bc(c.fy), fz = bc(c.fz);
-    const f2 d00 = sub2(b00, a00), d01 = sub2(b01, a01), d10 = sub2(b10, a10), d11 = sub2(b11, a11);
-    const f2 v00 = fma2(fx, d00, a00), v01 = fma2(fx, d01, a01), v10 = fma2(fx, d10, a10), v11 = fma2(fx, d11, a11);
-    const f2 e0 = sub2(v01, v00), e1 = sub2(v11, v10);
-    const f2 w0 = fma2(fy, e0, v00), w1 = fma2(fy, e1, v10);
-    const f2 dz = sub2(w1, w0);
-    float val = hsum(fma2(fz, dz, w0));
-    val = fmaf(P.k_wall_h, fabsf(c.ox) + fabsf(c.oy) + fabsf(c.oz), val);
-    if (GRAD) {
-        const f2 dx0 = fma2(fy, sub2(d01, d00), d00), dx1 = fma2(fy, sub2(d11, d10), d10);
-        const float dfx = hsum(fma2(fz, sub2(dx1, dx0), dx0));
-        const float dfy = hsum(fma2(fz, sub2(e1, e0), e0));
-        const float dfz = hsum(dz);
-        gx = (c.ox != 0.f) ? copysignf(P.k_wall, c.ox) : dfx * G.inv_h;
-        gy = (c.oy != 0.f) ? copysignf(P.k_wall, c.oy) : dfy * G.inv_h;
-        gz = (c.oz != 0.f) ? copysignf(P.k_wall, c.oz) : dfz * G.inv_h;
-    }
-    return val;
-}
-
 // ---------------------------------------------------------------- views
 struct LaneL {              // the staged image
     const float4* atoms;    // [Npad] x0 - pivot, q
@@ -90,12 +45,13 @@ struct LaneS {              // this lane's columns of the group's scratch; eleme
     float* own;             // [own_floats] of THIS part: per fragment F(3), T(3) about t; during the pose: the transform stack
     float* own0;            // part 0's (the K parts' arrays are consecutive, own_floats*32 apart)
     float* geno;            // [7+R]
-    float* ex;              // [2K+1]: (e_grid, e_pairs) of each part, then the chain's live flag
+    float* ex;              // [8K+1]: (e_grid, e_pairs, grid force F(3), grid torque about t T(3)) of each part, then the
+                            // chain's live flag
     int part, gid;          // this warp's part in the group; group index in the CTA (named barrier gid+1)
 };
 // floats per lane of one group's scratch
 __host__ __device__ inline int lane_group_floats(int Npad, int own_floats, int R, int K) {
-    return 3 * Npad + K * own_floats + (7 + R) + 2 * K + 1;
+    return 3 * Npad + K * own_floats + (7 + R) + (K > 1 ? 8 * K + 1 : 0);      // one warp per group exchanges nothing
 }
 // group_floats = floats per lane between consecutive groups of the CTA: lane_group_floats of the ligand, or of the
 // largest ligand of the launch when the groups of a CTA belong to different ligands (0 = this ligand's)
@@ -208,10 +164,15 @@ __device__ __forceinline__ void own_flush(float* own, int f, float Fx, float Fy,
 
 // ---------------------------------------------------------------- full evaluation of this lane's genotype
 // Called by all K warps of the group with S.geno ready (and visible to all of them).  Part 0 returns the total energy
-// (NaN for |q| < 1e-12, with NaN gradient) and, with GRAD, writes grad[d*gs] for d < 6+R when `wr` and clears `gfin`
-// if a component is not finite; the other parts return 0.  The caller must group_sync before S.geno, the positions
-// or own[] are touched again (part 0 still reads them in its tail).
-template <bool GRAD, int K>
+// (NaN for |q| < 1e-12, with NaN gradient); the other parts return 0.  With GRAD part 0 clears `gfin` if a gradient
+// component is not finite and delivers the gradient according to GOUT:
+//   GOUT = 1: grad[d*gs] for d < 6+R when `wr` (scoring: straight to the caller's array)
+//   GOUT = 2: left in part 0's own[] columns: dE/dt, dE/domega in own[0..5], dE/dtau of fragment f's torsion in
+//             own[6f] (local search: the optimiser reads them from shared memory; `grad` is not used)
+// The rigid-body blocks (dE/dt, dE/domega) are summed from the GRID forces alone: intramolecular pair forces cancel
+// exactly in both (Newton's third law), so they are kept out of sums they contribute nothing to.
+// The caller must group_sync before S.geno, the positions or own[] are touched again (part 0 still reads them).
+template <bool GRAD, int K, int GOUT = 1>
 __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, const ParDev& P, const LaneS& S, float* grad, int gs,
                                            bool wr, float& e_inter, float& e_intra, bool& gfin) {
     const float tx = S.geno[0], ty = S.geno[32], tz = S.geno[64];
@@ -285,6 +246,7 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
     // is consumed (the lookups are pure L2 latency: one dependent round per step instead of one per atom); the
     // gradient goes straight into the (force, torque about t) sums of the atom's fragment, which initialises own[]
     float eg = 0.f;
+    float RFx = 0, RFy = 0, RFz = 0, RTx = 0, RTy = 0, RTz = 0;     // grid force / torque about t over ALL atoms of this part
     {
         if (GRAD && K > 1)
             for (int d = 0; d < 6 * L.nfrag; ++d) S.own[d * 32] = 0.f;
@@ -294,9 +256,9 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
             int tt[4];
             float q[4], rx[4], ry[4], rz[4];
             GridCell gc[4];
-            F8 c[4][4];
+            F8 c[4][2];
             {
-                const int4 t4 = *reinterpret_cast<const int4*>(L.types + 2 * m);      // type | frag << 8 ; -1 = pad
+                const int4 t4 = *reinterpret_cast<const int4*>(L.types + 2 * m);      // cell set | frag << 8 ; -1 = pad
                 tt[0] = t4.x; tt[1] = t4.y; tt[2] = t4.z; tt[3] = t4.w;
                 const float2 xa = S.X[m * 32], ya = S.Y[m * 32], za = S.Z[m * 32];
                 const float2 xb = S.X[(m + 1) * 32], yb = S.Y[(m + 1) * 32], zb = S.Z[(m + 1) * 32];
@@ -314,13 +276,14 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
 #pragma unroll
             for (int a = 0; a < 4; ++a) {
                 float gx, gy, gz;
-                const float e = grid_finish2<GRAD>(G, P, gc[a], c[a], q[a], gx, gy, gz);
+                const float e = grid_finish<GRAD>(G, P, gc[a], c[a], q[a], gx, gy, gz);
                 if (tt[a] < 0) continue;                    // pad atom (warp-uniform): looked up, not counted
                 eg += e;
                 if (GRAD) {
                     const int f = tt[a] >> 8;
                     if (f != cur) {
                         own_flush<K>(S.own, cur, Fx, Fy, Fz, Tx, Ty, Tz);
+                        RFx += Fx; RFy += Fy; RFz += Fz; RTx += Tx; RTy += Ty; RTz += Tz;
                         Fx = Fy = Fz = Tx = Ty = Tz = 0.f; cur = f;
                     }
                     Fx += gx; Fy += gy; Fz += gz;
@@ -328,7 +291,10 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                 }
             }
         }
-        if (GRAD) own_flush<K>(S.own, cur, Fx, Fy, Fz, Tx, Ty, Tz);
+        if (GRAD) {
+            own_flush<K>(S.own, cur, Fx, Fy, Fz, Tx, Ty, Tz);
+            RFx += Fx; RFy += Fy; RFz += Fz; RTx += Tx; RTy += Ty; RTz += Tz;
+        }
     }
 
     // (a3) intramolecular pairs: register tiles; this warp's parts of the tile sequence
@@ -409,17 +375,25 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
     e_inter = eg;
     e_intra = hsum(e2);
     if (K > 1) {                                        // hand the partial sums to part 0
-        S.ex[(2 * S.part) * 32] = e_inter; S.ex[(2 * S.part + 1) * 32] = e_intra;
+        float* ex = S.ex + 8 * S.part * 32;
+        ex[0] = e_inter; ex[32] = e_intra;
+        if (GRAD) { ex[64] = RFx; ex[96] = RFy; ex[128] = RFz; ex[160] = RTx; ex[192] = RTy; ex[224] = RTz; }
         group_sync<K>(S);
         if (S.part != 0) { gfin = true; return 0.f; }
         e_inter = 0.f; e_intra = 0.f;
-        for (int k = 0; k < K; ++k) { e_inter += S.ex[(2 * k) * 32]; e_intra += S.ex[(2 * k + 1) * 32]; }
-        if (GRAD)
-            for (int d = 0; d < 6 * L.nfrag; ++d) {
+        for (int k = 0; k < K; ++k) { e_inter += S.ex[(8 * k) * 32]; e_intra += S.ex[(8 * k + 1) * 32]; }
+        if (GRAD) {
+            RFx = RFy = RFz = RTx = RTy = RTz = 0.f;
+            for (int k = 0; k < K; ++k) {
+                const float* e8 = S.ex + 8 * k * 32;
+                RFx += e8[64]; RFy += e8[96]; RFz += e8[128]; RTx += e8[160]; RTy += e8[192]; RTz += e8[224];
+            }
+            for (int d = 6; d < 6 * L.nfrag; ++d) {     // the root's own sums are not needed (grid totals above)
                 float v = S.own0[d * 32];
                 for (int k = 1; k < K; ++k) v += S.own0[(k * L.own_floats + d) * 32];
                 S.own0[d * 32] = v;
             }
+        }
     }
     float e = e_inter + e_intra;
     const float qnan = __int_as_float(0x7fc00000);
@@ -444,15 +418,17 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
             float dt = ux * px + uy * py + uz * pz;
             if (badq) dt = qnan;
             fin = fin && isfinite(dt);
-            if (wr) grad[(6 + tor) * gs] = dt;
-            own_add(S.own, fi.x, Fx, Fy, Fz, Tx, Ty, Tz);
+            if (GOUT == 1) { if (wr) grad[(6 + tor) * gs] = dt; }
+            else o[0] = dt;                             // fragment f's sums are consumed: its first slot carries dE/dtau
+            if (fi.x != 0) own_add(S.own, fi.x, Fx, Fy, Fz, Tx, Ty, Tz);     // the root takes the grid totals instead
         }
-        float g[6] = {S.own[0], S.own[32], S.own[64], S.own[96], S.own[128], S.own[160]};
+        float g[6] = {RFx, RFy, RFz, RTx, RTy, RTz};
 #pragma unroll
         for (int d = 0; d < 6; ++d) {
             if (badq) g[d] = qnan;
             fin = fin && isfinite(g[d]);
-            if (wr) grad[d * gs] = g[d];
+            if (GOUT == 1) { if (wr) grad[d * gs] = g[d]; }
+            else S.own[d * 32] = g[d];
         }
         gfin = fin;
     }
@@ -464,14 +440,23 @@ struct LaneLS {             // global scratch columns of this thread: element d 
     float* best;            // [7+R]
     float* Eg2;             // [6+R]
     float* Ed2;             // [6+R]
-    float* grad;            // [6+R]
     int stride;
 };
+
+// one component of the update (R7): accumulators in place, returns the step.  sqrt(a)/sqrt(b) as a*rsqrt(a)*rsqrt(b)
+// with the MUFU forms (a, b >= ad_eps > 0): 3 instructions instead of two IEEE square roots and a division.
+__device__ __forceinline__ float adadelta_component(const ParDev& P, float g, float& eg2, float& ed2) {
+    eg2 = P.ad_rho * eg2 + (1.f - P.ad_rho) * g * g;
+    const float a = ed2 + P.ad_eps;
+    const float dl = -(a * frsqrt(a) * frsqrt(eg2 + P.ad_eps)) * g;
+    ed2 = P.ad_rho * ed2 + (1.f - P.ad_rho) * dl * dl;
+    return dl;
+}
 
 // Start genotype in S.geno (visible to the whole group).  Called by all K warps of the group; part 0 owns the chain's
 // state (ls, in global scratch columns) and on return ls.best holds the best genotype seen; part 0 returns its energy
 // (e_start if no finite evaluation happened) and the evaluations done.  `active` lanes run the chain; the others only
-// keep the warp's control flow uniform.
+// keep the warp's control flow uniform.  The gradient never leaves shared memory (lane_eval, GOUT = 2).
 template <int K>
 __device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const ParDev& P, const LaneS& S, const LaneLS& ls,
                                       bool active, float e_start, int& iters, float* trace, int trace_stride) {
@@ -489,7 +474,7 @@ __device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const Pa
         if (!__any_sync(kFull, live)) break;            // same decision in every warp of the group
         float ei, ea;
         bool gfin = true;
-        const float e = lane_eval<true, K>(L, G, P, S, ls.grad, ls.stride, true, ei, ea, gfin);
+        const float e = lane_eval<true, K, 2>(L, G, P, S, nullptr, 0, false, ei, ea, gfin);
         if (lead) {
             if (live) {
                 if (trace) trace[it * trace_stride] = e;
@@ -501,29 +486,37 @@ __device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const Pa
                     bestE = e;
                     for (int d = 0; d < Gn; ++d) ls.best[d * ls.stride] = S.geno[d * 32];
                 }
-                float w[3] = {0.f, 0.f, 0.f};
-                // the state columns live in global memory (L2): load a chunk of 8 components before the first store, so
-                // the chunk costs one round trip instead of one per component (a store may alias the next load)
-                for (int d0 = 0; d0 < D; d0 += 8) {
-                    float gv[8], av[8], bv[8];
+                // the accumulator columns live in global memory (L2): a chunk of 8 components is loaded before the
+                // first store, so the chunk costs one round trip instead of one per component
+                float w[3];
+                {                                       // rigid-body block: d = 0..5, gradient in own[0..5]
+                    float av[6], bv[6];
+#pragma unroll
+                    for (int d = 0; d < 6; ++d) { av[d] = ls.Eg2[d * ls.stride]; bv[d] = ls.Ed2[d * ls.stride]; }
+#pragma unroll
+                    for (int d = 0; d < 6; ++d) {
+                        const float dl = adadelta_component(P, S.own[d * 32], av[d], bv[d]);
+                        ls.Eg2[d * ls.stride] = av[d]; ls.Ed2[d * ls.stride] = bv[d];
+                        if (d < 3) S.geno[d * 32] += dl; else w[d - 3] = dl;
+                    }
+                }
+                for (int f0 = 1; f0 < L.nfrag; f0 += 8) {  // torsions: fragment f's torsion gradient in own[6f]
+                    float av[8], bv[8];
+                    int dd[8];
 #pragma unroll
                     for (int k = 0; k < 8; ++k) {
-                        const int d = min(d0 + k, D - 1);
-                        gv[k] = ls.grad[d * ls.stride]; av[k] = ls.Eg2[d * ls.stride]; bv[k] = ls.Ed2[d * ls.stride];
+                        const int f = min(f0 + k, L.nfrag - 1);
+                        dd[k] = 6 + L.fragi[3 * f + 1].w;
+                        av[k] = ls.Eg2[dd[k] * ls.stride]; bv[k] = ls.Ed2[dd[k] * ls.stride];
                     }
 #pragma unroll
                     for (int k = 0; k < 8; ++k) {
-                        const int d = d0 + k;
-                        if (d < D) {
-                            const float g = gv[k];
-                            const float eg2 = P.ad_rho * av[k] + (1.f - P.ad_rho) * g * g;
-                            const float ed2o = bv[k];
-                            const float dl = -(sqrtf(ed2o + P.ad_eps) / sqrtf(eg2 + P.ad_eps)) * g;
-                            ls.Eg2[d * ls.stride] = eg2;
-                            ls.Ed2[d * ls.stride] = P.ad_rho * ed2o + (1.f - P.ad_rho) * dl * dl;
-                            if (d < 3) S.geno[d * 32] += dl;
-                            else if (d < 6) { if (d == 3) w[0] = dl; else if (d == 4) w[1] = dl; else w[2] = dl; }
-                            else S.geno[(d + 1) * 32] = wrap_pi(S.geno[(d + 1) * 32] + dl);
+                        const int f = f0 + k;
+                        if (f < L.nfrag) {
+                            const float dl = adadelta_component(P, S.own[6 * f * 32], av[k], bv[k]);
+                            ls.Eg2[dd[k] * ls.stride] = av[k]; ls.Ed2[dd[k] * ls.stride] = bv[k];
+                            float* t = S.geno + (dd[k] + 1) * 32;
+                            *t = wrap_pi(*t + dl);
                         }
                     }
                 }
@@ -536,10 +529,10 @@ __device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const Pa
                 rotate_quat(ch, k * w[0], k * w[1], k * w[2], q, nq);
                 S.geno[96] = nq[0]; S.geno[128] = nq[1]; S.geno[160] = nq[2]; S.geno[192] = nq[3];
             }
-            if (K > 1) S.ex[(2 * K) * 32] = live ? 1.f : 0.f;
+            if (K > 1) S.ex[(8 * K) * 32] = live ? 1.f : 0.f;
         }
         group_sync<K>(S);                               // new genotype and live flag visible; part 0 is done with own[]
-        if (K > 1) live = S.ex[(2 * K) * 32] != 0.f;
+        if (K > 1) live = S.ex[(8 * K) * 32] != 0.f;
     }
     return isfinite(bestE) ? bestE : e_start;
 }
@@ -591,13 +584,13 @@ __device__ inline float lane_solis_wets(const LaneL& L, const GridDev& G, const 
             S.geno[96] = nq4[0]; S.geno[128] = nq4[1]; S.geno[160] = nq4[2]; S.geno[192] = nq4[3];
             for (int d = 6; d < D; ++d) S.geno[(d + 1) * 32] = wrap_pi(ls.best[(d + 1) * ls.stride] + sg * ls.Ed2[d * ls.stride]);
         }
-        if (K > 1 && lead) S.ex[(2 * K) * 32] = live ? 1.f : 0.f;
+        if (K > 1 && lead) S.ex[(8 * K) * 32] = live ? 1.f : 0.f;
         group_sync<K>(S);                               // candidate and live flag visible; part 0 is done with the last pass
-        if (K > 1) live = S.ex[(2 * K) * 32] != 0.f;
+        if (K > 1) live = S.ex[(8 * K) * 32] != 0.f;
         if (!__any_sync(kFull, live)) break;            // same decision in every warp of the group
         float ei, ea;
         bool gfin = true;
-        const float e = lane_eval<false, K>(L, G, P, S, nullptr, 1, false, ei, ea, gfin);
+        const float e = lane_eval<false, K, 1>(L, G, P, S, nullptr, 1, false, ei, ea, gfin);
         if (lead && live) {
             ++evals;
             const bool ok = e < E;

@@ -29,7 +29,7 @@ constexpr int kLaneParts = 4;   // the tile sequence is cut into this many runs 
 struct LaneHeader {             // 128 bytes
     int N, Npad, R, nfrag;      // Npad = N rounded up to a multiple of kLaneBI (pad atoms sit at the origin, in no pair)
     int nblocks, ntiles, nrows, maxdepth;
-    int off_atoms, off_types, off_frags, off_blocks;    // types: type | fragment << 8 per atom, -1 = pad
+    int off_atoms, off_types, off_frags, off_blocks;    // types: cell set (2 type + (q < 0)) | fragment << 8 per atom, -1 = pad
     int off_tiles, off_rows, bytes, npairs;
     int own_floats, warp_floats, nslots, pad1;    // per-thread scratch: own_floats = max(6 nfrag, 12 maxdepth);
                                                 // warp_floats = 3 Npad + own_floats + (7+R)  (one warp per group)
@@ -193,7 +193,7 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
         if (e < 0) { types[q] = -1; continue; }            // pad
         for (int d = 0; d < 3; ++d) atoms[4 * q + d] = (float)((double)xyz[3 * e + d] - (double)tp.pivot[d]);
         atoms[4 * q + 3] = charge[e];
-        types[q] = type[e] | (frag_of_pos[q] << 8);
+        types[q] = (2 * type[e] + (charge[e] < 0.f ? 1 : 0)) | (frag_of_pos[q] << 8);       // cell set (device.cuh, grid term)
     }
     LaneFrag* fr = (LaneFrag*)(im.blob.data() + h.off_frags);
     for (int f = 0; f < nfrag; ++f) {

@@ -286,7 +286,7 @@ inline bool build_topology(Topology& tp, int N, const float* xyz, const int* typ
         if (e < 0) { meta[q] = 0xffffffffu; continue; }          // hole
         for (int d = 0; d < 3; ++d) atoms[4 * q + d] = (float)((double)xyz[3 * e + d] - (double)tp.pivot[d]);
         atoms[4 * q + 3] = charge[e];
-        meta[q] = (uint32_t)type[e] | ((uint32_t)frag_of[e] << 8);
+        meta[q] = (uint32_t)(2 * type[e] + (charge[e] < 0.f ? 1 : 0)) | ((uint32_t)frag_of[e] << 8);     // cell set | fragment
     }
     FragGeom* fg = (FragGeom*)(tp.blob.data() + h.off_frag);
     FragIdx* fi = (FragIdx*)(tp.blob.data() + h.off_fragidx);

@@ -90,21 +90,34 @@ def assert_energy(E, ref, what=""):
     assert len(bad) == 0, f"{what}: {len(bad)} energies off, worst {np.abs(E - ref)[bad].max()} at {bad[:5]} ref {ref[bad[:5]]}"
 
 
-def assert_gradient(g, ref, R, ok, what=""):
-    """ref: the oracle's score() dict (grad, scales)"""
+def assert_gradient(g, ref, R, ok, what="", plain_only=False):
+    """ref: the oracle's score() dict (grad, scales).
+    Rule 1 (SURVEY C10 as written; BASELINE.json "gradients within 1e-3 relative"): per block b in {t, omega, tau}
+        ||d_b|| <= 1e-3 * max(||g_b||, 1e-2 ||g||) + 1e-4.
+    Rule 2 (R10, clash poses only): ||d_b|| <= 1e-3 ||g_b|| + 1e-5 S_b + 1e-4, S_b = the oracle's `scales`
+        (fp32 cancellation floor of sums whose terms exceed the result by orders of magnitude).
+    plain_only: every pose must meet rule 1 (non-clashing workload).  Otherwise a pose may fall back to rule 2; the
+    fraction of poses that needed it is returned (and printed by the callers)."""
     g = g.astype(np.float64)
     rg, sc = ref["grad"], ref["scales"]
-    worst = 0.0
+    gall = np.linalg.norm(rg, axis=1)
+    need_floor = np.zeros(len(rg), bool)
     for b, (lo, hi) in enumerate(((0, 3), (3, 6), (6, 6 + R))):
         if hi == lo:
             continue
         d = np.linalg.norm(g[:, lo:hi] - rg[:, lo:hi], axis=1)
-        tol = 1e-3 * np.linalg.norm(rg[:, lo:hi], axis=1) + 1e-5 * sc[:, b] + 1e-4
-        bad = np.flatnonzero(ok & ~(d <= tol))
-        assert len(bad) == 0, f"{what}: block [{lo},{hi}) off for {len(bad)} poses, e.g. {bad[:5]}: {d[bad[:5]]} > {tol[bad[:5]]}"
-        if ok.any():
-            worst = max(worst, float((d / tol)[ok].max()))
-    return worst
+        gb = np.linalg.norm(rg[:, lo:hi], axis=1)
+        plain = 1e-3 * np.maximum(gb, 1e-2 * gall) + 1e-4
+        floor = 1e-3 * gb + 1e-5 * sc[:, b] + 1e-4
+        over = ok & ~(d <= plain)
+        if plain_only:
+            bad = np.flatnonzero(over)
+            assert len(bad) == 0, f"{what}: block [{lo},{hi}) off (plain rule) for {len(bad)} poses, e.g. {bad[:5]}: {d[bad[:5]]} > {plain[bad[:5]]}"
+        else:
+            bad = np.flatnonzero(over & ~(d <= floor))
+            assert len(bad) == 0, f"{what}: block [{lo},{hi}) off for {len(bad)} poses, e.g. {bad[:5]}: {d[bad[:5]]} > {floor[bad[:5]]}"
+            need_floor |= over
+    return float(need_floor[ok].mean()) if ok.any() else 0.0
 
 
 # ------------------------------------------------------------------------------- integer structure on the device path
@@ -123,6 +136,13 @@ def test_score_parity(B, orc, W, cases, dev, family, name, n):
     c = cases(name)
     G = W.make_genotypes(n, c.lig.R, c.grids, seed=100 + n)
     ref = orc.score(c.og, c.ol, c.op, G)
+    if name == "sweep128" and family in ("lane2", "lane4"):
+        # two or four warps per group do not fit 128 atoms (137 KB image + per-lane state): a forced family that
+        # cannot be honoured is an error, never a silent substitute
+        with pytest.raises(B.AdockError) as e:
+            gpu_score(B, c, G, dev)
+        assert e.value.code == B.ADOCK_ELIMIT
+        return
     E, terms, gr = gpu_score(B, c, G, dev)
     assert_energy(E, ref["E"], name)
     assert_energy(terms[:, 0], ref["terms"][:, 0], name + " inter")
@@ -131,7 +151,8 @@ def test_score_parity(B, orc, W, cases, dev, family, name, n):
     # an atom lies within 1e-3 of a cell face on some axis with probability ~6e-3: exp(-6e-3 N) of the poses stay
     assert ok.mean() > 0.6 * math.exp(-6e-3 * c.lig.N)
     w = assert_gradient(gr, ref, c.lig.R, ok, name)
-    print(f"{name}: worst gradient error / tolerance = {w:.3f}")
+    print(f"{name} [{family}]: {100 * w:.2f} % of the poses need the S_b floor of R10 (the rest meet the plain 1e-3 rule)")
+    assert w < 0.05
     # energy-only launch gives the same energies
     E2, _, _ = gpu_score(B, c, G, dev, grad=False)
     assert_energy(E2, ref["E"], name + " energy-only")
@@ -190,7 +211,7 @@ def test_score_affine_field_is_exact_property(B, orc, W, dev):
     coef = [[1.5, -2.0, 0.25, 3.0], [0.5, 1.0, -1.0, 0.0], [-4.0, 0.5, 2.0, 1.0], [9, 9, 9, 9], [7, 7, 7, 7]]
     grids = W.make_affine_grids(64, T, coef)
     lig = W.make_ligand(20, 4, T, seed=3, centre=0.5 * (grids.box_lo + grids.box_hi))
-    lig.charge[:] = 0; lig.pair_coeffs[:] = 0; lig.solpar[:] = 0
+    lig.charge[:] = 0; lig.pair_coeffs[..., :2] = 0; lig.solpar[:] = 0
     c = Case(B, orc, W, grids, lig)
     G = W.make_genotypes(4096, lig.R, grids, seed=1, wall_tail=0.0)
     E, _, gr = gpu_score(B, c, G, dev)
@@ -214,6 +235,137 @@ def test_score_full_size_sampled(B, orc, W, cases, dev):
     # launching twice gives bit-identical results (fixed reduction order, no float atomics)
     E2, _, gr2 = gpu_score(B, c, G, dev)
     assert np.array_equal(E, E2) and np.array_equal(gr, gr2)
+
+
+# ------------------------------------------------------------------------------- non-clashing workload, isolated terms
+@pytest.fixture(scope="module")
+def pocket(B, orc, W):
+    """DESIGN.md section 4, non-clashing workload: 40 atoms / 8 torsions / 7 types with atoms four or more bonds apart
+    kept >= 3.6 A apart, 64^3 maps whose carved pocket (11.5 A) fits the ligand, poses near the input conformation:
+    energies O(100) kcal/mol, like a real complex, instead of 1e6 clashes."""
+    grids = W.make_grids(64, 7, 600, 11.5, seed=21)
+    lig = W.make_ligand(40, 8, 7, seed=11, centre=0.5 * (grids.box_lo + grids.box_hi), far_sep=3.6, max_deg=3)
+    G = W.make_pocket_genotypes(2000, lig.R, grids, seed=5, sigma_t=0.7, sigma_tau=0.2)
+    # keep the poses the ORACLE calls non-clashing (a torsion kick now and then swings two branches into each other)
+    ref = orc.score(orc.Grids.from_workload(grids), orc.Ligand.from_workload(lig), orc.params(W.DEFAULT_PARAMS), G, want_grad=False)
+    keep = (np.abs(ref["E"]) < 1e3) & (np.abs(ref["terms"][:, 1]) < 50.0)
+    assert keep.mean() > 0.9
+    return grids, lig, G[keep]
+
+
+def test_score_parity_nonclashing_plain_tolerance(B, orc, W, pocket, dev, family):
+    """BASELINE.json north_star as written: energies 1e-4 relative or 1e-3 absolute, gradients 1e-3 relative
+    (no S_b term), on every pose."""
+    grids, lig, G = pocket
+    c = Case(B, orc, W, grids, lig)
+    ref = orc.score(c.og, c.ol, c.op, G)
+    assert np.median(np.abs(ref["E"])) < 1e3 and np.abs(ref["terms"][:, 1]).max() < 50.0        # non-clashing indeed
+    E, terms, gr = gpu_score(B, c, G, dev)
+    assert_energy(E, ref["E"], "pocket")
+    assert_energy(terms[:, 0], ref["terms"][:, 0], "pocket inter")
+    assert_energy(terms[:, 1], ref["terms"][:, 1], "pocket intra")
+    ok = ref["margins"][:, 0] > 1e-3
+    assert ok.mean() > 0.7
+    assert_gradient(gr, ref, lig.R, ok, "pocket", plain_only=True)
+
+
+def _variant(W, grids, lig, name):
+    """one term of the energy function at a time (van der Waals, hydrogen bond, electrostatics,
+    desolvation; line 116: the three map kinds).  Returns (grids, ligand, parameter overrides)."""
+    import dataclasses
+    maps = grids.maps.copy()
+    T = lig.T
+    pc0 = np.zeros_like(lig.pair_coeffs); pc0[..., 2] = lig.pair_coeffs[..., 2]       # keep the exponents valid
+    if name == "pair_elec_desolv":          # intra = electrostatics + desolvation
+        return grids, dataclasses.replace(lig, pair_coeffs=pc0), {}
+    if name == "pair_elec":
+        return grids, dataclasses.replace(lig, pair_coeffs=pc0), dict(w_desolv=0.0)
+    if name == "pair_desolv":
+        return grids, dataclasses.replace(lig, pair_coeffs=pc0), dict(elec_scale=0.0)
+    if name == "vdw_hbond":                 # no charges; most pairs of the 12-10 type pair (T-1, T-2)
+        ty = np.where(np.arange(lig.N) % 2 == 0, T - 1, T - 2).astype(np.int32)
+        ty[::7] = 0
+        return grids, dataclasses.replace(lig, type=ty, charge=np.zeros_like(lig.charge)), {}
+    if name == "grid_elec":                 # affinity and desolvation maps zeroed: q * map T alone
+        maps[:T] = 0; maps[T + 1] = 0
+    elif name == "grid_desolv":             # |q| * map T+1 alone
+        maps[:T + 1] = 0
+    elif name == "grid_affinity":           # type maps alone
+        maps[T:] = 0
+    else:
+        raise KeyError(name)
+    return dataclasses.replace(grids, maps=maps), dataclasses.replace(lig, pair_coeffs=pc0), dict(elec_scale=0.0, w_desolv=0.0)
+
+
+@pytest.mark.parametrize("variant", ["pair_elec_desolv", "pair_elec", "pair_desolv", "vdw_hbond", "grid_elec", "grid_desolv",
+                                     "grid_affinity"])
+@pytest.mark.parametrize("fam", ["warp", "lane1", "lane2"])
+def test_score_terms_in_isolation(B, orc, W, pocket, dev, fam, variant):
+    grids, lig, G = pocket
+    g2, l2, over = _variant(W, grids, lig, variant)
+    c = Case(B, orc, W, g2, l2, over)
+    G = G[:600]
+    ref = orc.score(c.og, c.ol, c.op, G)
+    if variant.startswith("grid"):
+        assert (ref["terms"][:, 1] == 0).all() and np.abs(ref["terms"][:, 0]).max() > 0
+    if variant == "vdw_hbond":
+        hb = (l2.type[c.ol.pairs[:, 0]] + l2.type[c.ol.pairs[:, 1]]) == 2 * l2.T - 3
+        assert hb.mean() > 0.3
+    B.adock_set_path(fam)
+    try:
+        E, terms, gr = gpu_score(B, c, G, dev)
+    finally:
+        B.adock_set_path("auto")
+    assert_energy(E, ref["E"], variant)
+    assert_energy(terms[:, 0], ref["terms"][:, 0], variant + " inter")
+    assert_energy(terms[:, 1], ref["terms"][:, 1], variant + " intra")
+    assert_gradient(gr, ref, l2.R, ref["margins"][:, 0] > 1e-3, variant, plain_only=True)
+
+
+# ------------------------------------------------------------------------------- configs[3]: large ligand, 126^3 x 10 maps
+@pytest.fixture(scope="module")
+def large(B, orc, W):
+    grids, lig = W.make_config("large")
+    assert grids.dims == (126, 126, 126) and grids.M == 10 and lig.N == 128 and lig.R == 32
+    return Case(B, orc, W, grids, lig, dict(lsit=40))
+
+
+@pytest.mark.parametrize("fam", ["auto", "warp", "lane1"])
+def test_large_config_score_parity(B, orc, W, large, dev, fam):
+    """BASELINE.json configs[3] on its real grid (126^3 x 10 maps; 40 A blind-docking box; Table 2
+    line 178: more than 10 torsions): sampled poses against the oracle, energies, both terms and gradients."""
+    c = large
+    n = 4096
+    G = W.make_genotypes(n, c.lig.R, c.grids, seed=33)
+    B.adock_set_path(fam)
+    try:
+        E, terms, gr = gpu_score(B, c, G, dev)
+    finally:
+        B.adock_set_path("auto")
+    idx = np.random.default_rng(3).choice(n, 256, replace=False)
+    ref = orc.score(c.og, c.ol, c.op, G[idx])
+    assert_energy(E[idx], ref["E"], "large")
+    assert_energy(terms[idx, 0], ref["terms"][:, 0], "large inter")
+    assert_energy(terms[idx, 1], ref["terms"][:, 1], "large intra")
+    ok = (ref["margins"][:, 0] > 1e-3) & (ref["margins"][:, 1] > 1e-3)
+    w = assert_gradient(gr[idx], ref, c.lig.R, ok, "large")
+    print(f"large [{fam}]: {100 * w:.2f} % of the sampled poses need the S_b floor")
+
+
+def test_large_config_short_docking(B, orc, large):
+    """a short LGA docking of the large ligand (50 runs x pop 150 as in configs[3], a few generations): accounting,
+    and the reported energies are the oracle's energies of the reported genotypes."""
+    c = large
+    nrun, P, lsit, gens = 50, 150, 40, 3
+    max_evals = P + gens * ((P - 1) + 9 * lsit)
+    r = B.adock_dock(c.gg, c.gl, c.gp, nrun, P, max_evals, seed=9)
+    assert (r["gens"] == gens).all() and (r["evals"] == max_evals).all()
+    chk = orc.score(c.og, c.ol, c.op, r["genotypes"], want_grad=False)["E"]
+    assert_energy(r["energies"], chk, "large dock result")
+    x = c.ol.pose(r["genotypes"][0].astype(np.float64))
+    assert np.abs(x - r["coords"][0]).max() < 5e-4
+    e0 = orc.score(c.og, c.ol, c.op, orc.ga_init(c.og, c.lig.R, 9, 0, P).astype(np.float32), want_grad=False)["E"].min()
+    assert r["energies"][0] <= e0 + 1e-3 * abs(e0)                  # the elite never gets worse than generation 0's best
 
 
 # ------------------------------------------------------------------------------- Philox (R8)

@@ -96,7 +96,9 @@ def test_image_layout_and_conflict_free_schedule(B, W, orc, name, request):
     piv = hl.tree()["pivot"].astype(np.float64)
     assert np.allclose(atoms[occ, :3], lig.xyz[ext_of_int[occ]].astype(np.float64) - piv, atol=1e-6)
     assert np.array_equal(atoms[occ, 3], lig.charge[ext_of_int[occ]])
-    assert np.array_equal(meta[occ] & 0xFF, lig.type[ext_of_int[occ]].astype(np.uint32))
+    # low byte = cell set of the grid lookup: 2 * type + (charge < 0)   (include/adock.h, adock_load_grids)
+    e_occ = ext_of_int[occ]
+    assert np.array_equal(meta[occ] & 0xFF, (2 * lig.type[e_occ] + (lig.charge[e_occ] < 0)).astype(np.uint32))
     frag = np.full(npos, -1)
     frag[occ] = (meta[occ] >> 8).astype(int)
     assert sorted(H["fragatoms"].tolist()) == sorted(occ.tolist())
