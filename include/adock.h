@@ -113,8 +113,9 @@ int adock_ligand_lane_image(const adock_ligand* l, int* bytes, const unsigned ch
 
 /* Kernel family used by the compute entry points of this process: 0 = chosen by problem
  * size (default), 1 = one warp per individual, 2 = one lane per individual with K = 1, 2 or 4 warps sharing the
- * work of each group of 32 individuals (K chosen by size; 21, 22, 24 force K = 1, 2, 4; a forced K whose per-lane state
- * does not fit in shared memory for a ligand makes the compute calls return ADOCK_ELIMIT).  All of them compute
+ * work of each group of 32 individuals (variant chosen by size; 21, 22, 24 force K = 1, 2, 4 with the atom positions in
+ * shared memory; 41, 42, 43 force K = 1 with the atom positions in tensor memory and at most 8, 12, 16 warps per SM; a
+ * forced variant whose per-lane state does not fit for a ligand makes the compute calls return ADOCK_ELIMIT).  All of them compute
  * the same function (R3-R7) and pass the same parity tests; they differ in summation order only.
  * 3 = the ADADELTA chains of adock_dock / adock_dock_many each run on a team (one CTA of 4 warps per individual,
  * threads over atoms and pairs), chosen by size when a launch holds too few chains to give every scheduler a warp

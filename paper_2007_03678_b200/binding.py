@@ -341,12 +341,13 @@ def adock_profile_read() -> dict:
     return dict(ls_ms=ms.value, ls_launches=n.value, ls_evals=ev.value)
 
 
-PATHS = {"auto": 0, "warp": 1, "lane": 2, "lane1": 21, "lane2": 22, "lane4": 24, "team": 3}
+PATHS = {"auto": 0, "warp": 1, "lane": 2, "lane1": 21, "lane2": 22, "lane4": 24, "tm8": 41, "tm12": 42, "tm16": 43, "team": 3}
 
 
 def adock_set_path(path) -> None:
     """kernel family: 'auto' (by problem size), 'warp' (warp per individual), 'lane' (lane per individual, warps per
-    group of 32 individuals chosen by size), 'lane1' / 'lane2' / 'lane4' (that number of warps per group) or 'team' (the
+    group of 32 individuals chosen by size), 'lane1' / 'lane2' / 'lane4' (that number of warps per group), 'tm8' / 'tm12' /
+    'tm16' (one warp per group, atom positions in tensor memory, at most that many warps per SM) or 'team' (the
     docking's ADADELTA chains each run on a CTA of 4 warps; everything else as 'warp')"""
     _check(lib().adock_set_path(PATHS[path] if isinstance(path, str) else int(path)))
 

@@ -43,7 +43,7 @@ struct adock_ligand {
 static thread_local std::string g_err;
 static thread_local long long g_launches = 0;
 static int g_path = 0;                                    // adock_set_path: 0 auto, 1 warp per individual, 2 lane per individual
-static int g_lane_k = 0;                                  // warps per lane group forced by adock_set_path(21|22|24); 0 = by size
+static int g_lane_var = -1;                               // lane-kernel variant forced by adock_set_path(21|22|24|41|42|43); -1 = by size
 static thread_local bool g_prof = false;                  // adock_profile: time every dock_ls_kernel launch
 static thread_local double g_ls_ms = 0;
 static thread_local long long g_ls_launches = 0, g_ls_evals = 0;
@@ -98,6 +98,7 @@ static ParDev make_pardev(const adock_params& p) {
     d.elec_sqrt = (float)std::sqrt((double)p.elec_scale); d.diel_A = p.diel_A; d.diel_B = p.diel_B; d.diel_k = p.diel_k;
     d.BlamB = (float)((double)p.diel_B * (double)p.diel_lambda * (double)p.diel_B);
     d.mlamB_log2e = (float)(-(double)p.diel_lambda * (double)p.diel_B * log2e);
+    d.log2_dk = (float)std::log2((double)p.diel_k);
     d.inv_sig2 = (float)(1.0 / ((double)p.ds_sigma * (double)p.ds_sigma));
     d.mhalf_inv_sig2_log2e = (float)(-0.5 * log2e / ((double)p.ds_sigma * (double)p.ds_sigma));
     d.rmin2 = p.r_min * p.r_min; d.k_wall = p.k_wall; d.k_wall_h = 0.f;    // k_wall_h set per grid
@@ -116,7 +117,8 @@ static int check_params(const adock_params* in, const adock_ligand* l, adock_par
     const float* f = &out.elec_scale;
     for (int i = 0; i < 18; ++i)
         if (!std::isfinite(f[i])) return fail(ADOCK_EINVAL, "non-finite parameter");
-    if (!(out.ds_sigma > 0) || !(out.r_min > 0) || !(out.elec_scale >= 0) || out.lsit < 0 || out.max_gens < 0 || !(out.ad_eps > 0))
+    if (!(out.ds_sigma > 0) || !(out.r_min > 0) || !(out.elec_scale >= 0) || out.lsit < 0 || out.max_gens < 0 || !(out.ad_eps > 0) ||
+        !(out.diel_k > 0))      // k <= 0 puts a pole into eps(r); the kernels evaluate k exp(-lambda B r) as 2^(.. + log2 k)
         return fail(ADOCK_EINVAL, "parameter out of range");
     const float* f2 = &out.sw_rho0;
     for (int i = 0; i < 7; ++i)
@@ -299,9 +301,12 @@ extern "C" int adock_ligand_lane_image(const adock_ligand* l, int* bytes, const 
 extern "C" int adock_last_dock_path(void) { return g_last_dock_path; }
 
 extern "C" int adock_set_path(int path) {
-    if (path == 21 || path == 22 || path == 24) { g_path = 2; g_lane_k = path - 20; return ADOCK_OK; }
-    if (path < 0 || path > 3) return fail(ADOCK_EINVAL, "path must be 0 (auto), 1 (warp per individual), 2 (lane per individual), 21/22/24 or 3 (team per individual)");
-    g_path = path; g_lane_k = 0;
+    if (path == 21 || path == 22 || path == 24) { g_path = 2; g_lane_var = path == 21 ? 0 : path == 22 ? 1 : 2; return ADOCK_OK; }
+    if (path == 41 || path == 42 || path == 43) { g_path = 2; g_lane_var = path - 38; return ADOCK_OK; }
+    if (path < 0 || path > 3)
+        return fail(ADOCK_EINVAL, "path must be 0 (auto), 1 (warp per individual), 2 (lane per individual), 21/22/24 (1, 2, 4 warps per group, "
+                                  "positions in shared memory), 41/42/43 (positions in tensor memory, 8/12/16 warps per SM) or 3 (team per individual)");
+    g_path = path; g_lane_var = -1;
     return ADOCK_OK;
 }
 
@@ -359,35 +364,62 @@ __global__ void __launch_bounds__(256) score_kernel(GridDev G, ParDev P, ScoreAr
 
 
 // =================================================================== lane-per-individual geometry (lane.cuh)
-// A group of K warps shares 32 individuals.  Warps per CTA are bounded by the register file: 8 (K=1, 255 registers per
-// thread), 12 (K=2, 170), 16 (K=4, 128), and by the shared memory of the groups.
-template <int K> struct LaneCfg { static constexpr int kMaxWarps = K == 1 ? 8 : K == 2 ? 12 : 16; };
-static int lane_max_warps(int K) { return K == 1 ? 8 : K == 2 ? 12 : 16; }
+// A group of K warps shares 32 individuals.  A variant of the lane kernels fixes K, the most warps per CTA W (the register
+// budget is 64 K / (32 W) per thread: 255 at 8 warps, 168 at 12, 128 at 16) and where the atom positions live: shared
+// memory, or tensor memory (TM; one warp per group only), which takes 62 % of the per-lane state of a 40-atom ligand out
+// of shared memory so that 12 or 16 warps fit where 8 did.
+template <int K_, int W_, bool TM_> struct LaneCfg {
+    static constexpr int K = K_, kMaxWarps = W_;
+    static constexpr bool TM = TM_;
+};
+struct LaneVar { int K, W; bool TM; double eff; };        // eff: measured throughput per SM at full residency, K = 1 / 8 warps = 1
+constexpr int kNumLaneVars = 6;
+static const LaneVar kLaneVars[kNumLaneVars] = {{1, 8, false, 1.0}, {2, 12, false, 0.95}, {4, 16, false, 0.85},
+                                                {1, 8, true, 1.0},  {1, 12, true, 1.0},   {1, 16, true, 1.0}};
+#define LANE_VARIANT(v, ...)                                                      \
+    switch (v) {                                                                  \
+        case 0: { using C = LaneCfg<1, 8, false>; __VA_ARGS__; } break;           \
+        case 1: { using C = LaneCfg<2, 12, false>; __VA_ARGS__; } break;          \
+        case 2: { using C = LaneCfg<4, 16, false>; __VA_ARGS__; } break;          \
+        case 3: { using C = LaneCfg<1, 8, true>; __VA_ARGS__; } break;            \
+        case 4: { using C = LaneCfg<1, 12, true>; __VA_ARGS__; } break;           \
+        default: { using C = LaneCfg<1, 16, true>; __VA_ARGS__; } break;          \
+    }
 struct LaneGeom { int bytes, npad, own, R; };            // of the largest ligand of a launch
 static LaneGeom lane_geom(const adock_ligand* l) { return LaneGeom{l->lane_bytes, l->lane_npad, l->lane_own, l->tp.R}; }
 static LaneGeom lane_geom_max(LaneGeom a, LaneGeom b) {
     return LaneGeom{std::max(a.bytes, b.bytes), std::max(a.npad, b.npad), std::max(a.own, b.own), std::max(a.R, b.R)};
 }
-static size_t lane_smem(const LaneGeom& g, int K, int groups) {
-    return 16 + (size_t)g.bytes + (size_t)groups * lane_group_floats(g.npad, g.own, g.R, K) * 128;
+static int lane_var_floats(const LaneGeom& g, int v) { return lane_group_floats(g.npad, g.own, g.R, kLaneVars[v].K, kLaneVars[v].TM); }
+// shared memory of a CTA of `groups` groups with `nimg` image slots
+static size_t lane_smem(const LaneGeom& g, int v, int groups, int nimg = 1) {
+    const size_t slot = ((size_t)g.bytes + 127) & ~(size_t)127;
+    return 16 + (size_t)nimg * slot + (size_t)groups * lane_var_floats(g, v) * 128;
+}
+static bool lane_fits(const LaneGeom& g, int v, int groups, int nimg = 1) {
+    if (kLaneVars[v].TM && 3 * g.npad > lane_tmem_columns(groups * kLaneVars[v].K)) return false;
+    return lane_smem(g, v, groups, nimg) <= (size_t)g_smem_optin;
 }
 // most groups per CTA that fit (0: not even one)
-static int lane_fit_groups(const LaneGeom& g, int K) {
-    int n = lane_max_warps(K) / K;
-    while (n > 0 && lane_smem(g, K, n) > (size_t)g_smem_optin) --n;
+static int lane_fit_groups(const LaneGeom& g, int v) {
+    int n = kLaneVars[v].W / kLaneVars[v].K;
+    while (n > 0 && !lane_fits(g, v, n)) --n;
     return n;
 }
 // the lane kernels want at least one warp per scheduler
 static bool lane_ok(const adock_ligand* l) {
     const LaneGeom g = lane_geom(l);
-    return lane_fit_groups(g, 1) >= 4 || lane_fit_groups(g, 2) >= 2 || lane_fit_groups(g, 4) >= 1;
+    for (int v = 0; v < kNumLaneVars; ++v)
+        if (lane_fit_groups(g, v) * kLaneVars[v].K >= 4) return true;
+    return false;
 }
 // ADADELTA chains (threads) from which the lane-per-individual kernels are preferred over warp-per-individual
-constexpr int kLaneMinChains = 148 * 64;     // measured cross-over on the drug config: between 32 and 64 ligands x 180 chains
+static long long lane_min_chains() { return (long long)g_sm_count * 64; }     // measured cross-over on the drug config: between 32 and 64 ligands x 180 chains
 // ---- launch plan of a lane-per-individual kernel over `total` groups of 32 individuals, `jg` consecutive groups per
 // ligand image (jg >= total: one image).  CTA b takes groups [b*ng, (b+1)*ng) and stages every image they touch.
 struct LanePlan {
-    int K = 0;              // warps per group (0: nothing fits)
+    int var = -1;           // variant (-1: nothing fits)
+    int K = 0;              // its warps per group
     int ng = 0;             // groups per CTA
     int nctas = 0;
     int nimg = 1;           // image slots per CTA
@@ -405,42 +437,37 @@ static int lane_plan_images(long long total, int jg, int ng) {        // most im
     }
     return worst;
 }
-static size_t lane_plan_smem(const LaneGeom& g, int K, int ng, int nimg) {
-    const size_t slot = ((size_t)g.bytes + 127) & ~(size_t)127;
-    return 16 + (size_t)nimg * slot + (size_t)ng * lane_group_floats(g.npad, g.own, g.R, K) * 128;
-}
-// Measured on sweep40 / drug (profiles/r01c_lane_plan.md): with enough groups K = 1 at 8 warps per SM is the fastest
-// (5.0e8 evals/s), K = 2 at 12 warps 0.95x, K = 4 at 16 warps 0.85x; K = 2 at 8 warps only 0.7x; with few groups per SM
-// the extra warps of K = 2, 4 win.  Model: an SM with w resident warps works at min(w, cap_K)/cap_K of its rate
-// (cap = the most warps of that K: 8, 12, 16), times the efficiency of K; waves of CTAs run one after another.
+// Model: an SM with w resident warps of a variant works at min(w, W)/W of the variant's rate eff (measured per SM at
+// full residency: profiles/r02_lane_variants.md); waves of CTAs run one after another.
 static LanePlan lane_plan(const LaneGeom& g, long long total, int jg) {
     LanePlan best;
     double best_t = 1e300;
     if (total < 1) total = 1;
     if (jg < 1) jg = 1;
-    for (int K = 1; K <= 4; K *= 2) {
-        if (g_lane_k && K != g_lane_k) continue;                // a forced K that does not fit is an error (ADOCK_ELIMIT), never a silent substitute
-        const double eff = K == 1 ? 1.0 : K == 2 ? 0.95 : 0.85;
-        for (int ng = lane_max_warps(K) / K; ng >= 1; --ng) {
-            if (lane_plan_smem(g, K, ng, lane_plan_images(total, jg, ng)) > (size_t)g_smem_optin) continue;
+    for (int v = 0; v < kNumLaneVars; ++v) {
+        if (g_lane_var >= 0 && v != g_lane_var) continue;       // a forced variant that does not fit is an error (ADOCK_ELIMIT), never a silent substitute
+        const LaneVar& V = kLaneVars[v];
+        for (int ng = V.W / V.K; ng >= 1; --ng) {
+            if (!lane_fits(g, v, ng, lane_plan_images(total, jg, ng))) continue;
             const long long nctas = (total + ng - 1) / ng, waves = (nctas + g_sm_count - 1) / g_sm_count;
-            const double t = (double)waves * ng / (eff * (double)(ng * K) / lane_max_warps(K));
+            const double t = (double)waves * ng / (V.eff * (double)(ng * V.K) / V.W);
             if (t < best_t * 0.999) {
                 best_t = t;
-                best.K = K; best.ng = ng;
+                best.var = v; best.ng = ng;
             }
         }
     }
-    if (!best.K) return best;
+    if (best.var < 0) return best;
+    best.K = kLaneVars[best.var].K;
     best.nctas = (int)((total + best.ng - 1) / best.ng);
     best.nimg = lane_plan_images(total, jg, best.ng);
     best.slot = (g.bytes + 127) & ~127;
-    best.gfloats = lane_group_floats(g.npad, g.own, g.R, best.K);
-    best.smem = lane_plan_smem(g, best.K, best.ng, best.nimg);
+    best.gfloats = lane_var_floats(g, best.var);
+    best.smem = lane_smem(g, best.var, best.ng, best.nimg);
     return best;
 }
-// warps per group for `ngroups` groups of 32 individuals of one ligand
-static int lane_pick_k(const LaneGeom& g, long long ngroups) { return lane_plan(g, ngroups, (int)std::min<long long>(ngroups, 1 << 30)).K; }
+// variant for `ngroups` groups of 32 individuals of one ligand (-1: none fits)
+static int lane_pick_var(const LaneGeom& g, long long ngroups) { return lane_plan(g, ngroups, (int)std::min<long long>(ngroups, 1 << 30)).var; }
 // groups per CTA: as many as fit, fewer when that would leave SMs idle
 static int lane_spread_groups(int fit, long long ngroups) {
     int n = fit;
@@ -448,14 +475,16 @@ static int lane_spread_groups(int fit, long long ngroups) {
     return n;
 }
 
-template <bool GRAD, int K>
-__global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) score_lane_kernel(GridDev G, ParDev P, ScoreArgs a) {
+template <bool GRAD, class C>
+__global__ void __launch_bounds__(C::kMaxWarps * 32, 1) score_lane_kernel(GridDev G, ParDev P, ScoreArgs a) {
+    constexpr int K = C::K;
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char* blob = smem + 16;
     stage_ligand(blob, a.blob, a.blob_bytes, reinterpret_cast<uint64_t*>(smem), 0);
+    const uint32_t tmem = lane_tmem_open<C::TM>(smem);
     const LaneL L = lane_view(blob);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, NG = (blockDim.x >> 5) / K;
-    const LaneS S = lane_scratch<K>(reinterpret_cast<float*>(blob + a.blob_bytes), L, warp, lane);
+    const LaneS S = lane_scratch<K, C::TM>(reinterpret_cast<float*>(blob + a.blob_bytes), L, warp, lane, 0, tmem);
     const int Gn = 7 + L.R;
     const int nchunks = (a.n + 31) >> 5;
     for (int c = blockIdx.x * NG + S.gid; c < nchunks; c += gridDim.x * NG) {
@@ -467,24 +496,25 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) score_lane_kern
         group_sync<K>(S);
         float ei, ea;
         bool gf;
-        const float e = lane_eval<GRAD, K>(L, G, P, S, GRAD ? a.grads + (size_t)src * a.dstride : nullptr, 1, act, ei, ea, gf);
+        const float e = lane_eval<GRAD, K, 1, C::TM>(L, G, P, S, GRAD ? a.grads + (size_t)src * a.dstride : nullptr, 1, act, ei, ea, gf);
         if (act && S.part == 0) {
             a.E[idx] = e;
             if (a.terms) { a.terms[2 * (size_t)idx] = ei; a.terms[2 * (size_t)idx + 1] = ea; }
         }
         group_sync<K>(S);                               // part 0 is done with the positions and own[]
     }
+    lane_tmem_close<C::TM>(tmem);
 }
 
-template <bool GRAD, int K>
-static int launch_score_lane_k(const adock_grids* grids, const adock_ligand* lig, const ParDev& P, const ScoreArgs& a, int ngroups,
+template <bool GRAD, class C>
+static int launch_score_lane_k(const adock_grids* grids, const adock_ligand* lig, const ParDev& P, const ScoreArgs& a, int var, int ngroups,
                                cudaStream_t st) {
     const LaneGeom g = lane_geom(lig);
-    const int NG = lane_spread_groups(lane_fit_groups(g, K), ngroups);
-    const size_t smem = lane_smem(g, K, NG);
+    const int NG = lane_spread_groups(lane_fit_groups(g, var), ngroups);
+    const size_t smem = lane_smem(g, var, NG);
     const int grid = (int)std::max<long long>(1, std::min<long long>(((long long)ngroups + NG - 1) / NG, g_sm_count));
-    CUDA_TRY(cudaFuncSetAttribute(score_lane_kernel<GRAD, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    score_lane_kernel<GRAD, K><<<grid, NG * K * 32, smem, st>>>(grids->dev, P, a);
+    CUDA_TRY(cudaFuncSetAttribute(score_lane_kernel<GRAD, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    score_lane_kernel<GRAD, C><<<grid, NG * C::K * 32, smem, st>>>(grids->dev, P, a);
     ++g_launches;
     CUDA_TRY(cudaGetLastError());
     return ADOCK_OK;
@@ -493,19 +523,15 @@ static int launch_score_lane_k(const adock_grids* grids, const adock_ligand* lig
 static int launch_score_lane(const adock_grids* grids, const adock_ligand* lig, const adock_params& p, const float* d_genos, int n,
                              int gstride, float* d_E, float* d_terms, float* d_grads, int dstride, cudaStream_t st) {
     const int ngroups = (n + 31) / 32;
-    const int K = lane_pick_k(lane_geom(lig), ngroups);
-    if (!K) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
+    const int var = lane_pick_var(lane_geom(lig), ngroups);
+    if (var < 0) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
     ParDev P = make_pardev(p);
     P.k_wall_h = p.k_wall * grids->dev.h;
     ScoreArgs a{lig->d_lane, d_genos, d_E, d_terms, d_grads, lig->lane_bytes, n, gstride, dstride};
-    if (d_grads) {
-        if (K == 1) return launch_score_lane_k<true, 1>(grids, lig, P, a, ngroups, st);
-        if (K == 2) return launch_score_lane_k<true, 2>(grids, lig, P, a, ngroups, st);
-        return launch_score_lane_k<true, 4>(grids, lig, P, a, ngroups, st);
-    }
-    if (K == 1) return launch_score_lane_k<false, 1>(grids, lig, P, a, ngroups, st);
-    if (K == 2) return launch_score_lane_k<false, 2>(grids, lig, P, a, ngroups, st);
-    return launch_score_lane_k<false, 4>(grids, lig, P, a, ngroups, st);
+    int rc = ADOCK_OK;
+    if (d_grads) { LANE_VARIANT(var, rc = launch_score_lane_k<true, C>(grids, lig, P, a, var, ngroups, st)) }
+    else { LANE_VARIANT(var, rc = launch_score_lane_k<false, C>(grids, lig, P, a, var, ngroups, st)) }
+    return rc;
 }
 
 static int launch_score(const adock_grids* grids, const adock_ligand* lig, const adock_params& p, const float* d_genos, int n,
@@ -630,14 +656,16 @@ __global__ void __launch_bounds__(128) ls_array_kernel(GridDev G, ParDev P, LsAr
 
 // lane-per-individual variant: lane c of the launch's groups runs chain c; ADADELTA state in global scratch columns
 // [row][all group lanes of the launch]
-template <int K, bool SW>
-__global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) ls_array_lane_kernel(GridDev G, ParDev P, LsArgs a, float* __restrict__ scratch) {
+template <class C, bool SW>
+__global__ void __launch_bounds__(C::kMaxWarps * 32, 1) ls_array_lane_kernel(GridDev G, ParDev P, LsArgs a, float* __restrict__ scratch) {
+    constexpr int K = C::K;
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char* blob = smem + 16;
     stage_ligand(blob, a.blob, a.blob_bytes, reinterpret_cast<uint64_t*>(smem), 0);
+    const uint32_t tmem = lane_tmem_open<C::TM>(smem);
     const LaneL L = lane_view(blob);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, NG = (blockDim.x >> 5) / K;
-    const LaneS S = lane_scratch<K>(reinterpret_cast<float*>(blob + a.blob_bytes), L, warp, lane);
+    const LaneS S = lane_scratch<K, C::TM>(reinterpret_cast<float*>(blob + a.blob_bytes), L, warp, lane, 0, tmem);
     const int Gn = 7 + L.R, D = 6 + L.R;
     const size_t tid = ((size_t)blockIdx.x * NG + S.gid) * 32 + lane, T = (size_t)gridDim.x * NG * 32;
     const bool act = tid < (size_t)a.n;
@@ -650,30 +678,31 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) ls_array_lane_k
     ls.stride = (int)T;
     int iters = 0;
     float* tr = a.trace ? a.trace + idx * P.lsit : nullptr;
-    const float e = SW ? lane_solis_wets<K>(L, G, P, S, ls, act, (act && S.part == 0) ? a.E[idx] : 0.f, a.seed, (uint32_t)idx, a.gen, iters, tr, 1)
-                       : lane_adadelta<K>(L, G, P, S, ls, act, __int_as_float(0x7fc00000), iters, tr, 1);
+    const float e = SW ? lane_solis_wets<K, C::TM>(L, G, P, S, ls, act, (act && S.part == 0) ? a.E[idx] : 0.f, a.seed, (uint32_t)idx, a.gen, iters, tr, 1)
+                       : lane_adadelta<K, C::TM>(L, G, P, S, ls, act, __int_as_float(0x7fc00000), iters, tr, 1);
     if (act && S.part == 0) {
         for (int d = 0; d < Gn; ++d) a.genos[idx * a.gstride + d] = ls.best[(size_t)d * T];
         a.E[idx] = e;
         if (a.iters) a.iters[idx] = iters;
     }
+    lane_tmem_close<C::TM>(tmem);
 }
 
-template <int K, bool SW>
-static int launch_ls_array_lane(const adock_grids* grids, const adock_ligand* ligand, const ParDev& P, LsArgs a, int n, cudaStream_t stm) {
+template <class C, bool SW>
+static int launch_ls_array_lane(const adock_grids* grids, const adock_ligand* ligand, const ParDev& P, LsArgs a, int var, int n, cudaStream_t stm) {
     const LaneGeom g = lane_geom(ligand);
     const int ngroups = (n + 31) / 32;
-    const int NG = lane_spread_groups(lane_fit_groups(g, K), ngroups);
+    const int NG = lane_spread_groups(lane_fit_groups(g, var), ngroups);
     const int grid = (ngroups + NG - 1) / NG;
-    const size_t smem = lane_smem(g, K, NG);
+    const size_t smem = lane_smem(g, var, NG);
     const size_t T = (size_t)grid * NG * 32;
     const int R = ligand->tp.R;
     float* scratch = nullptr;
     cudaError_t e = cudaMallocAsync(&scratch, T * (size_t)(7 + R + 2 * (6 + R)) * 4, stm);
     if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("ls scratch: ") + cudaGetErrorString(e));
-    e = cudaFuncSetAttribute(ls_array_lane_kernel<K, SW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    e = cudaFuncSetAttribute(ls_array_lane_kernel<C, SW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) {
-        ls_array_lane_kernel<K, SW><<<grid, NG * K * 32, smem, stm>>>(grids->dev, P, a, scratch);
+        ls_array_lane_kernel<C, SW><<<grid, NG * C::K * 32, smem, stm>>>(grids->dev, P, a, scratch);
         ++g_launches;
         e = cudaGetLastError();
     }
@@ -696,21 +725,16 @@ static int local_search_impl(const adock_grids* grids, const adock_ligand* ligan
     p.ls_method = method;
     rc = device_props();
     if (rc) return rc;
-    if (g_path == 2 || (g_path == 0 && n >= kLaneMinChains && lane_ok(ligand))) {
-        const int K = lane_pick_k(lane_geom(ligand), (n + 31) / 32);
-        if (!K) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
+    if (g_path == 2 || (g_path == 0 && n >= lane_min_chains() && lane_ok(ligand))) {
+        const int var = lane_pick_var(lane_geom(ligand), (n + 31) / 32);
+        if (var < 0) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
         ParDev P = make_pardev(p);
         P.k_wall_h = p.k_wall * grids->dev.h;
         LsArgs a{ligand->d_lane, d_genotypes, d_energies, d_iters, d_trace, ligand->lane_bytes, n, gstride, seed, gen};
         cudaStream_t stm = (cudaStream_t)cuda_stream;
-        if (method == 1) {
-            if (K == 1) return launch_ls_array_lane<1, true>(grids, ligand, P, a, n, stm);
-            if (K == 2) return launch_ls_array_lane<2, true>(grids, ligand, P, a, n, stm);
-            return launch_ls_array_lane<4, true>(grids, ligand, P, a, n, stm);
-        }
-        if (K == 1) return launch_ls_array_lane<1, false>(grids, ligand, P, a, n, stm);
-        if (K == 2) return launch_ls_array_lane<2, false>(grids, ligand, P, a, n, stm);
-        return launch_ls_array_lane<4, false>(grids, ligand, P, a, n, stm);
+        if (method == 1) { LANE_VARIANT(var, rc = launch_ls_array_lane<C, true>(grids, ligand, P, a, var, n, stm)) }
+        else { LANE_VARIANT(var, rc = launch_ls_array_lane<C, false>(grids, ligand, P, a, var, n, stm)) }
+        return rc;
     }
     const int W = fit_warps(ligand->blob_bytes, ligand->scratch_floats, 4);
     if (!W) return fail(ADOCK_ELIMIT, "ligand does not fit in shared memory");
@@ -958,16 +982,14 @@ __device__ __forceinline__ LaneCtaGroup lane_cta_group(unsigned char* smem, cons
 
 // ADADELTA on the selected individuals (Lamarckian write-back): lane c of a job's groups runs chain c = run*n_ls + l;
 // ADADELTA state in global scratch columns [row][all group lanes of the launch] (rows: Gmax best, 2 x Dmax)
-template <int K, bool SW>
-__global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_ls_lane_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs,
-                                                                                     DockDims dm, LaneDockArgs a) {
-    extern __shared__ __align__(128) unsigned char smem[];
-    const LaneCtaGroup cg = lane_cta_group<K>(smem, jobs, a);
-    if (!cg.valid) return;                              // whole groups leave: the named barriers are per group
+template <class C, bool SW>
+__device__ __forceinline__ void dock_ls_lane_group(const GridDev& G, const ParDev& P, const DockJob* __restrict__ jobs, const DockDims& dm,
+                                                   const LaneDockArgs& a, const LaneCtaGroup& cg, uint32_t tmem) {
+    constexpr int K = C::K;
     const DockJob job = jobs[cg.jidx];
     const LaneL L = lane_view(cg.blob);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const LaneS S = lane_scratch<K>(cg.scratch, L, warp, lane, a.group_floats);
+    const LaneS S = lane_scratch<K, C::TM>(cg.scratch, L, warp, lane, a.group_floats, tmem);
     const int Gn = job.Gn;
     const int c = cg.gi * 32 + lane;
     bool act = c < job.act[0] * dm.n_ls;
@@ -990,27 +1012,34 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_ls_lane_ke
     ls.stride = (int)T;
     int iters = 0;
     const float e0 = (act && S.part == 0) ? *e : 0.f;
-    const float be = SW ? lane_solis_wets<K>(L, G, P, S, ls, act, e0, job.seed, (uint32_t)(run * dm.P + slot), (uint32_t)st.gen + 1u, iters, nullptr, 0)
-                        : lane_adadelta<K>(L, G, P, S, ls, act, e0, iters, nullptr, 0);
+    const float be = SW ? lane_solis_wets<K, C::TM>(L, G, P, S, ls, act, e0, job.seed, (uint32_t)(run * dm.P + slot), (uint32_t)st.gen + 1u, iters, nullptr, 0)
+                        : lane_adadelta<K, C::TM>(L, G, P, S, ls, act, e0, iters, nullptr, 0);
     if (act && S.part == 0) {
         for (int d = 0; d < Gn; ++d) g[d] = ls.best[(size_t)d * T];
         *e = be;
         atomicAdd(&job.st[run].ls_acc, iters);
     }
 }
+template <class C, bool SW>
+__global__ void __launch_bounds__(C::kMaxWarps * 32, 1) dock_ls_lane_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs, DockDims dm,
+                                                                            LaneDockArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const LaneCtaGroup cg = lane_cta_group<C::K>(smem, jobs, a);
+    const uint32_t tmem = lane_tmem_open<C::TM>(smem);
+    if (cg.valid) dock_ls_lane_group<C, SW>(G, P, jobs, dm, a, cg, tmem);     // whole groups skip: the named barriers are per group
+    lane_tmem_close<C::TM>(tmem);
+}
 
 // energies of the offspring written by dock_ga_kernel<false> (slot 0, the elite, carries its energy): lane c of a
 // job's groups scores individual c = run*P + slot of the new population
-template <int K>
-__global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_score_lane_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs,
-                                                                                        DockDims dm, LaneDockArgs a) {
-    extern __shared__ __align__(128) unsigned char smem[];
-    const LaneCtaGroup cg = lane_cta_group<K>(smem, jobs, a);
-    if (!cg.valid) return;
+template <class C>
+__device__ __forceinline__ void dock_score_lane_group(const GridDev& G, const ParDev& P, const DockJob* __restrict__ jobs, const DockDims& dm,
+                                                      const LaneDockArgs& a, const LaneCtaGroup& cg, uint32_t tmem) {
+    constexpr int K = C::K;
     const DockJob job = jobs[cg.jidx];
     const LaneL L = lane_view(cg.blob);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const LaneS S = lane_scratch<K>(cg.scratch, L, warp, lane, a.group_floats);
+    const LaneS S = lane_scratch<K, C::TM>(cg.scratch, L, warp, lane, a.group_floats, tmem);
     const int Gn = job.Gn;
     const int c = cg.gi * 32 + lane, n = job.act[0] * dm.P;
     bool act = c < n;
@@ -1027,8 +1056,17 @@ __global__ void __launch_bounds__(LaneCfg<K>::kMaxWarps * 32, 1) dock_score_lane
     group_sync<K>(S);
     float ei, ea;
     bool gf;
-    const float e = lane_eval<false, K>(L, G, P, S, nullptr, 1, false, ei, ea, gf);
+    const float e = lane_eval<false, K, 1, C::TM>(L, G, P, S, nullptr, 1, false, ei, ea, gf);
     if (act && S.part == 0) job.E[(size_t)(st.cur ^ 1) * popsz + cc] = e;
+}
+template <class C>
+__global__ void __launch_bounds__(C::kMaxWarps * 32, 1) dock_score_lane_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs, DockDims dm,
+                                                                               LaneDockArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const LaneCtaGroup cg = lane_cta_group<C::K>(smem, jobs, a);
+    const uint32_t tmem = lane_tmem_open<C::TM>(smem);
+    if (cg.valid) dock_score_lane_group<C>(G, P, jobs, dm, a, cg, tmem);
+    lane_tmem_close<C::TM>(tmem);
 }
 
 // end of generation: eval accounting, buffer flip, termination test
@@ -1169,9 +1207,9 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     const LanePlan pl = lane_plan(lg, (long long)nlig * jg, jg);
     // Solis-Wets chains end after very different numbers of evaluations (28 to lsit iterations), which leaves most lanes
     // of a lane-per-chain warp idle; one warp per chain is 2x faster there (profiles/r01d_next_rows.md)
-    const bool many = g_path == 0 && lanes_fit && chains >= kLaneMinChains;
-    const bool ls_lane = pl.K > 0 && (g_path == 2 || (many && p.ls_method == 0));
-    if (g_path == 2 && !pl.K) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
+    const bool many = g_path == 0 && lanes_fit && chains >= lane_min_chains();
+    const bool ls_lane = pl.var >= 0 && (g_path == 2 || (many && p.ls_method == 0));
+    if (g_path == 2 && pl.var < 0) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
     // a team (CTA of kTeamW warps) per chain when one warp per chain would leave most schedulers without a warp
     const size_t smem_team = 16 + (size_t)maxblob + (size_t)maxteam * 4;
     const bool ls_team = !ls_lane && p.ls_method == 0 && smem_team <= (size_t)g_smem_optin &&
@@ -1180,7 +1218,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     // offspring scoring: lane-per-individual under the same condition (populations are 1/lsrat times larger)
     const int jgs = (int)(((long long)nrun * Pn + 31) / 32);
     const LanePlan ps = lane_plan(lg, (long long)nlig * jgs, jgs);
-    const bool ga_lane = ps.K > 0 && (g_path == 2 || many);
+    const bool ga_lane = ps.var >= 0 && (g_path == 2 || many);
     ParDev P = make_pardev(p);
     P.k_wall_h = p.k_wall * grids->dev.h;
     DockDims dm{};
@@ -1269,29 +1307,23 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         cudaError_t e2 = buf.alloc(&d_lscratch, T * (size_t)(Gmax + 2 * (Gmax - 1)) * 4);
         if (e2 != cudaSuccess) return fail(e2 == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("dock alloc: ") + cudaGetErrorString(e2));
         al = LaneDockArgs{d_lscratch, Gmax, pl.ng, nlig * jg, jg, pl.slot, pl.nimg, pl.gfloats};
-        if (pl.K == 1) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-        if (pl.K == 2) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-        if (pl.K == 4) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-        if (pl.K == 1) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-        if (pl.K == 2) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-        if (pl.K == 4) CUDA_TRY(cudaFuncSetAttribute(dock_ls_lane_kernel<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        cudaError_t e3 = cudaSuccess;
+        LANE_VARIANT(pl.var, e3 = cudaFuncSetAttribute(dock_ls_lane_kernel<C, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+                     if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(dock_ls_lane_kernel<C, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem))
+        CUDA_TRY(e3);
     }
     if (ga_lane) {
         as = LaneDockArgs{nullptr, Gmax, ps.ng, nlig * jgs, jgs, ps.slot, ps.nimg, ps.gfloats};
-        if (ps.K == 1) CUDA_TRY(cudaFuncSetAttribute(dock_score_lane_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps.smem));
-        if (ps.K == 2) CUDA_TRY(cudaFuncSetAttribute(dock_score_lane_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps.smem));
-        if (ps.K == 4) CUDA_TRY(cudaFuncSetAttribute(dock_score_lane_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps.smem));
+        cudaError_t e3 = cudaSuccess;
+        LANE_VARIANT(ps.var, e3 = cudaFuncSetAttribute(dock_score_lane_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ps.smem))
+        CUDA_TRY(e3);
         CUDA_TRY(cudaFuncSetAttribute(dock_ga_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ga));
     }
     auto launch_ls = [&]() {
         const int thr = pl.ng * pl.K * 32;
         const bool sw = p.ls_method == 1;
-        if (ls_lane && pl.K == 1 && !sw) dock_ls_lane_kernel<1, false><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
-        else if (ls_lane && pl.K == 2 && !sw) dock_ls_lane_kernel<2, false><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
-        else if (ls_lane && !sw) dock_ls_lane_kernel<4, false><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
-        else if (ls_lane && pl.K == 1) dock_ls_lane_kernel<1, true><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
-        else if (ls_lane && pl.K == 2) dock_ls_lane_kernel<2, true><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
-        else if (ls_lane) dock_ls_lane_kernel<4, true><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al);
+        if (ls_lane && !sw) { LANE_VARIANT(pl.var, dock_ls_lane_kernel<C, false><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al)) }
+        else if (ls_lane) { LANE_VARIANT(pl.var, dock_ls_lane_kernel<C, true><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al)) }
         else if (ls_team) dock_ls_team_kernel<<<dteam.upj * nlig, kTeamW * 32, smem_team, stm>>>(grids->dev, P, d_jobs, dteam);
         else dock_ls_kernel<<<dls.upj * nlig, Wls * 32, smem_ls, stm>>>(grids->dev, P, d_jobs, dls);
     };
@@ -1303,9 +1335,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         }
         dock_ga_kernel<false><<<dga.upj * nlig, Wga * 32, smem_ga, stm>>>(grids->dev, P, d_jobs, dga, nullptr);
         const int thr = ps.ng * ps.K * 32;
-        if (ps.K == 1) dock_score_lane_kernel<1><<<ps.nctas, thr, ps.smem, stm>>>(grids->dev, P, d_jobs, dm, as);
-        else if (ps.K == 2) dock_score_lane_kernel<2><<<ps.nctas, thr, ps.smem, stm>>>(grids->dev, P, d_jobs, dm, as);
-        else dock_score_lane_kernel<4><<<ps.nctas, thr, ps.smem, stm>>>(grids->dev, P, d_jobs, dm, as);
+        LANE_VARIANT(ps.var, dock_score_lane_kernel<C><<<ps.nctas, thr, ps.smem, stm>>>(grids->dev, P, d_jobs, dm, as))
         return 2;
     };
     dock_init_kernel<<<dga.upj * nlig, Wga * 32, smem_ga, stm>>>(grids->dev, P, d_jobs, dga);
@@ -1509,7 +1539,7 @@ extern "C" int adock_screen(const adock_grids* grids, const adock_params* params
         const adock_ligand_desc& d = ligs[order[0]];
         const int npad = (d.N + kLaneBI - 1) / kLaneBI * kLaneBI;
         LaneGeom g{2 * (8 * d.N * d.N + 512), npad, 6 * (d.R + 1), d.R};
-        const int ng = std::max(1, lane_fit_groups(g, 1));
+        const int ng = std::max(1, lane_fit_groups(g, 0));
         const int target = std::max(1, 3 * g_sm_count * ng / (2 * jg));
         const int nbat = (nlig + target - 1) / target;
         for (int b = 1; b < nbat; ++b) bstart.push_back((int)((long long)nlig * b / nbat));

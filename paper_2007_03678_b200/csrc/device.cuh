@@ -27,6 +27,7 @@ struct GridDev {
 
 struct ParDev {             // adock_params with the per-pair constants folded
     float elec_sqrt, diel_A, diel_B, diel_k, BlamB, mlamB_log2e;   // elec_sqrt = sqrt(elec_scale); BlamB = B*lambda*B
+    float log2_dk;          // log2(diel_k): the lane kernels fold k into the exponent of k exp(-lambda B r)
     float inv_sig2, mhalf_inv_sig2_log2e;
     float rmin2, k_wall, k_wall_h;
     float ad_rho, ad_eps;

@@ -9,11 +9,60 @@
 // them up and runs the serial tail.  More warps per individual = more warps per SM for the same shared memory (the
 // positions are shared) and shorter chains.  The pair loop keeps an I-block of 4 atoms in registers and evaluates
 // two rows at a time against an aligned J-pair with packed f32x2 arithmetic (FFMA2/FMUL2/FADD2).
+// TM variants (one warp per group only) keep the atom positions in TENSOR MEMORY instead of shared memory: TMEM is
+// 128 lanes x 512 columns of 32 bits per SM, a warp reaches the 32 lanes of its quarter with tcgen05.ld/st.32x32b, thread i
+// <-> lane i, and the column address is warp-uniform -- exactly the [index][lane] access pattern of the per-lane state.
+// Positions are 62 % of that state at 40 atoms; with them out of shared memory 12 or 16 warps per SM fit instead of 8.
 #pragma once
 #include "device.cuh"
 #include "lane_image.hpp"
 
 namespace adock {
+
+// ---------------------------------------------------------------- tensor memory as per-lane scratch
+// columns of one warp's slice when W warps share the 4 lane quarters
+__host__ __device__ inline int lane_tmem_columns(int W) { return 512 / ((W + 3) / 4); }
+__device__ __forceinline__ void tm_st1(uint32_t a, float v) { asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ void tm_ld1(uint32_t a, float& v) { asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=f"(v) : "r"(a) : "memory"); }
+__device__ __forceinline__ void tm_ld2(uint32_t a, float& v0, float& v1) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=f"(v0), "=f"(v1) : "r"(a) : "memory");
+}
+__device__ __forceinline__ void tm_ld4(uint32_t a, float& v0, float& v1, float& v2, float& v3) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];" : "=f"(v0), "=f"(v1), "=f"(v2), "=f"(v3) : "r"(a) : "memory");
+}
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// The loaded registers are in/out operands of the wait, so no use of them can be scheduled ahead of it.
+__device__ __forceinline__ void tm_wait_ld(float& a, float& b, float& c) { asm volatile("tcgen05.wait::ld.sync.aligned;" : "+f"(a), "+f"(b), "+f"(c)::"memory"); }
+__device__ __forceinline__ void tm_wait_ld(float& a, float& b, float& c, float& d, float& e, float& f) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;" : "+f"(a), "+f"(b), "+f"(c), "+f"(d), "+f"(e), "+f"(f)::"memory");
+}
+__device__ __forceinline__ void tm_wait_ld(float& a, float& b, float& c, float& d, float& e, float& f, float& g, float& h, float& i,
+                                           float& j, float& k, float& l) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+f"(a), "+f"(b), "+f"(c), "+f"(d), "+f"(e), "+f"(f), "+f"(g), "+f"(h), "+f"(i), "+f"(j), "+f"(k), "+f"(l)::"memory");
+}
+// All threads of the CTA call these.  open: one warp allocates all 512 columns (the kernels run one CTA per SM) and the
+// address travels through the word at smem + 8 (behind the bulk-copy barrier); close: after every warp is done.
+template <bool TM>
+__device__ __forceinline__ uint32_t lane_tmem_open(unsigned char* smem) {
+    if (!TM) return 0u;
+    uint32_t* slot = reinterpret_cast<uint32_t*>(smem + 8);
+    if ((threadIdx.x >> 5) == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(slot)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    return *slot;
+}
+template <bool TM>
+__device__ __forceinline__ void lane_tmem_close(uint32_t base) {
+    if (!TM) return;
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if ((threadIdx.x >> 5) == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(base) : "memory");
+}
 
 // ---------------------------------------------------------------- views
 struct LaneL {              // the staged image
@@ -41,7 +90,10 @@ __device__ inline LaneL lane_view(const unsigned char* blob) {
     return L;
 }
 struct LaneS {              // this lane's columns of the group's scratch; element k of an array sits at [k*32]
-    float2* X; float2* Y; float2* Z;    // [Npad/2]: positions RELATIVE TO t of atoms 2m (.x) and 2m+1 (.y)
+    float2* P;              // [Npad/2][3]: positions RELATIVE TO t of atoms 2m (.x) and 2m+1 (.y): component c of pair m at
+                            // P[(3m + c)*32] (one address register reaches x, y and z of a pair); unused by the TM variants
+    uint32_t tp;            // TM variants: tensor-memory address (lane quarter | first column) of this warp's position
+                            // columns: pair m at columns 6m .. 6m+5 = x0 x1 y0 y1 z0 z1
     float* own;             // [own_floats] of THIS part: per fragment F(3), T(3) about t; during the pose: the transform stack
     float* own0;            // part 0's (the K parts' arrays are consecutive, own_floats*32 apart)
     float* geno;            // [7+R]
@@ -49,23 +101,22 @@ struct LaneS {              // this lane's columns of the group's scratch; eleme
                             // chain's live flag
     int part, gid;          // this warp's part in the group; group index in the CTA (named barrier gid+1)
 };
-// floats per lane of one group's scratch
-__host__ __device__ inline int lane_group_floats(int Npad, int own_floats, int R, int K) {
-    return 3 * Npad + K * own_floats + (7 + R) + (K > 1 ? 8 * K + 1 : 0);      // one warp per group exchanges nothing
+// floats per lane of one group's shared-memory scratch (TM: the positions live in tensor memory)
+__host__ __device__ inline int lane_group_floats(int Npad, int own_floats, int R, int K, bool TM = false) {
+    return (TM ? 0 : 3 * Npad) + K * own_floats + (7 + R) + (K > 1 ? 8 * K + 1 : 0);      // one warp per group exchanges nothing
 }
 // group_floats = floats per lane between consecutive groups of the CTA: lane_group_floats of the ligand, or of the
 // largest ligand of the launch when the groups of a CTA belong to different ligands (0 = this ligand's)
-template <int K>
-__device__ inline LaneS lane_scratch(float* cta_base, const LaneL& L, int warp, int lane, int group_floats = 0) {
+// tmem = lane_tmem_open's result (TM variants): warp w owns lanes 32 (w mod 4) and the (w / 4)-th slice of the 512 columns
+template <int K, bool TM = false>
+__device__ inline LaneS lane_scratch(float* cta_base, const LaneL& L, int warp, int lane, int group_floats = 0, uint32_t tmem = 0) {
     LaneS S;
     S.gid = warp / K; S.part = warp % K;
-    if (group_floats == 0) group_floats = lane_group_floats(L.Npad, L.own_floats, L.R, K);
+    if (group_floats == 0) group_floats = lane_group_floats(L.Npad, L.own_floats, L.R, K, TM);
     float* base = cta_base + (size_t)S.gid * group_floats * 32;
-    const int half = L.Npad / 2;
-    S.X = reinterpret_cast<float2*>(base) + lane;
-    S.Y = S.X + half * 32;
-    S.Z = S.Y + half * 32;
-    S.own0 = base + 3 * L.Npad * 32 + lane;
+    S.P = reinterpret_cast<float2*>(base) + lane;
+    S.tp = tmem + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * lane_tmem_columns((int)(blockDim.x >> 5)));
+    S.own0 = base + (TM ? 0 : 3 * L.Npad) * 32 + lane;
     S.own = S.own0 + S.part * L.own_floats * 32;
     S.geno = S.own0 + K * L.own_floats * 32;
     S.ex = S.geno + (7 + L.R) * 32;
@@ -77,14 +128,54 @@ __device__ __forceinline__ void group_sync(const LaneS& S) {
     if (K > 1) asm volatile("bar.sync %0, %1;" ::"r"(S.gid + 1), "r"(K * 32) : "memory");
 }
 
+// ---------------------------------------------------------------- atom positions (shared memory, or tensor memory when TM)
+struct Pos6 { float x0, x1, y0, y1, z0, z1; };     // the J-pair (2m, 2m+1)
+// issue the loads of pair m; pos_wait before the first use
+template <bool TM>
+__device__ __forceinline__ void pos_issue(const LaneS& S, int m, Pos6& p) {
+    if (TM) {
+        tm_ld4(S.tp + 6 * m, p.x0, p.x1, p.y0, p.y1);
+        tm_ld2(S.tp + 6 * m + 4, p.z0, p.z1);
+    } else {
+        const float2* q = S.P + m * 96;
+        const float2 a = q[0], b = q[32], c = q[64];
+        p.x0 = a.x; p.x1 = a.y; p.y0 = b.x; p.y1 = b.y; p.z0 = c.x; p.z1 = c.y;
+    }
+}
+template <bool TM> __device__ __forceinline__ void pos_wait(Pos6& p) { if (TM) tm_wait_ld(p.x0, p.x1, p.y0, p.y1, p.z0, p.z1); }
+template <bool TM> __device__ __forceinline__ void pos_wait(Pos6& p, Pos6& q) {
+    if (TM) tm_wait_ld(p.x0, p.x1, p.y0, p.y1, p.z0, p.z1, q.x0, q.x1, q.y0, q.y1, q.z0, q.z1);
+}
+// one atom
+template <bool TM>
+__device__ __forceinline__ void pos_put(const LaneS& S, int i, float x, float y, float z) {
+    if (TM) {
+        const uint32_t a = S.tp + 6 * (i >> 1) + (i & 1);
+        tm_st1(a, x); tm_st1(a + 2, y); tm_st1(a + 4, z);
+    } else {
+        float* q = reinterpret_cast<float*>(S.P) + (i >> 1) * 192 + (i & 1);
+        q[0] = x; q[64] = y; q[128] = z;
+    }
+}
+template <bool TM>
+__device__ __forceinline__ void pos_issue1(const LaneS& S, int i, float& x, float& y, float& z) {
+    if (TM) {
+        const uint32_t a = S.tp + 6 * (i >> 1) + (i & 1);
+        tm_ld1(a, x); tm_ld1(a + 2, y); tm_ld1(a + 4, z);
+    } else {
+        const float* q = reinterpret_cast<const float*>(S.P) + (i >> 1) * 192 + (i & 1);
+        x = q[0]; y = q[64]; z = q[128];
+    }
+}
+
 // ---------------------------------------------------------------- one packed row of the pair tile (R5)
 struct PairK {              // packed constants
-    f2 k1, dk, one, A, B, BlamB, k2, six, isig2;
+    f2 k1, lk, one, A, B, BlamB, k2, six, isig2;
     float rmin2;
 };
 __device__ __forceinline__ PairK make_pairk(const ParDev& P) {
     PairK K;
-    K.k1 = bc(P.mlamB_log2e); K.dk = bc(P.diel_k); K.one = bc(1.f); K.A = bc(P.diel_A); K.B = bc(P.diel_B);
+    K.k1 = bc(P.mlamB_log2e); K.lk = bc(P.log2_dk); K.one = bc(1.f); K.A = bc(P.diel_A); K.B = bc(P.diel_B);
     K.BlamB = bc(P.BlamB); K.k2 = bc(P.mhalf_inv_sig2_log2e); K.six = bc(6.f); K.isig2 = bc(P.inv_sig2);
     K.rmin2 = P.rmin2;
     return K;
@@ -115,12 +206,12 @@ __device__ __forceinline__ void pair_row(const PairK& K, f2 xi, f2 yi, f2 zi, f2
         unpk(r6, l, h);
         rA = pk((hb & 1u) ? a : l, (hb & 2u) ? b : h);
     }
-    const f2 nuA = mul2(ncA, rA);               // -cA r^-A
-    const f2 evdw = add2(u12, nuA);
-    // electrostatics with the distance-dependent dielectric: eps = A + B/den, den = 1 + k exp(-lambda B r)
+    const f2 evdw = fma2(ncA, rA, u12);          // c12 r^-12 - cA r^-A
+    // electrostatics with the distance-dependent dielectric: eps = A + B/den, den = 1 + k exp(-lambda B r), and
+    // k exp(-lambda B r) = 2^(-lambda B log2(e) r + log2 k): the factor k rides in the exponent
     float tl, th;
-    unpk(mul2(rr, K.k1), tl, th);
-    const f2 kex = mul2(K.dk, pk(fex2(tl), fex2(th)));
+    unpk(fma2(rr, K.k1, K.lk), tl, th);
+    const f2 kex = pk(fex2(tl), fex2(th));
     const f2 den = add2(kex, K.one);
     const f2 num = fma2(K.A, den, K.B);          // eps = num/den
     unpk(mul2(den, num), tl, th);
@@ -135,7 +226,7 @@ __device__ __forceinline__ void pair_row(const PairK& K, f2 xi, f2 yi, f2 zi, f2
         // -dE/dr = rinv (12 u12 - nA uA + eel) + eel (deps/dr)/eps + (r/sigma^2) egs ;  ns = -(dE/dr)/r
         const f2 s = add2(evdw, u12);
         f2 A1 = fma2(K.six, s, eel);
-        if (HB) A1 = fma2(pk((hb & 1u) ? 4.f : 0.f, (hb & 2u) ? 4.f : 0.f), nuA, A1);
+        if (HB) A1 = fma2(pk((hb & 1u) ? 4.f : 0.f, (hb & 2u) ? 4.f : 0.f), mul2(ncA, rA), A1);
         const f2 dee = mul2(mul2(K.BlamB, kex), inv);
         const f2 A3 = fma2(eel, dee, mul2(A1, rinv));
         // desolvation: (r/sigma^2) egs / r = egs/sigma^2 (the clamped case is zeroed below)
@@ -172,7 +263,7 @@ __device__ __forceinline__ void own_flush(float* own, int f, float Fx, float Fy,
 // The rigid-body blocks (dE/dt, dE/domega) are summed from the GRID forces alone: intramolecular pair forces cancel
 // exactly in both (Newton's third law), so they are kept out of sums they contribute nothing to.
 // The caller must group_sync before S.geno, the positions or own[] are touched again (part 0 still reads them).
-template <bool GRAD, int K, int GOUT = 1>
+template <bool GRAD, int K, int GOUT = 1, bool TM = false>
 __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, const ParDev& P, const LaneS& S, float* grad, int gs,
                                            bool wr, float& e_inter, float& e_intra, bool& gfin) {
     const float tx = S.geno[0], ty = S.geno[32], tz = S.geno[64];
@@ -182,9 +273,7 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
     if (badq) { qw = 1.f; qx = qy = qz = 0.f; }
     const float qi = badq ? 1.f : 1.0f / sqrtf(qn2);
     qw *= qi; qx *= qi; qy *= qi; qz *= qi;
-    float* Xf = reinterpret_cast<float*>(S.X);
-    float* Yf = reinterpret_cast<float*>(S.Y);
-    float* Zf = reinterpret_cast<float*>(S.Z);
+    static_assert(!TM || K == 1, "tensor-memory positions are private to one warp");
 
     // (a1) pose: per-fragment transform = parent's o rotation about the reference-frame axis; positions relative to t.
     // With K > 1 part 0 builds the whole pose and the others wait: the chain of fragment transforms is serial, and
@@ -229,16 +318,12 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
             }
             for (int i = fi.z; i < fi.w; ++i) {
                 const float4 a = L.atoms[i];
-                const int o = (i >> 1) * 64 + (i & 1);
-                Xf[o] = fmaf(m00, a.x, fmaf(m01, a.y, fmaf(m02, a.z, m03)));
-                Yf[o] = fmaf(m10, a.x, fmaf(m11, a.y, fmaf(m12, a.z, m13)));
-                Zf[o] = fmaf(m20, a.x, fmaf(m21, a.y, fmaf(m22, a.z, m23)));
+                pos_put<TM>(S, i, fmaf(m00, a.x, fmaf(m01, a.y, fmaf(m02, a.z, m03))), fmaf(m10, a.x, fmaf(m11, a.y, fmaf(m12, a.z, m13))),
+                            fmaf(m20, a.x, fmaf(m21, a.y, fmaf(m22, a.z, m23))));
             }
         }
-        for (int i = L.N; i < L.Npad; ++i) {            // pad atoms: finite, in no pair
-            const int o = (i >> 1) * 64 + (i & 1);
-            Xf[o] = 0.f; Yf[o] = 0.f; Zf[o] = 0.f;
-        }
+        for (int i = L.N; i < L.Npad; ++i) pos_put<TM>(S, i, 0.f, 0.f, 0.f);      // pad atoms: finite, in no pair
+        if (TM) tm_wait_st();
     }
 
     group_sync<K>(S);                                   // the positions are in place
@@ -260,11 +345,13 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
             {
                 const int4 t4 = *reinterpret_cast<const int4*>(L.types + 2 * m);      // cell set | frag << 8 ; -1 = pad
                 tt[0] = t4.x; tt[1] = t4.y; tt[2] = t4.z; tt[3] = t4.w;
-                const float2 xa = S.X[m * 32], ya = S.Y[m * 32], za = S.Z[m * 32];
-                const float2 xb = S.X[(m + 1) * 32], yb = S.Y[(m + 1) * 32], zb = S.Z[(m + 1) * 32];
-                rx[0] = xa.x; rx[1] = xa.y; rx[2] = xb.x; rx[3] = xb.y;
-                ry[0] = ya.x; ry[1] = ya.y; ry[2] = yb.x; ry[3] = yb.y;
-                rz[0] = za.x; rz[1] = za.y; rz[2] = zb.x; rz[3] = zb.y;
+                Pos6 pa, pb;
+                pos_issue<TM>(S, m, pa);
+                pos_issue<TM>(S, m + 1, pb);
+                pos_wait<TM>(pa, pb);
+                rx[0] = pa.x0; rx[1] = pa.x1; rx[2] = pb.x0; rx[3] = pb.x1;
+                ry[0] = pa.y0; ry[1] = pa.y1; ry[2] = pb.y0; ry[3] = pb.y1;
+                rz[0] = pa.z0; rz[1] = pa.z1; rz[2] = pb.z0; rz[3] = pb.z1;
             }
 #pragma unroll
             for (int a = 0; a < 4; ++a) {
@@ -297,7 +384,9 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
         }
     }
 
-    // (a3) intramolecular pairs: register tiles; this warp's parts of the tile sequence
+    // (a3) intramolecular pairs: register tiles; this warp's parts of the tile sequence.  The record of tile t+1 is
+    // loaded while tile t computes (the tile array ends with a sentinel), and the J fragment's (force, torque) sums are
+    // loaded at the top of the tile that updates them, so the read-modify-write of own[] is not waited for.
     f2 e2 = bc(0.f);
     for (int part = S.part; part < kLaneParts; part += K) {
         const PairK PK = make_pairk(P);
@@ -305,36 +394,50 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
         const f2 zero = bc(0.f);
         for (int kb = L.part_blk[part]; kb < L.part_blk[part + 1]; ++kb) {
             const int4 blk = L.blocks[2 * kb], bf = L.blocks[2 * kb + 1];   // b, tile_begin, tile_end, - ; frags of rows 0-3, 4-7
+            uint2 tw = L.tiles[blk.y];
             float xi[kLaneBI], yi[kLaneBI], zi[kLaneBI];
+            {
+                Pos6 pi[kLaneBI / 2];
 #pragma unroll
-            for (int h2 = 0; h2 < kLaneBI / 2; ++h2) {
-                const int o = ((kLaneBI / 2) * blk.x + h2) * 32;
-                const float2 xa = S.X[o], ya = S.Y[o], za = S.Z[o];
-                xi[2 * h2] = xa.x; xi[2 * h2 + 1] = xa.y; yi[2 * h2] = ya.x; yi[2 * h2 + 1] = ya.y; zi[2 * h2] = za.x; zi[2 * h2 + 1] = za.y;
+                for (int h2 = 0; h2 < kLaneBI / 2; ++h2) pos_issue<TM>(S, (kLaneBI / 2) * blk.x + h2, pi[h2]);
+#pragma unroll
+                for (int h2 = 0; h2 < kLaneBI / 2; h2 += 2) pos_wait<TM>(pi[h2], pi[h2 + 1]);
+#pragma unroll
+                for (int h2 = 0; h2 < kLaneBI / 2; ++h2) {
+                    xi[2 * h2] = pi[h2].x0; xi[2 * h2 + 1] = pi[h2].x1; yi[2 * h2] = pi[h2].y0; yi[2 * h2 + 1] = pi[h2].y1;
+                    zi[2 * h2] = pi[h2].z0; zi[2 * h2 + 1] = pi[h2].z1;
+                }
             }
             f2 gix[kLaneBI], giy[kLaneBI], giz[kLaneBI];
 #pragma unroll
             for (int r = 0; r < kLaneBI; ++r) gix[r] = giy[r] = giz[r] = zero;
             for (int t = blk.y; t < blk.z; ++t) {
-                const uint2 tw = L.tiles[t];
-                const int jp = tw.x & 0xff;
-                const f2 xj = ld2(S.X + jp * 32), yj = ld2(S.Y + jp * 32), zj = ld2(S.Z + jp * 32);
+                const uint2 cw = tw;
+                tw = L.tiles[t + 1];                    // next tile (or the sentinel)
+                Pos6 pj;
+                pos_issue<TM>(S, cw.x & 0xff, pj);
+                const int f0 = (cw.y >> 16) & 0xff, f1 = cw.y >> 24;
+                float* o0 = S.own + f0 * 192;
+                float v0 = 0.f, v1 = 0.f, v2 = 0.f, v3 = 0.f, v4 = 0.f, v5 = 0.f;
+                if (GRAD) { v0 = o0[0]; v1 = o0[32]; v2 = o0[64]; v3 = o0[96]; v4 = o0[128]; v5 = o0[160]; }
+                pos_wait<TM>(pj);
+                const f2 xj = pk(pj.x0, pj.x1), yj = pk(pj.y0, pj.y1), zj = pk(pj.z0, pj.z1);
                 f2 gjx = zero, gjy = zero, gjz = zero;
 #pragma unroll
                 for (int hf = 0; hf < kLaneBI / 2; ++hf) {   // a half = two rows = two independent chains in one basic block
-                    if (tw.x & (0x100u << hf)) {
+                    if (cw.x & (0x100u << hf)) {
                         const float4 ra0 = rowp[0], rb0 = rowp[1], ra1 = rowp[2], rb1 = rowp[3];
                         rowp += 4;
                         const int r0 = 2 * hf, r1 = 2 * hf + 1;
-                        if (!(tw.x & (0x1000u << hf))) {
+                        if (!(cw.x & (0x1000u << hf))) {
                             pair_row<GRAD, false>(PK, bc(xi[r0]), bc(yi[r0]), bc(zi[r0]), xj, yj, zj, ra0, rb0, 0u, e2,
                                                   gix[r0], giy[r0], giz[r0], gjx, gjy, gjz);
                             pair_row<GRAD, false>(PK, bc(xi[r1]), bc(yi[r1]), bc(zi[r1]), xj, yj, zj, ra1, rb1, 0u, e2,
                                                   gix[r1], giy[r1], giz[r1], gjx, gjy, gjz);
                         } else {
-                            pair_row<GRAD, true>(PK, bc(xi[r0]), bc(yi[r0]), bc(zi[r0]), xj, yj, zj, ra0, rb0, (tw.y >> (2 * r0)) & 3u,
+                            pair_row<GRAD, true>(PK, bc(xi[r0]), bc(yi[r0]), bc(zi[r0]), xj, yj, zj, ra0, rb0, (cw.y >> (2 * r0)) & 3u,
                                                  e2, gix[r0], giy[r0], giz[r0], gjx, gjy, gjz);
-                            pair_row<GRAD, true>(PK, bc(xi[r1]), bc(yi[r1]), bc(zi[r1]), xj, yj, zj, ra1, rb1, (tw.y >> (2 * r1)) & 3u,
+                            pair_row<GRAD, true>(PK, bc(xi[r1]), bc(yi[r1]), bc(zi[r1]), xj, yj, zj, ra1, rb1, (cw.y >> (2 * r1)) & 3u,
                                                  e2, gix[r1], giy[r1], giz[r1], gjx, gjy, gjz);
                         }
                     }
@@ -343,14 +446,14 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                     const f2 tqx = fma2(yj, gjz, neg2(mul2(zj, gjy)));
                     const f2 tqy = fma2(zj, gjx, neg2(mul2(xj, gjz)));
                     const f2 tqz = fma2(xj, gjy, neg2(mul2(yj, gjx)));
-                    const int f0 = (tw.y >> 16) & 0xff, f1 = tw.y >> 24;
                     if (f0 == f1) {
-                        own_add(S.own, f0, hsum(gjx), hsum(gjy), hsum(gjz), hsum(tqx), hsum(tqy), hsum(tqz));
-                    } else {
+                        o0[0] = v0 + hsum(gjx); o0[32] = v1 + hsum(gjy); o0[64] = v2 + hsum(gjz);
+                        o0[96] = v3 + hsum(tqx); o0[128] = v4 + hsum(tqy); o0[160] = v5 + hsum(tqz);
+                    } else {                            // the J-pair straddles two fragments
                         float ax, bx, ay, by, az, bz, cx, dx, cy, dy, cz, dz;
                         unpk(gjx, ax, bx); unpk(gjy, ay, by); unpk(gjz, az, bz);
                         unpk(tqx, cx, dx); unpk(tqy, cy, dy); unpk(tqz, cz, dz);
-                        own_add(S.own, f0, ax, ay, az, cx, cy, cz);
+                        o0[0] = v0 + ax; o0[32] = v1 + ay; o0[64] = v2 + az; o0[96] = v3 + cx; o0[128] = v4 + cy; o0[160] = v5 + cz;
                         own_add(S.own, f1, bx, by, bz, dx, dy, dz);
                     }
                 }
@@ -408,9 +511,11 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
             float* o = S.own + f * 6 * 32;
             const float Fx = o[0], Fy = o[32], Fz = o[64], Tx = o[96], Ty = o[128], Tz = o[160];
             const int ia = ab & 0xffff, ib = ab >> 16;
-            const int oa = (ia >> 1) * 64 + (ia & 1), ob = (ib >> 1) * 64 + (ib & 1);
-            const float ax = Xf[oa], ay = Yf[oa], az = Zf[oa];
-            float ux = Xf[ob] - ax, uy = Yf[ob] - ay, uz = Zf[ob] - az;
+            float ax, ay, az, ux, uy, uz;
+            pos_issue1<TM>(S, ia, ax, ay, az);
+            pos_issue1<TM>(S, ib, ux, uy, uz);
+            if (TM) tm_wait_ld(ax, ay, az, ux, uy, uz);
+            ux -= ax; uy -= ay; uz -= az;
             const float un = rsqrtf(ux * ux + uy * uy + uz * uz);
             ux *= un; uy *= un; uz *= un;
             // torque about the pivot atom a: T - a x F
@@ -457,7 +562,7 @@ __device__ __forceinline__ float adadelta_component(const ParDev& P, float g, fl
 // state (ls, in global scratch columns) and on return ls.best holds the best genotype seen; part 0 returns its energy
 // (e_start if no finite evaluation happened) and the evaluations done.  `active` lanes run the chain; the others only
 // keep the warp's control flow uniform.  The gradient never leaves shared memory (lane_eval, GOUT = 2).
-template <int K>
+template <int K, bool TM = false>
 __device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const ParDev& P, const LaneS& S, const LaneLS& ls,
                                       bool active, float e_start, int& iters, float* trace, int trace_stride) {
     const int R = L.R, D = 6 + R, Gn = 7 + R;
@@ -474,7 +579,7 @@ __device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const Pa
         if (!__any_sync(kFull, live)) break;            // same decision in every warp of the group
         float ei, ea;
         bool gfin = true;
-        const float e = lane_eval<true, K, 2>(L, G, P, S, nullptr, 0, false, ei, ea, gfin);
+        const float e = lane_eval<true, K, 2, TM>(L, G, P, S, nullptr, 0, false, ei, ea, gfin);
         if (lead) {
             if (live) {
                 if (trace) trace[it * trace_stride] = e;
@@ -543,7 +648,7 @@ __device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const Pa
 // so a lane whose first trial succeeded draws its next step at once instead of idling through the other lanes'
 // second trial.  Part 0 owns the state: x in ls.best, bias in ls.Eg2, delta in ls.Ed2 (global scratch columns).
 // On return ls.best holds the accepted genotype; part 0 returns its energy and the evaluations done.
-template <int K>
+template <int K, bool TM = false>
 __device__ inline float lane_solis_wets(const LaneL& L, const GridDev& G, const ParDev& P, const LaneS& S, const LaneLS& ls,
                                         bool active, float e_start, unsigned long long seed, uint32_t id, uint32_t gen, int& evals,
                                         float* trace, int trace_stride) {
@@ -590,7 +695,7 @@ __device__ inline float lane_solis_wets(const LaneL& L, const GridDev& G, const 
         if (!__any_sync(kFull, live)) break;            // same decision in every warp of the group
         float ei, ea;
         bool gfin = true;
-        const float e = lane_eval<false, K, 1>(L, G, P, S, nullptr, 1, false, ei, ea, gfin);
+        const float e = lane_eval<false, K, 1, TM>(L, G, P, S, nullptr, 1, false, ei, ea, gfin);
         if (lead && live) {
             ++evals;
             const bool ok = e < E;

@@ -178,7 +178,8 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
     h.off_types = (int)off;  off = align16(off + (size_t)Npad * 4);
     h.off_frags = (int)off;  off = align16(off + (size_t)nfrag * sizeof(LaneFrag));
     h.off_blocks = (int)off; off = align16(off + blocks.size() * (sizeof(LaneBlock) + 0));
-    h.off_tiles = (int)off;  off = align16(off + tiles.size() * sizeof(LaneTile));
+    h.off_tiles = (int)off;  off = align16(off + (tiles.size() + 1) * sizeof(LaneTile));    // + a sentinel (J-pair 0, no half):
+                                                                                          // the tile loop reads one record ahead
     h.off_rows = (int)off;   off = align16(off + rows.size() * sizeof(LaneRow));
     h.bytes = (int)off;
     h.nslots = 2 * (int)rows.size();    // pair slots evaluated; npairs of them carry a pair

@@ -36,7 +36,7 @@ def dev():
     return torch.device("cuda:0")
 
 
-@pytest.fixture(params=["warp", "lane1", "lane2", "lane4", "team"])
+@pytest.fixture(params=["warp", "lane1", "lane2", "lane4", "tm8", "tm12", "tm16", "team"])
 def family(request, B):
     """run the test once per kernel family (warp per individual / thread per individual); restores 'auto'"""
     B.adock_set_path(request.param)
@@ -592,7 +592,7 @@ def test_dock_many_equals_single_docks(B, W, orc, cases, family):
         assert np.array_equal(many["genotypes"][k, :, :7 + l.R], one["genotypes"])
         assert np.array_equal(many["coords"][k, :, :l.N], one["coords"])
         assert np.array_equal(many["evals"][k], one["evals"])
-    assert B.adock_last_dock_path() == family[:4]
+    assert B.adock_last_dock_path() == ("lane" if family.startswith(("lane", "tm")) else family)
 
 
 def test_host_only_handle_is_rejected_by_compute_calls(B, cases, dev):
