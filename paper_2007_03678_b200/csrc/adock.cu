@@ -371,6 +371,7 @@ __global__ void __launch_bounds__(256) score_kernel(GridDev G, ParDev P, ScoreAr
 template <int K_, int W_, bool TM_> struct LaneCfg {
     static constexpr int K = K_, kMaxWarps = W_;
     static constexpr bool TM = TM_;
+    static constexpr bool ST = TM_;         // local-search state in shared memory (the room the positions left) instead of global columns
 };
 struct LaneVar { int K, W; bool TM; double eff; };        // eff: measured throughput per SM at full residency, K = 1 / 8 warps = 1
 constexpr int kNumLaneVars = 6;
@@ -390,27 +391,30 @@ static LaneGeom lane_geom(const adock_ligand* l) { return LaneGeom{l->lane_bytes
 static LaneGeom lane_geom_max(LaneGeom a, LaneGeom b) {
     return LaneGeom{std::max(a.bytes, b.bytes), std::max(a.npad, b.npad), std::max(a.own, b.own), std::max(a.R, b.R)};
 }
-static int lane_var_floats(const LaneGeom& g, int v) { return lane_group_floats(g.npad, g.own, g.R, kLaneVars[v].K, kLaneVars[v].TM); }
-// shared memory of a CTA of `groups` groups with `nimg` image slots
-static size_t lane_smem(const LaneGeom& g, int v, int groups, int nimg = 1) {
-    const size_t slot = ((size_t)g.bytes + 127) & ~(size_t)127;
-    return 16 + (size_t)nimg * slot + (size_t)groups * lane_var_floats(g, v) * 128;
+// ls: a local-search kernel (the TM variants keep the chain state in shared memory)
+static int lane_var_floats(const LaneGeom& g, int v, bool ls) {
+    return lane_group_floats(g.npad, g.own, g.R, kLaneVars[v].K, kLaneVars[v].TM, ls && kLaneVars[v].TM);
 }
-static bool lane_fits(const LaneGeom& g, int v, int groups, int nimg = 1) {
+// shared memory of a CTA of `groups` groups with `nimg` image slots
+static size_t lane_smem(const LaneGeom& g, int v, bool ls, int groups, int nimg = 1) {
+    const size_t slot = ((size_t)g.bytes + 127) & ~(size_t)127;
+    return 16 + (size_t)nimg * slot + (size_t)groups * lane_var_floats(g, v, ls) * 128;
+}
+static bool lane_fits(const LaneGeom& g, int v, bool ls, int groups, int nimg = 1) {
     if (kLaneVars[v].TM && 3 * g.npad > lane_tmem_columns(groups * kLaneVars[v].K)) return false;
-    return lane_smem(g, v, groups, nimg) <= (size_t)g_smem_optin;
+    return lane_smem(g, v, ls, groups, nimg) <= (size_t)g_smem_optin;
 }
 // most groups per CTA that fit (0: not even one)
-static int lane_fit_groups(const LaneGeom& g, int v) {
+static int lane_fit_groups(const LaneGeom& g, int v, bool ls) {
     int n = kLaneVars[v].W / kLaneVars[v].K;
-    while (n > 0 && !lane_fits(g, v, n)) --n;
+    while (n > 0 && !lane_fits(g, v, ls, n)) --n;
     return n;
 }
 // the lane kernels want at least one warp per scheduler
 static bool lane_ok(const adock_ligand* l) {
     const LaneGeom g = lane_geom(l);
     for (int v = 0; v < kNumLaneVars; ++v)
-        if (lane_fit_groups(g, v) * kLaneVars[v].K >= 4) return true;
+        if (lane_fit_groups(g, v, true) * kLaneVars[v].K >= 4) return true;
     return false;
 }
 // ADADELTA chains (threads) from which the lane-per-individual kernels are preferred over warp-per-individual
@@ -439,7 +443,7 @@ static int lane_plan_images(long long total, int jg, int ng) {        // most im
 }
 // Model: an SM with w resident warps of a variant works at min(w, W)/W of the variant's rate eff (measured per SM at
 // full residency: profiles/r02_lane_variants.md); waves of CTAs run one after another.
-static LanePlan lane_plan(const LaneGeom& g, long long total, int jg) {
+static LanePlan lane_plan(const LaneGeom& g, long long total, int jg, bool ls) {
     LanePlan best;
     double best_t = 1e300;
     if (total < 1) total = 1;
@@ -448,7 +452,7 @@ static LanePlan lane_plan(const LaneGeom& g, long long total, int jg) {
         if (g_lane_var >= 0 && v != g_lane_var) continue;       // a forced variant that does not fit is an error (ADOCK_ELIMIT), never a silent substitute
         const LaneVar& V = kLaneVars[v];
         for (int ng = V.W / V.K; ng >= 1; --ng) {
-            if (!lane_fits(g, v, ng, lane_plan_images(total, jg, ng))) continue;
+            if (!lane_fits(g, v, ls, ng, lane_plan_images(total, jg, ng))) continue;
             const long long nctas = (total + ng - 1) / ng, waves = (nctas + g_sm_count - 1) / g_sm_count;
             const double t = (double)waves * ng / (V.eff * (double)(ng * V.K) / V.W);
             if (t < best_t * 0.999) {
@@ -462,12 +466,12 @@ static LanePlan lane_plan(const LaneGeom& g, long long total, int jg) {
     best.nctas = (int)((total + best.ng - 1) / best.ng);
     best.nimg = lane_plan_images(total, jg, best.ng);
     best.slot = (g.bytes + 127) & ~127;
-    best.gfloats = lane_var_floats(g, best.var);
-    best.smem = lane_smem(g, best.var, best.ng, best.nimg);
+    best.gfloats = lane_var_floats(g, best.var, ls);
+    best.smem = lane_smem(g, best.var, ls, best.ng, best.nimg);
     return best;
 }
 // variant for `ngroups` groups of 32 individuals of one ligand (-1: none fits)
-static int lane_pick_var(const LaneGeom& g, long long ngroups) { return lane_plan(g, ngroups, (int)std::min<long long>(ngroups, 1 << 30)).var; }
+static int lane_pick_var(const LaneGeom& g, long long ngroups, bool ls) { return lane_plan(g, ngroups, (int)std::min<long long>(ngroups, 1 << 30), ls).var; }
 // groups per CTA: as many as fit, fewer when that would leave SMs idle
 static int lane_spread_groups(int fit, long long ngroups) {
     int n = fit;
@@ -510,8 +514,8 @@ template <bool GRAD, class C>
 static int launch_score_lane_k(const adock_grids* grids, const adock_ligand* lig, const ParDev& P, const ScoreArgs& a, int var, int ngroups,
                                cudaStream_t st) {
     const LaneGeom g = lane_geom(lig);
-    const int NG = lane_spread_groups(lane_fit_groups(g, var), ngroups);
-    const size_t smem = lane_smem(g, var, NG);
+    const int NG = lane_spread_groups(lane_fit_groups(g, var, false), ngroups);
+    const size_t smem = lane_smem(g, var, false, NG);
     const int grid = (int)std::max<long long>(1, std::min<long long>(((long long)ngroups + NG - 1) / NG, g_sm_count));
     CUDA_TRY(cudaFuncSetAttribute(score_lane_kernel<GRAD, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     score_lane_kernel<GRAD, C><<<grid, NG * C::K * 32, smem, st>>>(grids->dev, P, a);
@@ -523,7 +527,7 @@ static int launch_score_lane_k(const adock_grids* grids, const adock_ligand* lig
 static int launch_score_lane(const adock_grids* grids, const adock_ligand* lig, const adock_params& p, const float* d_genos, int n,
                              int gstride, float* d_E, float* d_terms, float* d_grads, int dstride, cudaStream_t st) {
     const int ngroups = (n + 31) / 32;
-    const int var = lane_pick_var(lane_geom(lig), ngroups);
+    const int var = lane_pick_var(lane_geom(lig), ngroups, false);
     if (var < 0) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
     ParDev P = make_pardev(p);
     P.k_wall_h = p.k_wall * grids->dev.h;
@@ -665,7 +669,8 @@ __global__ void __launch_bounds__(C::kMaxWarps * 32, 1) ls_array_lane_kernel(Gri
     const uint32_t tmem = lane_tmem_open<C::TM>(smem);
     const LaneL L = lane_view(blob);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, NG = (blockDim.x >> 5) / K;
-    const LaneS S = lane_scratch<K, C::TM>(reinterpret_cast<float*>(blob + a.blob_bytes), L, warp, lane, 0, tmem);
+    const LaneS S = lane_scratch<K, C::TM>(reinterpret_cast<float*>(blob + a.blob_bytes), L, warp, lane,
+                                           lane_group_floats(L.Npad, L.own_floats, L.R, K, C::TM, C::ST), tmem);
     const int Gn = 7 + L.R, D = 6 + L.R;
     const size_t tid = ((size_t)blockIdx.x * NG + S.gid) * 32 + lane, T = (size_t)gridDim.x * NG * 32;
     const bool act = tid < (size_t)a.n;
@@ -674,14 +679,14 @@ __global__ void __launch_bounds__(C::kMaxWarps * 32, 1) ls_array_lane_kernel(Gri
         for (int d = 0; d < Gn; ++d) S.geno[d * 32] = a.genos[idx * a.gstride + d];
     group_sync<K>(S);
     LaneLS ls;
-    ls.best = scratch + tid; ls.Eg2 = ls.best + (size_t)Gn * T; ls.Ed2 = ls.Eg2 + (size_t)D * T;
-    ls.stride = (int)T;
+    if (C::ST) { ls.best = S.state; ls.Eg2 = ls.best + Gn * 32; ls.Ed2 = ls.Eg2 + D * 32; ls.stride = 32; }
+    else { ls.best = scratch + tid; ls.Eg2 = ls.best + (size_t)Gn * T; ls.Ed2 = ls.Eg2 + (size_t)D * T; ls.stride = (int)T; }
     int iters = 0;
     float* tr = a.trace ? a.trace + idx * P.lsit : nullptr;
     const float e = SW ? lane_solis_wets<K, C::TM>(L, G, P, S, ls, act, (act && S.part == 0) ? a.E[idx] : 0.f, a.seed, (uint32_t)idx, a.gen, iters, tr, 1)
                        : lane_adadelta<K, C::TM>(L, G, P, S, ls, act, __int_as_float(0x7fc00000), iters, tr, 1);
     if (act && S.part == 0) {
-        for (int d = 0; d < Gn; ++d) a.genos[idx * a.gstride + d] = ls.best[(size_t)d * T];
+        for (int d = 0; d < Gn; ++d) a.genos[idx * a.gstride + d] = ls.best[(size_t)d * ls.stride];
         a.E[idx] = e;
         if (a.iters) a.iters[idx] = iters;
     }
@@ -692,13 +697,13 @@ template <class C, bool SW>
 static int launch_ls_array_lane(const adock_grids* grids, const adock_ligand* ligand, const ParDev& P, LsArgs a, int var, int n, cudaStream_t stm) {
     const LaneGeom g = lane_geom(ligand);
     const int ngroups = (n + 31) / 32;
-    const int NG = lane_spread_groups(lane_fit_groups(g, var), ngroups);
+    const int NG = lane_spread_groups(lane_fit_groups(g, var, true), ngroups);
     const int grid = (ngroups + NG - 1) / NG;
-    const size_t smem = lane_smem(g, var, NG);
+    const size_t smem = lane_smem(g, var, true, NG);
     const size_t T = (size_t)grid * NG * 32;
     const int R = ligand->tp.R;
     float* scratch = nullptr;
-    cudaError_t e = cudaMallocAsync(&scratch, T * (size_t)(7 + R + 2 * (6 + R)) * 4, stm);
+    cudaError_t e = cudaMallocAsync(&scratch, C::ST ? 16 : T * (size_t)(7 + R + 2 * (6 + R)) * 4, stm);
     if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("ls scratch: ") + cudaGetErrorString(e));
     e = cudaFuncSetAttribute(ls_array_lane_kernel<C, SW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) {
@@ -726,7 +731,7 @@ static int local_search_impl(const adock_grids* grids, const adock_ligand* ligan
     rc = device_props();
     if (rc) return rc;
     if (g_path == 2 || (g_path == 0 && n >= lane_min_chains() && lane_ok(ligand))) {
-        const int var = lane_pick_var(lane_geom(ligand), (n + 31) / 32);
+        const int var = lane_pick_var(lane_geom(ligand), (n + 31) / 32, true);
         if (var < 0) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
         ParDev P = make_pardev(p);
         P.k_wall_h = p.k_wall * grids->dev.h;
@@ -1008,14 +1013,14 @@ __device__ __forceinline__ void dock_ls_lane_group(const GridDev& G, const ParDe
     const size_t tid = ((size_t)blockIdx.x * a.ng + S.gid) * 32 + lane, T = (size_t)gridDim.x * a.ng * 32;
     const int Dmax = a.Gmax - 1;
     LaneLS ls;
-    ls.best = a.scratch + tid; ls.Eg2 = ls.best + (size_t)a.Gmax * T; ls.Ed2 = ls.Eg2 + (size_t)Dmax * T;
-    ls.stride = (int)T;
+    if (C::ST) { ls.best = S.state; ls.Eg2 = ls.best + Gn * 32; ls.Ed2 = ls.Eg2 + (Gn - 1) * 32; ls.stride = 32; }
+    else { ls.best = a.scratch + tid; ls.Eg2 = ls.best + (size_t)a.Gmax * T; ls.Ed2 = ls.Eg2 + (size_t)Dmax * T; ls.stride = (int)T; }
     int iters = 0;
     const float e0 = (act && S.part == 0) ? *e : 0.f;
     const float be = SW ? lane_solis_wets<K, C::TM>(L, G, P, S, ls, act, e0, job.seed, (uint32_t)(run * dm.P + slot), (uint32_t)st.gen + 1u, iters, nullptr, 0)
                         : lane_adadelta<K, C::TM>(L, G, P, S, ls, act, e0, iters, nullptr, 0);
     if (act && S.part == 0) {
-        for (int d = 0; d < Gn; ++d) g[d] = ls.best[(size_t)d * T];
+        for (int d = 0; d < Gn; ++d) g[d] = ls.best[(size_t)d * ls.stride];
         *e = be;
         atomicAdd(&job.st[run].ls_acc, iters);
     }
@@ -1204,7 +1209,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         lanes_fit = lanes_fit && lane_ok(ligs[l]);
     }
     const int jg = (nrun * n_ls0 + 31) / 32;                        // groups of 32 chains per job
-    const LanePlan pl = lane_plan(lg, (long long)nlig * jg, jg);
+    const LanePlan pl = lane_plan(lg, (long long)nlig * jg, jg, true);
     // Solis-Wets chains end after very different numbers of evaluations (28 to lsit iterations), which leaves most lanes
     // of a lane-per-chain warp idle; one warp per chain is 2x faster there (profiles/r01d_next_rows.md)
     const bool many = g_path == 0 && lanes_fit && chains >= lane_min_chains();
@@ -1217,7 +1222,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     g_last_dock_path = ls_lane ? 2 : ls_team ? 3 : 1;
     // offspring scoring: lane-per-individual under the same condition (populations are 1/lsrat times larger)
     const int jgs = (int)(((long long)nrun * Pn + 31) / 32);
-    const LanePlan ps = lane_plan(lg, (long long)nlig * jgs, jgs);
+    const LanePlan ps = lane_plan(lg, (long long)nlig * jgs, jgs, false);
     const bool ga_lane = ps.var >= 0 && (g_path == 2 || many);
     ParDev P = make_pardev(p);
     P.k_wall_h = p.k_wall * grids->dev.h;
@@ -1304,7 +1309,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     float* d_lscratch = nullptr;
     if (ls_lane && dm.n_ls > 0) {
         const size_t T = (size_t)pl.nctas * pl.ng * 32;
-        cudaError_t e2 = buf.alloc(&d_lscratch, T * (size_t)(Gmax + 2 * (Gmax - 1)) * 4);
+        cudaError_t e2 = buf.alloc(&d_lscratch, kLaneVars[pl.var].TM ? 16 : T * (size_t)(Gmax + 2 * (Gmax - 1)) * 4);
         if (e2 != cudaSuccess) return fail(e2 == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("dock alloc: ") + cudaGetErrorString(e2));
         al = LaneDockArgs{d_lscratch, Gmax, pl.ng, nlig * jg, jg, pl.slot, pl.nimg, pl.gfloats};
         cudaError_t e3 = cudaSuccess;
@@ -1539,7 +1544,7 @@ extern "C" int adock_screen(const adock_grids* grids, const adock_params* params
         const adock_ligand_desc& d = ligs[order[0]];
         const int npad = (d.N + kLaneBI - 1) / kLaneBI * kLaneBI;
         LaneGeom g{2 * (8 * d.N * d.N + 512), npad, 6 * (d.R + 1), d.R};
-        const int ng = std::max(1, lane_fit_groups(g, 0));
+        const int ng = std::max(1, lane_fit_groups(g, 0, true));
         const int target = std::max(1, 3 * g_sm_count * ng / (2 * jg));
         const int nbat = (nlig + target - 1) / target;
         for (int b = 1; b < nbat; ++b) bstart.push_back((int)((long long)nlig * b / nbat));

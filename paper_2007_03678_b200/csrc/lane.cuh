@@ -72,7 +72,7 @@ struct LaneL {              // the staged image
     const int4* blocks;
     const uint2* tiles;
     const float4* rows;
-    int N, Npad, R, nfrag, nblocks, own_floats;
+    int N, Npad, R, nfrag, nblocks, own_floats, own_a;
     const int* part_blk;    // [kLaneParts+1]
     const int* part_row;    // [kLaneParts+1]
 };
@@ -85,7 +85,7 @@ __device__ inline LaneL lane_view(const unsigned char* blob) {
     L.blocks = reinterpret_cast<const int4*>(blob + h->off_blocks);
     L.tiles = reinterpret_cast<const uint2*>(blob + h->off_tiles);
     L.rows = reinterpret_cast<const float4*>(blob + h->off_rows);
-    L.N = h->N; L.Npad = h->Npad; L.R = h->R; L.nfrag = h->nfrag; L.nblocks = h->nblocks; L.own_floats = h->own_floats;
+    L.N = h->N; L.Npad = h->Npad; L.R = h->R; L.nfrag = h->nfrag; L.nblocks = h->nblocks; L.own_floats = h->own_floats; L.own_a = h->own_a;
     L.part_blk = h->part_blk; L.part_row = h->part_row;
     return L;
 }
@@ -94,16 +94,21 @@ struct LaneS {              // this lane's columns of the group's scratch; eleme
                             // P[(3m + c)*32] (one address register reaches x, y and z of a pair); unused by the TM variants
     uint32_t tp;            // TM variants: tensor-memory address (lane quarter | first column) of this warp's position
                             // columns: pair m at columns 6m .. 6m+5 = x0 x1 y0 y1 z0 z1
-    float* own;             // [own_floats] of THIS part: per fragment F(3), T(3) about t; during the pose: the transform stack
-    float* own0;            // part 0's (the K parts' arrays are consecutive, own_floats*32 apart)
+    float4* oA;             // per-fragment sums of THIS part, read and written as vectors: fragment f = (Fx, Fy, Fz, Tx) in
+    float2* oB;             // oA[f*32] and (Ty, Tz) in oB[f*32] (force, torque about t); own_floats = 4 own_a + 2 nfrag floats.
+                            // During the pose oA holds the transform stack: depth d = rows oA[(3d .. 3d+2)*32] of a 3x4 matrix
+    int part_stride;        // floats between the own arrays of consecutive parts (own_floats*32); part 0's = this - part*stride
     float* geno;            // [7+R]
     float* ex;              // [8K+1]: (e_grid, e_pairs, grid force F(3), grid torque about t T(3)) of each part, then the
                             // chain's live flag
+    float* state;           // ST: ADADELTA / Solis-Wets state columns of this lane: best [7+R], Eg2 [6+R], Ed2 [6+R]
     int part, gid;          // this warp's part in the group; group index in the CTA (named barrier gid+1)
 };
 // floats per lane of one group's shared-memory scratch (TM: the positions live in tensor memory)
-__host__ __device__ inline int lane_group_floats(int Npad, int own_floats, int R, int K, bool TM = false) {
-    return (TM ? 0 : 3 * Npad) + K * own_floats + (7 + R) + (K > 1 ? 8 * K + 1 : 0);      // one warp per group exchanges nothing
+// ST: the local-search state (best genotype and two accumulators per degree of freedom) sits in shared memory as well
+__host__ __device__ inline int lane_group_floats(int Npad, int own_floats, int R, int K, bool TM = false, bool ST = false) {
+    return (TM ? 0 : 3 * Npad) + K * own_floats + (7 + R) + (K > 1 ? 8 * K + 1 : 0)      // one warp per group exchanges nothing
+           + (ST ? (7 + R) + 2 * (6 + R) : 0);
 }
 // group_floats = floats per lane between consecutive groups of the CTA: lane_group_floats of the ligand, or of the
 // largest ligand of the launch when the groups of a CTA belong to different ligands (0 = this ligand's)
@@ -112,14 +117,17 @@ template <int K, bool TM = false>
 __device__ inline LaneS lane_scratch(float* cta_base, const LaneL& L, int warp, int lane, int group_floats = 0, uint32_t tmem = 0) {
     LaneS S;
     S.gid = warp / K; S.part = warp % K;
-    if (group_floats == 0) group_floats = lane_group_floats(L.Npad, L.own_floats, L.R, K, TM);
+    if (group_floats == 0) group_floats = lane_group_floats(L.Npad, L.own_floats, L.R, K, TM);      // callers with ST pass it
     float* base = cta_base + (size_t)S.gid * group_floats * 32;
     S.P = reinterpret_cast<float2*>(base) + lane;
     S.tp = tmem + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * lane_tmem_columns((int)(blockDim.x >> 5)));
-    S.own0 = base + (TM ? 0 : 3 * L.Npad) * 32 + lane;
-    S.own = S.own0 + S.part * L.own_floats * 32;
-    S.geno = S.own0 + K * L.own_floats * 32;
+    float* own = base + (TM ? 0 : 3 * L.Npad) * 32;   // 128-byte aligned
+    S.part_stride = L.own_floats * 32;
+    S.oA = reinterpret_cast<float4*>(own + S.part * S.part_stride) + lane;
+    S.oB = reinterpret_cast<float2*>(own + S.part * S.part_stride + 4 * L.own_a * 32) + lane;
+    S.geno = own + K * S.part_stride + lane;
     S.ex = S.geno + (7 + L.R) * 32;
+    S.state = S.ex + (K > 1 ? 8 * K + 1 : 0) * 32;
     return S;
 }
 // barrier of the K warps of a group
@@ -239,18 +247,19 @@ __device__ __forceinline__ void pair_row(const PairK& K, f2 xi, f2 yi, f2 zi, f2
 }
 
 // own[f] += (F, T)
-__device__ __forceinline__ void own_add(float* own, int f, float Fx, float Fy, float Fz, float Tx, float Ty, float Tz) {
-    float* o = own + f * 6 * 32;
-    o[0] += Fx; o[32] += Fy; o[64] += Fz; o[96] += Tx; o[128] += Ty; o[160] += Tz;
+__device__ __forceinline__ void own_add(const LaneS& S, int f, float Fx, float Fy, float Fz, float Tx, float Ty, float Tz) {
+    float4 a = S.oA[f * 32];
+    float2 b = S.oB[f * 32];
+    a.x += Fx; a.y += Fy; a.z += Fz; a.w += Tx; b.x += Ty; b.y += Tz;
+    S.oA[f * 32] = a; S.oB[f * 32] = b;
 }
 
 // flush a fragment's (force, torque) sums: one warp per group visits every fragment exactly once (store); with K > 1 a
 // part may skip fragments, so own[] is zeroed first and the sums are added
 template <int K>
-__device__ __forceinline__ void own_flush(float* own, int f, float Fx, float Fy, float Fz, float Tx, float Ty, float Tz) {
-    float* o = own + f * 6 * 32;
-    if (K == 1) { o[0] = Fx; o[32] = Fy; o[64] = Fz; o[96] = Tx; o[128] = Ty; o[160] = Tz; }
-    else { o[0] += Fx; o[32] += Fy; o[64] += Fz; o[96] += Tx; o[128] += Ty; o[160] += Tz; }
+__device__ __forceinline__ void own_flush(const LaneS& S, int f, float Fx, float Fy, float Fz, float Tx, float Ty, float Tz) {
+    if (K == 1) { S.oA[f * 32] = make_float4(Fx, Fy, Fz, Tx); S.oB[f * 32] = make_float2(Ty, Tz); }
+    else own_add(S, f, Fx, Fy, Fz, Tx, Ty, Tz);
 }
 
 // ---------------------------------------------------------------- full evaluation of this lane's genotype
@@ -258,8 +267,8 @@ __device__ __forceinline__ void own_flush(float* own, int f, float Fx, float Fy,
 // (NaN for |q| < 1e-12, with NaN gradient); the other parts return 0.  With GRAD part 0 clears `gfin` if a gradient
 // component is not finite and delivers the gradient according to GOUT:
 //   GOUT = 1: grad[d*gs] for d < 6+R when `wr` (scoring: straight to the caller's array)
-//   GOUT = 2: left in part 0's own[] columns: dE/dt, dE/domega in own[0..5], dE/dtau of fragment f's torsion in
-//             own[6f] (local search: the optimiser reads them from shared memory; `grad` is not used)
+//   GOUT = 2: left in part 0's own[] columns: dE/dt, dE/domega in oA[0], oB[0], dE/dtau of fragment f's torsion in
+//             oA[f*32].x (local search: the optimiser reads them from shared memory; `grad` is not used)
 // The rigid-body blocks (dE/dt, dE/domega) are summed from the GRID forces alone: intramolecular pair forces cancel
 // exactly in both (Newton's third law), so they are kept out of sums they contribute nothing to.
 // The caller must group_sync before S.geno, the positions or own[] are touched again (part 0 still reads them).
@@ -290,10 +299,11 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                 const int4 fa = L.fragi[3 * f + 1], fb = L.fragi[3 * f + 2];
                 const float p0x = __int_as_float(fa.x), p0y = __int_as_float(fa.y), p0z = __int_as_float(fa.z);
                 const float ux = __int_as_float(fb.x), uy = __int_as_float(fb.y), uz = __int_as_float(fb.z);
-                const float* st = S.own + (depth - 1) * 12 * 32;
-                const float b00 = st[0], b01 = st[32], b02 = st[64], b03 = st[96];
-                const float b10 = st[128], b11 = st[160], b12 = st[192], b13 = st[224];
-                const float b20 = st[256], b21 = st[288], b22 = st[320], b23 = st[352];
+                const float4* st = S.oA + (depth - 1) * 3 * 32;
+                const float4 r0 = st[0], r1 = st[32], r2 = st[64];
+                const float b00 = r0.x, b01 = r0.y, b02 = r0.z, b03 = r0.w;
+                const float b10 = r1.x, b11 = r1.y, b12 = r1.z, b13 = r1.w;
+                const float b20 = r2.x, b21 = r2.y, b22 = r2.z, b23 = r2.w;
                 float s, c;
                 sincosf(S.geno[(7 + fa.w) * 32], &s, &c);
                 const float k = 1.f - c;
@@ -311,10 +321,10 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                 m23 = b20 * wx + b21 * wy + b22 * wz + b23;
             }
             if (fi.y >> 16) {                           // has children: push
-                float* st = S.own + depth * 12 * 32;
-                st[0] = m00; st[32] = m01; st[64] = m02; st[96] = m03;
-                st[128] = m10; st[160] = m11; st[192] = m12; st[224] = m13;
-                st[256] = m20; st[288] = m21; st[320] = m22; st[352] = m23;
+                float4* st = S.oA + depth * 3 * 32;
+                st[0] = make_float4(m00, m01, m02, m03);
+                st[32] = make_float4(m10, m11, m12, m13);
+                st[64] = make_float4(m20, m21, m22, m23);
             }
             for (int i = fi.z; i < fi.w; ++i) {
                 const float4 a = L.atoms[i];
@@ -334,7 +344,7 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
     float RFx = 0, RFy = 0, RFz = 0, RTx = 0, RTy = 0, RTz = 0;     // grid force / torque about t over ALL atoms of this part
     {
         if (GRAD && K > 1)
-            for (int d = 0; d < 6 * L.nfrag; ++d) S.own[d * 32] = 0.f;
+            for (int f = 0; f < L.nfrag; ++f) { S.oA[f * 32] = make_float4(0.f, 0.f, 0.f, 0.f); S.oB[f * 32] = make_float2(0.f, 0.f); }
         float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
         int cur = 0;
         for (int m = 2 * S.part; m < L.Npad / 2; m += 2 * K) {
@@ -369,7 +379,7 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                 if (GRAD) {
                     const int f = tt[a] >> 8;
                     if (f != cur) {
-                        own_flush<K>(S.own, cur, Fx, Fy, Fz, Tx, Ty, Tz);
+                        own_flush<K>(S, cur, Fx, Fy, Fz, Tx, Ty, Tz);
                         RFx += Fx; RFy += Fy; RFz += Fz; RTx += Tx; RTy += Ty; RTz += Tz;
                         Fx = Fy = Fz = Tx = Ty = Tz = 0.f; cur = f;
                     }
@@ -379,7 +389,7 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
             }
         }
         if (GRAD) {
-            own_flush<K>(S.own, cur, Fx, Fy, Fz, Tx, Ty, Tz);
+            own_flush<K>(S, cur, Fx, Fy, Fz, Tx, Ty, Tz);
             RFx += Fx; RFy += Fy; RFz += Fz; RTx += Tx; RTy += Ty; RTz += Tz;
         }
     }
@@ -417,9 +427,9 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                 Pos6 pj;
                 pos_issue<TM>(S, cw.x & 0xff, pj);
                 const int f0 = (cw.y >> 16) & 0xff, f1 = cw.y >> 24;
-                float* o0 = S.own + f0 * 192;
-                float v0 = 0.f, v1 = 0.f, v2 = 0.f, v3 = 0.f, v4 = 0.f, v5 = 0.f;
-                if (GRAD) { v0 = o0[0]; v1 = o0[32]; v2 = o0[64]; v3 = o0[96]; v4 = o0[128]; v5 = o0[160]; }
+                float4 va = make_float4(0.f, 0.f, 0.f, 0.f);
+                float2 vb = make_float2(0.f, 0.f);
+                if (GRAD) { va = S.oA[f0 * 32]; vb = S.oB[f0 * 32]; }
                 pos_wait<TM>(pj);
                 const f2 xj = pk(pj.x0, pj.x1), yj = pk(pj.y0, pj.y1), zj = pk(pj.z0, pj.z1);
                 f2 gjx = zero, gjy = zero, gjz = zero;
@@ -447,14 +457,15 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                     const f2 tqy = fma2(zj, gjx, neg2(mul2(xj, gjz)));
                     const f2 tqz = fma2(xj, gjy, neg2(mul2(yj, gjx)));
                     if (f0 == f1) {
-                        o0[0] = v0 + hsum(gjx); o0[32] = v1 + hsum(gjy); o0[64] = v2 + hsum(gjz);
-                        o0[96] = v3 + hsum(tqx); o0[128] = v4 + hsum(tqy); o0[160] = v5 + hsum(tqz);
+                        S.oA[f0 * 32] = make_float4(va.x + hsum(gjx), va.y + hsum(gjy), va.z + hsum(gjz), va.w + hsum(tqx));
+                        S.oB[f0 * 32] = make_float2(vb.x + hsum(tqy), vb.y + hsum(tqz));
                     } else {                            // the J-pair straddles two fragments
                         float ax, bx, ay, by, az, bz, cx, dx, cy, dy, cz, dz;
                         unpk(gjx, ax, bx); unpk(gjy, ay, by); unpk(gjz, az, bz);
                         unpk(tqx, cx, dx); unpk(tqy, cy, dy); unpk(tqz, cz, dz);
-                        o0[0] = v0 + ax; o0[32] = v1 + ay; o0[64] = v2 + az; o0[96] = v3 + cx; o0[128] = v4 + cy; o0[160] = v5 + cz;
-                        own_add(S.own, f1, bx, by, bz, dx, dy, dz);
+                        S.oA[f0 * 32] = make_float4(va.x + ax, va.y + ay, va.z + az, va.w + cx);
+                        S.oB[f0 * 32] = make_float2(vb.x + cy, vb.y + cz);
+                        own_add(S, f1, bx, by, bz, dx, dy, dz);
                     }
                 }
             }
@@ -468,7 +479,7 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                     Tx += yi[r] * gz - zi[r] * gy; Ty += zi[r] * gx - xi[r] * gz; Tz += xi[r] * gy - yi[r] * gx;
                     const int fr = frag_of_row(r);
                     if (r == kLaneBI - 1 || fr != frag_of_row(r + 1)) {
-                        own_add(S.own, fr, Fx, Fy, Fz, Tx, Ty, Tz);
+                        own_add(S, fr, Fx, Fy, Fz, Tx, Ty, Tz);
                         Fx = Fy = Fz = Tx = Ty = Tz = 0.f;
                     }
                 }
@@ -491,10 +502,15 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                 const float* e8 = S.ex + 8 * k * 32;
                 RFx += e8[64]; RFy += e8[96]; RFz += e8[128]; RTx += e8[160]; RTy += e8[192]; RTz += e8[224];
             }
-            for (int d = 6; d < 6 * L.nfrag; ++d) {     // the root's own sums are not needed (grid totals above)
-                float v = S.own0[d * 32];
-                for (int k = 1; k < K; ++k) v += S.own0[(k * L.own_floats + d) * 32];
-                S.own0[d * 32] = v;
+            for (int f = 1; f < L.nfrag; ++f) {         // the root's own sums are not needed (grid totals above)
+                float4 a = S.oA[f * 32];                // this is part 0
+                float2 b = S.oB[f * 32];
+                for (int k = 1; k < K; ++k) {
+                    const float4 c = *reinterpret_cast<const float4*>(reinterpret_cast<const float*>(S.oA + f * 32) + k * S.part_stride);
+                    const float2 d = *reinterpret_cast<const float2*>(reinterpret_cast<const float*>(S.oB + f * 32) + k * S.part_stride);
+                    a.x += c.x; a.y += c.y; a.z += c.z; a.w += c.w; b.x += d.x; b.y += d.y;
+                }
+                S.oA[f * 32] = a; S.oB[f * 32] = b;
             }
         }
     }
@@ -508,8 +524,9 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
         for (int f = L.nfrag - 1; f > 0; --f) {
             const int4 fi = L.fragi[3 * f];
             const int tor = L.fragi[3 * f + 1].w, ab = L.fragi[3 * f + 2].w;
-            float* o = S.own + f * 6 * 32;
-            const float Fx = o[0], Fy = o[32], Fz = o[64], Tx = o[96], Ty = o[128], Tz = o[160];
+            const float4 oa = S.oA[f * 32];
+            const float2 ob = S.oB[f * 32];
+            const float Fx = oa.x, Fy = oa.y, Fz = oa.z, Tx = oa.w, Ty = ob.x, Tz = ob.y;
             const int ia = ab & 0xffff, ib = ab >> 16;
             float ax, ay, az, ux, uy, uz;
             pos_issue1<TM>(S, ia, ax, ay, az);
@@ -524,8 +541,8 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
             if (badq) dt = qnan;
             fin = fin && isfinite(dt);
             if (GOUT == 1) { if (wr) grad[(6 + tor) * gs] = dt; }
-            else o[0] = dt;                             // fragment f's sums are consumed: its first slot carries dE/dtau
-            if (fi.x != 0) own_add(S.own, fi.x, Fx, Fy, Fz, Tx, Ty, Tz);     // the root takes the grid totals instead
+            else reinterpret_cast<float*>(S.oA + f * 32)[0] = dt;     // fragment f's sums are consumed: its first slot carries dE/dtau
+            if (fi.x != 0) own_add(S, fi.x, Fx, Fy, Fz, Tx, Ty, Tz);     // the root takes the grid totals instead
         }
         float g[6] = {RFx, RFy, RFz, RTx, RTy, RTz};
 #pragma unroll
@@ -533,8 +550,8 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
             if (badq) g[d] = qnan;
             fin = fin && isfinite(g[d]);
             if (GOUT == 1) { if (wr) grad[d * gs] = g[d]; }
-            else S.own[d * 32] = g[d];
         }
+        if (GOUT != 1) { S.oA[0] = make_float4(g[0], g[1], g[2], g[3]); S.oB[0] = make_float2(g[4], g[5]); }
         gfin = fin;
     }
     return e;
@@ -594,18 +611,21 @@ __device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const Pa
                 // the accumulator columns live in global memory (L2): a chunk of 8 components is loaded before the
                 // first store, so the chunk costs one round trip instead of one per component
                 float w[3];
-                {                                       // rigid-body block: d = 0..5, gradient in own[0..5]
+                {                                       // rigid-body block: d = 0..5, gradient in oA[0], oB[0]
+                    const float4 ga = S.oA[0];
+                    const float2 gb = S.oB[0];
+                    const float gr[6] = {ga.x, ga.y, ga.z, ga.w, gb.x, gb.y};
                     float av[6], bv[6];
 #pragma unroll
                     for (int d = 0; d < 6; ++d) { av[d] = ls.Eg2[d * ls.stride]; bv[d] = ls.Ed2[d * ls.stride]; }
 #pragma unroll
                     for (int d = 0; d < 6; ++d) {
-                        const float dl = adadelta_component(P, S.own[d * 32], av[d], bv[d]);
+                        const float dl = adadelta_component(P, gr[d], av[d], bv[d]);
                         ls.Eg2[d * ls.stride] = av[d]; ls.Ed2[d * ls.stride] = bv[d];
                         if (d < 3) S.geno[d * 32] += dl; else w[d - 3] = dl;
                     }
                 }
-                for (int f0 = 1; f0 < L.nfrag; f0 += 8) {  // torsions: fragment f's torsion gradient in own[6f]
+                for (int f0 = 1; f0 < L.nfrag; f0 += 8) {  // torsions: fragment f's torsion gradient in oA[f*32].x
                     float av[8], bv[8];
                     int dd[8];
 #pragma unroll
@@ -618,7 +638,7 @@ __device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const Pa
                     for (int k = 0; k < 8; ++k) {
                         const int f = f0 + k;
                         if (f < L.nfrag) {
-                            const float dl = adadelta_component(P, S.own[6 * f * 32], av[k], bv[k]);
+                            const float dl = adadelta_component(P, reinterpret_cast<const float*>(S.oA + f * 32)[0], av[k], bv[k]);
                             ls.Eg2[dd[k] * ls.stride] = av[k]; ls.Ed2[dd[k] * ls.stride] = bv[k];
                             float* t = S.geno + (dd[k] + 1) * 32;
                             *t = wrap_pi(*t + dl);

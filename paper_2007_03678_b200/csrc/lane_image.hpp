@@ -31,7 +31,8 @@ struct LaneHeader {             // 128 bytes
     int nblocks, ntiles, nrows, maxdepth;
     int off_atoms, off_types, off_frags, off_blocks;    // types: cell set (2 type + (q < 0)) | fragment << 8 per atom, -1 = pad
     int off_tiles, off_rows, bytes, npairs;
-    int own_floats, warp_floats, nslots, pad1;    // per-thread scratch: own_floats = max(6 nfrag, 12 maxdepth);
+    int own_floats, warp_floats, nslots, own_a; // per-thread scratch: own_a float4 (4 sums per fragment) + nfrag float2 (2 sums):
+                                                // own_floats = 4 own_a + 2 nfrag >= 12 maxdepth (the transform stack of the pose);
                                                 // warp_floats = 3 Npad + own_floats + (7+R)  (one warp per group)
     int part_blk[kLaneParts + 1];               // part p owns blocks [part_blk[p], part_blk[p+1])
     int part_row[kLaneParts + 1];               // and row records from part_row[p] on (a block may be cut between parts)
@@ -170,7 +171,8 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
     h.N = N; h.Npad = Npad; h.R = R; h.nfrag = nfrag;
     h.nblocks = (int)blocks.size(); h.ntiles = (int)tiles.size(); h.nrows = (int)rows.size(); h.maxdepth = maxdepth;
     h.npairs = (int)tp.pairs.size() / 2;
-    h.own_floats = std::max(6 * nfrag, 12 * maxdepth);
+    h.own_a = std::max(nfrag, (12 * maxdepth - 2 * nfrag + 3) / 4);     // the stack (12 floats per depth) may run on into the float2 part
+    h.own_floats = 4 * h.own_a + 2 * nfrag;
     h.warp_floats = 3 * Npad + h.own_floats + 7 + R;
     for (int q = 0; q <= kLaneParts; ++q) { h.part_blk[q] = part_blk[q]; h.part_row[q] = part_row[q]; }
     size_t off = sizeof(LaneHeader);
