@@ -415,7 +415,7 @@ def probe(argv):
             ast = int(argv[5]) if len(argv) > 5 else 0
             grids, lig0 = W.make_config("drug")
             centre = 0.5 * (grids.box_lo + grids.box_hi); c = W.CONFIGS["drug"]
-            ligs = [W.make_ligand(c["N"], c["R"], c["T"], 100 + i, centre) for i in range(L)]
+            ligs = [W.make_ligand(c["N"], c["R"], c["T"], 100 + (0 if os.environ.get("ADOCK_PROBE_SAME_LIGAND") else i), centre) for i in range(L)]
             nrun = NRUN
         else:
             L, path = 1, int(argv[1])

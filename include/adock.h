@@ -46,7 +46,7 @@ typedef struct adock_ligand adock_ligand; /* opaque, preprocessed topology on ho
  * baked into a ligand at adock_load_ligand; later calls must pass the same values (else ADOCK_EINVAL). */
 typedef struct adock_params {
     float elec_scale;  /* W_el * 332.06363 (R5) */
-    float diel_A, diel_B, diel_k, diel_lambda; /* eps(r) = A + B/(1 + k exp(-lambda B r)) (R5) */
+    float diel_A, diel_B, diel_k, diel_lambda; /* eps(r) = A + B/(1 + k exp(-lambda B r)) (R5); k > 0 */
     float w_desolv;    /* W_ds (R5) */
     float ds_sigma;    /* sigma of the desolvation Gaussian, Angstrom (R5) */
     float qasp;        /* S_i = solpar[type_i] + qasp*|q_i| (R5) */

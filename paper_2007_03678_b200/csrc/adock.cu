@@ -34,6 +34,7 @@ struct adock_ligand {
     int blob_bytes = 0;
     int scratch_floats = 0;
     float w_desolv = 0, qasp = 0, elec_scale = 0;
+    double elec_fold = 1;                   // lane_elec_fold of the parameters the lane image was built with
     LaneImage lane;                         // image of the lane-per-individual kernels (lane_image.hpp)
     unsigned char* d_lane = nullptr;
     int lane_bytes = 0, lane_npad = 0, lane_own = 0;      // group scratch = lane_group_floats(npad, own, R, K) per lane
@@ -92,6 +93,11 @@ extern "C" int adock_default_params(adock_params* p) {
     return ADOCK_OK;
 }
 
+// the lane image's electrostatic row coefficients are elec_scale q_i q_j / s with s = B lambda B (1 for a constant dielectric)
+static double lane_elec_fold(const adock_params& p) {
+    const double s = (double)p.diel_B * (double)p.diel_lambda * (double)p.diel_B;
+    return s != 0.0 ? s : 1.0;
+}
 static ParDev make_pardev(const adock_params& p) {
     const double log2e = 1.4426950408889634;
     ParDev d;
@@ -99,6 +105,12 @@ static ParDev make_pardev(const adock_params& p) {
     d.BlamB = (float)((double)p.diel_B * (double)p.diel_lambda * (double)p.diel_B);
     d.mlamB_log2e = (float)(-(double)p.diel_lambda * (double)p.diel_B * log2e);
     d.log2_dk = (float)std::log2((double)p.diel_k);
+    {   // lane kernels (lane.cuh, pair_row): constants of eps(r) scaled by s = B lambda B; a constant dielectric (s = 0) is
+        // passed as A = eps, B = 0, k exp(..) = 0 with s = 1
+        const double s = lane_elec_fold(p);
+        if ((double)p.diel_B * (double)p.diel_lambda * (double)p.diel_B != 0.0) { d.diel_As = (float)((double)p.diel_A / s); d.diel_Bs = (float)((double)p.diel_B / s); }
+        else { d.diel_As = (float)((double)p.diel_A + (double)p.diel_B / (1.0 + (double)p.diel_k)); d.diel_Bs = 0.f; d.log2_dk = -INFINITY; d.mlamB_log2e = 0.f; }
+    }
     d.inv_sig2 = (float)(1.0 / ((double)p.ds_sigma * (double)p.ds_sigma));
     d.mhalf_inv_sig2_log2e = (float)(-0.5 * log2e / ((double)p.ds_sigma * (double)p.ds_sigma));
     d.rmin2 = p.r_min * p.r_min; d.k_wall = p.k_wall; d.k_wall_h = 0.f;    // k_wall_h set per grid
@@ -127,8 +139,8 @@ static int check_params(const adock_params* in, const adock_ligand* l, adock_par
         !(out.sw_expand > 0) || !(out.sw_contract > 0) || std::isnan(out.as_tol) || (out.autostop && (out.as_window < 1 || out.as_window > kAsMaxWindow)))
         return fail(ADOCK_EINVAL, "parameter out of range");
     if (l && !l->d_blob) return fail(ADOCK_EINVAL, "host-only ligand handle (loaded with grids == NULL)");
-    if (l && (out.w_desolv != l->w_desolv || out.qasp != l->qasp || out.elec_scale != l->elec_scale))
-        return fail(ADOCK_EINVAL, "elec_scale/w_desolv/qasp differ from the values baked into the ligand at load time");
+    if (l && (out.w_desolv != l->w_desolv || out.qasp != l->qasp || out.elec_scale != l->elec_scale || lane_elec_fold(out) != l->elec_fold))
+        return fail(ADOCK_EINVAL, "elec_scale/w_desolv/qasp/diel_B/diel_lambda differ from the values baked into the ligand at load time");
     return ADOCK_OK;
 }
 
@@ -226,8 +238,8 @@ extern "C" int adock_load_ligand(const adock_grids* grids, const adock_params* p
         delete l;
         return fail(ADOCK_EINVAL, msg);
     }
-    l->w_desolv = p.w_desolv; l->qasp = p.qasp; l->elec_scale = p.elec_scale;
-    build_lane_image(l->lane, l->tp, xyz, type, charge, pair_coeffs, solpar, vol, p.w_desolv, p.qasp, p.elec_scale);
+    l->w_desolv = p.w_desolv; l->qasp = p.qasp; l->elec_scale = p.elec_scale; l->elec_fold = lane_elec_fold(p);
+    build_lane_image(l->lane, l->tp, xyz, type, charge, pair_coeffs, solpar, vol, p.w_desolv, p.qasp, (double)p.elec_scale / l->elec_fold);
     l->lane_bytes = (int)l->lane.blob.size();
     l->lane_npad = l->lane.npad; l->lane_own = l->lane.own_floats;
     l->blob_bytes = (int)l->tp.blob.size();

@@ -28,6 +28,8 @@ struct GridDev {
 struct ParDev {             // adock_params with the per-pair constants folded
     float elec_sqrt, diel_A, diel_B, diel_k, BlamB, mlamB_log2e;   // elec_sqrt = sqrt(elec_scale); BlamB = B*lambda*B
     float log2_dk;          // log2(diel_k): the lane kernels fold k into the exponent of k exp(-lambda B r)
+    float diel_As, diel_Bs; // lane kernels: A/s, B/s with s = B*lambda*B, so that 1/(den*(A/s*den + B/s)) = s/(den num) carries
+                            // the factor of d(eps)/dr; the row coefficients qq of the lane image are divided by s (lane_elec_fold)
     float inv_sig2, mhalf_inv_sig2_log2e;
     float rmin2, k_wall, k_wall_h;
     float ad_rho, ad_eps;
@@ -198,8 +200,8 @@ struct GridCell {
     float ox, oy, oz;       // signed distance outside the box in grid units (0 inside)
 };
 // `set` = 2*type + (q < 0)
-__device__ __forceinline__ GridCell grid_cell(const GridDev& G, int set, float x, float y, float z) {
-    const float ux = (x - G.ox) * G.inv_h, uy = (y - G.oy) * G.inv_h, uz = (z - G.oz) * G.inv_h;
+// (ux, uy, uz) = position in grid units
+__device__ __forceinline__ GridCell grid_cell_u(const GridDev& G, int set, float ux, float uy, float uz) {
     const float cx = fminf(fmaxf(ux, 0.f), (float)(G.nx - 1)), cy = fminf(fmaxf(uy, 0.f), (float)(G.ny - 1)),
                 cz = fminf(fmaxf(uz, 0.f), (float)(G.nz - 1));
     const int ix = min((int)cx, G.nx - 2), iy = min((int)cy, G.ny - 2), iz = min((int)cz, G.nz - 2);
@@ -208,6 +210,9 @@ __device__ __forceinline__ GridCell grid_cell(const GridDev& G, int set, float x
     c.ox = ux - cx; c.oy = uy - cy; c.oz = uz - cz;
     c.base = G.cells + (long long)set * G.set_stride + ((long long)(iz * (G.ny - 1) + iy) * (G.nx - 1) + ix) * 2;
     return c;
+}
+__device__ __forceinline__ GridCell grid_cell(const GridDev& G, int set, float x, float y, float z) {
+    return grid_cell_u(G, set, (x - G.ox) * G.inv_h, (y - G.oy) * G.inv_h, (z - G.oz) * G.inv_h);
 }
 // v[0] = plane iz, v[1] = plane iz+1; each {a,pm}(ix,iy) {a,pm}(ix+1,iy) | {a,pm}(ix,iy+1) {a,pm}(ix+1,iy+1)
 __device__ __forceinline__ void grid_fetch(const GridDev& G, const GridCell& c, F8 (&v)[2]) {

@@ -178,13 +178,13 @@ __device__ __forceinline__ void pos_issue1(const LaneS& S, int i, float& x, floa
 
 // ---------------------------------------------------------------- one packed row of the pair tile (R5)
 struct PairK {              // packed constants
-    f2 k1, lk, one, A, B, BlamB, k2, six, isig2;
+    f2 k1, lk, one, A, B, k2, six, isig2;    // A, B: diel_A/s, diel_B/s (ParDev)
     float rmin2;
 };
 __device__ __forceinline__ PairK make_pairk(const ParDev& P) {
     PairK K;
-    K.k1 = bc(P.mlamB_log2e); K.lk = bc(P.log2_dk); K.one = bc(1.f); K.A = bc(P.diel_A); K.B = bc(P.diel_B);
-    K.BlamB = bc(P.BlamB); K.k2 = bc(P.mhalf_inv_sig2_log2e); K.six = bc(6.f); K.isig2 = bc(P.inv_sig2);
+    K.k1 = bc(P.mlamB_log2e); K.lk = bc(P.log2_dk); K.one = bc(1.f); K.A = bc(P.diel_As); K.B = bc(P.diel_Bs);
+    K.k2 = bc(P.mhalf_inv_sig2_log2e); K.six = bc(6.f); K.isig2 = bc(P.inv_sig2);
     K.rmin2 = P.rmin2;
     return K;
 }
@@ -221,11 +221,11 @@ __device__ __forceinline__ void pair_row(const PairK& K, f2 xi, f2 yi, f2 zi, f2
     unpk(fma2(rr, K.k1, K.lk), tl, th);
     const f2 kex = pk(fex2(tl), fex2(th));
     const f2 den = add2(kex, K.one);
-    const f2 num = fma2(K.A, den, K.B);          // eps = num/den
+    const f2 num = fma2(K.A, den, K.B);          // eps = s num/den, s = B lambda B
     unpk(mul2(den, num), tl, th);
-    const f2 inv = pk(frcp(tl), frcp(th));       // 1/(den num)
-    const f2 ieps = mul2(mul2(den, den), inv);   // 1/eps
-    const f2 eel = mul2(mul2(qq, rinv), ieps);
+    const f2 inv = pk(frcp(tl), frcp(th));       // s/(den eps den)
+    const f2 ieps = mul2(mul2(den, den), inv);   // s/eps
+    const f2 eel = mul2(mul2(qq, rinv), ieps);   // the row's qq carries 1/s
     // desolvation
     unpk(mul2(r2c, K.k2), tl, th);
     const f2 egs = mul2(ds, pk(fex2(tl), fex2(th)));
@@ -235,7 +235,7 @@ __device__ __forceinline__ void pair_row(const PairK& K, f2 xi, f2 yi, f2 zi, f2
         const f2 s = add2(evdw, u12);
         f2 A1 = fma2(K.six, s, eel);
         if (HB) A1 = fma2(pk((hb & 1u) ? 4.f : 0.f, (hb & 2u) ? 4.f : 0.f), mul2(ncA, rA), A1);
-        const f2 dee = mul2(mul2(K.BlamB, kex), inv);
+        const f2 dee = mul2(kex, inv);              // (d eps/dr)/eps = B lambda B kex/(den^2 eps)
         const f2 A3 = fma2(eel, dee, mul2(A1, rinv));
         // desolvation: (r/sigma^2) egs / r = egs/sigma^2 (the clamped case is zeroed below)
         float nl, nh;
@@ -342,6 +342,7 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
     // gradient goes straight into the (force, torque about t) sums of the atom's fragment, which initialises own[]
     float eg = 0.f;
     float RFx = 0, RFy = 0, RFz = 0, RTx = 0, RTy = 0, RTz = 0;     // grid force / torque about t over ALL atoms of this part
+    const float ucx = (tx - G.ox) * G.inv_h, ucy = (ty - G.oy) * G.inv_h, ucz = (tz - G.oz) * G.inv_h;  // t in grid units
     {
         if (GRAD && K > 1)
             for (int f = 0; f < L.nfrag; ++f) { S.oA[f * 32] = make_float4(0.f, 0.f, 0.f, 0.f); S.oB[f * 32] = make_float2(0.f, 0.f); }
@@ -366,7 +367,7 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
 #pragma unroll
             for (int a = 0; a < 4; ++a) {
                 q[a] = L.atoms[2 * m + a].w;
-                gc[a] = grid_cell(G, tt[a] < 0 ? 0 : (tt[a] & 0xff), rx[a] + tx, ry[a] + ty, rz[a] + tz);
+                gc[a] = grid_cell_u(G, tt[a] < 0 ? 0 : (tt[a] & 0xff), fmaf(rx[a], G.inv_h, ucx), fmaf(ry[a], G.inv_h, ucy), fmaf(rz[a], G.inv_h, ucz));
             }
 #pragma unroll
             for (int a = 0; a < 4; ++a) grid_fetch(G, gc[a], c[a]);
@@ -452,20 +453,18 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                         }
                     }
                 }
-                if (GRAD) {                             // J side: gradient gj at rel (xj,yj,zj) -> fragment sums
-                    const f2 tqx = fma2(yj, gjz, neg2(mul2(zj, gjy)));
-                    const f2 tqy = fma2(zj, gjx, neg2(mul2(xj, gjz)));
-                    const f2 tqz = fma2(xj, gjy, neg2(mul2(yj, gjx)));
+                if (GRAD) {                             // J side: gradients (a | b) of atoms (j0 | j1) -> fragment sums, the torque
+                    float ax, bx, ay, by, az, bz;        // about t as chains of scalar fma on top of the loaded sums
+                    unpk(gjx, ax, bx); unpk(gjy, ay, by); unpk(gjz, az, bz);
+                    const float t0x = fmaf(pj.y0, az, -pj.z0 * ay), t0y = fmaf(pj.z0, ax, -pj.x0 * az), t0z = fmaf(pj.x0, ay, -pj.y0 * ax);
                     if (f0 == f1) {
-                        S.oA[f0 * 32] = make_float4(va.x + hsum(gjx), va.y + hsum(gjy), va.z + hsum(gjz), va.w + hsum(tqx));
-                        S.oB[f0 * 32] = make_float2(vb.x + hsum(tqy), vb.y + hsum(tqz));
+                        S.oA[f0 * 32] = make_float4((va.x + ax) + bx, (va.y + ay) + by, (va.z + az) + bz,
+                                                    fmaf(pj.y1, bz, fmaf(-pj.z1, by, va.w + t0x)));
+                        S.oB[f0 * 32] = make_float2(fmaf(pj.z1, bx, fmaf(-pj.x1, bz, vb.x + t0y)), fmaf(pj.x1, by, fmaf(-pj.y1, bx, vb.y + t0z)));
                     } else {                            // the J-pair straddles two fragments
-                        float ax, bx, ay, by, az, bz, cx, dx, cy, dy, cz, dz;
-                        unpk(gjx, ax, bx); unpk(gjy, ay, by); unpk(gjz, az, bz);
-                        unpk(tqx, cx, dx); unpk(tqy, cy, dy); unpk(tqz, cz, dz);
-                        S.oA[f0 * 32] = make_float4(va.x + ax, va.y + ay, va.z + az, va.w + cx);
-                        S.oB[f0 * 32] = make_float2(vb.x + cy, vb.y + cz);
-                        own_add(S, f1, bx, by, bz, dx, dy, dz);
+                        S.oA[f0 * 32] = make_float4(va.x + ax, va.y + ay, va.z + az, va.w + t0x);
+                        S.oB[f0 * 32] = make_float2(vb.x + t0y, vb.y + t0z);
+                        own_add(S, f1, bx, by, bz, fmaf(pj.y1, bz, -pj.z1 * by), fmaf(pj.z1, bx, -pj.x1 * bz), fmaf(pj.x1, by, -pj.y1 * bx));
                     }
                 }
             }

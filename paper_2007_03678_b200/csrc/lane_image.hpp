@@ -73,7 +73,7 @@ struct LaneImage {
 
 inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz, const int* type, const float* charge,
                              const float* coeffs, const float* solpar, const float* vol, float w_desolv, float qasp,
-                             float elec_scale) {
+                             double elec_scale) {       // elec_scale: already divided by the fold factor of pair_row (adock.cu)
     const int N = tp.N, R = tp.R, T = tp.T, nfrag = tp.nfrag;
     const int Npad = (N + kLaneBI - 1) / kLaneBI * kLaneBI;
     im.pos_of_ext.assign(N, -1);
@@ -123,7 +123,7 @@ inline void build_lane_image(LaneImage& im, const Topology& tp, const float* xyz
                     row.c12[h] = co[0];
                     row.ncA[h] = -co[1];
                     row.ds[h] = (float)((double)w_desolv * (Si * (double)vol[tj] + Sj * (double)vol[ti]));
-                    row.qq[h] = (float)((double)elec_scale * (double)charge[s.ei] * (double)charge[s.ej]);
+                    row.qq[h] = (float)(elec_scale * (double)charge[s.ei] * (double)charge[s.ej]);
                     if (co[2] > 8.0f) { hbmask |= 1u << (2 * r + h); hbhalf |= 1u << (r / 2); }
                     ++npair_slots;
                 }
