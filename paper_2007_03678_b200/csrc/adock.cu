@@ -385,10 +385,13 @@ template <int K_, int W_, bool TM_> struct LaneCfg {
     static constexpr bool TM = TM_;
     static constexpr bool ST = TM_;         // local-search state in shared memory (the room the positions left) instead of global columns
 };
-struct LaneVar { int K, W; bool TM; double eff; };        // eff: measured throughput per SM at full residency, K = 1 / 8 warps = 1
+struct LaneVar { int K, W; bool TM; double eff, eff_ls; };   // measured throughput per SM at full residency (K = 1 with 8 warps = 1):
+                                                              // eff of the scoring kernels, eff_ls of the local-search kernels
 constexpr int kNumLaneVars = 6;
-static const LaneVar kLaneVars[kNumLaneVars] = {{1, 8, false, 1.0}, {2, 12, false, 0.95}, {4, 16, false, 0.85},
-                                                {1, 8, true, 1.0},  {1, 12, true, 1.0},   {1, 16, true, 1.0}};
+// profiles/r02_lane_variants.md (sweep40 / drug).  16 warps leave the local-search kernels 128 registers (spills) and no room
+// for the chain state in shared memory.
+static const LaneVar kLaneVars[kNumLaneVars] = {{1, 8, false, 1.0, 1.0},  {2, 12, false, 1.04, 1.0}, {4, 16, false, 0.90, 0.78},
+                                                {1, 8, true, 1.02, 0.97}, {1, 12, true, 1.18, 1.21}, {1, 16, true, 1.23, 0.70}};
 #define LANE_VARIANT(v, ...)                                                      \
     switch (v) {                                                                  \
         case 0: { using C = LaneCfg<1, 8, false>; __VA_ARGS__; } break;           \
@@ -466,7 +469,7 @@ static LanePlan lane_plan(const LaneGeom& g, long long total, int jg, bool ls) {
         for (int ng = V.W / V.K; ng >= 1; --ng) {
             if (!lane_fits(g, v, ls, ng, lane_plan_images(total, jg, ng))) continue;
             const long long nctas = (total + ng - 1) / ng, waves = (nctas + g_sm_count - 1) / g_sm_count;
-            const double t = (double)waves * ng / (V.eff * (double)(ng * V.K) / V.W);
+            const double t = (double)waves * ng / ((ls ? V.eff_ls : V.eff) * (double)(ng * V.K) / V.W);
             if (t < best_t * 0.999) {
                 best_t = t;
                 best.var = v; best.ng = ng;
@@ -1556,7 +1559,7 @@ extern "C" int adock_screen(const adock_grids* grids, const adock_params* params
         const adock_ligand_desc& d = ligs[order[0]];
         const int npad = (d.N + kLaneBI - 1) / kLaneBI * kLaneBI;
         LaneGeom g{2 * (8 * d.N * d.N + 512), npad, 6 * (d.R + 1), d.R};
-        const int ng = std::max(1, lane_fit_groups(g, 0, true));
+        const int ng = std::max(1, lane_plan(g, 1 << 20, jg, true).ng);      // groups per CTA of the variant the docking will pick
         const int target = std::max(1, 3 * g_sm_count * ng / (2 * jg));
         const int nbat = (nlig + target - 1) / target;
         for (int b = 1; b < nbat; ++b) bstart.push_back((int)((long long)nlig * b / nbat));
