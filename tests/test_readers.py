@@ -75,3 +75,50 @@ def test_map_round_trip_and_geometry(W):
         RD.read_maps(["\n".join(texts[0].splitlines()[:-5]) + "\n"])
     with pytest.raises(ValueError, match="header"):
         RD.read_maps([texts[0].replace("SPACING", "SPACE")])
+
+
+# ------------------------------------------------------------------- hand-typed files in the public layouts (tests/golden)
+def _golden(name):
+    import os
+    return open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name)).read()
+
+
+def test_hand_typed_pdbqt_in_the_public_column_layout(orc):
+    """tests/golden/toy_ligand.pdbqt was typed by hand against the public PDBQT layout (PDB fixed columns: serial 7-11,
+    x 31-38, y 39-46, z 47-54, partial charge 71-76, AutoDock atom type 78-79; ROOT / ENDROOT, nested BRANCH a b /
+    ENDBRANCH a b, TORSDOF), not produced by write_pdbqt: a column mistake shared by reader and writer fails here.
+    Expected arrays typed independently below."""
+    text = _golden("toy_ligand.pdbqt")
+    # the columns, checked without the reader: atom 4 (file line 8)
+    ln = text.splitlines()[7]
+    assert ln[0:6] == "ATOM  " and ln[6:11] == "    4" and ln[30:38] == "   2.250" and ln[38:46] == "   1.299" and ln[46:54] == "   0.000"
+    assert ln[70:76] == "-0.350" and ln[77:79] == "OA"
+    names = ["C", "N", "OA", "HD"]
+    T = len(names)
+    lig = RD.read_pdbqt(text, names, np.zeros((T, T, 4), np.float32) + np.array([1, 1, 6, 0], np.float32), np.zeros(T), np.ones(T))
+    xyz = np.array([[0, 0, 0], [1.5, 0, 0], [-0.75, 1.299, 0], [2.25, 1.299, 0], [3.75, 1.299, 0], [4.5, 2.598, 0], [5.58, 2.598, 0],
+                    [-2.25, 1.299, 0]], np.float32)
+    assert lig.N == 8 and np.array_equal(lig.xyz, xyz)
+    assert np.array_equal(lig.charge, np.array([0.05, -0.02, -0.3, -0.35, 0.12, 0.01, 0.2, 0.09], np.float32))
+    assert lig.type.tolist() == [0, 0, 1, 2, 0, 0, 3, 0]
+    assert lig.root_atom == 0 and lig.R == 3
+    assert sorted(map(tuple, lig.rot_bonds.tolist())) == [(1, 3), (2, 7), (4, 5)]          # BRANCH serials 2-4, 3-8, 5-6
+    # no CONECT records: bonds from the distance rule (1.5 A heavy-atom bonds, 1.08 A C-H) plus the BRANCH bonds
+    assert sorted(map(tuple, lig.bonds.tolist())) == [(0, 1), (0, 2), (1, 3), (2, 7), (3, 4), (4, 5), (5, 6)]
+    # the oracle's preprocessing (R2) on it: 4 rigid fragments {0,1,2}, {3,4}, {5,6}, {7}; torsion 5-6 is nested in 2-4
+    ol = orc.Ligand.from_workload(lig)
+    assert ol.nfrag == 4 and ol.frag.tolist() == [0, 0, 0, 1, 1, 2, 2, 3]
+    moved = {(int(a), int(b)): ol.moved[k].nonzero()[0].tolist() for k, (a, b) in enumerate(ol.rot)}
+    assert moved == {(1, 3): [3, 4, 5, 6], (4, 5): [5, 6], (2, 7): [7]}
+
+
+def test_hand_typed_autogrid_map_in_the_public_layout():
+    """tests/golden/toy.C.map: six header lines (GRID_PARAMETER_FILE, GRID_DATA_FILE, MACROMOLECULE, SPACING, NELEMENTS =
+    numbers of INTERVALS, CENTER), then one value per line with x fastest, then y, then z; value = ix + 10 iy + 100 iz + 0.5."""
+    text = _golden("toy.C.map")
+    g = RD.read_maps([text, text, text])
+    assert g.maps.shape == (3, 3, 3, 3) and g.spacing == 0.375
+    assert np.allclose(g.origin, [1.0 - 0.375, 2.0 - 0.375, 3.0 - 0.375])                  # CENTER - spacing * NELEMENTS / 2
+    iz, iy, ix = np.meshgrid(np.arange(3), np.arange(3), np.arange(3), indexing="ij")
+    assert np.array_equal(g.maps[0], (ix + 10 * iy + 100 * iz + 0.5).astype(np.float32))    # [z][y][x]
+    assert g.maps[0][2, 1, 0] == 210.5 and g.maps[0][0, 1, 2] == 12.5
