@@ -5,6 +5,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <algorithm>
 #include <atomic>
@@ -981,7 +982,14 @@ struct LaneDockArgs {
     int ng, total_groups, jg;
     int slot_bytes, nimg;   // image slots per CTA (the most any CTA needs), slot size (multiple of 128)
     int group_floats;       // floats per lane between groups (largest ligand)
+    // queue mode of the local-search kernel (dock_ls_lane_queue_kernel): a CTA holds `tpc` teams of `jg` groups; team T of the
+    // launch docks the jobs q_job[q_off[T] .. q_off[T+1]) one after the other
+    int tpc;
+    const int* q_off;
+    const int* q_job;
 };
+constexpr int kLaneQueueHeader = 128;     // bulk-copy barrier of team t at byte 16 + 8 t (t < 7); tensor-memory address at byte 8
+constexpr int kLaneQueueMaxTeams = 7;
 struct LaneCtaGroup { int jidx, gi; const unsigned char* blob; float* scratch; bool valid; };
 template <int K>
 __device__ __forceinline__ LaneCtaGroup lane_cta_group(unsigned char* smem, const DockJob* __restrict__ jobs, const LaneDockArgs& a) {
@@ -1047,6 +1055,56 @@ __global__ void __launch_bounds__(C::kMaxWarps * 32, 1) dock_ls_lane_kernel(Grid
     const LaneCtaGroup cg = lane_cta_group<C::K>(smem, jobs, a);
     const uint32_t tmem = lane_tmem_open<C::TM>(smem);
     if (cg.valid) dock_ls_lane_group<C, SW>(G, P, jobs, dm, a, cg, tmem);     // whole groups skip: the named barriers are per group
+    lane_tmem_close<C::TM>(tmem);
+}
+
+// The same with a work queue per TEAM (the jg groups of one ligand: one image slot).  The flat partition above gives every
+// group slot exactly one group, so a launch lasts as long as its heaviest ligand and the slots of the light ones idle; here
+// the host deals the ligands of the launch (two or three per team) to the teams by estimated cost, longest first, and a
+// team stages the next ligand's image itself (bulk copy into its slot, its own mbarrier and named barrier) when it is done
+// with the previous one: the teams of a CTA never wait for each other.
+template <class C, bool SW>
+__global__ void __launch_bounds__(C::kMaxWarps * 32, 1) dock_ls_lane_queue_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs,
+                                                                                  DockDims dm, LaneDockArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tw = a.jg * C::K;                         // warps per team
+    const int team = warp / tw, wt = warp % tw;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem + 16) + team;
+    const bool leader = wt == 0 && lane == 0;
+    if (leader) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(bar)));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const uint32_t tmem = lane_tmem_open<C::TM>(smem);
+    unsigned char* slot = smem + kLaneQueueHeader + (size_t)team * a.slot_bytes;
+    float* scratch = reinterpret_cast<float*>(smem + kLaneQueueHeader + (size_t)a.tpc * a.slot_bytes);
+    const int T = blockIdx.x * a.tpc + team;
+    uint32_t phase = 0;
+    for (int q = a.q_off[T]; q < a.q_off[T + 1]; ++q) {
+        const int jidx = a.q_job[q];
+        if (leader) {
+            const int bytes = jobs[jidx].lane_bytes;
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(slot)),
+                         "l"(jobs[jidx].lane), "r"(bytes), "r"(smem_u32(bar))
+                         : "memory");
+        }
+        uint32_t done = 0;
+        while (!done) {
+            asm volatile(
+                "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                : "=r"(done)
+                : "r"(smem_u32(bar)), "r"(phase)
+                : "memory");
+        }
+        phase ^= 1u;
+        const LaneCtaGroup cg{jidx, wt / C::K, slot, scratch, true};
+        dock_ls_lane_group<C, SW>(G, P, jobs, dm, a, cg, tmem);
+        asm volatile("bar.sync %0, %1;" ::"r"(9 + team), "r"(tw * 32) : "memory");       // the team is done with this image
+    }
     lane_tmem_close<C::TM>(tmem);
 }
 
@@ -1269,12 +1327,12 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     // A ligand's docking does not depend on its position (every job carries its own buffers, seed and outputs).
     std::vector<int> jorder(nlig);
     std::iota(jorder.begin(), jorder.end(), 0);
+    std::vector<double> cost(nlig);
+    for (int l = 0; l < nlig; ++l) {
+        const LaneHeader* h = reinterpret_cast<const LaneHeader*>(ligs[l]->lane.blob.data());
+        cost[l] = 56.0 * h->nrows + 160.0 * h->N + 40.0 * h->ntiles + 1500.0;
+    }
     if (nlig > 2) {
-        std::vector<double> cost(nlig);
-        for (int l = 0; l < nlig; ++l) {
-            const LaneHeader* h = reinterpret_cast<const LaneHeader*>(ligs[l]->lane.blob.data());
-            cost[l] = 56.0 * h->nrows + 160.0 * h->N + 40.0 * h->ntiles + 1500.0;
-        }
         std::vector<int> by(nlig);
         std::iota(by.begin(), by.end(), 0);
         std::stable_sort(by.begin(), by.end(), [&](int a, int b) { return cost[a] > cost[b]; });
@@ -1322,11 +1380,66 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     // lane family: flat group sequence over all jobs (lane_plan)
     LaneDockArgs al{}, as{};
     float* d_lscratch = nullptr;
+    int q_tpc = 0, q_nctas = 0;                                 // queue mode of the local-search kernel (0: flat partition)
+    size_t q_smem = 0;
     if (ls_lane && dm.n_ls > 0) {
-        const size_t T = (size_t)pl.nctas * pl.ng * 32;
+        const size_t T = (size_t)std::max(pl.nctas, g_sm_count) * (kLaneVars[pl.var].W / kLaneVars[pl.var].K) * 32;   // either mode
         cudaError_t e2 = buf.alloc(&d_lscratch, kLaneVars[pl.var].TM ? 16 : T * (size_t)(Gmax + 2 * (Gmax - 1)) * 4);
         if (e2 != cudaSuccess) return fail(e2 == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("dock alloc: ") + cudaGetErrorString(e2));
-        al = LaneDockArgs{d_lscratch, Gmax, pl.ng, nlig * jg, jg, pl.slot, pl.nimg, pl.gfloats};
+        al = LaneDockArgs{d_lscratch, Gmax, pl.ng, nlig * jg, jg, pl.slot, pl.nimg, pl.gfloats, 0, nullptr, nullptr};
+        // queue mode: tpc teams of jg groups per CTA, as many as fit; taken when every team of a full wave gets a ligand and
+        // the ligands differ enough in cost for the balance to pay (the queue loop costs the evaluation 6 % of its speed:
+        // measured, profiles/r02_lane_variants.md)
+        const LaneVar& V = kLaneVars[pl.var];
+        const int floats = lane_var_floats(lg, pl.var, true);
+        for (int t = std::min(kLaneQueueMaxTeams, (V.W / V.K) / jg); t >= 1 && !q_tpc; --t) {
+            const size_t need = kLaneQueueHeader + (size_t)t * pl.slot + (size_t)t * jg * floats * 128;
+            const bool cols = !V.TM || 3 * lg.npad <= lane_tmem_columns(t * jg * V.K);
+            if (cols && need <= (size_t)g_smem_optin) { q_tpc = t; q_smem = need; }
+        }
+        if ((long long)nlig < (long long)q_tpc * g_sm_count) q_tpc = 0;     // fewer ligands than teams of a wave: the flat partition spreads them
+        {
+            double m = 0, v = 0;
+            for (double c : cost) m += c;
+            m /= nlig;
+            for (double c : cost) v += (c - m) * (c - m);
+            const double cv = std::sqrt(v / nlig) / m;
+            const char* force = std::getenv("ADOCK_LS_QUEUE");              // A/B switch of the profiles: 0 = flat, 1 = queue
+            if (force ? force[0] == '0' : cv < 0.08) q_tpc = 0;
+        }
+        if (q_tpc) {
+            q_nctas = std::min(g_sm_count, (nlig + q_tpc - 1) / q_tpc);
+            const int nteams = q_nctas * q_tpc;
+            // longest processing time first: jobs by decreasing cost, each to the CTA with the least work so far (the warps
+            // of an SM share its issue slots) and there to the least loaded team
+            std::vector<int> by(nlig);
+            std::iota(by.begin(), by.end(), 0);
+            std::stable_sort(by.begin(), by.end(), [&](int x, int y) { return cost[jorder[x]] > cost[jorder[y]]; });
+            std::vector<double> load(nteams, 0.0), cta_load(q_nctas, 0.0);
+            std::vector<std::vector<int>> q(nteams);
+            for (int k : by) {
+                const int c = (int)(std::min_element(cta_load.begin(), cta_load.end()) - cta_load.begin());
+                const int tmin = (int)(std::min_element(load.begin() + c * q_tpc, load.begin() + (c + 1) * q_tpc) - load.begin());
+                q[tmin].push_back(k);                           // k = position in jobs[]
+                load[tmin] += cost[jorder[k]];
+                cta_load[c] += cost[jorder[k]];
+            }
+            std::vector<int> off(nteams + 1, 0), flat;
+            for (int t = 0; t < nteams; ++t) { flat.insert(flat.end(), q[t].begin(), q[t].end()); off[t + 1] = (int)flat.size(); }
+            int *d_off = nullptr, *d_q = nullptr;
+            e2 = buf.alloc(&d_off, off.size() * 4);
+            if (e2 == cudaSuccess) e2 = buf.alloc(&d_q, flat.size() * 4);
+            if (e2 == cudaSuccess) e2 = cudaMemcpyAsync(d_off, off.data(), off.size() * 4, cudaMemcpyHostToDevice, stm);
+            if (e2 == cudaSuccess) e2 = cudaMemcpyAsync(d_q, flat.data(), flat.size() * 4, cudaMemcpyHostToDevice, stm);
+            if (e2 == cudaSuccess) e2 = cudaStreamSynchronize(stm);     // off / flat leave scope
+            if (e2 != cudaSuccess) return fail(ADOCK_ECUDA, std::string("dock queue: ") + cudaGetErrorString(e2));
+            al.ng = q_tpc * jg; al.nimg = q_tpc; al.tpc = q_tpc; al.q_off = d_off; al.q_job = d_q;
+            al.group_floats = floats;
+            cudaError_t e4 = cudaSuccess;
+            LANE_VARIANT(pl.var, e4 = cudaFuncSetAttribute(dock_ls_lane_queue_kernel<C, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)q_smem);
+                         if (e4 == cudaSuccess) e4 = cudaFuncSetAttribute(dock_ls_lane_queue_kernel<C, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)q_smem))
+            CUDA_TRY(e4);
+        }
         cudaError_t e3 = cudaSuccess;
         LANE_VARIANT(pl.var, e3 = cudaFuncSetAttribute(dock_ls_lane_kernel<C, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
                      if (e3 == cudaSuccess) e3 = cudaFuncSetAttribute(dock_ls_lane_kernel<C, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem))
@@ -1342,7 +1455,9 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     auto launch_ls = [&]() {
         const int thr = pl.ng * pl.K * 32;
         const bool sw = p.ls_method == 1;
-        if (ls_lane && !sw) { LANE_VARIANT(pl.var, dock_ls_lane_kernel<C, false><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al)) }
+        if (ls_lane && q_tpc && !sw) { LANE_VARIANT(pl.var, dock_ls_lane_queue_kernel<C, false><<<q_nctas, q_tpc * jg * C::K * 32, q_smem, stm>>>(grids->dev, P, d_jobs, dm, al)) }
+        else if (ls_lane && q_tpc) { LANE_VARIANT(pl.var, dock_ls_lane_queue_kernel<C, true><<<q_nctas, q_tpc * jg * C::K * 32, q_smem, stm>>>(grids->dev, P, d_jobs, dm, al)) }
+        else if (ls_lane && !sw) { LANE_VARIANT(pl.var, dock_ls_lane_kernel<C, false><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al)) }
         else if (ls_lane) { LANE_VARIANT(pl.var, dock_ls_lane_kernel<C, true><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al)) }
         else if (ls_team) dock_ls_team_kernel<<<dteam.upj * nlig, kTeamW * 32, smem_team, stm>>>(grids->dev, P, d_jobs, dteam);
         else dock_ls_kernel<<<dls.upj * nlig, Wls * 32, smem_ls, stm>>>(grids->dev, P, d_jobs, dls);

@@ -817,33 +817,36 @@ def test_pose_rmsd_and_clustering_match_oracle(B, orc, cases):
 
 
 def test_dock_bench_launch_configuration_sampled(B, W, orc):
-    """the launch configuration bench.py times (197 drug-like ligands x 20 runs x pop 150 in one adock_dock_many call:
-    lane-per-individual local search and offspring scoring, several ligand images per CTA), for three generations;
-    sampled ligands: reported energy = oracle energy of the reported genotype, eval accounting, and the same ligand
-    docked alone in the same kernel family gives the same result."""
+    """the launch configuration bench.py times (two drug-like ligands per SM and a ragged 37 more, x 20 runs x pop 150 in
+    one adock_dock_many call: lane-per-individual local search with the positions in tensor memory, one work queue per team
+    of six warps (some teams dock two ligands), lane-per-individual offspring scoring), for three generations; sampled
+    ligands: reported energy = oracle energy of the reported genotype, eval accounting, and the same ligand docked alone in
+    the same kernel variant (flat partition, one CTA) gives the same result bit for bit."""
     grids, lig0 = W.make_config("drug")
     centre = 0.5 * (grids.box_lo + grids.box_hi); c = W.CONFIGS["drug"]
-    ligs = W.share_type_table([W.make_ligand(c["N"], c["R"], c["T"], 100 + i, centre) for i in range(197)])
+    nl = 2 * torch.cuda.get_device_properties(0).multi_processor_count + 37
+    ligs = W.share_type_table([W.make_ligand(c["N"], c["R"], c["T"], 100 + i, centre) for i in range(nl)])
     gp, op = B.make_params(W.DEFAULT_PARAMS), orc.params(W.DEFAULT_PARAMS)
     gg = B.Grids.from_workload(grids); og = orc.Grids.from_workload(grids)
     gl = [B.Ligand.from_workload(gg, l, gp) for l in ligs]
     P, nrun = 150, 20
     max_evals = P + 2 * (P - 1 + 9 * 300) + 1                                  # ends after generation 3
-    seeds = [5000 + i for i in range(197)]
+    seeds = [5000 + i for i in range(nl)]
     B.adock_set_path("auto")
     r = B.adock_dock_many(gg, gl, gp, nrun, P, max_evals, seeds)
     assert B.lib().adock_last_dock_path() == 2
     assert (r["gens"] == 3).all() and (r["evals"] == P + 3 * (P - 1 + 9 * 300)).all()
-    for i in (0, 57, 131, 196):
+    for i in (0, 57, 131, nl - 1):
         l = ligs[i]
         chk = orc.score(og, orc.Ligand.from_workload(l), op, r["genotypes"][i][:, :7 + l.R], want_grad=False)["E"]
         assert_energy(r["energies"][i], chk, f"bench-configuration ligand {i}")
-    B.adock_set_path("lane1")
+    B.adock_set_path("tm12")
     try:
-        s = B.adock_dock(gg, gl[57], gp, nrun, P, max_evals, seed=seeds[57], want_coords=False)
+        for i in (57, nl - 1):
+            s = B.adock_dock(gg, gl[i], gp, nrun, P, max_evals, seed=seeds[i], want_coords=False)
+            assert np.array_equal(s["energies"], r["energies"][i]) and np.array_equal(s["genotypes"], r["genotypes"][i][:, :7 + ligs[i].R])
     finally:
         B.adock_set_path("auto")
-    assert np.array_equal(s["energies"], r["energies"][57]) and np.array_equal(s["genotypes"], r["genotypes"][57][:, :7 + ligs[57].R])
 
 
 def test_score_matches_golden_fixture(B, cases, dev, family):
