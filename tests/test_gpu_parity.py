@@ -833,7 +833,13 @@ def test_dock_bench_launch_configuration_sampled(B, W, orc):
     max_evals = P + 2 * (P - 1 + 9 * 300) + 1                                  # ends after generation 3
     seeds = [5000 + i for i in range(nl)]
     B.adock_set_path("auto")
-    r = B.adock_dock_many(gg, gl, gp, nrun, P, max_evals, seeds)
+    os.environ["ADOCK_LS_QUEUE"] = "1"          # the queue mode is chosen by the cost spread of the launch (screening); forced here
+    try:
+        r = B.adock_dock_many(gg, gl, gp, nrun, P, max_evals, seeds)
+    finally:
+        del os.environ["ADOCK_LS_QUEUE"]
+    r_flat = B.adock_dock_many(gg, gl, gp, nrun, P, max_evals, seeds)          # these ligands differ little: flat partition
+    assert np.array_equal(r["energies"], r_flat["energies"]) and np.array_equal(r["genotypes"], r_flat["genotypes"])
     assert B.lib().adock_last_dock_path() == 2
     assert (r["gens"] == 3).all() and (r["evals"] == P + 3 * (P - 1 + 9 * 300)).all()
     for i in (0, 57, 131, nl - 1):
