@@ -431,6 +431,7 @@ def probe(argv):
         python bench.py --probe large <path> [max_evals]                               # adock_dock, configs[3]
         python bench.py --probe screen <ligands> <batch>                               # adock_screen, configs[2] sample
         python bench.py --probe alu                                                    # adock_alu_peak
+        python bench.py --probe tmem                                                   # adock_tmem_probe (tensor memory as per-lane scratch)
 
     <path> is the argument of adock_set_path: 0 auto, 1 warp per individual, 2 / 21 / 22 / 24 lane per individual
     (K chosen / 1 / 2 / 4 warps per group), 3 team per individual.  Prints one line; not the bench contract."""
@@ -440,6 +441,16 @@ def probe(argv):
     dev = torch.device("cuda:0")
     if mode == "alu":
         print(B.adock_alu_peak(), flush=True)
+    elif mode == "tmem":
+        names = {1: "tensor memory, dependent tcgen05.ld.x1", 3: "shared memory, dependent LDS.32", 2: "tensor memory, 8 x tcgen05.ld.x2", 4: "shared memory, 8 x LDS.64"}
+        for w in (4, 8, 12):
+            r = B.adock_tmem_probe(w, 0)
+            print(f"W={w:2d} write / read-back of every column (.x1, .x4 + .x2 at columns 6m): errors = {r['errors']}", flush=True)
+            for m in (1, 3):
+                print(f"W={w:2d} {names[m]:40s} {B.adock_tmem_probe(w, m)['cycles_per_iteration']:.1f} cycles per load", flush=True)
+            for m in (2, 4):
+                c = B.adock_tmem_probe(w, m)["cycles_per_iteration"]
+                print(f"W={w:2d} {names[m]:40s} {c:.1f} cycles per 8 loads and warp = {w * 8 * 256 / c:.0f} B/clk/SM", flush=True)
     elif mode == "score":
         cfg, n, path = argv[1], int(argv[2]), int(argv[3])
         reps = int(argv[4]) if len(argv) > 4 else 10

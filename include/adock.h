@@ -241,6 +241,14 @@ int adock_profile_read(double* ls_ms, long long* ls_launches, long long* ls_eval
  * lane and clock).  Synchronous.  MEASURED_PEAKS.json carries HBM and tensor figures only; bench.py reports this one. */
 int adock_alu_peak(double* tflops, double* fma_lanes_per_clk_sm, void* cuda_stream);
 
+/* Measurement behind the TM variants of the lane kernels (atom positions in tensor memory, addressed
+ * thread i <-> lane i of the warp's quarter with a warp-uniform column): one CTA of `warps` (1..12) warps per SM.
+ * mode 0: write / read-back of every column of every warp's slice with tcgen05.st / tcgen05.ld (.x1, and .x4 + .x2 at
+ * columns 6m, the position layout): *errors = mismatches (must be 0).  mode 1 / 3: dependent-load latency of tensor memory /
+ * shared memory, cycles per load.  mode 2 / 4: 8 independent 64-bit loads per iteration from tensor memory / shared memory,
+ * cycles per iteration and warp.  Synchronous.  profiles/r02_tmem_scratch.md holds the numbers of this pool's B200. */
+int adock_tmem_probe(int warps, int mode, int iters, int* errors, double* cycles_per_iteration, void* cuda_stream);
+
 /* Kernel launches issued by this library on the calling thread since the last reset (bench accounting). */
 long long adock_launch_count(int reset);
 

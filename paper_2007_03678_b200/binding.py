@@ -19,7 +19,7 @@ ADOCK_OK, ADOCK_EINVAL, ADOCK_ENOMEM, ADOCK_ECUDA, ADOCK_ELIMIT = 0, -1, -2, -3,
 EXPORTS = ["adock_default_params", "adock_load_grids", "adock_free_grids", "adock_load_ligand", "adock_free_ligand",
            "adock_ligand_pairs", "adock_ligand_tree", "adock_ligand_image", "adock_score_batch", "adock_score_batch_host", "adock_local_search",
            "adock_philox", "adock_ga_generation", "adock_dock", "adock_dock_many", "adock_launch_count", "adock_last_error", "adock_profile", "adock_profile_read",
-           "adock_ligand_lane_image", "adock_set_path", "adock_last_dock_path", "adock_solis_wets", "adock_screen", "adock_pose_rmsd", "adock_alu_peak"]
+           "adock_ligand_lane_image", "adock_set_path", "adock_last_dock_path", "adock_solis_wets", "adock_screen", "adock_pose_rmsd", "adock_alu_peak", "adock_tmem_probe"]
 
 
 class adock_ligand_desc(C.Structure):
@@ -362,6 +362,14 @@ def adock_alu_peak() -> dict:
     lib().adock_alu_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p]
     _check(lib().adock_alu_peak(C.byref(t), C.byref(l), _stream()))
     return dict(tflops=t.value, fma_lanes_per_clk_sm=l.value)
+
+
+def adock_tmem_probe(warps: int, mode: int, iters: int = 20000) -> dict:
+    """tensor memory as per-lane scratch (include/adock.h): dict(errors, cycles_per_iteration)"""
+    err, cyc = C.c_int(), C.c_double()
+    lib().adock_tmem_probe.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_double), C.c_void_p]
+    _check(lib().adock_tmem_probe(int(warps), int(mode), int(iters), C.byref(err), C.byref(cyc), _stream()))
+    return dict(errors=err.value, cycles_per_iteration=cyc.value)
 
 
 def adock_launch_count(reset: bool = False) -> int:

@@ -1923,3 +1923,110 @@ extern "C" int adock_alu_peak(double* tflops, double* fma_lanes_per_clk_sm, void
     if (fma_lanes_per_clk_sm) *fma_lanes_per_clk_sm = lanes / (best * 1e-3 * khz * 1e3) / g_sm_count;
     return ADOCK_OK;
 }
+
+// =================================================================== tensor memory as per-lane scratch: the measurement
+// The TM variants of the lane kernels keep atom positions in tensor memory (lane.cuh).  This probe is the evidence that the
+// access pattern is sound and what it costs (profiles/r02_tmem_scratch.md): every warp of a CTA of `warps` warps writes a
+// pattern into its slice with tcgen05.st.32x32b and reads it back with .x1 / .x2 / .x4 loads at warp-uniform dynamic
+// columns (mode 0: mismatches counted); a pointer chase gives the dependent-load latency (mode 1: tensor memory, mode 3:
+// shared memory), 8 independent 64-bit loads per wait the throughput (mode 2: tcgen05.ld.x2, mode 4: LDS.64).
+template <int mode>
+__global__ void __launch_bounds__(512, 1) tmem_probe_kernel(int iters, int* errors, long long* cycles, float* sink) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
+    const uint32_t tmem = lane_tmem_open<true>(smem);
+    const int per = lane_tmem_columns(W);
+    const uint32_t mine = tmem + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * per);
+    float* sm = reinterpret_cast<float*>(smem + 16) + (size_t)warp * 128 * 32 + lane;        // 128 columns per lane
+    int err = 0;
+    long long t0 = 0, t1 = 0;
+    float acc = 0.f;
+    if (mode == 0) {
+        for (int c = 0; c < per; ++c) tm_st1(mine + c, (float)(warp * 4099 + lane * 67 + c));
+        tm_wait_st();
+        for (int c = per - 1; c >= 0; --c) {
+            float v, d0 = 0.f, d1 = 0.f;
+            tm_ld1(mine + c, v);
+            tm_wait_ld(v, d0, d1);
+            if (v != (float)(warp * 4099 + lane * 67 + c)) ++err;
+        }
+        for (int m = 0; 6 * m + 5 < per; ++m) {             // the position layout: .x4 at column 6m, .x2 at 6m + 4
+            float a, b, c, d, e, f;
+            tm_ld4(mine + 6 * m, a, b, c, d);
+            tm_ld2(mine + 6 * m + 4, e, f);
+            tm_wait_ld(a, b, c, d, e, f);
+            const float base = (float)(warp * 4099 + lane * 67 + 6 * m);
+            if (a != base || b != base + 1 || c != base + 2 || d != base + 3 || e != base + 4 || f != base + 5) ++err;
+        }
+    } else if (mode == 1 || mode == 3) {
+        for (int c = 0; c < 128; ++c) {
+            const float nxt = __int_as_float((c * 37 + 11) & 127);        // the next column, as raw bits (no conversion in the chase)
+            if (mode == 1) tm_st1(mine + c, nxt); else sm[c * 32] = nxt;
+        }
+        tm_wait_st();
+        __syncwarp();
+        int c = 0;
+        t0 = clock64();
+        for (int i = 0; i < iters; ++i) {
+            float v, d0 = 0.f, d1 = 0.f;
+            if (mode == 1) { tm_ld1(mine + c, v); tm_wait_ld(v, d0, d1); } else v = sm[c * 32];
+            c = __float_as_int(v);
+        }
+        t1 = clock64();
+        acc = (float)c;
+    } else {
+        for (int c = 0; c < 128; ++c) { tm_st1(mine + c, 1.0f + c); sm[c * 32] = 1.0f + c; }
+        tm_wait_st();
+        __syncwarp();
+        t0 = clock64();
+        for (int i = 0; i < iters; ++i) {
+            float v[16];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const int c = ((i + k * 6) & 63) * 2;
+                if (mode == 2) tm_ld2(mine + c, v[2 * k], v[2 * k + 1]);
+                else { const float2 q = *reinterpret_cast<const float2*>(reinterpret_cast<const float*>(smem + 16) + ((size_t)warp * 64 + (c >> 1)) * 64 + 2 * lane); v[2 * k] = q.x; v[2 * k + 1] = q.y; }
+            }
+            if (mode == 2) { tm_wait_ld(v[0], v[1], v[2], v[3], v[4], v[5], v[6], v[7], v[8], v[9], v[10], v[11]); tm_wait_ld(v[12], v[13], v[14]); }
+#pragma unroll
+            for (int k = 0; k < 16; ++k) acc += v[k];
+        }
+        t1 = clock64();
+    }
+    if (err) atomicAdd(errors, err);
+    if (lane == 0) cycles[blockIdx.x * W + warp] = t1 - t0;
+    sink[blockIdx.x * blockDim.x + threadIdx.x] = acc;
+    lane_tmem_close<true>(tmem);
+}
+
+extern "C" int adock_tmem_probe(int warps, int mode, int iters, int* errors, double* cycles_per_iteration, void* cuda_stream) {
+    if (warps < 1 || warps > 12 || mode < 0 || mode > 4 || iters < 1) return fail(ADOCK_EINVAL, "tmem probe: warps 1..12, mode 0..4, iters >= 1");
+    int rc = device_props();
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t smem = 16 + (size_t)warps * 128 * 32 * 4;
+    int* d_err = nullptr; long long* d_cyc = nullptr; float* d_sink = nullptr;
+    cudaError_t e = cudaMalloc(&d_err, 4);
+    if (e == cudaSuccess) e = cudaMalloc(&d_cyc, (size_t)g_sm_count * warps * 8);
+    if (e == cudaSuccess) e = cudaMalloc(&d_sink, (size_t)g_sm_count * warps * 32 * 4);
+    if (e == cudaSuccess) e = cudaMemsetAsync(d_err, 0, 4, st);
+    auto kern = mode == 0 ? tmem_probe_kernel<0> : mode == 1 ? tmem_probe_kernel<1> : mode == 2 ? tmem_probe_kernel<2> : mode == 3 ? tmem_probe_kernel<3> : tmem_probe_kernel<4>;
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    std::vector<long long> cyc((size_t)g_sm_count * warps);
+    int h_err = 0;
+    if (e == cudaSuccess) {
+        kern<<<g_sm_count, warps * 32, smem, st>>>(iters, d_err, d_cyc, d_sink);
+        ++g_launches;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&h_err, d_err, 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(cyc.data(), d_cyc, cyc.size() * 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d_err); cudaFree(d_cyc); cudaFree(d_sink);
+    if (e != cudaSuccess) return fail(ADOCK_ECUDA, std::string("tmem probe: ") + cudaGetErrorString(e));
+    double mean = 0;
+    for (long long c : cyc) mean += (double)c;
+    if (errors) *errors = h_err;
+    if (cycles_per_iteration) *cycles_per_iteration = mean / (double)cyc.size() / iters;
+    return ADOCK_OK;
+}

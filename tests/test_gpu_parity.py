@@ -891,3 +891,14 @@ def test_reader_output_runs_through_the_gpu_path(B, W, orc, dev):
     assert_energy(d_E.cpu().numpy(), ref["E"], "reader -> GPU")
     ok = (ref["margins"][:, 0] > 1e-3) & (ref["margins"][:, 1] > 1e-3)
     assert_gradient(d_gr.cpu().numpy(), ref, lig2.R, ok, "reader -> GPU")
+
+
+@pytest.mark.gpu
+def test_tensor_memory_scratch_reads_back(B):
+    """the access pattern of the TM variants: every column of every warp's slice of tensor memory,
+    written with tcgen05.st.32x32b and read back with .x1 and with .x4 + .x2 at columns 6m, thread i <-> lane i"""
+    for warps in (1, 4, 8, 12):
+        assert B.adock_tmem_probe(warps, 0)["errors"] == 0
+    lat_t, lat_s = B.adock_tmem_probe(8, 1, 2000)["cycles_per_iteration"], B.adock_tmem_probe(8, 3, 2000)["cycles_per_iteration"]
+    print(f"dependent load: tensor memory {lat_t:.1f} cycles, shared memory {lat_s:.1f} cycles")
+    assert 5 < lat_t < 200 and 5 < lat_s < 200
