@@ -941,18 +941,25 @@ __global__ void __launch_bounds__(128) dock_ls_kernel(GridDev G, ParDev P, const
     }
 }
 
-// ADADELTA with one TEAM (CTA of kTeamW warps) per chain: launches with too few chains to give every scheduler a warp.
-// 5 CTAs per SM (<= 102 registers): 4 ligands x 180 chains are one wave; at 4 CTAs per SM they were two (1.85 s -> 3.08 s).
-__global__ void __launch_bounds__(kTeamW * 32, 5) dock_ls_team_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs, DockDims dm) {
+// ADADELTA with one TEAM (kTeamW warps) per chain: launches with too few chains to give every scheduler a warp.
+// TPC teams share a CTA and its ligand image.  TPC = 1: 5 CTAs per SM (<= 102 registers): 4 ligands x 180 chains are one
+// wave; at 4 CTAs per SM they were two (1.85 s -> 3.08 s).  TPC = 4 (one CTA per SM, <= 128 registers): ligands whose image
+// fills most of the shared memory (128 atoms: 117 KB of pair records), where one team per CTA left three of the four
+// schedulers of an SM without a warp.
+template <int TPC>
+__global__ void __launch_bounds__(TPC * kTeamW * 32, TPC == 1 ? 5 : 1) dock_ls_team_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs,
+                                                                                          DockDims dm, int team_floats) {
     extern __shared__ __align__(128) unsigned char smem[];
     const DockJob job = jobs[blockIdx.x / dm.upj];
     unsigned char* blob = smem + 16;
     stage_ligand(blob, job.blob, job.blob_bytes, reinterpret_cast<uint64_t*>(smem), 0);
     const LigS L = lig_view(blob);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const TeamS T = team_view(reinterpret_cast<float*>(blob + job.blob_bytes), L, warp);
-    const int ind = blockIdx.x % dm.upj, Gn = job.Gn;
-    if (ind >= dm.nrun * dm.n_ls) return;
+    const int team = warp / kTeamW;
+    TeamS T = team_view(reinterpret_cast<float*>(blob + job.blob_bytes) + (size_t)team * team_floats, L, warp % kTeamW);
+    T.bar = 1 + team;
+    const int ind = (blockIdx.x % dm.upj) * TPC + team, Gn = job.Gn;
+    if (ind >= dm.nrun * dm.n_ls) return;               // whole teams leave: the barriers below are per team
     const int run = ind / dm.n_ls, l = ind % dm.n_ls;
     const RunState st = job.st[run];
     if (!st.active) return;
@@ -960,11 +967,11 @@ __global__ void __launch_bounds__(kTeamW * 32, 5) dock_ls_team_kernel(GridDev G,
     const int slot = job.picks[(size_t)run * dm.P + l];
     float* g = job.pop + ((size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P + slot) * Gn;
     float* e = job.E + (size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P + slot;
-    if (warp == 0) for (int d = lane; d < Gn; d += 32) T.S.geno[d] = g[d];
-    __syncthreads();
+    if (T.wi == 0) for (int d = lane; d < Gn; d += 32) T.S.geno[d] = g[d];
+    team_sync(T);
     int iters = 0;
     const float be = adadelta_search_team(L, G, P, T, lane, *e, iters);
-    if (warp == 0) {
+    if (T.wi == 0) {
         for (int d = lane; d < Gn; d += 32) g[d] = T.S.best[d];
         if (lane == 0) {
             *e = be;
@@ -1289,7 +1296,9 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     const bool ls_lane = pl.var >= 0 && (g_path == 2 || (many && p.ls_method == 0));
     if (g_path == 2 && pl.var < 0) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
     // a team (CTA of kTeamW warps) per chain when one warp per chain would leave most schedulers without a warp
-    const size_t smem_team = 16 + (size_t)maxblob + (size_t)maxteam * 4;
+    // teams per CTA: one where five CTAs fit an SM anyway (small images), four where the image lets only one CTA in
+    const int team_tpc = (5 * (16 + (size_t)maxblob + (size_t)maxteam * 4) <= (size_t)g_smem_optin || 16 + (size_t)maxblob + 4 * (size_t)maxteam * 4 > (size_t)g_smem_optin) ? 1 : 4;
+    const size_t smem_team = 16 + (size_t)maxblob + (size_t)team_tpc * maxteam * 4;
     const bool ls_team = !ls_lane && p.ls_method == 0 && smem_team <= (size_t)g_smem_optin &&
                          (g_path == 3 || (g_path == 0 && chains <= (long long)g_sm_count * 6));   // measured cross-over: 4..8 ligands x 180 chains
     g_last_dock_path = ls_lane ? 2 : ls_team ? 3 : 1;
@@ -1372,8 +1381,9 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     CUDA_TRY(cudaFuncSetAttribute(dock_final_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ls));
 
     DockDims dga = dm, dls = dm, dfin = dm, dteam = dm;
-    dteam.upj = std::max(1, nrun * dm.n_ls);                    // one CTA per chain
-    if (ls_team) CUDA_TRY(cudaFuncSetAttribute(dock_ls_team_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_team));
+    dteam.upj = std::max(1, (nrun * dm.n_ls + team_tpc - 1) / team_tpc);     // team_tpc chains per CTA
+    if (ls_team && team_tpc == 1) CUDA_TRY(cudaFuncSetAttribute(dock_ls_team_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_team));
+    if (ls_team && team_tpc == 4) CUDA_TRY(cudaFuncSetAttribute(dock_ls_team_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_team));
     dga.upj = (int)((popsz + Wga - 1) / Wga);
     dls.upj = std::max(1, (nrun * dm.n_ls + Wls - 1) / Wls);
     dfin.upj = (nrun + Wls - 1) / Wls;
@@ -1459,7 +1469,8 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         else if (ls_lane && q_tpc) { LANE_VARIANT(pl.var, dock_ls_lane_queue_kernel<C, true><<<q_nctas, q_tpc * jg * C::K * 32, q_smem, stm>>>(grids->dev, P, d_jobs, dm, al)) }
         else if (ls_lane && !sw) { LANE_VARIANT(pl.var, dock_ls_lane_kernel<C, false><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al)) }
         else if (ls_lane) { LANE_VARIANT(pl.var, dock_ls_lane_kernel<C, true><<<pl.nctas, thr, pl.smem, stm>>>(grids->dev, P, d_jobs, dm, al)) }
-        else if (ls_team) dock_ls_team_kernel<<<dteam.upj * nlig, kTeamW * 32, smem_team, stm>>>(grids->dev, P, d_jobs, dteam);
+        else if (ls_team && team_tpc == 1) dock_ls_team_kernel<1><<<dteam.upj * nlig, kTeamW * 32, smem_team, stm>>>(grids->dev, P, d_jobs, dteam, maxteam);
+        else if (ls_team) dock_ls_team_kernel<4><<<dteam.upj * nlig, 4 * kTeamW * 32, smem_team, stm>>>(grids->dev, P, d_jobs, dteam, maxteam);
         else dock_ls_kernel<<<dls.upj * nlig, Wls * 32, smem_ls, stm>>>(grids->dev, P, d_jobs, dls);
     };
     // one GA generation: offspring + their energies (one launch, or two when the scoring runs lane-per-individual)
@@ -1668,14 +1679,14 @@ extern "C" int adock_screen(const adock_grids* grids, const adock_params* params
         if (rc) return rc;
         const int jg = std::max(1, (nrun * n_ls_of(pp, pop_size) + 31) / 32);
         // geometry of the largest ligand (first in the order), estimated from its descriptor: image ~ 7.6 N^2 bytes (two
-        // slots), 6 accumulator floats per fragment.  Batch length = 1.5 waves of groups at that geometry (the ligands
-        // further down the order are smaller; measured on configs[2]: profiles/r01d_next_rows.md), equalised over the
-        // batches so that no small tail batch falls back to the warp-per-individual kernels.
+        // slots), 6 accumulator floats per fragment.  Batch length = two ligands per team of the local-search kernel at that
+        // geometry (its work queues balance them by cost; measured on configs[2]: profiles/r02_lane_variants.md), equalised
+        // over the batches so that no small tail batch falls back to the warp-per-individual kernels.
         const adock_ligand_desc& d = ligs[order[0]];
         const int npad = (d.N + kLaneBI - 1) / kLaneBI * kLaneBI;
         LaneGeom g{2 * (8 * d.N * d.N + 512), npad, 6 * (d.R + 1), d.R};
         const int ng = std::max(1, lane_plan(g, 1 << 20, jg, true).ng);      // groups per CTA of the variant the docking will pick
-        const int target = std::max(1, 3 * g_sm_count * ng / (2 * jg));
+        const int target = std::max(1, 2 * g_sm_count * ng / jg);
         const int nbat = (nlig + target - 1) / target;
         for (int b = 1; b < nbat; ++b) bstart.push_back((int)((long long)nlig * b / nbat));
     }

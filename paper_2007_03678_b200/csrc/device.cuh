@@ -605,7 +605,7 @@ __device__ inline void ga_make_child(const ParDev& P, int Pn, int R, unsigned lo
 }
 
 // ---------------------------------------------------------------- full evaluation of one genotype by a TEAM of W warps
-// One CTA-sized team per individual, threads over atoms and pairs: for launches with so few chains that one warp per
+// One team of kTeamW warps per individual (one or four teams per CTA, sharing the ligand image), threads over atoms and pairs: for launches with so few chains that one warp per
 // chain leaves most schedulers idle (a single ligand: 180 chains on 592 schedulers), the evaluation itself is split.
 // Warp 0 builds the fragment transforms; the 32 W threads take one atom each (pose + grid lookup); warp w takes the pair
 // rounds r = w (mod W) and adds their forces into its own gradient plane (plane 0 = S.blk's gx|gy|gz, planes 1..W-1 in
@@ -616,16 +616,16 @@ __host__ __device__ inline int team_scratch_floats(int N, int nfrag, int R) {
     return warp_scratch_floats(N, nfrag, R) + (kTeamW - 1) * ((N + 31) / 32) * 96 + 8 * kTeamW + 8;
 }
 // red: per warp w [8w .. 8w+8) = partial (e_grid, e_pairs, grid force F(3), grid torque about t T(3)); [8 kTeamW] = flag
-struct TeamS { WarpS S; float* gextra; float* red; int wi, gplane; };     // gplane = floats per extra plane
+struct TeamS { WarpS S; float* gextra; float* red; int wi, gplane, bar; };     // gplane = floats per extra plane; bar = the team's named barrier
 __device__ inline TeamS team_view(float* base, const LigS& L, int wi) {
     TeamS T;
     T.S = warp_view(base, L);
     T.gextra = T.S.blk + (L.npos / 32) * 256;
     T.red = T.gextra + (kTeamW - 1) * (L.npos / 32) * 96;
-    T.wi = wi; T.gplane = (L.npos / 32) * 96;
+    T.wi = wi; T.gplane = (L.npos / 32) * 96; T.bar = 1;
     return T;
 }
-__device__ __forceinline__ void team_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kTeamW * 32) : "memory"); }
+__device__ __forceinline__ void team_sync(const TeamS& T) { asm volatile("bar.sync %0, %1;" ::"r"(T.bar), "n"(kTeamW * 32) : "memory"); }
 // gradient words of the atom at blk offset `off` in plane w: +0, +32, +64
 __device__ __forceinline__ float* team_gptr(const TeamS& T, int w, int off) {
     return w == 0 ? T.S.blk + off + kGX : T.gextra + (w - 1) * T.gplane + (off >> 8) * 96 + (off & 31);
@@ -642,7 +642,7 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
     if (!(qn2 >= 1e-24f)) {                             // the same in every thread of the team
         if (GRAD && wi == 0) for (int d = lane; d < 6 + L.R; d += 32) S.grad[d] = __int_as_float(0x7fc00000);
         e_inter = e_intra = __int_as_float(0x7fc00000);
-        team_sync();
+        team_sync(T);
         return __int_as_float(0x7fc00000);
     }
     if (wi == 0) {                                      // (a1) fragment transforms: eval_pose's code on warp 0
@@ -692,7 +692,7 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
             }
         }
     }
-    team_sync();
+    team_sync(T);
     // (a1,a2) atoms: one thread per position (pose + trilinear lookup); the owner also clears the atom's extra planes
     float eg = 0.f, rFx = 0.f, rFy = 0.f, rFz = 0.f, rTx = 0.f, rTy = 0.f, rTz = 0.f;     // rigid-body sums: grid forces only (eval_pose)
     for (int i = wi * 32 + lane; i < L.npos; i += 32 * kTeamW) {
@@ -726,7 +726,7 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
             r[0] = rFx; r[1] = rFy; r[2] = rFz; r[3] = rTx; r[4] = rTy; r[5] = rTz;
         }
     }
-    team_sync();
+    team_sync(T);
 
     // (a3) intramolecular pairs: warp wi takes rounds wi, wi + W, ...; forces go to plane wi
     float ep = 0.f;
@@ -743,7 +743,7 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
     }
     eg = warp_sum(eg); ep = warp_sum(ep);
     if (lane == 0) { T.red[8 * wi] = eg; T.red[8 * wi + 1] = ep; }
-    team_sync();
+    team_sync(T);
     e_inter = 0.f; e_intra = 0.f;
 #pragma unroll
     for (int w = 0; w < kTeamW; ++w) { e_inter += T.red[8 * w]; e_intra += T.red[8 * w + 1]; }
@@ -760,7 +760,7 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
             for (int w = 1; w < kTeamW; ++w) { const float* g = team_gptr(T, w, off); gx += g[0]; gy += g[32]; gz += g[64]; }
             b[kGX] = gx; b[kGY] = gy; b[kGZ] = gz;
         }
-        team_sync();
+        team_sync(T);
         if (wi == 0) {
             for (int f = lane; f < L.nfrag; f += 32) {
                 const int4 ix = L.fi[f];
@@ -804,7 +804,7 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
                 }
             }
         }
-        team_sync();
+        team_sync(T);
     }
     return e_inter + e_intra;
 }
@@ -945,7 +945,7 @@ __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, co
                 if (lane == 3) { S.geno[3] = newq[0]; S.geno[4] = newq[1]; S.geno[5] = newq[2]; S.geno[6] = newq[3]; }
             }
         }
-        team_sync();                                    // new genotype and the flag are visible
+        team_sync(T);                                    // new genotype and the flag are visible
         if (T.red[8 * kTeamW] == 0.f) break;
     }
     iters = it;
