@@ -488,11 +488,18 @@ static LanePlan lane_plan(const LaneGeom& g, long long total, int jg, bool ls) {
 }
 // variant for `ngroups` groups of 32 individuals of one ligand (-1: none fits)
 static int lane_pick_var(const LaneGeom& g, long long ngroups, bool ls) { return lane_plan(g, ngroups, (int)std::min<long long>(ngroups, 1 << 30), ls).var; }
-// groups per CTA: as many as fit, fewer when that would leave SMs idle
-static int lane_spread_groups(int fit, long long ngroups) {
-    int n = fit;
-    while (n > 1 && (long long)g_sm_count * n > ngroups) --n;
-    return n;
+// groups per CTA of a launch of `ngroups` groups on one CTA per SM (each looping over its share, or wave after wave):
+// passes x time of a pass, where an SM with w = n K resident warps works at w / (w + 4) of its full rate (fitted to the
+// measured variants: 8 / 12 / 16 warps = 0.83 / 0.94 / 1 of the 16-warp rate), i.e. a pass of n groups lasts ~ n K + 4
+static int lane_spread_groups(int fit, long long ngroups, int K) {
+    int best = fit;
+    long long best_cost = -1;
+    for (int n = fit; n >= 1; --n) {
+        const long long passes = (ngroups + (long long)g_sm_count * n - 1) / ((long long)g_sm_count * n);
+        const long long cost = passes * (n * K + 4);
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = n; }
+    }
+    return best;
 }
 
 template <bool GRAD, class C>
@@ -530,7 +537,7 @@ template <bool GRAD, class C>
 static int launch_score_lane_k(const adock_grids* grids, const adock_ligand* lig, const ParDev& P, const ScoreArgs& a, int var, int ngroups,
                                cudaStream_t st) {
     const LaneGeom g = lane_geom(lig);
-    const int NG = lane_spread_groups(lane_fit_groups(g, var, false), ngroups);
+    const int NG = lane_spread_groups(lane_fit_groups(g, var, false), ngroups, C::K);
     const size_t smem = lane_smem(g, var, false, NG);
     const int grid = (int)std::max<long long>(1, std::min<long long>(((long long)ngroups + NG - 1) / NG, g_sm_count));
     CUDA_TRY(cudaFuncSetAttribute(score_lane_kernel<GRAD, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -713,7 +720,7 @@ template <class C, bool SW>
 static int launch_ls_array_lane(const adock_grids* grids, const adock_ligand* ligand, const ParDev& P, LsArgs a, int var, int n, cudaStream_t stm) {
     const LaneGeom g = lane_geom(ligand);
     const int ngroups = (n + 31) / 32;
-    const int NG = lane_spread_groups(lane_fit_groups(g, var, true), ngroups);
+    const int NG = lane_spread_groups(lane_fit_groups(g, var, true), ngroups, C::K);
     const int grid = (ngroups + NG - 1) / NG;
     const size_t smem = lane_smem(g, var, true, NG);
     const size_t T = (size_t)grid * NG * 32;
