@@ -1327,13 +1327,29 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     long long* d_out_evals = nullptr;
     int *d_out_gens = nullptr, *d_flag = nullptr;
     DockJob* d_jobs = nullptr;
-    cudaError_t e = buf.alloc(&d_out_geno, (size_t)nlig * nrun * gstride * 4);
-    if (e == cudaSuccess) e = buf.alloc(&d_out_E, (size_t)nlig * nrun * 4);
-    if (e == cudaSuccess && best_coords) e = buf.alloc(&d_out_xyz, (size_t)nlig * nrun * cstride * 12);
-    if (e == cudaSuccess) e = buf.alloc(&d_out_evals, (size_t)nlig * nrun * 8);
-    if (e == cudaSuccess) e = buf.alloc(&d_out_gens, (size_t)nlig * nrun * 4);
-    if (e == cudaSuccess) e = buf.alloc(&d_flag, 4);
-    if (e == cudaSuccess) e = buf.alloc(&d_jobs, (size_t)nlig * sizeof(DockJob));
+    // ONE device allocation per call for the outputs, the job table and every per-job buffer (device buffers are
+    // preallocated, not allocated per ligand): sizes first, then the slab is carved at 256-byte boundaries
+    auto up256 = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    size_t slab_bytes = 0;
+    auto reserve = [&](size_t bytes) { const size_t o = slab_bytes; slab_bytes += up256(bytes ? bytes : 1); return o; };
+    const size_t o_geno = reserve((size_t)nlig * nrun * gstride * 4), o_E = reserve((size_t)nlig * nrun * 4),
+                 o_xyz = best_coords ? reserve((size_t)nlig * nrun * cstride * 12) : 0, o_evals = reserve((size_t)nlig * nrun * 8),
+                 o_gens = reserve((size_t)nlig * nrun * 4), o_flag = reserve(4), o_jobs = reserve((size_t)nlig * sizeof(DockJob));
+    struct JobOff { size_t pop, E, st, picks, fy, act, hist; };
+    std::vector<JobOff> joff(nlig);
+    for (int l = 0; l < nlig; ++l) {
+        const size_t Gn = 7 + (size_t)ligs[l]->tp.R;
+        joff[l] = JobOff{reserve(2 * popsz * Gn * 4), reserve(2 * popsz * 4), reserve((size_t)nrun * sizeof(RunState)), reserve(popsz * 4),
+                         reserve(popsz * 4), reserve((size_t)(nrun + 1) * 4), p.autostop ? reserve((size_t)nrun * p.as_window * 4) : 0};
+    }
+    unsigned char* slab = nullptr;
+    cudaError_t e = buf.alloc(&slab, slab_bytes);
+    if (e == cudaSuccess) {
+        d_out_geno = reinterpret_cast<float*>(slab + o_geno); d_out_E = reinterpret_cast<float*>(slab + o_E);
+        d_out_xyz = best_coords ? reinterpret_cast<float*>(slab + o_xyz) : nullptr;
+        d_out_evals = reinterpret_cast<long long*>(slab + o_evals); d_out_gens = reinterpret_cast<int*>(slab + o_gens);
+        d_flag = reinterpret_cast<int*>(slab + o_flag); d_jobs = reinterpret_cast<DockJob*>(slab + o_jobs);
+    }
     std::vector<int> act0(nrun + 1);                    // every run starts active
     act0[0] = nrun;
     for (int r = 0; r < nrun; ++r) act0[1 + r] = r;
@@ -1361,15 +1377,12 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         j.blob = lg->d_blob; j.ext_of_int = lg->d_ext_of_int; j.blob_bytes = lg->blob_bytes;
         j.Gn = 7 + lg->tp.R; j.N = lg->tp.N; j.R = lg->tp.R; j.seed = seeds[l];
         j.lane = lg->d_lane; j.lane_bytes = lg->lane_bytes; j.pad0 = 0;
-        e = buf.alloc(&j.pop, 2 * popsz * j.Gn * 4);
-        if (e == cudaSuccess) e = buf.alloc(&j.E, 2 * popsz * 4);
-        if (e == cudaSuccess) e = buf.alloc(&j.st, (size_t)nrun * sizeof(RunState));
-        if (e == cudaSuccess) e = buf.alloc(&j.picks, popsz * 4);
-        if (e == cudaSuccess) e = buf.alloc(&j.fy, popsz * 4);
-        j.hist = nullptr;
-        if (e == cudaSuccess) e = buf.alloc(&j.act, (size_t)(nrun + 1) * 4);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(j.act, act0.data(), (size_t)(nrun + 1) * 4, cudaMemcpyHostToDevice, stm);
-        if (e == cudaSuccess && p.autostop) e = buf.alloc(&j.hist, (size_t)nrun * p.as_window * 4);
+        const JobOff& jo = joff[l];
+        j.pop = reinterpret_cast<float*>(slab + jo.pop); j.E = reinterpret_cast<float*>(slab + jo.E);
+        j.st = reinterpret_cast<RunState*>(slab + jo.st); j.picks = reinterpret_cast<int*>(slab + jo.picks);
+        j.fy = reinterpret_cast<int*>(slab + jo.fy); j.act = reinterpret_cast<int*>(slab + jo.act);
+        j.hist = p.autostop ? reinterpret_cast<float*>(slab + jo.hist) : nullptr;
+        e = cudaMemcpyAsync(j.act, act0.data(), (size_t)(nrun + 1) * 4, cudaMemcpyHostToDevice, stm);
         j.out_geno = d_out_geno + (size_t)l * nrun * gstride;
         j.out_E = d_out_E + (size_t)l * nrun;
         j.out_xyz = d_out_xyz ? d_out_xyz + (size_t)l * nrun * cstride * 3 : nullptr;
@@ -1497,7 +1510,11 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     const bool can_run = (long long)Pn < max_evals && p.max_gens > 0;
     int h_flag = can_run ? 1 : 0;
     const int poll = 8;
-    std::vector<cudaEvent_t> prof_ev;
+    struct EventList {                                  // destroyed on every way out of the function
+        std::vector<cudaEvent_t> v;
+        ~EventList() { for (cudaEvent_t ev : v) cudaEventDestroy(ev); }
+    } prof;
+    std::vector<cudaEvent_t>& prof_ev = prof.v;
     for (int g = 0; h_flag && g < p.max_gens; ++g) {
         g_launches += launch_ga() - 1;
         if (dm.n_ls > 0 && p.lsit > 0) {
@@ -1544,7 +1561,6 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
             g_ls_ms += ms;
             ++g_ls_launches;
         }
-        for (cudaEvent_t e2 : prof_ev) cudaEventDestroy(e2);
         for (size_t i = 0; i < h_gens.size(); ++i) g_ls_evals += h_evals[i] - Pn - (long long)h_gens[i] * (Pn - 1);
     }
     return ADOCK_OK;
