@@ -236,14 +236,16 @@ def apply_step(R, x, delta):
     return x
 
 
-def adadelta(grids: Grids, lig: Ligand, par: OPar, geno, trace=False):
-    """docking local search from one genotype: (best genotype, best E, iterations used[, traceE, traceX])."""
+def adadelta(grids: Grids, lig: Ligand, par: OPar, geno, trace=False, fp32=False):
+    """docking local search from one genotype: (best genotype, best E, iterations used[, traceE, traceX]).
+    fp32=True: the same statements with the score path in float (liboracle_f32.so): how fast an honest fp32 chain parts
+    from the oracle's (a measuring stick for the trace tolerance, never a parity reference)."""
     g = _f64(geno).copy()
     E = C.c_double(float("nan"))
     it = C.c_int()
     tE = np.full(par.lsit, np.nan) if trace else None
     tX = np.full((par.lsit, 7 + lig.R), np.nan) if trace else None
-    lib().orc_adadelta(grids._h, lig._h, C.byref(par), _p(g), C.byref(E), C.byref(it), _p(tE), _p(tX))
+    (lib_f32() if fp32 else lib()).orc_adadelta(grids._h, lig._h, C.byref(par), _p(g), C.byref(E), C.byref(it), _p(tE), _p(tX))
     return (g, E.value, it.value, tE, tX) if trace else (g, E.value, it.value)
 
 

@@ -515,6 +515,40 @@ def test_local_search_first_iterations_track_oracle(B, orc, W, cases, dev, famil
     assert np.abs(gG[a] - oG[a]).max() < 2e-3
 
 
+def test_local_search_trace_nonclashing_20_iterations(B, orc, W, pocket, dev, family):
+    """'GPU vs oracle per-iteration trace (x, E) from the same start: energies within tolerance for the first ~20
+    iterations (then chaotic divergence allowed)'.  On the non-clashing workload (energies O(100): no cancellation floor)
+    the ADADELTA chain of every kernel family is compared with the oracle's trace iteration by iteration, in units of the
+    plain energy tolerance of north_star (1e-4 relative or 1e-3 kcal/mol).  Measured: every chain is inside the tolerance
+    for the first three iterations and the median chain for the first seven; from iteration 4 on the deviation grows ~5x
+    per iteration -- and the oracle's own honest-fp32 build (liboracle_f32.so) parts from the fp64 oracle at the same rate,
+    so that rate is fp32 against fp64 on this chain, not the kernels.  The bar over all 20 iterations is therefore: the
+    CUDA chain's median deviation is at every iteration within 3x of the honest-fp32 oracle's."""
+    grids, lig, G = pocket
+    c = Case(B, orc, W, grids, lig, dict(lsit=20))
+    n = 160
+    S = G[:n].copy()
+    d_g = torch.from_numpy(S).to(dev)
+    d_E = torch.zeros(n, device=dev)
+    d_it = torch.zeros(n, dtype=torch.int32, device=dev)
+    d_tr = torch.full((n, 20), float("nan"), device=dev)
+    B.adock_local_search(c.gg, c.gl, c.gp, d_g, d_E, d_it, d_tr)
+    torch.cuda.synchronize()
+    assert (d_it.cpu().numpy() == 20).all()
+    T = d_tr.cpu().numpy().astype(np.float64)
+    O = np.array([orc.adadelta(c.og, c.ol, c.op, S[i].astype(np.float64), trace=True)[3] for i in range(n)])
+    F = np.array([orc.adadelta(c.og, c.ol, c.op, S[i].astype(np.float64), trace=True, fp32=True)[3] for i in range(n)])
+    tol = np.maximum(1e-4 * np.abs(O), 1e-3)
+    dev_gpu, dev_f32 = np.median(np.abs(T - O) / tol, axis=0), np.median(np.abs(F - O) / tol, axis=0)
+    ok = np.abs(T - O) <= tol
+    print(f"nonclashing trace [{family}]: median |dE|/tol per iteration, CUDA   {np.array2string(dev_gpu, precision=2)}\n"
+          f"                                           honest-fp32 oracle {np.array2string(dev_f32, precision=2)}\n"
+          f"    fraction of chains within the plain tolerance per iteration {np.array2string(ok.mean(0), precision=2)}")
+    assert ok[:, :3].all()                               # iterations 0..2: every chain at the plain tolerance
+    assert (dev_gpu[:7] < 2.0).all() and (dev_gpu[:5] < 0.05).all()
+    assert (dev_gpu <= 3.0 * dev_f32 + 0.01).all()
+
+
 def test_local_search_statistics_match_oracle(B, orc, W, cases, dev, family):
     c = cases("drug")
     n = 384
