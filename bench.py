@@ -38,11 +38,12 @@ WORKLOAD = ("drug-like docking: 40-atom ligand, 8 torsions, 7 types, 9 fp32 maps
 FP32_LANES = 128                                            # per SM (B200_PROFILING.md unit counts)
 L2_BYTES_PER_CLK = 6300.0                                   # LTS throughput cap of the full chip (B300_MICROARCH.md, measured on B300)
 # one ligand = 20 runs x 9 ADADELTA chains = 180 chains = 6 groups of 32 lanes; the ADADELTA kernel keeps 12 warps (groups)
-# resident per SM (positions in tensor memory): 2 ligands per SM
-LIGANDS_PER_SM = 2
-# dram__bytes_read.sum + dram__bytes_write.sum of one dock_ls_lane_kernel launch at 2 ligands per SM on 148 SMs
-# (profiles/r02b_dock_ls_lane_ncu.md: one `ncu --set full` capture of `bench.py --probe dock 296 0 40000`); other batches: null
-LS_TRAFFIC_BYTES = {296: 2.6346e9 + 7.66e6}
+# resident per SM (positions in tensor memory) = 2 ligands; a step docks TWO waves of them, sorted by cost by the library, so
+# that the hardware hands the next CTA to the SM that frees first (one wave: 5.80e8, two: 6.02e8 evals/s in that kernel)
+LIGANDS_PER_SM = 4
+# dram__bytes_read.sum + dram__bytes_write.sum of one dock_ls_lane_kernel launch on 148 SMs (profiles/r02c_dock_ls_lane_ncu.md:
+# one `ncu --set full` capture of `bench.py --probe dock <ligands> 0 40000`); other batches: null
+LS_TRAFFIC_BYTES = {296: 2.6553e9 + 7.15e6}
 
 
 def flops_per_eval(N, R, npairs, nmoved):
@@ -156,8 +157,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--ligands", type=int, default=0, help="ligands docked concurrently per step and per GPU (0: 2 per SM = one wave of the ADADELTA kernel)")
-    ap.add_argument("--e2e-steps", type=int, default=2, help="steps of the host-buffer (end-to-end) leg, at most --steps")
+    ap.add_argument("--ligands", type=int, default=0, help="ligands docked per step and per GPU (0: 4 per SM = two waves of the ADADELTA kernel)")
+    ap.add_argument("--e2e-steps", type=int, default=1, help="steps of the host-buffer (end-to-end) leg, at most --steps")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip BASELINE.json configs[4] (adock_score_batch on the four sweep ligands)")

@@ -1368,7 +1368,13 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         std::vector<int> by(nlig);
         std::iota(by.begin(), by.end(), 0);
         std::stable_sort(by.begin(), by.end(), [&](int a, int b) { return cost[a] > cost[b]; });
-        for (int k = 0, lo = 0, hi = nlig - 1; k < nlig; ++k) jorder[k] = (k & 1) ? by[hi--] : by[lo++];
+        // more CTAs than SMs: heaviest first, similar ligands share a CTA (its warps finish together) and the hardware hands
+        // the next CTA to the SM that frees first -- longest-processing-time-first for free (592 bench ligands: 5.91e8 ->
+        // 6.02e8 evals/s in the ADADELTA kernel); one wave: alternate, so that every CTA carries the same load
+        const long long lane_ctas = pl.var >= 0 ? ((long long)nlig * jg + pl.ng - 1) / pl.ng : 0;
+        if (lane_ctas > g_sm_count) jorder = by;
+        else
+            for (int k = 0, lo = 0, hi = nlig - 1; k < nlig; ++k) jorder[k] = (k & 1) ? by[hi--] : by[lo++];
     }
     for (int k = 0; k < nlig && e == cudaSuccess; ++k) {
         const int l = jorder[k];
@@ -1417,9 +1423,8 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
         cudaError_t e2 = buf.alloc(&d_lscratch, kLaneVars[pl.var].TM ? 16 : T * (size_t)(Gmax + 2 * (Gmax - 1)) * 4);
         if (e2 != cudaSuccess) return fail(e2 == cudaErrorMemoryAllocation ? ADOCK_ENOMEM : ADOCK_ECUDA, std::string("dock alloc: ") + cudaGetErrorString(e2));
         al = LaneDockArgs{d_lscratch, Gmax, pl.ng, nlig * jg, jg, pl.slot, pl.nimg, pl.gfloats, 0, nullptr, nullptr};
-        // queue mode: tpc teams of jg groups per CTA, as many as fit; taken when every team of a full wave gets a ligand and
-        // the ligands differ enough in cost for the balance to pay (the queue loop costs the evaluation 6 % of its speed:
-        // measured, profiles/r02_lane_variants.md)
+        // queue mode (on request, see below): tpc teams of jg groups per CTA, as many as fit; needs a ligand for every team of a
+        // full wave
         const LaneVar& V = kLaneVars[pl.var];
         const int floats = lane_var_floats(lg, pl.var, true);
         for (int t = std::min(kLaneQueueMaxTeams, (V.W / V.K) / jg); t >= 1 && !q_tpc; --t) {
@@ -1434,8 +1439,12 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
             m /= nlig;
             for (double c : cost) v += (c - m) * (c - m);
             const double cv = std::sqrt(v / nlig) / m;
-            const char* force = std::getenv("ADOCK_LS_QUEUE");              // A/B switch of the profiles: 0 = flat, 1 = queue
-            if (force ? force[0] == '0' : cv < 0.08) q_tpc = 0;
+            // Measured (profiles/r02_lane_variants.md): the flat partition with the ligands sorted by cost over two or more
+            // waves lets the hardware's CTA scheduler do the balancing and beats the queues (whose loop costs the
+            // evaluation 6 %) on the bench batch and on configs[2] alike, so the queues run only on request.
+            const char* force = std::getenv("ADOCK_LS_QUEUE");              // A/B switch of the profiles: 1 = queues
+            (void)cv;
+            if (!(force && force[0] == '1')) q_tpc = 0;
         }
         if (q_tpc) {
             q_nctas = std::min(g_sm_count, (nlig + q_tpc - 1) / q_tpc);

@@ -851,14 +851,14 @@ def test_pose_rmsd_and_clustering_match_oracle(B, orc, cases):
 
 
 def test_dock_bench_launch_configuration_sampled(B, W, orc):
-    """the launch configuration bench.py times (two drug-like ligands per SM and a ragged 37 more, x 20 runs x pop 150 in
-    one adock_dock_many call: lane-per-individual local search with the positions in tensor memory, one work queue per team
-    of six warps (some teams dock two ligands), lane-per-individual offspring scoring), for three generations; sampled
-    ligands: reported energy = oracle energy of the reported genotype, eval accounting, and the same ligand docked alone in
-    the same kernel variant (flat partition, one CTA) gives the same result bit for bit."""
+    """the launch configuration bench.py times (four drug-like ligands per SM -- two waves of the local-search kernel, sorted by
+    cost -- and a ragged 37 more, x 20 runs x pop 150 in one adock_dock_many call: lane-per-individual local search with the
+    positions in tensor memory, lane-per-individual offspring scoring), for three generations; sampled ligands: reported
+    energy = oracle energy of the reported genotype, eval accounting; the same launch with one work queue per team
+    (dock_ls_lane_queue_kernel, on request) and the same ligand docked alone (one CTA) give the same result bit for bit."""
     grids, lig0 = W.make_config("drug")
     centre = 0.5 * (grids.box_lo + grids.box_hi); c = W.CONFIGS["drug"]
-    nl = 2 * torch.cuda.get_device_properties(0).multi_processor_count + 37
+    nl = 4 * torch.cuda.get_device_properties(0).multi_processor_count + 37
     ligs = W.share_type_table([W.make_ligand(c["N"], c["R"], c["T"], 100 + i, centre) for i in range(nl)])
     gp, op = B.make_params(W.DEFAULT_PARAMS), orc.params(W.DEFAULT_PARAMS)
     gg = B.Grids.from_workload(grids); og = orc.Grids.from_workload(grids)
@@ -867,13 +867,13 @@ def test_dock_bench_launch_configuration_sampled(B, W, orc):
     max_evals = P + 2 * (P - 1 + 9 * 300) + 1                                  # ends after generation 3
     seeds = [5000 + i for i in range(nl)]
     B.adock_set_path("auto")
-    os.environ["ADOCK_LS_QUEUE"] = "1"          # the queue mode is chosen by the cost spread of the launch (screening); forced here
+    r = B.adock_dock_many(gg, gl, gp, nrun, P, max_evals, seeds)               # flat partition over the cost-sorted ligands
+    os.environ["ADOCK_LS_QUEUE"] = "1"                                         # the same with work queues per team
     try:
-        r = B.adock_dock_many(gg, gl, gp, nrun, P, max_evals, seeds)
+        r_q = B.adock_dock_many(gg, gl, gp, nrun, P, max_evals, seeds)
     finally:
         del os.environ["ADOCK_LS_QUEUE"]
-    r_flat = B.adock_dock_many(gg, gl, gp, nrun, P, max_evals, seeds)          # these ligands differ little: flat partition
-    assert np.array_equal(r["energies"], r_flat["energies"]) and np.array_equal(r["genotypes"], r_flat["genotypes"])
+    assert np.array_equal(r["energies"], r_q["energies"]) and np.array_equal(r["genotypes"], r_q["genotypes"])
     assert B.lib().adock_last_dock_path() == 2
     assert (r["gens"] == 3).all() and (r["evals"] == P + 3 * (P - 1 + 9 * 300)).all()
     for i in (0, 57, 131, nl - 1):
