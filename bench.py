@@ -41,9 +41,9 @@ L2_BYTES_PER_CLK = 6300.0                                   # LTS throughput cap
 # resident per SM (positions in tensor memory) = 2 ligands; a step docks TWO waves of them, sorted by cost by the library, so
 # that the hardware hands the next CTA to the SM that frees first (one wave: 5.80e8, two: 6.02e8 evals/s in that kernel)
 LIGANDS_PER_SM = 4
-# dram__bytes_read.sum + dram__bytes_write.sum of one dock_ls_lane_kernel launch on 148 SMs (profiles/r02c_dock_ls_lane_ncu.md:
-# one `ncu --set full` capture of `bench.py --probe dock <ligands> 0 40000`); other batches: null
-LS_TRAFFIC_BYTES = {296: 2.6553e9 + 7.15e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of one dock_ls_lane_kernel launch on 148 SMs (profiles/r02b_dock_ls_lane_ncu.md:
+# one `ncu --set full` capture each of `bench.py --probe dock <ligands> 0 40000`); other batches: null
+LS_TRAFFIC_BYTES = {296: 2.6553e9 + 7.15e6, 592: 5.345e9 + 14.64e6}
 
 
 def flops_per_eval(N, R, npairs, nmoved):
