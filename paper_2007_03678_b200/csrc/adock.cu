@@ -523,7 +523,7 @@ __global__ void __launch_bounds__(C::kMaxWarps * 32, 1) score_lane_kernel(GridDe
         group_sync<K>(S);
         float ei, ea;
         bool gf;
-        const float e = lane_eval<GRAD, K, 1, C::TM>(L, G, P, S, GRAD ? a.grads + (size_t)src * a.dstride : nullptr, 1, act, ei, ea, gf);
+        const float e = lane_eval<GRAD, K, 1, C::TM, C::kMaxWarps == 16>(L, G, P, S, GRAD ? a.grads + (size_t)src * a.dstride : nullptr, 1, act, ei, ea, gf);
         if (act && S.part == 0) {
             a.E[idx] = e;
             if (a.terms) { a.terms[2 * (size_t)idx] = ei; a.terms[2 * (size_t)idx + 1] = ea; }

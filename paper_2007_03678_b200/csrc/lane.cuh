@@ -272,7 +272,11 @@ __device__ __forceinline__ void own_flush(const LaneS& S, int f, float Fx, float
 // The rigid-body blocks (dE/dt, dE/domega) are summed from the GRID forces alone: intramolecular pair forces cancel
 // exactly in both (Newton's third law), so they are kept out of sums they contribute nothing to.
 // The caller must group_sync before S.geno, the positions or own[] are touched again (part 0 still reads them).
-template <bool GRAD, int K, int GOUT = 1, bool TM = false>
+// PRE: the J fragment's sums are loaded at the top of the tile that updates them (hides the read-modify-write latency, holds six
+// registers across the tile) instead of just before the update.  Which is faster is a matter of ptxas's register allocation
+// per variant (measured: the 16-warp scoring kernel 6.88e8 with, 6.75e8 without; the 12-warp ADADELTA kernel 6.02e8 with,
+// 6.09e8 without).
+template <bool GRAD, int K, int GOUT = 1, bool TM = false, bool PRE = false>
 __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, const ParDev& P, const LaneS& S, float* grad, int gs,
                                            bool wr, float& e_inter, float& e_intra, bool& gfin) {
     const float tx = S.geno[0], ty = S.geno[32], tz = S.geno[64];
@@ -430,7 +434,7 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                 const int f0 = (cw.y >> 16) & 0xff, f1 = cw.y >> 24;
                 float4 va = make_float4(0.f, 0.f, 0.f, 0.f);
                 float2 vb = make_float2(0.f, 0.f);
-                if (GRAD) { va = S.oA[f0 * 32]; vb = S.oB[f0 * 32]; }
+                if (GRAD && PRE) { va = S.oA[f0 * 32]; vb = S.oB[f0 * 32]; }
                 pos_wait<TM>(pj);
                 const f2 xj = pk(pj.x0, pj.x1), yj = pk(pj.y0, pj.y1), zj = pk(pj.z0, pj.z1);
                 f2 gjx = zero, gjy = zero, gjz = zero;
@@ -456,6 +460,7 @@ __device__ __forceinline__ float lane_eval(const LaneL& L, const GridDev& G, con
                 if (GRAD) {                             // J side: gradients (a | b) of atoms (j0 | j1) -> fragment sums, the torque
                     float ax, bx, ay, by, az, bz;        // about t as chains of scalar fma on top of the loaded sums
                     unpk(gjx, ax, bx); unpk(gjy, ay, by); unpk(gjz, az, bz);
+                    if (!PRE) { va = S.oA[f0 * 32]; vb = S.oB[f0 * 32]; }
                     const float t0x = fmaf(pj.y0, az, -pj.z0 * ay), t0y = fmaf(pj.z0, ax, -pj.x0 * az), t0z = fmaf(pj.x0, ay, -pj.y0 * ax);
                     if (f0 == f1) {
                         S.oA[f0 * 32] = make_float4((va.x + ax) + bx, (va.y + ay) + by, (va.z + az) + bz,
