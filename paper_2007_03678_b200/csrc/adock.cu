@@ -924,6 +924,55 @@ __global__ void __launch_bounds__(256) dock_ga_kernel(GridDev G, ParDev P, const
     }
 }
 
+// The same generation step with a THREAD per individual of the new population (no shared memory, no ligand image): the
+// warp-per-offspring kernel above spends a warp on work that is a dozen Philox draws (1.5 ms per generation for 592 ligands);
+// here the thread of slot 0 copies the elite and draws the local-search subset, every other thread makes its child
+// (ga_make_child_thread: bit-identical to ga_make_child).  Used with the lane-per-individual offspring scoring.
+__global__ void __launch_bounds__(128) dock_ga_lane_kernel(ParDev P, const DockJob* __restrict__ jobs, DockDims dm, int* __restrict__ decisions) {
+    const DockJob& job = jobs[blockIdx.x / dm.upj];
+    const int ind = (blockIdx.x % dm.upj) * blockDim.x + threadIdx.x;
+    if (ind >= dm.nrun * dm.P) return;
+    const int run = ind / dm.P, slot = ind % dm.P, Gn = job.Gn;
+    const RunState st = job.st[run];
+    if (!st.active) return;
+    const size_t popsz = (size_t)dm.nrun * dm.P;
+    const float* spop = job.pop + ((size_t)st.cur * popsz + (size_t)run * dm.P) * Gn;
+    const float* sE = job.E + (size_t)st.cur * popsz + (size_t)run * dm.P;
+    float* dpop = job.pop + ((size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P) * Gn;
+    float* dE = job.E + (size_t)(st.cur ^ 1) * popsz + (size_t)run * dm.P;
+    const uint32_t gen = (uint32_t)st.gen + 1u;
+    int* dec = decisions ? decisions + ((size_t)(blockIdx.x / dm.upj) * popsz + ind) * 10 : nullptr;
+    if (slot == 0) {
+        float be = __int_as_float(0x7f800000);
+        int bi = 0x7fffffff;
+        for (int s = 0; s < dm.P; ++s) {                // ties: the lowest slot (strict <, ascending)
+            const float e = sE[s];
+            if (e < be) { be = e; bi = s; }
+        }
+        if (bi == 0x7fffffff) bi = 0;                    // every energy non-finite: keep slot 0
+        for (int d = 0; d < Gn; ++d) dpop[d] = spop[(size_t)bi * Gn + d];
+        dE[0] = sE[bi];
+        if (dec) { for (int k = 0; k < 10; ++k) dec[k] = 0; dec[2] = bi; }
+        int* picks = job.picks + (size_t)run * dm.P;
+        if (dm.n_ls >= dm.P) {
+            for (int s = 0; s < dm.P; ++s) picks[s] = s;
+        } else if (dm.n_ls > 0) {
+            int* fy = job.fy + (size_t)run * dm.P;
+            for (int s = 0; s < dm.P - 1; ++s) fy[s] = s + 1;
+            picks[0] = 0;
+            uint4 r = make_uint4(0, 0, 0, 0);
+            for (int m = 0; m < dm.n_ls - 1; ++m) {
+                if ((m & 3) == 0) r = draw4(job.seed, (uint32_t)(m >> 2), kLsPick, (uint32_t)(run * dm.P), gen);
+                const int j = m + below(pick_word(r, m & 3), dm.P - 1 - m);
+                const int t = fy[m]; fy[m] = fy[j]; fy[j] = t;
+                picks[1 + m] = fy[m];
+            }
+        }
+        return;
+    }
+    ga_make_child_thread(P, dm.P, job.R, job.seed, (uint32_t)ind, gen, spop, sE, dpop + (size_t)slot * Gn, dec);
+}
+
 // ADADELTA on the selected individuals of the new population (Lamarckian write-back)
 __global__ void __launch_bounds__(128) dock_ls_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs, DockDims dm) {
     DOCK_PROLOGUE()
@@ -1406,7 +1455,8 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     CUDA_TRY(cudaFuncSetAttribute(dock_ls_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ls));
     CUDA_TRY(cudaFuncSetAttribute(dock_final_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ls));
 
-    DockDims dga = dm, dls = dm, dfin = dm, dteam = dm;
+    DockDims dga = dm, dls = dm, dfin = dm, dteam = dm, dgl = dm;
+    dgl.upj = (int)((popsz + 127) / 128);                       // thread per individual (dock_ga_lane_kernel)
     dteam.upj = std::max(1, (nrun * dm.n_ls + team_tpc - 1) / team_tpc);     // team_tpc chains per CTA
     if (ls_team && team_tpc == 1) CUDA_TRY(cudaFuncSetAttribute(dock_ls_team_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_team));
     if (ls_team && team_tpc == 4) CUDA_TRY(cudaFuncSetAttribute(dock_ls_team_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_team));
@@ -1508,7 +1558,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
             dock_ga_kernel<true><<<dga.upj * nlig, Wga * 32, smem_ga, stm>>>(grids->dev, P, d_jobs, dga, nullptr);
             return 1;
         }
-        dock_ga_kernel<false><<<dga.upj * nlig, Wga * 32, smem_ga, stm>>>(grids->dev, P, d_jobs, dga, nullptr);
+        dock_ga_lane_kernel<<<dgl.upj * nlig, 128, 0, stm>>>(P, d_jobs, dgl, nullptr);
         const int thr = ps.ng * ps.K * 32;
         LANE_VARIANT(ps.var, dock_score_lane_kernel<C><<<ps.nctas, thr, ps.smem, stm>>>(grids->dev, P, d_jobs, dm, as))
         return 2;
@@ -1900,8 +1950,14 @@ extern "C" int adock_ga_generation(const adock_grids* grids, const adock_ligand*
         CUDA_TRY(cudaMemcpyAsync(j.st, st.data(), nrun * sizeof(RunState), cudaMemcpyHostToDevice, stm));
         CUDA_TRY(cudaMemcpyAsync(j.pop, d_pop, popsz * Gn * 4, cudaMemcpyDeviceToDevice, stm));
         CUDA_TRY(cudaMemcpyAsync(j.E, d_energies, popsz * 4, cudaMemcpyDeviceToDevice, stm));
-        CUDA_TRY(cudaFuncSetAttribute(dock_ga_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        dock_ga_kernel<false><<<dm.upj, W * 32, smem, stm>>>(grids->dev, P, d_job, dm, d_decisions);
+        if (g_path == 2) {                              // lane family: the thread-per-individual kernel of the batched dockings
+            DockDims dl = dm;
+            dl.upj = (int)((popsz + 127) / 128);
+            dock_ga_lane_kernel<<<dl.upj, 128, 0, stm>>>(P, d_job, dl, d_decisions);
+        } else {
+            CUDA_TRY(cudaFuncSetAttribute(dock_ga_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            dock_ga_kernel<false><<<dm.upj, W * 32, smem, stm>>>(grids->dev, P, d_job, dm, d_decisions);
+        }
         ++g_launches;
         CUDA_TRY(cudaMemcpyAsync(d_newpop, j.pop + popsz * Gn, popsz * Gn * 4, cudaMemcpyDeviceToDevice, stm));
         if (d_ls_picks) CUDA_TRY(cudaMemcpyAsync(d_ls_picks, j.picks, popsz * 4, cudaMemcpyDeviceToDevice, stm));

@@ -604,6 +604,52 @@ __device__ inline void ga_make_child(const ParDev& P, int Pn, int R, unsigned lo
     __syncwarp();
 }
 
+// The same child, made by ONE thread straight into global memory (dock_ga_lane_kernel: a thread per individual of the
+// new population).  Same draws (counter = gene block, purpose, individual, generation) and the same expressions per
+// gene block as ga_make_child, so the integer decisions and the genotypes are identical bit for bit.
+__device__ inline void ga_make_child_thread(const ParDev& P, int Pn, int R, unsigned long long seed, uint32_t id, uint32_t gen,
+                                            const float* pop, const float* E, float* geno, int* dec) {
+    const int Gn = 7 + R, NB = 4 + R;
+    const int A = tournament(P, Pn, E, seed, kTournA, id, gen, dec);
+    const int B = tournament(P, Pn, E, seed, kTournB, id, gen, dec ? dec + 3 : nullptr);
+    const uint4 rx = draw4(seed, 0, kXover, id, gen);
+    const int c1 = below(rx.y, NB + 1), c2 = below(rx.z, NB + 1);
+    const int p1 = min(c1, c2), p2 = max(c1, c2);
+    const bool xo = u01(rx.x) < P.xover_rate;
+    if (dec) { dec[6] = xo; dec[7] = p1; dec[8] = p2; }
+    const float* gA = pop + (size_t)A * Gn;
+    const float* gB = pop + (size_t)B * Gn;
+    unsigned mutmask = 0;
+    for (int b = 0; b < NB; ++b) {
+        const float* src = (xo && b >= p1 && b < p2) ? gB : gA;
+        const uint4 rm = draw4(seed, (uint32_t)b, kMut, id, gen);
+        const bool mut = u01(rm.x) < P.mut_rate;
+        const float amt = 2.f * u01(rm.y) - 1.f;
+        if (b < 3) {
+            geno[b] = mut ? src[b] + amt * P.dmov : src[b];
+        } else if (b == 3) {
+            if (mut) {
+                const float ang = amt * P.dang, z = 2.f * u01(rm.z) - 1.f;
+                const float sxy = sqrtf(fmaxf(0.f, 1.f - z * z));
+                float sp, cp, sh, ch;
+                sincospif(2.f * u01(rm.w), &sp, &cp);
+                sincosf(0.5f * ang, &sh, &ch);
+                const float q[4] = {src[3], src[4], src[5], src[6]};
+                float o[4];
+                rotate_quat(ch, sh * sxy * cp, sh * sxy * sp, sh * z, q, o);
+                geno[3] = o[0]; geno[4] = o[1]; geno[5] = o[2]; geno[6] = o[3];
+            } else {
+                geno[3] = src[3]; geno[4] = src[4]; geno[5] = src[5]; geno[6] = src[6];
+            }
+        } else {
+            const int gi = 4 + b - 1;
+            geno[gi] = mut ? wrap_pi(src[gi] + amt * P.dang) : src[gi];
+        }
+        if (mut && b < 31) mutmask |= 1u << b;
+    }
+    if (dec) dec[9] = (int)mutmask;
+}
+
 // ---------------------------------------------------------------- full evaluation of one genotype by a TEAM of W warps
 // One team of kTeamW warps per individual (one or four teams per CTA, sharing the ligand image), threads over atoms and pairs: for launches with so few chains that one warp per
 // chain leaves most schedulers idle (a single ligand: 180 chains on 592 schedulers), the evaluation itself is split.

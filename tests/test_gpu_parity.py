@@ -434,7 +434,18 @@ def test_initial_population_matches_oracle(B, orc, cases, dev):
         assert np.abs(got[run] - want).max() < 4e-6          # exact uniforms; fp32 affine map / trig
 
 
-def test_ga_decisions_bit_exact_and_children_match(B, orc, cases, dev):
+@pytest.mark.parametrize("fam", ["warp", "lane"])
+def test_ga_decisions_bit_exact_and_children_match(B, orc, cases, dev, fam):
+    """fam = 'warp': dock_ga_kernel (a warp per offspring); 'lane': dock_ga_lane_kernel (a thread per individual, the kernel
+    of the batched dockings)"""
+    B.adock_set_path(fam)
+    try:
+        _ga_decisions(B, orc, cases, dev)
+    finally:
+        B.adock_set_path("auto")
+
+
+def _ga_decisions(B, orc, cases, dev):
     c = cases("drug")
     R = c.lig.R
     nrun, P, seed, G = 4, 150, 777, 7 + c.lig.R
