@@ -629,6 +629,16 @@ __device__ inline float lane_adadelta(const LaneL& L, const GridDev& G, const Pa
                         if (d < 3) S.geno[d * 32] += dl; else w[d - 3] = dl;
                     }
                 }
+                if (TM) {                                   // chain state in shared memory: no round trips to batch
+                    for (int f = 1; f < L.nfrag; ++f) {
+                        const int d = 6 + L.fragi[3 * f + 1].w;
+                        float av = ls.Eg2[d * 32], bv = ls.Ed2[d * 32];
+                        const float dl = adadelta_component(P, reinterpret_cast<const float*>(S.oA + f * 32)[0], av, bv);
+                        ls.Eg2[d * 32] = av; ls.Ed2[d * 32] = bv;
+                        float* t = S.geno + (d + 1) * 32;
+                        *t = wrap_pi(*t + dl);
+                    }
+                } else
                 for (int f0 = 1; f0 < L.nfrag; f0 += 8) {  // torsions: fragment f's torsion gradient in oA[f*32].x
                     float av[8], bv[8];
                     int dd[8];
