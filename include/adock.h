@@ -107,8 +107,8 @@ int adock_ligand_tree(const adock_ligand* l, const int** tor_order, const unsign
 int adock_ligand_image(const adock_ligand* l, int* bytes, const unsigned char** image, const int** int_of_ext);
 
 /* The ligand image of the lane-per-individual kernels (host copy, owned by the handle): atoms in fragment
- * DFS preorder, fragment tree, and the pair list cut into 4-row x 2-column register tiles (layout:
- * csrc/lane_image.hpp).  pos_of_ext [N] maps caller atom index -> position in that order. */
+ * DFS preorder, fragment tree, and the pair list cut into 4-row x 2-column register tiles with one 32-byte coefficient
+ * record per row (layout: csrc/lane_image.hpp).  pos_of_ext [N] maps caller atom index -> position in that order. */
 int adock_ligand_lane_image(const adock_ligand* l, int* bytes, const unsigned char** image, const int** pos_of_ext);
 
 /* Kernel family used by the compute entry points of this process: 0 = chosen by problem
@@ -181,7 +181,11 @@ int adock_dock(const adock_grids* grids, const adock_ligand* ligand, const adock
  * ligand-major, with per-ligand genotype stride gstride >= max_l(7+R_l) and coordinate stride
  * cstride >= max_l(N_l): best_genotypes [nlig][nrun][gstride], best_energies [nlig][nrun], best_coords
  * [nlig][nrun][cstride][3] or NULL, evals_used [nlig][nrun] or NULL, gens_used [nlig][nrun] or NULL (generations each
- * run lasted: below max_gens when the eval budget or autostop ended it).  Synchronous. */
+ * run lasted: below max_gens when the eval budget or autostop ended it).  Synchronous.
+ * A ligand's result does not depend on what else is in the batch (same kernel variant: bit-identical to adock_dock of that
+ * ligand and seed).  Launches with more CTAs than SMs take the ligands in order of decreasing estimated cost.  Environment
+ * switch for measurements only: ADOCK_LS_QUEUE=1 runs the local search with one work queue per team of warps instead
+ * (dock_ls_lane_queue_kernel; same results, profiles/r02_lane_variants.md). */
 int adock_dock_many(const adock_grids* grids, const adock_ligand* const* ligands, int nlig, const adock_params* params,
                     int nrun, int pop_size, long long max_evals, const unsigned long long* seeds, int gstride,
                     float* best_genotypes, float* best_energies, int cstride, float* best_coords, long long* evals_used,
