@@ -59,7 +59,7 @@ struct WarpS {
     float2* sc;             // [nfrag] sin,cos of the fragment's torsion
     float4* fragT;          // [nfrag][3] rows of the 3x4 fragment transform
     float4* fragAx;         // [nfrag][2] posed axis, posed pivot point - t
-    float4* fragFT;         // [nfrag][2] force, torque about the fragment's own pivot point
+    float4* fragFT;         // [nfrag][2] force, torque about the fragment's own pivot point (team kernel: about t)
     float* blk;             // pose block, 256 floats per 32 atoms: x|y|z|q|gx|gy|gz|-  (32 each), so atom a
                             // lives at slot(a) = (a>>5)*256 + (a&31) and distinct a mod 32 hit distinct banks
 };
@@ -794,60 +794,63 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
 #pragma unroll
     for (int w = 0; w < kTeamW; ++w) { e_inter += T.red[8 * w]; e_intra += T.red[8 * w + 1]; }
 
-    // (a4) the planes are summed per atom (one thread each, fixed order 0+1+2+3), then back-propagation on warp 0:
-    // eval_pose's code
+    // (a4) back-propagation over the whole team.  (i) a thread per atom sums the planes (fixed order 0+1+2+3) and leaves the
+    // atom's torque about t in its plane-1 words; (ii) a thread per (fragment f > 0, component c of F(3) | T(3)) sums c over
+    // the fragment's atoms; (iii) the same thread sums c over the fragment's subtree [f, sub_end), and lane c = 0 of the
+    // eight collects the six sums: torsion gradient = u . (T - p x F), p = the pivot relative to t (lane_eval's form).
+    // The root's sums are never needed: the rigid-body blocks are the grid-force sums of (a2).
     if (GRAD) {
         for (int i = wi * 32 + lane; i < L.npos; i += 32 * kTeamW) {
             if (L.meta[i] == 0xffffffffu) continue;
             const int off = atom_slot_dev(i);
             float* b = S.blk + off;
             float gx = b[kGX], gy = b[kGY], gz = b[kGZ];
+            float* g1 = team_gptr(T, 1, off);
+            gx += g1[0]; gy += g1[32]; gz += g1[64];
 #pragma unroll
-            for (int w = 1; w < kTeamW; ++w) { const float* g = team_gptr(T, w, off); gx += g[0]; gy += g[32]; gz += g[64]; }
+            for (int w = 2; w < kTeamW; ++w) { const float* g = team_gptr(T, w, off); gx += g[0]; gy += g[32]; gz += g[64]; }
             b[kGX] = gx; b[kGY] = gy; b[kGZ] = gz;
+            const float rx = b[kX] - tx, ry = b[kY] - ty, rz = b[kZ] - tz;
+            g1[0] = ry * gz - rz * gy; g1[32] = rz * gx - rx * gz; g1[64] = rx * gy - ry * gx;
         }
         team_sync(T);
-        if (wi == 0) {
-            for (int f = lane; f < L.nfrag; f += 32) {
-                const int4 ix = L.fi[f];
-                const float4 pv = S.fragAx[2 * f + 1];
-                const float px = tx + pv.x, py = ty + pv.y, pz = tz + pv.z;
-                float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
-                for (int k = ix.y; k < ix.z; ++k) {
-                    const int off = atom_slot_dev(L.fragatoms[k]);
-                    const float* b = S.blk + off;
-                    const float gx = b[kGX], gy = b[kGY], gz = b[kGZ];
-                    const float rx = b[kX] - px, ry = b[kY] - py, rz = b[kZ] - pz;
-                    Fx += gx; Fy += gy; Fz += gz;
-                    Tx += ry * gz - rz * gy; Ty += rz * gx - rx * gz; Tz += rx * gy - ry * gx;
-                }
-                S.fragFT[2 * f] = make_float4(Fx, Fy, Fz, 0.f);
-                S.fragFT[2 * f + 1] = make_float4(Tx, Ty, Tz, 0.f);
+        float* ft = reinterpret_cast<float*>(S.fragFT);                 // [nfrag][8]: F(3), T(3) about t
+        const int nitem = 8 * L.nfrag, tid = wi * 32 + lane;
+        for (int it = 8 + tid; it < nitem; it += 32 * kTeamW) {
+            const int f = it >> 3, c = it & 7;
+            if (c >= 6) continue;
+            const int4 ix = L.fi[f];
+            const float* src = c < 3 ? S.blk + kGX + 32 * c : T.gextra + 32 * (c - 3);
+            float v = 0.f;
+            for (int k = ix.y; k < ix.z; ++k) {
+                const int off = atom_slot_dev(L.fragatoms[k]);
+                v += src[c < 3 ? off : (off >> 8) * 96 + (off & 31)];
             }
-            __syncwarp();
-            for (int f = lane; f < L.nfrag; f += 32) {
-                const int w = L.fi[f].w;
+            ft[it] = v;
+        }
+        if (wi == kTeamW - 1 && lane < 6) {             // rigid-body blocks: the warps' grid-force sums, fixed order
+            float v = T.red[2 + lane];
+#pragma unroll
+            for (int w = 1; w < kTeamW; ++w) v += T.red[8 * w + 2 + lane];
+            S.grad[lane] = v;
+        }
+        team_sync(T);
+        for (int base = 8 + wi * 32; base < nitem; base += 32 * kTeamW) {       // the same for every lane of a warp
+            const int it = base + lane, f = it >> 3, c = it & 7;
+            int w = 0;
+            float v = 0.f;
+            if (it < nitem) {
+                w = L.fi[f].w;
                 const int sub_end = w & 0xffff;
-                const float4 pf = S.fragAx[2 * f + 1];
-                float Fx = 0, Fy = 0, Fz = 0, Tx = 0, Ty = 0, Tz = 0;
-                for (int g = f; g < sub_end; ++g) {
-                    const float4 F = S.fragFT[2 * g], Tq = S.fragFT[2 * g + 1], pg = S.fragAx[2 * g + 1];
-                    const float lx = pg.x - pf.x, ly = pg.y - pf.y, lz = pg.z - pf.z;
-                    Fx += F.x; Fy += F.y; Fz += F.z;
-                    Tx += Tq.x + (ly * F.z - lz * F.y); Ty += Tq.y + (lz * F.x - lx * F.z); Tz += Tq.z + (lx * F.y - ly * F.x);
-                }
-                if (f == 0) {                           // rigid-body blocks: the warps' grid-force sums, fixed order
-#pragma unroll
-                    for (int d = 0; d < 6; ++d) {
-                        float v = T.red[2 + d];
-#pragma unroll
-                        for (int w = 1; w < kTeamW; ++w) v += T.red[8 * w + 2 + d];
-                        S.grad[d] = v;
-                    }
-                } else {
-                    const float4 u = S.fragAx[2 * f];
-                    S.grad[6 + (w >> 16)] = u.x * Tx + u.y * Ty + u.z * Tz;
-                }
+                if (c < 6) for (int g = f; g < sub_end; ++g) v += ft[8 * g + c];
+            }
+            const int l0 = lane & ~7;
+            const float Fx = __shfl_sync(kFull, v, l0), Fy = __shfl_sync(kFull, v, l0 + 1), Fz = __shfl_sync(kFull, v, l0 + 2);
+            const float Tx = __shfl_sync(kFull, v, l0 + 3), Ty = __shfl_sync(kFull, v, l0 + 4), Tz = __shfl_sync(kFull, v, l0 + 5);
+            if (it < nitem && c == 0) {
+                const float4 u = S.fragAx[2 * f], pv = S.fragAx[2 * f + 1];
+                S.grad[6 + (w >> 16)] = u.x * (Tx - (pv.y * Fz - pv.z * Fy)) + u.y * (Ty - (pv.z * Fx - pv.x * Fz)) +
+                                        u.z * (Tz - (pv.x * Fy - pv.y * Fx));
             }
         }
         team_sync(T);
