@@ -260,6 +260,29 @@ __device__ __forceinline__ float grid_atom(const GridDev& G, const ParDev& P, in
     return grid_finish<GRAD>(G, P, c, v, q, gx, gy, gz);
 }
 
+// The team kernel looks an atom up after the pair rounds and asks for the two sectors before them (the cell is computed
+// twice; nothing is held in registers over the pair loop): prefetch into L1, then loads that may hit there.
+__device__ __forceinline__ void grid_prefetch(const GridDev& G, const GridCell& c) {
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(c.base));
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(c.base + (long long)(G.ny - 1) * (G.nx - 1) * 2));
+}
+__device__ __forceinline__ F8 ld_cell_l1(const float4* p) {
+    F8 r;
+    asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+        : "=f"(r.lo.x), "=f"(r.lo.y), "=f"(r.lo.z), "=f"(r.lo.w), "=f"(r.hi.x), "=f"(r.hi.y), "=f"(r.hi.z), "=f"(r.hi.w)
+        : "l"(p));
+    return r;
+}
+template <bool GRAD>
+__device__ __forceinline__ float grid_atom_l1(const GridDev& G, const ParDev& P, int set, float q, float x, float y, float z,
+                                              float& gx, float& gy, float& gz) {
+    const GridCell c = grid_cell(G, set, x, y, z);
+    F8 v[2];
+    v[0] = ld_cell_l1(c.base);
+    v[1] = ld_cell_l1(c.base + (long long)(G.ny - 1) * (G.nx - 1) * 2);
+    return grid_finish<GRAD>(G, P, c, v, q, gx, gy, gz);
+}
+
 // single-instruction MUFU forms (flush-to-zero): reciprocal, reciprocal square root, 2^x
 __device__ __forceinline__ float frcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float frsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
@@ -276,13 +299,14 @@ __device__ __forceinline__ float warp_sum(float v) {
 // atom occurs twice on a side (topology.hpp), so the read-modify-writes need no atomics and their order is fixed.
 // The arithmetic of a round (pair_compute) touches only positions and charges, so several rounds can be in flight at
 // once; the force updates (pair_apply) then run round by round in the fixed order.
-struct PairOut { float* pi; float* pj; float fx, fy, fz, e; bool valid; };
+struct PairOut { int oi, oj; float fx, fy, fz, e; bool valid; };        // oi, oj: the atoms' offsets in S.blk
 template <bool GRAD, bool MAYPAD>
 __device__ __forceinline__ PairOut pair_compute(const LigS& L, const ParDev& P, const WarpS& S, int r, int lane) {
     const uint4 rec = L.pairs[r * 32 + lane];
     const bool valid = !MAYPAD || ((rec.x >> 23) & 1u);
-    float* pi = S.blk + (rec.x & 0x7ffu);
-    float* pj = S.blk + ((rec.x >> 11) & 0x7ffu);
+    const int oi = (int)(rec.x & 0x7ffu), oj = (int)((rec.x >> 11) & 0x7ffu);
+    const float* pi = S.blk + oi;
+    const float* pj = S.blk + oj;
     const float dx = pi[kX] - pj[kX], dy = pi[kY] - pj[kY], dz = pi[kZ] - pj[kZ];
     const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
     const float r2c = fmaxf(r2, P.rmin2);
@@ -311,23 +335,24 @@ __device__ __forceinline__ PairOut pair_compute(const LigS& L, const ParDev& P, 
         const float fs = (r2 >= P.rmin2) ? fmaf(dv, rinv, del + dds) * rinv : 0.f;
         o.fx = fs * dx; o.fy = fs * dy; o.fz = fs * dz;
     }
-    o.pi = pi; o.pj = pj; o.valid = valid;
+    o.oi = oi; o.oj = oj; o.valid = valid;
     o.e = valid ? e : 0.f;
     return o;
 }
 template <bool GRAD>
-__device__ __forceinline__ float pair_apply(const PairOut& o) {
+__device__ __forceinline__ float pair_apply(const WarpS& S, const PairOut& o) {
     if (GRAD) {
-        if (o.valid) { o.pi[kGX] += o.fx; o.pi[kGY] += o.fy; o.pi[kGZ] += o.fz; }
+        float* pi = S.blk + o.oi, *pj = S.blk + o.oj;
+        if (o.valid) { pi[kGX] += o.fx; pi[kGY] += o.fy; pi[kGZ] += o.fz; }
         __syncwarp();
-        if (o.valid) { o.pj[kGX] -= o.fx; o.pj[kGY] -= o.fy; o.pj[kGZ] -= o.fz; }
+        if (o.valid) { pj[kGX] -= o.fx; pj[kGY] -= o.fy; pj[kGZ] -= o.fz; }
         __syncwarp();
     }
     return o.e;
 }
 template <bool GRAD, bool MAYPAD>
 __device__ __forceinline__ float pair_round(const LigS& L, const ParDev& P, const WarpS& S, int r, int lane) {
-    return pair_apply<GRAD>(pair_compute<GRAD, MAYPAD>(L, P, S, r, lane));
+    return pair_apply<GRAD>(S, pair_compute<GRAD, MAYPAD>(L, P, S, r, lane));
 }
 
 // ---------------------------------------------------------------- full evaluation of one genotype by one warp
@@ -437,7 +462,7 @@ __device__ __forceinline__ float eval_pose(const LigS& L, const GridDev& G, cons
     for (; r4 + 4 <= L.nfull; r4 += 4) {                // four rounds of arithmetic in flight, updates in round order
         const PairOut o0 = pair_compute<GRAD, false>(L, P, S, r4, lane), o1 = pair_compute<GRAD, false>(L, P, S, r4 + 1, lane),
                       o2 = pair_compute<GRAD, false>(L, P, S, r4 + 2, lane), o3 = pair_compute<GRAD, false>(L, P, S, r4 + 3, lane);
-        ep += pair_apply<GRAD>(o0); ep += pair_apply<GRAD>(o1); ep += pair_apply<GRAD>(o2); ep += pair_apply<GRAD>(o3);
+        ep += pair_apply<GRAD>(S, o0); ep += pair_apply<GRAD>(S, o1); ep += pair_apply<GRAD>(S, o2); ep += pair_apply<GRAD>(S, o3);
     }
     for (int r = r4; r < L.nfull; ++r) ep += pair_round<GRAD, false>(L, P, S, r, lane);
     for (int r = L.nfull; r < L.nrounds; ++r) ep += pair_round<GRAD, true>(L, P, S, r, lane);
@@ -654,27 +679,33 @@ __device__ inline void ga_make_child_thread(const ParDev& P, int Pn, int R, unsi
 // One team of kTeamW warps per individual (one or four teams per CTA, sharing the ligand image), threads over atoms and pairs: for launches with so few chains that one warp per
 // chain leaves most schedulers idle (a single ligand: 180 chains on 592 schedulers), the evaluation itself is split.
 // Warp 0 builds the fragment transforms; the 32 W threads take one atom each (pose + grid lookup); warp w takes the pair
-// rounds r = w (mod W) and adds their forces into its own gradient plane (plane 0 = S.blk's gx|gy|gz, planes 1..W-1 in
-// S.gextra), so no two warps ever update the same word; warp 0 sums the planes in a fixed order during
-// back-propagation.  Same arithmetic as eval_pose; the summation order differs (fixed, so results are reproducible).
+// rounds r = w (mod W), two rounds in flight, and adds their forces into its own gradient plane (W planes of gx|gy|gz, 96
+// floats per 32 atoms, in T.gpl), so no two warps ever update the same word; the atom's thread sums the planes in a fixed
+// order.  Same arithmetic as eval_pose; the summation order differs (fixed, so results are reproducible).
 constexpr int kTeamW = 4;
 __host__ __device__ inline int team_scratch_floats(int N, int nfrag, int R) {
-    return warp_scratch_floats(N, nfrag, R) + (kTeamW - 1) * ((N + 31) / 32) * 96 + 8 * kTeamW + 8;
+    return warp_scratch_floats(N, nfrag, R) + kTeamW * ((N + 31) / 32) * 96 + 8 * kTeamW + 8;
 }
 // red: per warp w [8w .. 8w+8) = partial (e_grid, e_pairs, grid force F(3), grid torque about t T(3)); [8 kTeamW] = flag
-struct TeamS { WarpS S; float* gextra; float* red; int wi, gplane, bar; };     // gplane = floats per extra plane; bar = the team's named barrier
+struct TeamS { WarpS S; float* gpl; float* red; int wi, gplane, bar; };        // gplane = floats per plane; bar = the team's named barrier
 __device__ inline TeamS team_view(float* base, const LigS& L, int wi) {
     TeamS T;
     T.S = warp_view(base, L);
-    T.gextra = T.S.blk + (L.npos / 32) * 256;
-    T.red = T.gextra + (kTeamW - 1) * (L.npos / 32) * 96;
+    T.gpl = T.S.blk + (L.npos / 32) * 256;
+    T.red = T.gpl + kTeamW * (L.npos / 32) * 96;
     T.wi = wi; T.gplane = (L.npos / 32) * 96; T.bar = 1;
     return T;
 }
 __device__ __forceinline__ void team_sync(const TeamS& T) { asm volatile("bar.sync %0, %1;" ::"r"(T.bar), "n"(kTeamW * 32) : "memory"); }
-// gradient words of the atom at blk offset `off` in plane w: +0, +32, +64
-__device__ __forceinline__ float* team_gptr(const TeamS& T, int w, int off) {
-    return w == 0 ? T.S.blk + off + kGX : T.gextra + (w - 1) * T.gplane + (off >> 8) * 96 + (off & 31);
+// index in a plane of the atom at blk offset `off` (256 floats per 32 atoms -> 96): words +0, +32, +64
+__device__ __forceinline__ int plane_index(int off) { return off - (off >> 8) * 160; }
+template <bool MAYPAD>
+__device__ __forceinline__ void team_pair_apply(float* plane, const PairOut& o) {
+    float* gi = plane + plane_index(o.oi), *gj = plane + plane_index(o.oj);
+    if (!MAYPAD || o.valid) { gi[0] += o.fx; gi[32] += o.fy; gi[64] += o.fz; }
+    __syncwarp();
+    if (!MAYPAD || o.valid) { gj[0] -= o.fx; gj[32] -= o.fy; gj[64] -= o.fz; }
+    __syncwarp();
 }
 
 template <bool GRAD>
@@ -739,8 +770,7 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
         }
     }
     team_sync(T);
-    // (a1,a2) atoms: one thread per position (pose + trilinear lookup); the owner also clears the atom's extra planes
-    float eg = 0.f, rFx = 0.f, rFy = 0.f, rFz = 0.f, rTx = 0.f, rTy = 0.f, rTz = 0.f;     // rigid-body sums: grid forces only (eval_pose)
+    // (a1) atoms: one thread per position (pose, request for the two map sectors); the owner also clears the atom's planes
     for (int i = wi * 32 + lane; i < L.npos; i += 32 * kTeamW) {
         const uint32_t m = L.meta[i];
         if (m == 0xffffffffu) continue;                  // hole
@@ -753,17 +783,60 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
         const int off = atom_slot_dev(i);
         float* b = S.blk + off;
         b[kX] = x; b[kY] = y; b[kZ] = z; b[kQ] = a.w * P.elec_sqrt;
-        float gx, gy, gz;
-        eg += grid_atom<GRAD>(G, P, (int)(m & 0xff), a.w, x, y, z, gx, gy, gz);
+        grid_prefetch(G, grid_cell(G, (int)(m & 0xff), x, y, z));
         if (GRAD) {
-            b[kGX] = gx; b[kGY] = gy; b[kGZ] = gz;
+            float* g = T.gpl + plane_index(off);
+#pragma unroll
+            for (int w = 0; w < kTeamW; ++w) { g[w * T.gplane] = 0.f; g[w * T.gplane + 32] = 0.f; g[w * T.gplane + 64] = 0.f; }
+        }
+    }
+    team_sync(T);
+
+    // (a3) intramolecular pairs: warp wi takes rounds wi, wi + W, ...; forces go to plane wi.  Two full rounds at a time:
+    // the arithmetic of both is independent of the force updates, which follow in round order.
+    float ep = 0.f;
+    float* plane = T.gpl + wi * T.gplane;
+    int r = wi;
+    for (; r + kTeamW < L.nfull; r += 2 * kTeamW) {
+        const PairOut o0 = pair_compute<GRAD, false>(L, P, S, r, lane), o1 = pair_compute<GRAD, false>(L, P, S, r + kTeamW, lane);
+        if (GRAD) { team_pair_apply<false>(plane, o0); team_pair_apply<false>(plane, o1); }
+        ep += o0.e; ep += o1.e;
+    }
+    for (; r < L.nrounds; r += kTeamW) {
+        const PairOut o = pair_compute<GRAD, true>(L, P, S, r, lane);
+        if (GRAD) team_pair_apply<true>(plane, o);
+        ep += o.e;
+    }
+    team_sync(T);
+
+    // (a2) trilinear lookups, after the pairs so that the sectors asked for in (a1) have arrived, and (a4) back-propagation
+    // over the whole team.  (i) a thread per atom looks the atom up, adds the planes to the grid gradient (fixed order
+    // grid+0+1+2+3) and leaves the atom's torque about t in its plane-0 words; (ii) a thread per (fragment f > 0, component c
+    // of F(3) | T(3)) sums c over the fragment's atoms; (iii) the same thread sums c over the fragment's subtree
+    // [f, sub_end), and lane c = 0 of the eight collects the six sums: torsion gradient = u . (T - p x F), p = the pivot
+    // relative to t (lane_eval's form).  The root's sums are never needed: the rigid-body blocks are the grid-force sums.
+    float eg = 0.f, rFx = 0.f, rFy = 0.f, rFz = 0.f, rTx = 0.f, rTy = 0.f, rTz = 0.f;     // rigid-body sums: grid forces only (eval_pose)
+    for (int i = wi * 32 + lane; i < L.npos; i += 32 * kTeamW) {
+        const uint32_t m = L.meta[i];
+        if (m == 0xffffffffu) continue;
+        const int off = atom_slot_dev(i);
+        float* b = S.blk + off;
+        const float x = b[kX], y = b[kY], z = b[kZ];
+        float gx, gy, gz;
+        eg += grid_atom_l1<GRAD>(G, P, (int)(m & 0xff), L.atoms[i].w, x, y, z, gx, gy, gz);
+        if (GRAD) {
             const float rx = x - tx, ry = y - ty, rz = z - tz;
             rFx += gx; rFy += gy; rFz += gz;
             rTx += ry * gz - rz * gy; rTy += rz * gx - rx * gz; rTz += rx * gy - ry * gx;
+            float* g = T.gpl + plane_index(off);
 #pragma unroll
-            for (int w = 1; w < kTeamW; ++w) { float* g = team_gptr(T, w, off); g[0] = 0.f; g[32] = 0.f; g[64] = 0.f; }
+            for (int w = 0; w < kTeamW; ++w) { gx += g[w * T.gplane]; gy += g[w * T.gplane + 32]; gz += g[w * T.gplane + 64]; }
+            b[kGX] = gx; b[kGY] = gy; b[kGZ] = gz;
+            g[0] = ry * gz - rz * gy; g[32] = rz * gx - rx * gz; g[64] = rx * gy - ry * gx;        // plane 0: the atom's torque
         }
     }
+    eg = warp_sum(eg); ep = warp_sum(ep);
+    if (lane == 0) { T.red[8 * wi] = eg; T.red[8 * wi + 1] = ep; }
     if (GRAD) {
         rFx = warp_sum(rFx); rFy = warp_sum(rFy); rFz = warp_sum(rFz);
         rTx = warp_sum(rTx); rTy = warp_sum(rTy); rTz = warp_sum(rTz);
@@ -773,54 +846,17 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
         }
     }
     team_sync(T);
-
-    // (a3) intramolecular pairs: warp wi takes rounds wi, wi + W, ...; forces go to plane wi
-    float ep = 0.f;
-    for (int r = wi; r < L.nrounds; r += kTeamW) {
-        PairOut o = r < L.nfull ? pair_compute<GRAD, false>(L, P, S, r, lane) : pair_compute<GRAD, true>(L, P, S, r, lane);
-        if (GRAD) {
-            float* gi = team_gptr(T, wi, (int)(o.pi - S.blk)), *gj = team_gptr(T, wi, (int)(o.pj - S.blk));
-            if (o.valid) { gi[0] += o.fx; gi[32] += o.fy; gi[64] += o.fz; }
-            __syncwarp();
-            if (o.valid) { gj[0] -= o.fx; gj[32] -= o.fy; gj[64] -= o.fz; }
-            __syncwarp();
-        }
-        ep += o.e;
-    }
-    eg = warp_sum(eg); ep = warp_sum(ep);
-    if (lane == 0) { T.red[8 * wi] = eg; T.red[8 * wi + 1] = ep; }
-    team_sync(T);
     e_inter = 0.f; e_intra = 0.f;
 #pragma unroll
     for (int w = 0; w < kTeamW; ++w) { e_inter += T.red[8 * w]; e_intra += T.red[8 * w + 1]; }
-
-    // (a4) back-propagation over the whole team.  (i) a thread per atom sums the planes (fixed order 0+1+2+3) and leaves the
-    // atom's torque about t in its plane-1 words; (ii) a thread per (fragment f > 0, component c of F(3) | T(3)) sums c over
-    // the fragment's atoms; (iii) the same thread sums c over the fragment's subtree [f, sub_end), and lane c = 0 of the
-    // eight collects the six sums: torsion gradient = u . (T - p x F), p = the pivot relative to t (lane_eval's form).
-    // The root's sums are never needed: the rigid-body blocks are the grid-force sums of (a2).
     if (GRAD) {
-        for (int i = wi * 32 + lane; i < L.npos; i += 32 * kTeamW) {
-            if (L.meta[i] == 0xffffffffu) continue;
-            const int off = atom_slot_dev(i);
-            float* b = S.blk + off;
-            float gx = b[kGX], gy = b[kGY], gz = b[kGZ];
-            float* g1 = team_gptr(T, 1, off);
-            gx += g1[0]; gy += g1[32]; gz += g1[64];
-#pragma unroll
-            for (int w = 2; w < kTeamW; ++w) { const float* g = team_gptr(T, w, off); gx += g[0]; gy += g[32]; gz += g[64]; }
-            b[kGX] = gx; b[kGY] = gy; b[kGZ] = gz;
-            const float rx = b[kX] - tx, ry = b[kY] - ty, rz = b[kZ] - tz;
-            g1[0] = ry * gz - rz * gy; g1[32] = rz * gx - rx * gz; g1[64] = rx * gy - ry * gx;
-        }
-        team_sync(T);
         float* ft = reinterpret_cast<float*>(S.fragFT);                 // [nfrag][8]: F(3), T(3) about t
         const int nitem = 8 * L.nfrag, tid = wi * 32 + lane;
         for (int it = 8 + tid; it < nitem; it += 32 * kTeamW) {
             const int f = it >> 3, c = it & 7;
             if (c >= 6) continue;
             const int4 ix = L.fi[f];
-            const float* src = c < 3 ? S.blk + kGX + 32 * c : T.gextra + 32 * (c - 3);
+            const float* src = c < 3 ? S.blk + kGX + 32 * c : T.gpl + 32 * (c - 3);
             float v = 0.f;
             for (int k = ix.y; k < ix.z; ++k) {
                 const int off = atom_slot_dev(L.fragatoms[k]);
@@ -835,7 +871,7 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
             S.grad[lane] = v;
         }
         team_sync(T);
-        for (int base = 8 + wi * 32; base < nitem; base += 32 * kTeamW) {       // the same for every lane of a warp
+        for (int base = 8 + wi * 32; base < nitem; base += 32 * kTeamW) {       // 8 lanes per fragment
             const int it = base + lane, f = it >> 3, c = it & 7;
             int w = 0;
             float v = 0.f;
