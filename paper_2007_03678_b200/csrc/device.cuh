@@ -59,7 +59,7 @@ struct WarpS {
     float2* sc;             // [nfrag] sin,cos of the fragment's torsion
     float4* fragT;          // [nfrag][3] rows of the 3x4 fragment transform
     float4* fragAx;         // [nfrag][2] posed axis, posed pivot point - t
-    float4* fragFT;         // [nfrag][2] force, torque about the fragment's own pivot point (team kernel: about t)
+    float4* fragFT;         // [nfrag][2] force, torque about the fragment's own pivot point
     float* blk;             // pose block, 256 floats per 32 atoms: x|y|z|q|gx|gy|gz|-  (32 each), so atom a
                             // lives at slot(a) = (a>>5)*256 + (a&31) and distinct a mod 32 hit distinct banks
 };
@@ -288,6 +288,19 @@ __device__ __forceinline__ float frcp(float x) { float r; asm("rcp.approx.ftz.f3
 __device__ __forceinline__ float frsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float fex2(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 
+// eight sums at once: returns, in every lane, the sum over the warp of v[(lane >> 2) & 7] (9 shuffles; fixed order)
+__device__ __forceinline__ float warp_sum8(const float (&v)[8], int lane) {
+    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+    float a[4], c[2];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) a[k] = (b4 ? v[k + 4] : v[k]) + __shfl_xor_sync(kFull, b4 ? v[k] : v[k + 4], 16);
+#pragma unroll
+    for (int k = 0; k < 2; ++k) c[k] = (b3 ? a[k + 2] : a[k]) + __shfl_xor_sync(kFull, b3 ? a[k] : a[k + 2], 8);
+    float d = (b2 ? c[1] : c[0]) + __shfl_xor_sync(kFull, b2 ? c[0] : c[1], 4);
+    d += __shfl_xor_sync(kFull, d, 2);
+    d += __shfl_xor_sync(kFull, d, 1);
+    return d;
+}
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
@@ -809,13 +822,9 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
     }
     team_sync(T);
 
-    // (a2) trilinear lookups, after the pairs so that the sectors asked for in (a1) have arrived, and (a4) back-propagation
-    // over the whole team.  (i) a thread per atom looks the atom up, adds the planes to the grid gradient (fixed order
-    // grid+0+1+2+3) and leaves the atom's torque about t in its plane-0 words; (ii) a thread per (fragment f > 0, component c
-    // of F(3) | T(3)) sums c over the fragment's atoms; (iii) the same thread sums c over the fragment's subtree
-    // [f, sub_end), and lane c = 0 of the eight collects the six sums: torsion gradient = u . (T - p x F), p = the pivot
-    // relative to t (lane_eval's form).  The root's sums are never needed: the rigid-body blocks are the grid-force sums.
-    float eg = 0.f, rFx = 0.f, rFy = 0.f, rFz = 0.f, rTx = 0.f, rTy = 0.f, rTz = 0.f;     // rigid-body sums: grid forces only (eval_pose)
+    // (a2) trilinear lookups, after the pairs so that the sectors asked for in (a1) have arrived: a thread per atom looks the
+    // atom up and adds the planes to the grid gradient (fixed order grid+0+1+2+3).
+    float red[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};      // e_grid, e_pairs, rigid-body sums F(3), T(3): grid forces only (eval_pose)
     for (int i = wi * 32 + lane; i < L.npos; i += 32 * kTeamW) {
         const uint32_t m = L.meta[i];
         if (m == 0xffffffffu) continue;
@@ -823,71 +832,63 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
         float* b = S.blk + off;
         const float x = b[kX], y = b[kY], z = b[kZ];
         float gx, gy, gz;
-        eg += grid_atom_l1<GRAD>(G, P, (int)(m & 0xff), L.atoms[i].w, x, y, z, gx, gy, gz);
+        red[0] += grid_atom_l1<GRAD>(G, P, (int)(m & 0xff), L.atoms[i].w, x, y, z, gx, gy, gz);
         if (GRAD) {
             const float rx = x - tx, ry = y - ty, rz = z - tz;
-            rFx += gx; rFy += gy; rFz += gz;
-            rTx += ry * gz - rz * gy; rTy += rz * gx - rx * gz; rTz += rx * gy - ry * gx;
-            float* g = T.gpl + plane_index(off);
+            red[2] += gx; red[3] += gy; red[4] += gz;
+            red[5] += ry * gz - rz * gy; red[6] += rz * gx - rx * gz; red[7] += rx * gy - ry * gx;
+            const float* g = T.gpl + plane_index(off);
 #pragma unroll
             for (int w = 0; w < kTeamW; ++w) { gx += g[w * T.gplane]; gy += g[w * T.gplane + 32]; gz += g[w * T.gplane + 64]; }
             b[kGX] = gx; b[kGY] = gy; b[kGZ] = gz;
-            g[0] = ry * gz - rz * gy; g[32] = rz * gx - rx * gz; g[64] = rx * gy - ry * gx;        // plane 0: the atom's torque
         }
     }
-    eg = warp_sum(eg); ep = warp_sum(ep);
-    if (lane == 0) { T.red[8 * wi] = eg; T.red[8 * wi + 1] = ep; }
-    if (GRAD) {
-        rFx = warp_sum(rFx); rFy = warp_sum(rFy); rFz = warp_sum(rFz);
-        rTx = warp_sum(rTx); rTy = warp_sum(rTy); rTz = warp_sum(rTz);
-        if (lane == 0) {
-            float* r = T.red + 8 * wi + 2;
-            r[0] = rFx; r[1] = rFy; r[2] = rFz; r[3] = rTx; r[4] = rTy; r[5] = rTz;
-        }
-    }
+    red[1] = ep;
+    const float part = warp_sum8(red, lane);
+    if ((lane & 3) == 0) T.red[8 * wi + (lane >> 2)] = part;
     team_sync(T);
     e_inter = 0.f; e_intra = 0.f;
 #pragma unroll
     for (int w = 0; w < kTeamW; ++w) { e_inter += T.red[8 * w]; e_intra += T.red[8 * w + 1]; }
+
+    // (a4) back-propagation: eight lanes per torsion share the atoms of its subtree (a contiguous range of the fragment-ordered
+    // atom list), each summing u . ((r - pivot) x g) over its atoms; eval_pose's terms in another (fixed) order.  The
+    // rigid-body blocks are the warps' grid-force sums.
     if (GRAD) {
-        float* ft = reinterpret_cast<float*>(S.fragFT);                 // [nfrag][8]: F(3), T(3) about t
-        const int nitem = 8 * L.nfrag, tid = wi * 32 + lane;
-        for (int it = 8 + tid; it < nitem; it += 32 * kTeamW) {
-            const int f = it >> 3, c = it & 7;
-            if (c >= 6) continue;
-            const int4 ix = L.fi[f];
-            const float* src = c < 3 ? S.blk + kGX + 32 * c : T.gpl + 32 * (c - 3);
-            float v = 0.f;
-            for (int k = ix.y; k < ix.z; ++k) {
-                const int off = atom_slot_dev(L.fragatoms[k]);
-                v += src[c < 3 ? off : (off >> 8) * 96 + (off & 31)];
+        const int nitem = 8 * (L.nfrag - 1);
+        for (int base = wi * 32; base < nitem; base += 32 * kTeamW) {
+            const int it = base + lane, f = 1 + (it >> 3);
+            float v0 = 0.f, v1 = 0.f;
+            int w = 0;
+            if (it < nitem) {
+                const int4 ix = L.fi[f];
+                w = ix.w;
+                const int kend = L.fi[(w & 0xffff) - 1].z;
+                const float4 u = S.fragAx[2 * f], pv = S.fragAx[2 * f + 1];
+                const float px = tx + pv.x, py = ty + pv.y, pz = tz + pv.z;
+                int k = ix.y + (it & 7);
+                for (; k + 8 < kend; k += 16) {
+                    const float* b0 = S.blk + atom_slot_dev(L.fragatoms[k]), *b1 = S.blk + atom_slot_dev(L.fragatoms[k + 8]);
+                    const float gx0 = b0[kGX], gy0 = b0[kGY], gz0 = b0[kGZ], rx0 = b0[kX] - px, ry0 = b0[kY] - py, rz0 = b0[kZ] - pz;
+                    const float gx1 = b1[kGX], gy1 = b1[kGY], gz1 = b1[kGZ], rx1 = b1[kX] - px, ry1 = b1[kY] - py, rz1 = b1[kZ] - pz;
+                    v0 += u.x * (ry0 * gz0 - rz0 * gy0) + u.y * (rz0 * gx0 - rx0 * gz0) + u.z * (rx0 * gy0 - ry0 * gx0);
+                    v1 += u.x * (ry1 * gz1 - rz1 * gy1) + u.y * (rz1 * gx1 - rx1 * gz1) + u.z * (rx1 * gy1 - ry1 * gx1);
+                }
+                if (k < kend) {
+                    const float* b0 = S.blk + atom_slot_dev(L.fragatoms[k]);
+                    const float gx0 = b0[kGX], gy0 = b0[kGY], gz0 = b0[kGZ], rx0 = b0[kX] - px, ry0 = b0[kY] - py, rz0 = b0[kZ] - pz;
+                    v0 += u.x * (ry0 * gz0 - rz0 * gy0) + u.y * (rz0 * gx0 - rx0 * gz0) + u.z * (rx0 * gy0 - ry0 * gx0);
+                }
             }
-            ft[it] = v;
+            float v = v0 + v1;
+            v += __shfl_xor_sync(kFull, v, 4); v += __shfl_xor_sync(kFull, v, 2); v += __shfl_xor_sync(kFull, v, 1);
+            if (it < nitem && (it & 7) == 0) S.grad[6 + (w >> 16)] = v;
         }
-        if (wi == kTeamW - 1 && lane < 6) {             // rigid-body blocks: the warps' grid-force sums, fixed order
+        if (wi == kTeamW - 1 && lane < 6) {             // rigid-body blocks, fixed order
             float v = T.red[2 + lane];
 #pragma unroll
             for (int w = 1; w < kTeamW; ++w) v += T.red[8 * w + 2 + lane];
             S.grad[lane] = v;
-        }
-        team_sync(T);
-        for (int base = 8 + wi * 32; base < nitem; base += 32 * kTeamW) {       // 8 lanes per fragment
-            const int it = base + lane, f = it >> 3, c = it & 7;
-            int w = 0;
-            float v = 0.f;
-            if (it < nitem) {
-                w = L.fi[f].w;
-                const int sub_end = w & 0xffff;
-                if (c < 6) for (int g = f; g < sub_end; ++g) v += ft[8 * g + c];
-            }
-            const int l0 = lane & ~7;
-            const float Fx = __shfl_sync(kFull, v, l0), Fy = __shfl_sync(kFull, v, l0 + 1), Fz = __shfl_sync(kFull, v, l0 + 2);
-            const float Tx = __shfl_sync(kFull, v, l0 + 3), Ty = __shfl_sync(kFull, v, l0 + 4), Tz = __shfl_sync(kFull, v, l0 + 5);
-            if (it < nitem && c == 0) {
-                const float4 u = S.fragAx[2 * f], pv = S.fragAx[2 * f + 1];
-                S.grad[6 + (w >> 16)] = u.x * (Tx - (pv.y * Fz - pv.z * Fy)) + u.y * (Ty - (pv.z * Fx - pv.x * Fz)) +
-                                        u.z * (Tz - (pv.x * Fy - pv.y * Fx));
-            }
         }
         team_sync(T);
     }
