@@ -736,22 +736,20 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
         return __int_as_float(0x7fc00000);
     }
     if (wi == 0) {                                      // (a1) fragment transforms: eval_pose's code on warp 0
+        if (GRAD && lane == 31) T.red[8 * kTeamW] = 1.f;                // "every gradient component is finite" until a writer says no
         const float qi = 1.0f / sqrtf(qn2);
         qw *= qi; qx *= qi; qy *= qi; qz *= qi;
         const float r00 = 1.f - 2.f * (qy * qy + qz * qz), r01 = 2.f * (qx * qy - qw * qz), r02 = 2.f * (qx * qz + qw * qy);
         const float r10 = 2.f * (qx * qy + qw * qz), r11 = 1.f - 2.f * (qx * qx + qz * qz), r12 = 2.f * (qy * qz - qw * qx);
         const float r20 = 2.f * (qx * qz - qw * qy), r21 = 2.f * (qy * qz + qw * qx), r22 = 1.f - 2.f * (qx * qx + qy * qy);
-        for (int f = lane; f < L.nfrag; f += 32) {
-            float s = 0.f, c = 1.f;
-            if (f > 0) sincosf(S.geno[7 + (L.fi[f].w >> 16)], &s, &c);
-            S.sc[f] = make_float2(s, c);
-        }
-        __syncwarp();
+        // S.sc[t] = (sin, cos) of torsion t: left there by the caller (team_sincos, adadelta_search_team's update)
         for (int f = lane; f < L.nfrag; f += 32) {
             float m00 = 1, m01 = 0, m02 = 0, m03 = 0, m10 = 0, m11 = 1, m12 = 0, m13 = 0, m20 = 0, m21 = 0, m22 = 1, m23 = 0;
-            for (int cur = f; cur > 0; cur = L.fi[cur].x) {
+            int4 ix;
+            for (int cur = f; cur > 0; cur = ix.x) {
+                ix = L.fi[cur];
                 const float4 p0 = L.fg[2 * cur], u = L.fg[2 * cur + 1];
-                const float2 sc = S.sc[cur];
+                const float2 sc = S.sc[ix.w >> 16];
                 const float s = sc.x, c = sc.y, k = 1.f - c;
                 const float a00 = fmaf(k * u.x, u.x, c), a01 = fmaf(k * u.x, u.y, -s * u.z), a02 = fmaf(k * u.x, u.z, s * u.y);
                 const float a10 = fmaf(k * u.x, u.y, s * u.z), a11 = fmaf(k * u.y, u.y, c), a12 = fmaf(k * u.y, u.z, -s * u.x);
@@ -882,13 +880,17 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
             }
             float v = v0 + v1;
             v += __shfl_xor_sync(kFull, v, 4); v += __shfl_xor_sync(kFull, v, 2); v += __shfl_xor_sync(kFull, v, 1);
-            if (it < nitem && (it & 7) == 0) S.grad[6 + (w >> 16)] = v;
+            if (it < nitem && (it & 7) == 0) {
+                S.grad[6 + (w >> 16)] = v;
+                if (!isfinite(v)) T.red[8 * kTeamW] = 0.f;
+            }
         }
         if (wi == kTeamW - 1 && lane < 6) {             // rigid-body blocks, fixed order
             float v = T.red[2 + lane];
 #pragma unroll
             for (int w = 1; w < kTeamW; ++w) v += T.red[8 * w + 2 + lane];
             S.grad[lane] = v;
+            if (!isfinite(v)) T.red[8 * kTeamW] = 0.f;
         }
         team_sync(T);
     }
@@ -965,74 +967,70 @@ __device__ inline float adadelta_search(const LigS& L, const GridDev& G, const P
 }
 
 // ---------------------------------------------------------------- ADADELTA local search (R7), one team
-// adadelta_search with the evaluation spread over the team; warp 0 owns the optimiser state and takes every decision,
-// the other warps follow through a flag in shared memory.  Called by all kTeamW warps with S.geno ready and visible.
+// adadelta_search with the evaluation spread over the team and the update spread over its threads: every thread sees the
+// energy and the "gradient finite" flag and takes the same decisions; thread d < 3 of warp 0 owns translation component d,
+// thread 32 + t torsion t (it also leaves sin/cos of the new angle for the next pose), lanes 0..2 of the last warp the
+// rotation components, whose steps lane 0 gathers for the quaternion.  A thread that overwrites a gene saves the old value
+// into S.best first when the pose improved.  Called by all kTeamW warps with S.geno ready and visible.
+__device__ __forceinline__ float adadelta_step(const ParDev& P, float g, float& Eg2, float& Ed2) {
+    Eg2 = P.ad_rho * Eg2 + (1.f - P.ad_rho) * g * g;
+    const float dl = -(sqrtf(Ed2 + P.ad_eps) / sqrtf(Eg2 + P.ad_eps)) * g;
+    Ed2 = P.ad_rho * Ed2 + (1.f - P.ad_rho) * dl * dl;
+    return dl;
+}
 __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, const ParDev& P, const TeamS& T, int lane, float e_start,
                                              int& iters) {
+    static_assert(kTeamW == 4, "thread roles below: warp 0 translation, warps 1..2 torsions (<= 64), warp 3 rotation");
     const WarpS& S = T.S;
-    const int R = L.R, D = 6 + R, Gn = 7 + R;
-    const bool lead = T.wi == 0;
-    float Eg2[3] = {0.f, 0.f, 0.f}, Ed2[3] = {0.f, 0.f, 0.f};         // component d = lane + 32*c on warp 0
+    const int R = L.R, Gn = 7 + R, tid = T.wi * 32 + lane;
+    const int tor = tid - 32;                           // this thread's torsion, if 0 <= tor < R
+    float Eg2 = 0.f, Ed2 = 0.f;                         // of the component this thread owns
     float bestE = __int_as_float(0x7f800000);
-    if (lead) for (int d = lane; d < Gn; d += 32) S.best[d] = S.geno[d];
+    for (int d = tid; d < Gn; d += 32 * kTeamW) S.best[d] = S.geno[d];
+    if (tor >= 0 && tor < R) {
+        float s, c;
+        sincosf(S.geno[7 + tor], &s, &c);
+        S.sc[tor] = make_float2(s, c);
+    }
+    team_sync(T);
     int it = 0;
     while (it < P.lsit) {
         float ei, ea;
-        const float e = eval_pose_team<true>(L, G, P, T, lane, ei, ea);      // ends with a team barrier: S.grad is visible
+        const float e = eval_pose_team<true>(L, G, P, T, lane, ei, ea);      // ends with a team barrier: S.grad and the flag are visible
         ++it;
-        if (lead) {
-            bool ok = isfinite(e);
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const int d = lane + 32 * c;
-                if (d < D) ok = ok && isfinite(S.grad[d]);
-            }
-            ok = __all_sync(kFull, ok);
-            if (lane == 0) T.red[8 * kTeamW] = ok ? 1.f : 0.f;
-            if (ok) {
-                if (e < bestE) {
-                    bestE = e;
-                    for (int d = lane; d < Gn; d += 32) S.best[d] = S.geno[d];
-                }
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    const int d = lane + 32 * c;
-                    if (d < D) {
-                        const float g = S.grad[d];
-                        Eg2[c] = P.ad_rho * Eg2[c] + (1.f - P.ad_rho) * g * g;
-                        const float dl = -(sqrtf(Ed2[c] + P.ad_eps) / sqrtf(Eg2[c] + P.ad_eps)) * g;
-                        Ed2[c] = P.ad_rho * Ed2[c] + (1.f - P.ad_rho) * dl * dl;
-                        S.grad[d] = dl;
-                    }
-                }
-                __syncwarp();
-                float newv[3];
-                float newq[4];
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    const int gI = lane + 32 * c;
-                    if (gI < 3) newv[c] = S.geno[gI] + S.grad[gI];
-                    else if (gI >= 7 && gI < Gn) newv[c] = wrap_pi(S.geno[gI] + S.grad[gI - 1]);
-                }
-                if (lane == 3) {
-                    const float wx = S.grad[3], wy = S.grad[4], wz = S.grad[5];
-                    const float th = sqrtf(wx * wx + wy * wy + wz * wz);
-                    float sh, ch;
-                    sincosf(0.5f * th, &sh, &ch);
-                    const float k = th > 1e-12f ? sh / th : 0.5f;
-                    rotate_quat(ch, k * wx, k * wy, k * wz, S.geno + 3, newq);
-                }
-                __syncwarp();
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    const int gI = lane + 32 * c;
-                    if (gI < 3 || (gI >= 7 && gI < Gn)) S.geno[gI] = newv[c];
-                }
-                if (lane == 3) { S.geno[3] = newq[0]; S.geno[4] = newq[1]; S.geno[5] = newq[2]; S.geno[6] = newq[3]; }
+        if (!(isfinite(e) && T.red[8 * kTeamW] != 0.f)) break;              // the same in every thread
+        const bool improved = e < bestE;
+        if (improved) bestE = e;
+        if (tid < 3) {
+            const float dl = adadelta_step(P, S.grad[tid], Eg2, Ed2);
+            const float old = S.geno[tid];
+            if (improved) S.best[tid] = old;
+            S.geno[tid] = old + dl;
+        } else if (tor >= 0 && tor < R) {
+            const float dl = adadelta_step(P, S.grad[6 + tor], Eg2, Ed2);
+            const float old = S.geno[7 + tor];
+            if (improved) S.best[7 + tor] = old;
+            const float nv = wrap_pi(old + dl);
+            S.geno[7 + tor] = nv;
+            float s, c;
+            sincosf(nv, &s, &c);
+            S.sc[tor] = make_float2(s, c);
+        } else if (T.wi == kTeamW - 1) {
+            float dl = 0.f;
+            if (lane < 3) dl = adadelta_step(P, S.grad[3 + lane], Eg2, Ed2);
+            const float wx = __shfl_sync(kFull, dl, 0), wy = __shfl_sync(kFull, dl, 1), wz = __shfl_sync(kFull, dl, 2);
+            if (lane == 0) {
+                float oldq[4] = {S.geno[3], S.geno[4], S.geno[5], S.geno[6]}, newq[4];
+                if (improved) { S.best[3] = oldq[0]; S.best[4] = oldq[1]; S.best[5] = oldq[2]; S.best[6] = oldq[3]; }
+                const float th = sqrtf(wx * wx + wy * wy + wz * wz);
+                float sh, ch;
+                sincosf(0.5f * th, &sh, &ch);
+                const float k = th > 1e-12f ? sh / th : 0.5f;
+                rotate_quat(ch, k * wx, k * wy, k * wz, oldq, newq);
+                S.geno[3] = newq[0]; S.geno[4] = newq[1]; S.geno[5] = newq[2]; S.geno[6] = newq[3];
             }
         }
-        team_sync(T);                                    // new genotype and the flag are visible
-        if (T.red[8 * kTeamW] == 0.f) break;
+        team_sync(T);                                    // new genotype visible
     }
     iters = it;
     return isfinite(bestE) ? bestE : e_start;
