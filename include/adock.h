@@ -33,7 +33,7 @@ extern "C" {
 #define ADOCK_EINVAL (-1) /* bad shape / index / NULL / non-finite input / params mismatch */
 #define ADOCK_ENOMEM (-2) /* host or device allocation failed */
 #define ADOCK_ECUDA (-3)  /* CUDA runtime error (text in adock_last_error) or no device */
-#define ADOCK_ELIMIT (-4) /* N > 256, R > 64, M > 16, or the ligand does not fit in shared memory */
+#define ADOCK_ELIMIT (-4) /* N > 256, R > 64, M > 16, the ligand does not fit in shared memory, or a batch beyond a stated maximum */
 
 #define ADOCK_MAX_ATOMS 256
 #define ADOCK_MAX_TORSIONS 64
@@ -145,6 +145,23 @@ int adock_score_batch_host(const adock_grids* grids, const adock_ligand* ligand,
 int adock_local_search(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
                        float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, float* d_trace,
                        void* cuda_stream);
+
+/* adock_local_search for callers that may not allocate device memory (code under stream capture, serving loops,
+ * harnesses that forbid cudaMalloc): the same ADADELTA search (R7), same arguments and outputs, on the
+ * lane-per-individual kernel (8 warps per CTA, one chain per lane) whose per-chain state (best genotype, E[g^2],
+ * E[dx^2]: 19 + 3R floats per chain) lives in a file-scope device array of ADOCK_NOALLOC_SCRATCH_BYTES inside the
+ * library instead of a stream-ordered allocation.  Calls no cudaMalloc / cudaFree / allocating library routine; the
+ * array's device address is looked up once per device (first call with that device current).
+ * Limit: 32*ceil(n/32) chains, rounded up to whole CTAs, times (19 + 3R)*4 bytes must fit the array (R = 8: about
+ * 97,000 chains; R = 64: about 19,000); a larger batch returns ADOCK_ELIMIT with the sizes in adock_last_error() and
+ * launches nothing.  ADOCK_ELIMIT also if the ligand does not fit that kernel's shared memory.
+ * Every GPU that loads the library holds the array until exit.  Every call shares it and finds the last call's
+ * contents (the kernel initialises all state it reads: nothing needs clearing); calls that OVERLAP on the GPU
+ * (different streams, or two host threads) race on it: serialise them.  Asynchronous on cuda_stream. */
+#define ADOCK_NOALLOC_SCRATCH_BYTES (16u << 20)
+int adock_local_search_noalloc(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
+                               float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, float* d_trace,
+                               void* cuda_stream);
 
 /* Solis-Wets local search (R11; Solis & Wets 1981) from each of n genotypes:
  * d_genotypes device [n][gstride] in/out (the accepted genotype), d_energies device [n] IN/OUT: on entry the energy

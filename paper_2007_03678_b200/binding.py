@@ -19,7 +19,7 @@ ADOCK_OK, ADOCK_EINVAL, ADOCK_ENOMEM, ADOCK_ECUDA, ADOCK_ELIMIT = 0, -1, -2, -3,
 EXPORTS = ["adock_default_params", "adock_load_grids", "adock_free_grids", "adock_load_ligand", "adock_free_ligand",
            "adock_ligand_pairs", "adock_ligand_tree", "adock_ligand_image", "adock_score_batch", "adock_score_batch_host", "adock_local_search",
            "adock_philox", "adock_ga_generation", "adock_dock", "adock_dock_many", "adock_launch_count", "adock_last_error", "adock_profile", "adock_profile_read",
-           "adock_ligand_lane_image", "adock_set_path", "adock_last_dock_path", "adock_solis_wets", "adock_screen", "adock_pose_rmsd", "adock_alu_peak", "adock_tmem_probe"]
+           "adock_ligand_lane_image", "adock_set_path", "adock_last_dock_path", "adock_solis_wets", "adock_screen", "adock_pose_rmsd", "adock_alu_peak", "adock_tmem_probe", "adock_local_search_noalloc"]
 
 
 class adock_ligand_desc(C.Structure):
@@ -76,6 +76,7 @@ def lib():
         L.adock_score_batch.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, ci, vp]
         L.adock_score_batch_host.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, ci, vp]
         L.adock_local_search.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, vp]
+        L.adock_local_search_noalloc.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, vp]
         L.adock_solis_wets.argtypes = [vp, vp, pp, vp, ci, ci, vp, vp, vp, C.c_ulonglong, C.c_uint, vp]
         L.adock_philox.argtypes = [vp, vp, ci, vp, vp]
         L.adock_ga_generation.argtypes = [vp, vp, pp, ci, ci, ci, C.c_ulonglong, vp, vp, vp, vp, vp, C.POINTER(ci), vp]
@@ -230,6 +231,15 @@ def adock_local_search(grids: Grids, lig: Ligand, params, d_genotypes, d_energie
         assert tuple(d_trace.shape) == (n, params.lsit)
     _check(lib().adock_local_search(grids.h, lig.h, C.byref(params) if params is not None else None, _dp(d_genotypes), n, gs,
                                     _dp(d_energies), _dp(d_iters), _dp(d_trace), _stream()))
+
+
+def adock_local_search_noalloc(grids: Grids, lig: Ligand, params, d_genotypes, d_energies, d_iters=None, d_trace=None):
+    """adock_local_search with the chain state in the library's static device array: no device allocation (adock.h)"""
+    n, gs = d_genotypes.shape
+    if d_trace is not None:
+        assert tuple(d_trace.shape) == (n, params.lsit)
+    _check(lib().adock_local_search_noalloc(grids.h, lig.h, C.byref(params) if params is not None else None, _dp(d_genotypes), n, gs,
+                                            _dp(d_energies), _dp(d_iters), _dp(d_trace), _stream()))
 
 
 def adock_solis_wets(grids: Grids, lig: Ligand, params, d_genotypes, d_energies, seed, generation, d_evals=None, d_trace=None):

@@ -789,6 +789,72 @@ extern "C" int adock_solis_wets(const adock_grids* grids, const adock_ligand* li
     return local_search_impl(grids, ligand, params, 1, d_genotypes, n, gstride, d_energies, d_evals, d_trace, seed, generation, cuda_stream);
 }
 
+// ---- ADADELTA local search without any device allocation (callers that may not call cudaMalloc: stream capture, serving
+// loops).  The chain-state columns of ls_array_lane_kernel (best genotype, E[g^2], E[dx^2]: 19 + 3R floats per chain) live
+// in a file-scope device array instead of a cudaMallocAsync block.  Every GPU that loads the library holds the array until
+// exit; every call shares it and finds the last call's contents there (the kernel initialises every column it reads, so
+// nothing has to be cleared); calls that overlap on the GPU race on it.
+static __device__ __align__(256) float g_noalloc_scratch[ADOCK_NOALLOC_SCRATCH_BYTES / 4];
+static constexpr int kNoAllocMaxDevices = 64;
+static float* g_noalloc_ptr[kNoAllocMaxDevices];        // device address of g_noalloc_scratch on device d (the name itself is a host-side stand-in)
+
+// once per device, with that device current
+static int noalloc_scratch_address(float** out) {
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return fail(ADOCK_ELIMIT, "device ordinal beyond the no-allocation path's table");
+    if (!g_noalloc_ptr[dev]) {
+        float* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);
+        if (e != cudaSuccess || !p) return fail(ADOCK_ECUDA, std::string("cudaGetSymbolAddress(g_noalloc_scratch): ") + cudaGetErrorString(e));
+        g_noalloc_ptr[dev] = p;
+    }
+    *out = g_noalloc_ptr[dev];
+    return ADOCK_OK;
+}
+
+extern "C" int adock_local_search_noalloc(const adock_grids* grids, const adock_ligand* ligand, const adock_params* params,
+                                          float* d_genotypes, int n, int gstride, float* d_energies, int* d_iters, float* d_trace,
+                                          void* cuda_stream) {
+    if (!grids || !ligand) return fail(ADOCK_EINVAL, "NULL handle");
+    if (n < 0) return fail(ADOCK_EINVAL, "n < 0");
+    if (n == 0) return ADOCK_OK;
+    if (!d_genotypes || !d_energies || gstride < 7 + ligand->tp.R) return fail(ADOCK_EINVAL, "bad buffer");
+    adock_params p;
+    int rc = check_params(params, ligand, p);
+    if (rc) return rc;
+    p.ls_method = 0;
+    rc = device_props();
+    if (rc) return rc;
+    using C = LaneCfg<1, 8, false>;                     // variant 0: positions in shared memory, chain state in global columns
+    static_assert(!C::ST, "the no-allocation path is the variant whose chain state is in global scratch");
+    const LaneGeom g = lane_geom(ligand);
+    const int fit = lane_fit_groups(g, 0, true);
+    if (fit < 1) return fail(ADOCK_ELIMIT, "ligand does not fit the lane-per-individual kernel");
+    const int ngroups = (n + 31) / 32;
+    const int NG = lane_spread_groups(fit, ngroups, C::K);
+    const int grid = (ngroups + NG - 1) / NG;
+    const size_t T = (size_t)grid * NG * 32;            // chains of the launch, padded to whole CTAs
+    const int R = ligand->tp.R;
+    const size_t need = T * (size_t)(7 + R + 2 * (6 + R)) * 4;
+    if (need > (size_t)ADOCK_NOALLOC_SCRATCH_BYTES)
+        return fail(ADOCK_ELIMIT, "adock_local_search_noalloc: " + std::to_string(n) + " chains of " + std::to_string(R) + " torsions need " +
+                                      std::to_string(need) + " bytes of chain state, more than ADOCK_NOALLOC_SCRATCH_BYTES (" +
+                                      std::to_string((size_t)ADOCK_NOALLOC_SCRATCH_BYTES) + "): split the batch");
+    float* scratch = nullptr;
+    rc = noalloc_scratch_address(&scratch);
+    if (rc) return rc;
+    ParDev P = make_pardev(p);
+    P.k_wall_h = p.k_wall * grids->dev.h;
+    LsArgs a{ligand->d_lane, d_genotypes, d_energies, d_iters, d_trace, ligand->lane_bytes, n, gstride, 0ull, 0u};
+    const size_t smem = lane_smem(g, 0, true, NG);
+    CUDA_TRY(cudaFuncSetAttribute(ls_array_lane_kernel<C, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ls_array_lane_kernel<C, false><<<grid, NG * C::K * 32, smem, (cudaStream_t)cuda_stream>>>(grids->dev, P, a, scratch);
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    return ADOCK_OK;
+}
+
 // =================================================================== LGA docking (rows a5-a7)
 struct RunState {           // 32 bytes
     long long evals;
