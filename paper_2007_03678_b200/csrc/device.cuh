@@ -697,17 +697,42 @@ __device__ inline void ga_make_child_thread(const ParDev& P, int Pn, int R, unsi
 // order.  Same arithmetic as eval_pose; the summation order differs (fixed, so results are reproducible).
 constexpr int kTeamW = 4;
 __host__ __device__ inline int team_scratch_floats(int N, int nfrag, int R) {
-    return warp_scratch_floats(N, nfrag, R) + kTeamW * ((N + 31) / 32) * 96 + 8 * kTeamW + 8;
+    return warp_scratch_floats(N, nfrag, R) + kTeamW * ((N + 31) / 32) * 96 + 8 * kTeamW + 8 + 4 * nfrag;
 }
 // red: per warp w [8w .. 8w+8) = partial (e_grid, e_pairs, grid force F(3), grid torque about t T(3)); [8 kTeamW] = flag
-struct TeamS { WarpS S; float* gpl; float* red; int wi, gplane, bar; };        // gplane = floats per plane; bar = the team's named barrier
+// Local transform of fragment f > 0 (rotation A by its torsion angle about its axis through p0: x -> A (x - p0) + p0) as three
+// rows (A_r0, A_r1, A_r2, p0_r): rows 0, 1 in S.fragFT[2f], S.fragFT[2f+1], row 2 in rowz[f]; slot 0 holds the rows of the
+// rigid-body rotation (w = 0).  Written by the thread that owns the torsion / the rotation (team_local_transform,
+// team_rotation), read by the pose builder.
+struct TeamS { WarpS S; float* gpl; float* red; float4* rowz; int wi, gplane, bar; };      // gplane = floats per plane; bar = the team's named barrier
 __device__ inline TeamS team_view(float* base, const LigS& L, int wi) {
     TeamS T;
     T.S = warp_view(base, L);
     T.gpl = T.S.blk + (L.npos / 32) * 256;
     T.red = T.gpl + kTeamW * (L.npos / 32) * 96;
+    T.rowz = reinterpret_cast<float4*>(T.red + 8 * kTeamW + 8);
     T.wi = wi; T.gplane = (L.npos / 32) * 96; T.bar = 1;
     return T;
+}
+// eval_pose's rotation about the torsion axis, for (sin, cos) of the angle
+__device__ __forceinline__ void team_local_transform(const LigS& L, const TeamS& T, int f, float s, float c) {
+    const float4 p0 = L.fg[2 * f], u = L.fg[2 * f + 1];
+    const float k = 1.f - c;
+    const float a00 = fmaf(k * u.x, u.x, c), a01 = fmaf(k * u.x, u.y, -s * u.z), a02 = fmaf(k * u.x, u.z, s * u.y);
+    const float a10 = fmaf(k * u.x, u.y, s * u.z), a11 = fmaf(k * u.y, u.y, c), a12 = fmaf(k * u.y, u.z, -s * u.x);
+    const float a20 = fmaf(k * u.x, u.z, -s * u.y), a21 = fmaf(k * u.y, u.z, s * u.x), a22 = fmaf(k * u.z, u.z, c);
+    T.S.fragFT[2 * f] = make_float4(a00, a01, a02, p0.x);
+    T.S.fragFT[2 * f + 1] = make_float4(a10, a11, a12, p0.y);
+    T.rowz[f] = make_float4(a20, a21, a22, p0.z);
+}
+// eval_pose's rotation matrix of the (re-normalised) quaternion q[4]
+__device__ __forceinline__ void team_rotation(const TeamS& T, const float* q) {
+    float qw = q[0], qx = q[1], qy = q[2], qz = q[3];
+    const float qi = 1.0f / sqrtf(qw * qw + qx * qx + qy * qy + qz * qz);
+    qw *= qi; qx *= qi; qy *= qi; qz *= qi;
+    T.S.fragFT[0] = make_float4(1.f - 2.f * (qy * qy + qz * qz), 2.f * (qx * qy - qw * qz), 2.f * (qx * qz + qw * qy), 0.f);
+    T.S.fragFT[1] = make_float4(2.f * (qx * qy + qw * qz), 1.f - 2.f * (qx * qx + qz * qz), 2.f * (qy * qz - qw * qx), 0.f);
+    T.rowz[0] = make_float4(2.f * (qx * qz - qw * qy), 2.f * (qy * qz + qw * qx), 1.f - 2.f * (qx * qx + qy * qy), 0.f);
 }
 __device__ __forceinline__ void team_sync(const TeamS& T) { asm volatile("bar.sync %0, %1;" ::"r"(T.bar), "n"(kTeamW * 32) : "memory"); }
 // index in a plane of the atom at blk offset `off` (256 floats per 32 atoms -> 96): words +0, +32, +64
@@ -735,48 +760,37 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
         team_sync(T);
         return __int_as_float(0x7fc00000);
     }
-    if (wi == 0) {                                      // (a1) fragment transforms: eval_pose's code on warp 0
-        if (GRAD && lane == 31) T.red[8 * kTeamW] = 1.f;                // "every gradient component is finite" until a writer says no
-        const float qi = 1.0f / sqrtf(qn2);
-        qw *= qi; qx *= qi; qy *= qi; qz *= qi;
-        const float r00 = 1.f - 2.f * (qy * qy + qz * qz), r01 = 2.f * (qx * qy - qw * qz), r02 = 2.f * (qx * qz + qw * qy);
-        const float r10 = 2.f * (qx * qy + qw * qz), r11 = 1.f - 2.f * (qx * qx + qz * qz), r12 = 2.f * (qy * qz - qw * qx);
-        const float r20 = 2.f * (qx * qz - qw * qy), r21 = 2.f * (qy * qz + qw * qx), r22 = 1.f - 2.f * (qx * qx + qy * qy);
-        // S.sc[t] = (sin, cos) of torsion t: left there by the caller (team_sincos, adadelta_search_team's update)
-        for (int f = lane; f < L.nfrag; f += 32) {
-            float m00 = 1, m01 = 0, m02 = 0, m03 = 0, m10 = 0, m11 = 1, m12 = 0, m13 = 0, m20 = 0, m21 = 0, m22 = 1, m23 = 0;
-            int4 ix;
-            for (int cur = f; cur > 0; cur = ix.x) {
-                ix = L.fi[cur];
-                const float4 p0 = L.fg[2 * cur], u = L.fg[2 * cur + 1];
-                const float2 sc = S.sc[ix.w >> 16];
-                const float s = sc.x, c = sc.y, k = 1.f - c;
-                const float a00 = fmaf(k * u.x, u.x, c), a01 = fmaf(k * u.x, u.y, -s * u.z), a02 = fmaf(k * u.x, u.z, s * u.y);
-                const float a10 = fmaf(k * u.x, u.y, s * u.z), a11 = fmaf(k * u.y, u.y, c), a12 = fmaf(k * u.y, u.z, -s * u.x);
-                const float a20 = fmaf(k * u.x, u.z, -s * u.y), a21 = fmaf(k * u.y, u.z, s * u.x), a22 = fmaf(k * u.z, u.z, c);
-                const float n00 = a00 * m00 + a01 * m10 + a02 * m20, n01 = a00 * m01 + a01 * m11 + a02 * m21, n02 = a00 * m02 + a01 * m12 + a02 * m22;
-                const float n10 = a10 * m00 + a11 * m10 + a12 * m20, n11 = a10 * m01 + a11 * m11 + a12 * m21, n12 = a10 * m02 + a11 * m12 + a12 * m22;
-                const float n20 = a20 * m00 + a21 * m10 + a22 * m20, n21 = a20 * m01 + a21 * m11 + a22 * m21, n22 = a20 * m02 + a21 * m12 + a22 * m22;
-                const float dx = m03 - p0.x, dy = m13 - p0.y, dz = m23 - p0.z;
-                const float n03 = a00 * dx + a01 * dy + a02 * dz + p0.x, n13 = a10 * dx + a11 * dy + a12 * dz + p0.y, n23 = a20 * dx + a21 * dy + a22 * dz + p0.z;
-                m00 = n00; m01 = n01; m02 = n02; m03 = n03; m10 = n10; m11 = n11; m12 = n12; m13 = n13;
-                m20 = n20; m21 = n21; m22 = n22; m23 = n23;
+    // (a1) fragment transforms, eight lanes per fragment: lanes 0..3 carry the columns of its 3x4 transform (the basis vectors
+    // and the origin), lane 4 its axis and lane 5 its pivot through the local transforms of the fragment and of its ancestors
+    // (left in shared memory by the caller: team_local_transform), then through the rigid-body rotation (team_rotation).
+    // eval_pose's arithmetic column by column.
+    if (GRAD && wi == 0 && lane == 31) T.red[8 * kTeamW] = 1.f;           // "every gradient component is finite" until a writer says no
+    {
+        const float4 R0 = S.fragFT[0], R1 = S.fragFT[1], R2 = T.rowz[0];
+        for (int base = wi * 32; base < 8 * L.nfrag; base += 32 * kTeamW) {
+            const int it = base + lane, f = it >> 3, j = it & 7;
+            if (f >= L.nfrag || j >= (GRAD ? 6 : 4)) continue;
+            const bool pt = j == 3 || j == 5;                           // a point (w = 1) or a direction
+            float vx = j == 0 ? 1.f : 0.f, vy = j == 1 ? 1.f : 0.f, vz = j == 2 ? 1.f : 0.f;
+            if (j >= 4 && f > 0) {
+                const float4 v = L.fg[2 * f + (j == 4 ? 1 : 0)];
+                vx = v.x; vy = v.y; vz = v.z;
             }
-            const float t00 = r00 * m00 + r01 * m10 + r02 * m20, t01 = r00 * m01 + r01 * m11 + r02 * m21,
-                        t02 = r00 * m02 + r01 * m12 + r02 * m22, t03 = r00 * m03 + r01 * m13 + r02 * m23;
-            const float t10 = r10 * m00 + r11 * m10 + r12 * m20, t11 = r10 * m01 + r11 * m11 + r12 * m21,
-                        t12 = r10 * m02 + r11 * m12 + r12 * m22, t13 = r10 * m03 + r11 * m13 + r12 * m23;
-            const float t20 = r20 * m00 + r21 * m10 + r22 * m20, t21 = r20 * m01 + r21 * m11 + r22 * m21,
-                        t22 = r20 * m02 + r21 * m12 + r22 * m22, t23 = r20 * m03 + r21 * m13 + r22 * m23;
-            S.fragT[3 * f] = make_float4(t00, t01, t02, t03 + tx);
-            S.fragT[3 * f + 1] = make_float4(t10, t11, t12, t13 + ty);
-            S.fragT[3 * f + 2] = make_float4(t20, t21, t22, t23 + tz);
-            if (GRAD && f == 0) S.fragAx[1] = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (GRAD && f > 0) {
-                const float4 p0 = L.fg[2 * f], u = L.fg[2 * f + 1];
-                S.fragAx[2 * f] = make_float4(t00 * u.x + t01 * u.y + t02 * u.z, t10 * u.x + t11 * u.y + t12 * u.z, t20 * u.x + t21 * u.y + t22 * u.z, 0.f);
-                S.fragAx[2 * f + 1] = make_float4(t00 * p0.x + t01 * p0.y + t02 * p0.z + t03, t10 * p0.x + t11 * p0.y + t12 * p0.z + t13,
-                                                  t20 * p0.x + t21 * p0.y + t22 * p0.z + t23, 0.f);
+            for (int cur = f; cur > 0;) {
+                const float4 a0 = S.fragFT[2 * cur], a1 = S.fragFT[2 * cur + 1], a2 = T.rowz[cur];
+                cur = L.fi[cur].x;
+                const float dx = pt ? vx - a0.w : vx, dy = pt ? vy - a1.w : vy, dz = pt ? vz - a2.w : vz;
+                vx = a0.x * dx + a0.y * dy + a0.z * dz + (pt ? a0.w : 0.f);
+                vy = a1.x * dx + a1.y * dy + a1.z * dz + (pt ? a1.w : 0.f);
+                vz = a2.x * dx + a2.y * dy + a2.z * dz + (pt ? a2.w : 0.f);
+            }
+            const float wx = R0.x * vx + R0.y * vy + R0.z * vz, wy = R1.x * vx + R1.y * vy + R1.z * vz,
+                        wz = R2.x * vx + R2.y * vy + R2.z * vz;
+            if (j < 4) {
+                float* o = reinterpret_cast<float*>(S.fragT + 3 * f) + j;
+                o[0] = j == 3 ? wx + tx : wx; o[4] = j == 3 ? wy + ty : wy; o[8] = j == 3 ? wz + tz : wz;
+            } else {
+                S.fragAx[2 * f + (j - 4)] = make_float4(wx, wy, wz, 0.f);      // root: (0, 0, 0)
             }
         }
     }
@@ -969,8 +983,8 @@ __device__ inline float adadelta_search(const LigS& L, const GridDev& G, const P
 // ---------------------------------------------------------------- ADADELTA local search (R7), one team
 // adadelta_search with the evaluation spread over the team and the update spread over its threads: every thread sees the
 // energy and the "gradient finite" flag and takes the same decisions; thread d < 3 of warp 0 owns translation component d,
-// thread 32 + t torsion t (it also leaves sin/cos of the new angle for the next pose), lanes 0..2 of the last warp the
-// rotation components, whose steps lane 0 gathers for the quaternion.  A thread that overwrites a gene saves the old value
+// thread 31 + f the torsion of fragment f (it also leaves the fragment's local transform for the next pose), lanes 0..2 of the
+// last warp the rotation components, whose steps lane 0 gathers for the quaternion and its rotation matrix.  A thread that overwrites a gene saves the old value
 // into S.best first when the pose improved.  Called by all kTeamW warps with S.geno ready and visible.
 __device__ __forceinline__ float adadelta_step(const ParDev& P, float g, float& Eg2, float& Ed2) {
     Eg2 = P.ad_rho * Eg2 + (1.f - P.ad_rho) * g * g;
@@ -983,15 +997,17 @@ __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, co
     static_assert(kTeamW == 4, "thread roles below: warp 0 translation, warps 1..2 torsions (<= 64), warp 3 rotation");
     const WarpS& S = T.S;
     const int R = L.R, Gn = 7 + R, tid = T.wi * 32 + lane;
-    const int tor = tid - 32;                           // this thread's torsion, if 0 <= tor < R
+    const int frag = tid - 31;                          // this thread's fragment and (tor) its torsion, if 1 <= frag <= R
+    const int tor = (frag >= 1 && frag <= R) ? (L.fi[frag].w >> 16) : -1;
     float Eg2 = 0.f, Ed2 = 0.f;                         // of the component this thread owns
     float bestE = __int_as_float(0x7f800000);
     for (int d = tid; d < Gn; d += 32 * kTeamW) S.best[d] = S.geno[d];
-    if (tor >= 0 && tor < R) {
+    if (tor >= 0) {
         float s, c;
         sincosf(S.geno[7 + tor], &s, &c);
-        S.sc[tor] = make_float2(s, c);
+        team_local_transform(L, T, frag, s, c);
     }
+    if (tid == 32 * (kTeamW - 1)) team_rotation(T, S.geno + 3);
     team_sync(T);
     int it = 0;
     while (it < P.lsit) {
@@ -1006,7 +1022,7 @@ __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, co
             const float old = S.geno[tid];
             if (improved) S.best[tid] = old;
             S.geno[tid] = old + dl;
-        } else if (tor >= 0 && tor < R) {
+        } else if (tor >= 0) {
             const float dl = adadelta_step(P, S.grad[6 + tor], Eg2, Ed2);
             const float old = S.geno[7 + tor];
             if (improved) S.best[7 + tor] = old;
@@ -1014,7 +1030,7 @@ __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, co
             S.geno[7 + tor] = nv;
             float s, c;
             sincosf(nv, &s, &c);
-            S.sc[tor] = make_float2(s, c);
+            team_local_transform(L, T, frag, s, c);
         } else if (T.wi == kTeamW - 1) {
             float dl = 0.f;
             if (lane < 3) dl = adadelta_step(P, S.grad[3 + lane], Eg2, Ed2);
@@ -1028,6 +1044,7 @@ __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, co
                 const float k = th > 1e-12f ? sh / th : 0.5f;
                 rotate_quat(ch, k * wx, k * wy, k * wz, oldq, newq);
                 S.geno[3] = newq[0]; S.geno[4] = newq[1]; S.geno[5] = newq[2]; S.geno[6] = newq[3];
+                team_rotation(T, newq);
             }
         }
         team_sync(T);                                    // new genotype visible
