@@ -1068,6 +1068,12 @@ __global__ void __launch_bounds__(128) dock_ls_kernel(GridDev G, ParDev P, const
 // wave; at 4 CTAs per SM they were two (1.85 s -> 3.08 s).  TPC = 4 (one CTA per SM, <= 128 registers): ligands whose image
 // fills most of the shared memory (128 atoms: 117 KB of pair records), where one team per CTA left three of the four
 // schedulers of an SM without a warp.
+#ifndef TEAM_NF1
+#define TEAM_NF1 2
+#endif
+#ifndef TEAM_NF4
+#define TEAM_NF4 4
+#endif
 template <int TPC>
 __global__ void __launch_bounds__(TPC * kTeamW * 32, TPC == 1 ? 5 : 1) dock_ls_team_kernel(GridDev G, ParDev P, const DockJob* __restrict__ jobs,
                                                                                           DockDims dm, int team_floats) {
@@ -1092,7 +1098,7 @@ __global__ void __launch_bounds__(TPC * kTeamW * 32, TPC == 1 ? 5 : 1) dock_ls_t
     if (T.wi == 0) for (int d = lane; d < Gn; d += 32) T.S.geno[d] = g[d];
     team_sync(T);
     int iters = 0;
-    const float be = adadelta_search_team(L, G, P, T, lane, *e, iters);
+    const float be = adadelta_search_team<TPC == 1 ? TEAM_NF1 : TEAM_NF4>(L, G, P, T, lane, *e, iters);
     if (T.wi == 0) {
         for (int d = lane; d < Gn; d += 32) g[d] = T.S.best[d];
         if (lane == 0) {

@@ -746,7 +746,8 @@ __device__ __forceinline__ void team_pair_apply(float* plane, const PairOut& o) 
     __syncwarp();
 }
 
-template <bool GRAD>
+// NF: full pair rounds in flight per warp (registers)
+template <bool GRAD, int NF>
 __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G, const ParDev& P, const TeamS& T, int lane,
                                                 float& e_inter, float& e_intra) {
     const WarpS& S = T.S;
@@ -817,16 +818,27 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
     }
     team_sync(T);
 
-    // (a3) intramolecular pairs: warp wi takes rounds wi, wi + W, ...; forces go to plane wi.  Two full rounds at a time:
-    // the arithmetic of both is independent of the force updates, which follow in round order.
+    // (a3) intramolecular pairs: warp wi takes rounds wi, wi + W, ...; forces go to plane wi.  NF full rounds at a time:
+    // their arithmetic is independent of the force updates, which follow in round order.
     float ep = 0.f;
     float* plane = T.gpl + wi * T.gplane;
     int r = wi;
-    for (; r + kTeamW < L.nfull; r += 2 * kTeamW) {
-        const PairOut o0 = pair_compute<GRAD, false>(L, P, S, r, lane), o1 = pair_compute<GRAD, false>(L, P, S, r + kTeamW, lane);
-        if (GRAD) { team_pair_apply<false>(plane, o0); team_pair_apply<false>(plane, o1); }
-        ep += o0.e; ep += o1.e;
+    for (; r + (NF - 1) * kTeamW < L.nfull; r += NF * kTeamW) {
+        PairOut o[NF];
+#pragma unroll
+        for (int k = 0; k < NF; ++k) o[k] = pair_compute<GRAD, false>(L, P, S, r + k * kTeamW, lane);
+#pragma unroll
+        for (int k = 0; k < NF; ++k) {
+            if (GRAD) team_pair_apply<false>(plane, o[k]);
+            ep += o[k].e;
+        }
     }
+    if (NF > 2)
+        for (; r + kTeamW < L.nfull; r += 2 * kTeamW) {
+            const PairOut o0 = pair_compute<GRAD, false>(L, P, S, r, lane), o1 = pair_compute<GRAD, false>(L, P, S, r + kTeamW, lane);
+            if (GRAD) { team_pair_apply<false>(plane, o0); team_pair_apply<false>(plane, o1); }
+            ep += o0.e; ep += o1.e;
+        }
     for (; r < L.nrounds; r += kTeamW) {
         const PairOut o = pair_compute<GRAD, true>(L, P, S, r, lane);
         if (GRAD) team_pair_apply<true>(plane, o);
@@ -992,6 +1004,7 @@ __device__ __forceinline__ float adadelta_step(const ParDev& P, float g, float& 
     Ed2 = P.ad_rho * Ed2 + (1.f - P.ad_rho) * dl * dl;
     return dl;
 }
+template <int NF>
 __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, const ParDev& P, const TeamS& T, int lane, float e_start,
                                              int& iters) {
     static_assert(kTeamW == 4, "thread roles below: warp 0 translation, warps 1..2 torsions (<= 64), warp 3 rotation");
@@ -1012,7 +1025,7 @@ __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, co
     int it = 0;
     while (it < P.lsit) {
         float ei, ea;
-        const float e = eval_pose_team<true>(L, G, P, T, lane, ei, ea);      // ends with a team barrier: S.grad and the flag are visible
+        const float e = eval_pose_team<true, NF>(L, G, P, T, lane, ei, ea);      // ends with a team barrier: S.grad and the flag are visible
         ++it;
         if (!(isfinite(e) && T.red[8 * kTeamW] != 0.f)) break;              // the same in every thread
         const bool improved = e < bestE;
