@@ -119,7 +119,8 @@ int adock_ligand_lane_image(const adock_ligand* l, int* bytes, const unsigned ch
  * the same function (R3-R7) and pass the same parity tests; they differ in summation order only.
  * 3 = the ADADELTA chains of adock_dock / adock_dock_many each run on a team (one CTA of 4 warps per individual,
  * threads over atoms and pairs), chosen by size when a launch holds too few chains to give every scheduler a warp
- * (a single ligand); every other entry point then behaves as with 1. */
+ * (a single ligand); adock_local_search then runs the same team code on its array of starts (if the ligand fits one
+ * team per CTA); every other entry point behaves as with 1. */
 int adock_set_path(int path);
 /* Family (1, 2 or 3) the local search of the last adock_dock / adock_dock_many on this thread ran in; 0 = none yet. */
 int adock_last_dock_path(void);

@@ -358,7 +358,7 @@ def adock_set_path(path) -> None:
     """kernel family: 'auto' (by problem size), 'warp' (warp per individual), 'lane' (lane per individual, warps per
     group of 32 individuals chosen by size), 'lane1' / 'lane2' / 'lane4' (that number of warps per group), 'tm8' / 'tm12' /
     'tm16' (one warp per group, atom positions in tensor memory, at most that many warps per SM) or 'team' (the
-    docking's ADADELTA chains each run on a CTA of 4 warps; everything else as 'warp')"""
+    ADADELTA chains of the dockings and of adock_local_search each run on a CTA of 4 warps; everything else as 'warp')"""
     _check(lib().adock_set_path(PATHS[path] if isinstance(path, str) else int(path)))
 
 

@@ -681,6 +681,29 @@ __global__ void __launch_bounds__(128) ls_array_kernel(GridDev G, ParDev P, LsAr
     }
 }
 
+// team-per-chain variant (ADADELTA; the docking's dock_ls_team_kernel<1> on an array of starts): one CTA of kTeamW warps per chain
+__global__ void __launch_bounds__(kTeamW * 32, 5) ls_array_team_kernel(GridDev G, ParDev P, LsArgs a) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned char* blob = smem + 16;
+    stage_ligand(blob, a.blob, a.blob_bytes, reinterpret_cast<uint64_t*>(smem), 0);
+    const LigS L = lig_view(blob);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const TeamS T = team_view(reinterpret_cast<float*>(blob + a.blob_bytes), L, warp);
+    const int Gn = 7 + L.R;
+    const size_t idx = blockIdx.x;
+    if (warp == 0) for (int d = lane; d < Gn; d += 32) T.S.geno[d] = a.genos[idx * a.gstride + d];
+    team_sync(T);
+    int iters = 0;
+    const float e = adadelta_search_team<2>(L, G, P, T, lane, __int_as_float(0x7fc00000), iters, a.trace ? a.trace + idx * P.lsit : nullptr);
+    if (warp == 0) {
+        for (int d = lane; d < Gn; d += 32) a.genos[idx * a.gstride + d] = T.S.best[d];
+        if (lane == 0) {
+            a.E[idx] = e;
+            if (a.iters) a.iters[idx] = iters;
+        }
+    }
+}
+
 // lane-per-individual variant: lane c of the launch's groups runs chain c; ADADELTA state in global scratch columns
 // [row][all group lanes of the launch]
 template <class C, bool SW>
@@ -763,6 +786,19 @@ static int local_search_impl(const adock_grids* grids, const adock_ligand* ligan
         if (method == 1) { LANE_VARIANT(var, rc = launch_ls_array_lane<C, true>(grids, ligand, P, a, var, n, stm)) }
         else { LANE_VARIANT(var, rc = launch_ls_array_lane<C, false>(grids, ligand, P, a, var, n, stm)) }
         return rc;
+    }
+    if (g_path == 3 && method == 0) {                   // the team family's ADADELTA chain, as the docking runs it
+        const size_t smem_team = 16 + (size_t)ligand->blob_bytes + (size_t)team_scratch_floats(ligand->tp.N, ligand->tp.nfrag, ligand->tp.R) * 4;
+        if (smem_team <= (size_t)g_smem_optin) {
+            CUDA_TRY(cudaFuncSetAttribute(ls_array_team_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_team));
+            ParDev P = make_pardev(p);
+            P.k_wall_h = p.k_wall * grids->dev.h;
+            LsArgs a{ligand->d_blob, d_genotypes, d_energies, d_iters, d_trace, ligand->blob_bytes, n, gstride, seed, gen};
+            ls_array_team_kernel<<<n, kTeamW * 32, smem_team, (cudaStream_t)cuda_stream>>>(grids->dev, P, a);
+            ++g_launches;
+            CUDA_TRY(cudaGetLastError());
+            return ADOCK_OK;
+        }
     }
     const int W = fit_warps(ligand->blob_bytes, ligand->scratch_floats, 4);
     if (!W) return fail(ADOCK_ELIMIT, "ligand does not fit in shared memory");

@@ -1006,7 +1006,7 @@ __device__ __forceinline__ float adadelta_step(const ParDev& P, float g, float& 
 }
 template <int NF>
 __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, const ParDev& P, const TeamS& T, int lane, float e_start,
-                                             int& iters) {
+                                             int& iters, float* trace = nullptr) {
     static_assert(kTeamW == 4, "thread roles below: warp 0 translation, warps 1..2 torsions (<= 64), warp 3 rotation");
     const WarpS& S = T.S;
     const int R = L.R, Gn = 7 + R, tid = T.wi * 32 + lane;
@@ -1026,6 +1026,7 @@ __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, co
     while (it < P.lsit) {
         float ei, ea;
         const float e = eval_pose_team<true, NF>(L, G, P, T, lane, ei, ea);      // ends with a team barrier: S.grad and the flag are visible
+        if (trace && tid == 0) trace[it] = e;
         ++it;
         if (!(isfinite(e) && T.red[8 * kTeamW] != 0.f)) break;              // the same in every thread
         const bool improved = e < bestE;
