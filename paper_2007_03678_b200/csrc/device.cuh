@@ -697,42 +697,49 @@ __device__ inline void ga_make_child_thread(const ParDev& P, int Pn, int R, unsi
 // order.  Same arithmetic as eval_pose; the summation order differs (fixed, so results are reproducible).
 constexpr int kTeamW = 4;
 __host__ __device__ inline int team_scratch_floats(int N, int nfrag, int R) {
-    return warp_scratch_floats(N, nfrag, R) + kTeamW * ((N + 31) / 32) * 96 + 8 * kTeamW + 8 + 4 * nfrag;
+    return warp_scratch_floats(N, nfrag, R) + kTeamW * ((N + 31) / 32) * 96 + 8 * kTeamW + 8 + 24 * nfrag + pad4(7 + R) + 4 * pad4(6 + R);
 }
-// red: per warp w [8w .. 8w+8) = partial (e_grid, e_pairs, grid force F(3), grid torque about t T(3)); [8 kTeamW] = flag
-// Local transform of fragment f > 0 (rotation A by its torsion angle about its axis through p0: x -> A (x - p0) + p0) as three
-// rows (A_r0, A_r1, A_r2, p0_r): rows 0, 1 in S.fragFT[2f], S.fragFT[2f+1], row 2 in rowz[f]; slot 0 holds the rows of the
-// rigid-body rotation (w = 0).  Written by the thread that owns the torsion / the rotation (team_local_transform,
-// team_rotation), read by the pose builder.
-struct TeamS { WarpS S; float* gpl; float* red; float4* rowz; int wi, gplane, bar; };      // gplane = floats per plane; bar = the team's named barrier
+// red: per warp w [8w .. 8w+8) = partial (e_grid, e_pairs, grid force F(3), grid torque about t T(3)); [8 kTeamW] = the
+// "every gradient component was finite" flag.
+// The ADADELTA chain keeps TWO copies of what a step changes, used alternately: the genotype (S.geno | geno1), the optimiser
+// state ad[b] = E[g^2](Dpad) | E[dx^2](Dpad), and the local transforms lt[b]: fragment f > 0 (rotation A by its torsion angle
+// about its axis through p0: x -> A (x - p0) + p0) as three rows (A_r, p0_r) at lt[b][3f + r]; slot 0 holds the rows of the
+// rigid-body rotation (w = 0).  While copy b is being evaluated the step to the next point is written into copy b ^ 1.
+struct TeamS {
+    WarpS S;
+    float* gpl; float* red; float* geno1; float* ad0; float4* lt0;     // copy b of the state at ad0 + b * 2 Dpad, of the transforms at lt0 + b * 3 nfrag
+    int wi, gplane, bar;                                // gplane = floats per plane; bar = the team's named barrier
+};
 __device__ inline TeamS team_view(float* base, const LigS& L, int wi) {
     TeamS T;
     T.S = warp_view(base, L);
     T.gpl = T.S.blk + (L.npos / 32) * 256;
     T.red = T.gpl + kTeamW * (L.npos / 32) * 96;
-    T.rowz = reinterpret_cast<float4*>(T.red + 8 * kTeamW + 8);
+    T.lt0 = reinterpret_cast<float4*>(T.red + 8 * kTeamW + 8);
+    T.geno1 = reinterpret_cast<float*>(T.lt0 + 6 * L.nfrag);
+    T.ad0 = T.geno1 + pad4(7 + L.R);
     T.wi = wi; T.gplane = (L.npos / 32) * 96; T.bar = 1;
     return T;
 }
 // eval_pose's rotation about the torsion axis, for (sin, cos) of the angle
-__device__ __forceinline__ void team_local_transform(const LigS& L, const TeamS& T, int f, float s, float c) {
+__device__ __forceinline__ void team_local_transform(const LigS& L, float4* lt, int f, float s, float c) {
     const float4 p0 = L.fg[2 * f], u = L.fg[2 * f + 1];
     const float k = 1.f - c;
     const float a00 = fmaf(k * u.x, u.x, c), a01 = fmaf(k * u.x, u.y, -s * u.z), a02 = fmaf(k * u.x, u.z, s * u.y);
     const float a10 = fmaf(k * u.x, u.y, s * u.z), a11 = fmaf(k * u.y, u.y, c), a12 = fmaf(k * u.y, u.z, -s * u.x);
     const float a20 = fmaf(k * u.x, u.z, -s * u.y), a21 = fmaf(k * u.y, u.z, s * u.x), a22 = fmaf(k * u.z, u.z, c);
-    T.S.fragFT[2 * f] = make_float4(a00, a01, a02, p0.x);
-    T.S.fragFT[2 * f + 1] = make_float4(a10, a11, a12, p0.y);
-    T.rowz[f] = make_float4(a20, a21, a22, p0.z);
+    lt[3 * f] = make_float4(a00, a01, a02, p0.x);
+    lt[3 * f + 1] = make_float4(a10, a11, a12, p0.y);
+    lt[3 * f + 2] = make_float4(a20, a21, a22, p0.z);
 }
 // eval_pose's rotation matrix of the (re-normalised) quaternion q[4]
-__device__ __forceinline__ void team_rotation(const TeamS& T, const float* q) {
+__device__ __forceinline__ void team_rotation(float4* lt, const float* q) {
     float qw = q[0], qx = q[1], qy = q[2], qz = q[3];
     const float qi = 1.0f / sqrtf(qw * qw + qx * qx + qy * qy + qz * qz);
     qw *= qi; qx *= qi; qy *= qi; qz *= qi;
-    T.S.fragFT[0] = make_float4(1.f - 2.f * (qy * qy + qz * qz), 2.f * (qx * qy - qw * qz), 2.f * (qx * qz + qw * qy), 0.f);
-    T.S.fragFT[1] = make_float4(2.f * (qx * qy + qw * qz), 1.f - 2.f * (qx * qx + qz * qz), 2.f * (qy * qz - qw * qx), 0.f);
-    T.rowz[0] = make_float4(2.f * (qx * qz - qw * qy), 2.f * (qy * qz + qw * qx), 1.f - 2.f * (qx * qx + qy * qy), 0.f);
+    lt[0] = make_float4(1.f - 2.f * (qy * qy + qz * qz), 2.f * (qx * qy - qw * qz), 2.f * (qx * qz + qw * qy), 0.f);
+    lt[1] = make_float4(2.f * (qx * qy + qw * qz), 1.f - 2.f * (qx * qx + qz * qz), 2.f * (qy * qz - qw * qx), 0.f);
+    lt[2] = make_float4(2.f * (qx * qz - qw * qy), 2.f * (qy * qz + qw * qx), 1.f - 2.f * (qx * qx + qy * qy), 0.f);
 }
 __device__ __forceinline__ void team_sync(const TeamS& T) { asm volatile("bar.sync %0, %1;" ::"r"(T.bar), "n"(kTeamW * 32) : "memory"); }
 // index in a plane of the atom at blk offset `off` (256 floats per 32 atoms -> 96): words +0, +32, +64
@@ -746,31 +753,36 @@ __device__ __forceinline__ void team_pair_apply(float* plane, const PairOut& o) 
     __syncwarp();
 }
 
+// Evaluation of copy b of the chain's point up to the per-atom gradients: pose, pairs, lookups (a1-a3 and the grid part of
+// a4).  On return (after a team barrier) S.blk holds positions and summed per-atom gradients, T.red the warps' partial
+// energies and rigid-body sums.  Returns the energy in every thread; NaN, before any barrier, for |q| < 1e-12.
 // NF: full pair rounds in flight per warp (registers)
-template <bool GRAD, int NF>
-__device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G, const ParDev& P, const TeamS& T, int lane,
-                                                float& e_inter, float& e_intra) {
+template <int NF>
+__device__ __forceinline__ float team_front(const LigS& L, const GridDev& G, const ParDev& P, const TeamS& T, int lane, int b,
+                                            float& e_inter, float& e_intra) {
+    constexpr bool GRAD = true;
     const WarpS& S = T.S;
     const int wi = T.wi;
-    const float tx = S.geno[0], ty = S.geno[1], tz = S.geno[2];
-    float qw = S.geno[3], qx = S.geno[4], qy = S.geno[5], qz = S.geno[6];
-    const float qn2 = qw * qw + qx * qx + qy * qy + qz * qz;
-    if (!(qn2 >= 1e-24f)) {                             // the same in every thread of the team
-        if (GRAD && wi == 0) for (int d = lane; d < 6 + L.R; d += 32) S.grad[d] = __int_as_float(0x7fc00000);
-        e_inter = e_intra = __int_as_float(0x7fc00000);
-        team_sync(T);
-        return __int_as_float(0x7fc00000);
+    const float* geno = b ? T.geno1 : S.geno;
+    const float4* lt = T.lt0 + b * 3 * L.nfrag;
+    const float tx = geno[0], ty = geno[1], tz = geno[2];
+    {
+        const float qw = geno[3], qx = geno[4], qy = geno[5], qz = geno[6];
+        const float qn2 = qw * qw + qx * qx + qy * qy + qz * qz;
+        if (!(qn2 >= 1e-24f)) {                         // the same in every thread of the team
+            e_inter = e_intra = __int_as_float(0x7fc00000);
+            return __int_as_float(0x7fc00000);
+        }
     }
     // (a1) fragment transforms, eight lanes per fragment: lanes 0..3 carry the columns of its 3x4 transform (the basis vectors
     // and the origin), lane 4 its axis and lane 5 its pivot through the local transforms of the fragment and of its ancestors
-    // (left in shared memory by the caller: team_local_transform), then through the rigid-body rotation (team_rotation).
-    // eval_pose's arithmetic column by column.
-    if (GRAD && wi == 0 && lane == 31) T.red[8 * kTeamW] = 1.f;           // "every gradient component is finite" until a writer says no
+    // (left in shared memory by the step that led here: team_local_transform), then through the rigid-body rotation
+    // (team_rotation).  eval_pose's arithmetic column by column.
     {
-        const float4 R0 = S.fragFT[0], R1 = S.fragFT[1], R2 = T.rowz[0];
+        const float4 R0 = lt[0], R1 = lt[1], R2 = lt[2];
         for (int base = wi * 32; base < 8 * L.nfrag; base += 32 * kTeamW) {
             const int it = base + lane, f = it >> 3, j = it & 7;
-            if (f >= L.nfrag || j >= (GRAD ? 6 : 4)) continue;
+            if (f >= L.nfrag || j >= 6) continue;
             const bool pt = j == 3 || j == 5;                           // a point (w = 1) or a direction
             float vx = j == 0 ? 1.f : 0.f, vy = j == 1 ? 1.f : 0.f, vz = j == 2 ? 1.f : 0.f;
             if (j >= 4 && f > 0) {
@@ -778,7 +790,7 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
                 vx = v.x; vy = v.y; vz = v.z;
             }
             for (int cur = f; cur > 0;) {
-                const float4 a0 = S.fragFT[2 * cur], a1 = S.fragFT[2 * cur + 1], a2 = T.rowz[cur];
+                const float4 a0 = lt[3 * cur], a1 = lt[3 * cur + 1], a2 = lt[3 * cur + 2];
                 cur = L.fi[cur].x;
                 const float dx = pt ? vx - a0.w : vx, dy = pt ? vy - a1.w : vy, dz = pt ? vz - a2.w : vz;
                 vx = a0.x * dx + a0.y * dy + a0.z * dz + (pt ? a0.w : 0.f);
@@ -875,51 +887,6 @@ __device__ __forceinline__ float eval_pose_team(const LigS& L, const GridDev& G,
 #pragma unroll
     for (int w = 0; w < kTeamW; ++w) { e_inter += T.red[8 * w]; e_intra += T.red[8 * w + 1]; }
 
-    // (a4) back-propagation: eight lanes per torsion share the atoms of its subtree (a contiguous range of the fragment-ordered
-    // atom list), each summing u . ((r - pivot) x g) over its atoms; eval_pose's terms in another (fixed) order.  The
-    // rigid-body blocks are the warps' grid-force sums.
-    if (GRAD) {
-        const int nitem = 8 * (L.nfrag - 1);
-        for (int base = wi * 32; base < nitem; base += 32 * kTeamW) {
-            const int it = base + lane, f = 1 + (it >> 3);
-            float v0 = 0.f, v1 = 0.f;
-            int w = 0;
-            if (it < nitem) {
-                const int4 ix = L.fi[f];
-                w = ix.w;
-                const int kend = L.fi[(w & 0xffff) - 1].z;
-                const float4 u = S.fragAx[2 * f], pv = S.fragAx[2 * f + 1];
-                const float px = tx + pv.x, py = ty + pv.y, pz = tz + pv.z;
-                int k = ix.y + (it & 7);
-                for (; k + 8 < kend; k += 16) {
-                    const float* b0 = S.blk + atom_slot_dev(L.fragatoms[k]), *b1 = S.blk + atom_slot_dev(L.fragatoms[k + 8]);
-                    const float gx0 = b0[kGX], gy0 = b0[kGY], gz0 = b0[kGZ], rx0 = b0[kX] - px, ry0 = b0[kY] - py, rz0 = b0[kZ] - pz;
-                    const float gx1 = b1[kGX], gy1 = b1[kGY], gz1 = b1[kGZ], rx1 = b1[kX] - px, ry1 = b1[kY] - py, rz1 = b1[kZ] - pz;
-                    v0 += u.x * (ry0 * gz0 - rz0 * gy0) + u.y * (rz0 * gx0 - rx0 * gz0) + u.z * (rx0 * gy0 - ry0 * gx0);
-                    v1 += u.x * (ry1 * gz1 - rz1 * gy1) + u.y * (rz1 * gx1 - rx1 * gz1) + u.z * (rx1 * gy1 - ry1 * gx1);
-                }
-                if (k < kend) {
-                    const float* b0 = S.blk + atom_slot_dev(L.fragatoms[k]);
-                    const float gx0 = b0[kGX], gy0 = b0[kGY], gz0 = b0[kGZ], rx0 = b0[kX] - px, ry0 = b0[kY] - py, rz0 = b0[kZ] - pz;
-                    v0 += u.x * (ry0 * gz0 - rz0 * gy0) + u.y * (rz0 * gx0 - rx0 * gz0) + u.z * (rx0 * gy0 - ry0 * gx0);
-                }
-            }
-            float v = v0 + v1;
-            v += __shfl_xor_sync(kFull, v, 4); v += __shfl_xor_sync(kFull, v, 2); v += __shfl_xor_sync(kFull, v, 1);
-            if (it < nitem && (it & 7) == 0) {
-                S.grad[6 + (w >> 16)] = v;
-                if (!isfinite(v)) T.red[8 * kTeamW] = 0.f;
-            }
-        }
-        if (wi == kTeamW - 1 && lane < 6) {             // rigid-body blocks, fixed order
-            float v = T.red[2 + lane];
-#pragma unroll
-            for (int w = 1; w < kTeamW; ++w) v += T.red[8 * w + 2 + lane];
-            S.grad[lane] = v;
-            if (!isfinite(v)) T.red[8 * kTeamW] = 0.f;
-        }
-        team_sync(T);
-    }
     return e_inter + e_intra;
 }
 
@@ -993,75 +960,121 @@ __device__ inline float adadelta_search(const LigS& L, const GridDev& G, const P
 }
 
 // ---------------------------------------------------------------- ADADELTA local search (R7), one team
-// adadelta_search with the evaluation spread over the team and the update spread over its threads: every thread sees the
-// energy and the "gradient finite" flag and takes the same decisions; thread d < 3 of warp 0 owns translation component d,
-// thread 31 + f the torsion of fragment f (it also leaves the fragment's local transform for the next pose), lanes 0..2 of the
-// last warp the rotation components, whose steps lane 0 gathers for the quaternion and its rotation matrix.  A thread that overwrites a gene saves the old value
-// into S.best first when the pose improved.  Called by all kTeamW warps with S.geno ready and visible.
-__device__ __forceinline__ float adadelta_step(const ParDev& P, float g, float& Eg2, float& Ed2) {
-    Eg2 = P.ad_rho * Eg2 + (1.f - P.ad_rho) * g * g;
-    const float dl = -(sqrtf(Ed2 + P.ad_eps) / sqrtf(Eg2 + P.ad_eps)) * g;
-    Ed2 = P.ad_rho * Ed2 + (1.f - P.ad_rho) * dl * dl;
+// adadelta_search with the evaluation spread over the team and the step computed where its gradient component appears,
+// before anyone knows whether the iteration counts: while copy b of (genotype, optimiser state, local transforms) is being
+// evaluated, the step to the next point goes into copy b ^ 1 -- the translation and rotation components (lanes 0..5 of the
+// last warp: gradient = the warps' grid-force sums, known after the lookups; lane 3 builds the quaternion and its rotation
+// matrix) alongside the torsion gradients (eight lanes per torsion over the atoms of its subtree: u . ((r - pivot) x g), eval_pose's
+// terms in another, fixed order; the lane that holds the sum steps the angle and leaves the fragment's local transform).  One
+// barrier later every thread sees the energy and the "all finite" flag and takes the same decision: stop, or note the
+// evaluated point as the best so far and move on to copy b ^ 1.  Five team barriers per iteration.
+// Called by all kTeamW warps with S.geno ready and visible; S.best holds the result.
+__device__ __forceinline__ float adadelta_step(const ParDev& P, float g, const float* st, float* st_next, int d, int Dp) {
+    const float Eg2 = P.ad_rho * st[d] + (1.f - P.ad_rho) * g * g;
+    const float dl = -(sqrtf(st[Dp + d] + P.ad_eps) / sqrtf(Eg2 + P.ad_eps)) * g;
+    st_next[d] = Eg2;
+    st_next[Dp + d] = P.ad_rho * st[Dp + d] + (1.f - P.ad_rho) * dl * dl;
     return dl;
 }
 template <int NF>
 __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, const ParDev& P, const TeamS& T, int lane, float e_start,
                                              int& iters, float* trace = nullptr) {
-    static_assert(kTeamW == 4, "thread roles below: warp 0 translation, warps 1..2 torsions (<= 64), warp 3 rotation");
     const WarpS& S = T.S;
-    const int R = L.R, Gn = 7 + R, tid = T.wi * 32 + lane;
-    const int frag = tid - 31;                          // this thread's fragment and (tor) its torsion, if 1 <= frag <= R
-    const int tor = (frag >= 1 && frag <= R) ? (L.fi[frag].w >> 16) : -1;
-    float Eg2 = 0.f, Ed2 = 0.f;                         // of the component this thread owns
+    const int R = L.R, Gn = 7 + R, Dp = pad4(6 + R), wi = T.wi, tid = wi * 32 + lane;
     float bestE = __int_as_float(0x7f800000);
     for (int d = tid; d < Gn; d += 32 * kTeamW) S.best[d] = S.geno[d];
-    if (tor >= 0) {
+    for (int d = tid; d < 2 * Dp; d += 32 * kTeamW) T.ad0[d] = 0.f;
+    for (int f = 1 + tid; f < L.nfrag; f += 32 * kTeamW) {
         float s, c;
-        sincosf(S.geno[7 + tor], &s, &c);
-        team_local_transform(L, T, frag, s, c);
+        sincosf(S.geno[7 + (L.fi[f].w >> 16)], &s, &c);
+        team_local_transform(L, T.lt0, f, s, c);
     }
-    if (tid == 32 * (kTeamW - 1)) team_rotation(T, S.geno + 3);
+    if (tid == 32 * (kTeamW - 1)) team_rotation(T.lt0, S.geno + 3);
+    float* flag = T.red + 8 * kTeamW;                   // "every gradient component so far was finite": cleared by the thread that sees otherwise
+    if (tid == 31) *flag = 1.f;
     team_sync(T);
-    int it = 0;
+    int it = 0, b = 0;
     while (it < P.lsit) {
         float ei, ea;
-        const float e = eval_pose_team<true, NF>(L, G, P, T, lane, ei, ea);      // ends with a team barrier: S.grad and the flag are visible
+        const float e = team_front<NF>(L, G, P, T, lane, b, ei, ea);         // ends with a team barrier (unless NaN: |q| ~ 0)
         if (trace && tid == 0) trace[it] = e;
         ++it;
-        if (!(isfinite(e) && T.red[8 * kTeamW] != 0.f)) break;              // the same in every thread
-        const bool improved = e < bestE;
-        if (improved) bestE = e;
-        if (tid < 3) {
-            const float dl = adadelta_step(P, S.grad[tid], Eg2, Ed2);
-            const float old = S.geno[tid];
-            if (improved) S.best[tid] = old;
-            S.geno[tid] = old + dl;
-        } else if (tor >= 0) {
-            const float dl = adadelta_step(P, S.grad[6 + tor], Eg2, Ed2);
-            const float old = S.geno[7 + tor];
-            if (improved) S.best[7 + tor] = old;
-            const float nv = wrap_pi(old + dl);
-            S.geno[7 + tor] = nv;
-            float s, c;
-            sincosf(nv, &s, &c);
-            team_local_transform(L, T, frag, s, c);
-        } else if (T.wi == kTeamW - 1) {
+        if (!isfinite(e)) break;                         // the same in every thread
+        const float* geno = b ? T.geno1 : S.geno;
+        float* gnext = b ? S.geno : T.geno1;
+        const float* st = T.ad0 + b * 2 * Dp;
+        float* st_next = T.ad0 + (b ^ 1) * 2 * Dp;
+        float4* lt_next = T.lt0 + (b ^ 1) * 3 * L.nfrag;
+        if (wi == kTeamW - 1) {                         // rigid-body blocks: the warps' grid-force sums, fixed order
             float dl = 0.f;
-            if (lane < 3) dl = adadelta_step(P, S.grad[3 + lane], Eg2, Ed2);
-            const float wx = __shfl_sync(kFull, dl, 0), wy = __shfl_sync(kFull, dl, 1), wz = __shfl_sync(kFull, dl, 2);
-            if (lane == 0) {
-                float oldq[4] = {S.geno[3], S.geno[4], S.geno[5], S.geno[6]}, newq[4];
-                if (improved) { S.best[3] = oldq[0]; S.best[4] = oldq[1]; S.best[5] = oldq[2]; S.best[6] = oldq[3]; }
+            if (lane < 6) {
+                float v = T.red[2 + lane];
+#pragma unroll
+                for (int w = 1; w < kTeamW; ++w) v += T.red[8 * w + 2 + lane];
+                if (!isfinite(v)) *flag = 0.f;
+                dl = adadelta_step(P, v, st, st_next, lane, Dp);
+                if (lane < 3) gnext[lane] = geno[lane] + dl;
+            }
+            const float wx = __shfl_sync(kFull, dl, 3), wy = __shfl_sync(kFull, dl, 4), wz = __shfl_sync(kFull, dl, 5);
+            if (lane == 3) {                            // q <- normalise(exp(dw/2) (x) q)
+                float newq[4];
                 const float th = sqrtf(wx * wx + wy * wy + wz * wz);
                 float sh, ch;
                 sincosf(0.5f * th, &sh, &ch);
                 const float k = th > 1e-12f ? sh / th : 0.5f;
-                rotate_quat(ch, k * wx, k * wy, k * wz, oldq, newq);
-                S.geno[3] = newq[0]; S.geno[4] = newq[1]; S.geno[5] = newq[2]; S.geno[6] = newq[3];
-                team_rotation(T, newq);
+                rotate_quat(ch, k * wx, k * wy, k * wz, geno + 3, newq);
+                gnext[3] = newq[0]; gnext[4] = newq[1]; gnext[5] = newq[2]; gnext[6] = newq[3];
+                team_rotation(lt_next, newq);
             }
         }
-        team_sync(T);                                    // new genotype visible
+        {
+            const float tx = geno[0], ty = geno[1], tz = geno[2];
+            const int nitem = 8 * (L.nfrag - 1);
+            for (int base = wi * 32; base < nitem; base += 32 * kTeamW) {
+                const int item = base + lane, f = 1 + (item >> 3);
+                float v0 = 0.f, v1 = 0.f;
+                int w = 0;
+                if (item < nitem) {
+                    const int4 ix = L.fi[f];
+                    w = ix.w;
+                    const int kend = L.fi[(w & 0xffff) - 1].z;
+                    const float4 u = S.fragAx[2 * f], pv = S.fragAx[2 * f + 1];
+                    const float px = tx + pv.x, py = ty + pv.y, pz = tz + pv.z;
+                    int k = ix.y + (item & 7);
+                    for (; k + 8 < kend; k += 16) {
+                        const float* b0 = S.blk + atom_slot_dev(L.fragatoms[k]), *b1 = S.blk + atom_slot_dev(L.fragatoms[k + 8]);
+                        const float gx0 = b0[kGX], gy0 = b0[kGY], gz0 = b0[kGZ], rx0 = b0[kX] - px, ry0 = b0[kY] - py, rz0 = b0[kZ] - pz;
+                        const float gx1 = b1[kGX], gy1 = b1[kGY], gz1 = b1[kGZ], rx1 = b1[kX] - px, ry1 = b1[kY] - py, rz1 = b1[kZ] - pz;
+                        v0 += u.x * (ry0 * gz0 - rz0 * gy0) + u.y * (rz0 * gx0 - rx0 * gz0) + u.z * (rx0 * gy0 - ry0 * gx0);
+                        v1 += u.x * (ry1 * gz1 - rz1 * gy1) + u.y * (rz1 * gx1 - rx1 * gz1) + u.z * (rx1 * gy1 - ry1 * gx1);
+                    }
+                    if (k < kend) {
+                        const float* b0 = S.blk + atom_slot_dev(L.fragatoms[k]);
+                        const float gx0 = b0[kGX], gy0 = b0[kGY], gz0 = b0[kGZ], rx0 = b0[kX] - px, ry0 = b0[kY] - py, rz0 = b0[kZ] - pz;
+                        v0 += u.x * (ry0 * gz0 - rz0 * gy0) + u.y * (rz0 * gx0 - rx0 * gz0) + u.z * (rx0 * gy0 - ry0 * gx0);
+                    }
+                }
+                float v = v0 + v1;
+                v += __shfl_xor_sync(kFull, v, 4); v += __shfl_xor_sync(kFull, v, 2); v += __shfl_xor_sync(kFull, v, 1);
+                if (item < nitem && (item & 7) == 0) {  // the torsion's gradient: step the angle, leave the local transform
+                    const int ti = w >> 16;
+                    if (!isfinite(v)) *flag = 0.f;
+                    const float dl = adadelta_step(P, v, st, st_next, 6 + ti, Dp);
+                    const float nv = wrap_pi(geno[7 + ti] + dl);
+                    gnext[7 + ti] = nv;
+                    float sn, cs;
+                    sincosf(nv, &sn, &cs);
+                    team_local_transform(L, lt_next, f, sn, cs);
+                }
+            }
+        }
+        team_sync(T);                                    // the step, the flag
+        if (*flag == 0.f) break;                         // the same in every thread
+        if (e < bestE) {
+            bestE = e;
+            for (int d = tid; d < Gn; d += 32 * kTeamW) S.best[d] = geno[d];     // copy b is not written again before four more barriers
+        }
+        b ^= 1;
     }
     iters = it;
     return isfinite(bestE) ? bestE : e_start;
