@@ -691,8 +691,7 @@ __device__ inline void ga_make_child_thread(const ParDev& P, int Pn, int R, unsi
 // ---------------------------------------------------------------- full evaluation of one genotype by a TEAM of W warps
 // One team of kTeamW warps per individual (one or four teams per CTA, sharing the ligand image), threads over atoms and pairs: for launches with so few chains that one warp per
 // chain leaves most schedulers idle (a single ligand: 180 chains on 592 schedulers), the evaluation itself is split.
-// Warp 0 builds the fragment transforms; the 32 W threads take one atom each (pose + grid lookup); warp w takes the pair
-// rounds r = w (mod W), two rounds in flight, and adds their forces into its own gradient plane (W planes of gx|gy|gz, 96
+// The 32 W threads take one atom each (pose, grid lookup); warp w takes the pair rounds r = w (mod W), several rounds in flight, and adds their forces into its own gradient plane (W planes of gx|gy|gz, 96
 // floats per 32 atoms, in T.gpl), so no two warps ever update the same word; the atom's thread sums the planes in a fixed
 // order.  Same arithmetic as eval_pose; the summation order differs (fixed, so results are reproducible).
 constexpr int kTeamW = 4;
@@ -774,21 +773,33 @@ __device__ __forceinline__ float team_front(const LigS& L, const GridDev& G, con
             return __int_as_float(0x7fc00000);
         }
     }
-    // (a1) fragment transforms, eight lanes per fragment: lanes 0..3 carry the columns of its 3x4 transform (the basis vectors
-    // and the origin), lane 4 its axis and lane 5 its pivot through the local transforms of the fragment and of its ancestors
-    // (left in shared memory by the step that led here: team_local_transform), then through the rigid-body rotation
-    // (team_rotation).  eval_pose's arithmetic column by column.
+    // (a1) pose: a thread per atom carries the atom's reference position through the local transforms of its fragment and of
+    // the fragment's ancestors (left in shared memory by the step that led here: team_local_transform), then through the
+    // rigid-body rotation (team_rotation) and the translation; it asks for the atom's two map sectors and clears the atom's
+    // gradient planes.  Two more threads per fragment f > 0 carry its axis (a direction) and its pivot (a point, kept
+    // relative to t) the same way, for the torsion gradients.  eval_pose's transforms applied one after the other instead of
+    // composed first.
     {
         const float4 R0 = lt[0], R1 = lt[1], R2 = lt[2];
-        for (int base = wi * 32; base < 8 * L.nfrag; base += 32 * kTeamW) {
-            const int it = base + lane, f = it >> 3, j = it & 7;
-            if (f >= L.nfrag || j >= 6) continue;
-            const bool pt = j == 3 || j == 5;                           // a point (w = 1) or a direction
-            float vx = j == 0 ? 1.f : 0.f, vy = j == 1 ? 1.f : 0.f, vz = j == 2 ? 1.f : 0.f;
-            if (j >= 4 && f > 0) {
-                const float4 v = L.fg[2 * f + (j == 4 ? 1 : 0)];
-                vx = v.x; vy = v.y; vz = v.z;
+        const int nitem = L.npos + 2 * L.nfrag;
+        for (int it = wi * 32 + lane; it < nitem; it += 32 * kTeamW) {
+            const bool atom = it < L.npos;
+            uint32_t m = 0;
+            float4 v;
+            int f;
+            bool pt = true;
+            if (atom) {
+                m = L.meta[it];
+                if (m == 0xffffffffu) continue;          // hole
+                v = L.atoms[it];
+                f = m >> 8;
+            } else {
+                f = (it - L.npos) >> 1;
+                if (f == 0) continue;
+                pt = (it - L.npos) & 1;
+                v = L.fg[2 * f + (pt ? 0 : 1)];
             }
+            float vx = v.x, vy = v.y, vz = v.z;
             for (int cur = f; cur > 0;) {
                 const float4 a0 = lt[3 * cur], a1 = lt[3 * cur + 1], a2 = lt[3 * cur + 2];
                 cur = L.fi[cur].x;
@@ -799,33 +810,18 @@ __device__ __forceinline__ float team_front(const LigS& L, const GridDev& G, con
             }
             const float wx = R0.x * vx + R0.y * vy + R0.z * vz, wy = R1.x * vx + R1.y * vy + R1.z * vz,
                         wz = R2.x * vx + R2.y * vy + R2.z * vz;
-            if (j < 4) {
-                float* o = reinterpret_cast<float*>(S.fragT + 3 * f) + j;
-                o[0] = j == 3 ? wx + tx : wx; o[4] = j == 3 ? wy + ty : wy; o[8] = j == 3 ? wz + tz : wz;
-            } else {
-                S.fragAx[2 * f + (j - 4)] = make_float4(wx, wy, wz, 0.f);      // root: (0, 0, 0)
-            }
-        }
-    }
-    team_sync(T);
-    // (a1) atoms: one thread per position (pose, request for the two map sectors); the owner also clears the atom's planes
-    for (int i = wi * 32 + lane; i < L.npos; i += 32 * kTeamW) {
-        const uint32_t m = L.meta[i];
-        if (m == 0xffffffffu) continue;                  // hole
-        const float4 a = L.atoms[i];
-        const int f = m >> 8;
-        const float4 t0 = S.fragT[3 * f], t1 = S.fragT[3 * f + 1], t2 = S.fragT[3 * f + 2];
-        const float x = fmaf(t0.x, a.x, fmaf(t0.y, a.y, fmaf(t0.z, a.z, t0.w)));
-        const float y = fmaf(t1.x, a.x, fmaf(t1.y, a.y, fmaf(t1.z, a.z, t1.w)));
-        const float z = fmaf(t2.x, a.x, fmaf(t2.y, a.y, fmaf(t2.z, a.z, t2.w)));
-        const int off = atom_slot_dev(i);
-        float* b = S.blk + off;
-        b[kX] = x; b[kY] = y; b[kZ] = z; b[kQ] = a.w * P.elec_sqrt;
-        grid_prefetch(G, grid_cell(G, (int)(m & 0xff), x, y, z));
-        if (GRAD) {
-            float* g = T.gpl + plane_index(off);
+            if (atom) {
+                const float x = wx + tx, y = wy + ty, z = wz + tz;
+                const int off = atom_slot_dev(it);
+                float* b = S.blk + off;
+                b[kX] = x; b[kY] = y; b[kZ] = z; b[kQ] = v.w * P.elec_sqrt;
+                grid_prefetch(G, grid_cell(G, (int)(m & 0xff), x, y, z));
+                float* g = T.gpl + plane_index(off);
 #pragma unroll
-            for (int w = 0; w < kTeamW; ++w) { g[w * T.gplane] = 0.f; g[w * T.gplane + 32] = 0.f; g[w * T.gplane + 64] = 0.f; }
+                for (int w = 0; w < kTeamW; ++w) { g[w * T.gplane] = 0.f; g[w * T.gplane + 32] = 0.f; g[w * T.gplane + 64] = 0.f; }
+            } else {
+                S.fragAx[2 * f + (pt ? 1 : 0)] = make_float4(wx, wy, wz, 0.f);
+            }
         }
     }
     team_sync(T);
