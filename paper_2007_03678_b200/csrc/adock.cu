@@ -1134,7 +1134,7 @@ __global__ void __launch_bounds__(TPC * kTeamW * 32, TPC == 1 ? 5 : 1) dock_ls_t
     if (T.wi == 0) for (int d = lane; d < Gn; d += 32) T.S.geno[d] = g[d];
     team_sync(T);
     int iters = 0;
-    const float be = adadelta_search_team<TPC == 1 ? TEAM_NF1 : TEAM_NF4>(L, G, P, T, lane, *e, iters);
+    const float be = adadelta_search_team<TPC == 1 ? TEAM_NF1 : TEAM_NF4, TPC == 4>(L, G, P, T, lane, *e, iters);
     if (T.wi == 0) {
         for (int d = lane; d < Gn; d += 32) g[d] = T.S.best[d];
         if (lane == 0) {

@@ -49,7 +49,7 @@ struct LigS {
     const float4* fg;       // FragGeom as 2 float4
     const int4* fi;         // FragIdx
     const uint4* pairs;     // PairRec rounds
-    int N, R, nfrag, nrounds, npos, nfull;
+    int N, R, nfrag, nrounds, npos, nfull, systolic;
 };
 
 struct WarpS {
@@ -81,7 +81,7 @@ __device__ inline LigS lig_view(const unsigned char* blob) {
     L.fi = reinterpret_cast<const int4*>(blob + h->off_fragidx);
     L.pairs = reinterpret_cast<const uint4*>(blob + h->off_pairs);
     L.fragatoms = reinterpret_cast<const uint16_t*>(blob + h->off_fragatoms);
-    L.N = h->N; L.R = h->R; L.nfrag = h->nfrag; L.nrounds = h->nrounds; L.npos = h->npos; L.nfull = h->nfull;
+    L.N = h->N; L.R = h->R; L.nfrag = h->nfrag; L.nrounds = h->nrounds; L.npos = h->npos; L.nfull = h->nfull; L.systolic = h->systolic;
     return L;
 }
 
@@ -313,14 +313,13 @@ __device__ __forceinline__ float warp_sum(float v) {
 // The arithmetic of a round (pair_compute) touches only positions and charges, so several rounds can be in flight at
 // once; the force updates (pair_apply) then run round by round in the fixed order.
 struct PairOut { int oi, oj; float fx, fy, fz, e; bool valid; };        // oi, oj: the atoms' offsets in S.blk
+// the pair of record `rec` with atom i given by value (position, scaled charge) and atom j read from the pose block
 template <bool GRAD, bool MAYPAD>
-__device__ __forceinline__ PairOut pair_compute(const LigS& L, const ParDev& P, const WarpS& S, int r, int lane) {
-    const uint4 rec = L.pairs[r * 32 + lane];
+__device__ __forceinline__ PairOut pair_core(const ParDev& P, const uint4 rec, float xi, float yi, float zi, float qi, const float* blk) {
     const bool valid = !MAYPAD || ((rec.x >> 23) & 1u);
     const int oi = (int)(rec.x & 0x7ffu), oj = (int)((rec.x >> 11) & 0x7ffu);
-    const float* pi = S.blk + oi;
-    const float* pj = S.blk + oj;
-    const float dx = pi[kX] - pj[kX], dy = pi[kY] - pj[kY], dz = pi[kZ] - pj[kZ];
+    const float* pj = blk + oj;
+    const float dx = xi - pj[kX], dy = yi - pj[kY], dz = zi - pj[kZ];
     const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
     const float r2c = fmaxf(r2, P.rmin2);
     const float rinv = frsqrt(r2c);
@@ -335,7 +334,7 @@ __device__ __forceinline__ PairOut pair_compute(const LigS& L, const ParDev& P, 
     const float rden = frcp(fmaf(P.diel_k, ex, 1.f));
     const float eps = fmaf(P.diel_B, rden, P.diel_A);
     const float inv_er = rinv * frcp(eps);
-    const float eel = pi[kQ] * pj[kQ] * inv_er;                 // charges are stored pre-scaled by sqrt(elec_scale)
+    const float eel = qi * pj[kQ] * inv_er;                     // charges are stored pre-scaled by sqrt(elec_scale)
     const float egs = ds * fex2(r2c * P.mhalf_inv_sig2_log2e);
     const float e = (u12 - uA) + eel + egs;
     PairOut o;
@@ -351,6 +350,86 @@ __device__ __forceinline__ PairOut pair_compute(const LigS& L, const ParDev& P, 
     o.oi = oi; o.oj = oj; o.valid = valid;
     o.e = valid ? e : 0.f;
     return o;
+}
+template <bool GRAD, bool MAYPAD>
+__device__ __forceinline__ PairOut pair_compute(const LigS& L, const ParDev& P, const WarpS& S, int r, int lane) {
+    const uint4 rec = L.pairs[r * 32 + lane];
+    const float* pi = S.blk + (rec.x & 0x7ffu);
+    return pair_core<GRAD, MAYPAD>(P, rec, pi[kX], pi[kY], pi[kZ], pi[kQ], S.blk);
+}
+// Two records of the same atom i (two partners ja, jb) as packed f32x2 arithmetic (lower half = ja): pair_core's
+// expressions two at a time; MUFU, min / max and selects on the halves.
+__device__ __forceinline__ void pair_core2(const ParDev& P, const uint4 reca, const uint4 recb, float xi, float yi, float zi, float qi,
+                                           const float* blk, PairOut& oa, PairOut& ob) {
+    oa.valid = (reca.x >> 23) & 1u; ob.valid = (recb.x >> 23) & 1u;
+    oa.oj = (int)((reca.x >> 11) & 0x7ffu); ob.oj = (int)((recb.x >> 11) & 0x7ffu);
+    const float* pja = blk + oa.oj, *pjb = blk + ob.oj;
+    const f2 dx = sub2(bc(xi), pk(pja[kX], pjb[kX])), dy = sub2(bc(yi), pk(pja[kY], pjb[kY])), dz = sub2(bc(zi), pk(pja[kZ], pjb[kZ]));
+    const f2 qq = mul2(bc(qi), pk(pja[kQ], pjb[kQ]));
+    const f2 r2 = fma2(dx, dx, fma2(dy, dy, mul2(dz, dz)));
+    float r2a, r2b, ta, tb, sa, sb;
+    unpk(r2, r2a, r2b);
+    const float r2ca = fmaxf(r2a, P.rmin2), r2cb = fmaxf(r2b, P.rmin2);
+    const f2 r2c = pk(r2ca, r2cb), rinv = pk(frsqrt(r2ca), frsqrt(r2cb));
+    const f2 rr = mul2(r2c, rinv), rinv2 = mul2(rinv, rinv);
+    const f2 r6 = mul2(mul2(rinv2, rinv2), rinv2), r12 = mul2(r6, r6);
+    const bool hba = (reca.x >> 22) & 1u, hbb = (recb.x >> 22) & 1u;
+    unpk(mul2(r12, r2c), ta, tb);
+    unpk(r6, sa, sb);
+    const f2 rA = pk(hba ? ta : sa, hbb ? tb : sb);
+    const f2 u12 = mul2(pk(__uint_as_float(reca.y), __uint_as_float(recb.y)), r12), uA = mul2(pk(__uint_as_float(reca.z), __uint_as_float(recb.z)), rA);
+    unpk(mul2(rr, bc(P.mlamB_log2e)), ta, tb);
+    unpk(fma2(bc(P.diel_k), pk(fex2(ta), fex2(tb)), bc(1.f)), ta, tb);
+    const f2 rden = pk(frcp(ta), frcp(tb));
+    const f2 eps = fma2(bc(P.diel_B), rden, bc(P.diel_A));
+    unpk(eps, ta, tb);
+    const f2 inv_er = mul2(rinv, pk(frcp(ta), frcp(tb)));
+    const f2 eel = mul2(qq, inv_er);
+    unpk(mul2(r2c, bc(P.mhalf_inv_sig2_log2e)), ta, tb);
+    const f2 egs = mul2(pk(__uint_as_float(reca.w), __uint_as_float(recb.w)), pk(fex2(ta), fex2(tb)));
+    unpk(add2(add2(sub2(u12, uA), eel), egs), ta, tb);
+    oa.e = oa.valid ? ta : 0.f; ob.e = ob.valid ? tb : 0.f;
+    const f2 dv = fma2(pk(hba ? 10.f : 6.f, hbb ? 10.f : 6.f), uA, mul2(bc(-12.f), u12));       // r * d(vdw)/dr
+    const f2 deps = mul2(mul2(bc(P.BlamB), sub2(bc(1.f), rden)), rden);
+    const f2 del = mul2(mul2(neg2(eel), fma2(deps, rr, eps)), inv_er);                         // d(elec)/dr
+    const f2 dds = mul2(mul2(neg2(rr), bc(P.inv_sig2)), egs);                                  // d(desolv)/dr
+    unpk(mul2(fma2(dv, rinv, add2(del, dds)), rinv), ta, tb);
+    const f2 fs = pk((oa.valid && r2a >= P.rmin2) ? ta : 0.f, (ob.valid && r2b >= P.rmin2) ? tb : 0.f);     // 0 for an empty slot
+    unpk(mul2(fs, dx), oa.fx, ob.fx);
+    unpk(mul2(fs, dy), oa.fy, ob.fy);
+    unpk(mul2(fs, dz), oa.fz, ob.fz);
+}
+// Systolic schedule (topology.hpp): block b of the positions, one atom per lane for npos/2 rounds -- its position and its force
+// sum stay in registers, the partners j = i + 1, i + 2, ... are read and updated in shared memory (consecutive lanes,
+// consecutive positions: no bank conflicts), two rounds in flight.  gptr(off) = where the gradient words (+0, +32, +64) of the
+// atom at block offset `off` live.  Returns the lane's energy sum.
+template <bool GRAD, int NF, class GP>
+__device__ __forceinline__ float pairs_systolic_block(const LigS& L, const ParDev& P, const float* blk, GP gptr, int b, int lane) {
+    const int nblk = L.npos >> 5, K = L.npos >> 1;
+    const int offi = b * 256 + lane;
+    const float xi = blk[offi + kX], yi = blk[offi + kY], zi = blk[offi + kZ], qi = blk[offi + kQ];
+    float fx = 0.f, fy = 0.f, fz = 0.f, ep = 0.f;
+    const uint4* rec = L.pairs + b * 32 + lane;
+    for (int k = 0; k < K; k += NF) {                    // K is a multiple of NF (npos = 128: 64)
+        PairOut o[NF];
+#pragma unroll
+        for (int n = 0; n < NF; n += 2) pair_core2(P, rec[(k + n) * nblk * 32], rec[(k + n + 1) * nblk * 32], xi, yi, zi, qi, blk, o[n], o[n + 1]);
+#pragma unroll
+        for (int n = 0; n < NF; ++n) {
+            if (GRAD) {                                  // an empty slot carries a zero force: no predicates on the updates
+                float* g = gptr(o[n].oj);
+                fx += o[n].fx; fy += o[n].fy; fz += o[n].fz; g[0] -= o[n].fx; g[32] -= o[n].fy; g[64] -= o[n].fz;
+                __syncwarp();
+            }
+            ep += o[n].e;
+        }
+    }
+    if (GRAD) {
+        float* g = gptr(offi);
+        g[0] += fx; g[32] += fy; g[64] += fz;
+        __syncwarp();
+    }
+    return ep;
 }
 template <bool GRAD>
 __device__ __forceinline__ float pair_apply(const WarpS& S, const PairOut& o) {
@@ -472,13 +551,18 @@ __device__ __forceinline__ float eval_pose(const LigS& L, const GridDev& G, cons
     // (a3) intramolecular pairs: conflict-free warp rounds; the first nfull rounds have no padding slot
     float ep = 0.f;
     int r4 = 0;
+    if (L.systolic) {                                   // one block of positions after the other, the lane's atom in registers
+        for (int b = 0; b < (L.npos >> 5); ++b)
+            ep += pairs_systolic_block<GRAD, 4>(L, P, S.blk, [&](int off) { return S.blk + off + kGX; }, b, lane);
+        r4 = L.nrounds;
+    }
     for (; r4 + 4 <= L.nfull; r4 += 4) {                // four rounds of arithmetic in flight, updates in round order
         const PairOut o0 = pair_compute<GRAD, false>(L, P, S, r4, lane), o1 = pair_compute<GRAD, false>(L, P, S, r4 + 1, lane),
                       o2 = pair_compute<GRAD, false>(L, P, S, r4 + 2, lane), o3 = pair_compute<GRAD, false>(L, P, S, r4 + 3, lane);
         ep += pair_apply<GRAD>(S, o0); ep += pair_apply<GRAD>(S, o1); ep += pair_apply<GRAD>(S, o2); ep += pair_apply<GRAD>(S, o3);
     }
     for (int r = r4; r < L.nfull; ++r) ep += pair_round<GRAD, false>(L, P, S, r, lane);
-    for (int r = L.nfull; r < L.nrounds; ++r) ep += pair_round<GRAD, true>(L, P, S, r, lane);
+    for (int r = max(r4, L.nfull); r < L.nrounds; ++r) ep += pair_round<GRAD, true>(L, P, S, r, lane);
     e_inter = warp_sum(eg);
     e_intra = warp_sum(ep);
 
@@ -755,8 +839,8 @@ __device__ __forceinline__ void team_pair_apply(float* plane, const PairOut& o) 
 // Evaluation of copy b of the chain's point up to the per-atom gradients: pose, pairs, lookups (a1-a3 and the grid part of
 // a4).  On return (after a team barrier) S.blk holds positions and summed per-atom gradients, T.red the warps' partial
 // energies and rigid-body sums.  Returns the energy in every thread; NaN, before any barrier, for |q| < 1e-12.
-// NF: full pair rounds in flight per warp (registers)
-template <int NF>
+// NF: full pair rounds in flight per warp (registers); SYS: knows the systolic pair schedule
+template <int NF, bool SYS>
 __device__ __forceinline__ float team_front(const LigS& L, const GridDev& G, const ParDev& P, const TeamS& T, int lane, int b,
                                             float& e_inter, float& e_intra) {
     constexpr bool GRAD = true;
@@ -831,6 +915,10 @@ __device__ __forceinline__ float team_front(const LigS& L, const GridDev& G, con
     float ep = 0.f;
     float* plane = T.gpl + wi * T.gplane;
     int r = wi;
+    if (SYS && L.systolic) {                            // block wi of the positions (npos / 32 = kTeamW), the thread's atom in registers
+        ep = pairs_systolic_block<GRAD, NF>(L, P, S.blk, [&](int off) { return plane + plane_index(off); }, wi, lane);
+        r = L.nrounds;
+    }
     for (; r + (NF - 1) * kTeamW < L.nfull; r += NF * kTeamW) {
         PairOut o[NF];
 #pragma unroll
@@ -972,7 +1060,7 @@ __device__ __forceinline__ float adadelta_step(const ParDev& P, float g, const f
     st_next[Dp + d] = P.ad_rho * st[Dp + d] + (1.f - P.ad_rho) * dl * dl;
     return dl;
 }
-template <int NF>
+template <int NF, bool SYS = false>
 __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, const ParDev& P, const TeamS& T, int lane, float e_start,
                                              int& iters, float* trace = nullptr) {
     const WarpS& S = T.S;
@@ -992,7 +1080,7 @@ __device__ inline float adadelta_search_team(const LigS& L, const GridDev& G, co
     int it = 0, b = 0;
     while (it < P.lsit) {
         float ei, ea;
-        const float e = team_front<NF>(L, G, P, T, lane, b, ei, ea);         // ends with a team barrier (unless NaN: |q| ~ 0)
+        const float e = team_front<NF, SYS>(L, G, P, T, lane, b, ei, ea);         // ends with a team barrier (unless NaN: |q| ~ 0)
         if (trace && tid == 0) trace[it] = e;
         ++it;
         if (!isfinite(e)) break;                         // the same in every thread

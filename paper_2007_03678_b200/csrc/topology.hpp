@@ -26,7 +26,7 @@ struct LigHeader {          // 80 bytes
     int nrounds, T, off_atoms, off_meta;
     int off_frag, off_fragidx, off_pairs, bytes;
     int max_frag_atoms, max_depth, npos, off_fragatoms;   // npos = 32*ceil(N/32) atom positions (some may be holes)
-    int nfull, pad1, pad2, pad3;                          // rounds [0,nfull) have all 32 slots valid
+    int nfull, systolic, pad2, pad3;                      // rounds [0,nfull) have all 32 slots valid; systolic: see the pair schedule
 };
 struct FragGeom {           // 32 bytes: torsion axis of the bond that attaches fragment f to its parent
     float p0[3]; float pad0;   // x0[a_k] - pivot
@@ -216,6 +216,28 @@ inline bool build_topology(Topology& tp, int N, const float* xyz, const int* typ
         return r;
     };
     int nrounds = 0, nfull = 0;
+    // Systolic schedule for ligands of exactly four position blocks (97..128 atoms), where the list schedule above spends most
+    // of its shared-memory bandwidth on loading both atoms and updating both forces of every pair: round k * 4 + b
+    // (k = 0 .. npos/2 - 1, b = block) pairs position i = 32 b + lane with j = (i + k + 1) mod npos, so a lane keeps ONE atom i
+    // for all its rounds (position and force sum in registers) and only the j side touches shared memory, conflict-free
+    // (consecutive lanes, consecutive positions).  Every unordered pair {i, j} comes up exactly once (for k + 1 = npos/2
+    // only from i < npos/2); excluded pairs and holes are slots with the valid bit clear.  The hard rule of the list
+    // schedule holds as well (a round's i are distinct, and so are its j), so kernels that do not know the schedule run it as
+    // nrounds padded rounds.
+    const bool systolic = npos == 128;
+    if (systolic) {
+        std::vector<char> has((size_t)npos * npos, 0);
+        for (auto& p : rem) has[(size_t)p.a * npos + p.b] = has[(size_t)p.b * npos + p.a] = 1;
+        for (int k = 0; k < npos / 2; ++k)
+            for (int b = 0; b < npos / 32; ++b)
+                for (int l = 0; l < 32; ++l) {
+                    const int i = 32 * b + l, j = (i + k + 1) % npos;
+                    const bool valid = has[(size_t)i * npos + j] && (k + 1 < npos / 2 || i < npos / 2);
+                    recs.push_back(valid ? make_rec(i, j) : PairRec{atom_slot(i) | (atom_slot(j) << 11), 0.f, 0.f, 0.f});
+                }
+        nrounds = (npos / 2) * (npos / 32);
+        rem.clear();
+    }
     while (!rem.empty()) {
         // highest remaining degree first, so crowded atoms are spread over the rounds
         std::stable_sort(rem.begin(), rem.end(), [&](const P& x, const P& y) {
@@ -248,7 +270,7 @@ inline bool build_topology(Topology& tp, int N, const float* xyz, const int* typ
         ++nrounds;
     }
 
-    {   // full rounds first (their kernel loop carries no validity tests), padded rounds after
+    if (!systolic) {    // full rounds first (their kernel loop carries no validity tests), padded rounds after
         std::vector<PairRec> full, part;
         for (int r = 0; r < nrounds; ++r) {
             bool all = true;
@@ -264,7 +286,7 @@ inline bool build_topology(Topology& tp, int N, const float* xyz, const int* typ
     auto align16 = [](size_t x) { return (x + 15) & ~(size_t)15; };
     LigHeader h{};
     h.N = N; h.R = R; h.nfrag = tp.nfrag; h.npairs = (int)tp.pairs.size() / 2; h.nrounds = nrounds; h.T = T;
-    h.npos = npos; h.nfull = nfull;
+    h.npos = npos; h.nfull = nfull; h.systolic = systolic ? 1 : 0;
     size_t off = sizeof(LigHeader);
     h.off_atoms = (int)off;     off = align16(off + (size_t)npos * 16);
     h.off_meta = (int)off;      off = align16(off + (size_t)npos * 4);

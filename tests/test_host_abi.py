@@ -64,9 +64,9 @@ def test_integer_structure_bit_exact_vs_oracle(B, W, orc, name, request):
 
 
 def _parse_image(blob):
-    h = struct.unpack_from("17i", blob, 0)
+    h = struct.unpack_from("18i", blob, 0)
     keys = ["N", "R", "nfrag", "npairs", "nrounds", "T", "off_atoms", "off_meta", "off_frag", "off_fragidx", "off_pairs",
-            "bytes", "max_frag_atoms", "max_depth", "npos", "off_fragatoms", "nfull"]
+            "bytes", "max_frag_atoms", "max_depth", "npos", "off_fragatoms", "nfull", "systolic"]
     H = dict(zip(keys, h))
     atoms = np.frombuffer(blob, np.float32, 4 * H["npos"], H["off_atoms"]).reshape(-1, 4)
     meta = np.frombuffer(blob, np.uint32, H["npos"], H["off_meta"])
@@ -120,7 +120,22 @@ def test_image_layout_and_conflict_free_schedule(B, W, orc, name, request):
             assert np.allclose(fg[f, 4:7], u / np.linalg.norm(u), atol=1e-6)
             assert np.allclose(fg[f, 0:3], lig.xyz[a].astype(np.float64) - piv, atol=1e-6)
     # schedule: a permutation of the canonical pair list, every atom at most once per side per round (hard rule);
-    # positions on one side distinct modulo 32 (soft rule, bank-conflict free) in nearly every round
+    # positions on one side distinct modulo 32 (soft rule, bank-conflict free) in nearly every round.
+    # Ligands of exactly four position blocks get the systolic schedule (topology.hpp): round 4 k + b pairs position
+    # i = 32 b + lane with j = (i + k + 1) mod npos; excluded pairs are slots with the valid bit clear and zero coefficients.
+    assert H["systolic"] == (1 if npos == 128 else 0)
+    if H["systolic"]:
+        assert H["nrounds"] == (npos // 2) * (npos // 32) and H["nfull"] == 0
+        for r in range(H["nrounds"]):
+            k, b = divmod(r, npos // 32)
+            i = 32 * b + np.arange(32)
+            j = (i + k + 1) % npos
+            ij = pr[r, :, 0]
+            assert np.array_equal(ij & 0x7FF, (i >> 5) * 256 + (i & 31)) and np.array_equal((ij >> 11) & 0x7FF, (j >> 5) * 256 + (j & 31))
+            valid = ((ij >> 23) & 1).astype(bool)
+            assert (pr[r, ~valid, 1:] == 0).all() and ((ij[~valid] >> 22) == 0).all()
+            if k + 1 == npos // 2:
+                assert not valid[i >= npos // 2].any()
     seen = []
     wavefronts = []
     for r in range(H["nrounds"]):
@@ -130,8 +145,10 @@ def test_image_layout_and_conflict_free_schedule(B, W, orc, name, request):
         i, j = (si >> 8) * 32 + (si & 31), (sj >> 8) * 32 + (sj & 31)
         assert ((si & 255) < 32).all() and ((sj & 255) < 32).all() and (ext_of_int[i] >= 0).all() and (ext_of_int[j] >= 0).all()
         assert len(set(i.tolist())) == len(i) and len(set(j.tolist())) == len(j)
-        wavefronts += [np.bincount(i & 31).max(), np.bincount(j & 31).max()]      # replays of one 4-byte access
-        assert (pr[r, ~valid] == 0).all() and (valid.all() == (r < H["nfull"]))
+        if len(i):
+            wavefronts += [np.bincount(i & 31).max(), np.bincount(j & 31).max()]      # replays of one 4-byte access
+        if not H["systolic"]:
+            assert (pr[r, ~valid] == 0).all() and (valid.all() == (r < H["nfull"]))
         for a, b, rec in zip(i, j, pr[r, valid]):
             ea, eb = int(ext_of_int[a]), int(ext_of_int[b])
             seen.append((min(ea, eb), max(ea, eb)))
@@ -144,6 +161,8 @@ def test_image_layout_and_conflict_free_schedule(B, W, orc, name, request):
     lower = max(int(np.ceil(ol.npairs / 32)), int(np.ceil(deg / 2)))
     assert H["nrounds"] <= int(np.ceil(1.3 * lower)) + 1, (H["nrounds"], lower)
     assert np.mean(wavefronts) <= 2.0 and max(wavefronts) <= 3, (np.mean(wavefronts), max(wavefronts))
+    if H["systolic"]:
+        assert max(wavefronts) == 1
 
 
 def test_load_ligand_rejects_bad_input(B, W):
