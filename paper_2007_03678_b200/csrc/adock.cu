@@ -681,21 +681,26 @@ __global__ void __launch_bounds__(128) ls_array_kernel(GridDev G, ParDev P, LsAr
     }
 }
 
-// team-per-chain variant (ADADELTA; the docking's dock_ls_team_kernel<1> on an array of starts): one CTA of kTeamW warps per chain
-__global__ void __launch_bounds__(kTeamW * 32, 5) ls_array_team_kernel(GridDev G, ParDev P, LsArgs a) {
+// team-per-chain variant (ADADELTA; the docking's dock_ls_team_kernel<TPC> on an array of starts): TPC teams of kTeamW warps per
+// CTA, one chain each, sharing the ligand image
+template <int TPC>
+__global__ void __launch_bounds__(TPC * kTeamW * 32, TPC == 1 ? 5 : 1) ls_array_team_kernel(GridDev G, ParDev P, LsArgs a, int team_floats) {
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char* blob = smem + 16;
     stage_ligand(blob, a.blob, a.blob_bytes, reinterpret_cast<uint64_t*>(smem), 0);
     const LigS L = lig_view(blob);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const TeamS T = team_view(reinterpret_cast<float*>(blob + a.blob_bytes), L, warp);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, team = warp / kTeamW;
+    TeamS T = team_view(reinterpret_cast<float*>(blob + a.blob_bytes) + (size_t)team * team_floats, L, warp % kTeamW);
+    T.bar = 1 + team;
     const int Gn = 7 + L.R;
-    const size_t idx = blockIdx.x;
-    if (warp == 0) for (int d = lane; d < Gn; d += 32) T.S.geno[d] = a.genos[idx * a.gstride + d];
+    const size_t idx = (size_t)blockIdx.x * TPC + team;
+    if (idx >= (size_t)a.n) return;                     // whole teams leave: the barriers below are per team
+    if (T.wi == 0) for (int d = lane; d < Gn; d += 32) T.S.geno[d] = a.genos[idx * a.gstride + d];
     team_sync(T);
     int iters = 0;
-    const float e = adadelta_search_team<2>(L, G, P, T, lane, __int_as_float(0x7fc00000), iters, a.trace ? a.trace + idx * P.lsit : nullptr);
-    if (warp == 0) {
+    const float e = adadelta_search_team<TPC == 1 ? 2 : 4, TPC == 4>(L, G, P, T, lane, __int_as_float(0x7fc00000), iters,
+                                                                     a.trace ? a.trace + idx * P.lsit : nullptr);
+    if (T.wi == 0) {
         for (int d = lane; d < Gn; d += 32) a.genos[idx * a.gstride + d] = T.S.best[d];
         if (lane == 0) {
             a.E[idx] = e;
@@ -787,14 +792,22 @@ static int local_search_impl(const adock_grids* grids, const adock_ligand* ligan
         else { LANE_VARIANT(var, rc = launch_ls_array_lane<C, false>(grids, ligand, P, a, var, n, stm)) }
         return rc;
     }
-    if (g_path == 3 && method == 0) {                   // the team family's ADADELTA chain, as the docking runs it
-        const size_t smem_team = 16 + (size_t)ligand->blob_bytes + (size_t)team_scratch_floats(ligand->tp.N, ligand->tp.nfrag, ligand->tp.R) * 4;
+    if (g_path == 3 && method == 0) {                   // the team family's ADADELTA chain, as the docking runs it (same choice of teams per CTA)
+        const size_t team = (size_t)team_scratch_floats(ligand->tp.N, ligand->tp.nfrag, ligand->tp.R);
+        const size_t one = 16 + (size_t)ligand->blob_bytes + team * 4, four = 16 + (size_t)ligand->blob_bytes + 4 * team * 4;
+        const int tpc = (5 * one <= (size_t)g_smem_optin || four > (size_t)g_smem_optin) ? 1 : 4;
+        const size_t smem_team = tpc == 1 ? one : four;
         if (smem_team <= (size_t)g_smem_optin) {
-            CUDA_TRY(cudaFuncSetAttribute(ls_array_team_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_team));
             ParDev P = make_pardev(p);
             P.k_wall_h = p.k_wall * grids->dev.h;
             LsArgs a{ligand->d_blob, d_genotypes, d_energies, d_iters, d_trace, ligand->blob_bytes, n, gstride, seed, gen};
-            ls_array_team_kernel<<<n, kTeamW * 32, smem_team, (cudaStream_t)cuda_stream>>>(grids->dev, P, a);
+            if (tpc == 1) {
+                CUDA_TRY(cudaFuncSetAttribute(ls_array_team_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_team));
+                ls_array_team_kernel<1><<<n, kTeamW * 32, smem_team, (cudaStream_t)cuda_stream>>>(grids->dev, P, a, (int)team);
+            } else {
+                CUDA_TRY(cudaFuncSetAttribute(ls_array_team_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_team));
+                ls_array_team_kernel<4><<<(n + 3) / 4, 4 * kTeamW * 32, smem_team, (cudaStream_t)cuda_stream>>>(grids->dev, P, a, (int)team);
+            }
             ++g_launches;
             CUDA_TRY(cudaGetLastError());
             return ADOCK_OK;

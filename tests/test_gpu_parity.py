@@ -368,6 +368,50 @@ def test_large_config_short_docking(B, orc, large):
     assert r["energies"][0] <= e0 + 1e-3 * abs(e0)                  # the elite never gets worse than generation 0's best
 
 
+@pytest.mark.parametrize("fam", ["warp", "team"])
+def test_large_config_local_search_trace(B, orc, W, large, dev, fam):
+    """The ADADELTA chain on the 128-atom ligand, iteration by iteration against the oracle: under 'team' this is the
+    four-teams-per-CTA kernel of the configs[3] docking with the systolic pair schedule (topology.hpp), under 'warp'
+    eval_pose on the same schedule.  Starts are relaxed poses (the oracle's own 60-iteration search from random genotypes
+    plus a small seeded kick), as in test_local_search_first_iterations_track_oracle and for its reason; E(x_0) is plain
+    scoring parity, E(x_1..3) is where a wrong gradient component or update would show (O(0.1) relative)."""
+    c = large
+    c4 = Case(B, orc, W, c.grids, c.lig, dict(lsit=4))
+    c60 = Case(B, orc, W, c.grids, c.lig, dict(lsit=60))
+    n = 48
+    G0 = W.make_genotypes(n, c.lig.R, c.grids, seed=41, wall_tail=0.0)
+    rng = np.random.default_rng(6)
+    S = np.zeros_like(G0)
+    for i in range(n):
+        g = orc.adadelta(c60.og, c60.ol, c60.op, G0[i].astype(np.float64))[0].copy()
+        g[0:3] += rng.normal(0, 0.05, 3)
+        g[7:] += rng.normal(0, 0.05, c.lig.R)
+        S[i] = g
+    d_g = torch.from_numpy(S).to(dev)
+    d_E = torch.zeros(n, device=dev)
+    d_it = torch.zeros(n, dtype=torch.int32, device=dev)
+    d_tr = torch.full((n, 4), float("nan"), device=dev)
+    B.adock_set_path(fam)
+    try:
+        B.adock_local_search(c4.gg, c4.gl, c4.gp, d_g, d_E, d_it, d_tr)
+        torch.cuda.synchronize()
+    finally:
+        B.adock_set_path("auto")
+    assert (d_it.cpu().numpy() == 4).all()
+    T = d_tr.cpu().numpy().astype(np.float64)
+    O = np.array([orc.adadelta(c4.og, c4.ol, c4.op, S[i].astype(np.float64), trace=True)[3] for i in range(n)])
+    assert_energy(T[:, 0].astype(np.float32), O[:, 0], f"large trace k=0 [{fam}]")
+    rel = np.abs(T - O) / np.maximum(np.abs(O), 1.0)
+    print(f"large trace [{fam}]: median / max relative deviation per iteration {np.median(rel, 0)} / {rel.max(0)}")
+    for k in (1, 2, 3):
+        assert np.median(rel[:, k]) < 1e-3 and (rel[:, k] < 2e-2).mean() >= 0.9, (fam, k, np.median(rel[:, k]), (rel[:, k] < 2e-2).mean())
+    # the best energy returned is the smallest of the trace, and the returned genotype has it
+    gE = d_E.cpu().numpy().astype(np.float64)
+    assert np.allclose(gE, T.min(1), rtol=1e-6)
+    chk = orc.score(c.og, c.ol, c.op, d_g.cpu().numpy(), want_grad=False)["E"]
+    assert_energy(gE.astype(np.float32), chk, f"large LS result [{fam}]")
+
+
 # ------------------------------------------------------------------------------- Philox (R8)
 def test_philox_bit_exact_vs_oracle(B, orc, dev):
     n = 1 << 20
