@@ -434,7 +434,7 @@ static bool lane_ok(const adock_ligand* l) {
     return false;
 }
 // ADADELTA chains (threads) from which the lane-per-individual kernels are preferred over warp-per-individual
-static long long lane_min_chains() { return (long long)g_sm_count * 64; }     // measured cross-over on the drug config: between 32 and 64 ligands x 180 chains
+static long long lane_min_chains() { return (long long)g_sm_count * 42; }     // measured cross-over on the drug config: 34 ligands x 180 chains (the lane kernel's partial wave costs the same from 1 to 64 ligands)
 // ---- launch plan of a lane-per-individual kernel over `total` groups of 32 individuals, `jg` consecutive groups per
 // ligand image (jg >= total: one image).  CTA b takes groups [b*ng, (b+1)*ng) and stages every image they touch.
 struct LanePlan {
@@ -1477,7 +1477,7 @@ static int dock_impl(const adock_grids* grids, const adock_ligand* const* ligs, 
     const int team_tpc = (5 * (16 + (size_t)maxblob + (size_t)maxteam * 4) <= (size_t)g_smem_optin || 16 + (size_t)maxblob + 4 * (size_t)maxteam * 4 > (size_t)g_smem_optin) ? 1 : 4;
     const size_t smem_team = 16 + (size_t)maxblob + (size_t)team_tpc * maxteam * 4;
     const bool ls_team = !ls_lane && p.ls_method == 0 && smem_team <= (size_t)g_smem_optin &&
-                         (g_path == 3 || (g_path == 0 && chains <= (long long)g_sm_count * 6));   // measured cross-over: 4..8 ligands x 180 chains
+                         (g_path == 3 || (g_path == 0 && chains <= (long long)g_sm_count * 24));  // measured cross-over against warp per chain: 20 ligands x 180 chains
     g_last_dock_path = ls_lane ? 2 : ls_team ? 3 : 1;
     // offspring scoring: lane-per-individual under the same condition (populations are 1/lsrat times larger)
     const int jgs = (int)(((long long)nrun * Pn + 31) / 32);
